@@ -1,0 +1,233 @@
+"""ctypes wrapper of oracle/krp_oracle.c -- TEST INFRASTRUCTURE, NOT THE PRODUCT.
+
+Argument marshalling only; all arithmetic is in krp_oracle.c.  Shares nothing
+with paper_2512_01283_b200 (neither imports the other).
+"""
+import ctypes as C
+import os
+import subprocess
+
+import numpy as np
+
+_HERE = os.path.dirname(os.path.abspath(__file__))
+_SRC = os.path.join(_HERE, "krp_oracle.c")
+_SO = os.path.join(_HERE, "libkrp_oracle.so")
+_lib = None
+
+
+def build(force=False):
+    """Compile krp_oracle.c with gcc (no fast-math: fp64 IEEE as written)."""
+    if force or not os.path.exists(_SO) or os.path.getmtime(_SO) < os.path.getmtime(_SRC):
+        tmp = _SO + ".tmp%d" % os.getpid()
+        subprocess.check_call(["gcc", "-O2", "-std=c11", "-fPIC", "-shared", "-ffp-contract=off",
+                               "-o", tmp, _SRC, "-lm"])
+        os.replace(tmp, _SO)
+    return _SO
+
+
+class OracleStats(C.Structure):
+    _fields_ = [(n, C.c_uint64) for n in ("packets", "events", "records", "steps_transport", "steps_image",
+                                          "contributions", "dropped", "overflow")] + \
+               [(n, C.c_double) for n in ("w_emitted", "w_escaped", "w_absorbed", "w_cut")]
+
+    def as_dict(self):
+        return {n: getattr(self, n) for n, _ in self._fields_}
+
+
+class _Events(C.Structure):
+    _fields_ = [("cap", C.c_int64), ("n", C.c_int64), ("cell", C.c_void_p), ("p", C.c_void_p),
+                ("n_in", C.c_void_p), ("S", C.c_void_p), ("id", C.c_void_p), ("k", C.c_void_p)]
+
+
+class Observer(C.Structure):
+    _fields_ = [("theta", C.c_double), ("phi", C.c_double), ("center", C.c_double * 3),
+                ("half_w", C.c_double), ("half_h", C.c_double)]
+
+    @staticmethod
+    def make(theta, phi, center, half_w, half_h=None):
+        o = Observer()
+        o.theta, o.phi = float(theta), float(phi)
+        o.center[:] = [float(c) for c in center]
+        o.half_w = float(half_w)
+        o.half_h = float(half_w if half_h is None else half_h)
+        return o
+
+
+class OracleEvents:
+    """Caller-allocated SoA event list (capacity cap)."""
+
+    def __init__(self, cap):
+        self.cap = int(cap)
+        self.cell = np.zeros(cap, np.int64)
+        self.p = np.zeros((cap, 3), np.float64)
+        self.n_in = np.zeros((cap, 3), np.float64)
+        self.S = np.zeros((cap, 4), np.float64)
+        self.id = np.zeros(cap, np.uint64)
+        self.k = np.zeros(cap, np.int32)
+        self.c = _Events(self.cap, 0, self.cell.ctypes.data, self.p.ctypes.data, self.n_in.ctypes.data,
+                         self.S.ctypes.data, self.id.ctypes.data, self.k.ctypes.data)
+
+    @property
+    def n(self):
+        return int(self.c.n)
+
+    def clear(self):
+        self.c.n = 0
+
+
+_D = C.POINTER(C.c_double)
+_dp = np.ctypeslib.ndpointer(np.float64, flags="C_CONTIGUOUS")
+_fp = np.ctypeslib.ndpointer(np.float32, flags="C_CONTIGUOUS")
+_ip = np.ctypeslib.ndpointer(np.int32, flags="C_CONTIGUOUS")
+_up = np.ctypeslib.ndpointer(np.uint32, flags="C_CONTIGUOUS")
+
+
+def lib():
+    global _lib
+    if _lib is not None:
+        return _lib
+    L = C.CDLL(build())
+    sig = {
+        "ora_philox": (None, [_up, _up, _up]),
+        "ora_u01": (C.c_double, [C.c_uint32]),
+        "ora_u53": (C.c_double, [C.c_uint32, C.c_uint32]),
+        "ora_quat_mul": (None, [_dp, _dp, _dp]),
+        "ora_quat_from_B": (None, [_dp, _dp]),
+        "ora_rot_to_gf": (None, [_dp, _dp, _dp]),
+        "ora_rot_to_lab": (None, [_dp, _dp, _dp]),
+        "ora_basis": (None, [_dp, _dp, _dp]),
+        "ora_eta_gf": (None, [_dp, _dp, _D, _D]),
+        "ora_rotate_qu": (None, [_dp, C.c_double, C.c_double]),
+        "ora_appA": (None, [_dp, C.c_double, C.c_double, C.c_double, C.c_double]),
+        "ora_event_solve": (C.c_double, [C.c_double] * 5),
+        "ora_model_create": (C.c_void_p, [C.c_int, C.c_int, C.c_int, _dp, C.c_void_p, C.c_void_p,
+                                          C.c_int, _fp, C.c_int, _fp, C.c_double, C.c_int]),
+        "ora_model_free": (None, [C.c_void_p]),
+        "ora_source_set": (None, [C.c_void_p, C.c_int, _dp, _dp, C.c_void_p, C.c_int]),
+        "ora_mueller_at": (None, [C.c_void_p, C.c_double, _dp]),
+        "ora_opac_at": (None, [C.c_void_p, C.c_double, _dp]),
+        "ora_dda_exit": (C.c_double, [C.c_void_p, _dp, _dp, C.POINTER(C.c_int)]),
+        "ora_cell_step": (None, [C.c_void_p, _dp, _dp, _dp, C.c_double]),
+        "ora_march": (C.c_int64, [C.c_void_p, _ip, _dp, _dp, _dp, C.c_int64, C.c_void_p, C.c_void_p]),
+        "ora_sample_theta": (C.c_double, [C.c_void_p, C.c_double]),
+        "ora_phi_accept": (C.c_int, [C.c_double] * 5),
+        "ora_scatter_angles": (None, [C.c_void_p, _dp, _dp, _dp, C.c_double, C.c_double, _dp, _dp]),
+        "ora_scatter": (C.c_int, [C.c_void_p, _dp, _dp, _dp, C.c_uint64, C.c_uint64, C.c_uint32, _dp, _dp, _D]),
+        "ora_transport": (C.c_int64, [C.c_void_p, C.c_uint64, C.c_uint64, C.c_uint64, C.POINTER(_Events),
+                                      C.POINTER(OracleStats), C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p,
+                                      C.c_void_p]),
+        "ora_peel": (None, [C.c_void_p, _dp, _dp, _dp, _dp]),
+        "ora_image": (None, [C.c_void_p, C.POINTER(_Events), C.POINTER(Observer), C.c_int, C.c_int, C.c_int,
+                             C.c_int, _dp, C.c_void_p, C.POINTER(OracleStats)]),
+    }
+    for name, (res, args) in sig.items():
+        f = getattr(L, name)
+        f.restype, f.argtypes = res, args
+    _lib = L
+    return L
+
+
+def _v(x, n):
+    a = np.ascontiguousarray(np.asarray(x, np.float64).reshape(n))
+    return a
+
+
+class OracleModel:
+    """Grid + tables + source.  density [nz,ny,nx] f32 (kappa*rho per unit length),
+    bfield [nz,ny,nx,3] f32 or None, mueller [n_ang,4] f32 (S11,S12,S33,S34 on
+    Theta_j = j*180/(n_ang-1) deg), opac [n_inc,4] f32 (a1,a2,a3,albedo on
+    mu_m = m/(n_inc-1), mu = |cos(angle(n,B))|)."""
+
+    def __init__(self, nx, ny, nz, bounds, density, bfield, mueller, opac, w_min=1e-4, max_scatter=64):
+        L = lib()
+        self.nx, self.ny, self.nz = int(nx), int(ny), int(nz)
+        self.bounds = _v(bounds, 6)
+        self.density = np.ascontiguousarray(np.asarray(density, np.float32).reshape(nz, ny, nx))
+        self.bfield = None if bfield is None else np.ascontiguousarray(
+            np.asarray(bfield, np.float32).reshape(nz, ny, nx, 3))
+        self.mueller = np.ascontiguousarray(np.asarray(mueller, np.float32).reshape(-1, 4))
+        self.opac = np.ascontiguousarray(np.asarray(opac, np.float32).reshape(-1, 4))
+        self._w = None
+        self.h = L.ora_model_create(self.nx, self.ny, self.nz, self.bounds, self.density.ctypes.data,
+                                    None if self.bfield is None else self.bfield.ctypes.data,
+                                    self.mueller.shape[0], self.mueller, self.opac.shape[0], self.opac,
+                                    float(w_min), int(max_scatter))
+        ctr = [(self.bounds[0] + self.bounds[1]) / 2, (self.bounds[2] + self.bounds[3]) / 2,
+               (self.bounds[4] + self.bounds[5]) / 2]
+        self.source_set(0, ctr, [0, 0, 1], None, 0)
+
+    def __del__(self):
+        if getattr(self, "h", None):
+            lib().ora_model_free(self.h)
+            self.h = None
+
+    def source_set(self, kind, pos, direction, cell_weight=None, emit_records=0):
+        """kind bit0: volume (else point at pos); bit1: collimated along direction (else isotropic)."""
+        self._w = None if cell_weight is None else np.ascontiguousarray(np.asarray(cell_weight, np.float32).ravel())
+        lib().ora_source_set(self.h, int(kind), _v(pos, 3), _v(direction, 3),
+                             None if self._w is None else self._w.ctypes.data, int(emit_records))
+
+    # --- per-step functions (pins) ---
+    def mueller_at(self, theta_deg):
+        F = np.zeros(4); lib().ora_mueller_at(self.h, float(theta_deg), F); return F
+
+    def opac_at(self, mu):
+        a = np.zeros(4); lib().ora_opac_at(self.h, float(mu), a); return a
+
+    def dda_exit(self, p, n):
+        ax = C.c_int(-1)
+        t = lib().ora_dda_exit(self.h, _v(p, 3), _v(n, 3), C.byref(ax))
+        return t, ax.value
+
+    def cell_step(self, b, n, S, dtau):
+        S = _v(S, 4).copy(); lib().ora_cell_step(self.h, _v(b, 3), _v(n, 3), S, float(dtau)); return S
+
+    def march(self, idx, p, n, S, log_cap=0):
+        S = _v(S, 4).copy()
+        lc = np.zeros(max(log_cap, 1), np.int64); ld = np.zeros(max(log_cap, 1), np.float64)
+        steps = lib().ora_march(self.h, np.ascontiguousarray(np.asarray(idx, np.int32)), _v(p, 3), _v(n, 3), S,
+                                int(log_cap), lc.ctypes.data, ld.ctypes.data)
+        m = min(int(steps), log_cap)
+        return S, int(steps), lc[:m], ld[:m]
+
+    def sample_theta(self, u):
+        return lib().ora_sample_theta(self.h, float(u))
+
+    def scatter_angles(self, b, n_in, S_in, theta_deg, phi):
+        no = np.zeros(3); So = np.zeros(4)
+        lib().ora_scatter_angles(self.h, _v(b, 3), _v(n_in, 3), _v(S_in, 4), float(theta_deg), float(phi), no, So)
+        return no, So
+
+    def scatter(self, b, n_in, S_in, seed, pid, k):
+        no = np.zeros(3); So = np.zeros(4); tn = C.c_double(0)
+        r = lib().ora_scatter(self.h, _v(b, 3), _v(n_in, 3), _v(S_in, 4), int(seed), int(pid), int(k), no, So,
+                              C.byref(tn))
+        return no, So, tn.value, r
+
+    def peel(self, n_in, S_in, n_obs):
+        So = np.zeros(4); lib().ora_peel(self.h, _v(n_in, 3), _v(S_in, 4), _v(n_obs, 3), So); return So
+
+    # --- whole-path functions ---
+    def transport(self, id0, n_packets, seed, events, stats=None, esc_cap=0):
+        st = stats if stats is not None else OracleStats()
+        esc = None
+        if esc_cap > 0:
+            esc = dict(n=np.zeros((esc_cap, 3)), S=np.zeros((esc_cap, 4)), id=np.zeros(esc_cap, np.uint64),
+                       k=np.zeros(esc_cap, np.int32))
+            ne = lib().ora_transport(self.h, int(id0), int(n_packets), int(seed), C.byref(events.c), C.byref(st),
+                                     int(esc_cap), esc["n"].ctypes.data, esc["S"].ctypes.data,
+                                     esc["id"].ctypes.data, esc["k"].ctypes.data)
+            esc = {k: v[:ne] for k, v in esc.items()}
+        else:
+            lib().ora_transport(self.h, int(id0), int(n_packets), int(seed), C.byref(events.c), C.byref(st),
+                                0, None, None, None, None)
+        return st, esc
+
+    def image(self, events, observers, npx, npy, flags=0, stats=None, second_moment=True):
+        st = stats if stats is not None else OracleStats()
+        n_obs = len(observers)
+        arr = (Observer * n_obs)(*observers)
+        img = np.zeros((n_obs, 4, npy, npx)); img2 = np.zeros_like(img) if second_moment else None
+        lib().ora_image(self.h, C.byref(events.c), arr, n_obs, int(npx), int(npy), int(flags), img,
+                        None if img2 is None else img2.ctypes.data, C.byref(st))
+        return img, img2, st
