@@ -1,0 +1,171 @@
+/*
+ * krp.h -- C ABI of the B200-native polarized Monte-Carlo radiative-transfer hot path
+ * (Kratos-polrad, arxiv 2512.01283; citations are PAPER.md:<line> of the extracted paper
+ * text, "R<n>" are the readings listed in DESIGN.md).
+ *
+ * The library computes, on one GPU and entirely in its own CUDA kernels:
+ *   transport  photon packets through a uniform Cartesian grid (cell interface to cell
+ *              interface) with Stokes-dependent extinction solved analytically
+ *              inside each cell (App. A), scattering in the grain frame
+ *              reached through the quaternion q_B (eq. 1-7) with angles
+ *              sampled from the tabulated Mueller matrix;
+ *   imaging    the second step of the two-step scheme (eq. 10-11): every
+ *              recorded scattering event sends its Stokes vector toward every observer and
+ *              is attenuated cell by cell to the grid edge, then summed into I,Q,U,V maps.
+ *
+ * Conventions
+ *   - every function returns KRP_OK (0) or a negative error code; it never throws or exits.
+ *     krp_last_error() gives a thread-local message for the last failing call.
+ *   - "DEVICE" pointers are CUDA device pointers valid on the current device, "HOST" pointers
+ *     are ordinary host memory.  The library copies what it needs: the caller keeps
+ *     ownership of every array it passes and may free it once the call's stream work is done
+ *     (for HOST inputs: as soon as the call returns).
+ *   - `stream` is a cudaStream_t passed as void* (NULL = the legacy default stream).  All
+ *     work is enqueued on it; only the calls marked "synchronises" wait for the device.
+ *   - arrays over cells are [nz][ny][nx] (x fastest).
+ *   - one krp_grid may be used from one host thread at a time.
+ */
+#ifndef KRP_H_
+#define KRP_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+enum {
+    KRP_OK = 0,
+    KRP_ERR_ARG = -1,        /* invalid argument (message says which) */
+    KRP_ERR_CUDA = -2,       /* a CUDA runtime call failed */
+    KRP_ERR_OOM = -3,        /* device allocation failed */
+    KRP_ERR_STATE = -4,      /* call made in the wrong order (e.g. image_get before image) */
+    KRP_ERR_EVENT_FULL = -5  /* the event buffer overflowed; see krp_stats.overflow */
+};
+
+enum { KRP_MEM_DEVICE = 0, KRP_MEM_HOST = 1 };
+
+const char* krp_last_error(void);
+/* library identification: "krp <version> sm_100a" */
+const char* krp_version(void);
+
+typedef struct krp_grid krp_grid; /* opaque; owns all device memory of one model */
+
+/* Lookup tables ("interpolation tables"; R8, R13).  HOST pointers, copied.
+ *   mueller  [n_ang][4] = S11,S12,S33,S34 on Theta_j = j*180/(n_ang-1) degrees, n_ang >= 2,
+ *            S11 > 0 and S11^2 >= S12^2+S33^2+S34^2 on every node; S11 need not be normalised
+ *            for sampling, but image units assume (1/2) int S11 sin(Theta) dTheta = 1.
+ *   opacity  [n_inc][4] = alpha1, alpha2, alpha3, albedo on mu_m = m/(n_inc-1),
+ *            mu = |cos(angle between n^ and B^)|, n_inc >= 1 (n_inc = 1: constant);
+ *            alpha1 > |alpha2|, 0 <= albedo <= 1.  The alphas are the elements of the App. A
+ *            matrix (R1) per unit of density*length.
+ *   w_min, max_scatter   a packet stops after a scattering that leaves its weight below
+ *            w_min or after max_scatter scatterings (R12; deterministic, no roulette). */
+typedef struct krp_tables {
+    int n_ang;
+    const float* mueller;
+    int n_inc;
+    const float* opacity;
+    float w_min;
+    int max_scatter;
+} krp_tables;
+
+/* Build a model.  bounds = xlo,xhi,ylo,yhi,zlo,zhi (HOST).  density [nz][ny][nx] >= 0 is
+ * kappa*rho per unit length (PAPER.md:101 lambda_ext^-1).  bfield [nz][ny][nx][3], any
+ * norm, zero vector = unaligned cell (B^ = z^), may be NULL (B^ = z^ everywhere).
+ * `mem` says where density/bfield live (KRP_MEM_DEVICE or KRP_MEM_HOST).  Cells are packed
+ * into the library's own layout here (not timed as part of the hot path).
+ * Errors: KRP_ERR_ARG for non-positive dims, non-increasing bounds, bad tables. */
+int krp_grid_create(krp_grid** out, int nx, int ny, int nz, const double bounds[6],
+                    const float* density, const float* bfield, int mem,
+                    const krp_tables* tables, void* stream);
+int krp_grid_destroy(krp_grid* g);
+
+/* Source of packets (PAPER.md:107 emission; R17).
+ *   kind bit0: 0 = all packets start at pos, 1 = start uniformly inside a cell drawn with
+ *              probability proportional to cell_weight (DEVICE, [ncell]; NULL = uniform);
+ *   kind bit1: 0 = isotropic directions, 1 = all along dir (need not be normalised).
+ *   emit_records != 0 also appends an "emission record" (event index k = 0) per packet so
+ *   that krp_image(flags bit0) can add the direct, unscattered light.
+ * Every packet starts unpolarised, Stokes (1,0,0,0), weight 1. */
+typedef struct krp_source {
+    int kind;
+    double pos[3];
+    double dir[3];
+    const float* cell_weight;
+    int emit_records;
+} krp_source;
+int krp_source_set(krp_grid* g, const krp_source* src, void* stream);
+
+/* Capacity of the event buffer (events held between krp_transport and krp_image).
+ * Optional: krp_transport grows it to 4 events per packet (at least 2^20) when unset.
+ * Events beyond the capacity are dropped, the packet stops, krp_stats.overflow counts them
+ * and the next synchronising call returns KRP_ERR_EVENT_FULL. */
+int krp_events_reserve(krp_grid* g, uint64_t max_events);
+
+/* Transport packets with global ids [next_id, next_id + n_packets) (next_id starts at 0 and
+ * persists across calls; krp_packet_id_set changes it), Philox4x32-10 keyed by `seed` with the
+ * counter schedule R11, so results do not depend on how the caller batches.  Appends one
+ * record per scattering event: position, cell, incoming direction, albedo*weight and the
+ * normalised Stokes state in the lab reference.  Does not synchronise. */
+int krp_transport(krp_grid* g, uint64_t n_packets, uint64_t seed, void* stream);
+int krp_packet_id_set(krp_grid* g, uint64_t next_id);
+
+/* Observer: direction toward the observer (theta, phi in radians, global spherical angles),
+ * image plane centred on `center` with half extents half_w (along phi^_obs, image x) and
+ * half_h (along -theta^_obs, image y); orthographic (R14). */
+typedef struct krp_observer {
+    double theta, phi;
+    double center[3];
+    double half_w, half_h;
+} krp_observer;
+
+/* Image every buffered event toward every observer (obs: HOST array) and add the result to
+ * the internal fp64 maps [n_obs][4][npix_y][npix_x] (I,Q,U,V relative to theta^_obs, sum of
+ * contributions per pixel, no area normalisation, R14).  flags bit0: include emission
+ * records (direct light).  Clears the event buffer afterwards.  The maps are (re)allocated
+ * and zeroed when the observer set or the pixel counts differ from the previous call.
+ * Does not synchronise. */
+int krp_image(krp_grid* g, const krp_observer* obs, int n_obs, int npix_x, int npix_y,
+              int flags, void* stream);
+/* Copy the maps to out ([n_obs][4][npix_y][npix_x] doubles; `mem` = where out lives).
+ * Synchronises when out is HOST memory. */
+int krp_image_get(krp_grid* g, double* out, int mem, void* stream);
+int krp_image_reset(krp_grid* g, void* stream);
+
+/* Counters (also the numerators of the roofline figures). */
+typedef struct krp_stats {
+    uint64_t packets;         /* packets emitted */
+    uint64_t events;          /* scattering events recorded */
+    uint64_t records;         /* emission records recorded */
+    uint64_t steps_transport; /* cell steps taken by transport flights */
+    uint64_t steps_image;     /* cell steps taken by imaging rays */
+    uint64_t contributions;   /* image contributions deposited */
+    uint64_t dropped;         /* contributions that fell outside the frame */
+    uint64_t overflow;        /* events lost to a full event buffer */
+    double w_emitted, w_escaped, w_absorbed, w_cut;
+} krp_stats;
+int krp_stats_get(krp_grid* g, krp_stats* out);  /* synchronises */
+int krp_stats_reset(krp_grid* g, void* stream);
+
+/* Debug / parity: dump the buffered events (HOST arrays of capacity cap, any may be NULL).
+ *   id[i], k[i]  packet id and event index (0 = emission record, k >= 1 = k-th scattering)
+ *   cell[i]      linear cell index (x fastest)
+ *   pos[i][3]    cell-local position in [0,1]^3
+ *   dir[i][3]    incoming direction n^_in
+ *   stokes[i][4] albedo*weight*(1,q,u,v), lab reference of n^_in
+ * *n receives the number of buffered events (which may exceed cap; only min(*n,cap) are
+ * written).  Order is not defined (the buffer is filled with atomics).  Synchronises. */
+int krp_events_get(krp_grid* g, uint64_t cap, uint64_t* n, uint64_t* id, int32_t* k,
+                   int64_t* cell, float* pos, float* dir, float* stokes);
+int krp_events_clear(krp_grid* g, void* stream);
+
+/* Launch-shape knobs, for measurement only (0 keeps the default). */
+int krp_tune(krp_grid* g, int transport_block, int image_block, int blocks_per_sm);
+/* Number of kernels the library has launched on behalf of g since creation. */
+uint64_t krp_launch_count(const krp_grid* g);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* KRP_H_ */

@@ -1,0 +1,550 @@
+// krp_api.cu -- the C ABI of include/krp.h: argument checks, device memory, table building,
+// kernel launches on the caller's stream.  No arithmetic of the method lives on the host
+// except the one-off table preparation (Theta CDF, observer bases).
+#include "../../include/krp.h"
+#include "krp_kernels.cuh"
+
+#include <cub/device/device_scan.cuh>
+
+#include <cmath>
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <new>
+#include <vector>
+
+static thread_local char g_err[512] = "";
+
+static int fail(int code, const char* fmt, ...)
+{
+    va_list ap;
+    va_start(ap, fmt);
+    vsnprintf(g_err, sizeof(g_err), fmt, ap);
+    va_end(ap);
+    return code;
+}
+
+#define CK(call)                                                                                   \
+    do {                                                                                           \
+        cudaError_t e_ = (call);                                                                   \
+        if (e_ != cudaSuccess)                                                                     \
+            return fail(e_ == cudaErrorMemoryAllocation ? KRP_ERR_OOM : KRP_ERR_CUDA, "%s: %s", #call, \
+                        cudaGetErrorString(e_));                                                   \
+    } while (0)
+
+struct krp_grid {
+    KrpModel m;
+    int device = 0, n_sm = 0;
+    // owned device memory
+    float* d_kr = nullptr;
+    float4* d_cell = nullptr;
+    float4* d_opac = nullptr;
+    float4* d_mueller = nullptr;
+    double* d_cdf = nullptr;
+    double* d_src_cdf = nullptr;
+    KrpCtl* d_ctl = nullptr;
+    KrpRecords q[2] = {};
+    uint64_t q_cap = 0;
+    KrpRecords ev = {};
+    uint64_t ev_cap = 0;
+    bool ev_reserved = false;
+    KrpObserverDev* d_obs = nullptr;
+    double* d_img = nullptr;
+    int n_obs = 0, npx = 0, npy = 0;
+    std::vector<krp_observer> obs_host;
+    uint64_t next_id = 0;
+    uint64_t launches = 0;
+    int max_waves = 0;
+    int transport_block = 256, image_block = 256, blocks_per_sm = 8;
+};
+
+extern "C" const char* krp_last_error(void) { return g_err; }
+extern "C" const char* krp_version(void) { return "krp 0.1 sm_100a"; }
+
+static void free_records(KrpRecords& r)
+{
+    cudaFree(r.pc); cudaFree(r.nk); cudaFree(r.S); cudaFree(r.tau); cudaFree(r.id);
+    r = KrpRecords{};
+}
+
+static int alloc_records(KrpRecords& r, uint64_t cap, bool with_tau)
+{
+    CK(cudaMalloc(&r.pc, cap * sizeof(float4)));
+    CK(cudaMalloc(&r.nk, cap * sizeof(float4)));
+    CK(cudaMalloc(&r.S, cap * sizeof(float4)));
+    if (with_tau) CK(cudaMalloc(&r.tau, cap * sizeof(double)));
+    CK(cudaMalloc(&r.id, cap * sizeof(unsigned long long)));
+    return KRP_OK;
+}
+
+extern "C" int krp_grid_destroy(krp_grid* g)
+{
+    if (!g) return KRP_OK;
+    cudaFree(g->d_kr); cudaFree(g->d_cell); cudaFree(g->d_opac); cudaFree(g->d_mueller); cudaFree(g->d_cdf);
+    cudaFree(g->d_src_cdf); cudaFree(g->d_ctl); cudaFree(g->d_obs); cudaFree(g->d_img);
+    free_records(g->q[0]); free_records(g->q[1]); free_records(g->ev);
+    delete g;
+    return KRP_OK;
+}
+
+static int check_tables(const krp_tables* t)
+{
+    if (!t) return fail(KRP_ERR_ARG, "tables is NULL");
+    if (t->n_ang < 2 || !t->mueller) return fail(KRP_ERR_ARG, "tables: n_ang must be >= 2 and mueller non-NULL");
+    if (t->n_inc < 1 || !t->opacity) return fail(KRP_ERR_ARG, "tables: n_inc must be >= 1 and opacity non-NULL");
+    if (!(t->w_min >= 0.f)) return fail(KRP_ERR_ARG, "tables: w_min must be >= 0");
+    if (t->max_scatter < 1) return fail(KRP_ERR_ARG, "tables: max_scatter must be >= 1");
+    for (int j = 0; j < t->n_ang; ++j) {
+        const float* f = t->mueller + 4 * j;
+        for (int s = 0; s < 4; ++s)
+            if (!std::isfinite(f[s])) return fail(KRP_ERR_ARG, "tables: mueller[%d][%d] is not finite", j, s);
+        if (!(f[0] > 0.f)) return fail(KRP_ERR_ARG, "tables: S11 must be positive (node %d)", j);
+        double lhs = (double)f[0] * f[0] * (1.0 + 1e-6), rhs = (double)f[1] * f[1] + (double)f[2] * f[2] + (double)f[3] * f[3];
+        if (lhs < rhs) return fail(KRP_ERR_ARG, "tables: S11^2 < S12^2+S33^2+S34^2 at node %d", j);
+    }
+    for (int j = 0; j < t->n_inc; ++j) {
+        const float* a = t->opacity + 4 * j;
+        for (int s = 0; s < 4; ++s)
+            if (!std::isfinite(a[s])) return fail(KRP_ERR_ARG, "tables: opacity[%d][%d] is not finite", j, s);
+        if (!(a[0] > std::fabs(a[1]))) return fail(KRP_ERR_ARG, "tables: alpha1 must exceed |alpha2| (node %d)", j);
+        if (!(a[3] >= 0.f && a[3] <= 1.f)) return fail(KRP_ERR_ARG, "tables: albedo outside [0,1] (node %d)", j);
+    }
+    return KRP_OK;
+}
+
+extern "C" int krp_grid_create(krp_grid** out, int nx, int ny, int nz, const double bounds[6], const float* density,
+                               const float* bfield, int mem, const krp_tables* tables, void* stream)
+{
+    if (!out) return fail(KRP_ERR_ARG, "out is NULL");
+    *out = nullptr;
+    if (nx < 1 || ny < 1 || nz < 1) return fail(KRP_ERR_ARG, "grid dims must be positive (%d,%d,%d)", nx, ny, nz);
+    if ((uint64_t)nx * ny * nz >= (1ull << 31)) return fail(KRP_ERR_ARG, "grid has too many cells (limit 2^31)");
+    if (!bounds) return fail(KRP_ERR_ARG, "bounds is NULL");
+    for (int a = 0; a < 3; ++a)
+        if (!(bounds[2 * a + 1] > bounds[2 * a]) || !std::isfinite(bounds[2 * a]) || !std::isfinite(bounds[2 * a + 1]))
+            return fail(KRP_ERR_ARG, "bounds must be finite and increasing on axis %d", a);
+    if (!density) return fail(KRP_ERR_ARG, "density is NULL");
+    if (mem != KRP_MEM_DEVICE && mem != KRP_MEM_HOST) return fail(KRP_ERR_ARG, "mem must be KRP_MEM_DEVICE or KRP_MEM_HOST");
+    int rc = check_tables(tables);
+    if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+
+    krp_grid* g = new (std::nothrow) krp_grid();
+    if (!g) return fail(KRP_ERR_OOM, "host allocation failed");
+    struct Guard { krp_grid* g; ~Guard() { if (g) krp_grid_destroy(g); } } guard{ g };
+
+    CK(cudaGetDevice(&g->device));
+    CK(cudaDeviceGetAttribute(&g->n_sm, cudaDevAttrMultiProcessorCount, g->device));
+    KrpModel& m = g->m;
+    memset(&m, 0, sizeof(m));
+    m.nx = nx; m.ny = ny; m.nz = nz; m.ncell = (uint32_t)((uint64_t)nx * ny * nz);
+    const int dims[3] = { nx, ny, nz };
+    for (int a = 0; a < 3; ++a) {
+        m.lo[a] = bounds[2 * a];
+        m.dd[a] = (bounds[2 * a + 1] - bounds[2 * a]) / dims[a];
+        m.d[a] = (float)m.dd[a];
+    }
+    // opacity table: n_inc = 1 becomes two equal rows so that the kernels always interpolate
+    const int n_inc = tables->n_inc == 1 ? 2 : tables->n_inc;
+    std::vector<float> op(4 * (size_t)n_inc);
+    for (int j = 0; j < n_inc; ++j)
+        memcpy(&op[4 * j], tables->opacity + 4 * (tables->n_inc == 1 ? 0 : j), 4 * sizeof(float));
+    bool constant = true, dichroic = false;
+    float rho = 0.f;
+    for (int j = 0; j < n_inc; ++j) {
+        for (int s = 0; s < 4; ++s) constant = constant && (op[4 * j + s] == op[s]);
+        dichroic = dichroic || op[4 * j + 1] != 0.f || op[4 * j + 2] != 0.f;
+        rho = std::fmax(rho, std::fabs(op[4 * j + 1]) / op[4 * j]);
+    }
+    m.scalar = (constant && !dichroic && bfield == nullptr) ? 1 : 0;
+    m.a1c = op[0]; m.omc = op[3]; m.rho = rho;
+    m.n_inc = n_inc; m.n_ang = tables->n_ang;
+    m.w_min = tables->w_min; m.max_scatter = tables->max_scatter;
+    // number of waves that can contain live packets: the weight after k scatterings is <= omega_max^k
+    {
+        float om_max = 0.f;
+        for (int j = 0; j < n_inc; ++j) om_max = std::fmax(om_max, op[4 * j + 3]);
+        int waves = tables->max_scatter;
+        if (om_max <= 0.f) waves = 1;
+        else if (om_max < 1.f && tables->w_min > 0.f) {
+            double kk = std::ceil(std::log((double)tables->w_min) / std::log((double)om_max)) + 1.0;
+            if (kk < waves) waves = (int)std::fmax(kk, 1.0);
+        }
+        g->max_waves = waves;
+    }
+    CK(cudaMalloc(&g->d_opac, sizeof(float4) * n_inc));
+    CK(cudaMemcpyAsync(g->d_opac, op.data(), sizeof(float4) * n_inc, cudaMemcpyHostToDevice, st));
+    CK(cudaMalloc(&g->d_mueller, sizeof(float4) * m.n_ang));
+    CK(cudaMemcpyAsync(g->d_mueller, tables->mueller, sizeof(float4) * m.n_ang, cudaMemcpyHostToDevice, st));
+    // Theta CDF: trapezoid of S11 sin(Theta) on the nodes, fp64 (R13)
+    std::vector<double> cdf(m.n_ang);
+    {
+        const double h = KRP_PI_D / (m.n_ang - 1);
+        double acc = 0.0, prev = 0.0;
+        cdf[0] = 0.0;
+        for (int j = 1; j < m.n_ang; ++j) {
+            double cur = (double)tables->mueller[4 * j] * std::sin(j * h);
+            acc += 0.5 * (prev + cur);
+            cdf[j] = acc;
+            prev = cur;
+        }
+        for (int j = 0; j < m.n_ang; ++j) cdf[j] /= acc;
+        cdf[m.n_ang - 1] = 1.0;
+    }
+    CK(cudaMalloc(&g->d_cdf, sizeof(double) * m.n_ang));
+    CK(cudaMemcpyAsync(g->d_cdf, cdf.data(), sizeof(double) * m.n_ang, cudaMemcpyHostToDevice, st));
+    m.opac = g->d_opac; m.mueller = g->d_mueller; m.cdf = g->d_cdf;
+
+    // cells
+    const float* d_den = density;
+    const float* d_b = bfield;
+    float* tmp_den = nullptr;
+    float* tmp_b = nullptr;
+    if (mem == KRP_MEM_HOST) {
+        if (m.scalar) {
+            // the packed layout of SCALAR mode is the density array itself
+            CK(cudaMalloc(&g->d_kr, sizeof(float) * (size_t)m.ncell));
+            CK(cudaMemcpyAsync(g->d_kr, density, sizeof(float) * (size_t)m.ncell, cudaMemcpyHostToDevice, st));
+            d_den = g->d_kr;
+        } else {
+            CK(cudaMalloc(&tmp_den, sizeof(float) * (size_t)m.ncell));
+            CK(cudaMemcpyAsync(tmp_den, density, sizeof(float) * (size_t)m.ncell, cudaMemcpyHostToDevice, st));
+            d_den = tmp_den;
+            if (bfield) {
+                CK(cudaMalloc(&tmp_b, sizeof(float) * 3 * (size_t)m.ncell));
+                CK(cudaMemcpyAsync(tmp_b, bfield, sizeof(float) * 3 * (size_t)m.ncell, cudaMemcpyHostToDevice, st));
+                d_b = tmp_b;
+            }
+        }
+    }
+    int* d_bad = nullptr;
+    CK(cudaMalloc(&d_bad, sizeof(int)));
+    CK(cudaMemsetAsync(d_bad, 0, sizeof(int), st));
+    if (m.scalar) {
+        if (!g->d_kr) CK(cudaMalloc(&g->d_kr, sizeof(float) * (size_t)m.ncell));
+    } else {
+        CK(cudaMalloc(&g->d_cell, sizeof(float4) * (size_t)m.ncell));
+    }
+    {
+        const int tb = 256;
+        const unsigned nb = (unsigned)((m.ncell + tb - 1) / tb);
+        krp_k_pack<<<nb, tb, 0, st>>>(d_den, d_b, m.ncell, g->d_cell, (m.scalar && d_den != g->d_kr) ? g->d_kr : nullptr, d_bad);
+        CK(cudaGetLastError());
+        g->launches++;
+    }
+    int bad = 0;
+    CK(cudaMemcpyAsync(&bad, d_bad, sizeof(int), cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    cudaFree(d_bad); cudaFree(tmp_den); cudaFree(tmp_b);
+    if (bad) return fail(KRP_ERR_ARG, "density has %d negative, NaN or infinite cells", bad);
+    m.kr = g->d_kr; m.cell = g->d_cell;
+
+    CK(cudaMalloc(&g->d_ctl, sizeof(KrpCtl)));
+    CK(cudaMemsetAsync(g->d_ctl, 0, sizeof(KrpCtl), st));
+    CK(cudaStreamSynchronize(st));
+    // default source: isotropic point source at the centre of the box
+    krp_source src;
+    memset(&src, 0, sizeof(src));
+    for (int a = 0; a < 3; ++a) src.pos[a] = 0.5 * (bounds[2 * a] + bounds[2 * a + 1]);
+    src.dir[2] = 1.0;
+    guard.g = nullptr;
+    rc = krp_source_set(g, &src, stream);
+    if (rc) { krp_grid_destroy(g); return rc; }
+    *out = g;
+    return KRP_OK;
+}
+
+extern "C" int krp_source_set(krp_grid* g, const krp_source* src, void* stream)
+{
+    if (!g || !src) return fail(KRP_ERR_ARG, "grid or source is NULL");
+    if (src->kind < 0 || src->kind > 3) return fail(KRP_ERR_ARG, "source kind must be in 0..3");
+    cudaStream_t st = (cudaStream_t)stream;
+    KrpModel& m = g->m;
+    if (src->kind & 2) {
+        double nn = src->dir[0] * src->dir[0] + src->dir[1] * src->dir[1] + src->dir[2] * src->dir[2];
+        if (!(nn > 0.0) || !std::isfinite(nn)) return fail(KRP_ERR_ARG, "collimated source needs a non-zero finite dir");
+    }
+    m.src_kind = src->kind; m.emit_records = src->emit_records ? 1 : 0;
+    const int dims[3] = { m.nx, m.ny, m.nz };
+    int idx[3];
+    for (int a = 0; a < 3; ++a) {
+        if (!std::isfinite(src->pos[a])) return fail(KRP_ERR_ARG, "source pos is not finite");
+        double x = (src->pos[a] - m.lo[a]) / m.dd[a];
+        int i = (int)std::floor(x);
+        i = i < 0 ? 0 : (i > dims[a] - 1 ? dims[a] - 1 : i);
+        double p = x - i;
+        p = p < 0.0 ? 0.0 : (p > 1.0 ? 1.0 : p);     // sources outside the box start on its surface
+        idx[a] = i; m.src_p[a] = (float)p;
+        m.src_n[a] = (float)src->dir[a];
+    }
+    m.src_cell = (uint32_t)(((int64_t)idx[2] * m.ny + idx[1]) * m.nx + idx[0]);
+    cudaFree(g->d_src_cdf); g->d_src_cdf = nullptr; m.src_cdf = nullptr;
+    if ((src->kind & 1) && src->cell_weight) {
+        double* tmp = nullptr;
+        CK(cudaMalloc(&tmp, sizeof(double) * (size_t)m.ncell));
+        CK(cudaMalloc(&g->d_src_cdf, sizeof(double) * (size_t)m.ncell));
+        const int tb = 256;
+        krp_k_f2d<<<(unsigned)((m.ncell + tb - 1) / tb), tb, 0, st>>>(src->cell_weight, m.ncell, tmp);
+        CK(cudaGetLastError());
+        void* scratch = nullptr; size_t bytes = 0;
+        CK(cub::DeviceScan::InclusiveSum(scratch, bytes, tmp, g->d_src_cdf, (int)m.ncell, st));
+        CK(cudaMalloc(&scratch, bytes));
+        CK(cub::DeviceScan::InclusiveSum(scratch, bytes, tmp, g->d_src_cdf, (int)m.ncell, st));
+        CK(cudaStreamSynchronize(st));
+        cudaFree(scratch); cudaFree(tmp);
+        g->launches += 2;
+        m.src_cdf = g->d_src_cdf;
+    }
+    return KRP_OK;
+}
+
+static int ensure_events(krp_grid* g, uint64_t cap)
+{
+    if (g->ev_cap >= cap) return KRP_OK;
+    // growing keeps nothing: only legal while the buffer is empty (checked by the callers)
+    free_records(g->ev);
+    g->ev_cap = 0;
+    int rc = alloc_records(g->ev, cap, false);
+    if (rc) { free_records(g->ev); return rc; }
+    g->ev_cap = cap;
+    return KRP_OK;
+}
+
+extern "C" int krp_events_reserve(krp_grid* g, uint64_t max_events)
+{
+    if (!g) return fail(KRP_ERR_ARG, "grid is NULL");
+    if (max_events < 1) return fail(KRP_ERR_ARG, "max_events must be positive");
+    CK(cudaDeviceSynchronize());
+    KrpCtl c;
+    CK(cudaMemcpy(&c, g->d_ctl, sizeof(c), cudaMemcpyDeviceToHost));
+    if (c.n_events != 0) return fail(KRP_ERR_STATE, "events_reserve with a non-empty event buffer");
+    if (max_events != g->ev_cap) { free_records(g->ev); g->ev_cap = 0; }
+    int rc = ensure_events(g, max_events);
+    if (rc) return rc;
+    g->ev_reserved = true;
+    unsigned long long cap = g->ev_cap;
+    CK(cudaMemcpy(&g->d_ctl->ev_cap, &cap, sizeof(cap), cudaMemcpyHostToDevice));
+    return KRP_OK;
+}
+
+extern "C" int krp_packet_id_set(krp_grid* g, uint64_t next_id)
+{
+    if (!g) return fail(KRP_ERR_ARG, "grid is NULL");
+    g->next_id = next_id;
+    return KRP_OK;
+}
+
+extern "C" int krp_transport(krp_grid* g, uint64_t n_packets, uint64_t seed, void* stream)
+{
+    if (!g) return fail(KRP_ERR_ARG, "grid is NULL");
+    if (n_packets == 0) return KRP_OK;
+    if (n_packets > 0x7fffffffull) return fail(KRP_ERR_ARG, "n_packets per call is limited to 2^31-1; batch the run");
+    cudaStream_t st = (cudaStream_t)stream;
+    if (g->q_cap < n_packets) {
+        CK(cudaStreamSynchronize(st));
+        free_records(g->q[0]); free_records(g->q[1]); g->q_cap = 0;
+        for (int s = 0; s < 2; ++s) {
+            int rc = alloc_records(g->q[s], n_packets, true);
+            if (rc) { free_records(g->q[0]); free_records(g->q[1]); return rc; }
+        }
+        g->q_cap = n_packets;
+    }
+    if (!g->ev_reserved && g->ev_cap < 4 * n_packets) {
+        // default capacity; only grown while the buffer is empty
+        CK(cudaStreamSynchronize(st));
+        KrpCtl c;
+        CK(cudaMemcpy(&c, g->d_ctl, sizeof(c), cudaMemcpyDeviceToHost));
+        if (c.n_events == 0 || g->ev_cap == 0) {
+            uint64_t cap = 4 * n_packets;
+            if (cap < (1ull << 20)) cap = 1ull << 20;
+            int rc = ensure_events(g, cap);
+            if (rc) return rc;
+            unsigned long long c64 = g->ev_cap;
+            CK(cudaMemcpy(&g->d_ctl->ev_cap, &c64, sizeof(c64), cudaMemcpyHostToDevice));
+        }
+    }
+    const unsigned n = (unsigned)n_packets;
+    const int tb = g->transport_block;
+    const unsigned grid_all = (n + 255u) / 256u;
+    krp_k_emit<<<grid_all, 256, 0, st>>>(g->m, g->d_ctl, g->q[0], g->ev, g->next_id, n, seed);
+    g->launches++;
+    unsigned pers = (unsigned)(g->n_sm * g->blocks_per_sm);
+    unsigned need = (n + tb - 1) / tb;
+    unsigned grid_f = need < pers ? need : pers;
+    unsigned grid_s = (n + 127u) / 128u;
+    if (grid_s > pers * 2) grid_s = pers * 2;
+    for (int w = 0; w < g->max_waves; ++w) {
+        const int in = w & 1;
+        krp_k_wave_prep<<<1, 1, 0, st>>>(g->d_ctl, in);
+        if (g->m.scalar) krp_k_flight<true><<<grid_f, tb, 0, st>>>(g->m, g->d_ctl, g->q[in], in, g->ev);
+        else             krp_k_flight<false><<<grid_f, tb, 0, st>>>(g->m, g->d_ctl, g->q[in], in, g->ev);
+        g->launches += 2;
+        if (w + 1 < g->max_waves) {
+            krp_k_scatter<<<grid_s, 128, 0, st>>>(g->m, g->d_ctl, g->ev, g->q[1 - in], 1 - in, seed);
+            g->launches++;
+        }
+    }
+    CK(cudaGetLastError());
+    g->next_id += n_packets;
+    return KRP_OK;
+}
+
+static void host_basis(const double n[3], double th[3], double ph[3])
+{
+    double s2 = n[0] * n[0] + n[1] * n[1], s = std::sqrt(s2), r = std::sqrt(s2 + n[2] * n[2]);
+    double cp = 1.0, sp = 0.0;
+    if (s2 >= 1e-24) { cp = n[0] / s; sp = n[1] / s; }
+    double ct = n[2] / r, st = s / r;
+    th[0] = ct * cp; th[1] = ct * sp; th[2] = -st;
+    ph[0] = -sp; ph[1] = cp; ph[2] = 0.0;
+}
+
+extern "C" int krp_image(krp_grid* g, const krp_observer* obs, int n_obs, int npix_x, int npix_y, int flags, void* stream)
+{
+    if (!g) return fail(KRP_ERR_ARG, "grid is NULL");
+    if (!obs || n_obs < 1) return fail(KRP_ERR_ARG, "need at least one observer");
+    if (npix_x < 1 || npix_y < 1) return fail(KRP_ERR_ARG, "pixel counts must be positive");
+    for (int o = 0; o < n_obs; ++o)
+        if (!(obs[o].half_w > 0.0) || !(obs[o].half_h > 0.0) || !std::isfinite(obs[o].theta) || !std::isfinite(obs[o].phi))
+            return fail(KRP_ERR_ARG, "observer %d: half extents must be positive and angles finite", o);
+    cudaStream_t st = (cudaStream_t)stream;
+    bool same = g->d_img && g->n_obs == n_obs && g->npx == npix_x && g->npy == npix_y &&
+                memcmp(g->obs_host.data(), obs, sizeof(krp_observer) * n_obs) == 0;
+    if (!same) {
+        CK(cudaStreamSynchronize(st));
+        cudaFree(g->d_img); cudaFree(g->d_obs); g->d_img = nullptr; g->d_obs = nullptr;
+        size_t bytes = sizeof(double) * 4 * (size_t)n_obs * npix_x * npix_y;
+        CK(cudaMalloc(&g->d_img, bytes));
+        CK(cudaMemsetAsync(g->d_img, 0, bytes, st));
+        std::vector<KrpObserverDev> od(n_obs);
+        for (int o = 0; o < n_obs; ++o) {
+            double st_ = std::sin(obs[o].theta), ct_ = std::cos(obs[o].theta);
+            double n[3] = { st_ * std::cos(obs[o].phi), st_ * std::sin(obs[o].phi), ct_ }, th[3], ph[3];
+            host_basis(n, th, ph);
+            for (int a = 0; a < 3; ++a) {
+                od[o].n[a] = (float)n[a]; od[o].th[a] = (float)th[a]; od[o].ph[a] = (float)ph[a];
+                od[o].thd[a] = th[a]; od[o].phd[a] = ph[a]; od[o].center[a] = obs[o].center[a];
+            }
+            od[o].inv_hw = 1.0 / obs[o].half_w; od[o].inv_hh = 1.0 / obs[o].half_h;
+        }
+        CK(cudaMalloc(&g->d_obs, sizeof(KrpObserverDev) * n_obs));
+        CK(cudaMemcpyAsync(g->d_obs, od.data(), sizeof(KrpObserverDev) * n_obs, cudaMemcpyHostToDevice, st));
+        CK(cudaStreamSynchronize(st));
+        g->obs_host.assign(obs, obs + n_obs);
+        g->n_obs = n_obs; g->npx = npix_x; g->npy = npix_y;
+    }
+    if (g->ev_cap == 0) return KRP_OK;   // nothing was ever transported
+    const int tb = g->image_block;
+    const unsigned grid = (unsigned)(g->n_sm * g->blocks_per_sm);
+    if (g->m.scalar) krp_k_image<true><<<grid, tb, 0, st>>>(g->m, g->d_ctl, g->ev, g->d_obs, n_obs, npix_x, npix_y, flags, g->d_img);
+    else             krp_k_image<false><<<grid, tb, 0, st>>>(g->m, g->d_ctl, g->ev, g->d_obs, n_obs, npix_x, npix_y, flags, g->d_img);
+    krp_k_events_clear<<<1, 1, 0, st>>>(g->d_ctl);
+    g->launches += 2;
+    CK(cudaGetLastError());
+    return KRP_OK;
+}
+
+extern "C" int krp_image_get(krp_grid* g, double* out, int mem, void* stream)
+{
+    if (!g || !out) return fail(KRP_ERR_ARG, "grid or out is NULL");
+    if (!g->d_img) return fail(KRP_ERR_STATE, "krp_image has not been called");
+    cudaStream_t st = (cudaStream_t)stream;
+    size_t bytes = sizeof(double) * 4 * (size_t)g->n_obs * g->npx * g->npy;
+    if (mem == KRP_MEM_HOST) {
+        CK(cudaMemcpyAsync(out, g->d_img, bytes, cudaMemcpyDeviceToHost, st));
+        CK(cudaStreamSynchronize(st));
+    } else if (mem == KRP_MEM_DEVICE) {
+        CK(cudaMemcpyAsync(out, g->d_img, bytes, cudaMemcpyDeviceToDevice, st));
+    } else {
+        return fail(KRP_ERR_ARG, "mem must be KRP_MEM_DEVICE or KRP_MEM_HOST");
+    }
+    return KRP_OK;
+}
+
+extern "C" int krp_image_reset(krp_grid* g, void* stream)
+{
+    if (!g) return fail(KRP_ERR_ARG, "grid is NULL");
+    if (!g->d_img) return KRP_OK;
+    size_t bytes = sizeof(double) * 4 * (size_t)g->n_obs * g->npx * g->npy;
+    CK(cudaMemsetAsync(g->d_img, 0, bytes, (cudaStream_t)stream));
+    return KRP_OK;
+}
+
+extern "C" int krp_stats_get(krp_grid* g, krp_stats* out)
+{
+    if (!g || !out) return fail(KRP_ERR_ARG, "grid or out is NULL");
+    CK(cudaDeviceSynchronize());
+    KrpCtl c;
+    CK(cudaMemcpy(&c, g->d_ctl, sizeof(c), cudaMemcpyDeviceToHost));
+    out->packets = c.stats.packets; out->events = c.stats.events; out->records = c.stats.records;
+    out->steps_transport = c.stats.steps_transport; out->steps_image = c.stats.steps_image;
+    out->contributions = c.stats.contributions; out->dropped = c.stats.dropped; out->overflow = c.stats.overflow;
+    out->w_emitted = c.stats.w_emitted; out->w_escaped = c.stats.w_escaped;
+    out->w_absorbed = c.stats.w_absorbed; out->w_cut = c.stats.w_cut;
+    if (c.stats.overflow) return fail(KRP_ERR_EVENT_FULL, "event buffer overflowed: %llu events lost (capacity %llu)",
+                                      (unsigned long long)c.stats.overflow, (unsigned long long)g->ev_cap);
+    return KRP_OK;
+}
+
+extern "C" int krp_stats_reset(krp_grid* g, void* stream)
+{
+    if (!g) return fail(KRP_ERR_ARG, "grid is NULL");
+    CK(cudaMemsetAsync(&g->d_ctl->stats, 0, sizeof(KrpStatsDev), (cudaStream_t)stream));
+    return KRP_OK;
+}
+
+extern "C" int krp_events_get(krp_grid* g, uint64_t cap, uint64_t* n, uint64_t* id, int32_t* k, int64_t* cell, float* pos,
+                              float* dir, float* stokes)
+{
+    if (!g || !n) return fail(KRP_ERR_ARG, "grid or n is NULL");
+    CK(cudaDeviceSynchronize());
+    KrpCtl c;
+    CK(cudaMemcpy(&c, g->d_ctl, sizeof(c), cudaMemcpyDeviceToHost));
+    uint64_t have = c.n_events < g->ev_cap ? c.n_events : g->ev_cap;
+    *n = have;
+    uint64_t m = have < cap ? have : cap;
+    if (m == 0) return KRP_OK;
+    std::vector<float4> pc(m), nk(m), S(m);
+    std::vector<unsigned long long> ids(m);
+    CK(cudaMemcpy(pc.data(), g->ev.pc, m * sizeof(float4), cudaMemcpyDeviceToHost));
+    CK(cudaMemcpy(nk.data(), g->ev.nk, m * sizeof(float4), cudaMemcpyDeviceToHost));
+    CK(cudaMemcpy(S.data(), g->ev.S, m * sizeof(float4), cudaMemcpyDeviceToHost));
+    CK(cudaMemcpy(ids.data(), g->ev.id, m * sizeof(unsigned long long), cudaMemcpyDeviceToHost));
+    for (uint64_t i = 0; i < m; ++i) {
+        uint32_t cb, kb;
+        memcpy(&cb, &pc[i].w, 4); memcpy(&kb, &nk[i].w, 4);
+        if (id) id[i] = ids[i];
+        if (k) k[i] = (int32_t)(kb & ~KRP_TERM_BIT);
+        if (cell) cell[i] = (int64_t)cb;
+        if (pos) { pos[3 * i] = pc[i].x; pos[3 * i + 1] = pc[i].y; pos[3 * i + 2] = pc[i].z; }
+        if (dir) { dir[3 * i] = nk[i].x; dir[3 * i + 1] = nk[i].y; dir[3 * i + 2] = nk[i].z; }
+        if (stokes) {
+            stokes[4 * i] = S[i].x; stokes[4 * i + 1] = S[i].x * S[i].y;
+            stokes[4 * i + 2] = S[i].x * S[i].z; stokes[4 * i + 3] = S[i].x * S[i].w;
+        }
+    }
+    return KRP_OK;
+}
+
+extern "C" int krp_events_clear(krp_grid* g, void* stream)
+{
+    if (!g) return fail(KRP_ERR_ARG, "grid is NULL");
+    krp_k_events_clear<<<1, 1, 0, (cudaStream_t)stream>>>(g->d_ctl);
+    g->launches++;
+    CK(cudaGetLastError());
+    return KRP_OK;
+}
+
+extern "C" int krp_tune(krp_grid* g, int transport_block, int image_block, int blocks_per_sm)
+{
+    if (!g) return fail(KRP_ERR_ARG, "grid is NULL");
+    auto okb = [](int b) { return b == 0 || (b >= 32 && b <= 256 && b % 32 == 0); };
+    if (!okb(transport_block) || !okb(image_block)) return fail(KRP_ERR_ARG, "block sizes must be multiples of 32 in 32..256");
+    if (blocks_per_sm < 0 || blocks_per_sm > 64) return fail(KRP_ERR_ARG, "blocks_per_sm must be in 0..64");
+    if (transport_block) g->transport_block = transport_block;
+    if (image_block) g->image_block = image_block;
+    if (blocks_per_sm) g->blocks_per_sm = blocks_per_sm;
+    return KRP_OK;
+}
+
+extern "C" uint64_t krp_launch_count(const krp_grid* g) { return g ? g->launches : 0; }

@@ -1,0 +1,308 @@
+// krp_device.cuh -- device-side building blocks of the polarized MCRT hot path (sm_100a).
+//
+// Citations: PAPER.md:<line> is the extracted text of arxiv 2512.01283; R<n> are the readings
+// in DESIGN.md.  Nothing here is shared with oracle/ (the fp64 CPU checker).
+//
+// Precision plan: the cell march is fp32; the two quantities that
+// decide *where* a packet scatters -- the optical depth still to go, D, and the normalised
+// intensity i -- are accumulated in fp64 from fp32 increments; scattering geometry (once per
+// event) is fp64 and the new direction is stored rounded to fp32 (R12).
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#define KRP_PI_D 3.14159265358979323846264338327950288
+#define KRP_TERM_BIT 0x80000000u
+
+// ------------------------------------------------------------------------------------------
+// by-value kernel parameters
+// ------------------------------------------------------------------------------------------
+struct KrpModel {
+    int nx, ny, nz;
+    uint32_t ncell;
+    float d[3];            // cell size per axis
+    double lo[3], dd[3];   // lower corner and cell size in fp64 (projection to the image)
+    const float* kr;       // SCALAR mode: kappa*rho per cell
+    const float4* cell;    // general mode: {kappa*rho, B^x, B^y, B^z}
+    const float4* opac;    // [n_inc] {alpha1, alpha2, alpha3, albedo} on mu_m = m/(n_inc-1)
+    int n_inc;
+    const float4* mueller; // [n_ang] {S11,S12,S33,S34}
+    int n_ang;
+    const double* cdf;     // [n_ang] Theta CDF of S11 sin(Theta)
+    float a1c, omc;        // SCALAR mode constants
+    float rho;             // max |alpha2|/alpha1 over the table
+    float w_min;
+    int max_scatter;
+    int scalar;
+    // source
+    int src_kind, emit_records;
+    float src_n[3];
+    uint32_t src_cell;
+    float src_p[3];
+    const double* src_cdf; // [ncell] running sum of cell weights or NULL
+};
+
+struct KrpStatsDev {
+    unsigned long long packets, events, records, steps_transport, steps_image, contributions, dropped, overflow;
+    double w_emitted, w_escaped, w_absorbed, w_cut;
+};
+
+struct KrpCtl {
+    unsigned long long n_events;   // fill of the event buffer (may run past ev_cap while a kernel is appending)
+    unsigned long long ev_begin;   // first event of the current wave
+    unsigned long long ev_cap;
+    unsigned int q_count[2];       // fill of the two packet queues
+    unsigned int work[2];          // dynamic work counters (march / image)
+    KrpStatsDev stats;
+};
+
+// packet queue / event buffer, structure of arrays
+struct KrpRecords {
+    float4* pc;                 // {p_x, p_y, p_z (cell-local, [0,1]), cell index bits}
+    float4* nk;                 // {n_x, n_y, n_z, k bits}
+    float4* S;                  // {W, q, u, v}: weight and normalised Stokes, lab reference of n
+    double* tau;                // queue only: optical depth to the next event
+    unsigned long long* id;     // global packet id
+};
+
+struct KrpObserverDev {
+    float n[3], th[3], ph[3];
+    double thd[3], phd[3], center[3], inv_hw, inv_hh;
+};
+
+// ------------------------------------------------------------------------------------------
+// S0  Philox4x32-10 (Salmon et al. 2011), counter = (id_lo, id_hi, k, block), key = seed (R11)
+// ------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint4 krp_philox(uint64_t seed, uint64_t id, uint32_t k, uint32_t blk)
+{
+    uint32_t c0 = (uint32_t)id, c1 = (uint32_t)(id >> 32), c2 = k, c3 = blk;
+    uint32_t k0 = (uint32_t)seed, k1 = (uint32_t)(seed >> 32);
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        const uint32_t M0 = 0xD2511F53u, M1 = 0xCD9E8D57u;
+        uint32_t h0 = __umulhi(M0, c0), l0 = M0 * c0;
+        uint32_t h1 = __umulhi(M1, c2), l1 = M1 * c2;
+        c0 = h1 ^ c1 ^ k0; c1 = l1; c2 = h0 ^ c3 ^ k1; c3 = l0;
+        k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
+    }
+    return make_uint4(c0, c1, c2, c3);
+}
+// (2j+1)/2^24 from the top 23 bits: exact in fp32 and fp64, never 0 or 1 (R11)
+__device__ __forceinline__ double krp_u01(uint32_t x) { return ((double)(x >> 9) + 0.5) * (1.0 / 8388608.0); }
+// 52-bit uniform from two words (volume-source cell pick)
+__device__ __forceinline__ double krp_u53(uint32_t x0, uint32_t x1)
+{
+    return ((double)(x0 >> 5) * 33554432.0 + (double)(x1 >> 7) + 0.5) * (1.0 / 4503599627370496.0);
+}
+
+// ------------------------------------------------------------------------------------------
+// A4  spherical basis of a direction (eq. 4-5), pole rule R10
+// ------------------------------------------------------------------------------------------
+template <typename T>
+__device__ __forceinline__ void krp_basis(const T n[3], T th[3], T ph[3])
+{
+    T s2 = n[0] * n[0] + n[1] * n[1];
+    T rr = sqrt(s2 + n[2] * n[2]);
+    T s = sqrt(s2);
+    T cp = T(1), sp = T(0);
+    if (s2 >= T(1e-24)) { cp = n[0] / s; sp = n[1] / s; }
+    T ct = n[2] / rr, st = s / rr;
+    th[0] = ct * cp; th[1] = ct * sp; th[2] = -st;
+    ph[0] = -sp; ph[1] = cp; ph[2] = T(0);
+}
+
+// ------------------------------------------------------------------------------------------
+// A11  cell-interface-to-interface march, R11b.  The ray keeps, per axis, the
+// distance still to go to the next face (re-based every step, so its rounding error is that
+// of a cell-local coordinate), the face-to-face distance, the linear-index stride and the
+// number of cells left before the grid edge.
+// ------------------------------------------------------------------------------------------
+struct KrpRay {
+    float rx, ry, rz;   // distance to the next x/y/z face
+    float tx, ty, tz;   // d/|n| per axis (inf when n = 0)
+    int sx, sy, sz;     // signed linear-index stride
+    int lx, ly, lz;     // cells left along the axis before leaving the grid
+    uint32_t c;         // linear cell index
+};
+
+__device__ __forceinline__ void krp_ray_axis(float n, float p, float d, int stride, int i, int N,
+                                             float& r, float& t, int& s, int& l)
+{
+    if (n > 0.f)      { t = d / n;  r = (1.f - p) * t; s = stride;  l = N - 1 - i; }
+    else if (n < 0.f) { t = d / -n; r = p * t;         s = -stride; l = i; }
+    else              { t = __int_as_float(0x7f800000); r = t; s = 0; l = 0x7fffffff; }
+}
+
+__device__ __forceinline__ void krp_ray_init(const KrpModel& g, uint32_t cell, const float p[3], const float n[3], KrpRay& r)
+{
+    int ix = (int)(cell % (uint32_t)g.nx);
+    uint32_t t = cell / (uint32_t)g.nx;
+    int iy = (int)(t % (uint32_t)g.ny), iz = (int)(t / (uint32_t)g.ny);
+    krp_ray_axis(n[0], p[0], g.d[0], 1, ix, g.nx, r.rx, r.tx, r.sx, r.lx);
+    krp_ray_axis(n[1], p[1], g.d[1], g.nx, iy, g.ny, r.ry, r.ty, r.sy, r.ly);
+    krp_ray_axis(n[2], p[2], g.d[2], g.nx * g.ny, iz, g.nz, r.rz, r.tz, r.sz, r.lz);
+    r.c = cell;
+}
+
+// length of the segment inside the current cell; ties x before y before z (R11b)
+__device__ __forceinline__ float krp_ray_ds(const KrpRay& r) { return fminf(r.rx, fminf(r.ry, r.rz)); }
+
+// cross the exit face; returns false when the ray leaves the grid
+__device__ __forceinline__ bool krp_ray_step(KrpRay& r, float ds)
+{
+    bool ax = (r.rx <= r.ry) & (r.rx <= r.rz);
+    bool ay = (!ax) & (r.ry <= r.rz);
+    bool az = !(ax | ay);
+    r.rx = ax ? r.tx : r.rx - ds;
+    r.ry = ay ? r.ty : r.ry - ds;
+    r.rz = az ? r.tz : r.rz - ds;
+    int s = ax ? r.sx : (ay ? r.sy : r.sz);
+    r.c += (uint32_t)s;
+    r.lx -= ax; r.ly -= ay; r.lz -= az;
+    return (r.lx | r.ly | r.lz) >= 0;
+}
+
+// cell-local position after moving `moved` from the point where the distances r were taken
+__device__ __forceinline__ float krp_local(float n, float r, float t, float moved, float p0)
+{
+    if (n == 0.f) return p0;
+    float f = (r - moved) / t;
+    f = fminf(fmaxf(f, 0.f), 1.f);
+    return n > 0.f ? 1.f - f : f;
+}
+
+// ------------------------------------------------------------------------------------------
+// D4  table look-ups, linear in the node variable (R13)
+// ------------------------------------------------------------------------------------------
+__device__ __forceinline__ float4 krp_opac_at(const float4* __restrict__ tab, int n_inc, float mu)
+{
+    mu = fminf(mu, 1.f);
+    float x = mu * (float)(n_inc - 1);
+    int j = min((int)x, n_inc - 2);
+    float w = x - (float)j;
+    float4 a = tab[j], b = tab[j + 1];
+    float w0 = 1.f - w;
+    return make_float4(w0 * a.x + w * b.x, w0 * a.y + w * b.y, w0 * a.z + w * b.z, w0 * a.w + w * b.w);
+}
+
+template <typename T>
+__device__ __forceinline__ void krp_mueller_at(const float4* __restrict__ tab, int n_ang, T theta_deg, T F[4])
+{
+    T x = theta_deg * (T)(n_ang - 1) / T(180);
+    int j = (int)floor(x);
+    j = max(0, min(j, n_ang - 2));
+    T w = x - (T)j, w0 = T(1) - w;
+    float4 a = tab[j], b = tab[j + 1];
+    F[0] = w0 * (T)a.x + w * (T)b.x; F[1] = w0 * (T)a.y + w * (T)b.y;
+    F[2] = w0 * (T)a.z + w * (T)b.z; F[3] = w0 * (T)a.w + w * (T)b.w;
+}
+
+// ------------------------------------------------------------------------------------------
+// A5  reference-frame angle between the lab basis (theta^, phi^) of n and the grain-frame
+// basis of the same ray (eq. 6-7, sign restored per R2).  theta^' expressed
+// in the lab is ((n.B)n - B)/sin(vartheta), so with a = theta^.B and b = phi^.B:
+// cos(eta) = -a/s, sin(eta) = -b/s, s^2 = a^2 + b^2; only 2*eta enters eq. 7.
+// ------------------------------------------------------------------------------------------
+template <typename T>
+__device__ __forceinline__ void krp_eta2(T a, T b, T& c2, T& s2)
+{
+    T ss = a * a + b * b;
+    if (ss < T(1e-24)) { c2 = T(1); s2 = T(0); return; }
+    T inv = T(1) / ss;
+    c2 = (a * a - b * b) * inv;
+    s2 = T(2) * a * b * inv;
+}
+
+// sinh(x) and cosh(x)-1 without cancellation for small x; |x| < ~80
+__device__ __forceinline__ void krp_sinh_coshm1(float x, float& sh, float& chm1)
+{
+    float ax = fabsf(x);
+    if (ax < 0.35f) {
+        float x2 = x * x;
+        sh = x * (1.f + x2 * (1.f / 6.f + x2 * (1.f / 120.f + x2 * (1.f / 5040.f))));
+        chm1 = x2 * (0.5f + x2 * (1.f / 24.f + x2 * (1.f / 720.f + x2 * (1.f / 40320.f))));
+    } else {
+        float e = expf(ax), ie = 1.f / e;
+        sh = copysignf(0.5f * (e - ie), x);
+        chm1 = 0.5f * (e + ie) - 1.f;
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// A12  source-free App. A solution (matrix of R1) over dtau in the grain-
+// frame reference, written for a Stokes vector carried as  e^{-A} (i, q, u, v):
+//   thin step  (|alpha2 dtau| < 0.35): returns the increment of i (so the caller can
+//       accumulate it in fp64), updates q,u,v, and the scalar depth grows by alpha1*dtau;
+//   thick step: the common factor e^{-|alpha2 dtau|} is moved into the scalar depth so that
+//       nothing overflows at dtau ~ 1e3.
+// On return `depth` is what was added to A.
+// ------------------------------------------------------------------------------------------
+__device__ __forceinline__ bool krp_appA(float i, float& qg, float& ug, float& v, float4 op, float dtau,
+                                         float& di, float& i_new, float& depth)
+{
+    float x = op.y * dtau, y = op.z * dtau;
+    float sy = 0.f, cy = 1.f;
+    if (y != 0.f) sincosf(y, &sy, &cy);
+    float ax = fabsf(x);
+    bool thick = ax >= 0.35f;
+    if (!thick) {
+        float sh, chm1;
+        krp_sinh_coshm1(x, sh, chm1);
+        di = i * chm1 - qg * sh;
+        float qn = qg + (qg * chm1 - i * sh);
+        float un = ug * cy - v * sy;
+        float vn = ug * sy + v * cy;
+        qg = qn; ug = un; v = vn;
+        i_new = i + di;
+        depth = op.x * dtau;
+    } else {
+        float E = expf(-2.f * ax);
+        float s = x > 0.f ? 1.f : -1.f;
+        float ip = 0.5f * ((i - s * qg) + (i + s * qg) * E);
+        float qp = 0.5f * ((qg - s * i) + (qg + s * i) * E);
+        float f = expf(-ax);
+        float un = f * (ug * cy - v * sy);
+        float vn = f * (ug * sy + v * cy);
+        i_new = ip; qg = qp; ug = un; v = vn;
+        di = 0.f;
+        depth = op.x * dtau - ax;
+    }
+    return thick;
+}
+
+// ------------------------------------------------------------------------------------------
+// warp-aggregated reservation of one slot per calling lane in a 64-bit / 32-bit counter
+// ------------------------------------------------------------------------------------------
+__device__ __forceinline__ unsigned long long krp_reserve64(unsigned long long* counter)
+{
+    unsigned m = __activemask();
+    int lane = threadIdx.x & 31;
+    int leader = __ffs(m) - 1;
+    unsigned long long base = 0;
+    if (lane == leader) base = atomicAdd(counter, (unsigned long long)__popc(m));
+    base = __shfl_sync(m, base, leader);
+    return base + (unsigned long long)__popc(m & ((1u << lane) - 1u));
+}
+__device__ __forceinline__ unsigned int krp_reserve32(unsigned int* counter)
+{
+    unsigned m = __activemask();
+    int lane = threadIdx.x & 31;
+    int leader = __ffs(m) - 1;
+    unsigned int base = 0;
+    if (lane == leader) base = atomicAdd(counter, (unsigned int)__popc(m));
+    base = __shfl_sync(m, base, leader);
+    return base + (unsigned int)__popc(m & ((1u << lane) - 1u));
+}
+
+__device__ __forceinline__ double krp_warp_sum(double v)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}
+__device__ __forceinline__ unsigned long long krp_warp_sum(unsigned long long v)
+{
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+    return v;
+}

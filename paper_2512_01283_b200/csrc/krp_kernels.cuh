@@ -1,0 +1,562 @@
+// krp_kernels.cuh -- the kernels of the hot path: emit, flight (cell march to the next
+// event), scatter, image.  See DESIGN.md "Kernels".  Transport is a wavefront pipeline:
+//   emit -> [ wave_prep -> flight -> scatter ] x waves
+// Flights run in fp32 and never execute scattering code; lanes that reach an event park the
+// packet in the event buffer, and the scatter kernel (fp64 geometry, all lanes busy) turns the
+// wave's events into the next queue.  The event buffer is what the imaging kernel consumes.
+#pragma once
+#include "krp_device.cuh"
+
+// ------------------------------------------------------------------------------------------
+// T1/T2  emission: draws of block 0 = (cos theta, phi, tau*, spare); blocks 1-2
+// place a volume-source packet (R11, R17).  One thread per packet.
+// ------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) krp_k_emit(KrpModel g, KrpCtl* ctl, KrpRecords q, KrpRecords ev,
+                                                  unsigned long long id0, unsigned int n, unsigned long long seed)
+{
+    unsigned int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i == 0) {
+        ctl->q_count[0] = n; ctl->q_count[1] = 0;
+        atomicAdd(&ctl->stats.packets, (unsigned long long)n);
+        atomicAdd(&ctl->stats.w_emitted, (double)n);
+    }
+    if (i >= n) return;
+    unsigned long long id = id0 + i;
+    uint4 w = krp_philox(seed, id, 0u, 0u);
+    double tau = -log(krp_u01(w.z));
+    float nn[3];
+    if (g.src_kind & 2) {
+        nn[0] = g.src_n[0]; nn[1] = g.src_n[1]; nn[2] = g.src_n[2];
+    } else {
+        double ct = 1.0 - 2.0 * krp_u01(w.x);
+        double st = sqrt(1.0 - ct * ct);
+        double sp, cp;
+        sincos(2.0 * KRP_PI_D * krp_u01(w.y), &sp, &cp);
+        nn[0] = (float)(st * cp); nn[1] = (float)(st * sp); nn[2] = (float)ct;   // R12
+    }
+    uint32_t cell; float p[3];
+    if (g.src_kind & 1) {
+        uint4 w1 = krp_philox(seed, id, 0u, 1u), w2 = krp_philox(seed, id, 0u, 2u);
+        double u = krp_u53(w1.x, w1.y);
+        if (g.src_cdf) {
+            double x = u * g.src_cdf[g.ncell - 1];
+            long long lo = -1, hi = (long long)g.ncell - 1;      // smallest c with cdf[c] > x
+            while (hi - lo > 1) { long long mid = lo + (hi - lo) / 2; if (g.src_cdf[mid] > x) hi = mid; else lo = mid; }
+            cell = (uint32_t)hi;
+        } else {
+            double c = floor(u * (double)g.ncell);
+            cell = (uint32_t)fmin(c, (double)(g.ncell - 1));
+        }
+        p[0] = (float)krp_u01(w2.x); p[1] = (float)krp_u01(w2.y); p[2] = (float)krp_u01(w2.z);
+    } else {
+        cell = g.src_cell; p[0] = g.src_p[0]; p[1] = g.src_p[1]; p[2] = g.src_p[2];
+    }
+    float4 pc = make_float4(p[0], p[1], p[2], __uint_as_float(cell));
+    q.pc[i] = pc;
+    q.nk[i] = make_float4(nn[0], nn[1], nn[2], __uint_as_float(0u));
+    q.S[i] = make_float4(1.f, 0.f, 0.f, 0.f);
+    q.tau[i] = tau;
+    q.id[i] = id;
+    if (g.emit_records) {
+        unsigned long long slot = krp_reserve64(&ctl->n_events);
+        if (slot < ctl->ev_cap) {
+            ev.pc[slot] = pc;
+            ev.nk[slot] = make_float4(nn[0], nn[1], nn[2], __uint_as_float(0u));
+            ev.S[slot] = make_float4(1.f, 0.f, 0.f, 0.f);
+            ev.id[slot] = id;
+            atomicAdd(&ctl->stats.records, 1ull);
+        } else {
+            atomicAdd(&ctl->stats.overflow, 1ull);
+        }
+    }
+}
+
+// one thread: open a wave.  Events appended from here on belong to this wave.
+__global__ void krp_k_wave_prep(KrpCtl* ctl, int in)
+{
+    if (ctl->n_events > ctl->ev_cap) ctl->n_events = ctl->ev_cap;
+    ctl->ev_begin = ctl->n_events;
+    ctl->q_count[1 - in] = 0;
+    ctl->work[0] = 0;
+}
+
+// ------------------------------------------------------------------------------------------
+// T4  in-cell event location (R7).  With the Stokes vector carried as e^{-A}(i,q,u,v) and
+// D = tau* - A the scalar depth still to go at cell entry, the event is at the t solving
+//   alpha1 t - ln( cosh(alpha2 t) - (q_g/i) sinh(alpha2 t) ) = D + ln i  =: R ,
+// whose left side is increasing and concave: Newton from R/alpha1 lands left of the root after
+// one step and then rises monotonically.  alpha2 = 0 is the closed form t = R/alpha1.
+// ------------------------------------------------------------------------------------------
+__device__ __forceinline__ float krp_event_solve(float R, float qq, float a1, float a2, float tmax)
+{
+    float t = R / a1;
+    if (a2 != 0.f) {
+#pragma unroll 1
+        for (int it = 0; it < 12; ++it) {
+            float sh, chm1;
+            krp_sinh_coshm1(a2 * t, sh, chm1);
+            float gm1 = chm1 - qq * sh;
+            float h = a1 * t - log1pf(gm1) - R;
+            float hp = a1 - a2 * (sh - qq * (1.f + chm1)) / (1.f + gm1);
+            float dt = h / hp;
+            t = fminf(fmaxf(t - dt, 0.f), tmax);
+            if (fabsf(dt) <= 2e-7f * t) break;
+        }
+    }
+    return fminf(fmaxf(t, 0.f), tmax);
+}
+
+// ------------------------------------------------------------------------------------------
+// T3/T4/T5  one flight per queue entry: march cell to cell applying the App. A
+// solution in every cell until the survival I(s)/I(0) falls to e^{-tau*} (R7)
+// or the packet leaves the grid; at an event append the pre-scatter record.
+// SCALAR = the opacity table does not depend on direction and alpha2 = alpha3 = 0: the cell is
+// 4 bytes (kappa*rho) and the Stokes vector only scales.
+// ------------------------------------------------------------------------------------------
+template <bool SCALAR>
+__global__ void __launch_bounds__(256) krp_k_flight(KrpModel g, KrpCtl* ctl, KrpRecords q, int in, KrpRecords ev)
+{
+    const unsigned int n_items = ctl->q_count[in];
+    unsigned long long steps = 0, n_ev = 0, n_over = 0;
+    double w_esc = 0.0, w_abs = 0.0, w_cut = 0.0;
+    for (unsigned int item = blockIdx.x * blockDim.x + threadIdx.x; item < n_items; item += gridDim.x * blockDim.x) {
+        const float4 pc = q.pc[item], nk = q.nk[item], S0 = q.S[item];
+        const float n[3] = { nk.x, nk.y, nk.z };
+        const float p0[3] = { pc.x, pc.y, pc.z };
+        const uint32_t k = __float_as_uint(nk.w);
+        const double tau0 = q.tau[item];
+        KrpRay ray;
+        krp_ray_init(g, __float_as_uint(pc.w), p0, n, ray);
+        float th[3], ph[3];
+        if (!SCALAR) krp_basis<float>(n, th, ph);
+        double D = tau0, i = 1.0;
+        float qs = S0.y, us = S0.z, vs = S0.w;      // lab reference
+        float Asum = 0.f;
+        const float tau0f = (float)tau0, guard = 1.f + g.rho + 1e-3f;
+        bool hit = false;
+        float moved = 0.f, omega = g.omc, ds = 0.f;
+        for (;;) {
+            ds = krp_ray_ds(ray);
+            ++steps;
+            if (SCALAR) {
+                float kr = __ldg(g.kr + ray.c);
+                float dt1 = g.a1c * kr * ds;
+                if ((double)dt1 >= D) {              // event inside this cell
+                    moved = (float)D / (g.a1c * kr);
+                    hit = true;
+                    break;
+                }
+                D -= (double)dt1;
+            } else {
+                float4 cl = __ldg(g.cell + ray.c);
+                float kr = cl.x;
+                if (kr > 0.f) {
+                    float mu = n[0] * cl.y + n[1] * cl.z + n[2] * cl.w;
+                    float4 op = krp_opac_at(g.opac, g.n_inc, fabsf(mu));
+                    float dtau = kr * ds;
+                    if (op.y == 0.f && op.z == 0.f) {
+                        float dt1 = op.x * dtau;
+                        double Dn = D - (double)dt1;
+                        Asum += dt1;
+                        if (Asum * guard >= tau0f) {
+                            double R = D + (double)logf((float)i);
+                            if ((double)dt1 >= R) {
+                                moved = ((float)R / op.x) / kr;
+                                float inv = 1.f / (float)i;
+                                qs *= inv; us *= inv; vs *= inv;
+                                omega = op.w; hit = true;
+                                break;
+                            }
+                        }
+                        D = Dn;
+                    } else {
+                        float a = th[0] * cl.y + th[1] * cl.z + th[2] * cl.w;
+                        float b = ph[0] * cl.y + ph[1] * cl.z + ph[2] * cl.w;
+                        float c2, s2;
+                        krp_eta2<float>(a, b, c2, s2);
+                        float qg = c2 * qs + s2 * us, ug = -s2 * qs + c2 * us, vg = vs;   // eq. 7
+                        const float qg_e = qg, ug_e = ug, vg_e = vg;
+                        const float i_f = (float)i;
+                        float di, i_new, depth;
+                        bool thick = krp_appA(i_f, qg, ug, vg, op, dtau, di, i_new, depth);
+                        double in_d = thick ? (double)i_new : i + (double)di;
+                        double Dn = D - (double)depth;
+                        Asum += op.x * dtau;
+                        if (Asum * guard >= tau0f) {
+                            // survival test on the exit state: ln(i') + D' <= 0
+                            if ((double)logf((float)in_d) + Dn <= 0.0) {
+                                float R = (float)(D + (double)logf(i_f));
+                                float qq = qg_e / i_f;
+                                float t = krp_event_solve(R, qq, op.x, op.y, dtau);
+                                // state at t, normalised to I = 1, back to the lab reference
+                                float sh, chm1, sy = 0.f, cy = 1.f;
+                                krp_sinh_coshm1(op.y * t, sh, chm1);
+                                if (op.z != 0.f) sincosf(op.z * t, &sy, &cy);
+                                float it = i_f + (i_f * chm1 - qg_e * sh);
+                                float qt = qg_e + (qg_e * chm1 - i_f * sh);
+                                float ut = ug_e * cy - vg_e * sy;
+                                float vt = ug_e * sy + vg_e * cy;
+                                float inv = 1.f / it;
+                                qt *= inv; ut *= inv; vt *= inv;
+                                qs = c2 * qt - s2 * ut; us = s2 * qt + c2 * ut; vs = vt;
+                                moved = t / kr;
+                                omega = op.w; hit = true;
+                                break;
+                            }
+                        }
+                        qs = c2 * qg - s2 * ug; us = s2 * qg + c2 * ug; vs = vg;
+                        i = in_d; D = Dn;
+                    }
+                }
+            }
+            if (!krp_ray_step(ray, ds)) break;
+        }
+        const float W = S0.x;
+        if (!hit) { w_esc += (double)W; continue; }
+        // T5: event record, albedo weighting, termination (R12)
+        float pe[3];
+        pe[0] = krp_local(n[0], ray.rx, ray.tx, moved, p0[0]);
+        pe[1] = krp_local(n[1], ray.ry, ray.ty, moved, p0[1]);
+        pe[2] = krp_local(n[2], ray.rz, ray.tz, moved, p0[2]);
+        const float Wn = omega * W;
+        const uint32_t kn = k + 1u;
+        const bool term = (Wn < g.w_min) || ((int)kn >= g.max_scatter);
+        w_abs += (double)W - (double)Wn;
+        unsigned long long slot = krp_reserve64(&ctl->n_events);
+        if (slot < ctl->ev_cap) {
+            ev.pc[slot] = make_float4(pe[0], pe[1], pe[2], __uint_as_float(ray.c));
+            ev.nk[slot] = make_float4(n[0], n[1], n[2], __uint_as_float(kn | (term ? KRP_TERM_BIT : 0u)));
+            ev.S[slot] = make_float4(Wn, qs, us, vs);
+            ev.id[slot] = q.id[item];
+            ++n_ev;
+            if (term) w_cut += (double)Wn;
+        } else {
+            ++n_over;
+            w_cut += (double)Wn;
+        }
+    }
+    // statistics: one atomic per warp and counter
+    steps = krp_warp_sum(steps); n_ev = krp_warp_sum(n_ev); n_over = krp_warp_sum(n_over);
+    w_esc = krp_warp_sum(w_esc); w_abs = krp_warp_sum(w_abs); w_cut = krp_warp_sum(w_cut);
+    if ((threadIdx.x & 31) == 0) {
+        if (steps) atomicAdd(&ctl->stats.steps_transport, steps);
+        if (n_ev) atomicAdd(&ctl->stats.events, n_ev);
+        if (n_over) atomicAdd(&ctl->stats.overflow, n_over);
+        if (w_esc != 0.0) atomicAdd(&ctl->stats.w_escaped, w_esc);
+        if (w_abs != 0.0) atomicAdd(&ctl->stats.w_absorbed, w_abs);
+        if (w_cut != 0.0) atomicAdd(&ctl->stats.w_cut, w_cut);
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// quaternion helpers (eq. 1-3): q = (w, a);  q* v q  and  q v q*  for a pure
+// quaternion v, expanded from the Hamilton product:  v -+ 2w (a x v) + 2 a x (a x v).
+// ------------------------------------------------------------------------------------------
+__device__ __forceinline__ void krp_cross(const double a[3], const double b[3], double o[3])
+{
+    o[0] = a[1] * b[2] - a[2] * b[1]; o[1] = a[2] * b[0] - a[0] * b[2]; o[2] = a[0] * b[1] - a[1] * b[0];
+}
+__device__ __forceinline__ double krp_dot(const double a[3], const double b[3]) { return a[0] * b[0] + a[1] * b[1] + a[2] * b[2]; }
+
+__device__ __forceinline__ void krp_quat_rotate(const double q[4], const double v[3], double sign, double o[3])
+{
+    const double a[3] = { q[1], q[2], q[3] };
+    double c1[3], c2[3];
+    krp_cross(a, v, c1);
+    krp_cross(a, c1, c2);
+    for (int j = 0; j < 3; ++j) o[j] = v[j] + 2.0 * (sign * q[0] * c1[j] + c2[j]);
+}
+
+// (Q,U) -> reference turned by eta (eq. 7), given cos(2 eta), sin(2 eta)
+__device__ __forceinline__ void krp_rot_qu(double& Q, double& U, double c2, double s2)
+{
+    double q = c2 * Q + s2 * U, u = -s2 * Q + c2 * U;
+    Q = q; U = u;
+}
+
+// ------------------------------------------------------------------------------------------
+// T6  scattering (step S5 of DESIGN.md).  One thread per event
+// of the wave, fp64.  Draws of block 0 of event k: (Theta, phi candidate, accept, next tau*);
+// blocks >= 1: two more (phi, accept) pairs each, at most 64 rounds.
+// ------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(128) krp_k_scatter(KrpModel g, KrpCtl* ctl, KrpRecords ev, KrpRecords qo, int out,
+                                                     unsigned long long seed)
+{
+    const unsigned long long e0 = ctl->ev_begin;
+    unsigned long long e1 = ctl->n_events;
+    if (e1 > ctl->ev_cap) e1 = ctl->ev_cap;
+    for (unsigned long long e = e0 + blockIdx.x * blockDim.x + threadIdx.x; e < e1; e += (unsigned long long)gridDim.x * blockDim.x) {
+        const float4 nk = ev.nk[e];
+        const uint32_t kb = __float_as_uint(nk.w);
+        if ((kb & KRP_TERM_BIT) || kb == 0u) continue;
+        const float4 pc = ev.pc[e], Se = ev.S[e];
+        const unsigned long long id = ev.id[e];
+        const uint32_t cell = __float_as_uint(pc.w);
+        double b[3] = { 0.0, 0.0, 1.0 };
+        if (!g.scalar) { float4 cl = g.cell[cell]; b[0] = cl.y; b[1] = cl.z; b[2] = cl.w; }
+        const double n[3] = { nk.x, nk.y, nk.z };
+        // A2: q_B from the direction angles of B (eq. 2)
+        double qB[4];
+        {
+            double rho = sqrt(b[0] * b[0] + b[1] * b[1]);
+            double thB = atan2(rho, b[2]), phB = rho > 0.0 ? atan2(b[1], b[0]) : 0.0;
+            double sh_t, ch_t, sh_p, ch_p;
+            sincos(0.5 * thB, &sh_t, &ch_t);
+            sincos(0.5 * phB, &sh_p, &ch_p);
+            qB[0] = ch_p * ch_t; qB[1] = -sh_p * sh_t; qB[2] = ch_p * sh_t; qB[3] = sh_p * ch_t;
+        }
+        // A3: direction in the grain frame (eq. 3)
+        double ng[3];
+        krp_quat_rotate(qB, n, -1.0, ng);
+        {
+            double r = 1.0 / sqrt(krp_dot(ng, ng));
+            ng[0] *= r; ng[1] *= r; ng[2] *= r;
+        }
+        // A5: Stokes reference lab -> grain frame
+        double th[3], ph[3];
+        krp_basis<double>(n, th, ph);
+        double c2, s2;
+        krp_eta2<double>(krp_dot(th, b), krp_dot(ph, b), c2, s2);
+        double Q = Se.y, U = Se.z, V = Se.w;
+        krp_rot_qu(Q, U, c2, s2);
+        // draws
+        uint4 w = krp_philox(seed, id, kb, 0u);
+        const double tau_next = -log(krp_u01(w.w));
+        double theta;   // degrees, from the piecewise-linear CDF (R13)
+        {
+            double u = krp_u01(w.x);
+            int lo = 0, hi = g.n_ang - 1;
+            while (hi - lo > 1) { int mid = (lo + hi) >> 1; if (g.cdf[mid] <= u) lo = mid; else hi = mid; }
+            double wd = g.cdf[lo + 1] - g.cdf[lo];
+            double f = wd > 0.0 ? (u - g.cdf[lo]) / wd : 0.5;
+            theta = ((double)lo + f) * 180.0 / (double)(g.n_ang - 1);
+        }
+        double F[4];
+        krp_mueller_at<double>(g.mueller, g.n_ang, theta, F);
+        const double p12 = F[1] / F[0];
+        const double bound = 1.0 + fabs(p12) * sqrt(Q * Q + U * U);
+        double phi = 2.0 * KRP_PI_D * krp_u01(w.y);
+        double sphi, cphi;
+        sincos(phi, &sphi, &cphi);
+        bool ok;
+        {
+            double c2p = cphi * cphi - sphi * sphi, s2p = 2.0 * sphi * cphi;
+            ok = krp_u01(w.z) * bound < 1.0 + p12 * (Q * c2p + U * s2p);
+        }
+        int rounds = 1;
+        for (uint32_t blk = 1; !ok && rounds < 64; ++blk) {
+            uint4 x = krp_philox(seed, id, kb, blk);
+            uint32_t cand[2] = { x.x, x.z }, acc[2] = { x.y, x.w };
+            for (int h = 0; h < 2 && !ok && rounds < 64; ++h) {
+                phi = 2.0 * KRP_PI_D * krp_u01(cand[h]);
+                sincos(phi, &sphi, &cphi);
+                double c2p = cphi * cphi - sphi * sphi, s2p = 2.0 * sphi * cphi;
+                ok = krp_u01(acc[h]) * bound < 1.0 + p12 * (Q * c2p + U * s2p);
+                ++rounds;
+            }
+        }
+        // scattering in the grain frame
+        double thp[3], php[3];
+        krp_basis<double>(ng, thp, php);
+        double st, ct;
+        sincos(theta * (KRP_PI_D / 180.0), &st, &ct);
+        double epar[3], nog[3], eout[3], shat[3];
+        for (int j = 0; j < 3; ++j) epar[j] = cphi * thp[j] + sphi * php[j];
+        for (int j = 0; j < 3; ++j) nog[j] = ct * ng[j] + st * epar[j];
+        krp_rot_qu(Q, U, cphi * cphi - sphi * sphi, 2.0 * sphi * cphi);      // reference e_par
+        {
+            double I2 = F[0] + F[1] * Q, Q2 = F[1] + F[0] * Q;                  // F(Theta) (1,Q,U,V)
+            double U2 = F[2] * U + F[3] * V, V2 = -F[3] * U + F[2] * V;
+            Q = Q2 / I2; U = U2 / I2; V = V2 / I2;
+        }
+        for (int j = 0; j < 3; ++j) eout[j] = ct * epar[j] - st * ng[j];
+        krp_cross(ng, epar, shat);
+        double th2[3], ph2[3];
+        krp_basis<double>(nog, th2, ph2);
+        {
+            double ce = krp_dot(eout, th2), se = krp_dot(th2, shat);
+            krp_rot_qu(Q, U, ce * ce - se * se, 2.0 * se * ce);                // reference theta^ of n'_GF
+        }
+        // back to the lab: inverse of eq. 3, direction stored in fp32 (R12)
+        double nl[3];
+        krp_quat_rotate(qB, nog, 1.0, nl);
+        const float nf[3] = { (float)nl[0], (float)nl[1], (float)nl[2] };
+        const double nd[3] = { nf[0], nf[1], nf[2] };
+        krp_basis<double>(nd, th, ph);
+        krp_eta2<double>(krp_dot(th, b), krp_dot(ph, b), c2, s2);
+        krp_rot_qu(Q, U, c2, -s2);
+        unsigned int slot = krp_reserve32(&ctl->q_count[out]);
+        qo.pc[slot] = pc;
+        qo.nk[slot] = make_float4(nf[0], nf[1], nf[2], __uint_as_float(kb));
+        qo.S[slot] = make_float4(Se.x, (float)Q, (float)U, (float)V);
+        qo.tau[slot] = tau_next;
+        qo.id[slot] = id;
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// I1  peel-off (PAPER.md:121 S_pp = Z(Omega_cam;Omega_pp) I_pp, eq. 10-11): Stokes vector sent
+// toward the observer by a scattering of the stored incoming state, in the reference
+// theta^_obs, times 1/(4 pi).
+// ------------------------------------------------------------------------------------------
+__device__ __forceinline__ void krp_rot_qu_f(float& Q, float& U, float ce, float se)
+{
+    float c2 = ce * ce - se * se, s2 = 2.f * se * ce;
+    float q = c2 * Q + s2 * U, u = -s2 * Q + c2 * U;
+    Q = q; U = u;
+}
+
+__device__ __forceinline__ void krp_peel(const KrpModel& g, const float n[3], float4 Se, const KrpObserverDev& ob, float S[4])
+{
+    float th[3], ph[3];
+    krp_basis<float>(n, th, ph);
+    float mu = n[0] * ob.n[0] + n[1] * ob.n[1] + n[2] * ob.n[2];
+    mu = fminf(fmaxf(mu, -1.f), 1.f);
+    float sh[3] = { n[1] * ob.n[2] - n[2] * ob.n[1], n[2] * ob.n[0] - n[0] * ob.n[2], n[0] * ob.n[1] - n[1] * ob.n[0] };
+    float sn = sqrtf(sh[0] * sh[0] + sh[1] * sh[1] + sh[2] * sh[2]);
+    if (sn < 1e-12f) { sh[0] = ph[0]; sh[1] = ph[1]; sh[2] = ph[2]; }
+    else { float r = 1.f / sn; sh[0] *= r; sh[1] *= r; sh[2] *= r; }
+    // e_par = s^ x n_in: reference of the incoming ray in the scattering plane
+    float ep[3] = { sh[1] * n[2] - sh[2] * n[1], sh[2] * n[0] - sh[0] * n[2], sh[0] * n[1] - sh[1] * n[0] };
+    float I = Se.x, Q = Se.x * Se.y, U = Se.x * Se.z, V = Se.x * Se.w;
+    krp_rot_qu_f(Q, U, th[0] * ep[0] + th[1] * ep[1] + th[2] * ep[2], ph[0] * ep[0] + ph[1] * ep[1] + ph[2] * ep[2]);
+    // scattering angle from atan2(|n x n_obs|, n.n_obs): well conditioned at both poles
+    float theta_deg = atan2f(sn, mu) * 57.29577951308232f;
+    float F[4];
+    krp_mueller_at<float>(g.mueller, g.n_ang, theta_deg, F);
+    float I2 = F[0] * I + F[1] * Q, Q2 = F[1] * I + F[0] * Q;
+    float U2 = F[2] * U + F[3] * V, V2 = -F[3] * U + F[2] * V;
+    // e_out = s^ x n_obs, then to theta^_obs
+    float eo[3] = { sh[1] * ob.n[2] - sh[2] * ob.n[1], sh[2] * ob.n[0] - sh[0] * ob.n[2], sh[0] * ob.n[1] - sh[1] * ob.n[0] };
+    krp_rot_qu_f(Q2, U2, eo[0] * ob.th[0] + eo[1] * ob.th[1] + eo[2] * ob.th[2],
+                 ob.th[0] * sh[0] + ob.th[1] * sh[1] + ob.th[2] * sh[2]);
+    const float c = 0.07957747154594767f;   // 1/(4 pi)
+    S[0] = c * I2; S[1] = c * Q2; S[2] = c * U2; S[3] = c * V2;
+}
+
+// ------------------------------------------------------------------------------------------
+// I1-I3  imaging: one item per (observer, event).  Peel-off, attenuation march to the grid
+// edge with the same in-cell solution and no survival test, orthographic
+// projection, fp64 atomic accumulation into img[obs][4][npy][npx] (R14).
+// ------------------------------------------------------------------------------------------
+template <bool SCALAR>
+__global__ void __launch_bounds__(256) krp_k_image(KrpModel g, KrpCtl* ctl, KrpRecords ev, const KrpObserverDev* __restrict__ obs,
+                                                   int n_obs, int npx, int npy, int flags, double* __restrict__ img)
+{
+    unsigned long long n_ev = ctl->n_events;
+    if (n_ev > ctl->ev_cap) n_ev = ctl->ev_cap;
+    const unsigned long long total = n_ev * (unsigned long long)n_obs;
+    unsigned long long steps = 0, n_con = 0, n_drop = 0;
+    for (unsigned long long item = blockIdx.x * (unsigned long long)blockDim.x + threadIdx.x; item < total;
+         item += (unsigned long long)gridDim.x * blockDim.x) {
+        const int o = (int)(item / n_ev);
+        const unsigned long long e = item - (unsigned long long)o * n_ev;
+        const float4 nk = ev.nk[e];
+        const uint32_t k = __float_as_uint(nk.w) & ~KRP_TERM_BIT;
+        if (k == 0u && !(flags & 1)) continue;
+        const float4 pc = ev.pc[e], Se = ev.S[e];
+        const KrpObserverDev& ob = obs[o];
+        float S[4];
+        if (k == 0u) { S[0] = Se.x * 0.07957747154594767f; S[1] = S[2] = S[3] = 0.f; }
+        else { const float n[3] = { nk.x, nk.y, nk.z }; krp_peel(g, n, Se, ob, S); }
+        const float p0[3] = { pc.x, pc.y, pc.z };
+        KrpRay ray;
+        krp_ray_init(g, __float_as_uint(pc.w), p0, ob.n, ray);
+        float A = 0.f;
+        if (SCALAR) {
+            float tau = 0.f;
+            for (;;) {
+                float ds = krp_ray_ds(ray);
+                ++steps;
+                tau = fmaf(__ldg(g.kr + ray.c), ds, tau);
+                if (!krp_ray_step(ray, ds)) break;
+            }
+            A = g.a1c * tau;
+        } else {
+            float i = S[0], qs = S[1], us = S[2], vs = S[3];
+            for (;;) {
+                float ds = krp_ray_ds(ray);
+                ++steps;
+                float4 cl = __ldg(g.cell + ray.c);
+                float kr = cl.x;
+                if (kr > 0.f) {
+                    float mu = ob.n[0] * cl.y + ob.n[1] * cl.z + ob.n[2] * cl.w;
+                    float4 op = krp_opac_at(g.opac, g.n_inc, fabsf(mu));
+                    float dtau = kr * ds;
+                    if (op.y == 0.f && op.z == 0.f) {
+                        A += op.x * dtau;
+                    } else {
+                        float a = ob.th[0] * cl.y + ob.th[1] * cl.z + ob.th[2] * cl.w;
+                        float b = ob.ph[0] * cl.y + ob.ph[1] * cl.z + ob.ph[2] * cl.w;
+                        float c2, s2;
+                        krp_eta2<float>(a, b, c2, s2);
+                        float qg = c2 * qs + s2 * us, ug = -s2 * qs + c2 * us, vg = vs;
+                        float di, i_new, depth;
+                        krp_appA(i, qg, ug, vg, op, dtau, di, i_new, depth);
+                        i = i_new; A += depth;
+                        qs = c2 * qg - s2 * ug; us = s2 * qg + c2 * ug; vs = vg;
+                    }
+                }
+                if (!krp_ray_step(ray, ds)) break;
+            }
+            S[0] = i; S[1] = qs; S[2] = us; S[3] = vs;
+        }
+        const float att = expf(-A);
+        // I3: orthographic projection of the event position (fp64, once per ray)
+        const uint32_t cell = __float_as_uint(pc.w);
+        const int ix0 = (int)(cell % (uint32_t)g.nx);
+        const uint32_t t = cell / (uint32_t)g.nx;
+        const int iy0 = (int)(t % (uint32_t)g.ny), iz0 = (int)(t / (uint32_t)g.ny);
+        const double x[3] = { g.lo[0] + ((double)ix0 + (double)pc.x) * g.dd[0] - ob.center[0],
+                              g.lo[1] + ((double)iy0 + (double)pc.y) * g.dd[1] - ob.center[1],
+                              g.lo[2] + ((double)iz0 + (double)pc.z) * g.dd[2] - ob.center[2] };
+        const double xi = (x[0] * ob.phd[0] + x[1] * ob.phd[1] + x[2] * ob.phd[2]) * ob.inv_hw;
+        const double yi = -(x[0] * ob.thd[0] + x[1] * ob.thd[1] + x[2] * ob.thd[2]) * ob.inv_hh;
+        const int px = (int)floor((xi + 1.0) * (double)npx / 2.0), py = (int)floor((yi + 1.0) * (double)npy / 2.0);
+        if (px < 0 || px >= npx || py < 0 || py >= npy) { ++n_drop; continue; }
+        ++n_con;
+        const size_t plane = (size_t)npx * npy;
+        double* at = img + (size_t)o * 4 * plane + (size_t)py * npx + px;
+        atomicAdd(at, (double)(att * S[0]));
+        atomicAdd(at + plane, (double)(att * S[1]));
+        atomicAdd(at + 2 * plane, (double)(att * S[2]));
+        atomicAdd(at + 3 * plane, (double)(att * S[3]));
+    }
+    steps = krp_warp_sum(steps); n_con = krp_warp_sum(n_con); n_drop = krp_warp_sum(n_drop);
+    if ((threadIdx.x & 31) == 0) {
+        if (steps) atomicAdd(&ctl->stats.steps_image, steps);
+        if (n_con) atomicAdd(&ctl->stats.contributions, n_con);
+        if (n_drop) atomicAdd(&ctl->stats.dropped, n_drop);
+    }
+}
+
+// end of imaging: the event buffer is consumed
+__global__ void krp_k_events_clear(KrpCtl* ctl) { ctl->n_events = 0; ctl->ev_begin = 0; }
+
+// ------------------------------------------------------------------------------------------
+// T0  setup kernels (not on the timed path)
+// ------------------------------------------------------------------------------------------
+__global__ void krp_k_pack(const float* __restrict__ density, const float* __restrict__ bfield, uint32_t ncell,
+                           float4* __restrict__ cell, float* __restrict__ kr, int* __restrict__ bad)
+{
+    uint32_t c = blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= ncell) return;
+    float d = density[c];
+    if (!(d >= 0.f) || isinf(d)) atomicAdd(bad, 1);
+    if (kr) kr[c] = d;
+    if (cell) {
+        double bx = 0.0, by = 0.0, bz = 1.0;
+        if (bfield) {
+            bx = bfield[3 * (size_t)c]; by = bfield[3 * (size_t)c + 1]; bz = bfield[3 * (size_t)c + 2];
+            double r = sqrt(bx * bx + by * by + bz * bz);
+            if (r > 0.0) { bx /= r; by /= r; bz /= r; } else { bx = 0.0; by = 0.0; bz = 1.0; }
+        }
+        cell[c] = make_float4(d, (float)bx, (float)by, (float)bz);
+    }
+}
+
+__global__ void krp_k_f2d(const float* __restrict__ w, uint32_t n, double* __restrict__ o)
+{
+    uint32_t c = blockIdx.x * blockDim.x + threadIdx.x;
+    if (c < n) o[c] = (double)w[c];
+}

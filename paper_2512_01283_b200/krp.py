@@ -1,0 +1,251 @@
+"""Thin ctypes binding of libkrp.so (include/krp.h): same names, argument marshalling only.
+
+Every step of the path runs in the library's CUDA kernels.  torch is used for device buffers
+and streams.  There is no CPU fallback: a missing library raises.
+"""
+import ctypes as C
+import os
+
+import numpy as np
+
+from . import _build
+
+OK, ERR_ARG, ERR_CUDA, ERR_OOM, ERR_STATE, ERR_EVENT_FULL = 0, -1, -2, -3, -4, -5
+MEM_DEVICE, MEM_HOST = 0, 1
+
+SYMBOLS = [
+    "krp_last_error", "krp_version", "krp_grid_create", "krp_grid_destroy", "krp_source_set",
+    "krp_events_reserve", "krp_transport", "krp_packet_id_set", "krp_image", "krp_image_get",
+    "krp_image_reset", "krp_stats_get", "krp_stats_reset", "krp_events_get", "krp_events_clear",
+    "krp_tune", "krp_launch_count",
+]
+
+
+class KrpError(RuntimeError):
+    def __init__(self, code, msg):
+        super().__init__("krp error %d: %s" % (code, msg))
+        self.code = code
+
+
+class Tables(C.Structure):
+    _fields_ = [("n_ang", C.c_int), ("mueller", C.c_void_p), ("n_inc", C.c_int), ("opacity", C.c_void_p),
+                ("w_min", C.c_float), ("max_scatter", C.c_int)]
+
+
+class Source(C.Structure):
+    _fields_ = [("kind", C.c_int), ("pos", C.c_double * 3), ("dir", C.c_double * 3),
+                ("cell_weight", C.c_void_p), ("emit_records", C.c_int)]
+
+
+class Observer(C.Structure):
+    _fields_ = [("theta", C.c_double), ("phi", C.c_double), ("center", C.c_double * 3),
+                ("half_w", C.c_double), ("half_h", C.c_double)]
+
+
+class Stats(C.Structure):
+    _fields_ = [(n, C.c_uint64) for n in ("packets", "events", "records", "steps_transport", "steps_image",
+                                          "contributions", "dropped", "overflow")] + \
+               [(n, C.c_double) for n in ("w_emitted", "w_escaped", "w_absorbed", "w_cut")]
+
+    def as_dict(self):
+        return {n: getattr(self, n) for n, _ in self._fields_}
+
+
+_lib = None
+
+
+def library_path():
+    return _build.LIB
+
+
+def lib():
+    """Load libkrp.so (building it if nvcc is here and the sources are newer)."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    path = _build.LIB
+    if _build.stale():
+        try:
+            _build.build()
+        except Exception as exc:  # no nvcc on this box and no prebuilt library: fail loudly
+            if not os.path.exists(path):
+                raise ImportError("libkrp.so is missing and could not be built (%s); "
+                                  "run `python -m paper_2512_01283_b200._build`" % exc) from exc
+    L = C.CDLL(path)
+    vp, u64, i32 = C.c_void_p, C.c_uint64, C.c_int
+    sig = {
+        "krp_last_error": (C.c_char_p, []),
+        "krp_version": (C.c_char_p, []),
+        "krp_grid_create": (i32, [C.POINTER(vp), i32, i32, i32, C.POINTER(C.c_double), vp, vp, i32,
+                                  C.POINTER(Tables), vp]),
+        "krp_grid_destroy": (i32, [vp]),
+        "krp_source_set": (i32, [vp, C.POINTER(Source), vp]),
+        "krp_events_reserve": (i32, [vp, u64]),
+        "krp_transport": (i32, [vp, u64, u64, vp]),
+        "krp_packet_id_set": (i32, [vp, u64]),
+        "krp_image": (i32, [vp, C.POINTER(Observer), i32, i32, i32, i32, vp]),
+        "krp_image_get": (i32, [vp, vp, i32, vp]),
+        "krp_image_reset": (i32, [vp, vp]),
+        "krp_stats_get": (i32, [vp, C.POINTER(Stats)]),
+        "krp_stats_reset": (i32, [vp, vp]),
+        "krp_events_get": (i32, [vp, u64, C.POINTER(u64), vp, vp, vp, vp, vp, vp]),
+        "krp_events_clear": (i32, [vp, vp]),
+        "krp_tune": (i32, [vp, i32, i32, i32]),
+        "krp_launch_count": (u64, [vp]),
+    }
+    for name, (res, args) in sig.items():
+        f = getattr(L, name)
+        f.restype, f.argtypes = res, args
+    _lib = L
+    return L
+
+
+def _check(rc):
+    if rc != OK:
+        raise KrpError(rc, lib().krp_last_error().decode())
+
+
+def _stream(stream):
+    if stream is None:
+        import torch
+        return C.c_void_p(torch.cuda.current_stream().cuda_stream)
+    if hasattr(stream, "cuda_stream"):
+        return C.c_void_p(stream.cuda_stream)
+    return C.c_void_p(int(stream))
+
+
+def _ptr_mem(a):
+    """(pointer, mem, keep-alive) of a torch CUDA tensor, a torch CPU tensor or a numpy array (float32)."""
+    if a is None:
+        return None, None, None
+    if isinstance(a, np.ndarray):
+        a = np.ascontiguousarray(a, np.float32)
+        return C.c_void_p(a.ctypes.data), MEM_HOST, a
+    import torch
+    if not isinstance(a, torch.Tensor):
+        raise TypeError("expected a torch tensor or numpy array")
+    if a.dtype != torch.float32:
+        raise TypeError("expected float32")
+    a = a.contiguous()
+    return C.c_void_p(a.data_ptr()), (MEM_DEVICE if a.is_cuda else MEM_HOST), a
+
+
+def make_observer(theta, phi, center, half_w, half_h=None):
+    o = Observer()
+    o.theta, o.phi = float(theta), float(phi)
+    o.center[:] = [float(c) for c in center]
+    o.half_w = float(half_w)
+    o.half_h = float(half_w if half_h is None else half_h)
+    return o
+
+
+class Grid:
+    """Owner of one krp_grid handle.  Methods mirror the C entry points one to one."""
+
+    def __init__(self, nx, ny, nz, bounds, density, bfield, mueller, opacity, w_min=1e-4, max_scatter=64,
+                 stream=None):
+        L = lib()
+        self._h = C.c_void_p()
+        dptr, dmem, dkeep = _ptr_mem(density)
+        bptr, bmem, bkeep = _ptr_mem(bfield)
+        if bptr is not None and bmem != dmem:
+            raise ValueError("density and bfield must live in the same memory space")
+        mu = np.ascontiguousarray(np.asarray(mueller, np.float32).reshape(-1, 4))
+        op = np.ascontiguousarray(np.asarray(opacity, np.float32).reshape(-1, 4))
+        t = Tables(mu.shape[0], mu.ctypes.data, op.shape[0], op.ctypes.data, float(w_min), int(max_scatter))
+        b = (C.c_double * 6)(*[float(x) for x in bounds])
+        self.shape = (int(nx), int(ny), int(nz))
+        self.bounds = [float(x) for x in bounds]
+        _check(L.krp_grid_create(C.byref(self._h), int(nx), int(ny), int(nz), b, dptr, bptr, dmem, C.byref(t),
+                                 _stream(stream)))
+        self.n_obs = self.npx = self.npy = 0
+        self._weights = None
+
+    def close(self):
+        if getattr(self, "_h", None) is not None and self._h:
+            lib().krp_grid_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def source_set(self, kind=0, pos=None, direction=(0, 0, 1), cell_weight=None, emit_records=0, stream=None):
+        s = Source()
+        s.kind = int(kind)
+        if pos is None:
+            pos = [(self.bounds[0] + self.bounds[1]) / 2, (self.bounds[2] + self.bounds[3]) / 2,
+                   (self.bounds[4] + self.bounds[5]) / 2]
+        s.pos[:] = [float(x) for x in pos]
+        s.dir[:] = [float(x) for x in direction]
+        s.emit_records = int(emit_records)
+        if cell_weight is not None:
+            if not cell_weight.is_cuda:
+                raise ValueError("cell_weight must be a CUDA tensor")
+            ptr, _, self._weights = _ptr_mem(cell_weight)
+            s.cell_weight = ptr
+        _check(lib().krp_source_set(self._h, C.byref(s), _stream(stream)))
+
+    def events_reserve(self, max_events):
+        _check(lib().krp_events_reserve(self._h, int(max_events)))
+
+    def transport(self, n_packets, seed, stream=None):
+        _check(lib().krp_transport(self._h, int(n_packets), int(seed), _stream(stream)))
+
+    def packet_id_set(self, next_id):
+        _check(lib().krp_packet_id_set(self._h, int(next_id)))
+
+    def image(self, observers, npix_x, npix_y, flags=0, stream=None):
+        n = len(observers)
+        arr = (Observer * n)(*observers)
+        _check(lib().krp_image(self._h, arr, n, int(npix_x), int(npix_y), int(flags), _stream(stream)))
+        self.n_obs, self.npx, self.npy = n, int(npix_x), int(npix_y)
+
+    def image_get(self, out=None, stream=None):
+        """Returns the maps [n_obs,4,npy,npx] fp64: a numpy array (host copy) unless `out` is a CUDA tensor."""
+        shape = (self.n_obs, 4, self.npy, self.npx)
+        if out is None:
+            out = np.empty(shape, np.float64)
+        if isinstance(out, np.ndarray):
+            assert out.dtype == np.float64 and out.flags.c_contiguous and out.size == int(np.prod(shape))
+            _check(lib().krp_image_get(self._h, C.c_void_p(out.ctypes.data), MEM_HOST, _stream(stream)))
+            return out.reshape(shape)
+        assert out.is_contiguous() and out.numel() == int(np.prod(shape))
+        _check(lib().krp_image_get(self._h, C.c_void_p(out.data_ptr()), MEM_DEVICE if out.is_cuda else MEM_HOST,
+                                   _stream(stream)))
+        return out
+
+    def image_reset(self, stream=None):
+        _check(lib().krp_image_reset(self._h, _stream(stream)))
+
+    def stats_get(self):
+        s = Stats()
+        _check(lib().krp_stats_get(self._h, C.byref(s)))
+        return s.as_dict()
+
+    def stats_reset(self, stream=None):
+        _check(lib().krp_stats_reset(self._h, _stream(stream)))
+
+    def events_get(self, cap=None):
+        n = C.c_uint64(0)
+        _check(lib().krp_events_get(self._h, 0, C.byref(n), None, None, None, None, None, None))
+        m = n.value if cap is None else min(int(cap), n.value)
+        ev = dict(id=np.zeros(m, np.uint64), k=np.zeros(m, np.int32), cell=np.zeros(m, np.int64),
+                  pos=np.zeros((m, 3), np.float32), dir=np.zeros((m, 3), np.float32),
+                  stokes=np.zeros((m, 4), np.float32))
+        if m:
+            _check(lib().krp_events_get(self._h, m, C.byref(n), ev["id"].ctypes.data, ev["k"].ctypes.data,
+                                        ev["cell"].ctypes.data, ev["pos"].ctypes.data, ev["dir"].ctypes.data,
+                                        ev["stokes"].ctypes.data))
+        return ev
+
+    def events_clear(self, stream=None):
+        _check(lib().krp_events_clear(self._h, _stream(stream)))
+
+    def tune(self, transport_block=0, image_block=0, blocks_per_sm=0):
+        _check(lib().krp_tune(self._h, int(transport_block), int(image_block), int(blocks_per_sm)))
+
+    def launch_count(self):
+        return int(lib().krp_launch_count(self._h))
