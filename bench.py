@@ -1,0 +1,429 @@
+#!/usr/bin/env python
+"""bench.py -- throughput of the hot path (transport + imaging) in photon packets/s.
+
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload c2] [--batch B] [--impl reference]
+
+A "step" is one pass of the whole hot path over one batch of B new packets of the workload:
+krp_transport(B) (emit, flights, scatterings, event records) followed by krp_image (every event toward
+every observer, attenuated to the grid edge, summed into the fp64 I,Q,U,V maps).  Packet ids continue
+from step to step, so K steps are K*B distinct packets of the job.  Inputs are seeded and synthetic
+(paper_2512_01283_b200.inputs, recipe in DESIGN.md); the default workload is BASELINE.json configs[1]
+(flared disk, 128^3 cells, 4 inclinations at 256x256).
+
+One JSON line goes to stdout (rank 0).  `value` is device-resident throughput; `e2e` is the same metric
+through the C ABI with HOST buffers (grid upload, transport, imaging, image download inside the timed
+region); `roofline` is the dominant kernel against its binding ceiling; `cpu_baseline` is the fp64 oracle
+on this box's host cores.  `--impl reference` times the oracle alone (rank 0 only).
+"""
+import argparse
+import json
+import math
+import os
+import subprocess
+import sys
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "photon packets/sec (transport+imaging)"
+UNIT = "packets/s"
+
+# Algorithmic work per unit: bytes that must move and thread-instructions that
+# must issue per cell step / event / image contribution, for the two cell layouts.
+ALGO = {
+    "scalar":  dict(cell_bytes=4,  step_inst=22, event_bytes=96, event_inst=300, contrib_bytes=32, contrib_inst=120),
+    "general": dict(cell_bytes=16, step_inst=110, event_bytes=96, event_inst=300, contrib_bytes=32, contrib_inst=120),
+}
+N_SM, LANES_PER_SM = 148, 128          # B200: 148 SMs x 4 sub-partitions x 32 FP32 lanes (B200_PROFILING.md)
+
+
+def parse_args():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=6)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="krp", choices=["krp", "reference"])
+    ap.add_argument("--workload", default="c2", choices=["c1", "c2", "c3", "c4", "c5"])
+    ap.add_argument("--batch", type=int, default=0, help="packets per step and GPU (0 = workload default)")
+    ap.add_argument("--n", type=int, default=0, help="override the grid size (testing only; marks the line reduced)")
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--cpu-seconds", type=float, default=15.0)
+    return ap.parse_args()
+
+
+DEFAULT_BATCH = {"c1": 100000, "c2": 1 << 22, "c3": 1 << 20, "c4": 1 << 21, "c5": 1 << 20}
+
+
+def make_workload(args):
+    from paper_2512_01283_b200 import inputs
+    kw = {}
+    if args.n:
+        kw["n"] = args.n
+    cfg = inputs.make(args.workload, **kw)
+    batch = args.batch or DEFAULT_BATCH[args.workload]
+    return cfg, batch
+
+
+def peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            p = json.load(f)
+        return dict(hbm_gbs=float(p["hbm_gbs"]), sm_max_mhz=float(p.get("sm_max_mhz", 1965.0)), source="measured")
+    return dict(hbm_gbs=6650.0, sm_max_mhz=1965.0, source="fallback")
+
+
+class ClockSampler:
+    """nvidia-smi clocks and throttle reasons sampled every 200 ms while the timed region runs."""
+    Q = "clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown," \
+        "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap"
+
+    def __init__(self, index):
+        self.proc = None
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", "-i", str(index), "--query-gpu=" + self.Q,
+                                          "--format=csv,noheader,nounits", "-lms", "200"],
+                                         stdout=subprocess.PIPE, stderr=subprocess.DEVNULL, text=True)
+        except OSError:
+            self.proc = None
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.25)
+        self.proc.terminate()
+        try:
+            out, _ = self.proc.communicate(timeout=5)
+        except subprocess.TimeoutExpired:
+            self.proc.kill()
+            out, _ = self.proc.communicate()
+        sm, mx, pw, reasons = [], [], [], set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for line in out.splitlines():
+            f = [x.strip() for x in line.split(",")]
+            if len(f) < 7:
+                continue
+            try:
+                sm.append(float(f[0])); mx.append(float(f[1])); pw.append(float(f[2]))
+            except ValueError:
+                continue
+            for name, v in zip(names, f[3:7]):
+                if v.lower().startswith("active"):
+                    reasons.add(name)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        return {"sm_mhz": float(np.median(sm)), "sm_max_mhz": float(max(mx)), "power_w_max": float(max(pw)),
+                "samples": len(sm), "reasons": sorted(reasons)}
+
+
+# ------------------------------------------------------------------------------------------
+# the oracle leg (cpu_baseline and --impl reference): oracle/ as it stands, one host thread
+# ------------------------------------------------------------------------------------------
+def oracle_setup(cfg):
+    from oracle import OracleModel, Observer as OraObserver
+    m = OracleModel(cfg["nx"], cfg["ny"], cfg["nz"], cfg["bounds"], cfg["density"], cfg["bfield"], cfg["mueller"],
+                    cfg["opacity"], w_min=cfg["w_min"], max_scatter=cfg["max_scatter"])
+    s = cfg["source"]
+    m.source_set(s["kind"], s["pos"], s["dir"], s.get("cell_weight"), s.get("emit_records", 0))
+    obs = [OraObserver.make(o["theta"], o["phi"], o["center"], o["half_w"], o["half_h"]) for o in cfg["observers"]]
+    return m, obs
+
+
+def oracle_step(m, obs, cfg, id0, n):
+    """Transport + image packets [id0, id0+n) with the oracle; returns (seconds, events)."""
+    from oracle import OracleEvents, OracleStats
+    ev = OracleEvents(max(1024, 64 * n))
+    st = OracleStats()
+    t0 = time.perf_counter()
+    m.transport(id0, n, cfg["seed"], ev, st)
+    m.image(ev, obs, cfg["npix"], cfg["npix"], stats=st, second_moment=False)
+    return time.perf_counter() - t0, st.as_dict()
+
+
+def oracle_timed(cfg, seconds, chunk=500):
+    """Time the oracle on packets [0, n) of the workload, n grown in chunks until `seconds` have passed."""
+    m, obs = oracle_setup(cfg)
+    oracle_step(m, obs, cfg, 0, 50)                     # touch the arrays once
+    t = 0.0
+    n = 0
+    events = 0
+    while t < seconds:
+        dt, st = oracle_step(m, obs, cfg, n, chunk)
+        t += dt
+        n += chunk
+        events += st["events"]
+    return dict(value=n / t, unit=UNIT, cores=1, kind="oracle", scatterings_per_s=events / t,
+                sample="packet ids [0,%d) of the workload, transport+imaging, single thread fp64, %.1f s" % (n, t))
+
+
+def run_reference(args):
+    rank = int(os.environ.get("RANK", "0"))
+    if rank != 0:
+        return 0
+    cfg, _ = make_workload(args)
+    m, obs = oracle_setup(cfg)
+    # each step is a bounded sample of the workload: `chunk` packets sized from a pilot so that the whole
+    # run (warm-up + steps) takes about two minutes at most
+    dt, _ = oracle_step(m, obs, cfg, 0, 200)
+    per_packet = dt / 200
+    total = max(args.steps + args.warmup, 1)
+    chunk = int(max(100, min(200000, 100.0 / total / per_packet)))
+    nid = 1000
+    for _ in range(args.warmup):
+        oracle_step(m, obs, cfg, nid, chunk); nid += chunk
+    t = 0.0
+    events = 0
+    for _ in range(args.steps):
+        dt, st = oracle_step(m, obs, cfg, nid, chunk); nid += chunk
+        t += dt
+        events += st["events"]
+    value = args.steps * chunk / t
+    sample = "%d packets per step of the workload's id stream, single thread fp64" % chunk
+    line = {
+        "impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+        "warmup": args.warmup, "ms_per_step": 1e3 * t / args.steps, "higher_is_better": True, "scaling": "weak",
+        "vs_baseline": None, "dtype": "f64", "data": "synthetic",
+        "config": {"workload": cfg["name"], "packets_per_step": chunk, "observers": len(cfg["observers"]),
+                   "npix": cfg["npix"], "note": "oracle (oracle/krp_oracle.c) on host cores, bounded sample per step"},
+        "scatterings_per_s": events / t,
+        "cpu_baseline": {"value": value, "unit": UNIT, "cores": 1, "kind": "oracle", "sample": sample},
+        "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+        "gpu_launches": 0,
+    }
+    print(json.dumps(line))
+    return 0
+
+
+# ------------------------------------------------------------------------------------------
+# the CUDA leg
+# ------------------------------------------------------------------------------------------
+# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
+# `ncu --set full` capture of this same command (profiles/, named per round); None until captured.
+NCU_TRAFFIC = {}
+
+
+def make_grid(krp, cfg, dens, bf, weight):
+    g = krp.Grid(cfg["nx"], cfg["ny"], cfg["nz"], cfg["bounds"], dens, bf, cfg["mueller"], cfg["opacity"],
+                 w_min=cfg["w_min"], max_scatter=cfg["max_scatter"])
+    s = cfg["source"]
+    g.source_set(s["kind"], s["pos"], s["dir"], weight, s.get("emit_records", 0))
+    return g
+
+
+def run_krp(args):
+    import torch
+    import torch.distributed as dist
+    from paper_2512_01283_b200 import krp, shard
+
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    rank = int(os.environ.get("RANK", "0"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py needs a CUDA device: there is no CPU fallback (use --impl reference for the oracle)")
+    torch.cuda.set_device(local)
+    dev = torch.device("cuda", local)
+    if world > 1:
+        dist.init_process_group("nccl", device_id=dev)
+
+    def barrier():
+        torch.cuda.synchronize()
+        if world > 1:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    cfg, batch = make_workload(args)
+    n_obs, npix, seed = len(cfg["observers"]), cfg["npix"], cfg["seed"]
+    dens = torch.from_numpy(cfg["density"]).to(dev)
+    bf = None if cfg["bfield"] is None else torch.from_numpy(cfg["bfield"]).to(dev)
+    w_host = cfg["source"].get("cell_weight")
+    weight = None if w_host is None else torch.from_numpy(np.ascontiguousarray(w_host, np.float32).ravel()).to(dev)
+    obs = [krp.make_observer(o["theta"], o["phi"], o["center"], o["half_w"], o["half_h"]) for o in cfg["observers"]]
+    g = make_grid(krp, cfg, dens, bf, weight)
+
+    # pilot (untimed): events per packet of this workload, to size the event buffer once
+    pilot = min(batch, 1 << 16)
+    g.packet_id_set(1 << 40)
+    g.transport(pilot, seed)
+    st = g.stats_get()
+    epp = st["events"] / max(st["packets"], 1)
+    g.events_clear()
+    torch.cuda.synchronize()
+    ev_cap = int(batch * (1.25 * epp + 0.05)) + (1 << 16)
+    g.events_reserve(ev_cap)
+
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)      # > 126 MB L2
+    total_steps = args.warmup + args.steps
+    E = lambda: torch.cuda.Event(enable_timing=True)
+    marks = [(E(), E(), E()) for _ in range(args.steps)]
+
+    def step(i, mark=None):
+        first, cnt = shard.step_id_range(i, rank, world, batch)
+        g.packet_id_set(first)
+        flush.zero_()
+        if mark:
+            mark[0].record()
+        g.transport(cnt, seed)
+        if mark:
+            mark[1].record()
+        g.image(obs, npix, npix)
+        if mark:
+            mark[2].record()
+
+    for i in range(args.warmup):
+        step(i)
+    g.stats_reset()
+    img = torch.zeros((n_obs, 4, npix, npix), dtype=torch.float64, device=dev)
+    launches0 = g.launch_count()
+    barrier()
+    sampler = ClockSampler(local) if rank == 0 else None
+    t_start, t_end = E(), E()
+    t_start.record()
+    for i in range(args.steps):
+        step(args.warmup + i, marks[i])
+    t_end.record()
+    barrier()
+    clocks = sampler.stop() if sampler else None
+    ms_total = t_start.elapsed_time(t_end)
+    launches = g.launch_count() - launches0
+    # end of job: the one exchange of the path, sum of the per-rank maps (outside the per-step timing)
+    g.image_get(out=img)
+    shard.reduce_images(img)
+    torch.cuda.synchronize()
+    t_tr = float(np.mean([m[0].elapsed_time(m[1]) for m in marks]))
+    t_im = float(np.mean([m[1].elapsed_time(m[2]) for m in marks]))
+    st = g.stats_get()
+    if world > 1:
+        t = torch.tensor([ms_total], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        ms_total = float(t.item())
+        cnt = torch.tensor([st["packets"], st["events"], st["steps_transport"], st["steps_image"], st["contributions"]],
+                           dtype=torch.float64, device=dev)
+        dist.all_reduce(cnt, op=dist.ReduceOp.SUM)
+        tot = dict(zip(["packets", "events", "steps_transport", "steps_image", "contributions"], cnt.tolist()))
+    else:
+        tot = st
+    sec = ms_total * 1e-3
+    value = tot["packets"] / sec
+    assert tot["packets"] == args.steps * batch * world, (tot["packets"], args.steps, batch, world)
+
+    # roofline of the dominant kernel (this rank's launches): krp_k_image, one launch per step
+    pk = peaks()
+    mode = "scalar" if (cfg["bfield"] is None and cfg["opacity"].shape[0] == 1) else "general"
+    A = ALGO[mode]
+    K = args.steps
+    rays = st["events"] * n_obs / K
+    im_bytes = (st["steps_image"] * A["cell_bytes"] + st["events"] * 48 + st["contributions"] * A["contrib_bytes"]) / K
+    im_inst = (st["steps_image"] * A["step_inst"]) / K + rays * A["contrib_inst"]
+    alu_peak = N_SM * LANES_PER_SM * pk["sm_max_mhz"] * 1e6          # thread-instructions/s at the maximum SM clock
+    f_hbm = im_bytes / (t_im * 1e-3) / (pk["hbm_gbs"] * 1e9)
+    f_alu = im_inst / (t_im * 1e-3) / alu_peak
+    if f_hbm >= f_alu:
+        roof = {"bound": "hbm", "achieved": im_bytes / (t_im * 1e-3) / 1e9, "peak": pk["hbm_gbs"], "unit": "GB/s", "frac": f_hbm}
+    else:
+        roof = {"bound": "alu", "achieved": im_inst / (t_im * 1e-3) / 1e12, "peak": alu_peak / 1e12,
+                "unit": "Tinst/s", "frac": f_alu}
+    roof.update({"kernel": "krp_k_image<%s>" % mode, "kernel_ms": t_im, "share_of_step": t_im / (t_tr + t_im),
+                 "traffic": NCU_TRAFFIC.get((args.workload, batch)), "peak_source": pk["source"],
+                 "cell_steps_per_launch": st["steps_image"] / K, "rays_per_launch": rays,
+                 "frac_hbm": f_hbm, "frac_alu": f_alu})
+    return dict(world=world, rank=rank, cfg=cfg, batch=batch, value=value, ms_total=ms_total, clocks=clocks, roof=roof,
+                t_tr=t_tr, t_im=t_im, tot=tot, launches=launches, epp=epp, mode=mode, krp=krp, obs=obs, dev=dev,
+                ev_cap=ev_cap, grid=g)
+
+
+def run_e2e(args, r):
+    """The same metric through the C ABI with HOST buffers: every step uploads the model from pinned host
+    memory (krp_grid_create with KRP_MEM_HOST), transports and images one batch and reads the maps back to
+    pinned host memory (krp_image_get with KRP_MEM_HOST)."""
+    import torch
+    krp, cfg, batch, obs, dev = r["krp"], r["cfg"], r["batch"], r["obs"], r["dev"]
+    rank, world = r["rank"], r["world"]
+    from paper_2512_01283_b200 import shard
+    n_obs, npix, seed = len(obs), cfg["npix"], cfg["seed"]
+    pin = lambda a: None if a is None else torch.from_numpy(np.ascontiguousarray(a, np.float32)).pin_memory()
+    h_dens, h_bf = pin(cfg["density"]), pin(cfg["bfield"])
+    w_host = cfg["source"].get("cell_weight")
+    h_w = None if w_host is None else pin(np.asarray(w_host).ravel())
+    h_img = torch.zeros((n_obs, 4, npix, npix), dtype=torch.float64).pin_memory()
+    h2d = h_dens.numel() * 4 + (0 if h_bf is None else h_bf.numel() * 4) + (0 if h_w is None else h_w.numel() * 4) \
+        + cfg["mueller"].nbytes + cfg["opacity"].nbytes
+    d2h = h_img.numel() * 8
+
+    def one(i):
+        first, cnt = shard.step_id_range(1000 + i, rank, world, batch)
+        weight = None if h_w is None else h_w.to(dev, non_blocking=True)
+        g = make_grid(krp, cfg, h_dens.numpy(), None if h_bf is None else h_bf.numpy(), weight)
+        g.events_reserve(r["ev_cap"])
+        g.packet_id_set(first)
+        g.transport(cnt, seed)
+        g.image(obs, npix, npix)
+        g.image_get(out=h_img.numpy())                 # synchronises
+        total_i = float(h_img[:, 0].sum())             # the step's result, read on the host
+        g.close()
+        return total_i
+
+    k = max(1, min(args.steps, 3))
+    one(0)
+    torch.cuda.synchronize()
+    if world > 1:
+        import torch.distributed as dist
+        dist.barrier()
+    t0 = time.perf_counter()
+    for i in range(k):
+        one(1 + i)
+    torch.cuda.synchronize()
+    dt = time.perf_counter() - t0
+    if world > 1:
+        t = torch.tensor([dt], dtype=torch.float64, device=dev)
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        dt = float(t.item())
+    return {"value": k * batch * world / dt, "unit": UNIT, "h2d_bytes_per_step": int(h2d), "d2h_bytes_per_step": int(d2h),
+            "steps": k, "ms_per_step": 1e3 * dt / k,
+            "path": "krp_grid_create(KRP_MEM_HOST, pinned) + krp_transport + krp_image + krp_image_get(KRP_MEM_HOST, pinned)"}
+
+
+def main():
+    args = parse_args()
+    if args.impl == "reference":
+        return run_reference(args)
+    r = run_krp(args)
+    r["grid"].close()
+    e2e = None if args.no_e2e else run_e2e(args, r)
+    if r["world"] > 1:
+        import torch.distributed as dist
+        dist.barrier()
+        dist.destroy_process_group()
+    if r["rank"] != 0:
+        return 0
+    cfg, tot = r["cfg"], r["tot"]
+    cpu = None
+    if r["world"] == 1 and not args.no_cpu_baseline:
+        cpu = oracle_timed(cfg, args.cpu_seconds)
+    sec = r["ms_total"] * 1e-3
+    line = {
+        "metric": METRIC, "value": r["value"], "unit": UNIT, "n_gpus": r["world"], "steps": args.steps, "warmup": args.warmup,
+        "ms_per_step": r["ms_total"] / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+        "dtype": "f32 transport, f64 image accumulation", "data": "synthetic",
+        "config": {"workload": cfg["name"], "grid": [cfg["nx"], cfg["ny"], cfg["nz"]], "packets_per_step_per_gpu": r["batch"],
+                   "observers": len(cfg["observers"]), "npix": cfg["npix"], "cell_layout": r["mode"],
+                   "job_packets": cfg["n_packets"], "events_per_packet": r["epp"],
+                   "l2": "flushed every step by a 256 MiB memset inside the timed region",
+                   "parallelism": "packet ids sharded over %d GPU(s), grid replicated, one fp64 image all-reduce at job end" % r["world"],
+                   "reduced": bool(args.n)},
+        "scatterings_per_s": tot["events"] / sec,
+        "cell_steps_per_s": (tot["steps_transport"] + tot["steps_image"]) / sec,
+        "kernel_ms": {"transport": r["t_tr"], "image": r["t_im"]},
+        "clocks": r["clocks"], "roofline": r["roof"], "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(r["launches"]),
+        "context": "paper: ~1.4e7 packets/s for its own (different) step 1 on an RTX 5090, ~1e2x over CPU codes (PAPER.md:125)",
+    }
+    print(json.dumps(line))
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())
