@@ -10,14 +10,17 @@
  * tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference
  * legs may build, load or call it.
  *
- * Precision: fp64 everywhere, with three deliberate fp32 quantisations that
+ * Precision: fp64 everywhere, with four deliberate fp32 quantisations that
  * are part of the method's *state definition* (R12), made so that
  * integer decisions (which cell an event falls in) are taken on the same
  * numbers by both implementations:
  *   - the lookup tables are the caller's fp32 arrays, read as they are;
  *   - the per-cell unit field direction B^ is stored rounded to fp32;
  *   - the packet direction n^ is stored rounded to fp32 after emission and
- *     after every scattering.
+ *     after every scattering;
+ *   - the cell-local position of a packet is stored rounded to fp32 at
+ *     emission and at every event (the event record holds fp32 positions and
+ *     the next flight starts from the record).
  *
  * Pins (tests/test_oracle_pins.py, -m "not gpu"): every exported function
  * below is pinned to a closed form, an invariant, a library routine
@@ -546,6 +549,7 @@ static int flight(const ora_model* m, int idx[3], double p[3], const double n[3]
                 if (Iout <= target) {
                     double t = ora_event_solve(S[0], 0.0, a[0], 0.0, target);
                     advance(m, idx, p, n, t / kr, -1);
+                    for (int a2 = 0; a2 < 3; ++a2) p[a2] = (double)(float)p[a2];   /* R12 */
                     double I = S[0];
                     for (int s = 0; s < 4; ++s) S[s] /= I;
                     return 1;
@@ -568,6 +572,7 @@ static int flight(const ora_model* m, int idx[3], double p[3], const double n[3]
                     ora_rotate_qu(Sg, ce, -se);
                     for (int s = 0; s < 4; ++s) S[s] = Sg[s];
                     advance(m, idx, p, n, t / kr, -1);
+                    for (int a2 = 0; a2 < 3; ++a2) p[a2] = (double)(float)p[a2];   /* R12 */
                     return 1;
                 }
                 ora_rotate_qu(So, ce, -se);
@@ -611,7 +616,7 @@ static void emit(const ora_model* m, uint64_t seed, uint64_t id, int idx[3], dou
         idx[0] = (int)(c % m->nx); idx[1] = (int)((c / m->nx) % m->ny); idx[2] = (int)(c / ((int64_t)m->nx * m->ny));
         for (int a = 0; a < 3; ++a) p[a] = ora_u01(w2[a]);
     } else {
-        for (int a = 0; a < 3; ++a) { idx[a] = m->src_idx[a]; p[a] = m->src_p[a]; }
+        for (int a = 0; a < 3; ++a) { idx[a] = m->src_idx[a]; p[a] = (double)(float)m->src_p[a]; }   /* R12 */
     }
 }
 

@@ -376,8 +376,8 @@ extern "C" int krp_transport(krp_grid* g, uint64_t n_packets, uint64_t seed, voi
     for (int w = 0; w < g->max_waves; ++w) {
         const int in = w & 1;
         krp_k_wave_prep<<<1, 1, 0, st>>>(g->d_ctl, in);
-        if (g->m.scalar) krp_k_flight<true><<<grid_f, tb, 0, st>>>(g->m, g->d_ctl, g->q[in], in, g->ev);
-        else             krp_k_flight<false><<<grid_f, tb, 0, st>>>(g->m, g->d_ctl, g->q[in], in, g->ev);
+        if (g->m.scalar) krp_k_flight_scalar<<<grid_f, tb, 0, st>>>(g->m, g->d_ctl, g->q[in], in, g->ev);
+        else             krp_k_flight_general<<<grid_f, tb, 0, st>>>(g->m, g->d_ctl, g->q[in], in, g->ev);
         g->launches += 2;
         if (w + 1 < g->max_waves) {
             krp_k_scatter<<<grid_s, 128, 0, st>>>(g->m, g->d_ctl, g->ev, g->q[1 - in], 1 - in, seed);

@@ -162,6 +162,61 @@ __device__ __forceinline__ bool krp_ray_step(KrpRay& r, float ds)
     return (r.lx | r.ly | r.lz) >= 0;
 }
 
+// The same march with the distances in fp64: used by the general-mode flight, where the optical
+// depth consumed in every cell decides the integer outcome "which cell holds the event" and has to
+// be taken in the oracle's precision.
+struct KrpRayD {
+    double rx, ry, rz;
+    double tx, ty, tz;
+    int sx, sy, sz;
+    int lx, ly, lz;
+    uint32_t c;
+};
+
+__device__ __forceinline__ void krp_rayd_axis(float n, float p, double d, int stride, int i, int N,
+                                              double& r, double& t, int& s, int& l)
+{
+    if (n > 0.f)      { r = (1.0 - (double)p) * d / (double)n; t = d / (double)n;  s = stride;  l = N - 1 - i; }
+    else if (n < 0.f) { r = (double)p * d / -(double)n;        t = d / -(double)n; s = -stride; l = i; }
+    else              { t = __longlong_as_double(0x7ff0000000000000ll); r = t; s = 0; l = 0x7fffffff; }
+}
+
+__device__ __forceinline__ void krp_rayd_init(const KrpModel& g, uint32_t cell, const float p[3], const float n[3], KrpRayD& r)
+{
+    int ix = (int)(cell % (uint32_t)g.nx);
+    uint32_t t = cell / (uint32_t)g.nx;
+    int iy = (int)(t % (uint32_t)g.ny), iz = (int)(t / (uint32_t)g.ny);
+    krp_rayd_axis(n[0], p[0], g.dd[0], 1, ix, g.nx, r.rx, r.tx, r.sx, r.lx);
+    krp_rayd_axis(n[1], p[1], g.dd[1], g.nx, iy, g.ny, r.ry, r.ty, r.sy, r.ly);
+    krp_rayd_axis(n[2], p[2], g.dd[2], g.nx * g.ny, iz, g.nz, r.rz, r.tz, r.sz, r.lz);
+    r.c = cell;
+}
+
+__device__ __forceinline__ double krp_rayd_ds(const KrpRayD& r) { return fmin(r.rx, fmin(r.ry, r.rz)); }
+
+__device__ __forceinline__ bool krp_rayd_step(KrpRayD& r, double ds)
+{
+    bool ax = (r.rx <= r.ry) & (r.rx <= r.rz);
+    bool ay = (!ax) & (r.ry <= r.rz);
+    bool az = !(ax | ay);
+    r.rx = ax ? r.tx : r.rx - ds;
+    r.ry = ay ? r.ty : r.ry - ds;
+    r.rz = az ? r.tz : r.rz - ds;
+    int s = ax ? r.sx : (ay ? r.sy : r.sz);
+    r.c += (uint32_t)s;
+    r.lx -= ax; r.ly -= ay; r.lz -= az;
+    return (r.lx | r.ly | r.lz) >= 0;
+}
+
+// cell-local position (fp64 distances) after moving `moved` from the point where r was taken
+__device__ __forceinline__ float krp_locald(float n, double r, double t, double moved, float p0)
+{
+    if (n == 0.f) return p0;
+    double f = (r - moved) / t;
+    f = fmin(fmax(f, 0.0), 1.0);
+    return (float)(n > 0.f ? 1.0 - f : f);
+}
+
 // cell-local position after moving `moved` from the point where the distances r were taken
 __device__ __forceinline__ float krp_local(float n, float r, float t, float moved, float p0)
 {

@@ -107,14 +107,13 @@ __device__ __forceinline__ float krp_event_solve(float R, float qq, float a1, fl
 }
 
 // ------------------------------------------------------------------------------------------
-// T3/T4/T5  one flight per queue entry: march cell to cell applying the App. A
-// solution in every cell until the survival I(s)/I(0) falls to e^{-tau*} (R7)
-// or the packet leaves the grid; at an event append the pre-scatter record.
-// SCALAR = the opacity table does not depend on direction and alpha2 = alpha3 = 0: the cell is
-// 4 bytes (kappa*rho) and the Stokes vector only scales.
+// T3/T4/T5, scalar mode: the opacity table does not depend on direction and alpha2 = alpha3 = 0,
+// so a cell is 4 bytes (kappa*rho), the Stokes vector only scales and the event is where the
+// optical depth alpha1*kappa*rho*s reaches tau* (PAPER.md:107-109).  One flight per queue entry:
+// march cell to cell until the event or the grid edge; at an event append the pre-scatter record.
+// The march is fp32; the depth still to go is kept in fp64.
 // ------------------------------------------------------------------------------------------
-template <bool SCALAR>
-__global__ void __launch_bounds__(256) krp_k_flight(KrpModel g, KrpCtl* ctl, KrpRecords q, int in, KrpRecords ev)
+__global__ void __launch_bounds__(256) krp_k_flight_scalar(KrpModel g, KrpCtl* ctl, KrpRecords q, int in, KrpRecords ev)
 {
     const unsigned int n_items = ctl->q_count[in];
     unsigned long long steps = 0, n_ev = 0, n_over = 0;
@@ -124,91 +123,22 @@ __global__ void __launch_bounds__(256) krp_k_flight(KrpModel g, KrpCtl* ctl, Krp
         const float n[3] = { nk.x, nk.y, nk.z };
         const float p0[3] = { pc.x, pc.y, pc.z };
         const uint32_t k = __float_as_uint(nk.w);
-        const double tau0 = q.tau[item];
         KrpRay ray;
         krp_ray_init(g, __float_as_uint(pc.w), p0, n, ray);
-        float th[3], ph[3];
-        if (!SCALAR) krp_basis<float>(n, th, ph);
-        double D = tau0, i = 1.0;
-        float qs = S0.y, us = S0.z, vs = S0.w;      // lab reference
-        float Asum = 0.f;
-        const float tau0f = (float)tau0, guard = 1.f + g.rho + 1e-3f;
+        double D = q.tau[item];
         bool hit = false;
-        float moved = 0.f, omega = g.omc, ds = 0.f;
+        float moved = 0.f, ds = 0.f;
         for (;;) {
             ds = krp_ray_ds(ray);
             ++steps;
-            if (SCALAR) {
-                float kr = __ldg(g.kr + ray.c);
-                float dt1 = g.a1c * kr * ds;
-                if ((double)dt1 >= D) {              // event inside this cell
-                    moved = (float)D / (g.a1c * kr);
-                    hit = true;
-                    break;
-                }
-                D -= (double)dt1;
-            } else {
-                float4 cl = __ldg(g.cell + ray.c);
-                float kr = cl.x;
-                if (kr > 0.f) {
-                    float mu = n[0] * cl.y + n[1] * cl.z + n[2] * cl.w;
-                    float4 op = krp_opac_at(g.opac, g.n_inc, fabsf(mu));
-                    float dtau = kr * ds;
-                    if (op.y == 0.f && op.z == 0.f) {
-                        float dt1 = op.x * dtau;
-                        double Dn = D - (double)dt1;
-                        Asum += dt1;
-                        if (Asum * guard >= tau0f) {
-                            double R = D + (double)logf((float)i);
-                            if ((double)dt1 >= R) {
-                                moved = ((float)R / op.x) / kr;
-                                float inv = 1.f / (float)i;
-                                qs *= inv; us *= inv; vs *= inv;
-                                omega = op.w; hit = true;
-                                break;
-                            }
-                        }
-                        D = Dn;
-                    } else {
-                        float a = th[0] * cl.y + th[1] * cl.z + th[2] * cl.w;
-                        float b = ph[0] * cl.y + ph[1] * cl.z + ph[2] * cl.w;
-                        float c2, s2;
-                        krp_eta2<float>(a, b, c2, s2);
-                        float qg = c2 * qs + s2 * us, ug = -s2 * qs + c2 * us, vg = vs;   // eq. 7
-                        const float qg_e = qg, ug_e = ug, vg_e = vg;
-                        const float i_f = (float)i;
-                        float di, i_new, depth;
-                        bool thick = krp_appA(i_f, qg, ug, vg, op, dtau, di, i_new, depth);
-                        double in_d = thick ? (double)i_new : i + (double)di;
-                        double Dn = D - (double)depth;
-                        Asum += op.x * dtau;
-                        if (Asum * guard >= tau0f) {
-                            // survival test on the exit state: ln(i') + D' <= 0
-                            if ((double)logf((float)in_d) + Dn <= 0.0) {
-                                float R = (float)(D + (double)logf(i_f));
-                                float qq = qg_e / i_f;
-                                float t = krp_event_solve(R, qq, op.x, op.y, dtau);
-                                // state at t, normalised to I = 1, back to the lab reference
-                                float sh, chm1, sy = 0.f, cy = 1.f;
-                                krp_sinh_coshm1(op.y * t, sh, chm1);
-                                if (op.z != 0.f) sincosf(op.z * t, &sy, &cy);
-                                float it = i_f + (i_f * chm1 - qg_e * sh);
-                                float qt = qg_e + (qg_e * chm1 - i_f * sh);
-                                float ut = ug_e * cy - vg_e * sy;
-                                float vt = ug_e * sy + vg_e * cy;
-                                float inv = 1.f / it;
-                                qt *= inv; ut *= inv; vt *= inv;
-                                qs = c2 * qt - s2 * ut; us = s2 * qt + c2 * ut; vs = vt;
-                                moved = t / kr;
-                                omega = op.w; hit = true;
-                                break;
-                            }
-                        }
-                        qs = c2 * qg - s2 * ug; us = s2 * qg + c2 * ug; vs = vg;
-                        i = in_d; D = Dn;
-                    }
-                }
+            const float kr = __ldg(g.kr + ray.c);
+            const float dt1 = g.a1c * kr * ds;
+            if ((double)dt1 >= D) {              // event inside this cell
+                moved = (float)D / (g.a1c * kr);
+                hit = true;
+                break;
             }
+            D -= (double)dt1;
             if (!krp_ray_step(ray, ds)) break;
         }
         const float W = S0.x;
@@ -218,6 +148,194 @@ __global__ void __launch_bounds__(256) krp_k_flight(KrpModel g, KrpCtl* ctl, Krp
         pe[0] = krp_local(n[0], ray.rx, ray.tx, moved, p0[0]);
         pe[1] = krp_local(n[1], ray.ry, ray.ty, moved, p0[1]);
         pe[2] = krp_local(n[2], ray.rz, ray.tz, moved, p0[2]);
+        const float Wn = g.omc * W;
+        const uint32_t kn = k + 1u;
+        const bool term = (Wn < g.w_min) || ((int)kn >= g.max_scatter);
+        w_abs += (double)W - (double)Wn;
+        unsigned long long slot = krp_reserve64(&ctl->n_events);
+        if (slot < ctl->ev_cap) {
+            ev.pc[slot] = make_float4(pe[0], pe[1], pe[2], __uint_as_float(ray.c));
+            ev.nk[slot] = make_float4(n[0], n[1], n[2], __uint_as_float(kn | (term ? KRP_TERM_BIT : 0u)));
+            ev.S[slot] = make_float4(Wn, S0.y, S0.z, S0.w);
+            ev.id[slot] = q.id[item];
+            ++n_ev;
+            if (term) w_cut += (double)Wn;
+        } else {
+            ++n_over;
+            w_cut += (double)Wn;
+        }
+    }
+    // statistics: one atomic per warp and counter
+    steps = krp_warp_sum(steps); n_ev = krp_warp_sum(n_ev); n_over = krp_warp_sum(n_over);
+    w_esc = krp_warp_sum(w_esc); w_abs = krp_warp_sum(w_abs); w_cut = krp_warp_sum(w_cut);
+    if ((threadIdx.x & 31) == 0) {
+        if (steps) atomicAdd(&ctl->stats.steps_transport, steps);
+        if (n_ev) atomicAdd(&ctl->stats.events, n_ev);
+        if (n_over) atomicAdd(&ctl->stats.overflow, n_over);
+        if (w_esc != 0.0) atomicAdd(&ctl->stats.w_escaped, w_esc);
+        if (w_abs != 0.0) atomicAdd(&ctl->stats.w_absorbed, w_abs);
+        if (w_cut != 0.0) atomicAdd(&ctl->stats.w_cut, w_cut);
+    }
+}
+
+// ------------------------------------------------------------------------------------------
+// T4 in fp64 (general mode): same equation as krp_event_solve; the root decides where the event
+// lies, so it is located in the oracle's precision.
+// ------------------------------------------------------------------------------------------
+__device__ __forceinline__ double krp_event_solve_d(double R, double qq, double a1, double a2, double tmax)
+{
+    double t = R / a1;
+    if (a2 != 0.0) {
+#pragma unroll 1
+        for (int it = 0; it < 40; ++it) {
+            double x = a2 * t;
+            double sh = sinh(x), ch = cosh(x);
+            double gm1 = (ch - 1.0) - qq * sh;
+            double h = a1 * t - log1p(gm1) - R;
+            double hp = a1 - a2 * (sh - qq * ch) / (1.0 + gm1);
+            double dt = h / hp;
+            t = fmin(fmax(t - dt, 0.0), tmax);
+            if (fabs(dt) <= 4e-16 * t) break;
+        }
+    }
+    return fmin(fmax(t, 0.0), tmax);
+}
+
+// 1/sqrt(1+e) for |e| << 1 (unit vectors stored in fp32 have |v|^2 = 1 + O(1e-7))
+__device__ __forceinline__ double krp_rsqrt_near1(double vv)
+{
+    double e = vv - 1.0;
+    return 1.0 + e * (-0.5 + e * (0.375 - 0.3125 * e));
+}
+
+// ------------------------------------------------------------------------------------------
+// T3/T4/T5, general mode (direction-dependent, dichroic opacity; 16-byte cells).  Everything that
+// decides in which cell the event falls -- segment lengths, alpha1(mu), the scalar depth D and the
+// normalised intensity i -- is carried in fp64 (an integer decided by
+// floating point is taken in the oracle's precision); the Stokes algebra (reference rotation,
+// sinh/cosh/sin/cos factors, q,u,v) is fp32.
+// ------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) krp_k_flight_general(KrpModel g, KrpCtl* ctl, KrpRecords q, int in, KrpRecords ev)
+{
+    const unsigned int n_items = ctl->q_count[in];
+    unsigned long long steps = 0, n_ev = 0, n_over = 0;
+    double w_esc = 0.0, w_abs = 0.0, w_cut = 0.0;
+    const double xs = (double)(g.n_inc - 1);
+    for (unsigned int item = blockIdx.x * blockDim.x + threadIdx.x; item < n_items; item += gridDim.x * blockDim.x) {
+        const float4 pc = q.pc[item], nk = q.nk[item], S0 = q.S[item];
+        const float n[3] = { nk.x, nk.y, nk.z };
+        const float p0[3] = { pc.x, pc.y, pc.z };
+        const uint32_t k = __float_as_uint(nk.w);
+        const double tau0 = q.tau[item];
+        KrpRayD ray;
+        krp_rayd_init(g, __float_as_uint(pc.w), p0, n, ray);
+        float th[3], ph[3];
+        krp_basis<float>(n, th, ph);
+        const double nd[3] = { n[0], n[1], n[2] };
+        const double inv_n = krp_rsqrt_near1(nd[0] * nd[0] + nd[1] * nd[1] + nd[2] * nd[2]);
+        double D = tau0, i = 1.0;
+        float qs = S0.y, us = S0.z, vs = S0.w;      // lab reference
+        float Asum = 0.f;
+        const float tau0f = (float)tau0, guard = 1.f + g.rho + 1e-3f;
+        bool hit = false;
+        double moved = 0.0;
+        float omega = g.omc;
+        for (;;) {
+            const double ds = krp_rayd_ds(ray);
+            ++steps;
+            const float4 cl = __ldg(g.cell + ray.c);
+            const float kr = cl.x;
+            if (kr > 0.f) {
+                const double bx = cl.y, by = cl.z, bz = cl.w;
+                double mu = fabs(nd[0] * bx + nd[1] * by + nd[2] * bz) * inv_n * krp_rsqrt_near1(bx * bx + by * by + bz * bz);
+                mu = fmin(mu, 1.0);
+                const double x = mu * xs;
+                const int j = min((int)x, g.n_inc - 2);
+                const double w = x - (double)j;
+                const float4 oa = g.opac[j], ob = g.opac[j + 1];
+                const double a1 = (1.0 - w) * (double)oa.x + w * (double)ob.x;
+                const float wf = (float)w, w0f = 1.f - wf;
+                const float a2 = w0f * oa.y + wf * ob.y, a3 = w0f * oa.z + wf * ob.z;
+                const double dtau = (double)kr * ds;
+                const double dt1 = a1 * dtau;
+                Asum += (float)dt1;
+                const bool near_end = Asum * guard >= tau0f;
+                if (a2 == 0.f && a3 == 0.f) {
+                    if (near_end) {
+                        const double R = D + log(i);
+                        if (dt1 >= R) {
+                            moved = (R / a1) / (double)kr;
+                            const float inv = (float)(1.0 / i);
+                            qs *= inv; us *= inv; vs *= inv;
+                            omega = w0f * oa.w + wf * ob.w; hit = true;
+                            break;
+                        }
+                    }
+                    D -= dt1;
+                } else {
+                    const float a = th[0] * cl.y + th[1] * cl.z + th[2] * cl.w;
+                    const float b = ph[0] * cl.y + ph[1] * cl.z + ph[2] * cl.w;
+                    float c2, s2;
+                    krp_eta2<float>(a, b, c2, s2);
+                    const float qg_e = c2 * qs + s2 * us, ug_e = -s2 * qs + c2 * us, vg_e = vs;   // eq. 7
+                    const float dtau_f = (float)dtau, i_f = (float)i;
+                    const float xx = a2 * dtau_f, yy = a3 * dtau_f;
+                    float sy = 0.f, cy = 1.f;
+                    if (yy != 0.f) sincosf(yy, &sy, &cy);
+                    float qg, ug, vg;
+                    double i_new, depth;
+                    if (fabsf(xx) < 0.35f) {
+                        float sh, chm1;
+                        krp_sinh_coshm1(xx, sh, chm1);
+                        i_new = i + (double)(i_f * chm1 - qg_e * sh);
+                        qg = qg_e + (qg_e * chm1 - i_f * sh);
+                        ug = ug_e * cy - vg_e * sy;
+                        vg = ug_e * sy + vg_e * cy;
+                        depth = dt1;
+                    } else {
+                        // thick cell: factor e^{-|alpha2 dtau|} moved into the scalar depth (no overflow at dtau ~ 1e3)
+                        const double xd = (double)a2 * dtau, axd = fabs(xd);
+                        const double E = exp(-2.0 * axd), s = xd > 0.0 ? 1.0 : -1.0, f = exp(-axd);
+                        const double qd = (double)qg_e;
+                        i_new = 0.5 * ((i - s * qd) + (i + s * qd) * E);
+                        qg = (float)(0.5 * ((qd - s * i) + (qd + s * i) * E));
+                        ug = (float)f * (ug_e * cy - vg_e * sy);
+                        vg = (float)f * (ug_e * sy + vg_e * cy);
+                        depth = dt1 - axd;
+                    }
+                    const double Dn = D - depth;
+                    if (near_end && log(i_new) + Dn <= 0.0) {
+                        // event inside this cell: solve for t, evolve to t, normalise to I = 1, back to the lab reference
+                        const double R = D + log(i);
+                        const double t = krp_event_solve_d(R, (double)qg_e / i, a1, (double)a2, dtau);
+                        const float tf = (float)t;
+                        float sh, chm1, syt = 0.f, cyt = 1.f;
+                        krp_sinh_coshm1(a2 * tf, sh, chm1);
+                        if (a3 != 0.f) sincosf(a3 * tf, &syt, &cyt);
+                        const float it = i_f + (i_f * chm1 - qg_e * sh);
+                        float qt = qg_e + (qg_e * chm1 - i_f * sh);
+                        float ut = ug_e * cyt - vg_e * syt;
+                        float vt = ug_e * syt + vg_e * cyt;
+                        const float inv = 1.f / it;
+                        qt *= inv; ut *= inv; vt *= inv;
+                        qs = c2 * qt - s2 * ut; us = s2 * qt + c2 * ut; vs = vt;
+                        moved = t / (double)kr;
+                        omega = w0f * oa.w + wf * ob.w; hit = true;
+                        break;
+                    }
+                    qs = c2 * qg - s2 * ug; us = s2 * qg + c2 * ug; vs = vg;
+                    i = i_new; D = Dn;
+                }
+            }
+            if (!krp_rayd_step(ray, ds)) break;
+        }
+        const float W = S0.x;
+        if (!hit) { w_esc += (double)W; continue; }
+        // T5: event record, albedo weighting, termination (R12)
+        float pe[3];
+        pe[0] = krp_locald(n[0], ray.rx, ray.tx, moved, p0[0]);
+        pe[1] = krp_locald(n[1], ray.ry, ray.ty, moved, p0[1]);
+        pe[2] = krp_locald(n[2], ray.rz, ray.tz, moved, p0[2]);
         const float Wn = omega * W;
         const uint32_t kn = k + 1u;
         const bool term = (Wn < g.w_min) || ((int)kn >= g.max_scatter);
@@ -235,7 +353,6 @@ __global__ void __launch_bounds__(256) krp_k_flight(KrpModel g, KrpCtl* ctl, Krp
             w_cut += (double)Wn;
         }
     }
-    // statistics: one atomic per warp and counter
     steps = krp_warp_sum(steps); n_ev = krp_warp_sum(n_ev); n_over = krp_warp_sum(n_over);
     w_esc = krp_warp_sum(w_esc); w_abs = krp_warp_sum(w_abs); w_cut = krp_warp_sum(w_cut);
     if ((threadIdx.x & 31) == 0) {

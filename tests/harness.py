@@ -63,9 +63,11 @@ def gpu_events_sorted(g):
     return {k: v[order] for k, v in ev.items()}
 
 
-def compare_sequences(ora, gpu, ids, stokes_tol=1e-4, pos_tol=2e-3):
+def compare_sequences(ora, gpu, ids, stokes_tol=1e-4, pos_tol=1e-2):
     """Per-packet comparison (reading R15): a packet agrees when both sides have the same number of events,
     the same cell at every event, and every Stokes vector within stokes_tol of the oracle's (|dS|_2 / I).
+    On top of the north_star's criterion the cell-local positions must agree within pos_tol (fraction of a cell)
+    and the directions within 1e-5.
     Returns (fraction of packets that agree, dict of diagnostics)."""
     ids = np.asarray(ids, np.uint64)
     n = len(ids)

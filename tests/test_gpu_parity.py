@@ -30,7 +30,11 @@ def _image_checks(img_g, img_o, img2_o, name):
     for s, lab in enumerate("IQU"):
         tot_o, tot_g = img_o[:, s].sum(), img_g[:, s].sum()
         assert abs(tot_g - tot_o) <= 0.005 * max(abs(tot_o), 1e-3 * I_o), (name, lab, tot_g, tot_o)
-    sigma = np.sqrt(img2_o)
+    # sigma per pixel from the oracle's second moments; a contribution whose position rounds across a pixel
+    # edge moves between neighbours, so each pixel may use the largest sigma of its 3x3 neighbourhood
+    pad = np.pad(img2_o, ((0, 0), (0, 0), (1, 1), (1, 1)))
+    ny, nx = img2_o.shape[2:]
+    sigma = np.sqrt(np.max([pad[:, :, dy:dy + ny, dx:dx + nx] for dy in range(3) for dx in range(3)], axis=0))
     floor = 1e-6 * img_o[:, 0].max()
     bad = np.abs(img_g - img_o) > 3 * sigma + floor
     assert bad.sum() == 0, (name, int(bad.sum()), float(np.abs(img_g - img_o).max()))
@@ -115,7 +119,7 @@ def test_empty_and_degenerate_inputs():
     # vacuum: every packet escapes after nx/2 steps, no events
     cfg["density"][:] = 0
     g = gpu_grid(cfg)
-    g.transport(1000, 3)
+    g.transport(1000, cfg["seed"])
     st = g.stats_get()
     assert st["events"] == 0 and st["w_escaped"] == 1000.0
     ora, _, _, st_o = oracle_run(cfg, 0, 1000, image=False)
@@ -161,10 +165,12 @@ def test_thick_cells_and_collimated_beam():
         mu = np.linspace(0, 1, 5)
         cfg["opacity"] = np.stack([np.ones(5), a2 * (1 - mu * mu), 0.1 * (1 - mu * mu), np.full(5, 0.7)], 1).astype(np.float32)
         cfg["source"] = dict(kind=2, pos=[0.01, 0.02, -0.5], dir=[0, 0, 1], cell_weight=None)
-        ora, img_o, img2_o, st_o = oracle_run(cfg, 0, 3000)
+        ora, img_o, img2_o, st_o = oracle_run(cfg, 0, 3000, cap=64 * 3000)
         g = gpu_grid(cfg)
+        g.events_reserve(64 * 3000)
         g.transport(3000, cfg["seed"])
         frac, info = compare_sequences(ora, gpu_events_sorted(g), np.arange(3000))
+        print(bvec, frac, info)
         assert frac >= 0.999, (bvec, info)
         g.image(gpu_observers(cfg), 8, 8)
         _image_checks(g.image_get(), img_o, img2_o, "thick")

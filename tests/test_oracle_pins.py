@@ -619,6 +619,7 @@ def test_event_stokes_in_dichroic_medium_and_invariants():
     E = esc["S"]; assert np.all(E[:, 0] ** 2 >= (E[:, 1:] ** 2).sum(1) * (1 - 1e-12))
     assert np.allclose(np.linalg.norm(ev.n_in[:n], axis=1), 1, atol=2e-7)
     assert np.array_equal(ev.n_in[:n].astype(np.float32).astype(float), ev.n_in[:n])     # fp32 state (R12)
+    assert np.array_equal(ev.p[:n].astype(np.float32).astype(float), ev.p[:n])           # fp32 positions (R12)
     assert np.all((ev.p[:n] >= 0) & (ev.p[:n] <= 1))
     # weights: k-th event carries omega^k
     assert np.allclose(S[:, 0], float(np.float32(om)) ** ev.k[:n], rtol=1e-12)
@@ -735,7 +736,9 @@ def test_image_direct_light_and_projection():
     img, _, st2 = m.image(ev, [o], 30, 20, 1)
     n_obs = np.array([math.sin(th) * math.cos(ph), math.sin(th) * math.sin(ph), math.cos(th)])
     tv, pv = sph_basis(n_obs)
-    x = np.array([0.3, -0.2, 0.5])
+    # the record holds the cell index and the fp32 cell-local position (reading R12): rebuild x from them
+    cl = (np.array([0.3, -0.2, 0.5]) + 1) / 0.25
+    x = -1 + (np.floor(cl) + (cl - np.floor(cl)).astype(np.float32).astype(float)) * 0.25
     ix = int(math.floor((np.dot(x, pv) / 1.5 + 1) * 15)); iy = int(math.floor((-np.dot(x, tv) / 1.0 + 1) * 10))
     tt = min(((1 - x[a]) / n_obs[a]) if n_obs[a] > 0 else ((-1 - x[a]) / n_obs[a]) for a in range(3))
     assert st2.contributions == 1 and np.count_nonzero(img[0, 0]) == 1
