@@ -39,6 +39,17 @@ struct krp_grid {
     float* d_kr = nullptr;
     float4* d_cell = nullptr;
     float4* d_opac = nullptr;
+    float4* d_opA = nullptr;
+    float4* d_opB = nullptr;
+    uint32_t npad = 0;
+    // imaging order (counting sort of the events by cell bin)
+    unsigned int* d_bins = nullptr;
+    uint32_t n_bins = 0;
+    int bin_shift = 0;
+    unsigned int* d_perm = nullptr;
+    uint64_t perm_cap = 0;
+    void* d_scan = nullptr;
+    size_t scan_bytes = 0;
     float4* d_mueller = nullptr;
     double* d_cdf = nullptr;
     double* d_src_cdf = nullptr;
@@ -52,6 +63,7 @@ struct krp_grid {
     double* d_img = nullptr;
     int n_obs = 0, npx = 0, npy = 0;
     std::vector<krp_observer> obs_host;
+    std::vector<KrpObserverDev> obs_dev;
     uint64_t next_id = 0;
     uint64_t launches = 0;
     int max_waves = 0;
@@ -82,6 +94,7 @@ extern "C" int krp_grid_destroy(krp_grid* g)
     if (!g) return KRP_OK;
     cudaFree(g->d_kr); cudaFree(g->d_cell); cudaFree(g->d_opac); cudaFree(g->d_mueller); cudaFree(g->d_cdf);
     cudaFree(g->d_src_cdf); cudaFree(g->d_ctl); cudaFree(g->d_obs); cudaFree(g->d_img);
+    cudaFree(g->d_opA); cudaFree(g->d_opB); cudaFree(g->d_bins); cudaFree(g->d_perm); cudaFree(g->d_scan);
     free_records(g->q[0]); free_records(g->q[1]); free_records(g->ev);
     delete g;
     return KRP_OK;
@@ -91,7 +104,7 @@ static int check_tables(const krp_tables* t)
 {
     if (!t) return fail(KRP_ERR_ARG, "tables is NULL");
     if (t->n_ang < 2 || !t->mueller) return fail(KRP_ERR_ARG, "tables: n_ang must be >= 2 and mueller non-NULL");
-    if (t->n_inc < 1 || !t->opacity) return fail(KRP_ERR_ARG, "tables: n_inc must be >= 1 and opacity non-NULL");
+    if (t->n_inc < 1 || t->n_inc > 1024 || !t->opacity) return fail(KRP_ERR_ARG, "tables: n_inc must be in 1..1024 and opacity non-NULL");
     if (!(t->w_min >= 0.f)) return fail(KRP_ERR_ARG, "tables: w_min must be >= 0");
     if (t->max_scatter < 1) return fail(KRP_ERR_ARG, "tables: max_scatter must be >= 1");
     for (int j = 0; j < t->n_ang; ++j) {
@@ -118,7 +131,7 @@ extern "C" int krp_grid_create(krp_grid** out, int nx, int ny, int nz, const dou
     if (!out) return fail(KRP_ERR_ARG, "out is NULL");
     *out = nullptr;
     if (nx < 1 || ny < 1 || nz < 1) return fail(KRP_ERR_ARG, "grid dims must be positive (%d,%d,%d)", nx, ny, nz);
-    if ((uint64_t)nx * ny * nz >= (1ull << 31)) return fail(KRP_ERR_ARG, "grid has too many cells (limit 2^31)");
+    if ((uint64_t)(nx + 2) * (ny + 2) * (nz + 2) >= (1ull << 31)) return fail(KRP_ERR_ARG, "grid has too many cells (limit 2^31 with halo)");
     if (!bounds) return fail(KRP_ERR_ARG, "bounds is NULL");
     for (int a = 0; a < 3; ++a)
         if (!(bounds[2 * a + 1] > bounds[2 * a]) || !std::isfinite(bounds[2 * a]) || !std::isfinite(bounds[2 * a + 1]))
@@ -138,6 +151,8 @@ extern "C" int krp_grid_create(krp_grid** out, int nx, int ny, int nz, const dou
     KrpModel& m = g->m;
     memset(&m, 0, sizeof(m));
     m.nx = nx; m.ny = ny; m.nz = nz; m.ncell = (uint32_t)((uint64_t)nx * ny * nz);
+    m.px = nx + 2; m.py = ny + 2; m.pxy = (uint32_t)m.px * (uint32_t)m.py;
+    g->npad = m.pxy * (uint32_t)(nz + 2);
     const int dims[3] = { nx, ny, nz };
     for (int a = 0; a < 3; ++a) {
         m.lo[a] = bounds[2 * a];
@@ -174,6 +189,21 @@ extern "C" int krp_grid_create(krp_grid** out, int nx, int ny, int nz, const dou
     }
     CK(cudaMalloc(&g->d_opac, sizeof(float4) * n_inc));
     CK(cudaMemcpyAsync(g->d_opac, op.data(), sizeof(float4) * n_inc, cudaMemcpyHostToDevice, st));
+    {   // the same table as intercept + slope per segment of x = mu*(n_inc-1): value = A_j + B_j x on [j, j+1]
+        std::vector<float> A(4 * (size_t)(n_inc - 1)), B(4 * (size_t)(n_inc - 1));
+        for (int j = 0; j + 1 < n_inc; ++j)
+            for (int s = 0; s < 4; ++s) {
+                double a = op[4 * j + s], b = op[4 * (j + 1) + s];
+                B[4 * j + s] = (float)(b - a);
+                A[4 * j + s] = (float)(a - (b - a) * j);
+            }
+        CK(cudaMalloc(&g->d_opA, sizeof(float4) * (n_inc - 1)));
+        CK(cudaMalloc(&g->d_opB, sizeof(float4) * (n_inc - 1)));
+        CK(cudaMemcpyAsync(g->d_opA, A.data(), sizeof(float4) * (n_inc - 1), cudaMemcpyHostToDevice, st));
+        CK(cudaMemcpyAsync(g->d_opB, B.data(), sizeof(float4) * (n_inc - 1), cudaMemcpyHostToDevice, st));
+        CK(cudaStreamSynchronize(st));          // A, B are locals
+        m.opA = g->d_opA; m.opB = g->d_opB;
+    }
     CK(cudaMalloc(&g->d_mueller, sizeof(float4) * m.n_ang));
     CK(cudaMemcpyAsync(g->d_mueller, tables->mueller, sizeof(float4) * m.n_ang, cudaMemcpyHostToDevice, st));
     // Theta CDF: trapezoid of S11 sin(Theta) on the nodes, fp64 (R13)
@@ -195,40 +225,30 @@ extern "C" int krp_grid_create(krp_grid** out, int nx, int ny, int nz, const dou
     CK(cudaMemcpyAsync(g->d_cdf, cdf.data(), sizeof(double) * m.n_ang, cudaMemcpyHostToDevice, st));
     m.opac = g->d_opac; m.mueller = g->d_mueller; m.cdf = g->d_cdf;
 
-    // cells
+    // cells: packed into the padded layout (one-cell halo with kappa*rho = -1)
     const float* d_den = density;
     const float* d_b = bfield;
     float* tmp_den = nullptr;
     float* tmp_b = nullptr;
     if (mem == KRP_MEM_HOST) {
-        if (m.scalar) {
-            // the packed layout of SCALAR mode is the density array itself
-            CK(cudaMalloc(&g->d_kr, sizeof(float) * (size_t)m.ncell));
-            CK(cudaMemcpyAsync(g->d_kr, density, sizeof(float) * (size_t)m.ncell, cudaMemcpyHostToDevice, st));
-            d_den = g->d_kr;
-        } else {
-            CK(cudaMalloc(&tmp_den, sizeof(float) * (size_t)m.ncell));
-            CK(cudaMemcpyAsync(tmp_den, density, sizeof(float) * (size_t)m.ncell, cudaMemcpyHostToDevice, st));
-            d_den = tmp_den;
-            if (bfield) {
-                CK(cudaMalloc(&tmp_b, sizeof(float) * 3 * (size_t)m.ncell));
-                CK(cudaMemcpyAsync(tmp_b, bfield, sizeof(float) * 3 * (size_t)m.ncell, cudaMemcpyHostToDevice, st));
-                d_b = tmp_b;
-            }
+        CK(cudaMalloc(&tmp_den, sizeof(float) * (size_t)m.ncell));
+        CK(cudaMemcpyAsync(tmp_den, density, sizeof(float) * (size_t)m.ncell, cudaMemcpyHostToDevice, st));
+        d_den = tmp_den;
+        if (bfield && !m.scalar) {
+            CK(cudaMalloc(&tmp_b, sizeof(float) * 3 * (size_t)m.ncell));
+            CK(cudaMemcpyAsync(tmp_b, bfield, sizeof(float) * 3 * (size_t)m.ncell, cudaMemcpyHostToDevice, st));
+            d_b = tmp_b;
         }
     }
     int* d_bad = nullptr;
     CK(cudaMalloc(&d_bad, sizeof(int)));
     CK(cudaMemsetAsync(d_bad, 0, sizeof(int), st));
-    if (m.scalar) {
-        if (!g->d_kr) CK(cudaMalloc(&g->d_kr, sizeof(float) * (size_t)m.ncell));
-    } else {
-        CK(cudaMalloc(&g->d_cell, sizeof(float4) * (size_t)m.ncell));
-    }
+    if (m.scalar) CK(cudaMalloc(&g->d_kr, sizeof(float) * (size_t)g->npad));
+    else          CK(cudaMalloc(&g->d_cell, sizeof(float4) * (size_t)g->npad));
     {
         const int tb = 256;
-        const unsigned nb = (unsigned)((m.ncell + tb - 1) / tb);
-        krp_k_pack<<<nb, tb, 0, st>>>(d_den, d_b, m.ncell, g->d_cell, (m.scalar && d_den != g->d_kr) ? g->d_kr : nullptr, d_bad);
+        const unsigned nb = (unsigned)((g->npad + tb - 1) / tb);
+        krp_k_pack<<<nb, tb, 0, st>>>(m, d_den, m.scalar ? nullptr : d_b, g->npad, g->d_cell, g->d_kr, d_bad);
         CK(cudaGetLastError());
         g->launches++;
     }
@@ -238,6 +258,13 @@ extern "C" int krp_grid_create(krp_grid** out, int nx, int ny, int nz, const dou
     cudaFree(d_bad); cudaFree(tmp_den); cudaFree(tmp_b);
     if (bad) return fail(KRP_ERR_ARG, "density has %d negative, NaN or infinite cells", bad);
     m.kr = g->d_kr; m.cell = g->d_cell;
+    // bins of the imaging order: one cache line of cells per bin (32 x 4 B or 8 x 16 B), at most 2^22 bins
+    g->bin_shift = m.scalar ? 5 : 3;
+    while ((g->npad >> g->bin_shift) >= (1u << 22)) g->bin_shift++;
+    g->n_bins = (g->npad >> g->bin_shift) + 1;
+    CK(cudaMalloc(&g->d_bins, sizeof(unsigned int) * ((size_t)g->n_bins + 1)));
+    CK(cub::DeviceScan::ExclusiveSum(nullptr, g->scan_bytes, g->d_bins, g->d_bins, (int)(g->n_bins + 1), st));
+    CK(cudaMalloc(&g->d_scan, g->scan_bytes ? g->scan_bytes : 16));
 
     CK(cudaMalloc(&g->d_ctl, sizeof(KrpCtl)));
     CK(cudaMemsetAsync(g->d_ctl, 0, sizeof(KrpCtl), st));
@@ -277,7 +304,7 @@ extern "C" int krp_source_set(krp_grid* g, const krp_source* src, void* stream)
         idx[a] = i; m.src_p[a] = (float)p;
         m.src_n[a] = (float)src->dir[a];
     }
-    m.src_cell = (uint32_t)(((int64_t)idx[2] * m.ny + idx[1]) * m.nx + idx[0]);
+    m.src_cell = ((uint32_t)(idx[2] + 1) * (uint32_t)m.py + (uint32_t)(idx[1] + 1)) * (uint32_t)m.px + (uint32_t)(idx[0] + 1);
     cudaFree(g->d_src_cdf); g->d_src_cdf = nullptr; m.src_cdf = nullptr;
     if ((src->kind & 1) && src->cell_weight) {
         double* tmp = nullptr;
@@ -412,7 +439,7 @@ extern "C" int krp_image(krp_grid* g, const krp_observer* obs, int n_obs, int np
                 memcmp(g->obs_host.data(), obs, sizeof(krp_observer) * n_obs) == 0;
     if (!same) {
         CK(cudaStreamSynchronize(st));
-        cudaFree(g->d_img); cudaFree(g->d_obs); g->d_img = nullptr; g->d_obs = nullptr;
+        cudaFree(g->d_img); g->d_img = nullptr;
         size_t bytes = sizeof(double) * 4 * (size_t)n_obs * npix_x * npix_y;
         CK(cudaMalloc(&g->d_img, bytes));
         CK(cudaMemsetAsync(g->d_img, 0, bytes, st));
@@ -426,20 +453,46 @@ extern "C" int krp_image(krp_grid* g, const krp_observer* obs, int n_obs, int np
                 od[o].thd[a] = th[a]; od[o].phd[a] = ph[a]; od[o].center[a] = obs[o].center[a];
             }
             od[o].inv_hw = 1.0 / obs[o].half_w; od[o].inv_hh = 1.0 / obs[o].half_h;
+            const int strides[3] = { 1, g->m.px, (int)g->m.pxy };
+            for (int a = 0; a < 3; ++a) {
+                const float nf = od[o].n[a];
+                od[o].dt[a] = nf != 0.f ? g->m.d[a] / std::fabs(nf) : INFINITY;
+                od[o].stride[a] = nf > 0.f ? strides[a] : (nf < 0.f ? -strides[a] : 0);
+            }
         }
-        CK(cudaMalloc(&g->d_obs, sizeof(KrpObserverDev) * n_obs));
-        CK(cudaMemcpyAsync(g->d_obs, od.data(), sizeof(KrpObserverDev) * n_obs, cudaMemcpyHostToDevice, st));
-        CK(cudaStreamSynchronize(st));
+        g->obs_dev = od;
         g->obs_host.assign(obs, obs + n_obs);
         g->n_obs = n_obs; g->npx = npix_x; g->npy = npix_y;
     }
     if (g->ev_cap == 0) return KRP_OK;   // nothing was ever transported
+    if (g->ev_cap >= (1ull << 32)) return fail(KRP_ERR_ARG, "krp_image handles at most 2^32-1 buffered events per call");
+    if (g->perm_cap < g->ev_cap) {
+        CK(cudaStreamSynchronize(st));
+        cudaFree(g->d_perm); g->d_perm = nullptr; g->perm_cap = 0;
+        CK(cudaMalloc(&g->d_perm, sizeof(unsigned int) * g->ev_cap));
+        g->perm_cap = g->ev_cap;
+    }
+    // I0: order the events by cell bin (count, scan, scatter)
+    const unsigned pers = (unsigned)(g->n_sm * g->blocks_per_sm);
+    CK(cudaMemsetAsync(g->d_bins, 0, sizeof(unsigned int) * ((size_t)g->n_bins + 1), st));
+    krp_k_sort_count<<<pers, 256, 0, st>>>(g->d_ctl, g->ev, g->bin_shift, flags, g->d_bins);
+    CK(cub::DeviceScan::ExclusiveSum(g->d_scan, g->scan_bytes, g->d_bins, g->d_bins, (int)(g->n_bins + 1), st));
+    krp_k_image_prep<<<1, 1, 0, st>>>(g->d_ctl, g->d_bins, g->n_bins);
+    krp_k_sort_scatter<<<pers, 256, 0, st>>>(g->d_ctl, g->ev, g->bin_shift, flags, g->d_bins, g->d_perm);
+    g->launches += 5;   // count, scan (2 kernels), prep, scatter
+    // I1-I3: one launch per observer (its constants are kernel parameters); launches rotate over
+    // KRP_MAX_OBS_PACK work counters, rewound when the rotation wraps
     const int tb = g->image_block;
-    const unsigned grid = (unsigned)(g->n_sm * g->blocks_per_sm);
-    if (g->m.scalar) krp_k_image<true><<<grid, tb, 0, st>>>(g->m, g->d_ctl, g->ev, g->d_obs, n_obs, npix_x, npix_y, flags, g->d_img);
-    else             krp_k_image<false><<<grid, tb, 0, st>>>(g->m, g->d_ctl, g->ev, g->d_obs, n_obs, npix_x, npix_y, flags, g->d_img);
+    const size_t smem = g->m.scalar ? 0 : 2 * sizeof(float4) * (size_t)(g->m.n_inc - 1);
+    for (int o = 0; o < n_obs; ++o) {
+        const int slot = o % KRP_MAX_OBS_PACK;
+        if (o > 0 && slot == 0) { krp_k_image_rewind<<<1, 1, 0, st>>>(g->d_ctl); g->launches++; }
+        if (g->m.scalar) krp_k_image<true><<<pers, tb, smem, st>>>(g->m, g->d_ctl, g->ev, g->d_perm, g->obs_dev[o], slot, o, npix_x, npix_y, g->d_img);
+        else             krp_k_image<false><<<pers, tb, smem, st>>>(g->m, g->d_ctl, g->ev, g->d_perm, g->obs_dev[o], slot, o, npix_x, npix_y, g->d_img);
+        g->launches++;
+    }
     krp_k_events_clear<<<1, 1, 0, st>>>(g->d_ctl);
-    g->launches += 2;
+    g->launches++;
     CK(cudaGetLastError());
     return KRP_OK;
 }
@@ -515,7 +568,11 @@ extern "C" int krp_events_get(krp_grid* g, uint64_t cap, uint64_t* n, uint64_t* 
         memcpy(&cb, &pc[i].w, 4); memcpy(&kb, &nk[i].w, 4);
         if (id) id[i] = ids[i];
         if (k) k[i] = (int32_t)(kb & ~KRP_TERM_BIT);
-        if (cell) cell[i] = (int64_t)cb;
+        if (cell) {
+            const KrpModel& mm = g->m;
+            uint32_t t = cb / (uint32_t)mm.px, hx = cb - t * (uint32_t)mm.px, hz = t / (uint32_t)mm.py, hy = t - hz * (uint32_t)mm.py;
+            cell[i] = ((int64_t)(hz - 1) * mm.ny + (int64_t)(hy - 1)) * mm.nx + (int64_t)(hx - 1);
+        }
         if (pos) { pos[3 * i] = pc[i].x; pos[3 * i + 1] = pc[i].y; pos[3 * i + 2] = pc[i].z; }
         if (dir) { dir[3 * i] = nk[i].x; dir[3 * i + 1] = nk[i].y; dir[3 * i + 2] = nk[i].z; }
         if (stokes) {

@@ -13,6 +13,7 @@
 
 #define KRP_PI_D 3.14159265358979323846264338327950288
 #define KRP_TERM_BIT 0x80000000u
+#define KRP_MAX_OBS_PACK 8
 
 // ------------------------------------------------------------------------------------------
 // by-value kernel parameters
@@ -20,11 +21,18 @@
 struct KrpModel {
     int nx, ny, nz;
     uint32_t ncell;
+    // Padded layout: the cell arrays carry a one-cell halo on every side whose
+    // kappa*rho is -1, so that a ray leaves the grid exactly when it loads a negative kappa*rho.  Cell ids
+    // inside the library are indices into this padded array: ((iz+1)*py + iy+1)*px + ix+1.
+    int px, py;            // padded pitches: px = nx+2, py = ny+2
+    uint32_t pxy;          // px*py
     float d[3];            // cell size per axis
     double lo[3], dd[3];   // lower corner and cell size in fp64 (projection to the image)
-    const float* kr;       // SCALAR mode: kappa*rho per cell
-    const float4* cell;    // general mode: {kappa*rho, B^x, B^y, B^z}
+    const float* kr;       // SCALAR mode: kappa*rho per padded cell
+    const float4* cell;    // general mode: {kappa*rho, B^x, B^y, B^z} per padded cell
     const float4* opac;    // [n_inc] {alpha1, alpha2, alpha3, albedo} on mu_m = m/(n_inc-1)
+    const float4* opA;     // [n_inc-1] intercepts and
+    const float4* opB;     // [n_inc-1] slopes of the same table: value = opA[j] + opB[j]*x on x = mu*(n_inc-1) in [j, j+1]
     int n_inc;
     const float4* mueller; // [n_ang] {S11,S12,S33,S34}
     int n_ang;
@@ -37,10 +45,24 @@ struct KrpModel {
     // source
     int src_kind, emit_records;
     float src_n[3];
-    uint32_t src_cell;
+    uint32_t src_cell;     // padded id
     float src_p[3];
-    const double* src_cdf; // [ncell] running sum of cell weights or NULL
+    const double* src_cdf; // [ncell] running sum of cell weights (unpadded order) or NULL
 };
+
+__device__ __forceinline__ uint32_t krp_pad_id(const KrpModel& g, int ix, int iy, int iz)
+{
+    return ((uint32_t)(iz + 1) * (uint32_t)g.py + (uint32_t)(iy + 1)) * (uint32_t)g.px + (uint32_t)(ix + 1);
+}
+// padded coordinates (0..n+1 per axis) of a padded id
+__device__ __forceinline__ void krp_pad_coords(const KrpModel& g, uint32_t c, int& hx, int& hy, int& hz)
+{
+    uint32_t t = c / (uint32_t)g.px;
+    hx = (int)(c - t * (uint32_t)g.px);
+    uint32_t z = t / (uint32_t)g.py;
+    hy = (int)(t - z * (uint32_t)g.py);
+    hz = (int)z;
+}
 
 struct KrpStatsDev {
     unsigned long long packets, events, records, steps_transport, steps_image, contributions, dropped, overflow;
@@ -52,7 +74,9 @@ struct KrpCtl {
     unsigned long long ev_begin;   // first event of the current wave
     unsigned long long ev_cap;
     unsigned int q_count[2];       // fill of the two packet queues
-    unsigned int work[2];          // dynamic work counters (march / image)
+    unsigned int work[2];          // dynamic work counters of the flight kernels
+    unsigned int n_sorted;         // events in the sorted order of the current imaging pass
+    unsigned int img_work[KRP_MAX_OBS_PACK];   // per-observer warp-tile counters of the imaging pass
     KrpStatsDev stats;
 };
 
@@ -67,7 +91,13 @@ struct KrpRecords {
 
 struct KrpObserverDev {
     float n[3], th[3], ph[3];
+    float dt[3];                // path length between faces per axis, d/|n| (inf when n = 0)
+    int stride[3];              // signed stride in the padded array per axis (0 when n = 0)
     double thd[3], phd[3], center[3], inv_hw, inv_hh;
+};
+// observers of one imaging launch, passed by value (constant bank): blockIdx.y picks one
+struct KrpObsPack {
+    KrpObserverDev o[KRP_MAX_OBS_PACK];
 };
 
 // ------------------------------------------------------------------------------------------
@@ -112,89 +142,120 @@ __device__ __forceinline__ void krp_basis(const T n[3], T th[3], T ph[3])
 }
 
 // ------------------------------------------------------------------------------------------
-// A11  cell-interface-to-interface march, R11b.  The ray keeps, per axis, the
-// distance still to go to the next face (re-based every step, so its rounding error is that
-// of a cell-local coordinate), the face-to-face distance, the linear-index stride and the
-// number of cells left before the grid edge.
+// A11  cell-interface-to-interface march, R11b, in two forms.
+//
+// KrpRay (flights): per axis the distance still to go to the next face, re-based every step, so
+// its rounding error is that of a cell-local coordinate whatever the length of the flight (what
+// decides the event cell has to stay within ~1e-7 of a cell).
+//
+// KrpRayA (imaging): per axis the absolute path length at the next face; one subtraction gives the
+// segment, one predicated add advances the axis crossed.
+//
+// Both walk the padded array: the ray has left the grid when the cell it loads has kappa*rho < 0.
+// Ties: x before y before z.
 // ------------------------------------------------------------------------------------------
+#define KRP_INF_F __int_as_float(0x7f800000)
+
 struct KrpRay {
     float rx, ry, rz;   // distance to the next x/y/z face
     float tx, ty, tz;   // d/|n| per axis (inf when n = 0)
-    int sx, sy, sz;     // signed linear-index stride
-    int lx, ly, lz;     // cells left along the axis before leaving the grid
-    uint32_t c;         // linear cell index
+    int sx, sy, sz;     // signed stride in the padded array
+    uint32_t c;         // padded cell id
 };
 
-__device__ __forceinline__ void krp_ray_axis(float n, float p, float d, int stride, int i, int N,
-                                             float& r, float& t, int& s, int& l)
+__device__ __forceinline__ void krp_ray_axis(float n, float p, float d, int stride, float& r, float& t, int& s)
 {
-    if (n > 0.f)      { t = d / n;  r = (1.f - p) * t; s = stride;  l = N - 1 - i; }
-    else if (n < 0.f) { t = d / -n; r = p * t;         s = -stride; l = i; }
-    else              { t = __int_as_float(0x7f800000); r = t; s = 0; l = 0x7fffffff; }
+    if (n > 0.f)      { t = d / n;  r = (1.f - p) * t; s = stride; }
+    else if (n < 0.f) { t = d / -n; r = p * t;         s = -stride; }
+    else              { t = KRP_INF_F; r = t; s = 0; }
 }
 
 __device__ __forceinline__ void krp_ray_init(const KrpModel& g, uint32_t cell, const float p[3], const float n[3], KrpRay& r)
 {
-    int ix = (int)(cell % (uint32_t)g.nx);
-    uint32_t t = cell / (uint32_t)g.nx;
-    int iy = (int)(t % (uint32_t)g.ny), iz = (int)(t / (uint32_t)g.ny);
-    krp_ray_axis(n[0], p[0], g.d[0], 1, ix, g.nx, r.rx, r.tx, r.sx, r.lx);
-    krp_ray_axis(n[1], p[1], g.d[1], g.nx, iy, g.ny, r.ry, r.ty, r.sy, r.ly);
-    krp_ray_axis(n[2], p[2], g.d[2], g.nx * g.ny, iz, g.nz, r.rz, r.tz, r.sz, r.lz);
+    krp_ray_axis(n[0], p[0], g.d[0], 1, r.rx, r.tx, r.sx);
+    krp_ray_axis(n[1], p[1], g.d[1], g.px, r.ry, r.ty, r.sy);
+    krp_ray_axis(n[2], p[2], g.d[2], (int)g.pxy, r.rz, r.tz, r.sz);
     r.c = cell;
 }
 
-// length of the segment inside the current cell; ties x before y before z (R11b)
+// length of the segment inside the current cell
 __device__ __forceinline__ float krp_ray_ds(const KrpRay& r) { return fminf(r.rx, fminf(r.ry, r.rz)); }
 
-// cross the exit face; returns false when the ray leaves the grid
-__device__ __forceinline__ bool krp_ray_step(KrpRay& r, float ds)
+// cross the exit face (the caller detects the grid edge from the next cell's kappa*rho)
+__device__ __forceinline__ void krp_ray_step(KrpRay& r, float ds)
 {
-    bool ax = (r.rx <= r.ry) & (r.rx <= r.rz);
-    bool ay = (!ax) & (r.ry <= r.rz);
-    bool az = !(ax | ay);
-    r.rx = ax ? r.tx : r.rx - ds;
-    r.ry = ay ? r.ty : r.ry - ds;
-    r.rz = az ? r.tz : r.rz - ds;
-    int s = ax ? r.sx : (ay ? r.sy : r.sz);
-    r.c += (uint32_t)s;
-    r.lx -= ax; r.ly -= ay; r.lz -= az;
-    return (r.lx | r.ly | r.lz) >= 0;
+    const bool ax = (r.rx <= r.ry) & (r.rx <= r.rz);
+    const bool ay = (!ax) & (r.ry <= r.rz);
+    r.rx -= ds; r.ry -= ds; r.rz -= ds;
+    if (ax)      { r.rx = r.tx; r.c += (uint32_t)r.sx; }
+    else if (ay) { r.ry = r.ty; r.c += (uint32_t)r.sy; }
+    else         { r.rz = r.tz; r.c += (uint32_t)r.sz; }
 }
 
-// The same march with the distances in fp64: used by the general-mode flight, where the optical
-// depth consumed in every cell decides the integer outcome "which cell holds the event" and has to
-// be taken in the oracle's precision.
+// cell-local coordinate after moving `moved` from the point where the distances r were taken (fp32; statistics only)
+__device__ __forceinline__ float krp_local(float n, float r, float t, float moved, float p0)
+{
+    if (n == 0.f) return p0;
+    float f = (r - moved) / t;
+    f = fminf(fmaxf(f, 0.f), 1.f);
+    return n > 0.f ? 1.f - f : f;
+}
+
+// Event position in fp64 without accumulated rounding: the flight started at
+// cell-local p0 (fp32 state, R12) of padded cell c0 and has its event in padded cell c, `t_len` beyond the
+// point where it entered c.  The entry path length is the largest of the per-axis path lengths to the entry
+// planes of c (slab form of the same march), each a single fp64 expression; the result is rounded to fp32 the
+// way the state is defined.
+__device__ __forceinline__ void krp_event_pos(const KrpModel& g, const float n[3], const float p0[3], uint32_t c0,
+                                              uint32_t c, double t_len, float pe[3])
+{
+    int h0[3], h[3];
+    krp_pad_coords(g, c0, h0[0], h0[1], h0[2]);
+    krp_pad_coords(g, c, h[0], h[1], h[2]);
+    double s_in = 0.0;
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        if (h[a] != h0[a]) {
+            const double plane = (double)(h[a] - h0[a]) + (n[a] > 0.f ? 0.0 : 1.0);
+            s_in = fmax(s_in, (plane - (double)p0[a]) * g.dd[a] / (double)n[a]);
+        }
+    }
+    const double s = s_in + t_len;
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        double x = (double)p0[a] + (double)n[a] * s / g.dd[a] - (double)(h[a] - h0[a]);
+        pe[a] = (float)fmin(fmax(x, 0.0), 1.0);
+    }
+}
+
+// The same re-based march with the distances in fp64: used by the general-mode flight, where the optical
+// depth consumed in every cell decides the integer outcome "which cell holds the event" and has to be taken
+// in the oracle's precision.
 struct KrpRayD {
     double rx, ry, rz;
     double tx, ty, tz;
     int sx, sy, sz;
-    int lx, ly, lz;
     uint32_t c;
 };
 
-__device__ __forceinline__ void krp_rayd_axis(float n, float p, double d, int stride, int i, int N,
-                                              double& r, double& t, int& s, int& l)
+__device__ __forceinline__ void krp_rayd_axis(float n, float p, double d, int stride, double& r, double& t, int& s)
 {
-    if (n > 0.f)      { r = (1.0 - (double)p) * d / (double)n; t = d / (double)n;  s = stride;  l = N - 1 - i; }
-    else if (n < 0.f) { r = (double)p * d / -(double)n;        t = d / -(double)n; s = -stride; l = i; }
-    else              { t = __longlong_as_double(0x7ff0000000000000ll); r = t; s = 0; l = 0x7fffffff; }
+    if (n > 0.f)      { r = (1.0 - (double)p) * d / (double)n; t = d / (double)n;  s = stride; }
+    else if (n < 0.f) { r = (double)p * d / -(double)n;        t = d / -(double)n; s = -stride; }
+    else              { t = __longlong_as_double(0x7ff0000000000000ll); r = t; s = 0; }
 }
 
 __device__ __forceinline__ void krp_rayd_init(const KrpModel& g, uint32_t cell, const float p[3], const float n[3], KrpRayD& r)
 {
-    int ix = (int)(cell % (uint32_t)g.nx);
-    uint32_t t = cell / (uint32_t)g.nx;
-    int iy = (int)(t % (uint32_t)g.ny), iz = (int)(t / (uint32_t)g.ny);
-    krp_rayd_axis(n[0], p[0], g.dd[0], 1, ix, g.nx, r.rx, r.tx, r.sx, r.lx);
-    krp_rayd_axis(n[1], p[1], g.dd[1], g.nx, iy, g.ny, r.ry, r.ty, r.sy, r.ly);
-    krp_rayd_axis(n[2], p[2], g.dd[2], g.nx * g.ny, iz, g.nz, r.rz, r.tz, r.sz, r.lz);
+    krp_rayd_axis(n[0], p[0], g.dd[0], 1, r.rx, r.tx, r.sx);
+    krp_rayd_axis(n[1], p[1], g.dd[1], g.px, r.ry, r.ty, r.sy);
+    krp_rayd_axis(n[2], p[2], g.dd[2], (int)g.pxy, r.rz, r.tz, r.sz);
     r.c = cell;
 }
 
 __device__ __forceinline__ double krp_rayd_ds(const KrpRayD& r) { return fmin(r.rx, fmin(r.ry, r.rz)); }
 
-__device__ __forceinline__ bool krp_rayd_step(KrpRayD& r, double ds)
+__device__ __forceinline__ void krp_rayd_step(KrpRayD& r, double ds)
 {
     bool ax = (r.rx <= r.ry) & (r.rx <= r.rz);
     bool ay = (!ax) & (r.ry <= r.rz);
@@ -204,8 +265,6 @@ __device__ __forceinline__ bool krp_rayd_step(KrpRayD& r, double ds)
     r.rz = az ? r.tz : r.rz - ds;
     int s = ax ? r.sx : (ay ? r.sy : r.sz);
     r.c += (uint32_t)s;
-    r.lx -= ax; r.ly -= ay; r.lz -= az;
-    return (r.lx | r.ly | r.lz) >= 0;
 }
 
 // cell-local position (fp64 distances) after moving `moved` from the point where r was taken
@@ -217,14 +276,11 @@ __device__ __forceinline__ float krp_locald(float n, double r, double t, double 
     return (float)(n > 0.f ? 1.0 - f : f);
 }
 
-// cell-local position after moving `moved` from the point where the distances r were taken
-__device__ __forceinline__ float krp_local(float n, float r, float t, float moved, float p0)
-{
-    if (n == 0.f) return p0;
-    float f = (r - moved) / t;
-    f = fminf(fmaxf(f, 0.f), 1.f);
-    return n > 0.f ? 1.f - f : f;
-}
+struct KrpRayA {
+    float t;            // path length at the entry of the current cell
+    float tx, ty, tz;   // path length at the next x/y/z face
+    uint32_t c;         // padded cell id
+};
 
 // ------------------------------------------------------------------------------------------
 // D4  table look-ups, linear in the node variable (R13)

@@ -7,6 +7,10 @@
 #pragma once
 #include "krp_device.cuh"
 
+#ifndef KRP_IMAGE_MIN_BLOCKS
+#define KRP_IMAGE_MIN_BLOCKS 6
+#endif
+
 // ------------------------------------------------------------------------------------------
 // T1/T2  emission: draws of block 0 = (cos theta, phi, tau*, spare); blocks 1-2
 // place a volume-source packet (R11, R17).  One thread per packet.
@@ -46,6 +50,12 @@ __global__ void __launch_bounds__(256) krp_k_emit(KrpModel g, KrpCtl* ctl, KrpRe
         } else {
             double c = floor(u * (double)g.ncell);
             cell = (uint32_t)fmin(c, (double)(g.ncell - 1));
+        }
+        {   // linear (x fastest) -> padded id
+            const uint32_t t = cell / (uint32_t)g.nx;
+            const int ix = (int)(cell - t * (uint32_t)g.nx);
+            const uint32_t iz = t / (uint32_t)g.ny;
+            cell = krp_pad_id(g, ix, (int)(t - iz * (uint32_t)g.ny), (int)iz);
         }
         p[0] = (float)krp_u01(w2.x); p[1] = (float)krp_u01(w2.y); p[2] = (float)krp_u01(w2.z);
     } else {
@@ -123,31 +133,32 @@ __global__ void __launch_bounds__(256) krp_k_flight_scalar(KrpModel g, KrpCtl* c
         const float n[3] = { nk.x, nk.y, nk.z };
         const float p0[3] = { pc.x, pc.y, pc.z };
         const uint32_t k = __float_as_uint(nk.w);
+        const uint32_t c0 = __float_as_uint(pc.w);
         KrpRay ray;
-        krp_ray_init(g, __float_as_uint(pc.w), p0, n, ray);
+        krp_ray_init(g, c0, p0, n, ray);
         double D = q.tau[item];
         bool hit = false;
-        float moved = 0.f, ds = 0.f;
+        double moved = 0.0;
+        float kr = __ldg(g.kr + ray.c);
         for (;;) {
-            ds = krp_ray_ds(ray);
+            const float ds = krp_ray_ds(ray);
             ++steps;
-            const float kr = __ldg(g.kr + ray.c);
             const float dt1 = g.a1c * kr * ds;
             if ((double)dt1 >= D) {              // event inside this cell
-                moved = (float)D / (g.a1c * kr);
+                moved = D / ((double)g.a1c * (double)kr);
                 hit = true;
                 break;
             }
             D -= (double)dt1;
-            if (!krp_ray_step(ray, ds)) break;
+            krp_ray_step(ray, ds);
+            kr = __ldg(g.kr + ray.c);
+            if (kr < 0.f) break;                 // halo: the packet left the grid
         }
         const float W = S0.x;
         if (!hit) { w_esc += (double)W; continue; }
         // T5: event record, albedo weighting, termination (R12)
         float pe[3];
-        pe[0] = krp_local(n[0], ray.rx, ray.tx, moved, p0[0]);
-        pe[1] = krp_local(n[1], ray.ry, ray.ty, moved, p0[1]);
-        pe[2] = krp_local(n[2], ray.rz, ray.tz, moved, p0[2]);
+        krp_event_pos(g, n, p0, c0, ray.c, moved, pe);
         const float Wn = g.omc * W;
         const uint32_t kn = k + 1u;
         const bool term = (Wn < g.w_min) || ((int)kn >= g.max_scatter);
@@ -229,6 +240,7 @@ __global__ void __launch_bounds__(256) krp_k_flight_general(KrpModel g, KrpCtl* 
         const double tau0 = q.tau[item];
         KrpRayD ray;
         krp_rayd_init(g, __float_as_uint(pc.w), p0, n, ray);
+        float4 cl = __ldg(g.cell + ray.c);
         float th[3], ph[3];
         krp_basis<float>(n, th, ph);
         const double nd[3] = { n[0], n[1], n[2] };
@@ -243,7 +255,6 @@ __global__ void __launch_bounds__(256) krp_k_flight_general(KrpModel g, KrpCtl* 
         for (;;) {
             const double ds = krp_rayd_ds(ray);
             ++steps;
-            const float4 cl = __ldg(g.cell + ray.c);
             const float kr = cl.x;
             if (kr > 0.f) {
                 const double bx = cl.y, by = cl.z, bz = cl.w;
@@ -327,7 +338,9 @@ __global__ void __launch_bounds__(256) krp_k_flight_general(KrpModel g, KrpCtl* 
                     i = i_new; D = Dn;
                 }
             }
-            if (!krp_rayd_step(ray, ds)) break;
+            krp_rayd_step(ray, ds);
+            cl = __ldg(g.cell + ray.c);
+            if (cl.x < 0.f) break;               // halo: the packet left the grid
         }
         const float W = S0.x;
         if (!hit) { w_esc += (double)W; continue; }
@@ -410,7 +423,7 @@ __global__ void __launch_bounds__(128) krp_k_scatter(KrpModel g, KrpCtl* ctl, Kr
         const unsigned long long id = ev.id[e];
         const uint32_t cell = __float_as_uint(pc.w);
         double b[3] = { 0.0, 0.0, 1.0 };
-        if (!g.scalar) { float4 cl = g.cell[cell]; b[0] = cl.y; b[1] = cl.z; b[2] = cl.w; }
+        if (!g.scalar) { float4 cl = g.cell[cell]; b[0] = cl.y; b[1] = cl.z; b[2] = cl.w; }   // cell is a padded id
         const double n[3] = { nk.x, nk.y, nk.z };
         // A2: q_B from the direction angles of B (eq. 2)
         double qB[4];
@@ -552,95 +565,261 @@ __device__ __forceinline__ void krp_peel(const KrpModel& g, const float n[3], fl
 }
 
 // ------------------------------------------------------------------------------------------
-// I1-I3  imaging: one item per (observer, event).  Peel-off, attenuation march to the grid
-// edge with the same in-cell solution and no survival test, orthographic
-// projection, fp64 atomic accumulation into img[obs][4][npy][npx] (R14).
+// I0  ordering of the event buffer for imaging: a counting sort of the event
+// indices by bin = padded cell id >> shift, entirely on the device (the event count never visits the
+// host).  Rays of one observer are parallel, so the 32 rays of a warp that start in neighbouring cells
+// walk through neighbouring cells for their whole length: their gathers share cache lines and they
+// leave the grid after nearly the same number of steps.
+//   krp_k_sort_count    histogram of the bins
+//   (exclusive scan of the histogram: cub::DeviceScan, in krp_api.cu)
+//   krp_k_sort_scatter  perm[slot] = event index, slot reserved in the event's bin
 // ------------------------------------------------------------------------------------------
-template <bool SCALAR>
-__global__ void __launch_bounds__(256) krp_k_image(KrpModel g, KrpCtl* ctl, KrpRecords ev, const KrpObserverDev* __restrict__ obs,
-                                                   int n_obs, int npx, int npy, int flags, double* __restrict__ img)
+__global__ void __launch_bounds__(256) krp_k_sort_count(KrpCtl* ctl, KrpRecords ev, int shift, int flags,
+                                                        unsigned int* __restrict__ bins)
 {
     unsigned long long n_ev = ctl->n_events;
     if (n_ev > ctl->ev_cap) n_ev = ctl->ev_cap;
-    const unsigned long long total = n_ev * (unsigned long long)n_obs;
-    unsigned long long steps = 0, n_con = 0, n_drop = 0;
-    for (unsigned long long item = blockIdx.x * (unsigned long long)blockDim.x + threadIdx.x; item < total;
-         item += (unsigned long long)gridDim.x * blockDim.x) {
-        const int o = (int)(item / n_ev);
-        const unsigned long long e = item - (unsigned long long)o * n_ev;
-        const float4 nk = ev.nk[e];
-        const uint32_t k = __float_as_uint(nk.w) & ~KRP_TERM_BIT;
+    for (unsigned long long e = blockIdx.x * (unsigned long long)blockDim.x + threadIdx.x; e < n_ev;
+         e += (unsigned long long)gridDim.x * blockDim.x) {
+        const uint32_t k = __float_as_uint(ev.nk[e].w) & ~KRP_TERM_BIT;
+        if (k == 0u && !(flags & 1)) continue;             // emission records take part only with direct light
+        atomicAdd(bins + (__float_as_uint(ev.pc[e].w) >> shift), 1u);
+    }
+}
+
+// after the scan `bins` holds the first slot of every bin; the last thread publishes the total
+__global__ void __launch_bounds__(256) krp_k_sort_scatter(KrpCtl* ctl, KrpRecords ev, int shift, int flags,
+                                                          unsigned int* __restrict__ bins, unsigned int* __restrict__ perm)
+{
+    unsigned long long n_ev = ctl->n_events;
+    if (n_ev > ctl->ev_cap) n_ev = ctl->ev_cap;
+    for (unsigned long long e = blockIdx.x * (unsigned long long)blockDim.x + threadIdx.x; e < n_ev;
+         e += (unsigned long long)gridDim.x * blockDim.x) {
+        const uint32_t k = __float_as_uint(ev.nk[e].w) & ~KRP_TERM_BIT;
         if (k == 0u && !(flags & 1)) continue;
-        const float4 pc = ev.pc[e], Se = ev.S[e];
-        const KrpObserverDev& ob = obs[o];
-        float S[4];
-        if (k == 0u) { S[0] = Se.x * 0.07957747154594767f; S[1] = S[2] = S[3] = 0.f; }
-        else { const float n[3] = { nk.x, nk.y, nk.z }; krp_peel(g, n, Se, ob, S); }
-        const float p0[3] = { pc.x, pc.y, pc.z };
-        KrpRay ray;
-        krp_ray_init(g, __float_as_uint(pc.w), p0, ob.n, ray);
-        float A = 0.f;
-        if (SCALAR) {
-            float tau = 0.f;
-            for (;;) {
-                float ds = krp_ray_ds(ray);
-                ++steps;
-                tau = fmaf(__ldg(g.kr + ray.c), ds, tau);
-                if (!krp_ray_step(ray, ds)) break;
-            }
-            A = g.a1c * tau;
-        } else {
-            float i = S[0], qs = S[1], us = S[2], vs = S[3];
-            for (;;) {
-                float ds = krp_ray_ds(ray);
-                ++steps;
-                float4 cl = __ldg(g.cell + ray.c);
-                float kr = cl.x;
-                if (kr > 0.f) {
-                    float mu = ob.n[0] * cl.y + ob.n[1] * cl.z + ob.n[2] * cl.w;
-                    float4 op = krp_opac_at(g.opac, g.n_inc, fabsf(mu));
-                    float dtau = kr * ds;
-                    if (op.y == 0.f && op.z == 0.f) {
-                        A += op.x * dtau;
-                    } else {
-                        float a = ob.th[0] * cl.y + ob.th[1] * cl.z + ob.th[2] * cl.w;
-                        float b = ob.ph[0] * cl.y + ob.ph[1] * cl.z + ob.ph[2] * cl.w;
-                        float c2, s2;
-                        krp_eta2<float>(a, b, c2, s2);
-                        float qg = c2 * qs + s2 * us, ug = -s2 * qs + c2 * us, vg = vs;
-                        float di, i_new, depth;
-                        krp_appA(i, qg, ug, vg, op, dtau, di, i_new, depth);
-                        i = i_new; A += depth;
-                        qs = c2 * qg - s2 * ug; us = s2 * qg + c2 * ug; vs = vg;
+        const unsigned int slot = atomicAdd(bins + (__float_as_uint(ev.pc[e].w) >> shift), 1u);
+        perm[slot] = (unsigned int)e;
+    }
+}
+
+// one thread: open an imaging pass.  n_sorted = events that take part = last bin's end after the scatter,
+// which the host cannot know; it is read from the scanned histogram's sentinel entry (bins[n_bins] = total).
+__global__ void krp_k_image_prep(KrpCtl* ctl, const unsigned int* __restrict__ bins, unsigned int n_bins)
+{
+    ctl->n_sorted = bins[n_bins];
+    for (int o = 0; o < KRP_MAX_OBS_PACK; ++o) ctl->img_work[o] = 0;
+}
+__global__ void krp_k_image_rewind(KrpCtl* ctl)
+{
+    for (int o = 0; o < KRP_MAX_OBS_PACK; ++o) ctl->img_work[o] = 0;
+}
+
+// ------------------------------------------------------------------------------------------
+// I1-I3  imaging.  One launch per observer, whose constants (direction, bases, per-axis face spacing
+// and stride) are kernel parameters, i.e. constant-bank operands of the march; a warp repeatedly takes
+// the next 32 events of the sorted order from the launch's counter.  Per ray: peel-off, attenuation march to the grid edge with the same in-cell solution and
+// no survival test, orthographic projection, fp64 accumulation into
+// img[obs][4][npy][npx] (R14) with one atomic per distinct pixel of the warp.
+//
+// The march carries the absolute path length at the next face of each axis (KrpRayA): per step one
+// min3, one subtraction, one 4- or 16-byte gather, the in-cell update, one predicated add per axis.
+// The Stokes vector is e^{-A}(i,q,u,v); thin cells (|alpha2 dtau|, |alpha3 dtau| < 0.1) take the
+// series of sinh, cosh-1, sin, cos-1 in "delta form"  S += R(-eta) dP R(eta) S, which needs no
+// special case where n is parallel to B (the rotation is undefined there and dP vanishes).
+// ------------------------------------------------------------------------------------------
+__device__ __forceinline__ void krp_appA_delta_thin(float x, float y, float i, float qg, float ug, float v,
+                                                    float& di, float& dqg, float& dug, float& dv)
+{
+    const float x2 = x * x, y2 = y * y;
+    const float sh = fmaf(x * x2, 1.f / 6.f, x);                   // sinh x,     |x| < 0.1: rel. error < 1e-6
+    const float chm1 = x2 * fmaf(x2, 1.f / 24.f, 0.5f);            // cosh x - 1
+    const float sy = fmaf(y * y2, -1.f / 6.f, y);                  // sin y
+    const float cym1 = y2 * fmaf(y2, 1.f / 24.f, -0.5f);           // cos y - 1
+    di = i * chm1 - qg * sh;
+    dqg = qg * chm1 - i * sh;
+    dug = ug * cym1 - v * sy;
+    dv = ug * sy + v * cym1;
+}
+
+// one step of the absolute-path-length march: returns the length of the segment in the current cell and moves
+// to the next one (ties: x before y before z).  dt and stride are launch constants (constant-bank operands).
+struct KrpRayAConst { float dtx, dty, dtz; int sx, sy, sz; float n[3], th[3], ph[3]; float xs; int nseg; };
+// The launch constants of the march, held in registers for the whole kernel: they are read back from shared
+// memory through volatile loads, which ptxas (unlike a kernel parameter) will not re-load inside the loop.
+__device__ __forceinline__ KrpRayAConst krp_raya_const(const KrpObserverDev& ob, int nseg, KrpRayAConst* sh)
+{
+    if (threadIdx.x == 0) {
+        sh->dtx = ob.dt[0]; sh->dty = ob.dt[1]; sh->dtz = ob.dt[2];
+        sh->sx = ob.stride[0]; sh->sy = ob.stride[1]; sh->sz = ob.stride[2];
+        for (int a = 0; a < 3; ++a) { sh->n[a] = ob.n[a]; sh->th[a] = ob.th[a]; sh->ph[a] = ob.ph[a]; }
+        sh->nseg = nseg; sh->xs = (float)nseg;
+    }
+    __syncthreads();
+    volatile KrpRayAConst* v = sh;
+    KrpRayAConst k;
+    k.dtx = v->dtx; k.dty = v->dty; k.dtz = v->dtz; k.sx = v->sx; k.sy = v->sy; k.sz = v->sz;
+    for (int a = 0; a < 3; ++a) { k.n[a] = v->n[a]; k.th[a] = v->th[a]; k.ph[a] = v->ph[a]; }
+    k.xs = v->xs; k.nseg = v->nseg;
+    return k;
+}
+// One step: min3 (FMNMX3), one subtraction, three compares, one predicated FADD + IADD per axis.
+// Returns the segment length in the current cell; t_next is the path length at its exit face.
+__device__ __forceinline__ float krp_raya_step(KrpRayA& r, const KrpRayAConst& k)
+{
+    float ds, tn;
+    asm("{\n\t.reg .pred px, py, pz;\n\t"
+        "min.f32 %1, %2, %3, %4;\n\t"
+        "sub.f32 %0, %1, %6;\n\t"
+        "setp.le.f32 px, %2, %1;\n\t"
+        "setp.le.and.f32 py, %3, %1, !px;\n\t"
+        "setp.gt.and.f32 pz, %3, %1, !px;\n\t"
+        "@px add.f32 %2, %2, %7;\n\t@px add.s32 %5, %5, %10;\n\t"
+        "@py add.f32 %3, %3, %8;\n\t@py add.s32 %5, %5, %11;\n\t"
+        "@pz add.f32 %4, %4, %9;\n\t@pz add.s32 %5, %5, %12;\n\t}"
+        : "=f"(ds), "=&f"(tn), "+f"(r.tx), "+f"(r.ty), "+f"(r.tz), "+r"(r.c)
+        : "f"(r.t), "f"(k.dtx), "f"(k.dty), "f"(k.dtz), "r"(k.sx), "r"(k.sy), "r"(k.sz));
+    r.t = tn;
+    return ds;
+}
+
+template <bool SCALAR>
+__global__ void __launch_bounds__(256, KRP_IMAGE_MIN_BLOCKS) krp_k_image(KrpModel g, KrpCtl* ctl, KrpRecords ev,
+                                                   const unsigned int* __restrict__ perm, const KrpObserverDev ob,
+                                                   int slot, int obs_index, int npx, int npy, double* __restrict__ img)
+{
+    extern __shared__ float4 s_tab[];                // [2*(n_inc-1)]: intercepts, slopes of the opacity table
+    const int nseg = g.n_inc - 1;
+    if (!SCALAR) {
+        for (int j = threadIdx.x; j < nseg; j += blockDim.x) { s_tab[j] = g.opA[j]; s_tab[nseg + j] = g.opB[j]; }
+        __syncthreads();
+    }
+    const unsigned int n_ev = ctl->n_sorted;
+    const int lane = threadIdx.x & 31;
+    __shared__ KrpRayAConst s_rc;
+    const KrpRayAConst rc = krp_raya_const(ob, nseg, &s_rc);
+    unsigned long long steps = 0, n_con = 0, n_drop = 0;
+    for (;;) {
+        unsigned int base = 0;
+        if (lane == 0) base = atomicAdd(&ctl->img_work[slot], 32u);
+        base = __shfl_sync(0xffffffffu, base, 0);
+        if (base >= n_ev) break;
+        const bool live = base + lane < n_ev;
+        int pixel = -1;
+        float out[4] = { 0.f, 0.f, 0.f, 0.f };
+        if (live) {
+            const unsigned int e = perm[base + lane];
+            const float4 nk = ev.nk[e], pc = ev.pc[e], Se = ev.S[e];
+            const uint32_t k = __float_as_uint(nk.w) & ~KRP_TERM_BIT;
+            float S[4];
+            if (k == 0u) { S[0] = Se.x * 0.07957747154594767f; S[1] = S[2] = S[3] = 0.f; }
+            else { const float n[3] = { nk.x, nk.y, nk.z }; krp_peel(g, n, Se, ob, S); }
+            // ray set-up
+            const uint32_t c0 = __float_as_uint(pc.w);
+            KrpRayA r;
+            r.t = 0.f; r.c = c0;
+            r.tx = ob.n[0] > 0.f ? (1.f - pc.x) * ob.dt[0] : (ob.n[0] < 0.f ? pc.x * ob.dt[0] : KRP_INF_F);
+            r.ty = ob.n[1] > 0.f ? (1.f - pc.y) * ob.dt[1] : (ob.n[1] < 0.f ? pc.y * ob.dt[1] : KRP_INF_F);
+            r.tz = ob.n[2] > 0.f ? (1.f - pc.z) * ob.dt[2] : (ob.n[2] < 0.f ? pc.z * ob.dt[2] : KRP_INF_F);
+            float A = 0.f;
+            if (SCALAR) {
+                float tau = 0.f;
+                float kr = __ldg(g.kr + r.c);
+#pragma unroll 2
+                do {
+                    const float ds = krp_raya_step(r, rc);
+                    tau = fmaf(kr, ds, tau);
+                    kr = __ldg(g.kr + r.c);
+                } while (kr >= 0.f);
+                A = g.a1c * tau;
+            } else {
+                float i = S[0], qs = S[1], us = S[2], vs = S[3];
+                float4 cl = __ldg(g.cell + r.c);
+                do {
+                    const float ds = krp_raya_step(r, rc);
+                    const float4 cn = __ldg(g.cell + r.c);      // next cell, in flight during the update below
+                    if (cl.x > 0.f) {
+                        const float mu = fminf(fabsf(rc.n[0] * cl.y + rc.n[1] * cl.z + rc.n[2] * cl.w), 1.f);
+                        const float x = mu * rc.xs;
+                        const int j = min((int)x, rc.nseg - 1);
+                        const float4 ta = s_tab[j], tb = s_tab[rc.nseg + j];
+                        const float dtau = cl.x * ds;
+                        const float a1 = fmaf(tb.x, x, ta.x), a2 = fmaf(tb.y, x, ta.y), a3 = fmaf(tb.z, x, ta.z);
+                        const float xx = a2 * dtau, yy = a3 * dtau;
+                        const float a = rc.th[0] * cl.y + rc.th[1] * cl.z + rc.th[2] * cl.w;
+                        const float b = rc.ph[0] * cl.y + rc.ph[1] * cl.z + rc.ph[2] * cl.w;
+                        const float aa = a * a, bb = b * b;
+                        const float inv = __fdividef(1.f, fmaxf(aa + bb, 1e-30f));
+                        const float c2 = (aa - bb) * inv, s2 = 2.f * a * b * inv;     // cos 2eta, sin 2eta (R2)
+                        const float qg = c2 * qs + s2 * us, ug = c2 * us - s2 * qs;   // eq. 7
+                        if (fmaxf(fabsf(xx), fabsf(yy)) < 0.1f) {
+                            float di, dqg, dug, dv;
+                            krp_appA_delta_thin(xx, yy, i, qg, ug, vs, di, dqg, dug, dv);
+                            i += di; vs += dv;
+                            qs += c2 * dqg - s2 * dug;
+                            us += s2 * dqg + c2 * dug;
+                            A = fmaf(a1, dtau, A);
+                        } else {
+                            // thick cell (rare outside C3): full in-cell solution; where n is parallel to B the
+                            // rotation is undefined and, alpha2 = alpha3 = 0 there in any physical table, irrelevant
+                            const bool pole = aa + bb < 1e-24f;
+                            const float c2t = pole ? 1.f : c2, s2t = pole ? 0.f : s2;
+                            float qg2 = c2t * qs + s2t * us, ug2 = c2t * us - s2t * qs, vg2 = vs, di, i_new, depth;
+                            krp_appA(i, qg2, ug2, vg2, make_float4(a1, a2, a3, 0.f), dtau, di, i_new, depth);
+                            i = i_new; A += depth; vs = vg2;
+                            qs = c2t * qg2 - s2t * ug2; us = s2t * qg2 + c2t * ug2;
+                            if (A > 104.f) { cl = cn; break; }      // e^{-A} is exactly 0 in fp32 from here on
+                        }
                     }
-                }
-                if (!krp_ray_step(ray, ds)) break;
+                    cl = cn;
+                } while (cl.x >= 0.f);
+                S[0] = i; S[1] = qs; S[2] = us; S[3] = vs;
             }
-            S[0] = i; S[1] = qs; S[2] = us; S[3] = vs;
+            const float att = expf(-A);
+            // steps taken = face crossings on the way from c0 to the last cell loaded
+            int h0[3], h1[3];
+            krp_pad_coords(g, c0, h0[0], h0[1], h0[2]);
+            krp_pad_coords(g, r.c, h1[0], h1[1], h1[2]);
+            steps += (unsigned long long)(abs(h1[0] - h0[0]) + abs(h1[1] - h0[1]) + abs(h1[2] - h0[2]));
+            // I3: orthographic projection of the event position (fp64, once per ray)
+            const double x[3] = { g.lo[0] + ((double)(h0[0] - 1) + (double)pc.x) * g.dd[0] - ob.center[0],
+                                  g.lo[1] + ((double)(h0[1] - 1) + (double)pc.y) * g.dd[1] - ob.center[1],
+                                  g.lo[2] + ((double)(h0[2] - 1) + (double)pc.z) * g.dd[2] - ob.center[2] };
+            const double xi = (x[0] * ob.phd[0] + x[1] * ob.phd[1] + x[2] * ob.phd[2]) * ob.inv_hw;
+            const double yi = -(x[0] * ob.thd[0] + x[1] * ob.thd[1] + x[2] * ob.thd[2]) * ob.inv_hh;
+            const int ix = (int)floor((xi + 1.0) * (double)npx / 2.0), iy = (int)floor((yi + 1.0) * (double)npy / 2.0);
+            if (ix < 0 || ix >= npx || iy < 0 || iy >= npy) { ++n_drop; }
+            else {
+                ++n_con;
+                pixel = iy * npx + ix;
+                out[0] = att * S[0]; out[1] = att * S[1]; out[2] = att * S[2]; out[3] = att * S[3];
+            }
         }
-        const float att = expf(-A);
-        // I3: orthographic projection of the event position (fp64, once per ray)
-        const uint32_t cell = __float_as_uint(pc.w);
-        const int ix0 = (int)(cell % (uint32_t)g.nx);
-        const uint32_t t = cell / (uint32_t)g.nx;
-        const int iy0 = (int)(t % (uint32_t)g.ny), iz0 = (int)(t / (uint32_t)g.ny);
-        const double x[3] = { g.lo[0] + ((double)ix0 + (double)pc.x) * g.dd[0] - ob.center[0],
-                              g.lo[1] + ((double)iy0 + (double)pc.y) * g.dd[1] - ob.center[1],
-                              g.lo[2] + ((double)iz0 + (double)pc.z) * g.dd[2] - ob.center[2] };
-        const double xi = (x[0] * ob.phd[0] + x[1] * ob.phd[1] + x[2] * ob.phd[2]) * ob.inv_hw;
-        const double yi = -(x[0] * ob.thd[0] + x[1] * ob.thd[1] + x[2] * ob.thd[2]) * ob.inv_hh;
-        const int px = (int)floor((xi + 1.0) * (double)npx / 2.0), py = (int)floor((yi + 1.0) * (double)npy / 2.0);
-        if (px < 0 || px >= npx || py < 0 || py >= npy) { ++n_drop; continue; }
-        ++n_con;
-        const size_t plane = (size_t)npx * npy;
-        double* at = img + (size_t)o * 4 * plane + (size_t)py * npx + px;
-        atomicAdd(at, (double)(att * S[0]));
-        atomicAdd(at + plane, (double)(att * S[1]));
-        atomicAdd(at + 2 * plane, (double)(att * S[2]));
-        atomicAdd(at + 3 * plane, (double)(att * S[3]));
+        // I3: one atomic per distinct pixel of the warp: the lowest lane of every group of equal pixels
+        // collects the group's values (fp64) one peer at a time
+        const unsigned peers = __match_any_sync(0xffffffffu, pixel);
+        const int leader = __ffs(peers) - 1;
+        unsigned rem = peers & ~(1u << leader);
+        double acc[4] = { (double)out[0], (double)out[1], (double)out[2], (double)out[3] };
+        while (__any_sync(0xffffffffu, rem != 0u && pixel >= 0)) {
+            const int src = rem ? __ffs(rem) - 1 : lane;
+#pragma unroll
+            for (int s = 0; s < 4; ++s) {
+                const float v = __shfl_sync(0xffffffffu, out[s], src);
+                if (rem) acc[s] += (double)v;
+            }
+            rem &= rem - 1u;
+        }
+        if (pixel >= 0 && lane == leader) {
+            const size_t plane = (size_t)npx * npy;
+            double* at = img + (size_t)obs_index * 4 * plane + pixel;
+            atomicAdd(at, acc[0]);
+            atomicAdd(at + plane, acc[1]);
+            atomicAdd(at + 2 * plane, acc[2]);
+            atomicAdd(at + 3 * plane, acc[3]);
+        }
     }
     steps = krp_warp_sum(steps); n_con = krp_warp_sum(n_con); n_drop = krp_warp_sum(n_drop);
-    if ((threadIdx.x & 31) == 0) {
+    if (lane == 0) {
         if (steps) atomicAdd(&ctl->stats.steps_image, steps);
         if (n_con) atomicAdd(&ctl->stats.contributions, n_con);
         if (n_drop) atomicAdd(&ctl->stats.dropped, n_drop);
@@ -653,23 +832,28 @@ __global__ void krp_k_events_clear(KrpCtl* ctl) { ctl->n_events = 0; ctl->ev_beg
 // ------------------------------------------------------------------------------------------
 // T0  setup kernels (not on the timed path)
 // ------------------------------------------------------------------------------------------
-__global__ void krp_k_pack(const float* __restrict__ density, const float* __restrict__ bfield, uint32_t ncell,
+__global__ void krp_k_pack(KrpModel g, const float* __restrict__ density, const float* __restrict__ bfield, uint32_t npad,
                            float4* __restrict__ cell, float* __restrict__ kr, int* __restrict__ bad)
 {
     uint32_t c = blockIdx.x * blockDim.x + threadIdx.x;
-    if (c >= ncell) return;
-    float d = density[c];
-    if (!(d >= 0.f) || isinf(d)) atomicAdd(bad, 1);
-    if (kr) kr[c] = d;
-    if (cell) {
-        double bx = 0.0, by = 0.0, bz = 1.0;
+    if (c >= npad) return;
+    int hx, hy, hz;
+    krp_pad_coords(g, c, hx, hy, hz);
+    const bool halo = hx == 0 || hy == 0 || hz == 0 || hx == g.nx + 1 || hy == g.ny + 1 || hz == g.nz + 1;
+    float d = -1.f;                                   // halo: negative kappa*rho marks the outside of the grid
+    double bx = 0.0, by = 0.0, bz = 1.0;
+    if (!halo) {
+        const size_t lin = ((size_t)(hz - 1) * g.ny + (hy - 1)) * g.nx + (hx - 1);
+        d = density[lin];
+        if (!(d >= 0.f) || isinf(d)) { atomicAdd(bad, 1); d = 0.f; }
         if (bfield) {
-            bx = bfield[3 * (size_t)c]; by = bfield[3 * (size_t)c + 1]; bz = bfield[3 * (size_t)c + 2];
+            bx = bfield[3 * lin]; by = bfield[3 * lin + 1]; bz = bfield[3 * lin + 2];
             double r = sqrt(bx * bx + by * by + bz * bz);
             if (r > 0.0) { bx /= r; by /= r; bz /= r; } else { bx = 0.0; by = 0.0; bz = 1.0; }
         }
-        cell[c] = make_float4(d, (float)bx, (float)by, (float)bz);
     }
+    if (kr) kr[c] = d;
+    if (cell) cell[c] = make_float4(d, (float)bx, (float)by, (float)bz);
 }
 
 __global__ void krp_k_f2d(const float* __restrict__ w, uint32_t n, double* __restrict__ o)

@@ -61,7 +61,11 @@ def test_sequences_and_images_small(name):
     assert st_g["packets"] == n and st_g["overflow"] == 0
     assert abs(st_g["events"] - st_o["events"]) <= max(2, 2e-3 * st_o["events"])
     assert abs(st_g["steps_transport"] - st_o["steps_transport"]) <= 2e-3 * st_o["steps_transport"]
-    assert abs(st_g["steps_image"] - st_o["steps_image"]) <= 2e-3 * st_o["steps_image"] + 2
+    # imaging rays stop once e^{-A} is exactly zero in fp32 (A > 104, thick cells only: C3), so the kernel
+    # may take fewer cell steps than the oracle there; everywhere else the counts agree
+    assert st_g["steps_image"] <= st_o["steps_image"] * (1 + 2e-3) + 2
+    if name != "c3":
+        assert abs(st_g["steps_image"] - st_o["steps_image"]) <= 2e-3 * st_o["steps_image"] + 2
     assert st_g["contributions"] + st_g["dropped"] == st_g["events"] * len(cfg["observers"])
     for kx in ("w_escaped", "w_absorbed", "w_cut"):
         assert abs(st_g[kx] - st_o[kx]) <= 2e-3 * n, (kx, st_g[kx], st_o[kx])
