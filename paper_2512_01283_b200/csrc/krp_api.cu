@@ -36,8 +36,10 @@ struct krp_grid {
     KrpModel m;
     int device = 0, n_sm = 0;
     // owned device memory
-    float* d_kr = nullptr;
-    float4* d_cell = nullptr;
+    float* d_kr = nullptr;          // = d_kr_alloc + margin
+    float4* d_cell = nullptr;       // = d_cell_alloc + margin
+    float* d_kr_alloc = nullptr;
+    float4* d_cell_alloc = nullptr;
     float4* d_opac = nullptr;
     float4* d_opA = nullptr;
     float4* d_opB = nullptr;
@@ -45,7 +47,7 @@ struct krp_grid {
     // imaging order (counting sort of the events by cell bin)
     unsigned int* d_bins = nullptr;
     uint32_t n_bins = 0;
-    int bin_shift = 0;
+    int bin_shift = 0, sub_bits = 0;
     unsigned int* d_perm = nullptr;
     uint64_t perm_cap = 0;
     void* d_scan = nullptr;
@@ -92,7 +94,7 @@ static int alloc_records(KrpRecords& r, uint64_t cap, bool with_tau)
 extern "C" int krp_grid_destroy(krp_grid* g)
 {
     if (!g) return KRP_OK;
-    cudaFree(g->d_kr); cudaFree(g->d_cell); cudaFree(g->d_opac); cudaFree(g->d_mueller); cudaFree(g->d_cdf);
+    cudaFree(g->d_kr_alloc); cudaFree(g->d_cell_alloc); cudaFree(g->d_opac); cudaFree(g->d_mueller); cudaFree(g->d_cdf);
     cudaFree(g->d_src_cdf); cudaFree(g->d_ctl); cudaFree(g->d_obs); cudaFree(g->d_img);
     cudaFree(g->d_opA); cudaFree(g->d_opB); cudaFree(g->d_bins); cudaFree(g->d_perm); cudaFree(g->d_scan);
     free_records(g->q[0]); free_records(g->q[1]); free_records(g->ev);
@@ -243,8 +245,18 @@ extern "C" int krp_grid_create(krp_grid** out, int nx, int ny, int nz, const dou
     int* d_bad = nullptr;
     CK(cudaMalloc(&d_bad, sizeof(int)));
     CK(cudaMemsetAsync(d_bad, 0, sizeof(int), st));
-    if (m.scalar) CK(cudaMalloc(&g->d_kr, sizeof(float) * (size_t)g->npad));
-    else          CK(cudaMalloc(&g->d_cell, sizeof(float4) * (size_t)g->npad));
+    // a margin of one padded plane on either side keeps the imaging march's look-ahead load (one cell past the
+    // halo cell that ends the ray) inside the allocation; its content is never used
+    const size_t margin = m.pxy, n_alloc = (size_t)g->npad + 2 * margin;
+    if (m.scalar) {
+        CK(cudaMalloc(&g->d_kr_alloc, sizeof(float) * n_alloc));
+        CK(cudaMemsetAsync(g->d_kr_alloc, 0xff, sizeof(float) * n_alloc, st));
+        g->d_kr = g->d_kr_alloc + margin;
+    } else {
+        CK(cudaMalloc(&g->d_cell_alloc, sizeof(float4) * n_alloc));
+        CK(cudaMemsetAsync(g->d_cell_alloc, 0xff, sizeof(float4) * n_alloc, st));
+        g->d_cell = g->d_cell_alloc + margin;
+    }
     {
         const int tb = 256;
         const unsigned nb = (unsigned)((g->npad + tb - 1) / tb);
@@ -262,6 +274,10 @@ extern "C" int krp_grid_create(krp_grid** out, int nx, int ny, int nz, const dou
     g->bin_shift = m.scalar ? 5 : 3;
     while ((g->npad >> g->bin_shift) >= (1u << 22)) g->bin_shift++;
     g->n_bins = (g->npad >> g->bin_shift) + 1;
+    // sub-counters per bin against atomic contention in hot cells: about 2^21 counters in all, at most 64 per bin
+    g->sub_bits = 0;
+    while (g->sub_bits < 6 && ((uint64_t)g->n_bins << (g->sub_bits + 1)) <= (1ull << 21)) g->sub_bits++;
+    g->n_bins <<= g->sub_bits;
     CK(cudaMalloc(&g->d_bins, sizeof(unsigned int) * ((size_t)g->n_bins + 1)));
     CK(cub::DeviceScan::ExclusiveSum(nullptr, g->scan_bytes, g->d_bins, g->d_bins, (int)(g->n_bins + 1), st));
     CK(cudaMalloc(&g->d_scan, g->scan_bytes ? g->scan_bytes : 16));
@@ -475,10 +491,10 @@ extern "C" int krp_image(krp_grid* g, const krp_observer* obs, int n_obs, int np
     // I0: order the events by cell bin (count, scan, scatter)
     const unsigned pers = (unsigned)(g->n_sm * g->blocks_per_sm);
     CK(cudaMemsetAsync(g->d_bins, 0, sizeof(unsigned int) * ((size_t)g->n_bins + 1), st));
-    krp_k_sort_count<<<pers, 256, 0, st>>>(g->d_ctl, g->ev, g->bin_shift, flags, g->d_bins);
+    krp_k_sort_count<<<pers, 256, 0, st>>>(g->d_ctl, g->ev, g->bin_shift, g->sub_bits, flags, g->d_bins);
     CK(cub::DeviceScan::ExclusiveSum(g->d_scan, g->scan_bytes, g->d_bins, g->d_bins, (int)(g->n_bins + 1), st));
     krp_k_image_prep<<<1, 1, 0, st>>>(g->d_ctl, g->d_bins, g->n_bins);
-    krp_k_sort_scatter<<<pers, 256, 0, st>>>(g->d_ctl, g->ev, g->bin_shift, flags, g->d_bins, g->d_perm);
+    krp_k_sort_scatter<<<pers, 256, 0, st>>>(g->d_ctl, g->ev, g->bin_shift, g->sub_bits, flags, g->d_bins, g->d_perm);
     g->launches += 5;   // count, scan (2 kernels), prep, scatter
     // I1-I3: one launch per observer (its constants are kernel parameters); launches rotate over
     // KRP_MAX_OBS_PACK work counters, rewound when the rotation wraps

@@ -123,70 +123,125 @@ __device__ __forceinline__ float krp_event_solve(float R, float qq, float a1, fl
 // march cell to cell until the event or the grid edge; at an event append the pre-scatter record.
 // The march is fp32; the depth still to go is kept in fp64.
 // ------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) krp_k_flight_scalar(KrpModel g, KrpCtl* ctl, KrpRecords q, int in, KrpRecords ev)
+// per-thread tallies of a flight kernel, reduced once per warp at the end
+struct KrpFlightTally {
+    unsigned long long steps, n_ev, n_over;
+    double w_esc, w_abs, w_cut;
+};
+__device__ __forceinline__ void krp_tally_flush(KrpFlightTally& t, KrpCtl* ctl)
+{
+    t.steps = krp_warp_sum(t.steps); t.n_ev = krp_warp_sum(t.n_ev); t.n_over = krp_warp_sum(t.n_over);
+    t.w_esc = krp_warp_sum(t.w_esc); t.w_abs = krp_warp_sum(t.w_abs); t.w_cut = krp_warp_sum(t.w_cut);
+    if ((threadIdx.x & 31) == 0) {
+        if (t.steps) atomicAdd(&ctl->stats.steps_transport, t.steps);
+        if (t.n_ev) atomicAdd(&ctl->stats.events, t.n_ev);
+        if (t.n_over) atomicAdd(&ctl->stats.overflow, t.n_over);
+        if (t.w_esc != 0.0) atomicAdd(&ctl->stats.w_escaped, t.w_esc);
+        if (t.w_abs != 0.0) atomicAdd(&ctl->stats.w_absorbed, t.w_abs);
+        if (t.w_cut != 0.0) atomicAdd(&ctl->stats.w_cut, t.w_cut);
+    }
+}
+
+// T5: event record (pre-scatter state), albedo weighting, termination (R12).  Called by the lanes whose flight
+// ended in an event; the slot is reserved with one atomic for all of them.
+__device__ __forceinline__ void krp_event_append(const KrpModel& g, KrpCtl* ctl, const KrpRecords& ev, unsigned long long id,
+                                                 uint32_t cell, const float pe[3], const float n[3], uint32_t k, float W,
+                                                 float omega, float qs, float us, float vs, KrpFlightTally& t)
+{
+    const float Wn = omega * W;
+    const uint32_t kn = k + 1u;
+    const bool term = (Wn < g.w_min) || ((int)kn >= g.max_scatter);
+    t.w_abs += (double)W - (double)Wn;
+    const unsigned long long slot = krp_reserve64(&ctl->n_events);
+    if (slot < ctl->ev_cap) {
+        ev.pc[slot] = make_float4(pe[0], pe[1], pe[2], __uint_as_float(cell));
+        ev.nk[slot] = make_float4(n[0], n[1], n[2], __uint_as_float(kn | (term ? KRP_TERM_BIT : 0u)));
+        ev.S[slot] = make_float4(Wn, qs, us, vs);
+        ev.id[slot] = id;
+        ++t.n_ev;
+        if (term) t.w_cut += (double)Wn;
+    } else {
+        ++t.n_over;
+        t.w_cut += (double)Wn;
+    }
+}
+
+// Flight kernels are persistent: a lane whose flight has ended (event or escape) takes the next queue entry
+// at the next refill point, KRP_FLIGHT_BURST cell steps apart, so that the lanes of a warp stay busy although
+// flight lengths are exponentially distributed (T7, north_star "warp-level compaction of live packets").
+#ifndef KRP_FLIGHT_BURST
+#define KRP_FLIGHT_BURST 16
+#endif
+
+enum { KRP_IDLE = 0, KRP_RUN = 1, KRP_HIT = 2, KRP_ESC = 3 };
+
+__global__ void __launch_bounds__(256, 4) krp_k_flight_scalar(KrpModel g, KrpCtl* ctl, KrpRecords q, int in, KrpRecords ev)
 {
     const unsigned int n_items = ctl->q_count[in];
-    unsigned long long steps = 0, n_ev = 0, n_over = 0;
-    double w_esc = 0.0, w_abs = 0.0, w_cut = 0.0;
-    for (unsigned int item = blockIdx.x * blockDim.x + threadIdx.x; item < n_items; item += gridDim.x * blockDim.x) {
-        const float4 pc = q.pc[item], nk = q.nk[item], S0 = q.S[item];
-        const float n[3] = { nk.x, nk.y, nk.z };
-        const float p0[3] = { pc.x, pc.y, pc.z };
-        const uint32_t k = __float_as_uint(nk.w);
-        const uint32_t c0 = __float_as_uint(pc.w);
-        KrpRay ray;
-        krp_ray_init(g, c0, p0, n, ray);
-        double D = q.tau[item];
-        bool hit = false;
-        double moved = 0.0;
-        float kr = __ldg(g.kr + ray.c);
-        for (;;) {
-            const float ds = krp_ray_ds(ray);
-            ++steps;
-            const float dt1 = g.a1c * kr * ds;
-            if ((double)dt1 >= D) {              // event inside this cell
-                moved = D / ((double)g.a1c * (double)kr);
-                hit = true;
-                break;
+    KrpFlightTally tl = { 0, 0, 0, 0.0, 0.0, 0.0 };
+    int status = KRP_IDLE;
+    bool more = true;
+    unsigned int item = 0;
+    float n[3] = { 0.f, 0.f, 1.f }, p0[3] = { 0.f, 0.f, 0.f }, kr = 0.f, a1kr = 0.f;
+    uint32_t c0 = 0;
+    KrpRay ray = {};
+    double D = 0.0;
+    for (;;) {
+        // refill point: the lanes whose flight ended during the last burst close it together, then take new work
+        if (status == KRP_HIT || status == KRP_ESC) {
+            int h0[3], h1[3];
+            krp_pad_coords(g, c0, h0[0], h0[1], h0[2]);
+            krp_pad_coords(g, ray.c, h1[0], h1[1], h1[2]);
+            const int crossings = abs(h1[0] - h0[0]) + abs(h1[1] - h0[1]) + abs(h1[2] - h0[2]);
+            const float4 S0 = q.S[item];
+            if (status == KRP_HIT) {
+                const double moved = D / ((double)g.a1c * (double)kr);
+                float pe[3];
+                krp_event_pos(g, n, p0, c0, ray.c, moved, pe);
+                tl.steps += (unsigned long long)(crossings + 1);
+                krp_event_append(g, ctl, ev, q.id[item], ray.c, pe, n, __float_as_uint(q.nk[item].w), S0.x, g.omc,
+                                 S0.y, S0.z, S0.w, tl);
+            } else {
+                tl.steps += (unsigned long long)crossings;
+                tl.w_esc += (double)S0.x;
             }
-            D -= (double)dt1;
-            krp_ray_step(ray, ds);
-            kr = __ldg(g.kr + ray.c);
-            if (kr < 0.f) break;                 // halo: the packet left the grid
+            status = KRP_IDLE;
         }
-        const float W = S0.x;
-        if (!hit) { w_esc += (double)W; continue; }
-        // T5: event record, albedo weighting, termination (R12)
-        float pe[3];
-        krp_event_pos(g, n, p0, c0, ray.c, moved, pe);
-        const float Wn = g.omc * W;
-        const uint32_t kn = k + 1u;
-        const bool term = (Wn < g.w_min) || ((int)kn >= g.max_scatter);
-        w_abs += (double)W - (double)Wn;
-        unsigned long long slot = krp_reserve64(&ctl->n_events);
-        if (slot < ctl->ev_cap) {
-            ev.pc[slot] = make_float4(pe[0], pe[1], pe[2], __uint_as_float(ray.c));
-            ev.nk[slot] = make_float4(n[0], n[1], n[2], __uint_as_float(kn | (term ? KRP_TERM_BIT : 0u)));
-            ev.S[slot] = make_float4(Wn, S0.y, S0.z, S0.w);
-            ev.id[slot] = q.id[item];
-            ++n_ev;
-            if (term) w_cut += (double)Wn;
-        } else {
-            ++n_over;
-            w_cut += (double)Wn;
+        if (status == KRP_IDLE && more) {
+            item = krp_reserve32(&ctl->work[0]);
+            if (item < n_items) {
+                const float4 pc = q.pc[item], nk = q.nk[item];
+                n[0] = nk.x; n[1] = nk.y; n[2] = nk.z;
+                p0[0] = pc.x; p0[1] = pc.y; p0[2] = pc.z;
+                c0 = __float_as_uint(pc.w);
+                krp_ray_init(g, c0, p0, n, ray);
+                D = q.tau[item];
+                kr = __ldg(g.kr + ray.c);
+                a1kr = g.a1c * kr;
+                status = KRP_RUN;
+            } else {
+                more = false;
+            }
+        }
+        if (!__any_sync(0xffffffffu, status == KRP_RUN)) break;
+#pragma unroll 1
+        for (int burst = 0; burst < KRP_FLIGHT_BURST; ++burst) {
+            if (status == KRP_RUN) {
+                const float ds = krp_ray_ds(ray);
+                const float dt1 = a1kr * ds;
+                if ((double)dt1 >= D) {
+                    status = KRP_HIT;                // event inside this cell, located at the refill point
+                } else {
+                    D -= (double)dt1;
+                    krp_ray_step(ray, ds);
+                    kr = __ldg(g.kr + ray.c);
+                    a1kr = g.a1c * kr;
+                    if (kr < 0.f) status = KRP_ESC;  // halo: the packet left the grid
+                }
+            }
         }
     }
-    // statistics: one atomic per warp and counter
-    steps = krp_warp_sum(steps); n_ev = krp_warp_sum(n_ev); n_over = krp_warp_sum(n_over);
-    w_esc = krp_warp_sum(w_esc); w_abs = krp_warp_sum(w_abs); w_cut = krp_warp_sum(w_cut);
-    if ((threadIdx.x & 31) == 0) {
-        if (steps) atomicAdd(&ctl->stats.steps_transport, steps);
-        if (n_ev) atomicAdd(&ctl->stats.events, n_ev);
-        if (n_over) atomicAdd(&ctl->stats.overflow, n_over);
-        if (w_esc != 0.0) atomicAdd(&ctl->stats.w_escaped, w_esc);
-        if (w_abs != 0.0) atomicAdd(&ctl->stats.w_absorbed, w_abs);
-        if (w_cut != 0.0) atomicAdd(&ctl->stats.w_cut, w_cut);
-    }
+    krp_tally_flush(tl, ctl);
 }
 
 // ------------------------------------------------------------------------------------------
@@ -223,74 +278,136 @@ __device__ __forceinline__ double krp_rsqrt_near1(double vv)
 // T3/T4/T5, general mode (direction-dependent, dichroic opacity; 16-byte cells).  Everything that
 // decides in which cell the event falls -- segment lengths, alpha1(mu), the scalar depth D and the
 // normalised intensity i -- is carried in fp64 (an integer decided by
-// floating point is taken in the oracle's precision); the Stokes algebra (reference rotation,
-// sinh/cosh/sin/cos factors, q,u,v) is fp32.
+// floating point is taken in the oracle's precision; in a clumpy medium a difference in the last
+// bit of an event position is amplified by the density contrast at every later scattering); the
+// Stokes algebra (reference rotation, sinh/cosh/sin/cos factors, q,u,v) is fp32.
 // ------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) krp_k_flight_general(KrpModel g, KrpCtl* ctl, KrpRecords q, int in, KrpRecords ev)
+struct KrpCellCoef {
+    double a1, dtau, dt1;      // alpha1(mu), kappa*rho*ds, alpha1*kappa*rho*ds
+    float a2, a3, omega;       // alpha2(mu), alpha3(mu), albedo(mu)
+};
+
+__device__ __forceinline__ void krp_cell_coef(const KrpModel& g, const float4 cl, const double nd[3], double inv_n, double xs,
+                                              double ds, KrpCellCoef& c)
+{
+    const double bx = cl.y, by = cl.z, bz = cl.w;
+    double mu = fabs(nd[0] * bx + nd[1] * by + nd[2] * bz) * inv_n * krp_rsqrt_near1(bx * bx + by * by + bz * bz);
+    mu = fmin(mu, 1.0);
+    const double x = mu * xs;
+    const int j = min((int)x, g.n_inc - 2);
+    const double w = x - (double)j;
+    const float4 oa = g.opac[j], ob = g.opac[j + 1];
+    c.a1 = (1.0 - w) * (double)oa.x + w * (double)ob.x;
+    const float wf = (float)w, w0f = 1.f - wf;
+    c.a2 = w0f * oa.y + wf * ob.y; c.a3 = w0f * oa.z + wf * ob.z; c.omega = w0f * oa.w + wf * ob.w;
+    c.dtau = (double)cl.x * ds;
+    c.dt1 = c.a1 * c.dtau;
+}
+
+__global__ void __launch_bounds__(256, 2) krp_k_flight_general(KrpModel g, KrpCtl* ctl, KrpRecords q, int in, KrpRecords ev)
 {
     const unsigned int n_items = ctl->q_count[in];
-    unsigned long long steps = 0, n_ev = 0, n_over = 0;
-    double w_esc = 0.0, w_abs = 0.0, w_cut = 0.0;
+    KrpFlightTally tl = { 0, 0, 0, 0.0, 0.0, 0.0 };
     const double xs = (double)(g.n_inc - 1);
-    for (unsigned int item = blockIdx.x * blockDim.x + threadIdx.x; item < n_items; item += gridDim.x * blockDim.x) {
-        const float4 pc = q.pc[item], nk = q.nk[item], S0 = q.S[item];
-        const float n[3] = { nk.x, nk.y, nk.z };
-        const float p0[3] = { pc.x, pc.y, pc.z };
-        const uint32_t k = __float_as_uint(nk.w);
-        const double tau0 = q.tau[item];
-        KrpRayD ray;
-        krp_rayd_init(g, __float_as_uint(pc.w), p0, n, ray);
-        float4 cl = __ldg(g.cell + ray.c);
-        float th[3], ph[3];
-        krp_basis<float>(n, th, ph);
-        const double nd[3] = { n[0], n[1], n[2] };
-        const double inv_n = krp_rsqrt_near1(nd[0] * nd[0] + nd[1] * nd[1] + nd[2] * nd[2]);
-        double D = tau0, i = 1.0;
-        float qs = S0.y, us = S0.z, vs = S0.w;      // lab reference
-        float Asum = 0.f;
-        const float tau0f = (float)tau0, guard = 1.f + g.rho + 1e-3f;
-        bool hit = false;
-        double moved = 0.0;
-        float omega = g.omc;
-        for (;;) {
+    const float guard = 1.f + g.rho + 1e-3f;
+    int status = KRP_IDLE;
+    bool more = true;
+    unsigned int item = 0;
+    // state of the flight in progress
+    float n[3] = { 0.f, 0.f, 1.f }, p0[3] = { 0.f, 0.f, 0.f }, th[3] = { 0.f, 0.f, 0.f }, ph[3] = { 0.f, 0.f, 0.f };
+    double nd[3] = { 0.0, 0.0, 1.0 }, inv_n = 1.0, D = 0.0, i = 1.0;
+    float qs = 0.f, us = 0.f, vs = 0.f, Asum = 0.f, tau0f = 0.f;
+    unsigned int nsteps = 0;
+    KrpRayD ray = {};
+    float4 cl = make_float4(0.f, 0.f, 0.f, 1.f);
+    for (;;) {
+        // refill point: the lanes whose flight ended during the last burst close it together
+        if (status == KRP_HIT) {
+            // the state is that of the entry into the event cell: solve for t, evolve to t, normalise to I = 1 (R7)
             const double ds = krp_rayd_ds(ray);
-            ++steps;
-            const float kr = cl.x;
-            if (kr > 0.f) {
-                const double bx = cl.y, by = cl.z, bz = cl.w;
-                double mu = fabs(nd[0] * bx + nd[1] * by + nd[2] * bz) * inv_n * krp_rsqrt_near1(bx * bx + by * by + bz * bz);
-                mu = fmin(mu, 1.0);
-                const double x = mu * xs;
-                const int j = min((int)x, g.n_inc - 2);
-                const double w = x - (double)j;
-                const float4 oa = g.opac[j], ob = g.opac[j + 1];
-                const double a1 = (1.0 - w) * (double)oa.x + w * (double)ob.x;
-                const float wf = (float)w, w0f = 1.f - wf;
-                const float a2 = w0f * oa.y + wf * ob.y, a3 = w0f * oa.z + wf * ob.z;
-                const double dtau = (double)kr * ds;
-                const double dt1 = a1 * dtau;
-                Asum += (float)dt1;
+            KrpCellCoef cc;
+            krp_cell_coef(g, cl, nd, inv_n, xs, ds, cc);
+            const double R = D + log(i);
+            double moved;
+            if (cc.a2 == 0.f && cc.a3 == 0.f) {
+                moved = (R / cc.a1) / (double)cl.x;
+                const float inv = (float)(1.0 / i);
+                qs *= inv; us *= inv; vs *= inv;
+            } else {
+                const float a = th[0] * cl.y + th[1] * cl.z + th[2] * cl.w;
+                const float b = ph[0] * cl.y + ph[1] * cl.z + ph[2] * cl.w;
+                float c2, s2;
+                krp_eta2<float>(a, b, c2, s2);
+                const float qg_e = c2 * qs + s2 * us, ug_e = -s2 * qs + c2 * us, vg_e = vs, i_f = (float)i;
+                const double t = krp_event_solve_d(R, (double)qg_e / i, cc.a1, (double)cc.a2, cc.dtau);
+                const float tf = (float)t;
+                float sh, chm1, syt = 0.f, cyt = 1.f;
+                krp_sinh_coshm1(cc.a2 * tf, sh, chm1);
+                if (cc.a3 != 0.f) sincosf(cc.a3 * tf, &syt, &cyt);
+                const float it = i_f + (i_f * chm1 - qg_e * sh);
+                float qt = qg_e + (qg_e * chm1 - i_f * sh);
+                float ut = ug_e * cyt - vg_e * syt;
+                float vt = ug_e * syt + vg_e * cyt;
+                const float inv = 1.f / it;
+                qt *= inv; ut *= inv; vt *= inv;
+                qs = c2 * qt - s2 * ut; us = s2 * qt + c2 * ut; vs = vt;
+                moved = t / (double)cl.x;
+            }
+            float pe[3];
+            pe[0] = krp_locald(n[0], ray.rx, ray.tx, moved, p0[0]);
+            pe[1] = krp_locald(n[1], ray.ry, ray.ty, moved, p0[1]);
+            pe[2] = krp_locald(n[2], ray.rz, ray.tz, moved, p0[2]);
+            tl.steps += nsteps;
+            krp_event_append(g, ctl, ev, q.id[item], ray.c, pe, n, __float_as_uint(q.nk[item].w), q.S[item].x, cc.omega,
+                             qs, us, vs, tl);
+            status = KRP_IDLE;
+        } else if (status == KRP_ESC) {
+            tl.steps += nsteps;
+            tl.w_esc += (double)q.S[item].x;
+            status = KRP_IDLE;
+        }
+        if (status == KRP_IDLE && more) {
+            item = krp_reserve32(&ctl->work[0]);
+            if (item < n_items) {
+                const float4 pc = q.pc[item], nk = q.nk[item], S0 = q.S[item];
+                n[0] = nk.x; n[1] = nk.y; n[2] = nk.z;
+                p0[0] = pc.x; p0[1] = pc.y; p0[2] = pc.z;
+                const double tau0 = q.tau[item];
+                krp_rayd_init(g, __float_as_uint(pc.w), p0, n, ray);
+                cl = __ldg(g.cell + ray.c);
+                krp_basis<float>(n, th, ph);
+                nd[0] = n[0]; nd[1] = n[1]; nd[2] = n[2];
+                inv_n = krp_rsqrt_near1(nd[0] * nd[0] + nd[1] * nd[1] + nd[2] * nd[2]);
+                D = tau0; i = 1.0;
+                qs = S0.y; us = S0.z; vs = S0.w;      // lab reference
+                Asum = 0.f; tau0f = (float)tau0; nsteps = 0;
+                status = KRP_RUN;
+            } else {
+                more = false;
+            }
+        }
+        if (!__any_sync(0xffffffffu, status == KRP_RUN)) break;
+#pragma unroll 1
+        for (int burst = 0; burst < KRP_FLIGHT_BURST; ++burst) {
+            if (status != KRP_RUN) continue;
+            const double ds = krp_rayd_ds(ray);
+            ++nsteps;
+            if (cl.x > 0.f) {
+                KrpCellCoef cc;
+                krp_cell_coef(g, cl, nd, inv_n, xs, ds, cc);
+                Asum += (float)cc.dt1;
                 const bool near_end = Asum * guard >= tau0f;
-                if (a2 == 0.f && a3 == 0.f) {
-                    if (near_end) {
-                        const double R = D + log(i);
-                        if (dt1 >= R) {
-                            moved = (R / a1) / (double)kr;
-                            const float inv = (float)(1.0 / i);
-                            qs *= inv; us *= inv; vs *= inv;
-                            omega = w0f * oa.w + wf * ob.w; hit = true;
-                            break;
-                        }
-                    }
-                    D -= dt1;
+                if (cc.a2 == 0.f && cc.a3 == 0.f) {
+                    if (near_end && cc.dt1 >= D + log(i)) { status = KRP_HIT; continue; }
+                    D -= cc.dt1;
                 } else {
                     const float a = th[0] * cl.y + th[1] * cl.z + th[2] * cl.w;
                     const float b = ph[0] * cl.y + ph[1] * cl.z + ph[2] * cl.w;
                     float c2, s2;
                     krp_eta2<float>(a, b, c2, s2);
                     const float qg_e = c2 * qs + s2 * us, ug_e = -s2 * qs + c2 * us, vg_e = vs;   // eq. 7
-                    const float dtau_f = (float)dtau, i_f = (float)i;
-                    const float xx = a2 * dtau_f, yy = a3 * dtau_f;
+                    const float dtau_f = (float)cc.dtau, i_f = (float)i;
+                    const float xx = cc.a2 * dtau_f, yy = cc.a3 * dtau_f;
                     float sy = 0.f, cy = 1.f;
                     if (yy != 0.f) sincosf(yy, &sy, &cy);
                     float qg, ug, vg;
@@ -302,80 +419,30 @@ __global__ void __launch_bounds__(256) krp_k_flight_general(KrpModel g, KrpCtl* 
                         qg = qg_e + (qg_e * chm1 - i_f * sh);
                         ug = ug_e * cy - vg_e * sy;
                         vg = ug_e * sy + vg_e * cy;
-                        depth = dt1;
+                        depth = cc.dt1;
                     } else {
                         // thick cell: factor e^{-|alpha2 dtau|} moved into the scalar depth (no overflow at dtau ~ 1e3)
-                        const double xd = (double)a2 * dtau, axd = fabs(xd);
-                        const double E = exp(-2.0 * axd), s = xd > 0.0 ? 1.0 : -1.0, f = exp(-axd);
+                        const double xd = (double)cc.a2 * cc.dtau, axd = fabs(xd);
+                        const double E = exp(-2.0 * axd), sg = xd > 0.0 ? 1.0 : -1.0, f = exp(-axd);
                         const double qd = (double)qg_e;
-                        i_new = 0.5 * ((i - s * qd) + (i + s * qd) * E);
-                        qg = (float)(0.5 * ((qd - s * i) + (qd + s * i) * E));
+                        i_new = 0.5 * ((i - sg * qd) + (i + sg * qd) * E);
+                        qg = (float)(0.5 * ((qd - sg * i) + (qd + sg * i) * E));
                         ug = (float)f * (ug_e * cy - vg_e * sy);
                         vg = (float)f * (ug_e * sy + vg_e * cy);
-                        depth = dt1 - axd;
+                        depth = cc.dt1 - axd;
                     }
                     const double Dn = D - depth;
-                    if (near_end && log(i_new) + Dn <= 0.0) {
-                        // event inside this cell: solve for t, evolve to t, normalise to I = 1, back to the lab reference
-                        const double R = D + log(i);
-                        const double t = krp_event_solve_d(R, (double)qg_e / i, a1, (double)a2, dtau);
-                        const float tf = (float)t;
-                        float sh, chm1, syt = 0.f, cyt = 1.f;
-                        krp_sinh_coshm1(a2 * tf, sh, chm1);
-                        if (a3 != 0.f) sincosf(a3 * tf, &syt, &cyt);
-                        const float it = i_f + (i_f * chm1 - qg_e * sh);
-                        float qt = qg_e + (qg_e * chm1 - i_f * sh);
-                        float ut = ug_e * cyt - vg_e * syt;
-                        float vt = ug_e * syt + vg_e * cyt;
-                        const float inv = 1.f / it;
-                        qt *= inv; ut *= inv; vt *= inv;
-                        qs = c2 * qt - s2 * ut; us = s2 * qt + c2 * ut; vs = vt;
-                        moved = t / (double)kr;
-                        omega = w0f * oa.w + wf * ob.w; hit = true;
-                        break;
-                    }
+                    if (near_end && log(i_new) + Dn <= 0.0) { status = KRP_HIT; continue; }   // state stays at cell entry
                     qs = c2 * qg - s2 * ug; us = s2 * qg + c2 * ug; vs = vg;
                     i = i_new; D = Dn;
                 }
             }
             krp_rayd_step(ray, ds);
             cl = __ldg(g.cell + ray.c);
-            if (cl.x < 0.f) break;               // halo: the packet left the grid
-        }
-        const float W = S0.x;
-        if (!hit) { w_esc += (double)W; continue; }
-        // T5: event record, albedo weighting, termination (R12)
-        float pe[3];
-        pe[0] = krp_locald(n[0], ray.rx, ray.tx, moved, p0[0]);
-        pe[1] = krp_locald(n[1], ray.ry, ray.ty, moved, p0[1]);
-        pe[2] = krp_locald(n[2], ray.rz, ray.tz, moved, p0[2]);
-        const float Wn = omega * W;
-        const uint32_t kn = k + 1u;
-        const bool term = (Wn < g.w_min) || ((int)kn >= g.max_scatter);
-        w_abs += (double)W - (double)Wn;
-        unsigned long long slot = krp_reserve64(&ctl->n_events);
-        if (slot < ctl->ev_cap) {
-            ev.pc[slot] = make_float4(pe[0], pe[1], pe[2], __uint_as_float(ray.c));
-            ev.nk[slot] = make_float4(n[0], n[1], n[2], __uint_as_float(kn | (term ? KRP_TERM_BIT : 0u)));
-            ev.S[slot] = make_float4(Wn, qs, us, vs);
-            ev.id[slot] = q.id[item];
-            ++n_ev;
-            if (term) w_cut += (double)Wn;
-        } else {
-            ++n_over;
-            w_cut += (double)Wn;
+            if (cl.x < 0.f) status = KRP_ESC;        // halo: the packet left the grid
         }
     }
-    steps = krp_warp_sum(steps); n_ev = krp_warp_sum(n_ev); n_over = krp_warp_sum(n_over);
-    w_esc = krp_warp_sum(w_esc); w_abs = krp_warp_sum(w_abs); w_cut = krp_warp_sum(w_cut);
-    if ((threadIdx.x & 31) == 0) {
-        if (steps) atomicAdd(&ctl->stats.steps_transport, steps);
-        if (n_ev) atomicAdd(&ctl->stats.events, n_ev);
-        if (n_over) atomicAdd(&ctl->stats.overflow, n_over);
-        if (w_esc != 0.0) atomicAdd(&ctl->stats.w_escaped, w_esc);
-        if (w_abs != 0.0) atomicAdd(&ctl->stats.w_absorbed, w_abs);
-        if (w_cut != 0.0) atomicAdd(&ctl->stats.w_cut, w_cut);
-    }
+    krp_tally_flush(tl, ctl);
 }
 
 // ------------------------------------------------------------------------------------------
@@ -569,35 +636,39 @@ __device__ __forceinline__ void krp_peel(const KrpModel& g, const float n[3], fl
 // indices by bin = padded cell id >> shift, entirely on the device (the event count never visits the
 // host).  Rays of one observer are parallel, so the 32 rays of a warp that start in neighbouring cells
 // walk through neighbouring cells for their whole length: their gathers share cache lines and they
-// leave the grid after nearly the same number of steps.
+// leave the grid after nearly the same number of steps.  Every bin has 2^sub_bits counters, picked by the low
+// bits of the event index, so that the many events of a hot cell (next to a point source) do not queue on one
+// atomic; the order inside a bin is arbitrary anyway.
 //   krp_k_sort_count    histogram of the bins
 //   (exclusive scan of the histogram: cub::DeviceScan, in krp_api.cu)
 //   krp_k_sort_scatter  perm[slot] = event index, slot reserved in the event's bin
 // ------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(256) krp_k_sort_count(KrpCtl* ctl, KrpRecords ev, int shift, int flags,
+__global__ void __launch_bounds__(256) krp_k_sort_count(KrpCtl* ctl, KrpRecords ev, int shift, int sub_bits, int flags,
                                                         unsigned int* __restrict__ bins)
 {
     unsigned long long n_ev = ctl->n_events;
     if (n_ev > ctl->ev_cap) n_ev = ctl->ev_cap;
+    const unsigned int sub_mask = (1u << sub_bits) - 1u;
     for (unsigned long long e = blockIdx.x * (unsigned long long)blockDim.x + threadIdx.x; e < n_ev;
          e += (unsigned long long)gridDim.x * blockDim.x) {
         const uint32_t k = __float_as_uint(ev.nk[e].w) & ~KRP_TERM_BIT;
         if (k == 0u && !(flags & 1)) continue;             // emission records take part only with direct light
-        atomicAdd(bins + (__float_as_uint(ev.pc[e].w) >> shift), 1u);
+        atomicAdd(bins + (((__float_as_uint(ev.pc[e].w) >> shift) << sub_bits) | ((unsigned int)e & sub_mask)), 1u);
     }
 }
 
 // after the scan `bins` holds the first slot of every bin; the last thread publishes the total
-__global__ void __launch_bounds__(256) krp_k_sort_scatter(KrpCtl* ctl, KrpRecords ev, int shift, int flags,
+__global__ void __launch_bounds__(256) krp_k_sort_scatter(KrpCtl* ctl, KrpRecords ev, int shift, int sub_bits, int flags,
                                                           unsigned int* __restrict__ bins, unsigned int* __restrict__ perm)
 {
     unsigned long long n_ev = ctl->n_events;
     if (n_ev > ctl->ev_cap) n_ev = ctl->ev_cap;
+    const unsigned int sub_mask = (1u << sub_bits) - 1u;
     for (unsigned long long e = blockIdx.x * (unsigned long long)blockDim.x + threadIdx.x; e < n_ev;
          e += (unsigned long long)gridDim.x * blockDim.x) {
         const uint32_t k = __float_as_uint(ev.nk[e].w) & ~KRP_TERM_BIT;
         if (k == 0u && !(flags & 1)) continue;
-        const unsigned int slot = atomicAdd(bins + (__float_as_uint(ev.pc[e].w) >> shift), 1u);
+        const unsigned int slot = atomicAdd(bins + (((__float_as_uint(ev.pc[e].w) >> shift) << sub_bits) | ((unsigned int)e & sub_mask)), 1u);
         perm[slot] = (unsigned int)e;
     }
 }
@@ -722,14 +793,21 @@ __global__ void __launch_bounds__(256, KRP_IMAGE_MIN_BLOCKS) krp_k_image(KrpMode
             r.tz = ob.n[2] > 0.f ? (1.f - pc.z) * ob.dt[2] : (ob.n[2] < 0.f ? pc.z * ob.dt[2] : KRP_INF_F);
             float A = 0.f;
             if (SCALAR) {
+                // two gathers in flight: the cell after next is requested before the next one is tested
                 float tau = 0.f;
-                float kr = __ldg(g.kr + r.c);
+                float kr_c = __ldg(g.kr + r.c);            // current cell (inside the grid)
+                float ds_c = krp_raya_step(r, rc);
+                float kr_n = __ldg(g.kr + r.c);            // next cell
+                uint32_t c_n = r.c;
 #pragma unroll 2
-                do {
-                    const float ds = krp_raya_step(r, rc);
-                    tau = fmaf(kr, ds, tau);
-                    kr = __ldg(g.kr + r.c);
-                } while (kr >= 0.f);
+                for (;;) {
+                    const float ds_n = krp_raya_step(r, rc);
+                    const float kr_nn = __ldg(g.kr + r.c); // look-ahead (may lie one cell past the halo: margin)
+                    tau = fmaf(kr_c, ds_c, tau);
+                    if (kr_n < 0.f) break;
+                    kr_c = kr_n; ds_c = ds_n; kr_n = kr_nn; c_n = r.c;
+                }
+                r.c = c_n;                                 // the halo cell that ended the ray
                 A = g.a1c * tau;
             } else {
                 float i = S[0], qs = S[1], us = S[2], vs = S[3];
