@@ -56,7 +56,7 @@ def parse_args():
     return ap.parse_args()
 
 
-DEFAULT_BATCH = {"c1": 100000, "c2": 1 << 22, "c3": 1 << 20, "c4": 1 << 21, "c5": 1 << 20}
+DEFAULT_BATCH = {"c1": 100000, "c2": 1 << 24, "c3": 1 << 22, "c4": 1 << 23, "c5": 1 << 22}
 
 
 def make_workload(args):

@@ -160,8 +160,10 @@ int krp_events_get(krp_grid* g, uint64_t cap, uint64_t* n, uint64_t* id, int32_t
                    int64_t* cell, float* pos, float* dir, float* stokes);
 int krp_events_clear(krp_grid* g, void* stream);
 
-/* Launch-shape knobs, for measurement only (0 keeps the default). */
-int krp_tune(krp_grid* g, int transport_block, int image_block, int blocks_per_sm);
+/* Launch-shape knobs, for measurement only (0 keeps the current value): threads per block of the
+ * flight and imaging kernels (multiples of 32 up to 256), persistent blocks per SM, and the number
+ * of cell steps a flight kernel takes between two points where idle lanes take new packets. */
+int krp_tune(krp_grid* g, int transport_block, int image_block, int blocks_per_sm, int flight_burst);
 /* Number of kernels the library has launched on behalf of g since creation. */
 uint64_t krp_launch_count(const krp_grid* g);
 

@@ -70,6 +70,7 @@ struct krp_grid {
     uint64_t launches = 0;
     int max_waves = 0;
     int transport_block = 256, image_block = 256, blocks_per_sm = 8;
+    int burst = KRP_FLIGHT_BURST;   // cell steps between refill points of the flight kernels
 };
 
 extern "C" const char* krp_last_error(void) { return g_err; }
@@ -155,11 +156,22 @@ extern "C" int krp_grid_create(krp_grid** out, int nx, int ny, int nz, const dou
     m.nx = nx; m.ny = ny; m.nz = nz; m.ncell = (uint32_t)((uint64_t)nx * ny * nz);
     m.px = nx + 2; m.py = ny + 2; m.pxy = (uint32_t)m.px * (uint32_t)m.py;
     g->npad = m.pxy * (uint32_t)(nz + 2);
+    {
+        auto magic = [](uint32_t d, uint32_t& mm, uint32_t& ss) {
+            uint32_t l = 0;
+            while ((1ull << l) < d) ++l;
+            mm = (uint32_t)(((1ull << 32) * ((1ull << l) - d)) / d + 1);
+            ss = l - 1;
+        };
+        magic((uint32_t)m.px, m.px_m, m.px_s);
+        magic((uint32_t)m.py, m.py_m, m.py_s);
+    }
     const int dims[3] = { nx, ny, nz };
     for (int a = 0; a < 3; ++a) {
         m.lo[a] = bounds[2 * a];
         m.dd[a] = (bounds[2 * a + 1] - bounds[2 * a]) / dims[a];
         m.d[a] = (float)m.dd[a];
+        m.inv_dd[a] = 1.0 / m.dd[a];
     }
     // opacity table: n_inc = 1 becomes two equal rows so that the kernels always interpolate
     const int n_inc = tables->n_inc == 1 ? 2 : tables->n_inc;
@@ -175,6 +187,8 @@ extern "C" int krp_grid_create(krp_grid** out, int nx, int ny, int nz, const dou
     }
     m.scalar = (constant && !dichroic && bfield == nullptr) ? 1 : 0;
     m.a1c = op[0]; m.omc = op[3]; m.rho = rho;
+    // scalar flights are short: static assignment; general flights are long: persistent lanes, refill every 32 steps
+    g->burst = m.scalar ? 1 : 32;
     m.n_inc = n_inc; m.n_ang = tables->n_ang;
     m.w_min = tables->w_min; m.max_scatter = tables->max_scatter;
     // number of waves that can contain live packets: the weight after k scatterings is <= omega_max^k
@@ -419,8 +433,9 @@ extern "C" int krp_transport(krp_grid* g, uint64_t n_packets, uint64_t seed, voi
     for (int w = 0; w < g->max_waves; ++w) {
         const int in = w & 1;
         krp_k_wave_prep<<<1, 1, 0, st>>>(g->d_ctl, in);
-        if (g->m.scalar) krp_k_flight_scalar<<<grid_f, tb, 0, st>>>(g->m, g->d_ctl, g->q[in], in, g->ev);
-        else             krp_k_flight_general<<<grid_f, tb, 0, st>>>(g->m, g->d_ctl, g->q[in], in, g->ev);
+        if (g->m.scalar && g->burst == 1) krp_k_flight_scalar_static<<<grid_f, tb, 0, st>>>(g->m, g->d_ctl, g->q[in], in, g->ev);
+        else if (g->m.scalar) krp_k_flight_scalar<<<grid_f, tb, 0, st>>>(g->m, g->d_ctl, g->q[in], in, g->ev, g->burst);
+        else             krp_k_flight_general<<<grid_f, tb, 0, st>>>(g->m, g->d_ctl, g->q[in], in, g->ev, g->burst);
         g->launches += 2;
         if (w + 1 < g->max_waves) {
             krp_k_scatter<<<grid_s, 128, 0, st>>>(g->m, g->d_ctl, g->ev, g->q[1 - in], 1 - in, seed);
@@ -608,7 +623,7 @@ extern "C" int krp_events_clear(krp_grid* g, void* stream)
     return KRP_OK;
 }
 
-extern "C" int krp_tune(krp_grid* g, int transport_block, int image_block, int blocks_per_sm)
+extern "C" int krp_tune(krp_grid* g, int transport_block, int image_block, int blocks_per_sm, int flight_burst)
 {
     if (!g) return fail(KRP_ERR_ARG, "grid is NULL");
     auto okb = [](int b) { return b == 0 || (b >= 32 && b <= 256 && b % 32 == 0); };
@@ -617,6 +632,8 @@ extern "C" int krp_tune(krp_grid* g, int transport_block, int image_block, int b
     if (transport_block) g->transport_block = transport_block;
     if (image_block) g->image_block = image_block;
     if (blocks_per_sm) g->blocks_per_sm = blocks_per_sm;
+    if (flight_burst < 0 || flight_burst > 4096) return fail(KRP_ERR_ARG, "flight_burst must be in 0..4096");
+    if (flight_burst) g->burst = flight_burst;
     return KRP_OK;
 }
 

@@ -26,8 +26,10 @@ struct KrpModel {
     // inside the library are indices into this padded array: ((iz+1)*py + iy+1)*px + ix+1.
     int px, py;            // padded pitches: px = nx+2, py = ny+2
     uint32_t pxy;          // px*py
+    uint32_t px_m, px_s, py_m, py_s;   // division by px, py as multiply-high + shifts (krp_fastdiv)
     float d[3];            // cell size per axis
     double lo[3], dd[3];   // lower corner and cell size in fp64 (projection to the image)
+    double inv_dd[3];      // 1/dd
     const float* kr;       // SCALAR mode: kappa*rho per padded cell
     const float4* cell;    // general mode: {kappa*rho, B^x, B^y, B^z} per padded cell
     const float4* opac;    // [n_inc] {alpha1, alpha2, alpha3, albedo} on mu_m = m/(n_inc-1)
@@ -54,12 +56,19 @@ __device__ __forceinline__ uint32_t krp_pad_id(const KrpModel& g, int ix, int iy
 {
     return ((uint32_t)(iz + 1) * (uint32_t)g.py + (uint32_t)(iy + 1)) * (uint32_t)g.px + (uint32_t)(ix + 1);
 }
+// floor(x / d) for any 32-bit x, with m = floor(2^32 (2^l - d) / d) + 1, l = ceil(log2 d), s = l - 1
+// (round-up method of Granlund & Montgomery; d >= 2 here because d is a padded pitch >= 3)
+__device__ __forceinline__ uint32_t krp_fastdiv(uint32_t x, uint32_t m, uint32_t s)
+{
+    const uint32_t t = __umulhi(x, m);
+    return (((x - t) >> 1) + t) >> s;
+}
 // padded coordinates (0..n+1 per axis) of a padded id
 __device__ __forceinline__ void krp_pad_coords(const KrpModel& g, uint32_t c, int& hx, int& hy, int& hz)
 {
-    uint32_t t = c / (uint32_t)g.px;
+    const uint32_t t = krp_fastdiv(c, g.px_m, g.px_s);
     hx = (int)(c - t * (uint32_t)g.px);
-    uint32_t z = t / (uint32_t)g.py;
+    const uint32_t z = krp_fastdiv(t, g.py_m, g.py_s);
     hy = (int)(t - z * (uint32_t)g.py);
     hz = (int)z;
 }
@@ -203,27 +212,23 @@ __device__ __forceinline__ float krp_local(float n, float r, float t, float move
 
 // Event position in fp64 without accumulated rounding: the flight started at
 // cell-local p0 (fp32 state, R12) of padded cell c0 and has its event in padded cell c, `t_len` beyond the
-// point where it entered c.  The entry path length is the largest of the per-axis path lengths to the entry
-// planes of c (slab form of the same march), each a single fp64 expression; the result is rounded to fp32 the
-// way the state is defined.
+// point where it entered c through the face of axis `axis` (-1: still in the first cell).  The entry path
+// length is a single fp64 expression, (plane - p0) d / n on that axis; the result is rounded to fp32 the way
+// the state is defined.
 __device__ __forceinline__ void krp_event_pos(const KrpModel& g, const float n[3], const float p0[3], uint32_t c0,
-                                              uint32_t c, double t_len, float pe[3])
+                                              uint32_t c, int axis, double t_len, float pe[3])
 {
     int h0[3], h[3];
     krp_pad_coords(g, c0, h0[0], h0[1], h0[2]);
     krp_pad_coords(g, c, h[0], h[1], h[2]);
-    double s_in = 0.0;
-#pragma unroll
-    for (int a = 0; a < 3; ++a) {
-        if (h[a] != h0[a]) {
-            const double plane = (double)(h[a] - h0[a]) + (n[a] > 0.f ? 0.0 : 1.0);
-            s_in = fmax(s_in, (plane - (double)p0[a]) * g.dd[a] / (double)n[a]);
-        }
+    double s = t_len;
+    if (axis >= 0) {
+        const double plane = (double)(h[axis] - h0[axis]) + (n[axis] > 0.f ? 0.0 : 1.0);
+        s += (plane - (double)p0[axis]) * g.dd[axis] / (double)n[axis];
     }
-    const double s = s_in + t_len;
 #pragma unroll
     for (int a = 0; a < 3; ++a) {
-        double x = (double)p0[a] + (double)n[a] * s / g.dd[a] - (double)(h[a] - h0[a]);
+        double x = (double)p0[a] + (double)n[a] * s * g.inv_dd[a] - (double)(h[a] - h0[a]);
         pe[a] = (float)fmin(fmax(x, 0.0), 1.0);
     }
 }

@@ -173,15 +173,46 @@ __device__ __forceinline__ void krp_event_append(const KrpModel& g, KrpCtl* ctl,
 #define KRP_FLIGHT_BURST 16
 #endif
 
+// Work distribution of the persistent flight kernels: a warp reserves KRP_FLIGHT_CHUNK consecutive queue
+// entries with one atomic and hands them to its idle lanes by rank, so the global counter sees one atomic per
+// chunk instead of one per refill.  wbase/wleft are warp-uniform.  Returns true when the calling lane got `item`.
+#ifndef KRP_FLIGHT_CHUNK
+#define KRP_FLIGHT_CHUNK 128
+#endif
+__device__ __forceinline__ bool krp_take_work(unsigned int* counter, unsigned int n_items, bool idle, unsigned int& wbase,
+                                              unsigned int& wleft, bool& more, unsigned int& item)
+{
+    const int lane = threadIdx.x & 31;
+    bool got = false;
+#pragma unroll 1
+    for (int pass = 0; pass < 2; ++pass) {
+        const unsigned want = __ballot_sync(0xffffffffu, idle && !got);
+        if (want == 0u) break;
+        if (wleft == 0u && more) {
+            unsigned int b = 0;
+            if (lane == 0) b = atomicAdd(counter, (unsigned int)KRP_FLIGHT_CHUNK);
+            b = __shfl_sync(0xffffffffu, b, 0);
+            if (b >= n_items) { more = false; }
+            else { wbase = b; wleft = min((unsigned int)KRP_FLIGHT_CHUNK, n_items - b); }
+        }
+        if (wleft == 0u) break;
+        const unsigned rank = __popc(want & ((1u << lane) - 1u));
+        if (idle && !got && rank < wleft) { item = wbase + rank; got = true; }
+        const unsigned used = min((unsigned)__popc(want), wleft);
+        wbase += used; wleft -= used;
+    }
+    return got;
+}
+
 enum { KRP_IDLE = 0, KRP_RUN = 1, KRP_HIT = 2, KRP_ESC = 3 };
 
-__global__ void __launch_bounds__(256, 4) krp_k_flight_scalar(KrpModel g, KrpCtl* ctl, KrpRecords q, int in, KrpRecords ev)
+__global__ void __launch_bounds__(256, 4) krp_k_flight_scalar(KrpModel g, KrpCtl* ctl, KrpRecords q, int in, KrpRecords ev, int n_burst)
 {
     const unsigned int n_items = ctl->q_count[in];
     KrpFlightTally tl = { 0, 0, 0, 0.0, 0.0, 0.0 };
     int status = KRP_IDLE;
     bool more = true;
-    unsigned int item = 0;
+    unsigned int item = 0, wbase = 0, wleft = 0;
     float n[3] = { 0.f, 0.f, 1.f }, p0[3] = { 0.f, 0.f, 0.f }, kr = 0.f, a1kr = 0.f;
     uint32_t c0 = 0;
     KrpRay ray = {};
@@ -196,8 +227,10 @@ __global__ void __launch_bounds__(256, 4) krp_k_flight_scalar(KrpModel g, KrpCtl
             const float4 S0 = q.S[item];
             if (status == KRP_HIT) {
                 const double moved = D / ((double)g.a1c * (double)kr);
+                // entry face of the event cell: the axis crossed last has its distance re-based to a full cell
+                const int axis = ray.c == c0 ? -1 : (ray.rx == ray.tx ? 0 : (ray.ry == ray.ty ? 1 : 2));
                 float pe[3];
-                krp_event_pos(g, n, p0, c0, ray.c, moved, pe);
+                krp_event_pos(g, n, p0, c0, ray.c, axis, moved, pe);
                 tl.steps += (unsigned long long)(crossings + 1);
                 krp_event_append(g, ctl, ev, q.id[item], ray.c, pe, n, __float_as_uint(q.nk[item].w), S0.x, g.omc,
                                  S0.y, S0.z, S0.w, tl);
@@ -207,9 +240,8 @@ __global__ void __launch_bounds__(256, 4) krp_k_flight_scalar(KrpModel g, KrpCtl
             }
             status = KRP_IDLE;
         }
-        if (status == KRP_IDLE && more) {
-            item = krp_reserve32(&ctl->work[0]);
-            if (item < n_items) {
+        if (krp_take_work(&ctl->work[0], n_items, status == KRP_IDLE, wbase, wleft, more, item)) {
+            {
                 const float4 pc = q.pc[item], nk = q.nk[item];
                 n[0] = nk.x; n[1] = nk.y; n[2] = nk.z;
                 p0[0] = pc.x; p0[1] = pc.y; p0[2] = pc.z;
@@ -219,13 +251,11 @@ __global__ void __launch_bounds__(256, 4) krp_k_flight_scalar(KrpModel g, KrpCtl
                 kr = __ldg(g.kr + ray.c);
                 a1kr = g.a1c * kr;
                 status = KRP_RUN;
-            } else {
-                more = false;
             }
         }
         if (!__any_sync(0xffffffffu, status == KRP_RUN)) break;
 #pragma unroll 1
-        for (int burst = 0; burst < KRP_FLIGHT_BURST; ++burst) {
+        for (int burst = 0; burst < n_burst; ++burst) {
             if (status == KRP_RUN) {
                 const float ds = krp_ray_ds(ray);
                 const float dt1 = a1kr * ds;
@@ -240,6 +270,47 @@ __global__ void __launch_bounds__(256, 4) krp_k_flight_scalar(KrpModel g, KrpCtl
                 }
             }
         }
+    }
+    krp_tally_flush(tl, ctl);
+}
+
+// The same flight with a static assignment (one queue entry per thread and grid stride, the warp's 32 flights
+// start and are closed together): no refill logic at all.  Cheaper when flights are short (C2: a point source
+// inside a dense ring, most flights end within a few cells), selected with flight_burst = 1.
+__global__ void __launch_bounds__(256, 4) krp_k_flight_scalar_static(KrpModel g, KrpCtl* ctl, KrpRecords q, int in, KrpRecords ev)
+{
+    const unsigned int n_items = ctl->q_count[in];
+    KrpFlightTally tl = { 0, 0, 0, 0.0, 0.0, 0.0 };
+    for (unsigned int item = blockIdx.x * blockDim.x + threadIdx.x; item < n_items; item += gridDim.x * blockDim.x) {
+        const float4 pc = q.pc[item], nk = q.nk[item], S0 = q.S[item];
+        const float n[3] = { nk.x, nk.y, nk.z };
+        const float p0[3] = { pc.x, pc.y, pc.z };
+        const uint32_t c0 = __float_as_uint(pc.w);
+        KrpRay ray;
+        krp_ray_init(g, c0, p0, n, ray);
+        double D = q.tau[item];
+        bool hit = false;
+        float kr = __ldg(g.kr + ray.c);
+        for (;;) {
+            const float ds = krp_ray_ds(ray);
+            const float dt1 = g.a1c * kr * ds;
+            if ((double)dt1 >= D) { hit = true; break; }      // event inside this cell
+            D -= (double)dt1;
+            krp_ray_step(ray, ds);
+            kr = __ldg(g.kr + ray.c);
+            if (kr < 0.f) break;                               // halo: the packet left the grid
+        }
+        int h0[3], h1[3];
+        krp_pad_coords(g, c0, h0[0], h0[1], h0[2]);
+        krp_pad_coords(g, ray.c, h1[0], h1[1], h1[2]);
+        const int crossings = abs(h1[0] - h0[0]) + abs(h1[1] - h0[1]) + abs(h1[2] - h0[2]);
+        if (!hit) { tl.steps += (unsigned long long)crossings; tl.w_esc += (double)S0.x; continue; }
+        tl.steps += (unsigned long long)(crossings + 1);
+        const double moved = D / ((double)g.a1c * (double)kr);
+        const int axis = ray.c == c0 ? -1 : (ray.rx == ray.tx ? 0 : (ray.ry == ray.ty ? 1 : 2));
+        float pe[3];
+        krp_event_pos(g, n, p0, c0, ray.c, axis, moved, pe);
+        krp_event_append(g, ctl, ev, q.id[item], ray.c, pe, n, __float_as_uint(nk.w), S0.x, g.omc, S0.y, S0.z, S0.w, tl);
     }
     krp_tally_flush(tl, ctl);
 }
@@ -304,7 +375,7 @@ __device__ __forceinline__ void krp_cell_coef(const KrpModel& g, const float4 cl
     c.dt1 = c.a1 * c.dtau;
 }
 
-__global__ void __launch_bounds__(256, 2) krp_k_flight_general(KrpModel g, KrpCtl* ctl, KrpRecords q, int in, KrpRecords ev)
+__global__ void __launch_bounds__(256, 2) krp_k_flight_general(KrpModel g, KrpCtl* ctl, KrpRecords q, int in, KrpRecords ev, int n_burst)
 {
     const unsigned int n_items = ctl->q_count[in];
     KrpFlightTally tl = { 0, 0, 0, 0.0, 0.0, 0.0 };
@@ -312,7 +383,7 @@ __global__ void __launch_bounds__(256, 2) krp_k_flight_general(KrpModel g, KrpCt
     const float guard = 1.f + g.rho + 1e-3f;
     int status = KRP_IDLE;
     bool more = true;
-    unsigned int item = 0;
+    unsigned int item = 0, wbase = 0, wleft = 0;
     // state of the flight in progress
     float n[3] = { 0.f, 0.f, 1.f }, p0[3] = { 0.f, 0.f, 0.f }, th[3] = { 0.f, 0.f, 0.f }, ph[3] = { 0.f, 0.f, 0.f };
     double nd[3] = { 0.0, 0.0, 1.0 }, inv_n = 1.0, D = 0.0, i = 1.0;
@@ -366,9 +437,8 @@ __global__ void __launch_bounds__(256, 2) krp_k_flight_general(KrpModel g, KrpCt
             tl.w_esc += (double)q.S[item].x;
             status = KRP_IDLE;
         }
-        if (status == KRP_IDLE && more) {
-            item = krp_reserve32(&ctl->work[0]);
-            if (item < n_items) {
+        if (krp_take_work(&ctl->work[0], n_items, status == KRP_IDLE, wbase, wleft, more, item)) {
+            {
                 const float4 pc = q.pc[item], nk = q.nk[item], S0 = q.S[item];
                 n[0] = nk.x; n[1] = nk.y; n[2] = nk.z;
                 p0[0] = pc.x; p0[1] = pc.y; p0[2] = pc.z;
@@ -382,13 +452,11 @@ __global__ void __launch_bounds__(256, 2) krp_k_flight_general(KrpModel g, KrpCt
                 qs = S0.y; us = S0.z; vs = S0.w;      // lab reference
                 Asum = 0.f; tau0f = (float)tau0; nsteps = 0;
                 status = KRP_RUN;
-            } else {
-                more = false;
             }
         }
         if (!__any_sync(0xffffffffu, status == KRP_RUN)) break;
 #pragma unroll 1
-        for (int burst = 0; burst < KRP_FLIGHT_BURST; ++burst) {
+        for (int burst = 0; burst < n_burst; ++burst) {
             if (status != KRP_RUN) continue;
             const double ds = krp_rayd_ds(ray);
             ++nsteps;

@@ -90,7 +90,7 @@ def lib():
         "krp_stats_reset": (i32, [vp, vp]),
         "krp_events_get": (i32, [vp, u64, C.POINTER(u64), vp, vp, vp, vp, vp, vp]),
         "krp_events_clear": (i32, [vp, vp]),
-        "krp_tune": (i32, [vp, i32, i32, i32]),
+        "krp_tune": (i32, [vp, i32, i32, i32, i32]),
         "krp_launch_count": (u64, [vp]),
     }
     for name, (res, args) in sig.items():
@@ -244,8 +244,8 @@ class Grid:
     def events_clear(self, stream=None):
         _check(lib().krp_events_clear(self._h, _stream(stream)))
 
-    def tune(self, transport_block=0, image_block=0, blocks_per_sm=0):
-        _check(lib().krp_tune(self._h, int(transport_block), int(image_block), int(blocks_per_sm)))
+    def tune(self, transport_block=0, image_block=0, blocks_per_sm=0, flight_burst=0):
+        _check(lib().krp_tune(self._h, int(transport_block), int(image_block), int(blocks_per_sm), int(flight_burst)))
 
     def launch_count(self):
         return int(lib().krp_launch_count(self._h))
