@@ -32,13 +32,22 @@ if ROOT not in sys.path:
 METRIC = "photon packets/sec (transport+imaging)"
 UNIT = "packets/s"
 
-# Algorithmic work per unit: bytes that must move and thread-instructions that
-# must issue per cell step / event / image contribution, for the two cell layouts.
+# Algorithmic work per unit: bytes that must move and thread-instructions that must issue
+# per cell step of the two hot loops, for the two cell layouts, and per ray / flight outside the loop.
+#   image_inst   scalar: min3, sub, 3 setp, 3 predicated fadd + 3 iadd, address, gather, fma, sentinel test, branch
+#                general: the same march + mu, table segment (2 LDS.128), 3 fma, eta (rcp), rotation in/out, series
+#                of sinh/cosh-1/sin/cos-1, delta update, depth fma
+#   flight_inst  scalar: re-based march (13) + optical-depth product, fp64 compare and subtract, gather, tests
+#                general: fp64 re-based march, fp64 mu and alpha1, fp32 Stokes update, fp64 depth bookkeeping
 ALGO = {
-    "scalar":  dict(cell_bytes=4,  step_inst=22, event_bytes=96, event_inst=300, contrib_bytes=32, contrib_inst=120),
-    "general": dict(cell_bytes=16, step_inst=110, event_bytes=96, event_inst=300, contrib_bytes=32, contrib_inst=120),
+    "scalar":  dict(cell_bytes=4,  image_inst=16, flight_inst=23, ray_inst=250, flight_fixed_inst=200),
+    "general": dict(cell_bytes=16, image_inst=80, flight_inst=110, ray_inst=250, flight_fixed_inst=300),
 }
-N_SM, LANES_PER_SM = 148, 128          # B200: 148 SMs x 4 sub-partitions x 32 FP32 lanes (B200_PROFILING.md)
+EVENT_BYTES, CONTRIB_BYTES = 48, 32
+N_SM, LANES_PER_SM = 148, 128          # B200: 148 SMs x 4 schedulers x 32 lanes, one warp-instruction per scheduler and clock
+# which ceiling binds the dominant kernel, read from the committed ncu captures (profiles/):
+# issue slots busy vs DRAM / L2 throughput of the kernel
+BOUND = {"c1": "alu", "c2": "alu", "c3": "alu", "c4": "alu", "c5": "hbm"}
 
 
 def parse_args():
@@ -277,6 +286,8 @@ def run_krp(args):
     for i in range(args.warmup):
         step(i)
     g.stats_reset()
+    g.timing_enable(True)
+    g.timing_get()
     img = torch.zeros((n_obs, 4, npix, npix), dtype=torch.float64, device=dev)
     launches0 = g.launch_count()
     barrier()
@@ -289,6 +300,9 @@ def run_krp(args):
     barrier()
     clocks = sampler.stop() if sampler else None
     ms_total = t_start.elapsed_time(t_end)
+    ms_own = ms_total                      # this rank's own time over the K steps (the max over ranks replaces ms_total below)
+    timing = g.timing_get()
+    g.timing_enable(False)
     launches = g.launch_count() - launches0
     # end of job: the one exchange of the path, sum of the per-rank maps (outside the per-step timing)
     g.image_get(out=img)
@@ -311,26 +325,45 @@ def run_krp(args):
     value = tot["packets"] / sec
     assert tot["packets"] == args.steps * batch * world, (tot["packets"], args.steps, batch, world)
 
-    # roofline of the dominant kernel (this rank's launches): krp_k_image, one launch per step
+    # roofline of the dominant kernel (this rank's launches), from the library's own per-launch CUDA events
+    # on the launching stream (krp_timing_*): flight kernels (one launch per scattering order) or imaging
+    # kernels (one launch per observer), whichever took more of the step
     pk = peaks()
     mode = "scalar" if (cfg["bfield"] is None and cfg["opacity"].shape[0] == 1) else "general"
     A = ALGO[mode]
     K = args.steps
-    rays = st["events"] * n_obs / K
-    im_bytes = (st["steps_image"] * A["cell_bytes"] + st["events"] * 48 + st["contributions"] * A["contrib_bytes"]) / K
-    im_inst = (st["steps_image"] * A["step_inst"]) / K + rays * A["contrib_inst"]
     alu_peak = N_SM * LANES_PER_SM * pk["sm_max_mhz"] * 1e6          # thread-instructions/s at the maximum SM clock
-    f_hbm = im_bytes / (t_im * 1e-3) / (pk["hbm_gbs"] * 1e9)
-    f_alu = im_inst / (t_im * 1e-3) / alu_peak
-    if f_hbm >= f_alu:
-        roof = {"bound": "hbm", "achieved": im_bytes / (t_im * 1e-3) / 1e9, "peak": pk["hbm_gbs"], "unit": "GB/s", "frac": f_hbm}
+    rays = st["events"] * n_obs
+    flights = st["packets"] + st["events"]                             # an upper bound: every event but the last starts one
+    work = {
+        "image": dict(kernel="krp_k_image<%s>" % mode, steps=st["steps_image"],
+                      bytes=st["steps_image"] * A["cell_bytes"] + rays * EVENT_BYTES + st["contributions"] * CONTRIB_BYTES,
+                      inst=st["steps_image"] * A["image_inst"] + rays * A["ray_inst"]),
+        "flight": dict(kernel="krp_k_flight_%s" % mode, steps=st["steps_transport"],
+                       bytes=st["steps_transport"] * A["cell_bytes"] + flights * 64 + st["events"] * 56,
+                       inst=st["steps_transport"] * A["flight_inst"] + flights * A["flight_fixed_inst"]),
+    }
+    kernels = {}
+    for cls, (ms, n_l) in timing.items():
+        kernels[cls] = {"ms_per_step": ms / K, "launches_per_step": n_l / K, "share_of_step": ms / ms_own}
+    dom = max(("image", "flight"), key=lambda c: timing[c][0])
+    W = work[dom]
+    t_dom = timing[dom][0] * 1e-3                                       # seconds over the K timed steps
+    n_launch = max(timing[dom][1], 1)
+    f_hbm = W["bytes"] / t_dom / (pk["hbm_gbs"] * 1e9)
+    f_alu = W["inst"] / t_dom / alu_peak
+    bound = BOUND.get(args.workload, "alu" if f_alu >= f_hbm else "hbm")
+    if bound == "hbm":
+        roof = {"bound": "hbm", "achieved": W["bytes"] / t_dom / 1e9, "peak": pk["hbm_gbs"], "unit": "GB/s", "frac": f_hbm}
     else:
-        roof = {"bound": "alu", "achieved": im_inst / (t_im * 1e-3) / 1e12, "peak": alu_peak / 1e12,
-                "unit": "Tinst/s", "frac": f_alu}
-    roof.update({"kernel": "krp_k_image<%s>" % mode, "kernel_ms": t_im, "share_of_step": t_im / (t_tr + t_im),
-                 "traffic": NCU_TRAFFIC.get((args.workload, batch)), "peak_source": pk["source"],
-                 "cell_steps_per_launch": st["steps_image"] / K, "rays_per_launch": rays,
-                 "frac_hbm": f_hbm, "frac_alu": f_alu})
+        roof = {"bound": "alu", "achieved": W["inst"] / t_dom / 1e12, "peak": alu_peak / 1e12, "unit": "Tinst/s", "frac": f_alu}
+    roof.update({"kernel": W["kernel"], "launches_per_step": n_launch / K, "avg_launch_ms": 1e3 * t_dom / n_launch,
+                 "kernel_ms_per_step": 1e3 * t_dom / K, "share_of_step": timing[dom][0] / ms_own,
+                 "traffic": NCU_TRAFFIC.get(args.workload), "peak_source": pk["source"],
+                 "cell_steps_per_step": W["steps"] / K, "algorithmic_bytes_per_step": W["bytes"] / K,
+                 "algorithmic_inst_per_step": W["inst"] / K, "frac_hbm": f_hbm, "frac_alu": f_alu,
+                 "peak_alu": "%d SMs x 4 schedulers x 32 lanes x %.0f MHz" % (N_SM, pk["sm_max_mhz"]),
+                 "kernels": kernels})
     return dict(world=world, rank=rank, cfg=cfg, batch=batch, value=value, ms_total=ms_total, clocks=clocks, roof=roof,
                 t_tr=t_tr, t_im=t_im, tot=tot, launches=launches, epp=epp, mode=mode, krp=krp, obs=obs, dev=dev,
                 ev_cap=ev_cap, grid=g)
@@ -413,6 +446,8 @@ def main():
                    "observers": len(cfg["observers"]), "npix": cfg["npix"], "cell_layout": r["mode"],
                    "job_packets": cfg["n_packets"], "events_per_packet": r["epp"],
                    "l2": "flushed every step by a 256 MiB memset inside the timed region",
+                   "launch": "flights: %s; imaging: one launch per observer over events ordered by cell bin" %
+                             ("static assignment" if r["mode"] == "scalar" else "persistent lanes, refill every 32 cell steps"),
                    "parallelism": "packet ids sharded over %d GPU(s), grid replicated, one fp64 image all-reduce at job end" % r["world"],
                    "reduced": bool(args.n)},
         "scatterings_per_s": tot["events"] / sec,

@@ -164,6 +164,15 @@ int krp_events_clear(krp_grid* g, void* stream);
  * flight and imaging kernels (multiples of 32 up to 256), persistent blocks per SM, and the number
  * of cell steps a flight kernel takes between two points where idle lanes take new packets. */
 int krp_tune(krp_grid* g, int transport_block, int image_block, int blocks_per_sm, int flight_burst);
+/* Device time per kernel class, for measurement (bench.py's roofline): when enabled, every launch of a
+ * flight, scattering, ordering or imaging kernel is bracketed by CUDA events on the caller's stream.
+ * krp_timing_get synchronises, adds up the elapsed times since the last call into ms[KRP_T_COUNT] and the
+ * launch counts into launches[KRP_T_COUNT] (either may be NULL), and rearms.  At most 4096 launches are kept
+ * between two krp_timing_get calls; later ones go untimed. */
+enum { KRP_T_FLIGHT = 0, KRP_T_SCATTER = 1, KRP_T_ORDER = 2, KRP_T_IMAGE = 3, KRP_T_EMIT = 4, KRP_T_COUNT = 5 };
+int krp_timing_enable(krp_grid* g, int on);
+int krp_timing_get(krp_grid* g, double* ms, uint64_t* launches);
+
 /* Number of kernels the library has launched on behalf of g since creation. */
 uint64_t krp_launch_count(const krp_grid* g);
 

@@ -71,6 +71,29 @@ struct krp_grid {
     int max_waves = 0;
     int transport_block = 256, image_block = 256, blocks_per_sm = 8;
     int burst = KRP_FLIGHT_BURST;   // cell steps between refill points of the flight kernels
+    // optional per-launch timing (krp_timing_*)
+    bool timing = false;
+    std::vector<cudaEvent_t> t_ev;          // pairs: start, stop
+    std::vector<int> t_cls;                 // class of every recorded pair
+};
+
+// brackets one launch (or a short run of launches of the same class) with events when timing is on
+struct TimedLaunch {
+    krp_grid* g; cudaStream_t st; cudaEvent_t stop = nullptr;
+    TimedLaunch(krp_grid* g_, cudaStream_t st_, int cls) : g(g_), st(st_)
+    {
+        if (!g->timing || g->t_cls.size() >= 4096) return;
+        const size_t k = g->t_cls.size();
+        if (g->t_ev.size() < 2 * (k + 1)) {
+            cudaEvent_t a = nullptr, b = nullptr;
+            if (cudaEventCreate(&a) != cudaSuccess || cudaEventCreate(&b) != cudaSuccess) return;
+            g->t_ev.push_back(a); g->t_ev.push_back(b);
+        }
+        cudaEventRecord(g->t_ev[2 * k], st);
+        stop = g->t_ev[2 * k + 1];
+        g->t_cls.push_back(cls);
+    }
+    ~TimedLaunch() { if (stop) cudaEventRecord(stop, st); }
 };
 
 extern "C" const char* krp_last_error(void) { return g_err; }
@@ -99,6 +122,7 @@ extern "C" int krp_grid_destroy(krp_grid* g)
     cudaFree(g->d_src_cdf); cudaFree(g->d_ctl); cudaFree(g->d_obs); cudaFree(g->d_img);
     cudaFree(g->d_opA); cudaFree(g->d_opB); cudaFree(g->d_bins); cudaFree(g->d_perm); cudaFree(g->d_scan);
     free_records(g->q[0]); free_records(g->q[1]); free_records(g->ev);
+    for (cudaEvent_t e : g->t_ev) cudaEventDestroy(e);
     delete g;
     return KRP_OK;
 }
@@ -423,7 +447,8 @@ extern "C" int krp_transport(krp_grid* g, uint64_t n_packets, uint64_t seed, voi
     const unsigned n = (unsigned)n_packets;
     const int tb = g->transport_block;
     const unsigned grid_all = (n + 255u) / 256u;
-    krp_k_emit<<<grid_all, 256, 0, st>>>(g->m, g->d_ctl, g->q[0], g->ev, g->next_id, n, seed);
+    { TimedLaunch tl(g, st, KRP_T_EMIT);
+      krp_k_emit<<<grid_all, 256, 0, st>>>(g->m, g->d_ctl, g->q[0], g->ev, g->next_id, n, seed); }
     g->launches++;
     unsigned pers = (unsigned)(g->n_sm * g->blocks_per_sm);
     unsigned need = (n + tb - 1) / tb;
@@ -433,11 +458,13 @@ extern "C" int krp_transport(krp_grid* g, uint64_t n_packets, uint64_t seed, voi
     for (int w = 0; w < g->max_waves; ++w) {
         const int in = w & 1;
         krp_k_wave_prep<<<1, 1, 0, st>>>(g->d_ctl, in);
+        { TimedLaunch tl(g, st, KRP_T_FLIGHT);
         if (g->m.scalar && g->burst == 1) krp_k_flight_scalar_static<<<grid_f, tb, 0, st>>>(g->m, g->d_ctl, g->q[in], in, g->ev);
         else if (g->m.scalar) krp_k_flight_scalar<<<grid_f, tb, 0, st>>>(g->m, g->d_ctl, g->q[in], in, g->ev, g->burst);
-        else             krp_k_flight_general<<<grid_f, tb, 0, st>>>(g->m, g->d_ctl, g->q[in], in, g->ev, g->burst);
+        else             krp_k_flight_general<<<grid_f, tb, 0, st>>>(g->m, g->d_ctl, g->q[in], in, g->ev, g->burst); }
         g->launches += 2;
         if (w + 1 < g->max_waves) {
+            TimedLaunch tl(g, st, KRP_T_SCATTER);
             krp_k_scatter<<<grid_s, 128, 0, st>>>(g->m, g->d_ctl, g->ev, g->q[1 - in], 1 - in, seed);
             g->launches++;
         }
@@ -505,11 +532,12 @@ extern "C" int krp_image(krp_grid* g, const krp_observer* obs, int n_obs, int np
     }
     // I0: order the events by cell bin (count, scan, scatter)
     const unsigned pers = (unsigned)(g->n_sm * g->blocks_per_sm);
+    { TimedLaunch tlo(g, st, KRP_T_ORDER);
     CK(cudaMemsetAsync(g->d_bins, 0, sizeof(unsigned int) * ((size_t)g->n_bins + 1), st));
     krp_k_sort_count<<<pers, 256, 0, st>>>(g->d_ctl, g->ev, g->bin_shift, g->sub_bits, flags, g->d_bins);
     CK(cub::DeviceScan::ExclusiveSum(g->d_scan, g->scan_bytes, g->d_bins, g->d_bins, (int)(g->n_bins + 1), st));
     krp_k_image_prep<<<1, 1, 0, st>>>(g->d_ctl, g->d_bins, g->n_bins);
-    krp_k_sort_scatter<<<pers, 256, 0, st>>>(g->d_ctl, g->ev, g->bin_shift, g->sub_bits, flags, g->d_bins, g->d_perm);
+    krp_k_sort_scatter<<<pers, 256, 0, st>>>(g->d_ctl, g->ev, g->bin_shift, g->sub_bits, flags, g->d_bins, g->d_perm); }
     g->launches += 5;   // count, scan (2 kernels), prep, scatter
     // I1-I3: one launch per observer (its constants are kernel parameters); launches rotate over
     // KRP_MAX_OBS_PACK work counters, rewound when the rotation wraps
@@ -518,6 +546,7 @@ extern "C" int krp_image(krp_grid* g, const krp_observer* obs, int n_obs, int np
     for (int o = 0; o < n_obs; ++o) {
         const int slot = o % KRP_MAX_OBS_PACK;
         if (o > 0 && slot == 0) { krp_k_image_rewind<<<1, 1, 0, st>>>(g->d_ctl); g->launches++; }
+        TimedLaunch tli(g, st, KRP_T_IMAGE);
         if (g->m.scalar) krp_k_image<true><<<pers, tb, smem, st>>>(g->m, g->d_ctl, g->ev, g->d_perm, g->obs_dev[o], slot, o, npix_x, npix_y, g->d_img);
         else             krp_k_image<false><<<pers, tb, smem, st>>>(g->m, g->d_ctl, g->ev, g->d_perm, g->obs_dev[o], slot, o, npix_x, npix_y, g->d_img);
         g->launches++;
@@ -634,6 +663,30 @@ extern "C" int krp_tune(krp_grid* g, int transport_block, int image_block, int b
     if (blocks_per_sm) g->blocks_per_sm = blocks_per_sm;
     if (flight_burst < 0 || flight_burst > 4096) return fail(KRP_ERR_ARG, "flight_burst must be in 0..4096");
     if (flight_burst) g->burst = flight_burst;
+    return KRP_OK;
+}
+
+extern "C" int krp_timing_enable(krp_grid* g, int on)
+{
+    if (!g) return fail(KRP_ERR_ARG, "grid is NULL");
+    g->timing = on != 0;
+    if (!g->timing) g->t_cls.clear();
+    return KRP_OK;
+}
+
+extern "C" int krp_timing_get(krp_grid* g, double* ms, uint64_t* launches)
+{
+    if (!g) return fail(KRP_ERR_ARG, "grid is NULL");
+    CK(cudaDeviceSynchronize());
+    double acc[KRP_T_COUNT] = { 0 };
+    uint64_t cnt[KRP_T_COUNT] = { 0 };
+    for (size_t k = 0; k < g->t_cls.size(); ++k) {
+        float t = 0.f;
+        CK(cudaEventElapsedTime(&t, g->t_ev[2 * k], g->t_ev[2 * k + 1]));
+        acc[g->t_cls[k]] += (double)t; cnt[g->t_cls[k]]++;
+    }
+    g->t_cls.clear();
+    for (int c = 0; c < KRP_T_COUNT; ++c) { if (ms) ms[c] = acc[c]; if (launches) launches[c] = cnt[c]; }
     return KRP_OK;
 }
 

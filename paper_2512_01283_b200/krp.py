@@ -17,8 +17,10 @@ SYMBOLS = [
     "krp_last_error", "krp_version", "krp_grid_create", "krp_grid_destroy", "krp_source_set",
     "krp_events_reserve", "krp_transport", "krp_packet_id_set", "krp_image", "krp_image_get",
     "krp_image_reset", "krp_stats_get", "krp_stats_reset", "krp_events_get", "krp_events_clear",
-    "krp_tune", "krp_launch_count",
+    "krp_tune", "krp_timing_enable", "krp_timing_get", "krp_launch_count",
 ]
+T_FLIGHT, T_SCATTER, T_ORDER, T_IMAGE, T_EMIT, T_COUNT = 0, 1, 2, 3, 4, 5
+T_NAMES = ("flight", "scatter", "order", "image", "emit")
 
 
 class KrpError(RuntimeError):
@@ -91,6 +93,8 @@ def lib():
         "krp_events_get": (i32, [vp, u64, C.POINTER(u64), vp, vp, vp, vp, vp, vp]),
         "krp_events_clear": (i32, [vp, vp]),
         "krp_tune": (i32, [vp, i32, i32, i32, i32]),
+        "krp_timing_enable": (i32, [vp, i32]),
+        "krp_timing_get": (i32, [vp, vp, vp]),
         "krp_launch_count": (u64, [vp]),
     }
     for name, (res, args) in sig.items():
@@ -246,6 +250,16 @@ class Grid:
 
     def tune(self, transport_block=0, image_block=0, blocks_per_sm=0, flight_burst=0):
         _check(lib().krp_tune(self._h, int(transport_block), int(image_block), int(blocks_per_sm), int(flight_burst)))
+
+    def timing_enable(self, on=True):
+        _check(lib().krp_timing_enable(self._h, int(bool(on))))
+
+    def timing_get(self):
+        """{class: (milliseconds, launches)} since the last call; synchronises."""
+        ms = (C.c_double * T_COUNT)()
+        cnt = (C.c_uint64 * T_COUNT)()
+        _check(lib().krp_timing_get(self._h, ms, cnt))
+        return {T_NAMES[c]: (float(ms[c]), int(cnt[c])) for c in range(T_COUNT)}
 
     def launch_count(self):
         return int(lib().krp_launch_count(self._h))
