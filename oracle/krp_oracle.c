@@ -10,7 +10,7 @@
  * tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference
  * legs may build, load or call it.
  *
- * Precision: fp64 everywhere, with four deliberate fp32 quantisations that
+ * Precision: fp64 everywhere, with five deliberate fp32 quantisations that
  * are part of the method's *state definition* (R12), made so that
  * integer decisions (which cell an event falls in) are taken on the same
  * numbers by both implementations:
@@ -20,7 +20,10 @@
  *     after every scattering;
  *   - the cell-local position of a packet is stored rounded to fp32 at
  *     emission and at every event (the event record holds fp32 positions and
- *     the next flight starts from the record).
+ *     the next flight starts from the record);
+ *   - the normalised Stokes components (q,u,v) are stored rounded to fp32 at
+ *     every event and after every scattering (the 48-byte event record and the
+ *     packet queue hold fp32 Stokes vectors).
  *
  * Pins (tests/test_oracle_pins.py, -m "not gpu"): every exported function
  * below is pinned to a closed form, an invariant, a library routine
@@ -649,6 +652,7 @@ int64_t ora_transport(const ora_model* m, uint64_t id0, uint64_t n_packets, uint
                 break;
             }
             ++k;
+            for (int s = 1; s < 4; ++s) S[s] = (double)(float)S[s];              /* R12: event record state */
             int64_t c = cell_of(m, idx);
             double b[3], a[4];
             cell_bhat(m, c, b);
@@ -662,7 +666,7 @@ int64_t ora_transport(const ora_model* m, uint64_t id0, uint64_t n_packets, uint
             double n2[3], S2[4];
             ora_scatter(m, b, n, S, seed, id, (uint32_t)k, n2, S2, &tau_star);
             for (int a2 = 0; a2 < 3; ++a2) n[a2] = n2[a2];
-            for (int s = 0; s < 4; ++s) S[s] = S2[s];
+            for (int s = 0; s < 4; ++s) S[s] = (double)(float)S2[s];             /* R12: queue state */
         }
     }
     return nesc;

@@ -350,12 +350,15 @@ __device__ __forceinline__ double krp_rsqrt_near1(double vv)
 // decides in which cell the event falls -- segment lengths, alpha1(mu), the scalar depth D and the
 // normalised intensity i -- is carried in fp64 (an integer decided by
 // floating point is taken in the oracle's precision; in a clumpy medium a difference in the last
-// bit of an event position is amplified by the density contrast at every later scattering); the
-// Stokes algebra (reference rotation, sinh/cosh/sin/cos factors, q,u,v) is fp32.
+// bit of an event position is amplified by the density contrast at every later scattering).  That
+// includes the Stokes vector: i depends on the grain-frame Q of every cell crossed, and in optically
+// thin cells (C5 at 512^3: kappa*rho*dx ~ 0.02) an error of 1e-10 in ln i moves the event by an fp32
+// ulp of the cell-local coordinate, so q,u,v and the reference rotation are fp64 here too (the
+// imaging march, which decides no integer but the pixel, is fp32).
 // ------------------------------------------------------------------------------------------
 struct KrpCellCoef {
-    double a1, dtau, dt1;      // alpha1(mu), kappa*rho*ds, alpha1*kappa*rho*ds
-    float a2, a3, omega;       // alpha2(mu), alpha3(mu), albedo(mu)
+    double a1, a2, a3, dtau, dt1;   // alpha_i(mu), kappa*rho*ds, alpha1*kappa*rho*ds
+    float omega;                    // albedo(mu)
 };
 
 __device__ __forceinline__ void krp_cell_coef(const KrpModel& g, const float4 cl, const double nd[3], double inv_n, double xs,
@@ -366,13 +369,76 @@ __device__ __forceinline__ void krp_cell_coef(const KrpModel& g, const float4 cl
     mu = fmin(mu, 1.0);
     const double x = mu * xs;
     const int j = min((int)x, g.n_inc - 2);
-    const double w = x - (double)j;
+    const double w = x - (double)j, w0 = 1.0 - w;
     const float4 oa = g.opac[j], ob = g.opac[j + 1];
-    c.a1 = (1.0 - w) * (double)oa.x + w * (double)ob.x;
-    const float wf = (float)w, w0f = 1.f - wf;
-    c.a2 = w0f * oa.y + wf * ob.y; c.a3 = w0f * oa.z + wf * ob.z; c.omega = w0f * oa.w + wf * ob.w;
+    c.a1 = w0 * (double)oa.x + w * (double)ob.x;
+    c.a2 = w0 * (double)oa.y + w * (double)ob.y;
+    c.a3 = w0 * (double)oa.z + w * (double)ob.z;
+    c.omega = (float)(w0 * (double)oa.w + w * (double)ob.w);
     c.dtau = (double)cl.x * ds;
     c.dt1 = c.a1 * c.dtau;
+}
+
+// sinh(x), cosh(x)-1 and sin(y), cos(y)-1 in fp64 for |x|, |y| < 0.35: Taylor series to x^15 / x^16 (remainder < 1e-19)
+__device__ __forceinline__ void krp_sinh_coshm1_d(double x, double& sh, double& chm1)
+{
+    const double z = x * x;
+    sh = x * (1.0 + z * (1.0 / 6 + z * (1.0 / 120 + z * (1.0 / 5040 + z * (1.0 / 362880 + z * (1.0 / 39916800 +
+         z * (1.0 / 6227020800.0 + z * (1.0 / 1307674368000.0))))))));
+    chm1 = z * (0.5 + z * (1.0 / 24 + z * (1.0 / 720 + z * (1.0 / 40320 + z * (1.0 / 3628800 + z * (1.0 / 479001600 +
+           z * (1.0 / 87178291200.0 + z * (1.0 / 20922789888000.0))))))));
+}
+__device__ __forceinline__ void krp_sin_cosm1_d(double y, double& sy, double& cym1)
+{
+    const double z = y * y;
+    sy = y * (1.0 - z * (1.0 / 6 - z * (1.0 / 120 - z * (1.0 / 5040 - z * (1.0 / 362880 - z * (1.0 / 39916800 -
+         z * (1.0 / 6227020800.0 - z * (1.0 / 1307674368000.0))))))));
+    cym1 = -z * (0.5 - z * (1.0 / 24 - z * (1.0 / 720 - z * (1.0 / 40320 - z * (1.0 / 3628800 - z * (1.0 / 479001600 -
+           z * (1.0 / 87178291200.0 - z * (1.0 / 20922789888000.0))))))));
+}
+
+// Source-free App. A step over the whole cell on the grain-frame state (i, qg, ug, v), fp64, with the common factor
+// e^{-alpha1 dtau} (thin) or e^{-(alpha1 - |alpha2|) dtau} (thick) left to the scalar depth; `depth` is what the
+// scalar depth grows by.
+__device__ __forceinline__ void krp_appA_d(double i, double qg, double ug, double v, const KrpCellCoef& c,
+                                           double& i_n, double& qg_n, double& ug_n, double& v_n, double& depth)
+{
+    const double x = c.a2 * c.dtau, y = c.a3 * c.dtau;
+    double sy, cym1;
+    if (fabs(y) < 0.35) krp_sin_cosm1_d(y, sy, cym1);
+    else { double cy; sincos(y, &sy, &cy); cym1 = cy - 1.0; }
+    const double un = ug + (ug * cym1 - v * sy), vn = v + (ug * sy + v * cym1);
+    if (fabs(x) < 0.35) {
+        double sh, chm1;
+        krp_sinh_coshm1_d(x, sh, chm1);
+        i_n = i + (i * chm1 - qg * sh);
+        qg_n = qg + (qg * chm1 - i * sh);
+        ug_n = un; v_n = vn;
+        depth = c.dt1;
+    } else {
+        // thick cell: factor e^{-|alpha2 dtau|} moved into the scalar depth (no overflow at dtau ~ 1e3)
+        const double ax = fabs(x), E = exp(-2.0 * ax), sg = x > 0.0 ? 1.0 : -1.0, f = exp(-ax);
+        i_n = 0.5 * ((i - sg * qg) + (i + sg * qg) * E);
+        qg_n = 0.5 * ((qg - sg * i) + (qg + sg * i) * E);
+        ug_n = f * un; v_n = f * vn;
+        depth = c.dt1 - ax;
+    }
+}
+
+// the same evolved to depth t inside the cell, thin or thick, normalised to I = 1 (R7)
+__device__ __forceinline__ void krp_appA_to_d(double i, double qg, double ug, double v, double a2, double a3, double t,
+                                              double& qt, double& ut, double& vt)
+{
+    const double x = a2 * t, y = a3 * t;
+    double sy, cy, sh, ch;
+    sincos(y, &sy, &cy);
+    if (fabs(x) < 0.35) { double chm1; krp_sinh_coshm1_d(x, sh, chm1); ch = 1.0 + chm1; }
+    else { sh = sinh(x); ch = cosh(x); }
+    const double it = i * ch - qg * sh;
+    const double inv = 1.0 / it;
+    qt = (qg * ch - i * sh) * inv;
+    ut = (ug * cy - v * sy) * inv;
+    vt = (ug * sy + v * cy) * inv;
 }
 
 __global__ void __launch_bounds__(256, 2) krp_k_flight_general(KrpModel g, KrpCtl* ctl, KrpRecords q, int in, KrpRecords ev, int n_burst)
@@ -384,10 +450,10 @@ __global__ void __launch_bounds__(256, 2) krp_k_flight_general(KrpModel g, KrpCt
     int status = KRP_IDLE;
     bool more = true;
     unsigned int item = 0, wbase = 0, wleft = 0;
-    // state of the flight in progress
-    float n[3] = { 0.f, 0.f, 1.f }, p0[3] = { 0.f, 0.f, 0.f }, th[3] = { 0.f, 0.f, 0.f }, ph[3] = { 0.f, 0.f, 0.f };
-    double nd[3] = { 0.0, 0.0, 1.0 }, inv_n = 1.0, D = 0.0, i = 1.0;
-    float qs = 0.f, us = 0.f, vs = 0.f, Asum = 0.f, tau0f = 0.f;
+    // state of the flight in progress (all fp64: it decides where the event falls)
+    double nd[3] = { 0.0, 0.0, 1.0 }, th[3] = { 0.0, 0.0, 0.0 }, ph[3] = { 0.0, 0.0, 0.0 };
+    double inv_n = 1.0, D = 0.0, i = 1.0, qs = 0.0, us = 0.0, vs = 0.0;
+    float Asum = 0.f, tau0f = 0.f;
     unsigned int nsteps = 0;
     KrpRayD ray = {};
     float4 cl = make_float4(0.f, 0.f, 0.f, 1.f);
@@ -400,37 +466,30 @@ __global__ void __launch_bounds__(256, 2) krp_k_flight_general(KrpModel g, KrpCt
             krp_cell_coef(g, cl, nd, inv_n, xs, ds, cc);
             const double R = D + log(i);
             double moved;
-            if (cc.a2 == 0.f && cc.a3 == 0.f) {
+            if (cc.a2 == 0.0 && cc.a3 == 0.0) {
                 moved = (R / cc.a1) / (double)cl.x;
-                const float inv = (float)(1.0 / i);
+                const double inv = 1.0 / i;
                 qs *= inv; us *= inv; vs *= inv;
             } else {
-                const float a = th[0] * cl.y + th[1] * cl.z + th[2] * cl.w;
-                const float b = ph[0] * cl.y + ph[1] * cl.z + ph[2] * cl.w;
-                float c2, s2;
-                krp_eta2<float>(a, b, c2, s2);
-                const float qg_e = c2 * qs + s2 * us, ug_e = -s2 * qs + c2 * us, vg_e = vs, i_f = (float)i;
-                const double t = krp_event_solve_d(R, (double)qg_e / i, cc.a1, (double)cc.a2, cc.dtau);
-                const float tf = (float)t;
-                float sh, chm1, syt = 0.f, cyt = 1.f;
-                krp_sinh_coshm1(cc.a2 * tf, sh, chm1);
-                if (cc.a3 != 0.f) sincosf(cc.a3 * tf, &syt, &cyt);
-                const float it = i_f + (i_f * chm1 - qg_e * sh);
-                float qt = qg_e + (qg_e * chm1 - i_f * sh);
-                float ut = ug_e * cyt - vg_e * syt;
-                float vt = ug_e * syt + vg_e * cyt;
-                const float inv = 1.f / it;
-                qt *= inv; ut *= inv; vt *= inv;
+                const double bx = cl.y, by = cl.z, bz = cl.w;
+                double c2, s2;
+                krp_eta2<double>(th[0] * bx + th[1] * by + th[2] * bz, ph[0] * bx + ph[1] * by + ph[2] * bz, c2, s2);
+                const double qg_e = c2 * qs + s2 * us, ug_e = -s2 * qs + c2 * us;
+                const double t = krp_event_solve_d(R, qg_e / i, cc.a1, cc.a2, cc.dtau);
+                double qt, ut, vt;
+                krp_appA_to_d(i, qg_e, ug_e, vs, cc.a2, cc.a3, t, qt, ut, vt);
                 qs = c2 * qt - s2 * ut; us = s2 * qt + c2 * ut; vs = vt;
                 moved = t / (double)cl.x;
             }
+            const float4 pc = q.pc[item], nk = q.nk[item];
+            const float n[3] = { nk.x, nk.y, nk.z };
             float pe[3];
-            pe[0] = krp_locald(n[0], ray.rx, ray.tx, moved, p0[0]);
-            pe[1] = krp_locald(n[1], ray.ry, ray.ty, moved, p0[1]);
-            pe[2] = krp_locald(n[2], ray.rz, ray.tz, moved, p0[2]);
+            pe[0] = krp_locald(n[0], ray.rx, ray.tx, moved, pc.x);
+            pe[1] = krp_locald(n[1], ray.ry, ray.ty, moved, pc.y);
+            pe[2] = krp_locald(n[2], ray.rz, ray.tz, moved, pc.z);
             tl.steps += nsteps;
-            krp_event_append(g, ctl, ev, q.id[item], ray.c, pe, n, __float_as_uint(q.nk[item].w), q.S[item].x, cc.omega,
-                             qs, us, vs, tl);
+            krp_event_append(g, ctl, ev, q.id[item], ray.c, pe, n, __float_as_uint(nk.w), q.S[item].x, cc.omega,
+                             (float)qs, (float)us, (float)vs, tl);
             status = KRP_IDLE;
         } else if (status == KRP_ESC) {
             tl.steps += nsteps;
@@ -438,21 +497,18 @@ __global__ void __launch_bounds__(256, 2) krp_k_flight_general(KrpModel g, KrpCt
             status = KRP_IDLE;
         }
         if (krp_take_work(&ctl->work[0], n_items, status == KRP_IDLE, wbase, wleft, more, item)) {
-            {
-                const float4 pc = q.pc[item], nk = q.nk[item], S0 = q.S[item];
-                n[0] = nk.x; n[1] = nk.y; n[2] = nk.z;
-                p0[0] = pc.x; p0[1] = pc.y; p0[2] = pc.z;
-                const double tau0 = q.tau[item];
-                krp_rayd_init(g, __float_as_uint(pc.w), p0, n, ray);
-                cl = __ldg(g.cell + ray.c);
-                krp_basis<float>(n, th, ph);
-                nd[0] = n[0]; nd[1] = n[1]; nd[2] = n[2];
-                inv_n = krp_rsqrt_near1(nd[0] * nd[0] + nd[1] * nd[1] + nd[2] * nd[2]);
-                D = tau0; i = 1.0;
-                qs = S0.y; us = S0.z; vs = S0.w;      // lab reference
-                Asum = 0.f; tau0f = (float)tau0; nsteps = 0;
-                status = KRP_RUN;
-            }
+            const float4 pc = q.pc[item], nk = q.nk[item], S0 = q.S[item];
+            const float n[3] = { nk.x, nk.y, nk.z }, p0[3] = { pc.x, pc.y, pc.z };
+            const double tau0 = q.tau[item];
+            krp_rayd_init(g, __float_as_uint(pc.w), p0, n, ray);
+            cl = __ldg(g.cell + ray.c);
+            nd[0] = n[0]; nd[1] = n[1]; nd[2] = n[2];
+            krp_basis<double>(nd, th, ph);
+            inv_n = krp_rsqrt_near1(nd[0] * nd[0] + nd[1] * nd[1] + nd[2] * nd[2]);
+            D = tau0; i = 1.0;
+            qs = S0.y; us = S0.z; vs = S0.w;      // lab reference
+            Asum = 0.f; tau0f = (float)tau0; nsteps = 0;
+            status = KRP_RUN;
         }
         if (!__any_sync(0xffffffffu, status == KRP_RUN)) break;
 #pragma unroll 1
@@ -465,40 +521,16 @@ __global__ void __launch_bounds__(256, 2) krp_k_flight_general(KrpModel g, KrpCt
                 krp_cell_coef(g, cl, nd, inv_n, xs, ds, cc);
                 Asum += (float)cc.dt1;
                 const bool near_end = Asum * guard >= tau0f;
-                if (cc.a2 == 0.f && cc.a3 == 0.f) {
+                if (cc.a2 == 0.0 && cc.a3 == 0.0) {
                     if (near_end && cc.dt1 >= D + log(i)) { status = KRP_HIT; continue; }
                     D -= cc.dt1;
                 } else {
-                    const float a = th[0] * cl.y + th[1] * cl.z + th[2] * cl.w;
-                    const float b = ph[0] * cl.y + ph[1] * cl.z + ph[2] * cl.w;
-                    float c2, s2;
-                    krp_eta2<float>(a, b, c2, s2);
-                    const float qg_e = c2 * qs + s2 * us, ug_e = -s2 * qs + c2 * us, vg_e = vs;   // eq. 7
-                    const float dtau_f = (float)cc.dtau, i_f = (float)i;
-                    const float xx = cc.a2 * dtau_f, yy = cc.a3 * dtau_f;
-                    float sy = 0.f, cy = 1.f;
-                    if (yy != 0.f) sincosf(yy, &sy, &cy);
-                    float qg, ug, vg;
-                    double i_new, depth;
-                    if (fabsf(xx) < 0.35f) {
-                        float sh, chm1;
-                        krp_sinh_coshm1(xx, sh, chm1);
-                        i_new = i + (double)(i_f * chm1 - qg_e * sh);
-                        qg = qg_e + (qg_e * chm1 - i_f * sh);
-                        ug = ug_e * cy - vg_e * sy;
-                        vg = ug_e * sy + vg_e * cy;
-                        depth = cc.dt1;
-                    } else {
-                        // thick cell: factor e^{-|alpha2 dtau|} moved into the scalar depth (no overflow at dtau ~ 1e3)
-                        const double xd = (double)cc.a2 * cc.dtau, axd = fabs(xd);
-                        const double E = exp(-2.0 * axd), sg = xd > 0.0 ? 1.0 : -1.0, f = exp(-axd);
-                        const double qd = (double)qg_e;
-                        i_new = 0.5 * ((i - sg * qd) + (i + sg * qd) * E);
-                        qg = (float)(0.5 * ((qd - sg * i) + (qd + sg * i) * E));
-                        ug = (float)f * (ug_e * cy - vg_e * sy);
-                        vg = (float)f * (ug_e * sy + vg_e * cy);
-                        depth = cc.dt1 - axd;
-                    }
+                    const double bx = cl.y, by = cl.z, bz = cl.w;
+                    double c2, s2;
+                    krp_eta2<double>(th[0] * bx + th[1] * by + th[2] * bz, ph[0] * bx + ph[1] * by + ph[2] * bz, c2, s2);
+                    const double qg_e = c2 * qs + s2 * us, ug_e = -s2 * qs + c2 * us;          // eq. 7
+                    double i_new, qg, ug, vg, depth;
+                    krp_appA_d(i, qg_e, ug_e, vs, cc, i_new, qg, ug, vg, depth);
                     const double Dn = D - depth;
                     if (near_end && log(i_new) + Dn <= 0.0) { status = KRP_HIT; continue; }   // state stays at cell entry
                     qs = c2 * qg - s2 * ug; us = s2 * qg + c2 * ug; vs = vg;
@@ -512,7 +544,6 @@ __global__ void __launch_bounds__(256, 2) krp_k_flight_general(KrpModel g, KrpCt
     }
     krp_tally_flush(tl, ctl);
 }
-
 // ------------------------------------------------------------------------------------------
 // quaternion helpers (eq. 1-3): q = (w, a);  q* v q  and  q v q*  for a pure
 // quaternion v, expanded from the Hamilton product:  v -+ 2w (a x v) + 2 a x (a x v).
