@@ -9,6 +9,7 @@
 #include <cmath>
 #include <cstdarg>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <vector>
@@ -52,6 +53,13 @@ struct krp_grid {
     uint64_t perm_cap = 0;
     void* d_scan = nullptr;
     size_t scan_bytes = 0;
+    // emission order of a point source (direction bins)
+    unsigned int* d_dir_bins = nullptr;
+    void* d_dir_scan = nullptr;
+    size_t dir_scan_bytes = 0;
+    int dir_sort = 1;
+    unsigned int* d_order = nullptr;
+    uint64_t order_cap = 0;
     float4* d_mueller = nullptr;
     double* d_cdf = nullptr;
     double* d_src_cdf = nullptr;
@@ -121,6 +129,7 @@ extern "C" int krp_grid_destroy(krp_grid* g)
     cudaFree(g->d_kr_alloc); cudaFree(g->d_cell_alloc); cudaFree(g->d_opac); cudaFree(g->d_mueller); cudaFree(g->d_cdf);
     cudaFree(g->d_src_cdf); cudaFree(g->d_ctl); cudaFree(g->d_obs); cudaFree(g->d_img);
     cudaFree(g->d_opA); cudaFree(g->d_opB); cudaFree(g->d_bins); cudaFree(g->d_perm); cudaFree(g->d_scan);
+    cudaFree(g->d_dir_bins); cudaFree(g->d_dir_scan); cudaFree(g->d_order);
     free_records(g->q[0]); free_records(g->q[1]); free_records(g->ev);
     for (cudaEvent_t e : g->t_ev) cudaEventDestroy(e);
     delete g;
@@ -213,6 +222,7 @@ extern "C" int krp_grid_create(krp_grid** out, int nx, int ny, int nz, const dou
     m.a1c = op[0]; m.omc = op[3]; m.rho = rho;
     // scalar flights are short: static assignment; general flights are long: persistent lanes, refill every 32 steps
     g->burst = m.scalar ? 1 : 32;
+    if (getenv("KRP_NO_DIR_SORT")) g->dir_sort = 0;   // A/B switch for measurement
     m.n_inc = n_inc; m.n_ang = tables->n_ang;
     m.w_min = tables->w_min; m.max_scatter = tables->max_scatter;
     // number of waves that can contain live packets: the weight after k scatterings is <= omega_max^k
@@ -447,8 +457,33 @@ extern "C" int krp_transport(krp_grid* g, uint64_t n_packets, uint64_t seed, voi
     const unsigned n = (unsigned)n_packets;
     const int tb = g->transport_block;
     const unsigned grid_all = (n + 255u) / 256u;
-    { TimedLaunch tl(g, st, KRP_T_EMIT);
-      krp_k_emit<<<grid_all, 256, 0, st>>>(g->m, g->d_ctl, g->q[0], g->ev, g->next_id, n, seed); }
+    KrpEmitSrc es0 = { nullptr, g->next_id, seed };     // first scattering order
+    {
+        TimedLaunch tl(g, st, KRP_T_EMIT);
+        if (g->m.src_kind == 0 && !g->m.emit_records && g->dir_sort && n >= (1u << 16)) {
+            // isotropic point source: the first flights take the packets in the order of their direction and
+            // compute the emission themselves (count, scan, order); nothing is written to the queue
+            if (!g->d_dir_bins) {
+                CK(cudaMalloc(&g->d_dir_bins, sizeof(unsigned int) * KRP_DIR_BINS));
+                CK(cub::DeviceScan::ExclusiveSum(nullptr, g->dir_scan_bytes, g->d_dir_bins, g->d_dir_bins, (int)KRP_DIR_BINS, st));
+                CK(cudaMalloc(&g->d_dir_scan, g->dir_scan_bytes ? g->dir_scan_bytes : 16));
+            }
+            if (g->order_cap < n_packets) {
+                CK(cudaStreamSynchronize(st));
+                cudaFree(g->d_order); g->d_order = nullptr; g->order_cap = 0;
+                CK(cudaMalloc(&g->d_order, sizeof(unsigned int) * n_packets));
+                g->order_cap = n_packets;
+            }
+            CK(cudaMemsetAsync(g->d_dir_bins, 0, sizeof(unsigned int) * KRP_DIR_BINS, st));
+            krp_k_emit_count<<<grid_all, 256, 0, st>>>(g->next_id, n, seed, g->d_dir_bins);
+            CK(cub::DeviceScan::ExclusiveSum(g->d_dir_scan, g->dir_scan_bytes, g->d_dir_bins, g->d_dir_bins, (int)KRP_DIR_BINS, st));
+            krp_k_emit_order<<<grid_all, 256, 0, st>>>(g->d_ctl, g->next_id, n, seed, g->d_dir_bins, g->d_order);
+            g->launches += 3;
+            es0.order = g->d_order;
+        } else {
+            krp_k_emit<<<grid_all, 256, 0, st>>>(g->m, g->d_ctl, g->q[0], g->ev, g->next_id, n, seed, nullptr);
+        }
+    }
     g->launches++;
     unsigned pers = (unsigned)(g->n_sm * g->blocks_per_sm);
     unsigned need = (n + tb - 1) / tb;
@@ -459,9 +494,10 @@ extern "C" int krp_transport(krp_grid* g, uint64_t n_packets, uint64_t seed, voi
         const int in = w & 1;
         krp_k_wave_prep<<<1, 1, 0, st>>>(g->d_ctl, in);
         { TimedLaunch tl(g, st, KRP_T_FLIGHT);
-        if (g->m.scalar && g->burst == 1) krp_k_flight_scalar_static<<<grid_f, tb, 0, st>>>(g->m, g->d_ctl, g->q[in], in, g->ev);
-        else if (g->m.scalar) krp_k_flight_scalar<<<grid_f, tb, 0, st>>>(g->m, g->d_ctl, g->q[in], in, g->ev, g->burst);
-        else             krp_k_flight_general<<<grid_f, tb, 0, st>>>(g->m, g->d_ctl, g->q[in], in, g->ev, g->burst); }
+        const KrpEmitSrc es = w == 0 ? es0 : KrpEmitSrc{ nullptr, 0, 0 };
+        if (g->m.scalar && g->burst == 1) krp_k_flight_scalar_static<<<grid_f, tb, 0, st>>>(g->m, g->d_ctl, g->q[in], in, g->ev, es);
+        else if (g->m.scalar) krp_k_flight_scalar<<<grid_f, tb, 0, st>>>(g->m, g->d_ctl, g->q[in], in, g->ev, g->burst, es);
+        else             krp_k_flight_general<<<grid_f, tb, 0, st>>>(g->m, g->d_ctl, g->q[in], in, g->ev, g->burst, es); }
         g->launches += 2;
         if (w + 1 < g->max_waves) {
             TimedLaunch tl(g, st, KRP_T_SCATTER);

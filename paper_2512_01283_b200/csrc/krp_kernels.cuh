@@ -15,8 +15,66 @@
 // T1/T2  emission: draws of block 0 = (cos theta, phi, tau*, spare); blocks 1-2
 // place a volume-source packet (R11, R17).  One thread per packet.
 // ------------------------------------------------------------------------------------------
+// Direction bins of an isotropic point source (T7): packets whose flights start in the same cell are queued in
+// the order of their direction (128 bins in cos(theta) x 256 in phi, read off the uniform words, 32 counters
+// per bin against contention), so that the 32 flights of a warp walk through the same cells -- their gathers hit
+// the same lines and they leave the grid together.  The queue order has no meaning for the results.
+#define KRP_DIR_BINS (1u << 20)
+__device__ __forceinline__ unsigned int krp_dir_bin(uint4 w, unsigned int i)
+{
+    return ((((w.x >> 25) << 8) | (w.y >> 24)) << 5) | (i & 31u);
+}
+__global__ void __launch_bounds__(256) krp_k_emit_count(unsigned long long id0, unsigned int n, unsigned long long seed,
+                                                        unsigned int* __restrict__ dir_bins)
+{
+    unsigned int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= n) return;
+    atomicAdd(dir_bins + krp_dir_bin(krp_philox(seed, id0 + i, 0u, 0u), i), 1u);
+}
+
+// order[slot] = index of the packet within the batch, slot taken from the scanned direction bins
+__global__ void __launch_bounds__(256) krp_k_emit_order(KrpCtl* ctl, unsigned long long id0, unsigned int n, unsigned long long seed,
+                                                        unsigned int* __restrict__ dir_bins, unsigned int* __restrict__ order)
+{
+    unsigned int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i == 0) {
+        ctl->q_count[0] = n; ctl->q_count[1] = 0;
+        atomicAdd(&ctl->stats.packets, (unsigned long long)n);
+        atomicAdd(&ctl->stats.w_emitted, (double)n);
+    }
+    if (i >= n) return;
+    order[atomicAdd(dir_bins + krp_dir_bin(krp_philox(seed, id0 + i, 0u, 0u), i), 1u)] = i;
+}
+
+// Where a flight kernel takes its queue entries from: the packet queue, or (first scattering order of an isotropic
+// point source) the emission itself, computed on the fly for packet id0 + order[item] -- the 64-byte queue entry of
+// a fresh packet is never written or read.
+struct KrpEmitSrc {
+    const unsigned int* order;     // NULL: read the queue
+    unsigned long long id0, seed;
+};
+__device__ __forceinline__ void krp_item_load(const KrpModel& g, const KrpRecords& q, const KrpEmitSrc& es, unsigned int item,
+                                              float4& pc, float4& nk, float4& S0, double& tau, unsigned long long& id)
+{
+    if (es.order) {
+        id = es.id0 + es.order[item];
+        const uint4 w = krp_philox(es.seed, id, 0u, 0u);
+        tau = -log(krp_u01(w.z));
+        const double ct = 1.0 - 2.0 * krp_u01(w.x);
+        const double st = sqrt(1.0 - ct * ct);
+        double sp, cp;
+        sincos(2.0 * KRP_PI_D * krp_u01(w.y), &sp, &cp);
+        nk = make_float4((float)(st * cp), (float)(st * sp), (float)ct, __uint_as_float(0u));   // R12
+        pc = make_float4(g.src_p[0], g.src_p[1], g.src_p[2], __uint_as_float(g.src_cell));
+        S0 = make_float4(1.f, 0.f, 0.f, 0.f);
+    } else {
+        pc = q.pc[item]; nk = q.nk[item]; S0 = q.S[item]; tau = q.tau[item]; id = q.id[item];
+    }
+}
+
 __global__ void __launch_bounds__(256) krp_k_emit(KrpModel g, KrpCtl* ctl, KrpRecords q, KrpRecords ev,
-                                                  unsigned long long id0, unsigned int n, unsigned long long seed)
+                                                  unsigned long long id0, unsigned int n, unsigned long long seed,
+                                                  unsigned int* __restrict__ dir_bins)
 {
     unsigned int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i == 0) {
@@ -62,11 +120,12 @@ __global__ void __launch_bounds__(256) krp_k_emit(KrpModel g, KrpCtl* ctl, KrpRe
         cell = g.src_cell; p[0] = g.src_p[0]; p[1] = g.src_p[1]; p[2] = g.src_p[2];
     }
     float4 pc = make_float4(p[0], p[1], p[2], __uint_as_float(cell));
-    q.pc[i] = pc;
-    q.nk[i] = make_float4(nn[0], nn[1], nn[2], __uint_as_float(0u));
-    q.S[i] = make_float4(1.f, 0.f, 0.f, 0.f);
-    q.tau[i] = tau;
-    q.id[i] = id;
+    const unsigned int slot = dir_bins ? atomicAdd(dir_bins + krp_dir_bin(w, i), 1u) : i;   // scanned counters: first slot of the bin
+    q.pc[slot] = pc;
+    q.nk[slot] = make_float4(nn[0], nn[1], nn[2], __uint_as_float(0u));
+    q.S[slot] = make_float4(1.f, 0.f, 0.f, 0.f);
+    q.tau[slot] = tau;
+    q.id[slot] = id;
     if (g.emit_records) {
         unsigned long long slot = krp_reserve64(&ctl->n_events);
         if (slot < ctl->ev_cap) {
@@ -206,7 +265,7 @@ __device__ __forceinline__ bool krp_take_work(unsigned int* counter, unsigned in
 
 enum { KRP_IDLE = 0, KRP_RUN = 1, KRP_HIT = 2, KRP_ESC = 3 };
 
-__global__ void __launch_bounds__(256, 4) krp_k_flight_scalar(KrpModel g, KrpCtl* ctl, KrpRecords q, int in, KrpRecords ev, int n_burst)
+__global__ void __launch_bounds__(256, 4) krp_k_flight_scalar(KrpModel g, KrpCtl* ctl, KrpRecords q, int in, KrpRecords ev, int n_burst, KrpEmitSrc es)
 {
     const unsigned int n_items = ctl->q_count[in];
     KrpFlightTally tl = { 0, 0, 0, 0.0, 0.0, 0.0 };
@@ -224,7 +283,8 @@ __global__ void __launch_bounds__(256, 4) krp_k_flight_scalar(KrpModel g, KrpCtl
             krp_pad_coords(g, c0, h0[0], h0[1], h0[2]);
             krp_pad_coords(g, ray.c, h1[0], h1[1], h1[2]);
             const int crossings = abs(h1[0] - h0[0]) + abs(h1[1] - h0[1]) + abs(h1[2] - h0[2]);
-            const float4 S0 = q.S[item];
+            float4 pc_, nk_, S0; double tau_; unsigned long long id_;
+            krp_item_load(g, q, es, item, pc_, nk_, S0, tau_, id_);
             if (status == KRP_HIT) {
                 const double moved = D / ((double)g.a1c * (double)kr);
                 // entry face of the event cell: the axis crossed last has its distance re-based to a full cell
@@ -232,8 +292,7 @@ __global__ void __launch_bounds__(256, 4) krp_k_flight_scalar(KrpModel g, KrpCtl
                 float pe[3];
                 krp_event_pos(g, n, p0, c0, ray.c, axis, moved, pe);
                 tl.steps += (unsigned long long)(crossings + 1);
-                krp_event_append(g, ctl, ev, q.id[item], ray.c, pe, n, __float_as_uint(q.nk[item].w), S0.x, g.omc,
-                                 S0.y, S0.z, S0.w, tl);
+                krp_event_append(g, ctl, ev, id_, ray.c, pe, n, __float_as_uint(nk_.w), S0.x, g.omc, S0.y, S0.z, S0.w, tl);
             } else {
                 tl.steps += (unsigned long long)crossings;
                 tl.w_esc += (double)S0.x;
@@ -242,12 +301,12 @@ __global__ void __launch_bounds__(256, 4) krp_k_flight_scalar(KrpModel g, KrpCtl
         }
         if (krp_take_work(&ctl->work[0], n_items, status == KRP_IDLE, wbase, wleft, more, item)) {
             {
-                const float4 pc = q.pc[item], nk = q.nk[item];
+                float4 pc, nk, S0_; unsigned long long id_;
+                krp_item_load(g, q, es, item, pc, nk, S0_, D, id_);
                 n[0] = nk.x; n[1] = nk.y; n[2] = nk.z;
                 p0[0] = pc.x; p0[1] = pc.y; p0[2] = pc.z;
                 c0 = __float_as_uint(pc.w);
                 krp_ray_init(g, c0, p0, n, ray);
-                D = q.tau[item];
                 kr = __ldg(g.kr + ray.c);
                 a1kr = g.a1c * kr;
                 status = KRP_RUN;
@@ -277,18 +336,18 @@ __global__ void __launch_bounds__(256, 4) krp_k_flight_scalar(KrpModel g, KrpCtl
 // The same flight with a static assignment (one queue entry per thread and grid stride, the warp's 32 flights
 // start and are closed together): no refill logic at all.  Cheaper when flights are short (C2: a point source
 // inside a dense ring, most flights end within a few cells), selected with flight_burst = 1.
-__global__ void __launch_bounds__(256, 4) krp_k_flight_scalar_static(KrpModel g, KrpCtl* ctl, KrpRecords q, int in, KrpRecords ev)
+__global__ void __launch_bounds__(256, 4) krp_k_flight_scalar_static(KrpModel g, KrpCtl* ctl, KrpRecords q, int in, KrpRecords ev, KrpEmitSrc es)
 {
     const unsigned int n_items = ctl->q_count[in];
     KrpFlightTally tl = { 0, 0, 0, 0.0, 0.0, 0.0 };
     for (unsigned int item = blockIdx.x * blockDim.x + threadIdx.x; item < n_items; item += gridDim.x * blockDim.x) {
-        const float4 pc = q.pc[item], nk = q.nk[item], S0 = q.S[item];
+        float4 pc, nk, S0; double D; unsigned long long id;
+        krp_item_load(g, q, es, item, pc, nk, S0, D, id);
         const float n[3] = { nk.x, nk.y, nk.z };
         const float p0[3] = { pc.x, pc.y, pc.z };
         const uint32_t c0 = __float_as_uint(pc.w);
         KrpRay ray;
         krp_ray_init(g, c0, p0, n, ray);
-        double D = q.tau[item];
         bool hit = false;
         float kr = __ldg(g.kr + ray.c);
         for (;;) {
@@ -310,7 +369,7 @@ __global__ void __launch_bounds__(256, 4) krp_k_flight_scalar_static(KrpModel g,
         const int axis = ray.c == c0 ? -1 : (ray.rx == ray.tx ? 0 : (ray.ry == ray.ty ? 1 : 2));
         float pe[3];
         krp_event_pos(g, n, p0, c0, ray.c, axis, moved, pe);
-        krp_event_append(g, ctl, ev, q.id[item], ray.c, pe, n, __float_as_uint(nk.w), S0.x, g.omc, S0.y, S0.z, S0.w, tl);
+        krp_event_append(g, ctl, ev, id, ray.c, pe, n, __float_as_uint(nk.w), S0.x, g.omc, S0.y, S0.z, S0.w, tl);
     }
     krp_tally_flush(tl, ctl);
 }
@@ -441,7 +500,7 @@ __device__ __forceinline__ void krp_appA_to_d(double i, double qg, double ug, do
     vt = (ug * sy + v * cy) * inv;
 }
 
-__global__ void __launch_bounds__(256, 2) krp_k_flight_general(KrpModel g, KrpCtl* ctl, KrpRecords q, int in, KrpRecords ev, int n_burst)
+__global__ void __launch_bounds__(256, 2) krp_k_flight_general(KrpModel g, KrpCtl* ctl, KrpRecords q, int in, KrpRecords ev, int n_burst, KrpEmitSrc es)
 {
     const unsigned int n_items = ctl->q_count[in];
     KrpFlightTally tl = { 0, 0, 0, 0.0, 0.0, 0.0 };
@@ -481,25 +540,26 @@ __global__ void __launch_bounds__(256, 2) krp_k_flight_general(KrpModel g, KrpCt
                 qs = c2 * qt - s2 * ut; us = s2 * qt + c2 * ut; vs = vt;
                 moved = t / (double)cl.x;
             }
-            const float4 pc = q.pc[item], nk = q.nk[item];
+            float4 pc, nk, S0_; double tau_; unsigned long long id_;
+            krp_item_load(g, q, es, item, pc, nk, S0_, tau_, id_);
             const float n[3] = { nk.x, nk.y, nk.z };
             float pe[3];
             pe[0] = krp_locald(n[0], ray.rx, ray.tx, moved, pc.x);
             pe[1] = krp_locald(n[1], ray.ry, ray.ty, moved, pc.y);
             pe[2] = krp_locald(n[2], ray.rz, ray.tz, moved, pc.z);
             tl.steps += nsteps;
-            krp_event_append(g, ctl, ev, q.id[item], ray.c, pe, n, __float_as_uint(nk.w), q.S[item].x, cc.omega,
+            krp_event_append(g, ctl, ev, id_, ray.c, pe, n, __float_as_uint(nk.w), S0_.x, cc.omega,
                              (float)qs, (float)us, (float)vs, tl);
             status = KRP_IDLE;
         } else if (status == KRP_ESC) {
             tl.steps += nsteps;
-            tl.w_esc += (double)q.S[item].x;
+            tl.w_esc += es.order ? 1.0 : (double)q.S[item].x;
             status = KRP_IDLE;
         }
         if (krp_take_work(&ctl->work[0], n_items, status == KRP_IDLE, wbase, wleft, more, item)) {
-            const float4 pc = q.pc[item], nk = q.nk[item], S0 = q.S[item];
+            float4 pc, nk, S0; double tau0; unsigned long long id_;
+            krp_item_load(g, q, es, item, pc, nk, S0, tau0, id_);
             const float n[3] = { nk.x, nk.y, nk.z }, p0[3] = { pc.x, pc.y, pc.z };
-            const double tau0 = q.tau[item];
             krp_rayd_init(g, __float_as_uint(pc.w), p0, n, ray);
             cl = __ldg(g.cell + ray.c);
             nd[0] = n[0]; nd[1] = n[1]; nd[2] = n[2];

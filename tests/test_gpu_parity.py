@@ -17,7 +17,7 @@ from harness import (oracle_run, gpu_grid, gpu_observers, gpu_events_sorted, com
 pytestmark = pytest.mark.gpu
 
 SMALL = {
-    "c1": dict(n=32, n_packets=20000, npix=64),          # the full C1 grid and image
+    "c1": dict(n=32, n_packets=100000, npix=64),         # BASELINE configs[0] in full (direction-ordered first flights)
     "c2": dict(n=48, n_packets=6000, npix=64),
     "c3": dict(n=12, n_packets=1500, npix=32),
     "c4": dict(n=40, n_packets=4000, npix=48),
