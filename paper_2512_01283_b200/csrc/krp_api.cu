@@ -70,6 +70,8 @@ struct krp_grid {
     uint64_t ev_cap = 0;
     bool ev_reserved = false;
     KrpObserverDev* d_obs = nullptr;
+    float4* d_obs_cells = nullptr;  // [n_obs][npad] per-observer cell coefficients (general mode), or NULL
+    int obs_pre = 1;
     double* d_img = nullptr;
     int n_obs = 0, npx = 0, npy = 0;
     std::vector<krp_observer> obs_host;
@@ -127,7 +129,7 @@ extern "C" int krp_grid_destroy(krp_grid* g)
 {
     if (!g) return KRP_OK;
     cudaFree(g->d_kr_alloc); cudaFree(g->d_cell_alloc); cudaFree(g->d_opac); cudaFree(g->d_mueller); cudaFree(g->d_cdf);
-    cudaFree(g->d_src_cdf); cudaFree(g->d_ctl); cudaFree(g->d_obs); cudaFree(g->d_img);
+    cudaFree(g->d_src_cdf); cudaFree(g->d_ctl); cudaFree(g->d_obs); cudaFree(g->d_img); cudaFree(g->d_obs_cells);
     cudaFree(g->d_opA); cudaFree(g->d_opB); cudaFree(g->d_bins); cudaFree(g->d_perm); cudaFree(g->d_scan);
     cudaFree(g->d_dir_bins); cudaFree(g->d_dir_scan); cudaFree(g->d_order);
     free_records(g->q[0]); free_records(g->q[1]); free_records(g->ev);
@@ -222,7 +224,8 @@ extern "C" int krp_grid_create(krp_grid** out, int nx, int ny, int nz, const dou
     m.a1c = op[0]; m.omc = op[3]; m.rho = rho;
     // scalar flights are short: static assignment; general flights are long: persistent lanes, refill every 32 steps
     g->burst = m.scalar ? 1 : 32;
-    if (getenv("KRP_NO_DIR_SORT")) g->dir_sort = 0;   // A/B switch for measurement
+    if (getenv("KRP_NO_DIR_SORT")) g->dir_sort = 0;   // A/B switches for measurement
+    if (getenv("KRP_NO_OBS_PRE")) g->obs_pre = 0;
     m.n_inc = n_inc; m.n_ang = tables->n_ang;
     m.w_min = tables->w_min; m.max_scatter = tables->max_scatter;
     // number of waves that can contain live packets: the weight after k scatterings is <= omega_max^k
@@ -318,9 +321,9 @@ extern "C" int krp_grid_create(krp_grid** out, int nx, int ny, int nz, const dou
     cudaFree(d_bad); cudaFree(tmp_den); cudaFree(tmp_b);
     if (bad) return fail(KRP_ERR_ARG, "density has %d negative, NaN or infinite cells", bad);
     m.kr = g->d_kr; m.cell = g->d_cell;
-    // bins of the imaging order: one cache line of cells per bin (32 x 4 B or 8 x 16 B), at most 2^22 bins
+    // bins of the imaging order: one cache line of cells per bin (32 x 4 B or 8 x 16 B), at most 2^25 bins
     g->bin_shift = m.scalar ? 5 : 3;
-    while ((g->npad >> g->bin_shift) >= (1u << 22)) g->bin_shift++;
+    while ((g->npad >> g->bin_shift) >= (1u << 25)) g->bin_shift++;
     g->n_bins = (g->npad >> g->bin_shift) + 1;
     // sub-counters per bin against atomic contention in hot cells: about 2^21 counters in all, at most 64 per bin
     g->sub_bits = 0;
@@ -556,6 +559,23 @@ extern "C" int krp_image(krp_grid* g, const krp_observer* obs, int n_obs, int np
         }
         g->obs_dev = od;
         g->obs_host.assign(obs, obs + n_obs);
+        // I0b: per-observer cell coefficients (general mode), when n_obs arrays of 16 B per padded cell fit
+        cudaFree(g->d_obs_cells); g->d_obs_cells = nullptr;
+        if (!g->m.scalar && g->obs_pre) {
+            size_t free_b = 0, total_b = 0;
+            CK(cudaMemGetInfo(&free_b, &total_b));
+            const size_t need = sizeof(float4) * (size_t)g->npad * (size_t)n_obs;
+            if (need + (4ull << 30) < free_b && cudaMalloc(&g->d_obs_cells, need) == cudaSuccess) {
+                const unsigned nb = (unsigned)((g->npad + 255u) / 256u);
+                for (int o = 0; o < n_obs; ++o)
+                    krp_k_obs_cells<<<nb, 256, 0, st>>>(g->m, od[o], g->npad, g->d_obs_cells + (size_t)o * g->npad);
+                CK(cudaGetLastError());
+                g->launches += (uint64_t)n_obs;
+            } else {
+                cudaGetLastError();
+                g->d_obs_cells = nullptr;
+            }
+        }
         g->n_obs = n_obs; g->npx = npix_x; g->npy = npix_y;
     }
     if (g->ev_cap == 0) return KRP_OK;   // nothing was ever transported
@@ -583,8 +603,13 @@ extern "C" int krp_image(krp_grid* g, const krp_observer* obs, int n_obs, int np
         const int slot = o % KRP_MAX_OBS_PACK;
         if (o > 0 && slot == 0) { krp_k_image_rewind<<<1, 1, 0, st>>>(g->d_ctl); g->launches++; }
         TimedLaunch tli(g, st, KRP_T_IMAGE);
-        if (g->m.scalar) krp_k_image<true><<<pers, tb, smem, st>>>(g->m, g->d_ctl, g->ev, g->d_perm, g->obs_dev[o], slot, o, npix_x, npix_y, g->d_img);
-        else             krp_k_image<false><<<pers, tb, smem, st>>>(g->m, g->d_ctl, g->ev, g->d_perm, g->obs_dev[o], slot, o, npix_x, npix_y, g->d_img);
+        if (g->m.scalar)
+            krp_k_image<true, false><<<pers, tb, 0, st>>>(g->m, g->d_ctl, g->ev, g->d_perm, g->obs_dev[o], nullptr, slot, o, npix_x, npix_y, g->d_img);
+        else if (g->d_obs_cells)
+            krp_k_image<false, true><<<pers, tb, 0, st>>>(g->m, g->d_ctl, g->ev, g->d_perm, g->obs_dev[o],
+                                                          g->d_obs_cells + (size_t)o * g->npad, slot, o, npix_x, npix_y, g->d_img);
+        else
+            krp_k_image<false, false><<<pers, tb, smem, st>>>(g->m, g->d_ctl, g->ev, g->d_perm, g->obs_dev[o], nullptr, slot, o, npix_x, npix_y, g->d_img);
         g->launches++;
     }
     krp_k_events_clear<<<1, 1, 0, st>>>(g->d_ctl);

@@ -873,6 +873,38 @@ __device__ __forceinline__ void krp_appA_delta_thin(float x, float y, float i, f
 
 // one step of the absolute-path-length march: returns the length of the segment in the current cell and moves
 // to the next one (ties: x before y before z).  dt and stride are launch constants (constant-bank operands).
+// ------------------------------------------------------------------------------------------
+// I0b  per-observer cell coefficients.  All rays of one observer share the direction, so what the in-cell
+// solution needs from a cell -- alpha_i(mu) with mu = |n_obs . B^| (R8, R13) and the angle eta between the
+// observer's reference and the grain frame (eq. 6-7, R2) -- depends on the cell only.  They are tabulated
+// once per observer set as float4 {kappa*rho*alpha1, kappa*rho*alpha2, kappa*rho*alpha3, 2*eta} in the padded
+// order (halo: first component -1), which takes the two table look-ups, nine dot-product terms and the
+// reciprocal out of the march and halves its traffic through the L1 data pipe (profiles/: the shared-memory
+// table reads were 49 % of that pipe on C5).  Used when n_obs such arrays fit in device memory.
+// ------------------------------------------------------------------------------------------
+__global__ void __launch_bounds__(256) krp_k_obs_cells(KrpModel g, const KrpObserverDev ob, uint32_t npad, float4* __restrict__ out)
+{
+    const uint32_t c = blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= npad) return;
+    const float4 cl = g.cell[c];
+    float4 o = make_float4(cl.x, 0.f, 0.f, 0.f);
+    if (cl.x > 0.f) {
+        const int nseg = g.n_inc - 1;
+        const float mu = fminf(fabsf(ob.n[0] * cl.y + ob.n[1] * cl.z + ob.n[2] * cl.w), 1.f);
+        const float x = mu * (float)nseg;
+        const int j = min((int)x, nseg - 1);
+        const float4 ta = g.opA[j], tb = g.opB[j];
+        const float a = ob.th[0] * cl.y + ob.th[1] * cl.z + ob.th[2] * cl.w;
+        const float b = ob.ph[0] * cl.y + ob.ph[1] * cl.z + ob.ph[2] * cl.w;
+        const float aa = a * a, bb = b * b;
+        o.x = cl.x * fmaf(tb.x, x, ta.x);
+        o.y = cl.x * fmaf(tb.y, x, ta.y);
+        o.z = cl.x * fmaf(tb.z, x, ta.z);
+        o.w = aa + bb < 1e-24f ? 0.f : atan2f(2.f * a * b, aa - bb);   // cos 2eta ~ a^2 - b^2, sin 2eta ~ 2ab (R2)
+    }
+    out[c] = o;
+}
+
 struct KrpRayAConst { float dtx, dty, dtz; int sx, sy, sz; float n[3], th[3], ph[3]; float xs; int nseg; };
 // The launch constants of the march, held in registers for the whole kernel: they are read back from shared
 // memory through volatile loads, which ptxas (unlike a kernel parameter) will not re-load inside the loop.
@@ -912,14 +944,15 @@ __device__ __forceinline__ float krp_raya_step(KrpRayA& r, const KrpRayAConst& k
     return ds;
 }
 
-template <bool SCALAR>
+template <bool SCALAR, bool PRE>
 __global__ void __launch_bounds__(256, KRP_IMAGE_MIN_BLOCKS) krp_k_image(KrpModel g, KrpCtl* ctl, KrpRecords ev,
                                                    const unsigned int* __restrict__ perm, const KrpObserverDev ob,
+                                                   const float4* __restrict__ obs_cell,
                                                    int slot, int obs_index, int npx, int npy, double* __restrict__ img)
 {
     extern __shared__ float4 s_tab[];                // [2*(n_inc-1)]: intercepts, slopes of the opacity table
     const int nseg = g.n_inc - 1;
-    if (!SCALAR) {
+    if (!SCALAR && !PRE) {
         for (int j = threadIdx.x; j < nseg; j += blockDim.x) { s_tab[j] = g.opA[j]; s_tab[nseg + j] = g.opB[j]; }
         __syncthreads();
     }
@@ -968,6 +1001,36 @@ __global__ void __launch_bounds__(256, KRP_IMAGE_MIN_BLOCKS) krp_k_image(KrpMode
                 }
                 r.c = c_n;                                 // the halo cell that ended the ray
                 A = g.a1c * tau;
+            } else if (PRE) {
+                // march over the observer's own coefficient array {kr a1, kr a2, kr a3, 2 eta}
+                float i = S[0], qs = S[1], us = S[2], vs = S[3];
+                float4 cl = __ldg(obs_cell + r.c);
+                do {
+                    const float ds = krp_raya_step(r, rc);
+                    const float4 cn = __ldg(obs_cell + r.c);    // next cell, in flight during the update below
+                    if (cl.x > 0.f) {
+                        const float xx = cl.y * ds, yy = cl.z * ds;
+                        float s2, c2;
+                        __sincosf(cl.w, &s2, &c2);
+                        const float qg = c2 * qs + s2 * us, ug = c2 * us - s2 * qs;   // eq. 7
+                        if (fmaxf(fabsf(xx), fabsf(yy)) < 0.1f) {
+                            float di, dqg, dug, dv;
+                            krp_appA_delta_thin(xx, yy, i, qg, ug, vs, di, dqg, dug, dv);
+                            i += di; vs += dv;
+                            qs += c2 * dqg - s2 * dug;
+                            us += s2 * dqg + c2 * dug;
+                            A = fmaf(cl.x, ds, A);
+                        } else {
+                            float qg2 = qg, ug2 = ug, vg2 = vs, di, i_new, depth;
+                            krp_appA(i, qg2, ug2, vg2, make_float4(cl.x, cl.y, cl.z, 0.f), ds, di, i_new, depth);
+                            i = i_new; A += depth; vs = vg2;
+                            qs = c2 * qg2 - s2 * ug2; us = s2 * qg2 + c2 * ug2;
+                            if (A > 104.f) { cl = cn; break; }      // e^{-A} is exactly 0 in fp32 from here on
+                        }
+                    }
+                    cl = cn;
+                } while (cl.x >= 0.f);
+                S[0] = i; S[1] = qs; S[2] = us; S[3] = vs;
             } else {
                 float i = S[0], qs = S[1], us = S[2], vs = S[3];
                 float4 cl = __ldg(g.cell + r.c);
