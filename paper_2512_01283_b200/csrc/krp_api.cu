@@ -44,6 +44,8 @@ struct krp_grid {
     float4* d_opac = nullptr;
     float4* d_opA = nullptr;
     float4* d_opB = nullptr;
+    double4* d_opA_d = nullptr;
+    double4* d_opB_d = nullptr;
     uint32_t npad = 0;
     // imaging order (counting sort of the events by cell bin)
     unsigned int* d_bins = nullptr;
@@ -130,7 +132,7 @@ extern "C" int krp_grid_destroy(krp_grid* g)
     if (!g) return KRP_OK;
     cudaFree(g->d_kr_alloc); cudaFree(g->d_cell_alloc); cudaFree(g->d_opac); cudaFree(g->d_mueller); cudaFree(g->d_cdf);
     cudaFree(g->d_src_cdf); cudaFree(g->d_ctl); cudaFree(g->d_obs); cudaFree(g->d_img); cudaFree(g->d_obs_cells);
-    cudaFree(g->d_opA); cudaFree(g->d_opB); cudaFree(g->d_bins); cudaFree(g->d_perm); cudaFree(g->d_scan);
+    cudaFree(g->d_opA); cudaFree(g->d_opB); cudaFree(g->d_opA_d); cudaFree(g->d_opB_d); cudaFree(g->d_bins); cudaFree(g->d_perm); cudaFree(g->d_scan);
     cudaFree(g->d_dir_bins); cudaFree(g->d_dir_scan); cudaFree(g->d_order);
     free_records(g->q[0]); free_records(g->q[1]); free_records(g->ev);
     for (cudaEvent_t e : g->t_ev) cudaEventDestroy(e);
@@ -254,8 +256,19 @@ extern "C" int krp_grid_create(krp_grid** out, int nx, int ny, int nz, const dou
         CK(cudaMalloc(&g->d_opB, sizeof(float4) * (n_inc - 1)));
         CK(cudaMemcpyAsync(g->d_opA, A.data(), sizeof(float4) * (n_inc - 1), cudaMemcpyHostToDevice, st));
         CK(cudaMemcpyAsync(g->d_opB, B.data(), sizeof(float4) * (n_inc - 1), cudaMemcpyHostToDevice, st));
+        std::vector<double> Ad(4 * (size_t)(n_inc - 1)), Bd(4 * (size_t)(n_inc - 1));
+        for (int j = 0; j + 1 < n_inc; ++j)
+            for (int s = 0; s < 4; ++s) {
+                double a = op[4 * j + s], b = op[4 * (j + 1) + s];
+                Bd[4 * j + s] = b - a;
+                Ad[4 * j + s] = a - (b - a) * j;
+            }
+        CK(cudaMalloc(&g->d_opA_d, sizeof(double4) * (n_inc - 1)));
+        CK(cudaMalloc(&g->d_opB_d, sizeof(double4) * (n_inc - 1)));
+        CK(cudaMemcpyAsync(g->d_opA_d, Ad.data(), sizeof(double4) * (n_inc - 1), cudaMemcpyHostToDevice, st));
+        CK(cudaMemcpyAsync(g->d_opB_d, Bd.data(), sizeof(double4) * (n_inc - 1), cudaMemcpyHostToDevice, st));
         CK(cudaStreamSynchronize(st));          // A, B are locals
-        m.opA = g->d_opA; m.opB = g->d_opB;
+        m.opA = g->d_opA; m.opB = g->d_opB; m.opA_d = g->d_opA_d; m.opB_d = g->d_opB_d;
     }
     CK(cudaMalloc(&g->d_mueller, sizeof(float4) * m.n_ang));
     CK(cudaMemcpyAsync(g->d_mueller, tables->mueller, sizeof(float4) * m.n_ang, cudaMemcpyHostToDevice, st));

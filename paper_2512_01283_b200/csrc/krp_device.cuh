@@ -35,6 +35,8 @@ struct KrpModel {
     const float4* opac;    // [n_inc] {alpha1, alpha2, alpha3, albedo} on mu_m = m/(n_inc-1)
     const float4* opA;     // [n_inc-1] intercepts and
     const float4* opB;     // [n_inc-1] slopes of the same table: value = opA[j] + opB[j]*x on x = mu*(n_inc-1) in [j, j+1]
+    const double4* opA_d;  // the same in fp64 (general-mode flight)
+    const double4* opB_d;
     int n_inc;
     const float4* mueller; // [n_ang] {S11,S12,S33,S34}
     int n_ang;
@@ -327,6 +329,18 @@ __device__ __forceinline__ void krp_eta2(T a, T b, T& c2, T& s2)
     T inv = T(1) / ss;
     c2 = (a * a - b * b) * inv;
     s2 = T(2) * a * b * inv;
+}
+
+// fp64 form with the reciprocal by Newton from the fp32 one (two steps: relative error < 1e-16), cheaper than a division
+__device__ __forceinline__ void krp_eta2_d(double a, double b, double& c2, double& s2)
+{
+    const double aa = a * a, bb = b * b, ss = aa + bb;
+    if (ss < 1e-24) { c2 = 1.0; s2 = 0.0; return; }
+    double r = (double)__frcp_rn((float)ss);
+    r = r * (2.0 - ss * r);
+    r = r * (2.0 - ss * r);
+    c2 = (aa - bb) * r;
+    s2 = 2.0 * a * b * r;
 }
 
 // sinh(x) and cosh(x)-1 without cancellation for small x; |x| < ~80

@@ -7,6 +7,9 @@
 #pragma once
 #include "krp_device.cuh"
 
+#ifndef KRP_FLIGHT_GENERAL_MIN_BLOCKS
+#define KRP_FLIGHT_GENERAL_MIN_BLOCKS 3
+#endif
 #ifndef KRP_IMAGE_MIN_BLOCKS
 #define KRP_IMAGE_MIN_BLOCKS 6
 #endif
@@ -428,32 +431,43 @@ __device__ __forceinline__ void krp_cell_coef(const KrpModel& g, const float4 cl
     mu = fmin(mu, 1.0);
     const double x = mu * xs;
     const int j = min((int)x, g.n_inc - 2);
-    const double w = x - (double)j, w0 = 1.0 - w;
-    const float4 oa = g.opac[j], ob = g.opac[j + 1];
-    c.a1 = w0 * (double)oa.x + w * (double)ob.x;
-    c.a2 = w0 * (double)oa.y + w * (double)ob.y;
-    c.a3 = w0 * (double)oa.z + w * (double)ob.z;
-    c.omega = (float)(w0 * (double)oa.w + w * (double)ob.w);
+    // the table as fp64 intercept + slope per segment (same piecewise-linear function, R13)
+    const double4 ta = g.opA_d[j], tb = g.opB_d[j];
+    c.a1 = fma(tb.x, x, ta.x);
+    c.a2 = fma(tb.y, x, ta.y);
+    c.a3 = fma(tb.z, x, ta.z);
+    c.omega = (float)fma(tb.w, x, ta.w);
     c.dtau = (double)cl.x * ds;
     c.dt1 = c.a1 * c.dtau;
 }
 
-// sinh(x), cosh(x)-1 and sin(y), cos(y)-1 in fp64 for |x|, |y| < 0.35: Taylor series to x^15 / x^16 (remainder < 1e-19)
+// sinh(x), cosh(x)-1 and sin(y), cos(y)-1 in fp64 for |x|, |y| < 0.35: Taylor series, 4 terms below 0.02 (remainder
+// < 1e-19 relative), 8 terms (to x^15 / x^16) otherwise
 __device__ __forceinline__ void krp_sinh_coshm1_d(double x, double& sh, double& chm1)
 {
     const double z = x * x;
-    sh = x * (1.0 + z * (1.0 / 6 + z * (1.0 / 120 + z * (1.0 / 5040 + z * (1.0 / 362880 + z * (1.0 / 39916800 +
-         z * (1.0 / 6227020800.0 + z * (1.0 / 1307674368000.0))))))));
-    chm1 = z * (0.5 + z * (1.0 / 24 + z * (1.0 / 720 + z * (1.0 / 40320 + z * (1.0 / 3628800 + z * (1.0 / 479001600 +
-           z * (1.0 / 87178291200.0 + z * (1.0 / 20922789888000.0))))))));
+    if (z < 4e-4) {
+        sh = x * (1.0 + z * (1.0 / 6 + z * (1.0 / 120 + z * (1.0 / 5040))));
+        chm1 = z * (0.5 + z * (1.0 / 24 + z * (1.0 / 720 + z * (1.0 / 40320))));
+    } else {
+        sh = x * (1.0 + z * (1.0 / 6 + z * (1.0 / 120 + z * (1.0 / 5040 + z * (1.0 / 362880 + z * (1.0 / 39916800 +
+             z * (1.0 / 6227020800.0 + z * (1.0 / 1307674368000.0))))))));
+        chm1 = z * (0.5 + z * (1.0 / 24 + z * (1.0 / 720 + z * (1.0 / 40320 + z * (1.0 / 3628800 + z * (1.0 / 479001600 +
+               z * (1.0 / 87178291200.0 + z * (1.0 / 20922789888000.0))))))));
+    }
 }
 __device__ __forceinline__ void krp_sin_cosm1_d(double y, double& sy, double& cym1)
 {
     const double z = y * y;
-    sy = y * (1.0 - z * (1.0 / 6 - z * (1.0 / 120 - z * (1.0 / 5040 - z * (1.0 / 362880 - z * (1.0 / 39916800 -
-         z * (1.0 / 6227020800.0 - z * (1.0 / 1307674368000.0))))))));
-    cym1 = -z * (0.5 - z * (1.0 / 24 - z * (1.0 / 720 - z * (1.0 / 40320 - z * (1.0 / 3628800 - z * (1.0 / 479001600 -
-           z * (1.0 / 87178291200.0 - z * (1.0 / 20922789888000.0))))))));
+    if (z < 4e-4) {
+        sy = y * (1.0 - z * (1.0 / 6 - z * (1.0 / 120 - z * (1.0 / 5040))));
+        cym1 = -z * (0.5 - z * (1.0 / 24 - z * (1.0 / 720 - z * (1.0 / 40320))));
+    } else {
+        sy = y * (1.0 - z * (1.0 / 6 - z * (1.0 / 120 - z * (1.0 / 5040 - z * (1.0 / 362880 - z * (1.0 / 39916800 -
+             z * (1.0 / 6227020800.0 - z * (1.0 / 1307674368000.0))))))));
+        cym1 = -z * (0.5 - z * (1.0 / 24 - z * (1.0 / 720 - z * (1.0 / 40320 - z * (1.0 / 3628800 - z * (1.0 / 479001600 -
+               z * (1.0 / 87178291200.0 - z * (1.0 / 20922789888000.0))))))));
+    }
 }
 
 // Source-free App. A step over the whole cell on the grain-frame state (i, qg, ug, v), fp64, with the common factor
@@ -500,7 +514,7 @@ __device__ __forceinline__ void krp_appA_to_d(double i, double qg, double ug, do
     vt = (ug * sy + v * cy) * inv;
 }
 
-__global__ void __launch_bounds__(256, 2) krp_k_flight_general(KrpModel g, KrpCtl* ctl, KrpRecords q, int in, KrpRecords ev, int n_burst, KrpEmitSrc es)
+__global__ void __launch_bounds__(256, KRP_FLIGHT_GENERAL_MIN_BLOCKS) krp_k_flight_general(KrpModel g, KrpCtl* ctl, KrpRecords q, int in, KrpRecords ev, int n_burst, KrpEmitSrc es)
 {
     const unsigned int n_items = ctl->q_count[in];
     KrpFlightTally tl = { 0, 0, 0, 0.0, 0.0, 0.0 };
@@ -532,7 +546,7 @@ __global__ void __launch_bounds__(256, 2) krp_k_flight_general(KrpModel g, KrpCt
             } else {
                 const double bx = cl.y, by = cl.z, bz = cl.w;
                 double c2, s2;
-                krp_eta2<double>(th[0] * bx + th[1] * by + th[2] * bz, ph[0] * bx + ph[1] * by + ph[2] * bz, c2, s2);
+                krp_eta2_d(th[0] * bx + th[1] * by + th[2] * bz, ph[0] * bx + ph[1] * by + ph[2] * bz, c2, s2);
                 const double qg_e = c2 * qs + s2 * us, ug_e = -s2 * qs + c2 * us;
                 const double t = krp_event_solve_d(R, qg_e / i, cc.a1, cc.a2, cc.dtau);
                 double qt, ut, vt;
@@ -576,6 +590,9 @@ __global__ void __launch_bounds__(256, 2) krp_k_flight_general(KrpModel g, KrpCt
             if (status != KRP_RUN) continue;
             const double ds = krp_rayd_ds(ray);
             ++nsteps;
+            // the next cell is requested now, so that its latency overlaps the fp64 update of this one
+            const uint32_t c_next = ray.c + (uint32_t)((ray.rx <= ray.ry) & (ray.rx <= ray.rz) ? ray.sx : (ray.ry <= ray.rz ? ray.sy : ray.sz));
+            const float4 cn = __ldg(g.cell + c_next);
             if (cl.x > 0.f) {
                 KrpCellCoef cc;
                 krp_cell_coef(g, cl, nd, inv_n, xs, ds, cc);
@@ -587,7 +604,7 @@ __global__ void __launch_bounds__(256, 2) krp_k_flight_general(KrpModel g, KrpCt
                 } else {
                     const double bx = cl.y, by = cl.z, bz = cl.w;
                     double c2, s2;
-                    krp_eta2<double>(th[0] * bx + th[1] * by + th[2] * bz, ph[0] * bx + ph[1] * by + ph[2] * bz, c2, s2);
+                    krp_eta2_d(th[0] * bx + th[1] * by + th[2] * bz, ph[0] * bx + ph[1] * by + ph[2] * bz, c2, s2);
                     const double qg_e = c2 * qs + s2 * us, ug_e = -s2 * qs + c2 * us;          // eq. 7
                     double i_new, qg, ug, vg, depth;
                     krp_appA_d(i, qg_e, ug_e, vs, cc, i_new, qg, ug, vg, depth);
@@ -598,7 +615,7 @@ __global__ void __launch_bounds__(256, 2) krp_k_flight_general(KrpModel g, KrpCt
                 }
             }
             krp_rayd_step(ray, ds);
-            cl = __ldg(g.cell + ray.c);
+            cl = cn;
             if (cl.x < 0.f) status = KRP_ESC;        // halo: the packet left the grid
         }
     }
