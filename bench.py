@@ -35,13 +35,13 @@ UNIT = "packets/s"
 # Algorithmic work per unit: bytes that must move and thread-instructions that must issue
 # per cell step of the two hot loops, for the two cell layouts, and per ray / flight outside the loop.
 #   image_inst   scalar: min3, sub, 3 setp, 3 predicated fadd + 3 iadd, address, gather, fma, sentinel test, branch
-#                general: the same march + mu, table segment (2 LDS.128), 3 fma, eta (rcp), rotation in/out, series
-#                of sinh/cosh-1/sin/cos-1, delta update, depth fma
+#                general (per-observer coefficient array): the same march + 2 products, sincos of 2 eta, rotation
+#                in, series of sinh/cosh-1/sin/cos-1, delta update rotated back, depth fma
 #   flight_inst  scalar: re-based march (13) + optical-depth product, fp64 compare and subtract, gather, tests
 #                general: fp64 re-based march, fp64 mu and alpha1, fp32 Stokes update, fp64 depth bookkeeping
 ALGO = {
     "scalar":  dict(cell_bytes=4,  image_inst=16, flight_inst=23, ray_inst=250, flight_fixed_inst=200),
-    "general": dict(cell_bytes=16, image_inst=80, flight_inst=110, ray_inst=250, flight_fixed_inst=300),
+    "general": dict(cell_bytes=16, image_inst=56, flight_inst=110, ray_inst=250, flight_fixed_inst=300),
 }
 EVENT_BYTES, CONTRIB_BYTES = 48, 32
 N_SM, LANES_PER_SM = 148, 128          # B200: 148 SMs x 4 schedulers x 32 lanes, one warp-instruction per scheduler and clock

@@ -668,30 +668,30 @@ __global__ void __launch_bounds__(128) krp_k_scatter(KrpModel g, KrpCtl* ctl, Kr
         double b[3] = { 0.0, 0.0, 1.0 };
         if (!g.scalar) { float4 cl = g.cell[cell]; b[0] = cl.y; b[1] = cl.z; b[2] = cl.w; }   // cell is a padded id
         const double n[3] = { nk.x, nk.y, nk.z };
-        // A2: q_B from the direction angles of B (eq. 2)
-        double qB[4];
-        {
+        // A2: q_B from the direction angles of B (eq. 2).  Without a field (scalar mode) B^ = z^, q_B = 1: the grain
+        // frame is the lab frame and every step below that involves q_B or eta is the identity
+        double qB[4] = { 1.0, 0.0, 0.0, 0.0 };
+        double ng[3] = { n[0], n[1], n[2] };
+        double th[3], ph[3], c2 = 1.0, s2 = 0.0;
+        double Q = Se.y, U = Se.z, V = Se.w;
+        if (!g.scalar) {
             double rho = sqrt(b[0] * b[0] + b[1] * b[1]);
             double thB = atan2(rho, b[2]), phB = rho > 0.0 ? atan2(b[1], b[0]) : 0.0;
             double sh_t, ch_t, sh_p, ch_p;
             sincos(0.5 * thB, &sh_t, &ch_t);
             sincos(0.5 * phB, &sh_p, &ch_p);
             qB[0] = ch_p * ch_t; qB[1] = -sh_p * sh_t; qB[2] = ch_p * sh_t; qB[3] = sh_p * ch_t;
+            // A3: direction in the grain frame (eq. 3)
+            krp_quat_rotate(qB, n, -1.0, ng);
+            // A5: Stokes reference lab -> grain frame
+            krp_basis<double>(n, th, ph);
+            krp_eta2<double>(krp_dot(th, b), krp_dot(ph, b), c2, s2);
+            krp_rot_qu(Q, U, c2, s2);
         }
-        // A3: direction in the grain frame (eq. 3)
-        double ng[3];
-        krp_quat_rotate(qB, n, -1.0, ng);
         {
             double r = 1.0 / sqrt(krp_dot(ng, ng));
             ng[0] *= r; ng[1] *= r; ng[2] *= r;
         }
-        // A5: Stokes reference lab -> grain frame
-        double th[3], ph[3];
-        krp_basis<double>(n, th, ph);
-        double c2, s2;
-        krp_eta2<double>(krp_dot(th, b), krp_dot(ph, b), c2, s2);
-        double Q = Se.y, U = Se.z, V = Se.w;
-        krp_rot_qu(Q, U, c2, s2);
         // draws
         uint4 w = krp_philox(seed, id, kb, 0u);
         const double tau_next = -log(krp_u01(w.w));
@@ -751,13 +751,15 @@ __global__ void __launch_bounds__(128) krp_k_scatter(KrpModel g, KrpCtl* ctl, Kr
             krp_rot_qu(Q, U, ce * ce - se * se, 2.0 * se * ce);                // reference theta^ of n'_GF
         }
         // back to the lab: inverse of eq. 3, direction stored in fp32 (R12)
-        double nl[3];
-        krp_quat_rotate(qB, nog, 1.0, nl);
+        double nl[3] = { nog[0], nog[1], nog[2] };
+        if (!g.scalar) krp_quat_rotate(qB, nog, 1.0, nl);
         const float nf[3] = { (float)nl[0], (float)nl[1], (float)nl[2] };
-        const double nd[3] = { nf[0], nf[1], nf[2] };
-        krp_basis<double>(nd, th, ph);
-        krp_eta2<double>(krp_dot(th, b), krp_dot(ph, b), c2, s2);
-        krp_rot_qu(Q, U, c2, -s2);
+        if (!g.scalar) {
+            const double nd[3] = { nf[0], nf[1], nf[2] };
+            krp_basis<double>(nd, th, ph);
+            krp_eta2<double>(krp_dot(th, b), krp_dot(ph, b), c2, s2);
+            krp_rot_qu(Q, U, c2, -s2);
+        }
         unsigned int slot = krp_reserve32(&ctl->q_count[out]);
         qo.pc[slot] = pc;
         qo.nk[slot] = make_float4(nf[0], nf[1], nf[2], __uint_as_float(kb));
