@@ -46,8 +46,9 @@ ALGO = {
 EVENT_BYTES, CONTRIB_BYTES = 48, 32
 N_SM, LANES_PER_SM = 148, 128          # B200: 148 SMs x 4 schedulers x 32 lanes, one warp-instruction per scheduler and clock
 # which ceiling binds the dominant kernel, read from the committed ncu captures (profiles/):
-# issue slots busy vs DRAM / L2 throughput of the kernel
-BOUND = {"c1": "alu", "c2": "alu", "c3": "alu", "c4": "alu", "c5": "hbm"}
+# issue slots busy vs DRAM / L2 throughput of the kernel (r1d: C2 flight 56 % issue vs 1 % DRAM, C2 image 56 % vs 23 %,
+# C4 flight 52 % vs 35 %, C4 image 71 % vs 38 %, C5 image 70 % vs 41 %)
+BOUND = {"c1": "alu", "c2": "alu", "c3": "alu", "c4": "alu", "c5": "alu"}
 
 
 def parse_args():
@@ -213,7 +214,11 @@ def run_reference(args):
 # ------------------------------------------------------------------------------------------
 # dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
 # `ncu --set full` capture of this same command (profiles/, named per round); None until captured.
-NCU_TRAFFIC = {}
+NCU_TRAFFIC = {   # bytes, profiles/r1d_ncu_full_*.txt: the first-order flight launch (C2, C4), one observer's imaging launch (C5)
+    "c2": 83.664384e6 + 162.73996e6,
+    "c4": 42.137358e9 + 2.835999e9,
+    "c5": 227.68106e9 + 1.778706e9,
+}
 
 
 def make_grid(krp, cfg, dens, bf, weight):

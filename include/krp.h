@@ -107,7 +107,9 @@ int krp_events_reserve(krp_grid* g, uint64_t max_events);
  * persists across calls; krp_packet_id_set changes it), Philox4x32-10 keyed by `seed` with the
  * counter schedule R11, so results do not depend on how the caller batches.  Appends one
  * record per scattering event: position, cell, incoming direction, albedo*weight and the
- * normalised Stokes state in the lab reference.  Does not synchronise. */
+ * normalised Stokes state in the lab reference.  Does not synchronise (it does once, when a
+ * larger batch than any before makes it grow its queues).  The order in which packets are processed and
+ * events are appended is not defined (an isotropic point source is processed in direction order). */
 int krp_transport(krp_grid* g, uint64_t n_packets, uint64_t seed, void* stream);
 int krp_packet_id_set(krp_grid* g, uint64_t next_id);
 
@@ -124,8 +126,9 @@ typedef struct krp_observer {
  * the internal fp64 maps [n_obs][4][npix_y][npix_x] (I,Q,U,V relative to theta^_obs, sum of
  * contributions per pixel, no area normalisation, R14).  flags bit0: include emission
  * records (direct light).  Clears the event buffer afterwards.  The maps are (re)allocated
- * and zeroed when the observer set or the pixel counts differ from the previous call.
- * Does not synchronise. */
+ * and zeroed when the observer set or the pixel counts differ from the previous call; with a field
+ * (16-byte cells) the call then also tabulates 16 bytes per cell and observer if that fits in device memory.
+ * Does not synchronise except on such a change. */
 int krp_image(krp_grid* g, const krp_observer* obs, int n_obs, int npix_x, int npix_y,
               int flags, void* stream);
 /* Copy the maps to out ([n_obs][4][npix_y][npix_x] doubles; `mem` = where out lives).
