@@ -66,7 +66,7 @@ def parse_args():
     return ap.parse_args()
 
 
-DEFAULT_BATCH = {"c1": 100000, "c2": 1 << 24, "c3": 1 << 22, "c4": 1 << 23, "c5": 1 << 22}
+DEFAULT_BATCH = {"c1": 100000, "c2": 1 << 25, "c3": 1 << 22, "c4": 1 << 23, "c5": 1 << 22}
 
 
 def make_workload(args):

@@ -10,6 +10,9 @@
 #ifndef KRP_FLIGHT_GENERAL_MIN_BLOCKS
 #define KRP_FLIGHT_GENERAL_MIN_BLOCKS 3
 #endif
+#ifndef KRP_IMAGE_SCALAR_MIN_BLOCKS
+#define KRP_IMAGE_SCALAR_MIN_BLOCKS 8
+#endif
 #ifndef KRP_IMAGE_MIN_BLOCKS
 #define KRP_IMAGE_MIN_BLOCKS 6
 #endif
@@ -339,6 +342,26 @@ __global__ void __launch_bounds__(256, 4) krp_k_flight_scalar(KrpModel g, KrpCtl
 // The same flight with a static assignment (one queue entry per thread and grid stride, the warp's 32 flights
 // start and are closed together): no refill logic at all.  Cheaper when flights are short (C2: a point source
 // inside a dense ring, most flights end within a few cells), selected with flight_burst = 1.
+// one re-based step in registers: returns the length of the segment in the current cell and the axis of the face
+// crossed (ties x before y before z), moves to the next cell
+__device__ __forceinline__ float krp_ray_advance(KrpRay& r, int& axis)
+{
+    float ds;
+    asm("{\n\t.reg .pred px, py, pz;\n\t"
+        "min.f32 %0, %1, %2, %3;\n\t"
+        "setp.le.f32 px, %1, %0;\n\t"
+        "setp.le.and.f32 py, %2, %0, !px;\n\t"
+        "setp.gt.and.f32 pz, %2, %0, !px;\n\t"
+        "sub.f32 %1, %1, %0;\n\tsub.f32 %2, %2, %0;\n\tsub.f32 %3, %3, %0;\n\t"
+        "selp.s32 %5, 1, 2, py;\n\tselp.s32 %5, 0, %5, px;\n\t"
+        "@px mov.f32 %1, %6;\n\t@px add.s32 %4, %4, %9;\n\t"
+        "@py mov.f32 %2, %7;\n\t@py add.s32 %4, %4, %10;\n\t"
+        "@pz mov.f32 %3, %8;\n\t@pz add.s32 %4, %4, %11;\n\t}"
+        : "=&f"(ds), "+f"(r.rx), "+f"(r.ry), "+f"(r.rz), "+r"(r.c), "=&r"(axis)
+        : "f"(r.tx), "f"(r.ty), "f"(r.tz), "r"(r.sx), "r"(r.sy), "r"(r.sz));
+    return ds;
+}
+
 __global__ void __launch_bounds__(256, 4) krp_k_flight_scalar_static(KrpModel g, KrpCtl* ctl, KrpRecords q, int in, KrpRecords ev, KrpEmitSrc es)
 {
     const unsigned int n_items = ctl->q_count[in];
@@ -351,28 +374,39 @@ __global__ void __launch_bounds__(256, 4) krp_k_flight_scalar_static(KrpModel g,
         const uint32_t c0 = __float_as_uint(pc.w);
         KrpRay ray;
         krp_ray_init(g, c0, p0, n, ray);
+        // The march runs two cells ahead of the optical-depth test, so that two gathers are in flight: the stages hold
+        // the cell id, the axis of its entry face, its segment length and its kappa*rho.  The look-ahead may step one
+        // cell past the halo cell that ends the flight (inside the allocation's margin); its value is never used.
         bool hit = false;
-        float kr = __ldg(g.kr + ray.c);
+        int ax_cur = -1, ax_nxt, ax_new;
+        uint32_t c_cur = ray.c;
+        float kr_cur = __ldg(g.kr + c_cur);
+        float ds_cur = krp_ray_advance(ray, ax_nxt);
+        uint32_t c_nxt = ray.c;
+        float kr_nxt = __ldg(g.kr + c_nxt);
+        float ds_nxt = krp_ray_advance(ray, ax_new);
+#pragma unroll 2
         for (;;) {
-            const float ds = krp_ray_ds(ray);
-            const float dt1 = g.a1c * kr * ds;
-            if ((double)dt1 >= D) { hit = true; break; }      // event inside this cell
+            const uint32_t c_new = ray.c;
+            const float kr_new = __ldg(g.kr + (int)c_new);       // signed: the look-ahead may sit before the array's first cell
+            const float dt1 = g.a1c * kr_cur * ds_cur;
+            if ((double)dt1 >= D) { hit = true; break; }      // event inside the current cell
             D -= (double)dt1;
-            krp_ray_step(ray, ds);
-            kr = __ldg(g.kr + ray.c);
-            if (kr < 0.f) break;                               // halo: the packet left the grid
+            if (kr_nxt < 0.f) { c_cur = c_nxt; break; }        // halo: the packet left the grid
+            c_cur = c_nxt; ax_cur = ax_nxt; kr_cur = kr_nxt; ds_cur = ds_nxt;
+            c_nxt = c_new; ax_nxt = ax_new; kr_nxt = kr_new;
+            ds_nxt = krp_ray_advance(ray, ax_new);
         }
         int h0[3], h1[3];
         krp_pad_coords(g, c0, h0[0], h0[1], h0[2]);
-        krp_pad_coords(g, ray.c, h1[0], h1[1], h1[2]);
+        krp_pad_coords(g, c_cur, h1[0], h1[1], h1[2]);
         const int crossings = abs(h1[0] - h0[0]) + abs(h1[1] - h0[1]) + abs(h1[2] - h0[2]);
         if (!hit) { tl.steps += (unsigned long long)crossings; tl.w_esc += (double)S0.x; continue; }
         tl.steps += (unsigned long long)(crossings + 1);
-        const double moved = D / ((double)g.a1c * (double)kr);
-        const int axis = ray.c == c0 ? -1 : (ray.rx == ray.tx ? 0 : (ray.ry == ray.ty ? 1 : 2));
+        const double moved = D / ((double)g.a1c * (double)kr_cur);
         float pe[3];
-        krp_event_pos(g, n, p0, c0, ray.c, axis, moved, pe);
-        krp_event_append(g, ctl, ev, id, ray.c, pe, n, __float_as_uint(nk.w), S0.x, g.omc, S0.y, S0.z, S0.w, tl);
+        krp_event_pos(g, n, p0, c0, c_cur, ax_cur, moved, pe);
+        krp_event_append(g, ctl, ev, id, c_cur, pe, n, __float_as_uint(nk.w), S0.x, g.omc, S0.y, S0.z, S0.w, tl);
     }
     krp_tally_flush(tl, ctl);
 }
@@ -964,7 +998,7 @@ __device__ __forceinline__ float krp_raya_step(KrpRayA& r, const KrpRayAConst& k
 }
 
 template <bool SCALAR, bool PRE>
-__global__ void __launch_bounds__(256, KRP_IMAGE_MIN_BLOCKS) krp_k_image(KrpModel g, KrpCtl* ctl, KrpRecords ev,
+__global__ void __launch_bounds__(256, SCALAR ? KRP_IMAGE_SCALAR_MIN_BLOCKS : KRP_IMAGE_MIN_BLOCKS) krp_k_image(KrpModel g, KrpCtl* ctl, KrpRecords ev,
                                                    const unsigned int* __restrict__ perm, const KrpObserverDev ob,
                                                    const float4* __restrict__ obs_cell,
                                                    int slot, int obs_index, int npx, int npy, double* __restrict__ img)
@@ -1013,7 +1047,7 @@ __global__ void __launch_bounds__(256, KRP_IMAGE_MIN_BLOCKS) krp_k_image(KrpMode
 #pragma unroll 2
                 for (;;) {
                     const float ds_n = krp_raya_step(r, rc);
-                    const float kr_nn = __ldg(g.kr + r.c); // look-ahead (may lie one cell past the halo: margin)
+                    const float kr_nn = __ldg(g.kr + (int)r.c); // look-ahead (may lie one cell past the halo, on either side: margin, signed index)
                     tau = fmaf(kr_c, ds_c, tau);
                     if (kr_n < 0.f) break;
                     kr_c = kr_n; ds_c = ds_n; kr_n = kr_nn; c_n = r.c;
