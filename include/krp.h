@@ -142,7 +142,7 @@ typedef struct krp_stats {
     uint64_t events;          /* scattering events recorded */
     uint64_t records;         /* emission records recorded */
     uint64_t steps_transport; /* cell steps taken by transport flights */
-    uint64_t steps_image;     /* cell steps taken by imaging rays */
+    uint64_t steps_image;     /* cell steps taken by imaging rays (a ray stops once its attenuation is 0 in fp32) */
     uint64_t contributions;   /* image contributions deposited */
     uint64_t dropped;         /* contributions that fell outside the frame */
     uint64_t overflow;        /* events lost to a full event buffer */

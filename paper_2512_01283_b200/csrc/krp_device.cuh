@@ -3,10 +3,10 @@
 // Citations: PAPER.md:<line> is the extracted text of arxiv 2512.01283; R<n> are the readings
 // in DESIGN.md.  Nothing here is shared with oracle/ (the fp64 CPU checker).
 //
-// Precision plan: the cell march is fp32; the two quantities that
-// decide *where* a packet scatters -- the optical depth still to go, D, and the normalised
-// intensity i -- are accumulated in fp64 from fp32 increments; scattering geometry (once per
-// event) is fp64 and the new direction is stored rounded to fp32 (R12).
+// Precision plan: the imaging march is fp32; whatever decides *where* a
+// packet scatters is fp64 (scalar mode: the optical depth still to go, from fp32 segments; general
+// mode: segments, alpha_i(mu), depth, normalised intensity and the Stokes vector); scattering
+// geometry (once per event) is fp64 and the new direction is stored rounded to fp32 (R12).
 #pragma once
 #include <cuda_runtime.h>
 #include <stdint.h>
@@ -106,10 +106,7 @@ struct KrpObserverDev {
     int stride[3];              // signed stride in the padded array per axis (0 when n = 0)
     double thd[3], phd[3], center[3], inv_hw, inv_hh;
 };
-// observers of one imaging launch, passed by value (constant bank): blockIdx.y picks one
-struct KrpObsPack {
-    KrpObserverDev o[KRP_MAX_OBS_PACK];
-};
+
 
 // ------------------------------------------------------------------------------------------
 // S0  Philox4x32-10 (Salmon et al. 2011), counter = (id_lo, id_hi, k, block), key = seed (R11)
@@ -201,15 +198,6 @@ __device__ __forceinline__ void krp_ray_step(KrpRay& r, float ds)
     if (ax)      { r.rx = r.tx; r.c += (uint32_t)r.sx; }
     else if (ay) { r.ry = r.ty; r.c += (uint32_t)r.sy; }
     else         { r.rz = r.tz; r.c += (uint32_t)r.sz; }
-}
-
-// cell-local coordinate after moving `moved` from the point where the distances r were taken (fp32; statistics only)
-__device__ __forceinline__ float krp_local(float n, float r, float t, float moved, float p0)
-{
-    if (n == 0.f) return p0;
-    float f = (r - moved) / t;
-    f = fminf(fmaxf(f, 0.f), 1.f);
-    return n > 0.f ? 1.f - f : f;
 }
 
 // Event position in fp64 without accumulated rounding: the flight started at

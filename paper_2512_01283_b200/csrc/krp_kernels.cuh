@@ -1,9 +1,9 @@
 // krp_kernels.cuh -- the kernels of the hot path: emit, flight (cell march to the next
 // event), scatter, image.  See DESIGN.md "Kernels".  Transport is a wavefront pipeline:
 //   emit -> [ wave_prep -> flight -> scatter ] x waves
-// Flights run in fp32 and never execute scattering code; lanes that reach an event park the
-// packet in the event buffer, and the scatter kernel (fp64 geometry, all lanes busy) turns the
-// wave's events into the next queue.  The event buffer is what the imaging kernel consumes.
+// Flights never execute scattering code; lanes that reach an event append the packet to the event
+// buffer, and the scatter kernel (fp64 geometry, all lanes busy) turns the wave's events into the
+// next queue.  The event buffer is what the imaging kernels consume (ordered by cell bin first).
 #pragma once
 #include "krp_device.cuh"
 
@@ -155,31 +155,6 @@ __global__ void krp_k_wave_prep(KrpCtl* ctl, int in)
     ctl->work[0] = 0;
 }
 
-// ------------------------------------------------------------------------------------------
-// T4  in-cell event location (R7).  With the Stokes vector carried as e^{-A}(i,q,u,v) and
-// D = tau* - A the scalar depth still to go at cell entry, the event is at the t solving
-//   alpha1 t - ln( cosh(alpha2 t) - (q_g/i) sinh(alpha2 t) ) = D + ln i  =: R ,
-// whose left side is increasing and concave: Newton from R/alpha1 lands left of the root after
-// one step and then rises monotonically.  alpha2 = 0 is the closed form t = R/alpha1.
-// ------------------------------------------------------------------------------------------
-__device__ __forceinline__ float krp_event_solve(float R, float qq, float a1, float a2, float tmax)
-{
-    float t = R / a1;
-    if (a2 != 0.f) {
-#pragma unroll 1
-        for (int it = 0; it < 12; ++it) {
-            float sh, chm1;
-            krp_sinh_coshm1(a2 * t, sh, chm1);
-            float gm1 = chm1 - qq * sh;
-            float h = a1 * t - log1pf(gm1) - R;
-            float hp = a1 - a2 * (sh - qq * (1.f + chm1)) / (1.f + gm1);
-            float dt = h / hp;
-            t = fminf(fmaxf(t - dt, 0.f), tmax);
-            if (fabsf(dt) <= 2e-7f * t) break;
-        }
-    }
-    return fminf(fmaxf(t, 0.f), tmax);
-}
 
 // ------------------------------------------------------------------------------------------
 // T3/T4/T5, scalar mode: the opacity table does not depend on direction and alpha2 = alpha3 = 0,
@@ -412,8 +387,12 @@ __global__ void __launch_bounds__(256, 4) krp_k_flight_scalar_static(KrpModel g,
 }
 
 // ------------------------------------------------------------------------------------------
-// T4 in fp64 (general mode): same equation as krp_event_solve; the root decides where the event
-// lies, so it is located in the oracle's precision.
+// T4  in-cell event location (R7), general mode, fp64 (the root decides where the event lies).  With the
+// Stokes vector carried as e^{-A}(i,q,u,v) and D = tau* - A the scalar depth still to go at cell entry,
+// the event is at the t solving
+//   alpha1 t - ln( cosh(alpha2 t) - (q_g/i) sinh(alpha2 t) ) = D + ln i  =: R ,
+// whose left side is increasing and concave: Newton from R/alpha1 lands left of the root after one step
+// and then rises monotonically.  alpha2 = 0 is the closed form t = R/alpha1.
 // ------------------------------------------------------------------------------------------
 __device__ __forceinline__ double krp_event_solve_d(double R, double qq, double a1, double a2, double tmax)
 {

@@ -269,3 +269,34 @@ def test_launch_shapes_do_not_change_results():
                     assert np.array_equal(ref_ev[key], ev[key]), (name, tune, key)
                 assert np.allclose(img, ref_img, rtol=1e-11, atol=1e-13 * ref_img[:, 0].max()), (name, tune)
             g.close()
+
+
+def test_scheduling_switches_do_not_change_results(monkeypatch):
+    """The two scheduling features that only large batches / general mode reach -- direction-ordered first flights of a
+    point source (emission computed inside the flight kernel) and per-observer cell coefficient arrays in the imaging
+    march -- against the plain paths (A/B switches read at krp_grid_create): events bit-identical, maps equal to the
+    rounding of the fp32 march."""
+    cfg = inputs.make("c5", n=32, n_packets=70000, npix=48)          # point source, general mode, >= 2^16 packets
+    res = {}
+    for label, env in (("on", {}), ("off", {"KRP_NO_DIR_SORT": "1", "KRP_NO_OBS_PRE": "1"})):
+        for k in ("KRP_NO_DIR_SORT", "KRP_NO_OBS_PRE"):
+            monkeypatch.delenv(k, raising=False)
+        for k, v in env.items():
+            monkeypatch.setenv(k, v)
+        g = gpu_grid(cfg)
+        g.events_reserve(20 * cfg["n_packets"])
+        g.transport(cfg["n_packets"], cfg["seed"])
+        ev = gpu_events_sorted(g)
+        g.image(gpu_observers(cfg), cfg["npix"], cfg["npix"])
+        res[label] = (ev, g.image_get(), g.stats_get())
+        g.close()
+    ev_on, img_on, st_on = res["on"]
+    ev_off, img_off, st_off = res["off"]
+    for key in ev_on:
+        assert np.array_equal(ev_on[key], ev_off[key]), key
+    assert st_on["steps_transport"] == st_off["steps_transport"] and st_on["events"] == st_off["events"]
+    for o in range(img_on.shape[0]):
+        for s in range(4):
+            scale = np.abs(img_off[o, 0]).max()
+            assert np.abs(img_on[o, s] - img_off[o, s]).max() <= 2e-5 * scale, (o, s)
+    assert abs(img_on[:, 0].sum() - img_off[:, 0].sum()) <= 1e-6 * img_off[:, 0].sum()
