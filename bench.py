@@ -47,8 +47,10 @@ EVENT_BYTES, CONTRIB_BYTES = 48, 32
 N_SM, LANES_PER_SM = 148, 128          # B200: 148 SMs x 4 schedulers x 32 lanes, one warp-instruction per scheduler and clock
 # which ceiling binds the dominant kernel, read from the committed ncu captures (profiles/):
 # issue slots busy vs DRAM / L2 throughput of the kernel (r1d: C2 flight 56 % issue vs 1 % DRAM, C2 image 56 % vs 23 %,
-# C4 flight 52 % vs 35 %, C4 image 71 % vs 38 %, C5 image 70 % vs 41 %)
-BOUND = {"c1": "alu", "c2": "alu", "c3": "alu", "c4": "alu", "c5": "alu"}
+# C4 flight 52 % vs 35 %, C4 image 71 % vs 38 %, C5 image 70 % vs 41 %).  C4's dominant kernel is the general flight, whose
+# gathers are random DRAM accesses: 31 % of its stall samples wait on the cell gather and it runs at 88 % of the measured
+# random-gather rate of a 256 MiB array ("gather" in the roofline object), so HBM is what binds it.
+BOUND = {"c1": "alu", "c2": "alu", "c3": "alu", "c4": "hbm", "c5": "alu"}
 
 
 def parse_args():
@@ -362,7 +364,18 @@ def run_krp(args):
         roof = {"bound": "hbm", "achieved": W["bytes"] / t_dom / 1e9, "peak": pk["hbm_gbs"], "unit": "GB/s", "frac": f_hbm}
     else:
         roof = {"bound": "alu", "achieved": W["inst"] / t_dom / 1e12, "peak": alu_peak / 1e12, "unit": "Tinst/s", "frac": f_alu}
-    roof.update({"kernel": W["kernel"], "launches_per_step": n_launch / K, "avg_launch_ms": 1e3 * t_dom / n_launch,
+    # gather ceiling (north_star: "L2/HBM gather bandwidth"): the measured rate of independent random gathers of one cell
+    # from an array of the grid's size (krp_probe_gather, run now, outside the timed region).  A flight is one such
+    # gather per cell step; an imaging march over events ordered by cell is coherent and can exceed it.
+    cell_b = A["cell_bytes"]
+    grid_bytes = cell_b * (cfg["nx"] + 2) * (cfg["ny"] + 2) * (cfg["nz"] + 2)
+    probe_bytes = max(grid_bytes, 1 << 20)
+    gather_peak = krp.probe_gather(probe_bytes, cell_b)
+    gather = {c: {"cell_steps_per_s": work[c]["steps"] / (timing[c][0] * 1e-3), "peak_gathers_per_s": gather_peak,
+                  "frac": work[c]["steps"] / (timing[c][0] * 1e-3) / gather_peak} for c in ("flight", "image")}
+    roof.update({"gather": {"probe": "random %d-B gathers from an array of the grid's size, %d MiB" % (cell_b, probe_bytes >> 20),
+                            **gather},
+                 "kernel": W["kernel"], "launches_per_step": n_launch / K, "avg_launch_ms": 1e3 * t_dom / n_launch,
                  "kernel_ms_per_step": 1e3 * t_dom / K, "share_of_step": timing[dom][0] / ms_own,
                  "traffic": NCU_TRAFFIC.get(args.workload), "peak_source": pk["source"],
                  "cell_steps_per_step": W["steps"] / K, "algorithmic_bytes_per_step": W["bytes"] / K,

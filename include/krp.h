@@ -176,6 +176,13 @@ enum { KRP_T_FLIGHT = 0, KRP_T_SCATTER = 1, KRP_T_ORDER = 2, KRP_T_IMAGE = 3, KR
 int krp_timing_enable(krp_grid* g, int on);
 int krp_timing_get(krp_grid* g, double* ms, uint64_t* launches);
 
+/* Measurement utility (bench.py's gather ceiling): the rate at which this GPU serves independent random
+ * gathers of elem_bytes (4 or 16) from an array of array_bytes (1 MiB .. 32 GiB, fewer than 2^32 elements),
+ * every thread of a full grid issuing 64 of them.  This is the ceiling of a cell march whose rays are not
+ * coherent: one gather per cell step from a grid of that size (L2-resident or not).  Allocates and frees its
+ * own array, synchronises, writes gathers per second to *gathers_per_s. */
+int krp_probe_gather(uint64_t array_bytes, int elem_bytes, double* gathers_per_s, void* stream);
+
 /* Number of kernels the library has launched on behalf of g since creation. */
 uint64_t krp_launch_count(const krp_grid* g);
 

@@ -740,6 +740,64 @@ extern "C" int krp_tune(krp_grid* g, int transport_block, int image_block, int b
     return KRP_OK;
 }
 
+// ------------------------------------------------------------------------------------------
+// measurement utility: random-gather rate (include/krp.h)
+// ------------------------------------------------------------------------------------------
+__device__ __forceinline__ uint32_t krp_probe_mix(uint32_t x)
+{
+    x ^= x >> 16; x *= 0x7feb352du; x ^= x >> 15; x *= 0x846ca68bu; x ^= x >> 16;
+    return x;
+}
+template <typename T>
+__global__ void __launch_bounds__(256) krp_k_probe_gather(const T* __restrict__ a, uint32_t n_elem, int iters, float* __restrict__ sink)
+{
+    const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
+    uint32_t h = krp_probe_mix(i * 2654435761u + 12345u);
+    float acc = 0.f;
+    for (int k = 0; k < iters; ++k) {
+        h = krp_probe_mix(h + (uint32_t)k);
+        const T v = __ldg(a + __umulhi(h, n_elem));      // uniform over [0, n_elem)
+        acc += *reinterpret_cast<const float*>(&v);
+    }
+    if (acc == 123.456f) sink[0] = acc;      // never true for a zeroed array: keeps the loads alive
+}
+
+extern "C" int krp_probe_gather(uint64_t array_bytes, int elem_bytes, double* gathers_per_s, void* stream)
+{
+    if (!gathers_per_s) return fail(KRP_ERR_ARG, "gathers_per_s is NULL");
+    if (elem_bytes != 4 && elem_bytes != 16) return fail(KRP_ERR_ARG, "elem_bytes must be 4 or 16");
+    if (array_bytes < (1ull << 20) || array_bytes > (1ull << 35)) return fail(KRP_ERR_ARG, "array_bytes must be in 2^20..2^35");
+    const uint64_t bytes = array_bytes - array_bytes % 16;
+    if (bytes / (uint64_t)elem_bytes >= (1ull << 32)) return fail(KRP_ERR_ARG, "too many elements for the probe");
+    cudaStream_t st = (cudaStream_t)stream;
+    int dev = 0, n_sm = 0;
+    CK(cudaGetDevice(&dev));
+    CK(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
+    void* a = nullptr; float* sink = nullptr;
+    CK(cudaMalloc(&a, bytes));
+    if (cudaMalloc(&sink, sizeof(float)) != cudaSuccess) { cudaFree(a); return fail(KRP_ERR_OOM, "probe allocation failed"); }
+    cudaEvent_t e0 = nullptr, e1 = nullptr;
+    cudaEventCreate(&e0); cudaEventCreate(&e1);
+    cudaMemsetAsync(a, 0, bytes, st);
+    const int iters = 64, blocks = n_sm * 16, tb = 256;
+    const uint32_t mask = (uint32_t)(bytes / (uint64_t)elem_bytes);     // number of elements
+    float ms = 0.f;
+    cudaError_t err = cudaSuccess;
+    for (int rep = 0; rep < 3 && err == cudaSuccess; ++rep) {
+        cudaEventRecord(e0, st);
+        if (elem_bytes == 16) krp_k_probe_gather<float4><<<blocks, tb, 0, st>>>((const float4*)a, mask, iters, sink);
+        else                  krp_k_probe_gather<float><<<blocks, tb, 0, st>>>((const float*)a, mask, iters, sink);
+        cudaEventRecord(e1, st);
+        err = cudaEventSynchronize(e1);
+        if (err == cudaSuccess) err = cudaEventElapsedTime(&ms, e0, e1);
+    }
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    cudaFree(a); cudaFree(sink);
+    if (err != cudaSuccess) return fail(KRP_ERR_CUDA, "probe: %s", cudaGetErrorString(err));
+    *gathers_per_s = (double)blocks * tb * iters / ((double)ms * 1e-3);
+    return KRP_OK;
+}
+
 extern "C" int krp_timing_enable(krp_grid* g, int on)
 {
     if (!g) return fail(KRP_ERR_ARG, "grid is NULL");

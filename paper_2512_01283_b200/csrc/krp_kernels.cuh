@@ -463,6 +463,7 @@ __device__ __forceinline__ void krp_sinh_coshm1_d(double x, double& sh, double& 
         sh = x * (1.0 + z * (1.0 / 6 + z * (1.0 / 120 + z * (1.0 / 5040))));
         chm1 = z * (0.5 + z * (1.0 / 24 + z * (1.0 / 720 + z * (1.0 / 40320))));
     } else {
+        asm volatile("");      // keeps the long series a real branch (ptxas otherwise evaluates both and selects)
         sh = x * (1.0 + z * (1.0 / 6 + z * (1.0 / 120 + z * (1.0 / 5040 + z * (1.0 / 362880 + z * (1.0 / 39916800 +
              z * (1.0 / 6227020800.0 + z * (1.0 / 1307674368000.0))))))));
         chm1 = z * (0.5 + z * (1.0 / 24 + z * (1.0 / 720 + z * (1.0 / 40320 + z * (1.0 / 3628800 + z * (1.0 / 479001600 +
@@ -476,6 +477,7 @@ __device__ __forceinline__ void krp_sin_cosm1_d(double y, double& sy, double& cy
         sy = y * (1.0 - z * (1.0 / 6 - z * (1.0 / 120 - z * (1.0 / 5040))));
         cym1 = -z * (0.5 - z * (1.0 / 24 - z * (1.0 / 720 - z * (1.0 / 40320))));
     } else {
+        asm volatile("");
         sy = y * (1.0 - z * (1.0 / 6 - z * (1.0 / 120 - z * (1.0 / 5040 - z * (1.0 / 362880 - z * (1.0 / 39916800 -
              z * (1.0 / 6227020800.0 - z * (1.0 / 1307674368000.0))))))));
         cym1 = -z * (0.5 - z * (1.0 / 24 - z * (1.0 / 720 - z * (1.0 / 40320 - z * (1.0 / 3628800 - z * (1.0 / 479001600 -
@@ -622,7 +624,14 @@ __global__ void __launch_bounds__(256, KRP_FLIGHT_GENERAL_MIN_BLOCKS) krp_k_flig
                     double i_new, qg, ug, vg, depth;
                     krp_appA_d(i, qg_e, ug_e, vs, cc, i_new, qg, ug, vg, depth);
                     const double Dn = D - depth;
-                    if (near_end && log(i_new) + Dn <= 0.0) { status = KRP_HIT; continue; }   // state stays at cell entry
+                    // ln i >= u - u^2 for u = i - 1 in [-1/2, 0] (and >= 0 above): the fp64 log, which a warp would execute
+                    // for the one or two lanes that are near their event, is taken only when this bound does not already
+                    // rule the event out
+                    if (near_end) {
+                        const double u = i_new - 1.0;
+                        const double lb = u >= 0.0 ? 0.0 : (u >= -0.5 ? u - u * u : -1e300);
+                        if (lb + Dn <= 0.0 && log(i_new) + Dn <= 0.0) { status = KRP_HIT; continue; }   // state stays at cell entry
+                    }
                     qs = c2 * qg - s2 * ug; us = s2 * qg + c2 * ug; vs = vg;
                     i = i_new; D = Dn;
                 }

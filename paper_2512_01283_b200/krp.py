@@ -17,7 +17,7 @@ SYMBOLS = [
     "krp_last_error", "krp_version", "krp_grid_create", "krp_grid_destroy", "krp_source_set",
     "krp_events_reserve", "krp_transport", "krp_packet_id_set", "krp_image", "krp_image_get",
     "krp_image_reset", "krp_stats_get", "krp_stats_reset", "krp_events_get", "krp_events_clear",
-    "krp_tune", "krp_timing_enable", "krp_timing_get", "krp_launch_count",
+    "krp_tune", "krp_timing_enable", "krp_timing_get", "krp_probe_gather", "krp_launch_count",
 ]
 T_FLIGHT, T_SCATTER, T_ORDER, T_IMAGE, T_EMIT, T_COUNT = 0, 1, 2, 3, 4, 5
 T_NAMES = ("flight", "scatter", "order", "image", "emit")
@@ -95,6 +95,7 @@ def lib():
         "krp_tune": (i32, [vp, i32, i32, i32, i32]),
         "krp_timing_enable": (i32, [vp, i32]),
         "krp_timing_get": (i32, [vp, vp, vp]),
+        "krp_probe_gather": (i32, [u64, i32, C.POINTER(C.c_double), vp]),
         "krp_launch_count": (u64, [vp]),
     }
     for name, (res, args) in sig.items():
@@ -132,6 +133,13 @@ def _ptr_mem(a):
         raise TypeError("expected float32")
     a = a.contiguous()
     return C.c_void_p(a.data_ptr()), (MEM_DEVICE if a.is_cuda else MEM_HOST), a
+
+
+def probe_gather(array_bytes, elem_bytes, stream=None):
+    """Random-gather rate of this GPU for an array of that size (gathers/s); measurement utility."""
+    out = C.c_double(0.0)
+    _check(lib().krp_probe_gather(int(array_bytes), int(elem_bytes), C.byref(out), _stream(stream)))
+    return out.value
 
 
 def make_observer(theta, phi, center, half_w, half_h=None):
