@@ -394,24 +394,7 @@ __global__ void __launch_bounds__(256, 4) krp_k_flight_scalar_static(KrpModel g,
 // whose left side is increasing and concave: Newton from R/alpha1 lands left of the root after one step
 // and then rises monotonically.  alpha2 = 0 is the closed form t = R/alpha1.
 // ------------------------------------------------------------------------------------------
-__device__ __forceinline__ double krp_event_solve_d(double R, double qq, double a1, double a2, double tmax)
-{
-    double t = R / a1;
-    if (a2 != 0.0) {
-#pragma unroll 1
-        for (int it = 0; it < 40; ++it) {
-            double x = a2 * t;
-            double sh = sinh(x), ch = cosh(x);
-            double gm1 = (ch - 1.0) - qq * sh;
-            double h = a1 * t - log1p(gm1) - R;
-            double hp = a1 - a2 * (sh - qq * ch) / (1.0 + gm1);
-            double dt = h / hp;
-            t = fmin(fmax(t - dt, 0.0), tmax);
-            if (fabs(dt) <= 4e-16 * t) break;
-        }
-    }
-    return fmin(fmax(t, 0.0), tmax);
-}
+__device__ __forceinline__ double krp_event_solve_d(double R, double qq, double a1, double a2, double tmax);
 
 // 1/sqrt(1+e) for |e| << 1 (unit vectors stored in fp32 have |v|^2 = 1 + O(1e-7))
 __device__ __forceinline__ double krp_rsqrt_near1(double vv)
@@ -485,6 +468,37 @@ __device__ __forceinline__ void krp_sin_cosm1_d(double y, double& sy, double& cy
     }
 }
 
+// (defined here, after the series it uses)  In a thin cell (|alpha2 tmax| < 0.35, every cell of C4 and C5) the
+// hyperbolic functions and the logarithm of the Newton step come from short series instead of the library routines.
+__device__ __forceinline__ double krp_event_solve_d(double R, double qq, double a1, double a2, double tmax)
+{
+    double t = R / a1;
+    if (a2 != 0.0) {
+        const bool thin = fabs(a2 * tmax) < 0.35;
+#pragma unroll 1
+        for (int it = 0; it < 40; ++it) {
+            const double x = a2 * t;
+            double sh, chm1;
+            if (thin) krp_sinh_coshm1_d(x, sh, chm1);
+            else { sh = sinh(x); chm1 = cosh(x) - 1.0; }
+            const double gm1 = chm1 - qq * sh;
+            double lg;
+            if (fabs(gm1) < 0.01) {       // ln(1+g) = g - g^2/2 + ... to g^8 (remainder < 1e-19)
+                lg = gm1 * (1.0 - gm1 * (0.5 - gm1 * (1.0 / 3 - gm1 * (0.25 - gm1 * (0.2 - gm1 * (1.0 / 6 - gm1 * (1.0 / 7 - gm1 * 0.125)))))));
+            } else {
+                asm volatile("");
+                lg = log1p(gm1);
+            }
+            const double h = a1 * t - lg - R;
+            const double hp = a1 - a2 * (sh - qq * (1.0 + chm1)) / (1.0 + gm1);
+            const double dt = h / hp;
+            t = fmin(fmax(t - dt, 0.0), tmax);
+            if (fabs(dt) <= 4e-16 * t) break;
+        }
+    }
+    return fmin(fmax(t, 0.0), tmax);
+}
+
 // Source-free App. A step over the whole cell on the grain-frame state (i, qg, ug, v), fp64, with the common factor
 // e^{-alpha1 dtau} (thin) or e^{-(alpha1 - |alpha2|) dtau} (thick) left to the scalar depth; `depth` is what the
 // scalar depth grows by.
@@ -519,7 +533,8 @@ __device__ __forceinline__ void krp_appA_to_d(double i, double qg, double ug, do
 {
     const double x = a2 * t, y = a3 * t;
     double sy, cy, sh, ch;
-    sincos(y, &sy, &cy);
+    if (fabs(y) < 0.35) { double cym1; krp_sin_cosm1_d(y, sy, cym1); cy = 1.0 + cym1; }
+    else { asm volatile(""); sincos(y, &sy, &cy); }
     if (fabs(x) < 0.35) { double chm1; krp_sinh_coshm1_d(x, sh, chm1); ch = 1.0 + chm1; }
     else { sh = sinh(x); ch = cosh(x); }
     const double it = i * ch - qg * sh;
