@@ -459,7 +459,8 @@ def main():
     line = {
         "metric": METRIC, "value": r["value"], "unit": UNIT, "n_gpus": r["world"], "steps": args.steps, "warmup": args.warmup,
         "ms_per_step": r["ms_total"] / args.steps, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
-        "dtype": "f32 transport, f64 image accumulation", "data": "synthetic",
+        "dtype": ("f32 march with f64 optical depth, f64 image sums" if r["mode"] == "scalar"
+                  else "f64 flights (event location), f32 imaging march, f64 image sums"), "data": "synthetic",
         "config": {"workload": cfg["name"], "grid": [cfg["nx"], cfg["ny"], cfg["nz"]], "packets_per_step_per_gpu": r["batch"],
                    "observers": len(cfg["observers"]), "npix": cfg["npix"], "cell_layout": r["mode"],
                    "job_packets": cfg["n_packets"], "events_per_packet": r["epp"],

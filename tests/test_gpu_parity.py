@@ -300,3 +300,32 @@ def test_scheduling_switches_do_not_change_results(monkeypatch):
             scale = np.abs(img_off[o, 0]).max()
             assert np.abs(img_on[o, s] - img_off[o, s]).max() <= 2e-5 * scale, (o, s)
     assert abs(img_on[:, 0].sum() - img_off[:, 0].sum()) <= 1e-6 * img_off[:, 0].sum()
+
+
+def test_many_observers_and_non_square_images():
+    """More observers than work counters in one rotation (the counters are rewound every 8 launches), a non-square
+    image, off-centre and partly out-of-frame views, in both cell layouts."""
+    import math as m
+    for name, kw in (("c1", dict(n=16, n_packets=3000, npix=24)), ("c4", dict(n=16, n_packets=1500, npix=24))):
+        cfg = inputs.make(name, **kw)
+        obs = []
+        for j in range(11):
+            obs.append(dict(theta=m.radians(10 + 15 * j), phi=m.radians(33 * j), center=[0.05 * (j % 3), -0.04 * (j % 2), 0.02 * j],
+                            half_w=0.35 + 0.03 * j, half_h=0.5 - 0.02 * j))
+        cfg["observers"] = obs
+        n = cfg["n_packets"]
+        from harness import oracle_model, oracle_observers
+        from oracle import OracleEvents, OracleStats
+        mo = oracle_model(cfg)
+        ev = OracleEvents(16 * n); st = OracleStats()
+        mo.transport(0, n, cfg["seed"], ev, st)
+        img_o, img2_o, _ = mo.image(ev, oracle_observers(cfg), 40, 24, flags=0, stats=st)      # npix_x = 40, npix_y = 24
+        g = gpu_grid(cfg)
+        g.transport(n, cfg["seed"])
+        g.image(gpu_observers(cfg), 40, 24)
+        img_g = g.image_get()
+        assert img_g.shape == (11, 4, 24, 40)
+        st_g = g.stats_get()
+        assert st_g["dropped"] > 0 and abs(st_g["dropped"] - st.dropped) <= max(3, 2e-3 * st.dropped)
+        _image_checks(img_g, img_o, img2_o, name + "-11obs")
+        g.close()
