@@ -81,6 +81,13 @@ int krp_grid_create(krp_grid** out, int nx, int ny, int nz, const double bounds[
                     const krp_tables* tables, void* stream);
 int krp_grid_destroy(krp_grid* g);
 
+/* Replace the density (and field) of an existing model, e.g. the next snapshot of the simulation the dust
+ * belongs to (the method runs inside a hydrodynamics code): same dimensions, bounds and tables,
+ * arrays laid out as for krp_grid_create, bfield non-NULL exactly when the model was created with one.
+ * Re-packs the cells without re-allocating anything; buffered events and image maps are left as they are.
+ * Synchronises (it reports bad densities).  Errors as krp_grid_create. */
+int krp_grid_update(krp_grid* g, const float* density, const float* bfield, int mem, void* stream);
+
 /* Source of packets (PAPER.md:107 emission; R17).
  *   kind bit0: 0 = all packets start at pos, 1 = start uniformly inside a cell drawn with
  *              probability proportional to cell_weight (DEVICE, [ncell]; NULL = uniform);

@@ -41,6 +41,11 @@ struct krp_grid {
     float4* d_cell = nullptr;       // = d_cell_alloc + margin
     float* d_kr_alloc = nullptr;
     float4* d_cell_alloc = nullptr;
+    float* d_stage_den = nullptr;   // staging of host inputs (krp_grid_create / krp_grid_update with KRP_MEM_HOST)
+    float* d_stage_b = nullptr;
+    int* d_bad = nullptr;
+    bool has_bfield = false;
+    bool obs_cells_stale = false;   // cells changed since the per-observer coefficient arrays were built
     float4* d_opac = nullptr;
     float4* d_opA = nullptr;
     float4* d_opB = nullptr;
@@ -130,7 +135,7 @@ static int alloc_records(KrpRecords& r, uint64_t cap, bool with_tau)
 extern "C" int krp_grid_destroy(krp_grid* g)
 {
     if (!g) return KRP_OK;
-    cudaFree(g->d_kr_alloc); cudaFree(g->d_cell_alloc); cudaFree(g->d_opac); cudaFree(g->d_mueller); cudaFree(g->d_cdf);
+    cudaFree(g->d_kr_alloc); cudaFree(g->d_cell_alloc); cudaFree(g->d_stage_den); cudaFree(g->d_stage_b); cudaFree(g->d_bad); cudaFree(g->d_opac); cudaFree(g->d_mueller); cudaFree(g->d_cdf);
     cudaFree(g->d_src_cdf); cudaFree(g->d_ctl); cudaFree(g->d_obs); cudaFree(g->d_img); cudaFree(g->d_obs_cells);
     cudaFree(g->d_opA); cudaFree(g->d_opB); cudaFree(g->d_opA_d); cudaFree(g->d_opB_d); cudaFree(g->d_bins); cudaFree(g->d_perm); cudaFree(g->d_scan);
     cudaFree(g->d_dir_bins); cudaFree(g->d_dir_scan); cudaFree(g->d_order);
@@ -162,6 +167,39 @@ static int check_tables(const krp_tables* t)
         if (!(a[0] > std::fabs(a[1]))) return fail(KRP_ERR_ARG, "tables: alpha1 must exceed |alpha2| (node %d)", j);
         if (!(a[3] >= 0.f && a[3] <= 1.f)) return fail(KRP_ERR_ARG, "tables: albedo outside [0,1] (node %d)", j);
     }
+    return KRP_OK;
+}
+
+// T0: (re)pack the caller's density / field arrays into the padded cell array of g (halo included)
+static int upload_cells(krp_grid* g, const float* density, const float* bfield, int mem, cudaStream_t st)
+{
+    KrpModel& m = g->m;
+    const float* d_den = density;
+    const float* d_b = bfield;
+    const bool want_b = bfield && !m.scalar;
+    if (mem == KRP_MEM_HOST) {
+        // staging buffers are kept for later krp_grid_update calls
+        if (!g->d_stage_den) CK(cudaMalloc(&g->d_stage_den, sizeof(float) * (size_t)m.ncell));
+        CK(cudaMemcpyAsync(g->d_stage_den, density, sizeof(float) * (size_t)m.ncell, cudaMemcpyHostToDevice, st));
+        d_den = g->d_stage_den;
+        if (want_b) {
+            if (!g->d_stage_b) CK(cudaMalloc(&g->d_stage_b, sizeof(float) * 3 * (size_t)m.ncell));
+            CK(cudaMemcpyAsync(g->d_stage_b, bfield, sizeof(float) * 3 * (size_t)m.ncell, cudaMemcpyHostToDevice, st));
+            d_b = g->d_stage_b;
+        }
+    }
+    if (!g->d_bad) CK(cudaMalloc(&g->d_bad, sizeof(int)));
+    CK(cudaMemsetAsync(g->d_bad, 0, sizeof(int), st));
+    const int tb = 256;
+    const unsigned nb = (unsigned)((g->npad + tb - 1) / tb);
+    krp_k_pack<<<nb, tb, 0, st>>>(m, d_den, want_b ? d_b : nullptr, g->npad, g->d_cell, g->d_kr, g->d_bad);
+    CK(cudaGetLastError());
+    g->launches++;
+    int bad = 0;
+    CK(cudaMemcpyAsync(&bad, g->d_bad, sizeof(int), cudaMemcpyDeviceToHost, st));
+    CK(cudaStreamSynchronize(st));
+    if (bad) return fail(KRP_ERR_ARG, "density has %d negative, NaN or infinite cells", bad);
+    g->obs_cells_stale = true;
     return KRP_OK;
 }
 
@@ -291,48 +329,24 @@ extern "C" int krp_grid_create(krp_grid** out, int nx, int ny, int nz, const dou
     CK(cudaMemcpyAsync(g->d_cdf, cdf.data(), sizeof(double) * m.n_ang, cudaMemcpyHostToDevice, st));
     m.opac = g->d_opac; m.mueller = g->d_mueller; m.cdf = g->d_cdf;
 
-    // cells: packed into the padded layout (one-cell halo with kappa*rho = -1)
-    const float* d_den = density;
-    const float* d_b = bfield;
-    float* tmp_den = nullptr;
-    float* tmp_b = nullptr;
-    if (mem == KRP_MEM_HOST) {
-        CK(cudaMalloc(&tmp_den, sizeof(float) * (size_t)m.ncell));
-        CK(cudaMemcpyAsync(tmp_den, density, sizeof(float) * (size_t)m.ncell, cudaMemcpyHostToDevice, st));
-        d_den = tmp_den;
-        if (bfield && !m.scalar) {
-            CK(cudaMalloc(&tmp_b, sizeof(float) * 3 * (size_t)m.ncell));
-            CK(cudaMemcpyAsync(tmp_b, bfield, sizeof(float) * 3 * (size_t)m.ncell, cudaMemcpyHostToDevice, st));
-            d_b = tmp_b;
+    // cells: packed into the padded layout (one-cell halo with kappa*rho = -1).  A margin of one padded plane on
+    // either side keeps the look-ahead loads of the marches (one cell past the halo cell that ends a ray) inside
+    // the allocation; its content is never used.
+    {
+        const size_t margin = m.pxy, n_alloc = (size_t)g->npad + 2 * margin;
+        if (m.scalar) {
+            CK(cudaMalloc(&g->d_kr_alloc, sizeof(float) * n_alloc));
+            CK(cudaMemsetAsync(g->d_kr_alloc, 0xff, sizeof(float) * n_alloc, st));
+            g->d_kr = g->d_kr_alloc + margin;
+        } else {
+            CK(cudaMalloc(&g->d_cell_alloc, sizeof(float4) * n_alloc));
+            CK(cudaMemsetAsync(g->d_cell_alloc, 0xff, sizeof(float4) * n_alloc, st));
+            g->d_cell = g->d_cell_alloc + margin;
         }
     }
-    int* d_bad = nullptr;
-    CK(cudaMalloc(&d_bad, sizeof(int)));
-    CK(cudaMemsetAsync(d_bad, 0, sizeof(int), st));
-    // a margin of one padded plane on either side keeps the imaging march's look-ahead load (one cell past the
-    // halo cell that ends the ray) inside the allocation; its content is never used
-    const size_t margin = m.pxy, n_alloc = (size_t)g->npad + 2 * margin;
-    if (m.scalar) {
-        CK(cudaMalloc(&g->d_kr_alloc, sizeof(float) * n_alloc));
-        CK(cudaMemsetAsync(g->d_kr_alloc, 0xff, sizeof(float) * n_alloc, st));
-        g->d_kr = g->d_kr_alloc + margin;
-    } else {
-        CK(cudaMalloc(&g->d_cell_alloc, sizeof(float4) * n_alloc));
-        CK(cudaMemsetAsync(g->d_cell_alloc, 0xff, sizeof(float4) * n_alloc, st));
-        g->d_cell = g->d_cell_alloc + margin;
-    }
-    {
-        const int tb = 256;
-        const unsigned nb = (unsigned)((g->npad + tb - 1) / tb);
-        krp_k_pack<<<nb, tb, 0, st>>>(m, d_den, m.scalar ? nullptr : d_b, g->npad, g->d_cell, g->d_kr, d_bad);
-        CK(cudaGetLastError());
-        g->launches++;
-    }
-    int bad = 0;
-    CK(cudaMemcpyAsync(&bad, d_bad, sizeof(int), cudaMemcpyDeviceToHost, st));
-    CK(cudaStreamSynchronize(st));
-    cudaFree(d_bad); cudaFree(tmp_den); cudaFree(tmp_b);
-    if (bad) return fail(KRP_ERR_ARG, "density has %d negative, NaN or infinite cells", bad);
+    g->has_bfield = bfield != nullptr;
+    rc = upload_cells(g, density, bfield, mem, st);
+    if (rc) return rc;
     m.kr = g->d_kr; m.cell = g->d_cell;
     // bins of the imaging order: one cache line of cells per bin (32 x 4 B or 8 x 16 B), at most 2^25 bins
     g->bin_shift = m.scalar ? 5 : 3;
@@ -359,6 +373,14 @@ extern "C" int krp_grid_create(krp_grid** out, int nx, int ny, int nz, const dou
     if (rc) { krp_grid_destroy(g); return rc; }
     *out = g;
     return KRP_OK;
+}
+
+extern "C" int krp_grid_update(krp_grid* g, const float* density, const float* bfield, int mem, void* stream)
+{
+    if (!g || !density) return fail(KRP_ERR_ARG, "grid or density is NULL");
+    if (mem != KRP_MEM_DEVICE && mem != KRP_MEM_HOST) return fail(KRP_ERR_ARG, "mem must be KRP_MEM_DEVICE or KRP_MEM_HOST");
+    if ((bfield != nullptr) != g->has_bfield) return fail(KRP_ERR_ARG, "bfield must be given exactly when the grid was created with one");
+    return upload_cells(g, density, bfield, mem, (cudaStream_t)stream);
 }
 
 extern "C" int krp_source_set(krp_grid* g, const krp_source* src, void* stream)
@@ -584,12 +606,22 @@ extern "C" int krp_image(krp_grid* g, const krp_observer* obs, int n_obs, int np
                     krp_k_obs_cells<<<nb, 256, 0, st>>>(g->m, od[o], g->npad, g->d_obs_cells + (size_t)o * g->npad);
                 CK(cudaGetLastError());
                 g->launches += (uint64_t)n_obs;
+                g->obs_cells_stale = false;
             } else {
                 cudaGetLastError();
                 g->d_obs_cells = nullptr;
             }
         }
         g->n_obs = n_obs; g->npx = npix_x; g->npy = npix_y;
+    }
+    if (g->d_obs_cells && g->obs_cells_stale) {
+        // the cells changed (krp_grid_update) since the coefficient arrays were built
+        const unsigned nb = (unsigned)((g->npad + 255u) / 256u);
+        for (int o = 0; o < n_obs; ++o)
+            krp_k_obs_cells<<<nb, 256, 0, st>>>(g->m, g->obs_dev[o], g->npad, g->d_obs_cells + (size_t)o * g->npad);
+        CK(cudaGetLastError());
+        g->launches += (uint64_t)n_obs;
+        g->obs_cells_stale = false;
     }
     if (g->ev_cap == 0) return KRP_OK;   // nothing was ever transported
     if (g->ev_cap >= (1ull << 32)) return fail(KRP_ERR_ARG, "krp_image handles at most 2^32-1 buffered events per call");

@@ -14,7 +14,7 @@ OK, ERR_ARG, ERR_CUDA, ERR_OOM, ERR_STATE, ERR_EVENT_FULL = 0, -1, -2, -3, -4, -
 MEM_DEVICE, MEM_HOST = 0, 1
 
 SYMBOLS = [
-    "krp_last_error", "krp_version", "krp_grid_create", "krp_grid_destroy", "krp_source_set",
+    "krp_last_error", "krp_version", "krp_grid_create", "krp_grid_destroy", "krp_grid_update", "krp_source_set",
     "krp_events_reserve", "krp_transport", "krp_packet_id_set", "krp_image", "krp_image_get",
     "krp_image_reset", "krp_stats_get", "krp_stats_reset", "krp_events_get", "krp_events_clear",
     "krp_tune", "krp_timing_enable", "krp_timing_get", "krp_probe_gather", "krp_launch_count",
@@ -81,6 +81,7 @@ def lib():
         "krp_grid_create": (i32, [C.POINTER(vp), i32, i32, i32, C.POINTER(C.c_double), vp, vp, i32,
                                   C.POINTER(Tables), vp]),
         "krp_grid_destroy": (i32, [vp]),
+        "krp_grid_update": (i32, [vp, vp, vp, i32, vp]),
         "krp_source_set": (i32, [vp, C.POINTER(Source), vp]),
         "krp_events_reserve": (i32, [vp, u64]),
         "krp_transport": (i32, [vp, u64, u64, vp]),
@@ -183,6 +184,14 @@ class Grid:
             self.close()
         except Exception:
             pass
+
+    def update(self, density, bfield=None, stream=None):
+        """New density (and field) for the same grid: arrays as for the constructor."""
+        dptr, dmem, dkeep = _ptr_mem(density)
+        bptr, bmem, bkeep = _ptr_mem(bfield)
+        if bptr is not None and bmem != dmem:
+            raise ValueError("density and bfield must live in the same memory space")
+        _check(lib().krp_grid_update(self._h, dptr, bptr, dmem, _stream(stream)))
 
     def source_set(self, kind=0, pos=None, direction=(0, 0, 1), cell_weight=None, emit_records=0, stream=None):
         s = Source()

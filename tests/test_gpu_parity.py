@@ -329,3 +329,40 @@ def test_many_observers_and_non_square_images():
         assert st_g["dropped"] > 0 and abs(st_g["dropped"] - st.dropped) <= max(3, 2e-3 * st.dropped)
         _image_checks(img_g, img_o, img2_o, name + "-11obs")
         g.close()
+
+
+def test_grid_update_equals_a_new_grid():
+    """krp_grid_update (next snapshot on the same grid) gives what a grid created from the new arrays gives, in both
+    cell layouts, from host and device arrays, with the per-observer coefficient arrays refreshed."""
+    import torch
+    for name, kw in (("c2", dict(n=24, n_packets=4000, npix=24)), ("c4", dict(n=16, n_packets=3000, npix=24))):
+        cfg = inputs.make(name, **kw)
+        rng = np.random.default_rng(3)
+        dens2 = (cfg["density"] * rng.uniform(0.5, 1.5, size=cfg["density"].shape)).astype(np.float32)
+        bf2 = None if cfg["bfield"] is None else (cfg["bfield"] + 0.3 * rng.normal(size=cfg["bfield"].shape)).astype(np.float32)
+        g = gpu_grid(cfg)
+        g.transport(500, cfg["seed"]); g.image(gpu_observers(cfg), cfg["npix"], cfg["npix"])     # builds the coefficient arrays
+        g.image_reset(); g.stats_reset(); g.packet_id_set(0)
+        g.update(dens2, bf2)                                                                       # host arrays
+        g.transport(cfg["n_packets"], cfg["seed"])
+        ev_u = gpu_events_sorted(g)
+        g.image(gpu_observers(cfg), cfg["npix"], cfg["npix"])
+        img_u = g.image_get()
+        cfg2 = dict(cfg, density=dens2, bfield=bf2)
+        h = gpu_grid(cfg2)
+        h.transport(cfg["n_packets"], cfg["seed"])
+        ev_n = gpu_events_sorted(h)
+        h.image(gpu_observers(cfg), cfg["npix"], cfg["npix"])
+        img_n = h.image_get()
+        for key in ev_n:
+            assert np.array_equal(ev_u[key], ev_n[key]), (name, key)
+        assert np.allclose(img_u, img_n, rtol=1e-11, atol=1e-13 * img_n[:, 0].max())
+        # device arrays, and argument errors
+        g.update(torch.from_numpy(dens2).cuda(), None if bf2 is None else torch.from_numpy(bf2).cuda())
+        from paper_2512_01283_b200 import krp
+        with pytest.raises(krp.KrpError):
+            g.update(-dens2, bf2)
+        if bf2 is not None:
+            with pytest.raises(krp.KrpError):
+                g.update(dens2, None)
+        g.close(); h.close()
