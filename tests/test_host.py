@@ -135,3 +135,30 @@ def test_input_recipe_is_seeded_and_valid():
     c2 = inputs.make("c2", n=32, n_packets=10, npix=8)
     row = c2["density"][16, 16, 16:]
     assert abs(row.sum() * (1.0 / 32) - 20.0) < 1e-3                       # midplane tau = 20 centre -> edge
+
+
+def test_bench_reference_arm_runs_without_a_gpu():
+    """`bench.py --impl reference` times the oracle on host cores and prints one JSON line with the contract's keys;
+    under torchrun only rank 0 prints."""
+    import json
+    cmd = [sys.executable, os.path.join(ROOT, "bench.py"), "--impl", "reference", "--workload", "c1", "--n", "8",
+           "--steps", "1", "--warmup", "1"]
+    out = subprocess.check_output(cmd, text=True, timeout=600, env=dict(os.environ, RANK="0", WORLD_SIZE="1"))
+    line = json.loads(out.strip().splitlines()[-1])
+    for key in ("impl", "metric", "value", "unit", "n_gpus", "steps", "warmup", "ms_per_step", "higher_is_better", "scaling",
+                "vs_baseline", "dtype", "data", "config", "cpu_baseline", "e2e"):
+        assert key in line, key
+    assert line["impl"] == "reference" and line["value"] > 0 and line["unit"] == "packets/s"
+    assert line["cpu_baseline"]["kind"] == "oracle" and line["cpu_baseline"]["cores"] == 1
+    assert line["e2e"]["h2d_bytes_per_step"] == 0 and line["e2e"]["d2h_bytes_per_step"] == 0
+    out = subprocess.check_output(cmd, text=True, timeout=600, env=dict(os.environ, RANK="1", WORLD_SIZE="2"))
+    assert out.strip() == ""
+
+
+def test_bench_refuses_to_run_the_product_arm_without_a_gpu():
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("a GPU is present")
+    p = subprocess.run([sys.executable, os.path.join(ROOT, "bench.py"), "--workload", "c1", "--n", "8", "--steps", "1"],
+                       capture_output=True, text=True, timeout=600)
+    assert p.returncode != 0 and "no CPU fallback" in (p.stderr + p.stdout)
