@@ -135,7 +135,8 @@ typedef struct krp_observer {
  * records (direct light).  Clears the event buffer afterwards.  The maps are (re)allocated
  * and zeroed when the observer set or the pixel counts differ from the previous call; with a field
  * (16-byte cells) the call then also tabulates 16 bytes per cell and observer if that fits in device memory.
- * Does not synchronise except on such a change. */
+ * Does not synchronise except on such a change.  The order in which the events are imaged is not defined
+ * (they are ordered by cell when the rays of earlier passes were long enough for that to pay). */
 int krp_image(krp_grid* g, const krp_observer* obs, int n_obs, int npix_x, int npix_y,
               int flags, void* stream);
 /* Copy the maps to out ([n_obs][4][npix_y][npix_x] doubles; `mem` = where out lives).

@@ -77,6 +77,13 @@ struct krp_grid {
     uint64_t ev_cap = 0;
     bool ev_reserved = false;
     KrpObserverDev* d_obs = nullptr;
+    // ordering of the events before imaging: policy 0 never, 1 by the measured ray length, 2 always
+    int order_policy = 1;
+    bool order_events = true;
+    unsigned long long* h_ray_stats = nullptr;          // pinned: steps_image, contributions, dropped
+    unsigned long long ray_stats_prev[3] = { 0, 0, 0 };
+    cudaEvent_t ray_stats_ev = nullptr;
+    bool ray_stats_pending = false;
     float4* d_obs_cells = nullptr;  // [n_obs][npad] per-observer cell coefficients (general mode), or NULL
     int obs_pre = 1;
     double* d_img = nullptr;
@@ -141,6 +148,8 @@ extern "C" int krp_grid_destroy(krp_grid* g)
     cudaFree(g->d_dir_bins); cudaFree(g->d_dir_scan); cudaFree(g->d_order);
     free_records(g->q[0]); free_records(g->q[1]); free_records(g->ev);
     for (cudaEvent_t e : g->t_ev) cudaEventDestroy(e);
+    if (g->h_ray_stats) cudaFreeHost(g->h_ray_stats);
+    if (g->ray_stats_ev) cudaEventDestroy(g->ray_stats_ev);
     delete g;
     return KRP_OK;
 }
@@ -266,6 +275,8 @@ extern "C" int krp_grid_create(krp_grid** out, int nx, int ny, int nz, const dou
     g->burst = m.scalar ? 1 : 32;
     if (getenv("KRP_NO_DIR_SORT")) g->dir_sort = 0;   // A/B switches for measurement
     if (getenv("KRP_NO_OBS_PRE")) g->obs_pre = 0;
+    if (getenv("KRP_ORDER_POLICY")) g->order_policy = atoi(getenv("KRP_ORDER_POLICY"));
+    g->order_events = g->order_policy != 0;
     m.n_inc = n_inc; m.n_ang = tables->n_ang;
     m.w_min = tables->w_min; m.max_scatter = tables->max_scatter;
     // number of waves that can contain live packets: the weight after k scatterings is <= omega_max^k
@@ -631,15 +642,31 @@ extern "C" int krp_image(krp_grid* g, const krp_observer* obs, int n_obs, int np
         CK(cudaMalloc(&g->d_perm, sizeof(unsigned int) * g->ev_cap));
         g->perm_cap = g->ev_cap;
     }
-    // I0: order the events by cell bin (count, scan, scatter)
+    // I0: order the events by cell bin (count, scan, scatter) -- unless the rays of this model are so short that the
+    // order does not pay: the decision follows the cell steps per ray of the previous imaging passes, read back
+    // without waiting (a pinned copy of the counters taken after every pass; the first passes are ordered)
     const unsigned pers = (unsigned)(g->n_sm * g->blocks_per_sm);
+    if (g->h_ray_stats && g->ray_stats_pending && cudaEventQuery(g->ray_stats_ev) == cudaSuccess) {
+        // (the counters may have been reset by krp_stats_reset in between: then they count from zero)
+        auto delta = [&](int j) { return g->h_ray_stats[j] >= g->ray_stats_prev[j] ? g->h_ray_stats[j] - g->ray_stats_prev[j] : g->h_ray_stats[j]; };
+        const unsigned long long steps = delta(0), rays = delta(1) + delta(2);
+        if (rays > 0) g->order_events = g->order_policy == 2 || (g->order_policy == 1 && (double)steps / (double)rays >= 12.0);
+        g->ray_stats_prev[0] = g->h_ray_stats[0]; g->ray_stats_prev[1] = g->h_ray_stats[1]; g->ray_stats_prev[2] = g->h_ray_stats[2];
+        g->ray_stats_pending = false;
+    }
+    const unsigned int* perm = g->order_events ? g->d_perm : nullptr;
     { TimedLaunch tlo(g, st, KRP_T_ORDER);
-    CK(cudaMemsetAsync(g->d_bins, 0, sizeof(unsigned int) * ((size_t)g->n_bins + 1), st));
-    krp_k_sort_count<<<pers, 256, 0, st>>>(g->d_ctl, g->ev, g->bin_shift, g->sub_bits, flags, g->d_bins);
-    CK(cub::DeviceScan::ExclusiveSum(g->d_scan, g->scan_bytes, g->d_bins, g->d_bins, (int)(g->n_bins + 1), st));
-    krp_k_image_prep<<<1, 1, 0, st>>>(g->d_ctl, g->d_bins, g->n_bins);
-    krp_k_sort_scatter<<<pers, 256, 0, st>>>(g->d_ctl, g->ev, g->bin_shift, g->sub_bits, flags, g->d_bins, g->d_perm); }
-    g->launches += 5;   // count, scan (2 kernels), prep, scatter
+    if (g->order_events) {
+        CK(cudaMemsetAsync(g->d_bins, 0, sizeof(unsigned int) * ((size_t)g->n_bins + 1), st));
+        krp_k_sort_count<<<pers, 256, 0, st>>>(g->d_ctl, g->ev, g->bin_shift, g->sub_bits, flags, g->d_bins);
+        CK(cub::DeviceScan::ExclusiveSum(g->d_scan, g->scan_bytes, g->d_bins, g->d_bins, (int)(g->n_bins + 1), st));
+        krp_k_image_prep<<<1, 1, 0, st>>>(g->d_ctl, g->d_bins, g->n_bins);
+        krp_k_sort_scatter<<<pers, 256, 0, st>>>(g->d_ctl, g->ev, g->bin_shift, g->sub_bits, flags, g->d_bins, g->d_perm);
+        g->launches += 5;   // count, scan (2 kernels), prep, scatter
+    } else {
+        krp_k_image_prep_plain<<<1, 1, 0, st>>>(g->d_ctl);
+        g->launches++;
+    } }
     // I1-I3: one launch per observer (its constants are kernel parameters); launches rotate over
     // KRP_MAX_OBS_PACK work counters, rewound when the rotation wraps
     const int tb = g->image_block;
@@ -649,17 +676,29 @@ extern "C" int krp_image(krp_grid* g, const krp_observer* obs, int n_obs, int np
         if (o > 0 && slot == 0) { krp_k_image_rewind<<<1, 1, 0, st>>>(g->d_ctl); g->launches++; }
         TimedLaunch tli(g, st, KRP_T_IMAGE);
         if (g->m.scalar)
-            krp_k_image<true, false><<<pers, tb, 0, st>>>(g->m, g->d_ctl, g->ev, g->d_perm, g->obs_dev[o], nullptr, slot, o, npix_x, npix_y, g->d_img);
+            krp_k_image<true, false><<<pers, tb, 0, st>>>(g->m, g->d_ctl, g->ev, perm, g->obs_dev[o], nullptr, slot, o, npix_x, npix_y, flags, g->d_img);
         else if (g->d_obs_cells)
-            krp_k_image<false, true><<<pers, tb, 0, st>>>(g->m, g->d_ctl, g->ev, g->d_perm, g->obs_dev[o],
-                                                          g->d_obs_cells + (size_t)o * g->npad, slot, o, npix_x, npix_y, g->d_img);
+            krp_k_image<false, true><<<pers, tb, 0, st>>>(g->m, g->d_ctl, g->ev, perm, g->obs_dev[o],
+                                                          g->d_obs_cells + (size_t)o * g->npad, slot, o, npix_x, npix_y, flags, g->d_img);
         else
-            krp_k_image<false, false><<<pers, tb, smem, st>>>(g->m, g->d_ctl, g->ev, g->d_perm, g->obs_dev[o], nullptr, slot, o, npix_x, npix_y, g->d_img);
+            krp_k_image<false, false><<<pers, tb, smem, st>>>(g->m, g->d_ctl, g->ev, perm, g->obs_dev[o], nullptr, slot, o, npix_x, npix_y, flags, g->d_img);
         g->launches++;
     }
     krp_k_events_clear<<<1, 1, 0, st>>>(g->d_ctl);
     g->launches++;
     CK(cudaGetLastError());
+    // counters of this pass for the ordering decision of a later one (never waited for)
+    if (g->order_policy == 1 && !g->ray_stats_pending) {
+        if (!g->h_ray_stats) {
+            CK(cudaMallocHost(&g->h_ray_stats, 3 * sizeof(unsigned long long)));
+            g->h_ray_stats[0] = g->h_ray_stats[1] = g->h_ray_stats[2] = 0;
+            CK(cudaEventCreateWithFlags(&g->ray_stats_ev, cudaEventDisableTiming));
+        }
+        // steps_image, contributions, dropped are consecutive in KrpStatsDev
+        CK(cudaMemcpyAsync(g->h_ray_stats, &g->d_ctl->stats.steps_image, 3 * sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
+        CK(cudaEventRecord(g->ray_stats_ev, st));
+        g->ray_stats_pending = true;
+    }
     return KRP_OK;
 }
 

@@ -895,6 +895,15 @@ __global__ void krp_k_image_prep(KrpCtl* ctl, const unsigned int* __restrict__ b
     ctl->n_sorted = bins[n_bins];
     for (int o = 0; o < KRP_MAX_OBS_PACK; ++o) ctl->img_work[o] = 0;
 }
+// the same without an order: every buffered event takes part in the order of the buffer (perm = NULL in the
+// imaging kernel, which then skips emission records itself when they are not wanted)
+__global__ void krp_k_image_prep_plain(KrpCtl* ctl)
+{
+    unsigned long long n_ev = ctl->n_events;
+    if (n_ev > ctl->ev_cap) n_ev = ctl->ev_cap;
+    ctl->n_sorted = (unsigned int)n_ev;
+    for (int o = 0; o < KRP_MAX_OBS_PACK; ++o) ctl->img_work[o] = 0;
+}
 __global__ void krp_k_image_rewind(KrpCtl* ctl)
 {
     for (int o = 0; o < KRP_MAX_OBS_PACK; ++o) ctl->img_work[o] = 0;
@@ -1004,7 +1013,7 @@ template <bool SCALAR, bool PRE>
 __global__ void __launch_bounds__(256, SCALAR ? KRP_IMAGE_SCALAR_MIN_BLOCKS : KRP_IMAGE_MIN_BLOCKS) krp_k_image(KrpModel g, KrpCtl* ctl, KrpRecords ev,
                                                    const unsigned int* __restrict__ perm, const KrpObserverDev ob,
                                                    const float4* __restrict__ obs_cell,
-                                                   int slot, int obs_index, int npx, int npy, double* __restrict__ img)
+                                                   int slot, int obs_index, int npx, int npy, int flags, double* __restrict__ img)
 {
     extern __shared__ float4 s_tab[];                // [2*(n_inc-1)]: intercepts, slopes of the opacity table
     const int nseg = g.n_inc - 1;
@@ -1022,12 +1031,18 @@ __global__ void __launch_bounds__(256, SCALAR ? KRP_IMAGE_SCALAR_MIN_BLOCKS : KR
         if (lane == 0) base = atomicAdd(&ctl->img_work[slot], 32u);
         base = __shfl_sync(0xffffffffu, base, 0);
         if (base >= n_ev) break;
-        const bool live = base + lane < n_ev;
+        bool live = base + lane < n_ev;
         int pixel = -1;
         float out[4] = { 0.f, 0.f, 0.f, 0.f };
+        const unsigned int e = live ? (perm ? perm[base + lane] : base + lane) : 0u;
+        float4 nk = make_float4(0.f, 0.f, 1.f, 0.f);
         if (live) {
-            const unsigned int e = perm[base + lane];
-            const float4 nk = ev.nk[e], pc = ev.pc[e], Se = ev.S[e];
+            nk = ev.nk[e];
+            // without an order (perm = NULL) emission records are still in the list: they take part only with direct light
+            if (!perm && (__float_as_uint(nk.w) & ~KRP_TERM_BIT) == 0u && !(flags & 1)) live = false;
+        }
+        if (live) {
+            const float4 pc = ev.pc[e], Se = ev.S[e];
             const uint32_t k = __float_as_uint(nk.w) & ~KRP_TERM_BIT;
             float S[4];
             if (k == 0u) { S[0] = Se.x * 0.07957747154594767f; S[1] = S[2] = S[3] = 0.f; }

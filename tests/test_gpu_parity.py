@@ -272,14 +272,15 @@ def test_launch_shapes_do_not_change_results():
 
 
 def test_scheduling_switches_do_not_change_results(monkeypatch):
-    """The two scheduling features that only large batches / general mode reach -- direction-ordered first flights of a
-    point source (emission computed inside the flight kernel) and per-observer cell coefficient arrays in the imaging
-    march -- against the plain paths (A/B switches read at krp_grid_create): events bit-identical, maps equal to the
-    rounding of the fp32 march."""
+    """The scheduling features that only large batches / general mode reach -- direction-ordered first flights of a
+    point source (emission computed inside the flight kernel), per-observer cell coefficient arrays in the imaging
+    march, events ordered by cell before imaging (policy 2: always, 0: never; the default decides by the measured
+    ray length) -- against the plain paths (A/B switches read at krp_grid_create): events bit-identical, maps equal
+    to the rounding of the fp32 march."""
     cfg = inputs.make("c5", n=32, n_packets=70000, npix=48)          # point source, general mode, >= 2^16 packets
     res = {}
-    for label, env in (("on", {}), ("off", {"KRP_NO_DIR_SORT": "1", "KRP_NO_OBS_PRE": "1"})):
-        for k in ("KRP_NO_DIR_SORT", "KRP_NO_OBS_PRE"):
+    for label, env in (("on", {"KRP_ORDER_POLICY": "2"}), ("off", {"KRP_NO_DIR_SORT": "1", "KRP_NO_OBS_PRE": "1", "KRP_ORDER_POLICY": "0"})):
+        for k in ("KRP_NO_DIR_SORT", "KRP_NO_OBS_PRE", "KRP_ORDER_POLICY"):
             monkeypatch.delenv(k, raising=False)
         for k, v in env.items():
             monkeypatch.setenv(k, v)
