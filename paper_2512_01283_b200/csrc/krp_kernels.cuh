@@ -689,7 +689,7 @@ __device__ __forceinline__ void krp_rot_qu(double& Q, double& U, double c2, doub
 // of the wave, fp64.  Draws of block 0 of event k: (Theta, phi candidate, accept, next tau*);
 // blocks >= 1: two more (phi, accept) pairs each, at most 64 rounds.
 // ------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(128) krp_k_scatter(KrpModel g, KrpCtl* ctl, KrpRecords ev, KrpRecords qo, int out,
+__global__ void __launch_bounds__(128, 8) krp_k_scatter(KrpModel g, KrpCtl* ctl, KrpRecords ev, KrpRecords qo, int out,
                                                      unsigned long long seed)
 {
     const unsigned long long e0 = ctl->ev_begin;
