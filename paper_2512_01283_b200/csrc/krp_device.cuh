@@ -235,8 +235,9 @@ struct KrpRayD {
 
 __device__ __forceinline__ void krp_rayd_axis(float n, float p, double d, int stride, double& r, double& t, int& s)
 {
-    if (n > 0.f)      { r = (1.0 - (double)p) * d / (double)n; t = d / (double)n;  s = stride; }
-    else if (n < 0.f) { r = (double)p * d / -(double)n;        t = d / -(double)n; s = -stride; }
+    // one division per axis: the distance to the first face is that fraction of the face spacing (1e-16 from the other order)
+    if (n > 0.f)      { t = d / (double)n;  r = (1.0 - (double)p) * t; s = stride; }
+    else if (n < 0.f) { t = d / -(double)n; r = (double)p * t;         s = -stride; }
     else              { t = __longlong_as_double(0x7ff0000000000000ll); r = t; s = 0; }
 }
 
@@ -263,10 +264,10 @@ __device__ __forceinline__ void krp_rayd_step(KrpRayD& r, double ds)
 }
 
 // cell-local position (fp64 distances) after moving `moved` from the point where r was taken
-__device__ __forceinline__ float krp_locald(float n, double r, double t, double moved, float p0)
+__device__ __forceinline__ float krp_locald(float n, double r, double inv_d, double moved, float p0)
 {
     if (n == 0.f) return p0;
-    double f = (r - moved) / t;
+    double f = (r - moved) * fabs((double)n) * inv_d;      // 1/t = |n|/d
     f = fmin(fmax(f, 0.0), 1.0);
     return (float)(n > 0.f ? 1.0 - f : f);
 }

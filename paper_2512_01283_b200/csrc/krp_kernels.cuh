@@ -588,9 +588,9 @@ __global__ void __launch_bounds__(256, KRP_FLIGHT_GENERAL_MIN_BLOCKS) krp_k_flig
             krp_item_load(g, q, es, item, pc, nk, S0_, tau_, id_);
             const float n[3] = { nk.x, nk.y, nk.z };
             float pe[3];
-            pe[0] = krp_locald(n[0], ray.rx, ray.tx, moved, pc.x);
-            pe[1] = krp_locald(n[1], ray.ry, ray.ty, moved, pc.y);
-            pe[2] = krp_locald(n[2], ray.rz, ray.tz, moved, pc.z);
+            pe[0] = krp_locald(n[0], ray.rx, g.inv_dd[0], moved, pc.x);
+            pe[1] = krp_locald(n[1], ray.ry, g.inv_dd[1], moved, pc.y);
+            pe[2] = krp_locald(n[2], ray.rz, g.inv_dd[2], moved, pc.z);
             tl.steps += nsteps;
             krp_event_append(g, ctl, ev, id_, ray.c, pe, n, __float_as_uint(nk.w), S0_.x, cc.omega,
                              (float)qs, (float)us, (float)vs, tl);
