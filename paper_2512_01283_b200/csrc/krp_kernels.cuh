@@ -607,8 +607,16 @@ __global__ void __launch_bounds__(256, KRP_FLIGHT_GENERAL_MIN_BLOCKS) krp_k_flig
             krp_rayd_init(g, __float_as_uint(pc.w), p0, n, ray);
             cl = __ldg(g.cell + ray.c);
             nd[0] = n[0]; nd[1] = n[1]; nd[2] = n[2];
-            krp_basis<double>(nd, th, ph);
             inv_n = krp_rsqrt_near1(nd[0] * nd[0] + nd[1] * nd[1] + nd[2] * nd[2]);
+            {   // spherical basis of n (eq. 4-5, pole rule R10) with one division: |n| = 1 + O(1e-7) is divided out by series
+                const double s2 = nd[0] * nd[0] + nd[1] * nd[1];
+                double cp = 1.0, sp = 0.0, st = 0.0;
+                if (s2 >= 1e-24) { const double s = sqrt(s2), is = 1.0 / s; cp = nd[0] * is; sp = nd[1] * is; st = s * inv_n; }
+                else st = sqrt(s2) * inv_n;
+                const double ct = nd[2] * inv_n;
+                th[0] = ct * cp; th[1] = ct * sp; th[2] = -st;
+                ph[0] = -sp; ph[1] = cp; ph[2] = 0.0;
+            }
             D = tau0; i = 1.0;
             qs = S0.y; us = S0.z; vs = S0.w;      // lab reference
             Asum = 0.f; tau0f = (float)tau0; nsteps = 0;
