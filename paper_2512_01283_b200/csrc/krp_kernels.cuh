@@ -493,7 +493,7 @@ __device__ __forceinline__ double krp_event_solve_d(double R, double qq, double 
             const double hp = a1 - a2 * (sh - qq * (1.0 + chm1)) / (1.0 + gm1);
             const double dt = h / hp;
             t = fmin(fmax(t - dt, 0.0), tmax);
-            if (fabs(dt) <= 4e-16 * t) break;
+            if (fabs(dt) <= 1e-13 * t) break;      // quadratic convergence: the step after this one would be ~1e-26 t
         }
     }
     return fmin(fmax(t, 0.0), tmax);
