@@ -403,6 +403,20 @@ __device__ __forceinline__ double krp_rsqrt_near1(double vv)
     return 1.0 + e * (-0.5 + e * (0.375 - 0.3125 * e));
 }
 
+// spherical basis (eq. 4-5, pole rule R10) of a direction that is unit to within fp32 rounding, fp64, with one
+// division and one square root: |n| is divided out by the series of krp_rsqrt_near1
+__device__ __forceinline__ void krp_basis_unit_d(const double n[3], double th[3], double ph[3])
+{
+    const double s2 = n[0] * n[0] + n[1] * n[1];
+    const double inv_r = krp_rsqrt_near1(s2 + n[2] * n[2]);
+    const double s = sqrt(s2);
+    double cp = 1.0, sp = 0.0;
+    if (s2 >= 1e-24) { const double is = 1.0 / s; cp = n[0] * is; sp = n[1] * is; }
+    const double ct = n[2] * inv_r, st = s * inv_r;
+    th[0] = ct * cp; th[1] = ct * sp; th[2] = -st;
+    ph[0] = -sp; ph[1] = cp; ph[2] = 0.0;
+}
+
 // ------------------------------------------------------------------------------------------
 // T3/T4/T5, general mode (direction-dependent, dichroic opacity; 16-byte cells).  Everything that
 // decides in which cell the event falls -- segment lengths, alpha1(mu), the scalar depth D and the
@@ -608,15 +622,7 @@ __global__ void __launch_bounds__(256, KRP_FLIGHT_GENERAL_MIN_BLOCKS) krp_k_flig
             cl = __ldg(g.cell + ray.c);
             nd[0] = n[0]; nd[1] = n[1]; nd[2] = n[2];
             inv_n = krp_rsqrt_near1(nd[0] * nd[0] + nd[1] * nd[1] + nd[2] * nd[2]);
-            {   // spherical basis of n (eq. 4-5, pole rule R10) with one division: |n| = 1 + O(1e-7) is divided out by series
-                const double s2 = nd[0] * nd[0] + nd[1] * nd[1];
-                double cp = 1.0, sp = 0.0, st = 0.0;
-                if (s2 >= 1e-24) { const double s = sqrt(s2), is = 1.0 / s; cp = nd[0] * is; sp = nd[1] * is; st = s * inv_n; }
-                else st = sqrt(s2) * inv_n;
-                const double ct = nd[2] * inv_n;
-                th[0] = ct * cp; th[1] = ct * sp; th[2] = -st;
-                ph[0] = -sp; ph[1] = cp; ph[2] = 0.0;
-            }
+            krp_basis_unit_d(nd, th, ph);
             D = tau0; i = 1.0;
             qs = S0.y; us = S0.z; vs = S0.w;      // lab reference
             Asum = 0.f; tau0f = (float)tau0; nsteps = 0;
@@ -729,7 +735,7 @@ __global__ void __launch_bounds__(128, 8) krp_k_scatter(KrpModel g, KrpCtl* ctl,
             // A3: direction in the grain frame (eq. 3)
             krp_quat_rotate(qB, n, -1.0, ng);
             // A5: Stokes reference lab -> grain frame
-            krp_basis<double>(n, th, ph);
+            krp_basis_unit_d(n, th, ph);
             krp_eta2<double>(krp_dot(th, b), krp_dot(ph, b), c2, s2);
             krp_rot_qu(Q, U, c2, s2);
         }
@@ -775,7 +781,7 @@ __global__ void __launch_bounds__(128, 8) krp_k_scatter(KrpModel g, KrpCtl* ctl,
         }
         // scattering in the grain frame
         double thp[3], php[3];
-        krp_basis<double>(ng, thp, php);
+        krp_basis_unit_d(ng, thp, php);
         double st, ct;
         sincos(theta * (KRP_PI_D / 180.0), &st, &ct);
         double epar[3], nog[3], eout[3], shat[3];
@@ -790,7 +796,7 @@ __global__ void __launch_bounds__(128, 8) krp_k_scatter(KrpModel g, KrpCtl* ctl,
         for (int j = 0; j < 3; ++j) eout[j] = ct * epar[j] - st * ng[j];
         krp_cross(ng, epar, shat);
         double th2[3], ph2[3];
-        krp_basis<double>(nog, th2, ph2);
+        krp_basis_unit_d(nog, th2, ph2);
         {
             double ce = krp_dot(eout, th2), se = krp_dot(th2, shat);
             krp_rot_qu(Q, U, ce * ce - se * se, 2.0 * se * ce);                // reference theta^ of n'_GF
@@ -801,7 +807,7 @@ __global__ void __launch_bounds__(128, 8) krp_k_scatter(KrpModel g, KrpCtl* ctl,
         const float nf[3] = { (float)nl[0], (float)nl[1], (float)nl[2] };
         if (!g.scalar) {
             const double nd[3] = { nf[0], nf[1], nf[2] };
-            krp_basis<double>(nd, th, ph);
+            krp_basis_unit_d(nd, th, ph);
             krp_eta2<double>(krp_dot(th, b), krp_dot(ph, b), c2, s2);
             krp_rot_qu(Q, U, c2, -s2);
         }
