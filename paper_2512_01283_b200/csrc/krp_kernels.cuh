@@ -726,11 +726,19 @@ __global__ void __launch_bounds__(128, 8) krp_k_scatter(KrpModel g, KrpCtl* ctl,
         double th[3], ph[3], c2 = 1.0, s2 = 0.0;
         double Q = Se.y, U = Se.z, V = Se.w;
         if (!g.scalar) {
-            double rho = sqrt(b[0] * b[0] + b[1] * b[1]);
-            double thB = atan2(rho, b[2]), phB = rho > 0.0 ? atan2(b[1], b[0]) : 0.0;
-            double sh_t, ch_t, sh_p, ch_p;
-            sincos(0.5 * thB, &sh_t, &ch_t);
-            sincos(0.5 * phB, &sh_p, &ch_p);
+            // half angles of theta_B in [0, pi] and phi_B in (-pi, pi] from their cosines and sines (no atan2, no sincos):
+            // cos(a/2) = sqrt((1 + cos a)/2), sin(a/2) = sin a / (2 cos(a/2)) on the side where that does not cancel
+            const double rho2 = b[0] * b[0] + b[1] * b[1], rho = sqrt(rho2);
+            const double inv_r = krp_rsqrt_near1(rho2 + b[2] * b[2]);       // B^ is unit to fp32 rounding
+            const double cth = b[2] * inv_r, sth = rho * inv_r;
+            double ch_t, sh_t, ch_p = 1.0, sh_p = 0.0;
+            if (cth >= 0.0) { ch_t = sqrt(0.5 * (1.0 + cth)); sh_t = sth / (2.0 * ch_t); }
+            else            { sh_t = sqrt(0.5 * (1.0 - cth)); ch_t = sth / (2.0 * sh_t); }
+            if (rho > 0.0) {
+                const double ir = 1.0 / rho, cph = b[0] * ir, sph = b[1] * ir;
+                if (cph >= 0.0) { ch_p = sqrt(0.5 * (1.0 + cph)); sh_p = sph / (2.0 * ch_p); }
+                else            { sh_p = copysign(sqrt(0.5 * (1.0 - cph)), sph); ch_p = sph / (2.0 * sh_p); }
+            }
             qB[0] = ch_p * ch_t; qB[1] = -sh_p * sh_t; qB[2] = ch_p * sh_t; qB[3] = sh_p * ch_t;
             // A3: direction in the grain frame (eq. 3)
             krp_quat_rotate(qB, n, -1.0, ng);
