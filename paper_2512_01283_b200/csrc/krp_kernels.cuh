@@ -69,7 +69,7 @@ __device__ __forceinline__ void krp_item_load(const KrpModel& g, const KrpRecord
         const double ct = 1.0 - 2.0 * krp_u01(w.x);
         const double st = sqrt(1.0 - ct * ct);
         double sp, cp;
-        sincos(2.0 * KRP_PI_D * krp_u01(w.y), &sp, &cp);
+        sincospi(2.0 * krp_u01(w.y), &sp, &cp);
         nk = make_float4((float)(st * cp), (float)(st * sp), (float)ct, __uint_as_float(0u));   // R12
         pc = make_float4(g.src_p[0], g.src_p[1], g.src_p[2], __uint_as_float(g.src_cell));
         S0 = make_float4(1.f, 0.f, 0.f, 0.f);
@@ -99,7 +99,7 @@ __global__ void __launch_bounds__(256) krp_k_emit(KrpModel g, KrpCtl* ctl, KrpRe
         double ct = 1.0 - 2.0 * krp_u01(w.x);
         double st = sqrt(1.0 - ct * ct);
         double sp, cp;
-        sincos(2.0 * KRP_PI_D * krp_u01(w.y), &sp, &cp);
+        sincospi(2.0 * krp_u01(w.y), &sp, &cp);
         nn[0] = (float)(st * cp); nn[1] = (float)(st * sp); nn[2] = (float)ct;   // R12
     }
     uint32_t cell; float p[3];
@@ -767,9 +767,8 @@ __global__ void __launch_bounds__(128, 8) krp_k_scatter(KrpModel g, KrpCtl* ctl,
         krp_mueller_at<double>(g.mueller, g.n_ang, theta, F);
         const double p12 = F[1] / F[0];
         const double bound = 1.0 + fabs(p12) * sqrt(Q * Q + U * U);
-        double phi = 2.0 * KRP_PI_D * krp_u01(w.y);
         double sphi, cphi;
-        sincos(phi, &sphi, &cphi);
+        sincospi(2.0 * krp_u01(w.y), &sphi, &cphi);           // phi = 2 pi u: no range reduction needed
         bool ok;
         {
             double c2p = cphi * cphi - sphi * sphi, s2p = 2.0 * sphi * cphi;
@@ -780,8 +779,7 @@ __global__ void __launch_bounds__(128, 8) krp_k_scatter(KrpModel g, KrpCtl* ctl,
             uint4 x = krp_philox(seed, id, kb, blk);
             uint32_t cand[2] = { x.x, x.z }, acc[2] = { x.y, x.w };
             for (int h = 0; h < 2 && !ok && rounds < 64; ++h) {
-                phi = 2.0 * KRP_PI_D * krp_u01(cand[h]);
-                sincos(phi, &sphi, &cphi);
+                sincospi(2.0 * krp_u01(cand[h]), &sphi, &cphi);
                 double c2p = cphi * cphi - sphi * sphi, s2p = 2.0 * sphi * cphi;
                 ok = krp_u01(acc[h]) * bound < 1.0 + p12 * (Q * c2p + U * s2p);
                 ++rounds;
@@ -791,7 +789,7 @@ __global__ void __launch_bounds__(128, 8) krp_k_scatter(KrpModel g, KrpCtl* ctl,
         double thp[3], php[3];
         krp_basis_unit_d(ng, thp, php);
         double st, ct;
-        sincos(theta * (KRP_PI_D / 180.0), &st, &ct);
+        sincospi(theta * (1.0 / 180.0), &st, &ct);
         double epar[3], nog[3], eout[3], shat[3];
         for (int j = 0; j < 3; ++j) epar[j] = cphi * thp[j] + sphi * php[j];
         for (int j = 0; j < 3; ++j) nog[j] = ct * ng[j] + st * epar[j];
