@@ -1096,6 +1096,7 @@ __global__ void __launch_bounds__(256, SCALAR ? KRP_IMAGE_SCALAR_MIN_BLOCKS : KR
                 // march over the observer's own coefficient array {kr a1, kr a2, kr a3, 2 eta}
                 float i = S[0], qs = S[1], us = S[2], vs = S[3];
                 float4 cl = __ldg(obs_cell + r.c);
+#pragma unroll 2
                 do {
                     const float ds = krp_raya_step(r, rc);
                     const float4 cn = __ldg(obs_cell + r.c);    // next cell, in flight during the update below
