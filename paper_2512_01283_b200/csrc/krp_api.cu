@@ -275,6 +275,8 @@ extern "C" int krp_grid_create(krp_grid** out, int nx, int ny, int nz, const dou
     g->burst = m.scalar ? 1 : 32;
     if (getenv("KRP_NO_DIR_SORT")) g->dir_sort = 0;   // A/B switches for measurement
     if (getenv("KRP_NO_OBS_PRE")) g->obs_pre = 0;
+    if (m.scalar)
+        CK(cudaFuncSetAttribute(krp_k_flight_scalar, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(8 * sizeof(KrpWarpShared))));
     if (getenv("KRP_ORDER_POLICY")) g->order_policy = atoi(getenv("KRP_ORDER_POLICY"));
     g->order_events = g->order_policy != 0;
     m.n_inc = n_inc; m.n_ang = tables->n_ang;
@@ -545,7 +547,7 @@ extern "C" int krp_transport(krp_grid* g, uint64_t n_packets, uint64_t seed, voi
         { TimedLaunch tl(g, st, KRP_T_FLIGHT);
         const KrpEmitSrc es = w == 0 ? es0 : KrpEmitSrc{ nullptr, 0, 0 };
         if (g->m.scalar && g->burst == 1) krp_k_flight_scalar_static<<<grid_f, tb, 0, st>>>(g->m, g->d_ctl, g->q[in], in, g->ev, es);
-        else if (g->m.scalar) krp_k_flight_scalar<<<grid_f, tb, 0, st>>>(g->m, g->d_ctl, g->q[in], in, g->ev, g->burst, es);
+        else if (g->m.scalar) krp_k_flight_scalar<<<grid_f, tb, (size_t)(tb / 32) * sizeof(KrpWarpShared), st>>>(g->m, g->d_ctl, g->q[in], in, g->ev, g->burst, es);
         else             krp_k_flight_general<<<grid_f, tb, 0, st>>>(g->m, g->d_ctl, g->q[in], in, g->ev, g->burst, es); }
         g->launches += 2;
         if (w + 1 < g->max_waves) {

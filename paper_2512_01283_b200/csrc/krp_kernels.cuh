@@ -246,77 +246,6 @@ __device__ __forceinline__ bool krp_take_work(unsigned int* counter, unsigned in
 
 enum { KRP_IDLE = 0, KRP_RUN = 1, KRP_HIT = 2, KRP_ESC = 3 };
 
-__global__ void __launch_bounds__(256, 4) krp_k_flight_scalar(KrpModel g, KrpCtl* ctl, KrpRecords q, int in, KrpRecords ev, int n_burst, KrpEmitSrc es)
-{
-    const unsigned int n_items = ctl->q_count[in];
-    KrpFlightTally tl = { 0, 0, 0, 0.0, 0.0, 0.0 };
-    int status = KRP_IDLE;
-    bool more = true;
-    unsigned int item = 0, wbase = 0, wleft = 0;
-    float n[3] = { 0.f, 0.f, 1.f }, p0[3] = { 0.f, 0.f, 0.f }, kr = 0.f, a1kr = 0.f;
-    uint32_t c0 = 0;
-    KrpRay ray = {};
-    double D = 0.0;
-    for (;;) {
-        // refill point: the lanes whose flight ended during the last burst close it together, then take new work
-        if (status == KRP_HIT || status == KRP_ESC) {
-            int h0[3], h1[3];
-            krp_pad_coords(g, c0, h0[0], h0[1], h0[2]);
-            krp_pad_coords(g, ray.c, h1[0], h1[1], h1[2]);
-            const int crossings = abs(h1[0] - h0[0]) + abs(h1[1] - h0[1]) + abs(h1[2] - h0[2]);
-            float4 pc_, nk_, S0; double tau_; unsigned long long id_;
-            krp_item_load(g, q, es, item, pc_, nk_, S0, tau_, id_);
-            if (status == KRP_HIT) {
-                const double moved = D / ((double)g.a1c * (double)kr);
-                // entry face of the event cell: the axis crossed last has its distance re-based to a full cell
-                const int axis = ray.c == c0 ? -1 : (ray.rx == ray.tx ? 0 : (ray.ry == ray.ty ? 1 : 2));
-                float pe[3];
-                krp_event_pos(g, n, p0, c0, ray.c, axis, moved, pe);
-                tl.steps += (unsigned long long)(crossings + 1);
-                krp_event_append(g, ctl, ev, id_, ray.c, pe, n, __float_as_uint(nk_.w), S0.x, g.omc, S0.y, S0.z, S0.w, tl);
-            } else {
-                tl.steps += (unsigned long long)crossings;
-                tl.w_esc += (double)S0.x;
-            }
-            status = KRP_IDLE;
-        }
-        if (krp_take_work(&ctl->work[0], n_items, status == KRP_IDLE, wbase, wleft, more, item)) {
-            {
-                float4 pc, nk, S0_; unsigned long long id_;
-                krp_item_load(g, q, es, item, pc, nk, S0_, D, id_);
-                n[0] = nk.x; n[1] = nk.y; n[2] = nk.z;
-                p0[0] = pc.x; p0[1] = pc.y; p0[2] = pc.z;
-                c0 = __float_as_uint(pc.w);
-                krp_ray_init(g, c0, p0, n, ray);
-                kr = __ldg(g.kr + ray.c);
-                a1kr = g.a1c * kr;
-                status = KRP_RUN;
-            }
-        }
-        if (!__any_sync(0xffffffffu, status == KRP_RUN)) break;
-#pragma unroll 1
-        for (int burst = 0; burst < n_burst; ++burst) {
-            if (status == KRP_RUN) {
-                const float ds = krp_ray_ds(ray);
-                const float dt1 = a1kr * ds;
-                if ((double)dt1 >= D) {
-                    status = KRP_HIT;                // event inside this cell, located at the refill point
-                } else {
-                    D -= (double)dt1;
-                    krp_ray_step(ray, ds);
-                    kr = __ldg(g.kr + ray.c);
-                    a1kr = g.a1c * kr;
-                    if (kr < 0.f) status = KRP_ESC;  // halo: the packet left the grid
-                }
-            }
-        }
-    }
-    krp_tally_flush(tl, ctl);
-}
-
-// The same flight with a static assignment (one queue entry per thread and grid stride, the warp's 32 flights
-// start and are closed together): no refill logic at all.  Cheaper when flights are short (C2: a point source
-// inside a dense ring, most flights end within a few cells), selected with flight_burst = 1.
 // one re-based step in registers: returns the length of the segment in the current cell and the axis of the face
 // crossed (ties x before y before z), moves to the next cell
 __device__ __forceinline__ float krp_ray_advance(KrpRay& r, int& axis)
@@ -337,6 +266,166 @@ __device__ __forceinline__ float krp_ray_advance(KrpRay& r, int& axis)
     return ds;
 }
 
+// Persistent form with a refill point that never waits for memory (T7).  Per warp, in shared memory: a stage of the
+// next 64 queue entries (loaded coalesced, one wait per 64 flights) and a ring of finished event records (flushed 32 at
+// a time: one atomic and coalesced stores per 32 events).  At a refill point a lane whose flight has ended builds its
+// record from registers, drops it in the ring and starts the next staged entry; the only memory access on its way back
+// into the march is the first cell gather.  Everything is warp-local: no block barrier.
+#define KRP_STAGE 64
+struct KrpWarpShared {
+    float4 s_pc[KRP_STAGE], s_nk[KRP_STAGE], s_S[KRP_STAGE];      // staged queue entries
+    double s_tau[KRP_STAGE];
+    unsigned long long s_id[KRP_STAGE];
+    float4 r_pc[64], r_nk[64], r_S[64];                            // ring of event records
+    unsigned long long r_id[64];
+};
+
+__global__ void __launch_bounds__(256, 3) krp_k_flight_scalar(KrpModel g, KrpCtl* ctl, KrpRecords q, int in, KrpRecords ev, int n_burst, KrpEmitSrc es)
+{
+    extern __shared__ __align__(16) unsigned char s_raw[];
+    KrpWarpShared& sh = reinterpret_cast<KrpWarpShared*>(s_raw)[threadIdx.x >> 5];
+    const int lane = threadIdx.x & 31;
+    const unsigned int n_items = ctl->q_count[in];
+    KrpFlightTally tl = { 0, 0, 0, 0.0, 0.0, 0.0 };
+    int status = KRP_IDLE;
+    bool more = true;
+    unsigned int stage_n = 0, stage_pos = 0, ring_n = 0;           // warp-uniform
+    // the flight in progress
+    float n[3] = { 0.f, 0.f, 1.f }, p0[3] = { 0.f, 0.f, 0.f }, kr = 0.f;
+    float4 S0 = make_float4(0.f, 0.f, 0.f, 0.f);
+    unsigned long long id = 0;
+    uint32_t c0 = 0, k = 0;
+    int ax = -1;
+    KrpRay ray = {};
+    double D = 0.0;
+    for (;;) {
+        // ---- refill point -------------------------------------------------------------------------------------
+        bool rec = false;
+        float4 rpc, rnk, rS;
+        if (status == KRP_HIT || status == KRP_ESC) {
+            int h0[3], h1[3];
+            krp_pad_coords(g, c0, h0[0], h0[1], h0[2]);
+            krp_pad_coords(g, ray.c, h1[0], h1[1], h1[2]);
+            const int crossings = abs(h1[0] - h0[0]) + abs(h1[1] - h0[1]) + abs(h1[2] - h0[2]);
+            if (status == KRP_HIT) {
+                const double moved = D / ((double)g.a1c * (double)kr);
+                float pe[3];
+                krp_event_pos(g, n, p0, c0, ray.c, ax, moved, pe);
+                tl.steps += (unsigned long long)(crossings + 1);
+                const float Wn = g.omc * S0.x;
+                const uint32_t kn = k + 1u;
+                const bool term = (Wn < g.w_min) || ((int)kn >= g.max_scatter);
+                tl.w_abs += (double)S0.x - (double)Wn;
+                if (term) tl.w_cut += (double)Wn;            // (an overflowing record is accounted at the flush)
+                rpc = make_float4(pe[0], pe[1], pe[2], __uint_as_float(ray.c));
+                rnk = make_float4(n[0], n[1], n[2], __uint_as_float(kn | (term ? KRP_TERM_BIT : 0u)));
+                rS = make_float4(Wn, S0.y, S0.z, S0.w);
+                rec = true;
+            } else {
+                tl.steps += (unsigned long long)crossings;
+                tl.w_esc += (double)S0.x;
+            }
+            status = KRP_IDLE;
+        }
+        {   // records of this point go to the ring (it has room for 32: it is flushed as soon as it holds 32)
+            const unsigned m = __ballot_sync(0xffffffffu, rec);
+            if (rec) {
+                const unsigned slot = ring_n + __popc(m & ((1u << lane) - 1u));
+                sh.r_pc[slot] = rpc; sh.r_nk[slot] = rnk; sh.r_S[slot] = rS; sh.r_id[slot] = id;
+            }
+            ring_n += __popc(m);
+            __syncwarp();
+        }
+        // ---- take new work from the stage; re-stage when it runs dry ---------------------------------------------
+#pragma unroll 1
+        for (int pass = 0; pass < 2; ++pass) {
+            const unsigned want = __ballot_sync(0xffffffffu, status == KRP_IDLE);
+            if (want == 0u) break;
+            if (stage_pos == stage_n && more) {
+                unsigned int base = 0;
+                if (lane == 0) base = atomicAdd(&ctl->work[0], (unsigned int)KRP_STAGE);
+                base = __shfl_sync(0xffffffffu, base, 0);
+                if (base >= n_items) { more = false; }
+                else {
+                    stage_n = min((unsigned int)KRP_STAGE, n_items - base); stage_pos = 0;
+                    for (unsigned int j = lane; j < stage_n; j += 32) {
+                        float4 pc_, nk_, S_; double tau_; unsigned long long id_;
+                        krp_item_load(g, q, es, base + j, pc_, nk_, S_, tau_, id_);
+                        sh.s_pc[j] = pc_; sh.s_nk[j] = nk_; sh.s_S[j] = S_; sh.s_tau[j] = tau_; sh.s_id[j] = id_;
+                    }
+                    __syncwarp();
+                }
+            }
+            const unsigned avail = stage_n - stage_pos;
+            if (avail == 0u) break;
+            const unsigned rank = __popc(want & ((1u << lane) - 1u));
+            if (status == KRP_IDLE && rank < avail) {
+                const unsigned j = stage_pos + rank;
+                const float4 pc_ = sh.s_pc[j], nk_ = sh.s_nk[j];
+                S0 = sh.s_S[j]; D = sh.s_tau[j]; id = sh.s_id[j];
+                n[0] = nk_.x; n[1] = nk_.y; n[2] = nk_.z; k = __float_as_uint(nk_.w);
+                p0[0] = pc_.x; p0[1] = pc_.y; p0[2] = pc_.z; c0 = __float_as_uint(pc_.w);
+                krp_ray_init(g, c0, p0, n, ray);
+                ax = -1;
+                kr = __ldg(g.kr + ray.c);
+                status = KRP_RUN;
+            }
+            stage_pos += min((unsigned)__popc(want), avail);
+            __syncwarp();
+        }
+        const bool any_run = __any_sync(0xffffffffu, status == KRP_RUN);
+        // ---- flush 32 records (or, at the end, what is left): one atomic, coalesced stores ---------------------------
+        while (ring_n >= 32u || (!any_run && ring_n > 0u)) {
+            const unsigned int cnt = min(ring_n, 32u);
+            unsigned long long base = 0;
+            if (lane == 0) base = atomicAdd(&ctl->n_events, (unsigned long long)cnt);
+            base = __shfl_sync(0xffffffffu, base, 0);
+            if ((unsigned)lane < cnt) {
+                const unsigned long long slot = base + lane;
+                const float4 a = sh.r_pc[lane], b = sh.r_nk[lane], c = sh.r_S[lane];
+                if (slot < ctl->ev_cap) {
+                    ev.pc[slot] = a; ev.nk[slot] = b; ev.S[slot] = c; ev.id[slot] = sh.r_id[lane];
+                    ++tl.n_ev;
+                } else {
+                    ++tl.n_over;
+                    if (!(__float_as_uint(b.w) & KRP_TERM_BIT)) tl.w_cut += (double)c.x;     // a lost packet counts as cut
+                }
+            }
+            __syncwarp();
+            {   // move the rest to the front
+                const bool mv = ring_n > 32u && (unsigned)lane < ring_n - 32u;
+                float4 a = make_float4(0.f, 0.f, 0.f, 0.f), b = a, c = a;
+                unsigned long long d = 0;
+                if (mv) { a = sh.r_pc[32 + lane]; b = sh.r_nk[32 + lane]; c = sh.r_S[32 + lane]; d = sh.r_id[32 + lane]; }
+                __syncwarp();
+                if (mv) { sh.r_pc[lane] = a; sh.r_nk[lane] = b; sh.r_S[lane] = c; sh.r_id[lane] = d; }
+            }
+            ring_n -= cnt;
+            __syncwarp();
+        }
+        if (!any_run) break;
+        // ---- burst ---------------------------------------------------------------------------------------------------
+#pragma unroll 1
+        for (int burst = 0; burst < n_burst; ++burst) {
+            if (status == KRP_RUN) {
+                const float dt1 = g.a1c * kr * krp_ray_ds(ray);
+                if ((double)dt1 >= D) {
+                    status = KRP_HIT;                // event inside this cell, located at the refill point
+                } else {
+                    D -= (double)dt1;
+                    krp_ray_advance(ray, ax);
+                    kr = __ldg(g.kr + ray.c);
+                    if (kr < 0.f) status = KRP_ESC;  // halo: the packet left the grid
+                }
+            }
+        }
+    }
+    krp_tally_flush(tl, ctl);
+}
+
+// The same flight with a static assignment (one queue entry per thread and grid stride, the warp's 32 flights
+// start and are closed together): no refill logic at all.  Cheaper when flights are short (C2: a point source
+// inside a dense ring, most flights end within a few cells), selected with flight_burst = 1.
 __global__ void __launch_bounds__(256, 4) krp_k_flight_scalar_static(KrpModel g, KrpCtl* ctl, KrpRecords q, int in, KrpRecords ev, KrpEmitSrc es)
 {
     const unsigned int n_items = ctl->q_count[in];
