@@ -662,7 +662,8 @@ __global__ void __launch_bounds__(256, KRP_FLIGHT_GENERAL_MIN_BLOCKS) krp_k_flig
     float Asum = 0.f, tau0f = 0.f;
     unsigned int nsteps = 0;
     KrpRayD ray = {};
-    float4 cl = make_float4(0.f, 0.f, 0.f, 1.f);
+    float4 cl = make_float4(0.f, 0.f, 0.f, 1.f), cl_f = cl;
+    bool fresh = false;
     for (;;) {
         // refill point: the lanes whose flight ended during the last burst close it together
         if (status == KRP_HIT) {
@@ -708,7 +709,10 @@ __global__ void __launch_bounds__(256, KRP_FLIGHT_GENERAL_MIN_BLOCKS) krp_k_flig
             krp_item_load(g, q, es, item, pc, nk, S0, tau0, id_);
             const float n[3] = { nk.x, nk.y, nk.z }, p0[3] = { pc.x, pc.y, pc.z };
             krp_rayd_init(g, __float_as_uint(pc.w), p0, n, ray);
-            cl = __ldg(g.cell + ray.c);
+            // the first cell of the new flight goes to registers of its own and is taken over one step later: the warp's other
+            // flights march on while it is in flight (a register is scoreboarded per warp, whoever's lanes wait for it)
+            asm volatile("ld.global.nc.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(cl_f.x), "=f"(cl_f.y), "=f"(cl_f.z), "=f"(cl_f.w) : "l"(g.cell + ray.c));
+            fresh = true;
             nd[0] = n[0]; nd[1] = n[1]; nd[2] = n[2];
             inv_n = krp_rsqrt_near1(nd[0] * nd[0] + nd[1] * nd[1] + nd[2] * nd[2]);
             krp_basis_unit_d(nd, th, ph);
@@ -721,11 +725,16 @@ __global__ void __launch_bounds__(256, KRP_FLIGHT_GENERAL_MIN_BLOCKS) krp_k_flig
 #pragma unroll 1
         for (int burst = 0; burst < n_burst; ++burst) {
             if (status != KRP_RUN) continue;
+            if (fresh) {
+                if (burst == 0 && n_burst > 1) continue;
+                cl = cl_f; fresh = false;
+            }
             const double ds = krp_rayd_ds(ray);
             ++nsteps;
             // the next cell is requested now, so that its latency overlaps the fp64 update of this one
             const uint32_t c_next = ray.c + (uint32_t)((ray.rx <= ray.ry) & (ray.rx <= ray.rz) ? ray.sx : (ray.ry <= ray.rz ? ray.sy : ray.sz));
-            const float4 cn = __ldg(g.cell + c_next);
+            float4 cn;      // a load the compiler may neither duplicate nor move: it has to be in flight during the update below
+            asm volatile("ld.global.nc.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(cn.x), "=f"(cn.y), "=f"(cn.z), "=f"(cn.w) : "l"(g.cell + c_next));
             if (cl.x > 0.f) {
                 KrpCellCoef cc;
                 krp_cell_coef(g, cl, nd, inv_n, xs, ds, cc);
