@@ -522,11 +522,11 @@ struct KrpCellCoef {
     float omega;                    // albedo(mu)
 };
 
-__device__ __forceinline__ void krp_cell_coef(const KrpModel& g, const float4 cl, const double nd[3], double inv_n, double xs,
+__device__ __forceinline__ void krp_cell_coef(const KrpModel& g, const float4 cl, const double nd[3], double xs,
                                               double ds, KrpCellCoef& c)
 {
     const double bx = cl.y, by = cl.z, bz = cl.w;
-    double mu = fabs(nd[0] * bx + nd[1] * by + nd[2] * bz) * inv_n * krp_rsqrt_near1(bx * bx + by * by + bz * bz);
+    double mu = fabs(nd[0] * bx + nd[1] * by + nd[2] * bz) * krp_rsqrt_near1(bx * bx + by * by + bz * bz);
     mu = fmin(mu, 1.0);
     const double x = mu * xs;
     const int j = min((int)x, g.n_inc - 2);
@@ -658,7 +658,7 @@ __global__ void __launch_bounds__(256, KRP_FLIGHT_GENERAL_MIN_BLOCKS) krp_k_flig
     unsigned int item = 0, wbase = 0, wleft = 0;
     // state of the flight in progress (all fp64: it decides where the event falls)
     double nd[3] = { 0.0, 0.0, 1.0 }, th[3] = { 0.0, 0.0, 0.0 }, ph[3] = { 0.0, 0.0, 0.0 };
-    double inv_n = 1.0, D = 0.0, i = 1.0, qs = 0.0, us = 0.0, vs = 0.0;
+    double D = 0.0, i = 1.0, qs = 0.0, us = 0.0, vs = 0.0;
     float Asum = 0.f, tau0f = 0.f;
     unsigned int nsteps = 0;
     KrpRayD ray = {};
@@ -670,7 +670,7 @@ __global__ void __launch_bounds__(256, KRP_FLIGHT_GENERAL_MIN_BLOCKS) krp_k_flig
             // the state is that of the entry into the event cell: solve for t, evolve to t, normalise to I = 1 (R7)
             const double ds = krp_rayd_ds(ray);
             KrpCellCoef cc;
-            krp_cell_coef(g, cl, nd, inv_n, xs, ds, cc);
+            krp_cell_coef(g, cl, nd, xs, ds, cc);
             const double R = D + log(i);
             double moved;
             if (cc.a2 == 0.0 && cc.a3 == 0.0) {
@@ -714,8 +714,11 @@ __global__ void __launch_bounds__(256, KRP_FLIGHT_GENERAL_MIN_BLOCKS) krp_k_flig
             asm volatile("ld.global.nc.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(cl_f.x), "=f"(cl_f.y), "=f"(cl_f.z), "=f"(cl_f.w) : "l"(g.cell + ray.c));
             fresh = true;
             nd[0] = n[0]; nd[1] = n[1]; nd[2] = n[2];
-            inv_n = krp_rsqrt_near1(nd[0] * nd[0] + nd[1] * nd[1] + nd[2] * nd[2]);
             krp_basis_unit_d(nd, th, ph);
+            {   // n^ = n/|n| once per flight (|n|^2 = 1 + O(1e-7)): mu = |n^ . B| / |B| in every cell
+                const double inv_n = krp_rsqrt_near1(nd[0] * nd[0] + nd[1] * nd[1] + nd[2] * nd[2]);
+                nd[0] *= inv_n; nd[1] *= inv_n; nd[2] *= inv_n;
+            }
             D = tau0; i = 1.0;
             qs = S0.y; us = S0.z; vs = S0.w;      // lab reference
             Asum = 0.f; tau0f = (float)tau0; nsteps = 0;
@@ -737,7 +740,7 @@ __global__ void __launch_bounds__(256, KRP_FLIGHT_GENERAL_MIN_BLOCKS) krp_k_flig
             asm volatile("ld.global.nc.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(cn.x), "=f"(cn.y), "=f"(cn.z), "=f"(cn.w) : "l"(g.cell + c_next));
             if (cl.x > 0.f) {
                 KrpCellCoef cc;
-                krp_cell_coef(g, cl, nd, inv_n, xs, ds, cc);
+                krp_cell_coef(g, cl, nd, xs, ds, cc);
                 Asum += (float)cc.dt1;
                 const bool near_end = Asum * guard >= tau0f;
                 if (cc.a2 == 0.0 && cc.a3 == 0.0) {
