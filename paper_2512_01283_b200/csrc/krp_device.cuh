@@ -38,6 +38,8 @@ struct KrpModel {
     const double4* opA_d;  // the same in fp64 (general-mode flight)
     const double4* opB_d;
     int n_inc;
+    double xs;             // n_inc - 1 as fp64 (x = mu*xs)
+    float guard;           // 1 + rho + 1e-3: margin of the fp32 depth sum that arms the fp64 event test of the general flight
     const float4* mueller; // [n_ang] {S11,S12,S33,S34}
     int n_ang;
     const double* cdf;     // [n_ang] Theta CDF of S11 sin(Theta)
@@ -324,7 +326,7 @@ __device__ __forceinline__ void krp_eta2(T a, T b, T& c2, T& s2)
 __device__ __forceinline__ void krp_eta2_d(double a, double b, double& c2, double& s2)
 {
     const double aa = a * a, bb = b * b, ss = aa + bb;
-    if (ss < 1e-24) { c2 = 1.0; s2 = 0.0; return; }
+    if (__double2hiint(ss) < 0x3af357c2) { c2 = 1.0; s2 = 0.0; return; }     // ss < 1e-24, on the high word (ss >= 0)
     double r = (double)__frcp_rn((float)ss);
     r = r * (2.0 - ss * r);
     r = r * (2.0 - ss * r);

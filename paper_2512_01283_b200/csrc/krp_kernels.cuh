@@ -526,9 +526,8 @@ __device__ __forceinline__ void krp_cell_coef(const KrpModel& g, const float4 cl
                                               double ds, KrpCellCoef& c)
 {
     const double bx = cl.y, by = cl.z, bz = cl.w;
-    double mu = fabs(nd[0] * bx + nd[1] * by + nd[2] * bz) * krp_rsqrt_near1(bx * bx + by * by + bz * bz);
-    mu = fmin(mu, 1.0);
-    const double x = mu * xs;
+    const double mu = fabs(nd[0] * bx + nd[1] * by + nd[2] * bz) * krp_rsqrt_near1(bx * bx + by * by + bz * bz);
+    const double x = mu * xs;        // mu <= 1 up to rounding: the index is clamped, the last segment extends by that much
     const int j = min((int)x, g.n_inc - 2);
     // the table as fp64 intercept + slope per segment (same piecewise-linear function, R13)
     const double4 ta = g.opA_d[j], tb = g.opB_d[j];
@@ -541,33 +540,41 @@ __device__ __forceinline__ void krp_cell_coef(const KrpModel& g, const float4 cl
 }
 
 // sinh(x), cosh(x)-1 and sin(y), cos(y)-1 in fp64 for |x|, |y| < 0.35: Taylor series, 4 terms below 0.02 (remainder
-// < 1e-19 relative), 8 terms (to x^15 / x^16) otherwise
+// < 1e-19 relative), 8 terms (to x^15 / x^16) otherwise.  The coefficients sit in constant memory: a DFMA takes one
+// operand straight from a constant bank, whereas a 64-bit literal costs two moves to build every time it is used
+// (a third of the instructions of the flight loop before); the range tests look at the high word only.
+__constant__ double KRP_SER[14] = {
+    1.0 / 6, 1.0 / 120, 1.0 / 5040, 1.0 / 362880, 1.0 / 39916800, 1.0 / 6227020800.0, 1.0 / 1307674368000.0,       // odd: x^3 .. x^15
+    1.0 / 24, 1.0 / 720, 1.0 / 40320, 1.0 / 3628800, 1.0 / 479001600, 1.0 / 87178291200.0, 1.0 / 20922789888000.0  // even: x^4 .. x^16
+};
+__device__ __forceinline__ bool krp_abs_below(double x, int hi) { return (__double2hiint(x) & 0x7fffffff) < hi; }
+#define KRP_HI_0P35 0x3fd66666      // high word of 0.35
+#define KRP_HI_4EM4 0x3f3a36e2      // high word of 4e-4
+
 __device__ __forceinline__ void krp_sinh_coshm1_d(double x, double& sh, double& chm1)
 {
     const double z = x * x;
-    if (z < 4e-4) {
-        sh = x * (1.0 + z * (1.0 / 6 + z * (1.0 / 120 + z * (1.0 / 5040))));
-        chm1 = z * (0.5 + z * (1.0 / 24 + z * (1.0 / 720 + z * (1.0 / 40320))));
+    const double* c = KRP_SER;
+    if (__double2hiint(z) < KRP_HI_4EM4) {
+        sh = x * (1.0 + z * (c[0] + z * (c[1] + z * c[2])));
+        chm1 = z * (0.5 + z * (c[7] + z * (c[8] + z * c[9])));
     } else {
         asm volatile("");      // keeps the long series a real branch (ptxas otherwise evaluates both and selects)
-        sh = x * (1.0 + z * (1.0 / 6 + z * (1.0 / 120 + z * (1.0 / 5040 + z * (1.0 / 362880 + z * (1.0 / 39916800 +
-             z * (1.0 / 6227020800.0 + z * (1.0 / 1307674368000.0))))))));
-        chm1 = z * (0.5 + z * (1.0 / 24 + z * (1.0 / 720 + z * (1.0 / 40320 + z * (1.0 / 3628800 + z * (1.0 / 479001600 +
-               z * (1.0 / 87178291200.0 + z * (1.0 / 20922789888000.0))))))));
+        sh = x * (1.0 + z * (c[0] + z * (c[1] + z * (c[2] + z * (c[3] + z * (c[4] + z * (c[5] + z * c[6])))))));
+        chm1 = z * (0.5 + z * (c[7] + z * (c[8] + z * (c[9] + z * (c[10] + z * (c[11] + z * (c[12] + z * c[13])))))));
     }
 }
 __device__ __forceinline__ void krp_sin_cosm1_d(double y, double& sy, double& cym1)
 {
     const double z = y * y;
-    if (z < 4e-4) {
-        sy = y * (1.0 - z * (1.0 / 6 - z * (1.0 / 120 - z * (1.0 / 5040))));
-        cym1 = -z * (0.5 - z * (1.0 / 24 - z * (1.0 / 720 - z * (1.0 / 40320))));
+    const double* c = KRP_SER;
+    if (__double2hiint(z) < KRP_HI_4EM4) {
+        sy = y * (1.0 - z * (c[0] - z * (c[1] - z * c[2])));
+        cym1 = -z * (0.5 - z * (c[7] - z * (c[8] - z * c[9])));
     } else {
         asm volatile("");
-        sy = y * (1.0 - z * (1.0 / 6 - z * (1.0 / 120 - z * (1.0 / 5040 - z * (1.0 / 362880 - z * (1.0 / 39916800 -
-             z * (1.0 / 6227020800.0 - z * (1.0 / 1307674368000.0))))))));
-        cym1 = -z * (0.5 - z * (1.0 / 24 - z * (1.0 / 720 - z * (1.0 / 40320 - z * (1.0 / 3628800 - z * (1.0 / 479001600 -
-               z * (1.0 / 87178291200.0 - z * (1.0 / 20922789888000.0))))))));
+        sy = y * (1.0 - z * (c[0] - z * (c[1] - z * (c[2] - z * (c[3] - z * (c[4] - z * (c[5] - z * c[6])))))));
+        cym1 = -z * (0.5 - z * (c[7] - z * (c[8] - z * (c[9] - z * (c[10] - z * (c[11] - z * (c[12] - z * c[13])))))));
     }
 }
 
@@ -610,10 +617,10 @@ __device__ __forceinline__ void krp_appA_d(double i, double qg, double ug, doubl
 {
     const double x = c.a2 * c.dtau, y = c.a3 * c.dtau;
     double sy, cym1;
-    if (fabs(y) < 0.35) krp_sin_cosm1_d(y, sy, cym1);
+    if (krp_abs_below(y, KRP_HI_0P35)) krp_sin_cosm1_d(y, sy, cym1);
     else { double cy; sincos(y, &sy, &cy); cym1 = cy - 1.0; }
     const double un = ug + (ug * cym1 - v * sy), vn = v + (ug * sy + v * cym1);
-    if (fabs(x) < 0.35) {
+    if (krp_abs_below(x, KRP_HI_0P35)) {
         double sh, chm1;
         krp_sinh_coshm1_d(x, sh, chm1);
         i_n = i + (i * chm1 - qg * sh);
@@ -651,8 +658,8 @@ __global__ void __launch_bounds__(256, KRP_FLIGHT_GENERAL_MIN_BLOCKS) krp_k_flig
 {
     const unsigned int n_items = ctl->q_count[in];
     KrpFlightTally tl = { 0, 0, 0, 0.0, 0.0, 0.0 };
-    const double xs = (double)(g.n_inc - 1);
-    const float guard = 1.f + g.rho + 1e-3f;
+    const double xs = g.xs;
+    const float guard = g.guard;
     int status = KRP_IDLE;
     bool more = true;
     unsigned int item = 0, wbase = 0, wleft = 0;
