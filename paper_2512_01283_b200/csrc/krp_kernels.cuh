@@ -739,10 +739,14 @@ __global__ void __launch_bounds__(256, KRP_FLIGHT_GENERAL_MIN_BLOCKS) krp_k_flig
                 if (burst == 0 && n_burst > 1) continue;
                 cl = cl_f; fresh = false;
             }
-            const double ds = krp_rayd_ds(ray);
+            // face crossed next (ties x before y before z), decided once per step: segment length, next cell and the
+            // re-based distances all follow from the two predicates
+            const bool ax = (ray.rx <= ray.ry) & (ray.rx <= ray.rz);
+            const bool ay = !ax & (ray.ry <= ray.rz);
+            const double ds = ax ? ray.rx : (ay ? ray.ry : ray.rz);
             ++nsteps;
             // the next cell is requested now, so that its latency overlaps the fp64 update of this one
-            const uint32_t c_next = ray.c + (uint32_t)((ray.rx <= ray.ry) & (ray.rx <= ray.rz) ? ray.sx : (ray.ry <= ray.rz ? ray.sy : ray.sz));
+            const uint32_t c_next = ray.c + (uint32_t)(ax ? ray.sx : (ay ? ray.sy : ray.sz));
             float4 cn;      // a load the compiler may neither duplicate nor move: it has to be in flight during the update below
             asm volatile("ld.global.nc.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(cn.x), "=f"(cn.y), "=f"(cn.z), "=f"(cn.w) : "l"(g.cell + c_next));
             if (cl.x > 0.f) {
@@ -773,7 +777,10 @@ __global__ void __launch_bounds__(256, KRP_FLIGHT_GENERAL_MIN_BLOCKS) krp_k_flig
                     i = i_new; D = Dn;
                 }
             }
-            krp_rayd_step(ray, ds);
+            ray.rx = ax ? ray.tx : ray.rx - ds;
+            ray.ry = ay ? ray.ty : ray.ry - ds;
+            ray.rz = (ax | ay) ? ray.rz - ds : ray.tz;
+            ray.c = c_next;
             cl = cn;
             if (cl.x < 0.f) status = KRP_ESC;        // halo: the packet left the grid
         }
