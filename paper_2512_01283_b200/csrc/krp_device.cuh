@@ -327,7 +327,9 @@ __device__ __forceinline__ void krp_eta2_d(double a, double b, double& c2, doubl
 {
     const double aa = a * a, bb = b * b, ss = aa + bb;
     if (__double2hiint(ss) < 0x3af357c2) { c2 = 1.0; s2 = 0.0; return; }     // ss < 1e-24, on the high word (ss >= 0)
-    double r = (double)__frcp_rn((float)ss);
+    float rf;       // 1/ss: the hardware approximation (2^-23) and two Newton steps (1e-14, 1e-28); ss is in [1e-24, 1]
+    asm("rcp.approx.ftz.f32 %0, %1;" : "=f"(rf) : "f"((float)ss));
+    double r = (double)rf;
     r = r * (2.0 - ss * r);
     r = r * (2.0 - ss * r);
     c2 = (aa - bb) * r;

@@ -687,7 +687,7 @@ __global__ void __launch_bounds__(256, KRP_FLIGHT_GENERAL_MIN_BLOCKS) krp_k_flig
             } else {
                 const double bx = cl.y, by = cl.z, bz = cl.w;
                 double c2, s2;
-                krp_eta2_d(th[0] * bx + th[1] * by + th[2] * bz, ph[0] * bx + ph[1] * by + ph[2] * bz, c2, s2);
+                krp_eta2_d(th[0] * bx + th[1] * by + th[2] * bz, ph[0] * bx + ph[1] * by, c2, s2);      // phi^_z = 0
                 const double qg_e = c2 * qs + s2 * us, ug_e = -s2 * qs + c2 * us;
                 const double t = krp_event_solve_d(R, qg_e / i, cc.a1, cc.a2, cc.dtau);
                 double qt, ut, vt;
@@ -760,7 +760,7 @@ __global__ void __launch_bounds__(256, KRP_FLIGHT_GENERAL_MIN_BLOCKS) krp_k_flig
                 } else {
                     const double bx = cl.y, by = cl.z, bz = cl.w;
                     double c2, s2;
-                    krp_eta2_d(th[0] * bx + th[1] * by + th[2] * bz, ph[0] * bx + ph[1] * by + ph[2] * bz, c2, s2);
+                    krp_eta2_d(th[0] * bx + th[1] * by + th[2] * bz, ph[0] * bx + ph[1] * by, c2, s2);      // phi^_z = 0
                     const double qg_e = c2 * qs + s2 * us, ug_e = -s2 * qs + c2 * us;          // eq. 7
                     double i_new, qg, ug, vg, depth;
                     krp_appA_d(i, qg_e, ug_e, vs, cc, i_new, qg, ug, vg, depth);
