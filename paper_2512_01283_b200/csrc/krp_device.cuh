@@ -42,6 +42,7 @@ struct KrpModel {
     float guard;           // 1 + rho + 1e-3: margin of the fp32 depth sum that arms the fp64 event test of the general flight
     const float4* mueller; // [n_ang] {S11,S12,S33,S34}
     int n_ang;
+    double inv_nang1;      // 1/(n_ang-1)
     const double* cdf;     // [n_ang] Theta CDF of S11 sin(Theta)
     float a1c, omc;        // SCALAR mode constants
     float rho;             // max |alpha2|/alpha1 over the table

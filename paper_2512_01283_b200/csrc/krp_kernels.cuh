@@ -863,23 +863,30 @@ __global__ void __launch_bounds__(128, 8) krp_k_scatter(KrpModel g, KrpCtl* ctl,
             krp_rot_qu(Q, U, c2, s2);
         }
         {
-            double r = 1.0 / sqrt(krp_dot(ng, ng));
+            double r = krp_rsqrt_near1(krp_dot(ng, ng));       // a rotation of a direction that is unit to fp32 rounding
             ng[0] *= r; ng[1] *= r; ng[2] *= r;
         }
         // draws
         uint4 w = krp_philox(seed, id, kb, 0u);
         const double tau_next = -log(krp_u01(w.w));
-        double theta;   // degrees, from the piecewise-linear CDF (R13)
+        double theta;   // Theta from the piecewise-linear CDF (R13), in units of the table spacing 180 deg/(n_ang-1)
         {
             double u = krp_u01(w.x);
             int lo = 0, hi = g.n_ang - 1;
             while (hi - lo > 1) { int mid = (lo + hi) >> 1; if (g.cdf[mid] <= u) lo = mid; else hi = mid; }
             double wd = g.cdf[lo + 1] - g.cdf[lo];
             double f = wd > 0.0 ? (u - g.cdf[lo]) / wd : 0.5;
-            theta = ((double)lo + f) * 180.0 / (double)(g.n_ang - 1);
+            theta = (double)lo + f;
         }
+        // Theta in units of the table spacing: the Mueller row is linear in it (R13), Theta/180 deg = theta/(n_ang-1)
         double F[4];
-        krp_mueller_at<double>(g.mueller, g.n_ang, theta, F);
+        {
+            const int j = max(0, min((int)theta, g.n_ang - 2));
+            const double w1 = theta - (double)j, w0 = 1.0 - w1;
+            const float4 a = g.mueller[j], b2 = g.mueller[j + 1];
+            F[0] = w0 * (double)a.x + w1 * (double)b2.x; F[1] = w0 * (double)a.y + w1 * (double)b2.y;
+            F[2] = w0 * (double)a.z + w1 * (double)b2.z; F[3] = w0 * (double)a.w + w1 * (double)b2.w;
+        }
         const double p12 = F[1] / F[0];
         const double bound = 1.0 + fabs(p12) * sqrt(Q * Q + U * U);
         double sphi, cphi;
@@ -904,7 +911,7 @@ __global__ void __launch_bounds__(128, 8) krp_k_scatter(KrpModel g, KrpCtl* ctl,
         double thp[3], php[3];
         krp_basis_unit_d(ng, thp, php);
         double st, ct;
-        sincospi(theta * (1.0 / 180.0), &st, &ct);
+        sincospi(theta * g.inv_nang1, &st, &ct);
         double epar[3], nog[3], eout[3], shat[3];
         for (int j = 0; j < 3; ++j) epar[j] = cphi * thp[j] + sphi * php[j];
         for (int j = 0; j < 3; ++j) nog[j] = ct * ng[j] + st * epar[j];
@@ -912,7 +919,8 @@ __global__ void __launch_bounds__(128, 8) krp_k_scatter(KrpModel g, KrpCtl* ctl,
         {
             double I2 = F[0] + F[1] * Q, Q2 = F[1] + F[0] * Q;                  // F(Theta) (1,Q,U,V)
             double U2 = F[2] * U + F[3] * V, V2 = -F[3] * U + F[2] * V;
-            Q = Q2 / I2; U = U2 / I2; V = V2 / I2;
+            const double inv = 1.0 / I2;
+            Q = Q2 * inv; U = U2 * inv; V = V2 * inv;
         }
         for (int j = 0; j < 3; ++j) eout[j] = ct * epar[j] - st * ng[j];
         krp_cross(ng, epar, shat);
