@@ -93,7 +93,8 @@ struct krp_grid {
     uint64_t next_id = 0;
     uint64_t launches = 0;
     int max_waves = 0;
-    int transport_block = 256, image_block = 256, blocks_per_sm = 8;
+    int transport_block = 256, image_block = 256, blocks_per_sm = 8;   // general mode: transport_block 128 (krp_grid_create)
+    int bps_tuned = 0;
     int burst = KRP_FLIGHT_BURST;   // cell steps between refill points of the flight kernels
     // optional per-launch timing (krp_timing_*)
     bool timing = false;
@@ -273,6 +274,7 @@ extern "C" int krp_grid_create(krp_grid** out, int nx, int ny, int nz, const dou
     m.a1c = op[0]; m.omc = op[3]; m.rho = rho;
     // scalar flights are short: static assignment; general flights are long: persistent lanes, refill every 32 steps
     g->burst = m.scalar ? 1 : 32;
+    if (!m.scalar) g->transport_block = 128;
     if (getenv("KRP_NO_DIR_SORT")) g->dir_sort = 0;   // A/B switches for measurement
     if (getenv("KRP_NO_OBS_PRE")) g->obs_pre = 0;
     if (m.scalar)
@@ -540,6 +542,10 @@ extern "C" int krp_transport(krp_grid* g, uint64_t n_packets, uint64_t seed, voi
     unsigned pers = (unsigned)(g->n_sm * g->blocks_per_sm);
     unsigned need = (n + tb - 1) / tb;
     unsigned grid_f = need < pers ? need : pers;
+    // general flight: persistent lanes, one resident set of blocks (640 threads per SM up to 128 per block, else 768) unless
+    // krp_tune set blocks_per_sm
+    const unsigned pers_g = (unsigned)g->n_sm * (unsigned)(g->bps_tuned ? g->blocks_per_sm : (tb <= 128 ? 640 / tb : 768 / tb));
+    const unsigned grid_g = need < pers_g ? need : pers_g;
     unsigned grid_s = (n + 127u) / 128u;
     if (grid_s > pers * 2) grid_s = pers * 2;
     for (int w = 0; w < g->max_waves; ++w) {
@@ -549,7 +555,8 @@ extern "C" int krp_transport(krp_grid* g, uint64_t n_packets, uint64_t seed, voi
         const KrpEmitSrc es = w == 0 ? es0 : KrpEmitSrc{ nullptr, 0, 0 };
         if (g->m.scalar && g->burst == 1) krp_k_flight_scalar_static<<<grid_f, tb, 0, st>>>(g->m, g->d_ctl, g->q[in], in, g->ev, es);
         else if (g->m.scalar) krp_k_flight_scalar<<<grid_f, tb, (size_t)(tb / 32) * sizeof(KrpWarpShared), st>>>(g->m, g->d_ctl, g->q[in], in, g->ev, g->burst, es);
-        else             krp_k_flight_general<<<grid_f, tb, 0, st>>>(g->m, g->d_ctl, g->q[in], in, g->ev, g->burst, es); }
+        else if (tb <= 128) krp_k_flight_general<128, 5><<<grid_g, tb, 0, st>>>(g->m, g->d_ctl, g->q[in], in, g->ev, g->burst, es);
+        else                krp_k_flight_general<256, 3><<<grid_g, tb, 0, st>>>(g->m, g->d_ctl, g->q[in], in, g->ev, g->burst, es); }
         g->launches += 2;
         if (w + 1 < g->max_waves) {
             TimedLaunch tl(g, st, KRP_T_SCATTER);
@@ -808,7 +815,7 @@ extern "C" int krp_tune(krp_grid* g, int transport_block, int image_block, int b
     if (blocks_per_sm < 0 || blocks_per_sm > 64) return fail(KRP_ERR_ARG, "blocks_per_sm must be in 0..64");
     if (transport_block) g->transport_block = transport_block;
     if (image_block) g->image_block = image_block;
-    if (blocks_per_sm) g->blocks_per_sm = blocks_per_sm;
+    if (blocks_per_sm) { g->blocks_per_sm = blocks_per_sm; g->bps_tuned = 1; }
     if (flight_burst < 0 || flight_burst > 4096) return fail(KRP_ERR_ARG, "flight_burst must be in 0..4096");
     if (flight_burst) g->burst = flight_burst;
     return KRP_OK;

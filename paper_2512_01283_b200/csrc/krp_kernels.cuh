@@ -7,9 +7,6 @@
 #pragma once
 #include "krp_device.cuh"
 
-#ifndef KRP_FLIGHT_GENERAL_MIN_BLOCKS
-#define KRP_FLIGHT_GENERAL_MIN_BLOCKS 3
-#endif
 #ifndef KRP_IMAGE_SCALAR_MIN_BLOCKS
 #define KRP_IMAGE_SCALAR_MIN_BLOCKS 8
 #endif
@@ -654,7 +651,10 @@ __device__ __forceinline__ void krp_appA_to_d(double i, double qg, double ug, do
     vt = (ug * sy + v * cy) * inv;
 }
 
-__global__ void __launch_bounds__(256, KRP_FLIGHT_GENERAL_MIN_BLOCKS) krp_k_flight_general(KrpModel g, KrpCtl* ctl, KrpRecords q, int in, KrpRecords ev, int n_burst, KrpEmitSrc es)
+// Two builds: blocks of up to 128 threads, five per SM (20 warps, 96 registers: the default, measured best of 16, 18, 20, 24 and 32
+// warps per SM on C4 and C5) and blocks of up to 256 threads, three per SM (24 warps, 80 registers) for krp_tune's larger blocks.
+template <int TPB, int MINB>
+__global__ void __launch_bounds__(TPB, MINB) krp_k_flight_general(KrpModel g, KrpCtl* ctl, KrpRecords q, int in, KrpRecords ev, int n_burst, KrpEmitSrc es)
 {
     const unsigned int n_items = ctl->q_count[in];
     KrpFlightTally tl = { 0, 0, 0, 0.0, 0.0, 0.0 };
