@@ -581,13 +581,16 @@ __device__ __forceinline__ double krp_event_solve_d(double R, double qq, double 
 {
     double t = R / a1;
     if (a2 != 0.0) {
-        const bool thin = fabs(a2 * tmax) < 0.35;
 #pragma unroll 1
         for (int it = 0; it < 40; ++it) {
             const double x = a2 * t;
             double sh, chm1;
-            if (thin) krp_sinh_coshm1_d(x, sh, chm1);
-            else { sh = sinh(x); chm1 = cosh(x) - 1.0; }
+            if (krp_abs_below(x, KRP_HI_0P35)) krp_sinh_coshm1_d(x, sh, chm1);
+            else {      // one exponential and one division for both (no cancellation from |x| = 0.35 on)
+                asm volatile("");
+                const double e = exp(fabs(x)), ie = 1.0 / e;
+                sh = copysign(0.5 * (e - ie), x); chm1 = 0.5 * (e + ie) - 1.0;
+            }
             const double gm1 = chm1 - qq * sh;
             double lg;
             if (fabs(gm1) < 0.01) {       // ln(1+g) = g - g^2/2 + ... to g^8 (remainder < 1e-19)
@@ -643,7 +646,7 @@ __device__ __forceinline__ void krp_appA_to_d(double i, double qg, double ug, do
     if (fabs(y) < 0.35) { double cym1; krp_sin_cosm1_d(y, sy, cym1); cy = 1.0 + cym1; }
     else { asm volatile(""); sincos(y, &sy, &cy); }
     if (fabs(x) < 0.35) { double chm1; krp_sinh_coshm1_d(x, sh, chm1); ch = 1.0 + chm1; }
-    else { sh = sinh(x); ch = cosh(x); }
+    else { const double e = exp(fabs(x)), ie = 1.0 / e; sh = copysign(0.5 * (e - ie), x); ch = 0.5 * (e + ie); }
     const double it = i * ch - qg * sh;
     const double inv = 1.0 / it;
     qt = (qg * ch - i * sh) * inv;

@@ -252,7 +252,8 @@ def test_launch_shapes_do_not_change_results():
         cfg = inputs.make(name, **kw)
         ref_ev = ref_img = None
         for tune in (dict(), dict(flight_burst=1), dict(flight_burst=5), dict(flight_burst=64, transport_block=128),
-                     dict(blocks_per_sm=2, image_block=64), dict(blocks_per_sm=16, flight_burst=16)):
+                     dict(blocks_per_sm=2, image_block=64), dict(blocks_per_sm=16, flight_burst=16),
+                     dict(transport_block=256), dict(transport_block=64, blocks_per_sm=4)):   # both builds of the general flight
             g = gpu_grid(cfg)
             g.tune(**tune)
             g.timing_enable(True)
