@@ -95,6 +95,7 @@ struct krp_grid {
     int max_waves = 0;
     int transport_block = 256, image_block = 256, blocks_per_sm = 8;   // general mode: transport_block 128 (krp_grid_create)
     int bps_tuned = 0;
+    int ev_has_emission = 0;        // emission records (k = 0) may be in the event buffer
     int burst = KRP_FLIGHT_BURST;   // cell steps between refill points of the flight kernels
     // optional per-launch timing (krp_timing_*)
     bool timing = false;
@@ -509,6 +510,7 @@ extern "C" int krp_transport(krp_grid* g, uint64_t n_packets, uint64_t seed, voi
         }
     }
     const unsigned n = (unsigned)n_packets;
+    if (g->m.emit_records) g->ev_has_emission = 1;
     const int tb = g->transport_block;
     const unsigned grid_all = (n + 255u) / 256u;
     KrpEmitSrc es0 = { nullptr, g->next_id, seed };     // first scattering order
@@ -668,10 +670,11 @@ extern "C" int krp_image(krp_grid* g, const krp_observer* obs, int n_obs, int np
     { TimedLaunch tlo(g, st, KRP_T_ORDER);
     if (g->order_events) {
         CK(cudaMemsetAsync(g->d_bins, 0, sizeof(unsigned int) * ((size_t)g->n_bins + 1), st));
-        krp_k_sort_count<<<pers, 256, 0, st>>>(g->d_ctl, g->ev, g->bin_shift, g->sub_bits, flags, g->d_bins);
+        const int sflags = flags | (g->ev_has_emission ? 0 : 2);       // bit 1: no emission records to look for
+        krp_k_sort_count<<<pers, 256, 0, st>>>(g->d_ctl, g->ev, g->bin_shift, g->sub_bits, sflags, g->d_bins);
         CK(cub::DeviceScan::ExclusiveSum(g->d_scan, g->scan_bytes, g->d_bins, g->d_bins, (int)(g->n_bins + 1), st));
         krp_k_image_prep<<<1, 1, 0, st>>>(g->d_ctl, g->d_bins, g->n_bins);
-        krp_k_sort_scatter<<<pers, 256, 0, st>>>(g->d_ctl, g->ev, g->bin_shift, g->sub_bits, flags, g->d_bins, g->d_perm);
+        krp_k_sort_scatter<<<pers, 256, 0, st>>>(g->d_ctl, g->ev, g->bin_shift, g->sub_bits, sflags, g->d_bins, g->d_perm);
         g->launches += 5;   // count, scan (2 kernels), prep, scatter
     } else {
         krp_k_image_prep_plain<<<1, 1, 0, st>>>(g->d_ctl);
@@ -695,6 +698,7 @@ extern "C" int krp_image(krp_grid* g, const krp_observer* obs, int n_obs, int np
         g->launches++;
     }
     krp_k_events_clear<<<1, 1, 0, st>>>(g->d_ctl);
+    g->ev_has_emission = 0;
     g->launches++;
     CK(cudaGetLastError());
     // counters of this pass for the ordering decision of a later one (never waited for)
@@ -802,6 +806,7 @@ extern "C" int krp_events_clear(krp_grid* g, void* stream)
 {
     if (!g) return fail(KRP_ERR_ARG, "grid is NULL");
     krp_k_events_clear<<<1, 1, 0, (cudaStream_t)stream>>>(g->d_ctl);
+    g->ev_has_emission = 0;
     g->launches++;
     CK(cudaGetLastError());
     return KRP_OK;

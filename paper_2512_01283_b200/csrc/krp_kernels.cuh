@@ -1012,8 +1012,8 @@ __global__ void __launch_bounds__(256) krp_k_sort_count(KrpCtl* ctl, KrpRecords 
     const unsigned int sub_mask = (1u << sub_bits) - 1u;
     for (unsigned long long e = blockIdx.x * (unsigned long long)blockDim.x + threadIdx.x; e < n_ev;
          e += (unsigned long long)gridDim.x * blockDim.x) {
-        const uint32_t k = __float_as_uint(ev.nk[e].w) & ~KRP_TERM_BIT;
-        if (k == 0u && !(flags & 1)) continue;             // emission records take part only with direct light
+        // emission records take part only with direct light (flags bit 1: the buffer holds none, no need to look)
+        if (!(flags & 3) && (__float_as_uint(ev.nk[e].w) & ~KRP_TERM_BIT) == 0u) continue;
         atomicAdd(bins + (((__float_as_uint(ev.pc[e].w) >> shift) << sub_bits) | ((unsigned int)e & sub_mask)), 1u);
     }
 }
@@ -1027,8 +1027,7 @@ __global__ void __launch_bounds__(256) krp_k_sort_scatter(KrpCtl* ctl, KrpRecord
     const unsigned int sub_mask = (1u << sub_bits) - 1u;
     for (unsigned long long e = blockIdx.x * (unsigned long long)blockDim.x + threadIdx.x; e < n_ev;
          e += (unsigned long long)gridDim.x * blockDim.x) {
-        const uint32_t k = __float_as_uint(ev.nk[e].w) & ~KRP_TERM_BIT;
-        if (k == 0u && !(flags & 1)) continue;
+        if (!(flags & 3) && (__float_as_uint(ev.nk[e].w) & ~KRP_TERM_BIT) == 0u) continue;
         const unsigned int slot = atomicAdd(bins + (((__float_as_uint(ev.pc[e].w) >> shift) << sub_bits) | ((unsigned int)e & sub_mask)), 1u);
         perm[slot] = (unsigned int)e;
     }
