@@ -7,6 +7,9 @@
 #pragma once
 #include "krp_device.cuh"
 
+#ifndef KRP_IMG_CHUNK
+#define KRP_IMG_CHUNK 128     // events a warp of the imaging kernels takes per atomic (a multiple of 32)
+#endif
 #ifndef KRP_IMAGE_SCALAR_MIN_BLOCKS
 #define KRP_IMAGE_SCALAR_MIN_BLOCKS 8
 #endif
@@ -1171,11 +1174,20 @@ __global__ void __launch_bounds__(256, SCALAR ? KRP_IMAGE_SCALAR_MIN_BLOCKS : KR
     __shared__ KrpRayAConst s_rc;
     const KrpRayAConst rc = krp_raya_const(ob, nseg, &s_rc);
     unsigned long long steps = 0, n_con = 0, n_drop = 0;
+    // a warp takes KRP_IMG_CHUNK consecutive events of the order per visit to the launch's counter (32 when the events are
+    // few, for the balance of the tail): with 32 per visit a large launch queues on that one address (3.4 x 10^5 atomics per
+    // 10^7 rays; C2's imaging 8.9 -> 8.1 ms)
+    const unsigned int chunk = n_ev >= (1u << 21) ? (unsigned int)KRP_IMG_CHUNK : 32u;
+    unsigned int cbase = 0, cleft = 0;
     for (;;) {
-        unsigned int base = 0;
-        if (lane == 0) base = atomicAdd(&ctl->img_work[slot], 32u);
-        base = __shfl_sync(0xffffffffu, base, 0);
-        if (base >= n_ev) break;
+        if (cleft == 0u) {
+            if (lane == 0) cbase = atomicAdd(&ctl->img_work[slot], chunk);
+            cbase = __shfl_sync(0xffffffffu, cbase, 0);
+            cleft = chunk;
+        }
+        const unsigned int base = cbase;
+        cbase += 32u; cleft -= 32u;
+        if (base >= n_ev) break;            // so are all later chunks
         bool live = base + lane < n_ev;
         int pixel = -1;
         float out[4] = { 0.f, 0.f, 0.f, 0.f };
