@@ -1174,10 +1174,11 @@ __global__ void __launch_bounds__(256, SCALAR ? KRP_IMAGE_SCALAR_MIN_BLOCKS : KR
     __shared__ KrpRayAConst s_rc;
     const KrpRayAConst rc = krp_raya_const(ob, nseg, &s_rc);
     unsigned long long steps = 0, n_con = 0, n_drop = 0;
-    // a warp takes KRP_IMG_CHUNK consecutive events of the order per visit to the launch's counter (32 when the events are
-    // few, for the balance of the tail): with 32 per visit a large launch queues on that one address (3.4 x 10^5 atomics per
-    // 10^7 rays; C2's imaging 8.9 -> 8.1 ms)
-    const unsigned int chunk = n_ev >= (1u << 21) ? (unsigned int)KRP_IMG_CHUNK : 32u;
+    // SCALAR mode: a warp takes KRP_IMG_CHUNK consecutive events of the order per visit to the launch's counter (32 when the
+    // events are few, for the balance of the tail): with 32 per visit a large launch of short rays queues on that one address
+    // (3.4 x 10^5 atomics per 10^7 rays; C2's imaging 8.9 -> 8.1 ms).  General mode keeps 32: its rays are long, and the
+    // warps of an SM then work on one narrow window of the order and share its cells in L1/L2 (C5: 512 ms, 564 ms with 128).
+    const unsigned int chunk = (SCALAR && n_ev >= (1u << 21)) ? (unsigned int)KRP_IMG_CHUNK : 32u;
     unsigned int cbase = 0, cleft = 0;
     for (;;) {
         if (cleft == 0u) {
