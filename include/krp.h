@@ -172,8 +172,9 @@ int krp_events_get(krp_grid* g, uint64_t cap, uint64_t* n, uint64_t* id, int32_t
 int krp_events_clear(krp_grid* g, void* stream);
 
 /* Launch-shape knobs, for measurement only (0 keeps the current value): threads per block of the
- * flight and imaging kernels (multiples of 32 up to 256), persistent blocks per SM, and the number
- * of cell steps a flight kernel takes between two points where idle lanes take new packets. */
+ * flight and imaging kernels (multiples of 32 up to 256; defaults 256, general-mode flights 128),
+ * persistent blocks per SM (default: 8; the general-mode flight fills an SM once, 640 threads), and
+ * the number of cell steps a flight kernel takes between two points where idle lanes take new packets. */
 int krp_tune(krp_grid* g, int transport_block, int image_block, int blocks_per_sm, int flight_burst);
 /* Device time per kernel class, for measurement (bench.py's roofline): when enabled, every launch of a
  * flight, scattering, ordering or imaging kernel is bracketed by CUDA events on the caller's stream.
