@@ -218,7 +218,7 @@ def run_reference(args):
 # `ncu --set full` capture of this same command (profiles/, named per round); None until captured.
 NCU_TRAFFIC = {   # bytes, profiles/r1d_ncu_full_*.txt: the first-order flight launch (C2, C4), one observer's imaging launch (C5)
     "c2": 154.27788e6 + 375.54688e6,        # profiles/r1e_ncu_full_c2_flight.txt
-    "c4": 42.137358e9 + 2.835999e9,
+    "c4": 40.274337e9 + 1.702403e9,         # profiles/r1h_ncu_full_c4_flight.txt
     "c5": 227.68106e9 + 1.778706e9,
 }
 
