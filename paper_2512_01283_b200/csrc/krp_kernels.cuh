@@ -665,14 +665,14 @@ __global__ void __launch_bounds__(TPB, MINB) krp_k_flight_general(KrpModel g, Kr
     const unsigned int n_items = ctl->q_count[in];
     KrpFlightTally tl = { 0, 0, 0, 0.0, 0.0, 0.0 };
     const double xs = g.xs;
-    const float guard = g.guard;
+    const float inv_guard = 1.f / g.guard;
     int status = KRP_IDLE;
     bool more = true;
     unsigned int item = 0, wbase = 0, wleft = 0;
     // state of the flight in progress (all fp64: it decides where the event falls)
     double nd[3] = { 0.0, 0.0, 1.0 }, th[3] = { 0.0, 0.0, 0.0 }, ph[3] = { 0.0, 0.0, 0.0 };
     double D = 0.0, i = 1.0, qs = 0.0, us = 0.0, vs = 0.0;
-    float Asum = 0.f, tau0f = 0.f;
+    float arm = 0.f;        // tau*/guard minus the fp32 sum of alpha1 dtau: the fp64 event test is armed once it is <= 0
     unsigned int nsteps = 0;
     KrpRayD ray = {};
     float4 cl = make_float4(0.f, 0.f, 0.f, 1.f), cl_f = cl;
@@ -734,7 +734,7 @@ __global__ void __launch_bounds__(TPB, MINB) krp_k_flight_general(KrpModel g, Kr
             }
             D = tau0; i = 1.0;
             qs = S0.y; us = S0.z; vs = S0.w;      // lab reference
-            Asum = 0.f; tau0f = (float)tau0; nsteps = 0;
+            arm = (float)tau0 * inv_guard; nsteps = 0;
             status = KRP_RUN;
         }
         if (!__any_sync(0xffffffffu, status == KRP_RUN)) break;
@@ -758,8 +758,8 @@ __global__ void __launch_bounds__(TPB, MINB) krp_k_flight_general(KrpModel g, Kr
             if (cl.x > 0.f) {
                 KrpCellCoef cc;
                 krp_cell_coef(g, cl, nd, xs, ds, cc);
-                Asum += (float)cc.dt1;
-                const bool near_end = Asum * guard >= tau0f;
+                arm -= (float)cc.dt1;
+                const bool near_end = arm <= 0.f;
                 if (cc.a2 == 0.0 && cc.a3 == 0.0) {
                     if (near_end && cc.dt1 >= D + log(i)) { status = KRP_HIT; continue; }
                     D -= cc.dt1;
