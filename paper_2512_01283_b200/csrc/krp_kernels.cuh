@@ -1324,20 +1324,30 @@ __global__ void __launch_bounds__(256, SCALAR ? KRP_IMAGE_SCALAR_MIN_BLOCKS : KR
                 out[0] = att * S[0]; out[1] = att * S[1]; out[2] = att * S[2]; out[3] = att * S[3];
             }
         }
-        // I3: one atomic per distinct pixel of the warp: the lowest lane of every group of equal pixels
-        // collects the group's values (fp64) one peer at a time
+        // I3: one atomic per distinct pixel of the warp: the values of every group of equal pixels are summed (fp64)
+        // into its lowest lane
         const unsigned peers = __match_any_sync(0xffffffffu, pixel);
         const int leader = __ffs(peers) - 1;
-        unsigned rem = peers & ~(1u << leader);
         double acc[4] = { (double)out[0], (double)out[1], (double)out[2], (double)out[3] };
-        while (__any_sync(0xffffffffu, rem != 0u && pixel >= 0)) {
-            const int src = rem ? __ffs(rem) - 1 : lane;
+        {
+            // tree over the lanes of each group, by their rank in it: in every round the lanes of even rank add the
+            // partial sum of the next lane of their group still in play, those of odd rank leave: at most five
+            // rounds (a group of 32), where collecting one peer at a time took up to 31
+            int rank = __popc(peers & ((1u << lane) - 1u));
+            bool in_play = pixel >= 0;
+            unsigned above = in_play ? peers & (0xfffffffeu << lane) : 0u;     // lanes of the group above this one, still in play
+            while (__any_sync(0xffffffffu, above != 0u)) {
+                const int src = above ? __ffs(above) - 1 : lane;
 #pragma unroll
-            for (int s = 0; s < 4; ++s) {
-                const float v = __shfl_sync(0xffffffffu, out[s], src);
-                if (rem) acc[s] += (double)v;
+                for (int s = 0; s < 4; ++s) {
+                    const double v = __shfl_sync(0xffffffffu, acc[s], src);
+                    if (above) acc[s] += v;
+                }
+                const unsigned stay = __ballot_sync(0xffffffffu, in_play && !(rank & 1));
+                if (rank & 1) in_play = false;                              // added to its neighbour below
+                above = in_play ? above & stay : 0u;
+                rank >>= 1;
             }
-            rem &= rem - 1u;
         }
         if (pixel >= 0 && lane == leader) {
             const size_t plane = (size_t)npx * npy;
