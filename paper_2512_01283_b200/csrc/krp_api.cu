@@ -284,6 +284,7 @@ extern "C" int krp_grid_create(krp_grid** out, int nx, int ny, int nz, const dou
     g->order_events = g->order_policy != 0;
     m.n_inc = n_inc; m.n_ang = tables->n_ang;
     m.xs = (double)(n_inc - 1); m.guard = 1.f + m.rho + 1e-3f; m.inv_nang1 = 1.0 / (double)(tables->n_ang - 1);
+    m.nang1_over_pi = (float)((double)(tables->n_ang - 1) / 3.14159265358979323846);
     m.w_min = tables->w_min; m.max_scatter = tables->max_scatter;
     // number of waves that can contain live packets: the weight after k scatterings is <= omega_max^k
     {

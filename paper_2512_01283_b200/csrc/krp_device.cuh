@@ -43,6 +43,7 @@ struct KrpModel {
     const float4* mueller; // [n_ang] {S11,S12,S33,S34}
     int n_ang;
     double inv_nang1;      // 1/(n_ang-1)
+    float nang1_over_pi;   // (n_ang-1)/pi: scattering angle in radians -> units of the table spacing
     const double* cdf;     // [n_ang] Theta CDF of S11 sin(Theta)
     float a1c, omc;        // SCALAR mode constants
     float rho;             // max |alpha2|/alpha1 over the table

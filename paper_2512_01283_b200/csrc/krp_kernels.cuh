@@ -969,22 +969,39 @@ __device__ __forceinline__ void krp_rot_qu_f(float& Q, float& U, float ce, float
 
 __device__ __forceinline__ void krp_peel(const KrpModel& g, const float n[3], float4 Se, const KrpObserverDev& ob, float S[4])
 {
+    // spherical basis of n (eq. 4-5, R10) and the unit normal of the scattering plane with the hardware reciprocal
+    // square root (2 ulp): this runs once per (event, observer), and IEEE divisions and square roots were a fifth of it
     float th[3], ph[3];
-    krp_basis<float>(n, th, ph);
+    {
+        const float s2 = n[0] * n[0] + n[1] * n[1];
+        const float inv_rr = rsqrtf(s2 + n[2] * n[2]);
+        float cp = 1.f, sp = 0.f, s = 0.f;
+        if (s2 >= 1e-24f) { const float inv_s = rsqrtf(s2); s = s2 * inv_s; cp = n[0] * inv_s; sp = n[1] * inv_s; }
+        const float ct = n[2] * inv_rr, st = s * inv_rr;
+        th[0] = ct * cp; th[1] = ct * sp; th[2] = -st;
+        ph[0] = -sp; ph[1] = cp; ph[2] = 0.f;
+    }
     float mu = n[0] * ob.n[0] + n[1] * ob.n[1] + n[2] * ob.n[2];
     mu = fminf(fmaxf(mu, -1.f), 1.f);
     float sh[3] = { n[1] * ob.n[2] - n[2] * ob.n[1], n[2] * ob.n[0] - n[0] * ob.n[2], n[0] * ob.n[1] - n[1] * ob.n[0] };
-    float sn = sqrtf(sh[0] * sh[0] + sh[1] * sh[1] + sh[2] * sh[2]);
-    if (sn < 1e-12f) { sh[0] = ph[0]; sh[1] = ph[1]; sh[2] = ph[2]; }
-    else { float r = 1.f / sn; sh[0] *= r; sh[1] *= r; sh[2] *= r; }
+    const float ss = sh[0] * sh[0] + sh[1] * sh[1] + sh[2] * sh[2];
+    float sn = 0.f;
+    if (ss < 1e-24f) { sh[0] = ph[0]; sh[1] = ph[1]; sh[2] = ph[2]; }
+    else { const float r = rsqrtf(ss); sn = ss * r; sh[0] *= r; sh[1] *= r; sh[2] *= r; }
     // e_par = s^ x n_in: reference of the incoming ray in the scattering plane
     float ep[3] = { sh[1] * n[2] - sh[2] * n[1], sh[2] * n[0] - sh[0] * n[2], sh[0] * n[1] - sh[1] * n[0] };
     float I = Se.x, Q = Se.x * Se.y, U = Se.x * Se.z, V = Se.x * Se.w;
     krp_rot_qu_f(Q, U, th[0] * ep[0] + th[1] * ep[1] + th[2] * ep[2], ph[0] * ep[0] + ph[1] * ep[1] + ph[2] * ep[2]);
     // scattering angle from atan2(|n x n_obs|, n.n_obs): well conditioned at both poles
-    float theta_deg = atan2f(sn, mu) * 57.29577951308232f;
+    // (in units of the table spacing: the Mueller row is linear in it, R13)
+    const float x = atan2f(sn, mu) * g.nang1_over_pi;
     float F[4];
-    krp_mueller_at<float>(g.mueller, g.n_ang, theta_deg, F);
+    {
+        const int j = max(0, min((int)x, g.n_ang - 2));
+        const float w = x - (float)j, w0 = 1.f - w;
+        const float4 a = g.mueller[j], b = g.mueller[j + 1];
+        F[0] = w0 * a.x + w * b.x; F[1] = w0 * a.y + w * b.y; F[2] = w0 * a.z + w * b.z; F[3] = w0 * a.w + w * b.w;
+    }
     float I2 = F[0] * I + F[1] * Q, Q2 = F[1] * I + F[0] * Q;
     float U2 = F[2] * U + F[3] * V, V2 = -F[3] * U + F[2] * V;
     // e_out = s^ x n_obs, then to theta^_obs
