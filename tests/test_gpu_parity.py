@@ -187,7 +187,7 @@ def test_full_size_c2_sampled_ids():
     hold at any size."""
     cfg = inputs.make("c2")
     g = gpu_grid(cfg)
-    ids0, ns = 5000000, 1500
+    ids0, ns = 5000000, 12000
     g.packet_id_set(ids0)
     g.transport(ns, cfg["seed"])
     gev = gpu_events_sorted(g)
@@ -222,7 +222,7 @@ def test_full_size_c2_sampled_ids():
     assert abs(img[0, 1].sum()) < 0.01 * img[0, 0].sum() and abs(img[0, 2].sum()) < 0.01 * img[0, 0].sum()
 
 
-@pytest.mark.parametrize("name,ns", [("c3", 600), ("c4", 1200), ("c5", 250)])
+@pytest.mark.parametrize("name,ns", [("c3", 3000), ("c4", 4000), ("c5", 800)])
 def test_full_size_general_mode_sampled_ids(name, ns):
     """BASELINE configs[2..4] at full grid and image size (64x64x256, 256^3, 512^3; general cell layout, persistent
     flights): a sample of the job's packet ids replayed by the oracle one by one, sequences and maps of those ids."""
