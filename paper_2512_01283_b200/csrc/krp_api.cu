@@ -64,6 +64,7 @@ struct krp_grid {
     unsigned int* d_dir_bins = nullptr;
     void* d_dir_scan = nullptr;
     size_t dir_scan_bytes = 0;
+    size_t dir_bins_cap = 0;         // counters d_dir_bins holds
     int dir_sort = 1;
     unsigned int* d_order = nullptr;
     uint64_t order_cap = 0;
@@ -520,10 +521,17 @@ extern "C" int krp_transport(krp_grid* g, uint64_t n_packets, uint64_t seed, voi
         if (g->m.src_kind == 0 && !g->m.emit_records && g->dir_sort && n >= (1u << 16)) {
             // isotropic point source: the first flights take the packets in the order of their direction and
             // compute the emission themselves (count, scan, order); nothing is written to the queue
-            if (!g->d_dir_bins) {
-                CK(cudaMalloc(&g->d_dir_bins, sizeof(unsigned int) * KRP_DIR_BINS));
-                CK(cub::DeviceScan::ExclusiveSum(nullptr, g->dir_scan_bytes, g->d_dir_bins, g->d_dir_bins, (int)KRP_DIR_BINS, st));
+            // sub-batches of 2^23 packets (32 MiB of slots each; measured on C2 against 2^21, 2^22 and one batch)
+            unsigned sub_shift = KRP_DIR_SUB_SHIFT;
+            while (((n - 1u) >> sub_shift) + 1u > KRP_DIR_SUBS_MAX) ++sub_shift;
+            const size_t n_bins = (size_t)(((n - 1u) >> sub_shift) + 1u) * KRP_DIR_BINS;
+            if (g->dir_bins_cap < n_bins) {
+                CK(cudaStreamSynchronize(st));
+                cudaFree(g->d_dir_bins); cudaFree(g->d_dir_scan); g->d_dir_bins = nullptr; g->d_dir_scan = nullptr; g->dir_bins_cap = 0;
+                CK(cudaMalloc(&g->d_dir_bins, sizeof(unsigned int) * n_bins));
+                CK(cub::DeviceScan::ExclusiveSum(nullptr, g->dir_scan_bytes, g->d_dir_bins, g->d_dir_bins, (int)n_bins, st));
                 CK(cudaMalloc(&g->d_dir_scan, g->dir_scan_bytes ? g->dir_scan_bytes : 16));
+                g->dir_bins_cap = n_bins;
             }
             if (g->order_cap < n_packets) {
                 CK(cudaStreamSynchronize(st));
@@ -531,10 +539,10 @@ extern "C" int krp_transport(krp_grid* g, uint64_t n_packets, uint64_t seed, voi
                 CK(cudaMalloc(&g->d_order, sizeof(unsigned int) * n_packets));
                 g->order_cap = n_packets;
             }
-            CK(cudaMemsetAsync(g->d_dir_bins, 0, sizeof(unsigned int) * KRP_DIR_BINS, st));
-            krp_k_emit_count<<<grid_all, 256, 0, st>>>(g->next_id, n, seed, g->d_dir_bins);
-            CK(cub::DeviceScan::ExclusiveSum(g->d_dir_scan, g->dir_scan_bytes, g->d_dir_bins, g->d_dir_bins, (int)KRP_DIR_BINS, st));
-            krp_k_emit_order<<<grid_all, 256, 0, st>>>(g->d_ctl, g->next_id, n, seed, g->d_dir_bins, g->d_order);
+            CK(cudaMemsetAsync(g->d_dir_bins, 0, sizeof(unsigned int) * n_bins, st));
+            krp_k_emit_count<<<grid_all, 256, 0, st>>>(g->next_id, n, seed, g->d_dir_bins, sub_shift);
+            CK(cub::DeviceScan::ExclusiveSum(g->d_dir_scan, g->dir_scan_bytes, g->d_dir_bins, g->d_dir_bins, (int)n_bins, st));
+            krp_k_emit_order<<<grid_all, 256, 0, st>>>(g->d_ctl, g->next_id, n, seed, g->d_dir_bins, g->d_order, sub_shift);
             g->launches += 3;
             es0.order = g->d_order;
         } else {

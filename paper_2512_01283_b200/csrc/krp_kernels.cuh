@@ -25,22 +25,27 @@
 // the order of their direction (128 bins in cos(theta) x 256 in phi, read off the uniform words, 32 counters
 // per bin against contention), so that the 32 flights of a warp walk through the same cells -- their gathers hit
 // the same lines and they leave the grid together.  The queue order has no meaning for the results.
+// A large batch is ordered in sub-batches of 2^sub_shift packets (the sub-batch is the leading key): the slots one
+// sub-batch writes then span a few tens of MB, so that the 4-byte writes of a bin meet in L2 before they go to DRAM.
 #define KRP_DIR_BINS (1u << 20)
-__device__ __forceinline__ unsigned int krp_dir_bin(uint4 w, unsigned int i)
+#define KRP_DIR_SUBS_MAX 16u
+#define KRP_DIR_SUB_SHIFT 23u
+__device__ __forceinline__ unsigned int krp_dir_bin(uint4 w, unsigned int i, unsigned int sub_shift)
 {
-    return ((((w.x >> 25) << 8) | (w.y >> 24)) << 5) | (i & 31u);
+    return ((i >> sub_shift) << 20) | ((((w.x >> 25) << 8) | (w.y >> 24)) << 5) | (i & 31u);
 }
 __global__ void __launch_bounds__(256) krp_k_emit_count(unsigned long long id0, unsigned int n, unsigned long long seed,
-                                                        unsigned int* __restrict__ dir_bins)
+                                                        unsigned int* __restrict__ dir_bins, unsigned int sub_shift)
 {
     unsigned int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= n) return;
-    atomicAdd(dir_bins + krp_dir_bin(krp_philox(seed, id0 + i, 0u, 0u), i), 1u);
+    atomicAdd(dir_bins + krp_dir_bin(krp_philox(seed, id0 + i, 0u, 0u), i, sub_shift), 1u);
 }
 
 // order[slot] = index of the packet within the batch, slot taken from the scanned direction bins
 __global__ void __launch_bounds__(256) krp_k_emit_order(KrpCtl* ctl, unsigned long long id0, unsigned int n, unsigned long long seed,
-                                                        unsigned int* __restrict__ dir_bins, unsigned int* __restrict__ order)
+                                                        unsigned int* __restrict__ dir_bins, unsigned int* __restrict__ order,
+                                                        unsigned int sub_shift)
 {
     unsigned int i = blockIdx.x * blockDim.x + threadIdx.x;
     if (i == 0) {
@@ -49,7 +54,7 @@ __global__ void __launch_bounds__(256) krp_k_emit_order(KrpCtl* ctl, unsigned lo
         atomicAdd(&ctl->stats.w_emitted, (double)n);
     }
     if (i >= n) return;
-    order[atomicAdd(dir_bins + krp_dir_bin(krp_philox(seed, id0 + i, 0u, 0u), i), 1u)] = i;
+    order[atomicAdd(dir_bins + krp_dir_bin(krp_philox(seed, id0 + i, 0u, 0u), i, sub_shift), 1u)] = i;
 }
 
 // Where a flight kernel takes its queue entries from: the packet queue, or (first scattering order of an isotropic
@@ -126,7 +131,7 @@ __global__ void __launch_bounds__(256) krp_k_emit(KrpModel g, KrpCtl* ctl, KrpRe
         cell = g.src_cell; p[0] = g.src_p[0]; p[1] = g.src_p[1]; p[2] = g.src_p[2];
     }
     float4 pc = make_float4(p[0], p[1], p[2], __uint_as_float(cell));
-    const unsigned int slot = dir_bins ? atomicAdd(dir_bins + krp_dir_bin(w, i), 1u) : i;   // scanned counters: first slot of the bin
+    const unsigned int slot = dir_bins ? atomicAdd(dir_bins + krp_dir_bin(w, i, 31u), 1u) : i;   // scanned counters: first slot of the bin
     q.pc[slot] = pc;
     q.nk[slot] = make_float4(nn[0], nn[1], nn[2], __uint_as_float(0u));
     q.S[slot] = make_float4(1.f, 0.f, 0.f, 0.f);
@@ -1024,17 +1029,27 @@ __device__ __forceinline__ void krp_peel(const KrpModel& g, const float n[3], fl
 //   (exclusive scan of the histogram: cub::DeviceScan, in krp_api.cu)
 //   krp_k_sort_scatter  perm[slot] = event index, slot reserved in the event's bin
 // ------------------------------------------------------------------------------------------
+// Both kernels walk the buffer in aligned groups of 32 events, one group per warp and visit; the lanes of a group that
+// fall into the same bin are counted (and given their slots) by one atomic of their first lane (__match_any_sync), on the
+// bin's sub-counter number (group index mod 2^sub_bits): the events next to a point source, which are a large share of
+// every group, would otherwise queue on the one L2 slice that holds their bin's counters.
 __global__ void __launch_bounds__(256) krp_k_sort_count(KrpCtl* ctl, KrpRecords ev, int shift, int sub_bits, int flags,
                                                         unsigned int* __restrict__ bins)
 {
     unsigned long long n_ev = ctl->n_events;
     if (n_ev > ctl->ev_cap) n_ev = ctl->ev_cap;
     const unsigned int sub_mask = (1u << sub_bits) - 1u;
-    for (unsigned long long e = blockIdx.x * (unsigned long long)blockDim.x + threadIdx.x; e < n_ev;
-         e += (unsigned long long)gridDim.x * blockDim.x) {
+    const unsigned int lane = threadIdx.x & 31u;
+    for (unsigned long long e0 = blockIdx.x * (unsigned long long)blockDim.x + (threadIdx.x & ~31u); e0 < n_ev;
+         e0 += (unsigned long long)gridDim.x * blockDim.x) {
+        const unsigned long long e = e0 + lane;
         // emission records take part only with direct light (flags bit 1: the buffer holds none, no need to look)
-        if (!(flags & 3) && (__float_as_uint(ev.nk[e].w) & ~KRP_TERM_BIT) == 0u) continue;
-        atomicAdd(bins + (((__float_as_uint(ev.pc[e].w) >> shift) << sub_bits) | ((unsigned int)e & sub_mask)), 1u);
+        bool valid = e < n_ev;
+        if (valid && !(flags & 3) && (__float_as_uint(ev.nk[e].w) & ~KRP_TERM_BIT) == 0u) valid = false;
+        const unsigned int bin = valid ? (__float_as_uint(ev.pc[e].w) >> shift) : 0xffffffffu;
+        const unsigned int peers = __match_any_sync(0xffffffffu, bin);
+        if (valid && lane == (unsigned int)(__ffs(peers) - 1))
+            atomicAdd(bins + ((bin << sub_bits) | ((unsigned int)(e0 >> 5) & sub_mask)), (unsigned int)__popc(peers));
     }
 }
 
@@ -1045,11 +1060,20 @@ __global__ void __launch_bounds__(256) krp_k_sort_scatter(KrpCtl* ctl, KrpRecord
     unsigned long long n_ev = ctl->n_events;
     if (n_ev > ctl->ev_cap) n_ev = ctl->ev_cap;
     const unsigned int sub_mask = (1u << sub_bits) - 1u;
-    for (unsigned long long e = blockIdx.x * (unsigned long long)blockDim.x + threadIdx.x; e < n_ev;
-         e += (unsigned long long)gridDim.x * blockDim.x) {
-        if (!(flags & 3) && (__float_as_uint(ev.nk[e].w) & ~KRP_TERM_BIT) == 0u) continue;
-        const unsigned int slot = atomicAdd(bins + (((__float_as_uint(ev.pc[e].w) >> shift) << sub_bits) | ((unsigned int)e & sub_mask)), 1u);
-        perm[slot] = (unsigned int)e;
+    const unsigned int lane = threadIdx.x & 31u;
+    for (unsigned long long e0 = blockIdx.x * (unsigned long long)blockDim.x + (threadIdx.x & ~31u); e0 < n_ev;
+         e0 += (unsigned long long)gridDim.x * blockDim.x) {
+        const unsigned long long e = e0 + lane;
+        bool valid = e < n_ev;
+        if (valid && !(flags & 3) && (__float_as_uint(ev.nk[e].w) & ~KRP_TERM_BIT) == 0u) valid = false;
+        const unsigned int bin = valid ? (__float_as_uint(ev.pc[e].w) >> shift) : 0xffffffffu;
+        const unsigned int peers = __match_any_sync(0xffffffffu, bin);
+        const int first = __ffs(peers) - 1;
+        unsigned int base = 0u;
+        if (valid && lane == (unsigned int)first)
+            base = atomicAdd(bins + ((bin << sub_bits) | ((unsigned int)(e0 >> 5) & sub_mask)), (unsigned int)__popc(peers));
+        base = __shfl_sync(0xffffffffu, base, first);
+        if (valid) perm[base + __popc(peers & ((1u << lane) - 1u))] = (unsigned int)e;
     }
 }
 
