@@ -371,9 +371,14 @@ extern "C" int krp_grid_create(krp_grid** out, int nx, int ny, int nz, const dou
     g->bin_shift = m.scalar ? 5 : 3;
     while ((g->npad >> g->bin_shift) >= (1u << 25)) g->bin_shift++;
     g->n_bins = (g->npad >> g->bin_shift) + 1;
-    // sub-counters per bin against atomic contention in hot cells: about 2^21 counters in all, at most 64 per bin
+    // sub-counters per bin against atomic contention in hot cells.  A grid of few bins (up to 2^17: C1, C2) collects hundreds
+    // of events per bin and takes up to 128 counters per bin (four lines, 2^24 counters at most; measured on C2: 16 per bin
+    // 0.85 ms, 64 0.86 ms, 128 0.57 ms, 256 0.61 ms); a large grid has a few events per bin and pays for every extra counter in the
+    // scan (C4: 1 per bin 0.63 ms, 2 0.76 ms, 4 0.88 ms): about 2^21 counters in all, at most 64 per bin
+    const bool few_bins = g->n_bins <= (1u << 17);
+    const int sub_max = few_bins ? 7 : 6, cap_log2 = few_bins ? 24 : 21;
     g->sub_bits = 0;
-    while (g->sub_bits < 6 && ((uint64_t)g->n_bins << (g->sub_bits + 1)) <= (1ull << 21)) g->sub_bits++;
+    while (g->sub_bits < sub_max && ((uint64_t)g->n_bins << (g->sub_bits + 1)) <= (1ull << cap_log2)) g->sub_bits++;
     g->n_bins <<= g->sub_bits;
     CK(cudaMalloc(&g->d_bins, sizeof(unsigned int) * ((size_t)g->n_bins + 1)));
     CK(cub::DeviceScan::ExclusiveSum(nullptr, g->scan_bytes, g->d_bins, g->d_bins, (int)(g->n_bins + 1), st));
