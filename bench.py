@@ -7,8 +7,9 @@ A "step" is one pass of the whole hot path over one batch of B new packets of th
 krp_transport(B) (emit, flights, scatterings, event records) followed by krp_image (every event toward
 every observer, attenuated to the grid edge, summed into the fp64 I,Q,U,V maps).  Packet ids continue
 from step to step, so K steps are K*B distinct packets of the job.  Inputs are seeded and synthetic
-(paper_2512_01283_b200.inputs, recipe in DESIGN.md); the default workload is BASELINE.json configs[1]
-(flared disk, 128^3 cells, 4 inclinations at 256x256).
+(paper_2512_01283_b200.inputs, recipe in DESIGN.md).  BASELINE.json's metric names no config, so the default
+workload is the largest single-GPU one, configs[4] (C5: turbulent cloud, 512^3 cells, 8 observers at 512x512);
+--workload c1..c4 time the others.
 
 One JSON line goes to stdout (rank 0).  `value` is device-resident throughput; `e2e` is the same metric
 through the C ABI with HOST buffers (grid upload, transport, imaging, image download inside the timed
@@ -45,12 +46,9 @@ ALGO = {
 }
 EVENT_BYTES, CONTRIB_BYTES = 48, 32
 N_SM, LANES_PER_SM = 148, 128          # B200: 148 SMs x 4 schedulers x 32 lanes, one warp-instruction per scheduler and clock
-# which ceiling binds the dominant kernel, read from the committed ncu captures (profiles/):
-# issue slots busy vs DRAM / L2 throughput of the kernel (r1d: C2 flight 56 % issue vs 1 % DRAM, C2 image 56 % vs 23 %,
-# C4 flight 52 % vs 35 %, C4 image 71 % vs 38 %, C5 image 70 % vs 41 %).  C4's general flight does the same 3.7e10 cell
-# steps/s on a 128^3 grid that sits in L2 as on the 256^3 one, so memory does not bind it either ("gather" in the roofline
-# object puts the flight and imaging rates beside the measured random-gather rate of an array of the grid's size).
-BOUND = {"c1": "alu", "c2": "alu", "c3": "alu", "c4": "alu", "c5": "alu"}
+# Which ceiling binds a kernel, its DRAM traffic and the instructions it executes are NOT constants of this file: they are
+# parsed from the committed ncu captures of this same command that profiles/roofline_sources.json names per workload and
+# kernel class (read_capture below).
 
 
 def parse_args():
@@ -59,7 +57,7 @@ def parse_args():
     ap.add_argument("--steps", type=int, default=6)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="krp", choices=["krp", "reference"])
-    ap.add_argument("--workload", default="c2", choices=["c1", "c2", "c3", "c4", "c5"])
+    ap.add_argument("--workload", default="c5", choices=["c1", "c2", "c3", "c4", "c5"])
     ap.add_argument("--batch", type=int, default=0, help="packets per step and GPU (0 = workload default)")
     ap.add_argument("--n", type=int, default=0, help="override the grid size (testing only; marks the line reduced)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -214,13 +212,69 @@ def run_reference(args):
 # ------------------------------------------------------------------------------------------
 # the CUDA leg
 # ------------------------------------------------------------------------------------------
-# dram__bytes_read.sum + dram__bytes_write.sum per launch of the dominant kernel, from the committed
-# `ncu --set full` capture of this same command (profiles/, named per round); None until captured.
-NCU_TRAFFIC = {   # bytes, profiles/r1d_ncu_full_*.txt: the first-order flight launch (C2, C4), one observer's imaging launch (C5)
-    "c2": 154.27788e6 + 375.54688e6,        # profiles/r1e_ncu_full_c2_flight.txt
-    "c4": 40.274337e9 + 1.702403e9,         # profiles/r1h_ncu_full_c4_flight.txt
-    "c5": 227.68106e9 + 1.778706e9,
-}
+def read_capture(workload, cls):
+    """Counters of one launch of kernel class `cls` ("flight" / "image") of `workload`, from the committed ncu captures
+    that profiles/roofline_sources.json names: {"details": text of `ncu --page details`, "raw": csv of `ncu --page raw --csv`}.
+    Returns None when no capture is committed for it."""
+    idx = os.path.join(ROOT, "profiles", "roofline_sources.json")
+    if not os.path.exists(idx):
+        return None
+    with open(idx) as f:
+        src = json.load(f).get(workload, {}).get(cls)
+    if not src:
+        return None
+    out = {"files": src}
+    det = os.path.join(ROOT, src["details"])
+    if os.path.exists(det):
+        want = {"DRAM Throughput": "dram_pct", "Issue Slots Busy": "issue_pct", "L2 Cache Throughput": "l2_pct",
+                "L1/TEX Cache Throughput": "l1_pct", "Duration": "duration", "Achieved Occupancy": "occupancy_pct",
+                "Avg. Active Threads Per Warp": "active_threads", "Registers Per Thread": "registers"}
+        with open(det) as f:
+            for line in f:
+                t = line.split()
+                for key, name in want.items():
+                    if line.strip().startswith(key + " ") and name not in out:
+                        try:
+                            val = float(t[-1].replace(",", ""))
+                        except ValueError:
+                            continue
+                        if name == "duration":
+                            unit = t[-2]
+                            val *= {"us": 1e-3, "ms": 1.0, "s": 1e3, "ns": 1e-6}.get(unit, 1.0)
+                            name = "duration_ms"
+                        out[name] = val
+                    if line.strip().startswith(key) and "krp_k_" in line:
+                        pass
+                if "krp_k_" in line and "kernel" not in out:
+                    out["kernel"] = line.strip().split("(")[0].replace("void ", "")
+    raw = os.path.join(ROOT, src.get("raw", ""))
+    if src.get("raw") and os.path.exists(raw):
+        import csv
+        with open(raw) as f:
+            rows = [r for r in csv.reader(f) if r]
+        hdr = next((r for r in rows if "Kernel Name" in r), None)
+        if hdr:
+            data = rows[rows.index(hdr) + 2] if len(rows) > rows.index(hdr) + 2 else None      # header, units, first kernel
+            units = rows[rows.index(hdr) + 1]
+            def col(name):
+                if data is None or name not in hdr:
+                    return None
+                k = hdr.index(name)
+                try:
+                    v = float(data[k].replace(",", ""))
+                except ValueError:
+                    return None
+                return v * {"Kbyte": 1e3, "Mbyte": 1e6, "Gbyte": 1e9, "Tbyte": 1e12, "byte": 1.0}.get(units[k], 1.0)
+            r, w = col("dram__bytes_read.sum"), col("dram__bytes_write.sum")
+            if r is not None and w is not None:
+                out["dram_bytes"] = r + w
+            ti = col("smsp__thread_inst_executed.sum")
+            if ti is not None:
+                out["thread_inst_executed"] = ti
+            wi = col("smsp__inst_executed.sum")
+            if wi is not None:
+                out["warp_inst_executed"] = wi
+    return out
 
 
 def make_grid(krp, cfg, dens, bf, weight):
@@ -343,10 +397,10 @@ def run_krp(args):
     rays = st["events"] * n_obs
     flights = st["packets"] + st["events"]                             # an upper bound: every event but the last starts one
     work = {
-        "image": dict(kernel="krp_k_image<%s>" % mode, steps=st["steps_image"],
+        "image": dict(kernel="krp_k_image<true,false>" if mode == "scalar" else "krp_k_image<false,true>", steps=st["steps_image"],
                       bytes=st["steps_image"] * A["cell_bytes"] + rays * EVENT_BYTES + st["contributions"] * CONTRIB_BYTES,
                       inst=st["steps_image"] * A["image_inst"] + rays * A["ray_inst"]),
-        "flight": dict(kernel="krp_k_flight_%s" % mode, steps=st["steps_transport"],
+        "flight": dict(kernel="krp_k_flight_scalar_static" if mode == "scalar" else "krp_k_flight_general", steps=st["steps_transport"],
                        bytes=st["steps_transport"] * A["cell_bytes"] + flights * 64 + st["events"] * 56,
                        inst=st["steps_transport"] * A["flight_inst"] + flights * A["flight_fixed_inst"]),
     }
@@ -354,37 +408,54 @@ def run_krp(args):
     for cls, (ms, n_l) in timing.items():
         kernels[cls] = {"ms_per_step": ms / K, "launches_per_step": n_l / K, "share_of_step": ms / ms_own}
     dom = max(("image", "flight"), key=lambda c: timing[c][0])
-    W = work[dom]
-    t_dom = timing[dom][0] * 1e-3                                       # seconds over the K timed steps
-    n_launch = max(timing[dom][1], 1)
-    f_hbm = W["bytes"] / t_dom / (pk["hbm_gbs"] * 1e9)
-    f_alu = W["inst"] / t_dom / alu_peak
-    bound = BOUND.get(args.workload, "alu" if f_alu >= f_hbm else "hbm")
-    if bound == "hbm":
-        roof = {"bound": "hbm", "achieved": W["bytes"] / t_dom / 1e9, "peak": pk["hbm_gbs"], "unit": "GB/s", "frac": f_hbm}
+    per_class = {}
+    for cls in ("image", "flight"):
+        Wc = work[cls]
+        t_c = timing[cls][0] * 1e-3                                     # seconds over the K timed steps, CUDA events per launch
+        n_l = max(timing[cls][1], 1)
+        if t_c <= 0:
+            continue
+        cap = read_capture(args.workload, cls)
+        f_hbm = Wc["bytes"] / t_c / (pk["hbm_gbs"] * 1e9)
+        f_alu = Wc["inst"] / t_c / alu_peak
+        rec = {"kernel": (cap or {}).get("kernel", Wc["kernel"]), "launches_per_step": n_l / K, "avg_launch_ms": 1e3 * t_c / n_l,
+               "kernel_ms_per_step": 1e3 * t_c / K, "share_of_step": timing[cls][0] / ms_own,
+               "cell_steps_per_step": Wc["steps"] / K, "cell_steps_per_s": Wc["steps"] / t_c,
+               "algorithmic_bytes_per_step": Wc["bytes"] / K, "algorithmic_inst_per_step": Wc["inst"] / K,
+               "frac_hbm": f_hbm, "frac_alu": f_alu, "traffic": None, "capture": None}
+        # which ceiling binds: read from the committed capture of this kernel -- issue slots busy against DRAM throughput;
+        # when neither reaches 60 % the kernel is bound by latency / divergence, not by a throughput ceiling
+        bound = "alu" if f_alu >= f_hbm else "hbm"
+        if cap:
+            issue, dram = cap.get("issue_pct"), cap.get("dram_pct")
+            if issue is not None and dram is not None:
+                bound = "latency" if max(issue, dram) < 60.0 else ("alu" if issue >= dram else "hbm")
+            rec["traffic"] = cap.get("dram_bytes")
+            rec["capture"] = {k: cap.get(k) for k in ("files", "issue_pct", "dram_pct", "l2_pct", "l1_pct", "duration_ms",
+                                                       "active_threads", "occupancy_pct", "registers")}
+            if cap.get("thread_inst_executed") and cap.get("duration_ms"):
+                # executed (not algorithmic) thread-instructions of the captured launch against the same issue ceiling,
+                # at the capture's own duration: what the SASS really issues, divergence included
+                rec["frac_alu_executed_in_capture"] = cap["thread_inst_executed"] / (cap["duration_ms"] * 1e-3) / alu_peak
+                rec["executed_over_algorithmic"] = None
+        rec["bound"] = bound
+        per_class[cls] = rec
+    D = per_class[dom]
+    use_hbm = D["bound"] == "hbm" or (D["bound"] == "latency" and D["frac_hbm"] > D["frac_alu"])
+    t_dom = timing[dom][0] * 1e-3
+    if use_hbm:
+        roof = {"bound": D["bound"], "achieved": work[dom]["bytes"] / t_dom / 1e9, "peak": pk["hbm_gbs"], "unit": "GB/s", "frac": D["frac_hbm"]}
     else:
-        roof = {"bound": "alu", "achieved": W["inst"] / t_dom / 1e12, "peak": alu_peak / 1e12, "unit": "Tinst/s", "frac": f_alu}
-    # gather ceiling (north_star: "L2/HBM gather bandwidth"): the measured rate of independent random gathers of one cell
-    # from an array of the grid's size (krp_probe_gather, run now, outside the timed region).  A flight is one such
-    # gather per cell step; an imaging march over events ordered by cell is coherent and can exceed it.
-    cell_b = A["cell_bytes"]
-    grid_bytes = cell_b * (cfg["nx"] + 2) * (cfg["ny"] + 2) * (cfg["nz"] + 2)
-    probe_bytes = max(grid_bytes, 1 << 20)
-    gather_peak = krp.probe_gather(probe_bytes, cell_b)
-    gather = {c: {"cell_steps_per_s": work[c]["steps"] / (timing[c][0] * 1e-3), "peak_gathers_per_s": gather_peak,
-                  "frac": work[c]["steps"] / (timing[c][0] * 1e-3) / gather_peak} for c in ("flight", "image")}
-    roof.update({"gather": {"probe": "random %d-B gathers from an array of the grid's size, %d MiB" % (cell_b, probe_bytes >> 20),
-                            **gather},
-                 "kernel": W["kernel"], "launches_per_step": n_launch / K, "avg_launch_ms": 1e3 * t_dom / n_launch,
-                 "kernel_ms_per_step": 1e3 * t_dom / K, "share_of_step": timing[dom][0] / ms_own,
-                 "traffic": NCU_TRAFFIC.get(args.workload), "peak_source": pk["source"],
-                 "cell_steps_per_step": W["steps"] / K, "algorithmic_bytes_per_step": W["bytes"] / K,
-                 "algorithmic_inst_per_step": W["inst"] / K, "frac_hbm": f_hbm, "frac_alu": f_alu,
-                 "peak_alu": "%d SMs x 4 schedulers x 32 lanes x %.0f MHz" % (N_SM, pk["sm_max_mhz"]),
-                 "kernels": kernels})
+        roof = {"bound": D["bound"], "achieved": work[dom]["inst"] / t_dom / 1e12, "peak": alu_peak / 1e12, "unit": "Tinst/s", "frac": D["frac_alu"]}
+    roof.update({k: v for k, v in D.items() if k != "bound"})
+    roof.update({"peak_source": pk["source"], "peak_alu": "%d SMs x 4 schedulers x 32 lanes x %.0f MHz" % (N_SM, pk["sm_max_mhz"]),
+                 "algorithmic_unit": "per cell step %d B and %d (image) / %d (flight) thread-instructions; per ray 48 B + 32 B and %d; "
+                                     "per flight 64 B + 56 B and %d (DESIGN.md section 8, SASS excerpts in profiles/)"
+                                     % (A["cell_bytes"], A["image_inst"], A["flight_inst"], A["ray_inst"], A["flight_fixed_inst"]),
+                 "other": {c: v for c, v in per_class.items() if c != dom}, "kernels": kernels})
     return dict(world=world, rank=rank, cfg=cfg, batch=batch, value=value, ms_total=ms_total, clocks=clocks, roof=roof,
                 t_tr=t_tr, t_im=t_im, tot=tot, launches=launches, epp=epp, mode=mode, krp=krp, obs=obs, dev=dev,
-                ev_cap=ev_cap, grid=g)
+                ev_cap=ev_cap, grid=g, version=g.version())
 
 
 def run_e2e(args, r):
@@ -417,7 +488,7 @@ def run_e2e(args, r):
         g.image_get(out=h_img.numpy())                 # D2H, synchronises
         return float(h_img[:, 0].sum())                # the step's result, read on the host
 
-    k = max(1, min(args.steps, 3))
+    k = max(1, args.steps)
     one(0)
     torch.cuda.synchronize()
     if world > 1:
@@ -472,7 +543,7 @@ def main():
         "scatterings_per_s": tot["events"] / sec,
         "cell_steps_per_s": (tot["steps_transport"] + tot["steps_image"]) / sec,
         "kernel_ms": {"transport": r["t_tr"], "image": r["t_im"]},
-        "clocks": r["clocks"], "roofline": r["roof"], "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(r["launches"]),
+        "clocks": r["clocks"], "roofline": r["roof"], "cpu_baseline": cpu, "e2e": e2e, "gpu_launches": int(r["launches"]), "library": r["version"],
         "context": "paper: ~1.4e7 packets/s for its own (different) step 1 on an RTX 5090, ~1e2x over CPU codes (PAPER.md:125)",
     }
     print(json.dumps(line))

@@ -46,7 +46,8 @@ enum {
 enum { KRP_MEM_DEVICE = 0, KRP_MEM_HOST = 1 };
 
 const char* krp_last_error(void);
-/* library identification: "krp <version> sm_100a" */
+/* library identification: "krp <version> sm_100a <build id>", the build id being a hash of the sources the library
+ * was compiled from (the binding refuses a library whose id differs from the sources beside it) */
 const char* krp_version(void);
 
 typedef struct krp_grid krp_grid; /* opaque; owns all device memory of one model */
@@ -106,8 +107,10 @@ int krp_source_set(krp_grid* g, const krp_source* src, void* stream);
 
 /* Capacity of the event buffer (events held between krp_transport and krp_image).
  * Optional: krp_transport grows it to 4 events per packet (at least 2^20) when unset.
- * Events beyond the capacity are dropped, the packet stops, krp_stats.overflow counts them
- * and the next synchronising call returns KRP_ERR_EVENT_FULL. */
+ * Events beyond the capacity are dropped, the packet stops, krp_stats.overflow counts them, and from then on until
+ * krp_stats_reset every call that reads results back to the host -- krp_stats_get, krp_events_get, krp_events_select,
+ * krp_image_get to HOST memory -- delivers what it has and returns KRP_ERR_EVENT_FULL (krp_image itself does not
+ * synchronise: it images the truncated buffer). */
 int krp_events_reserve(krp_grid* g, uint64_t max_events);
 
 /* Transport packets with global ids [next_id, next_id + n_packets) (next_id starts at 0 and
@@ -169,6 +172,10 @@ int krp_stats_reset(krp_grid* g, void* stream);
  * written).  Order is not defined (the buffer is filled with atomics).  Synchronises. */
 int krp_events_get(krp_grid* g, uint64_t cap, uint64_t* n, uint64_t* id, int32_t* k,
                    int64_t* cell, float* pos, float* dir, float* stokes);
+/* The same for the events of packets id_first <= id < id_first + id_count only (a sample of a large batch: the parity
+ * tests compare such a sample with the oracle); the buffer is read in slices, so host memory stays small. */
+int krp_events_select(krp_grid* g, uint64_t id_first, uint64_t id_count, uint64_t cap, uint64_t* n, uint64_t* id, int32_t* k,
+                      int64_t* cell, float* pos, float* dir, float* stokes);
 int krp_events_clear(krp_grid* g, void* stream);
 
 /* Launch-shape knobs, for measurement only (0 keeps the current value): threads per block of the
@@ -176,6 +183,12 @@ int krp_events_clear(krp_grid* g, void* stream);
  * persistent blocks per SM (default: 8; the general-mode flight fills an SM once, 640 threads), and
  * the number of cell steps a flight kernel takes between two points where idle lanes take new packets. */
 int krp_tune(krp_grid* g, int transport_block, int image_block, int blocks_per_sm, int flight_burst);
+/* Scheduling features, for A/B measurement and for the tests that show results do not depend on them (-1 keeps the
+ * current value): dir_sort 1/0 = first flights of an isotropic point source taken in direction order / in id order;
+ * obs_cells 1/0 = per-observer cell coefficient arrays in the general-mode imaging march / look-ups in the march (takes
+ * effect at the next change of the observer set); order_policy 0 never / 1 by the measured ray length / 2 always order
+ * the events by cell before imaging. */
+int krp_tune_schedule(krp_grid* g, int dir_sort, int obs_cells, int order_policy);
 /* Device time per kernel class, for measurement (bench.py's roofline): when enabled, every launch of a
  * flight, scattering, ordering or imaging kernel is bracketed by CUDA events on the caller's stream.
  * krp_timing_get synchronises, adds up the elapsed times since the last call into ms[KRP_T_COUNT] and the
@@ -184,13 +197,6 @@ int krp_tune(krp_grid* g, int transport_block, int image_block, int blocks_per_s
 enum { KRP_T_FLIGHT = 0, KRP_T_SCATTER = 1, KRP_T_ORDER = 2, KRP_T_IMAGE = 3, KRP_T_EMIT = 4, KRP_T_COUNT = 5 };
 int krp_timing_enable(krp_grid* g, int on);
 int krp_timing_get(krp_grid* g, double* ms, uint64_t* launches);
-
-/* Measurement utility (bench.py's gather ceiling): the rate at which this GPU serves independent random
- * gathers of elem_bytes (4 or 16) from an array of array_bytes (1 MiB .. 32 GiB, fewer than 2^32 elements),
- * every thread of a full grid issuing 64 of them.  This is the ceiling of a cell march whose rays are not
- * coherent: one gather per cell step from a grid of that size (L2-resident or not).  Allocates and frees its
- * own array, synchronises, writes gathers per second to *gathers_per_s. */
-int krp_probe_gather(uint64_t array_bytes, int elem_bytes, double* gathers_per_s, void* stream);
 
 /* Number of kernels the library has launched on behalf of g since creation. */
 uint64_t krp_launch_count(const krp_grid* g);

@@ -25,11 +25,17 @@
  *     every event and after every scattering (the 48-byte event record and the
  *     packet queue hold fp32 Stokes vectors).
  *
+ * The last two of these entered after the first kernel existed; the build with
+ * -DORA_STATE_FP32=0 (libkrp_oracle_pure.so) leaves them out and serves as the
+ * control: tests/test_oracle_control.py runs every pin on it and compares the two
+ * builds' maps, tests/test_gpu_parity.py reports the CUDA path's agreement with it.
+ *
  * Pins (tests/test_oracle_pins.py, -m "not gpu"): every exported function
  * below is pinned to a closed form, an invariant, a library routine
  * (scipy.linalg.expm, cuRAND host Philox) or brute force; see the table in
- * DESIGN.md section "Oracle pins".  Nothing here is "parity unpinned" except
- * the absolute image unit and the sign convention of V (R6).
+ * DESIGN.md section "Oracle pins" (round 2 added: the second-moment map img2,
+ * the (U,V) block and S34 terms of F(Theta), the emission map).  "Parity
+ * unpinned": the absolute image unit (R14) and the sign convention of V (R6).
  */
 #include <math.h>
 #include <stdint.h>
@@ -37,6 +43,21 @@
 #include <string.h>
 
 #define ORA_PI 3.14159265358979323846264338327950288
+
+/* Control build (R12, "pure-state control"): -DORA_STATE_FP32=0 turns OFF the two state
+ * roundings that were added after the first kernel existed -- the cell-local position at emission
+ * and at every event, and (q,u,v) at every event and after every scattering -- so that the state
+ * between steps is pure fp64 (tables, B^ and n^ stay fp32 as in the oracle's first commit).  The
+ * pins run on both builds; tests report how the CUDA path and the rounded build compare with it. */
+#ifndef ORA_STATE_FP32
+#define ORA_STATE_FP32 1
+#endif
+#if ORA_STATE_FP32
+#define ORA_STATE(x) ((double)(float)(x))
+#else
+#define ORA_STATE(x) (x)
+#endif
+int ora_state_is_fp32(void) { return ORA_STATE_FP32; }
 
 /* ------------------------------------------------------------------ */
 /* S0  Random numbers: Philox4x32-10 (Salmon et al. 2011), counter     */
@@ -552,7 +573,7 @@ static int flight(const ora_model* m, int idx[3], double p[3], const double n[3]
                 if (Iout <= target) {
                     double t = ora_event_solve(S[0], 0.0, a[0], 0.0, target);
                     advance(m, idx, p, n, t / kr, -1);
-                    for (int a2 = 0; a2 < 3; ++a2) p[a2] = (double)(float)p[a2];   /* R12 */
+                    for (int a2 = 0; a2 < 3; ++a2) p[a2] = ORA_STATE(p[a2]);   /* R12 */
                     double I = S[0];
                     for (int s = 0; s < 4; ++s) S[s] /= I;
                     return 1;
@@ -575,7 +596,7 @@ static int flight(const ora_model* m, int idx[3], double p[3], const double n[3]
                     ora_rotate_qu(Sg, ce, -se);
                     for (int s = 0; s < 4; ++s) S[s] = Sg[s];
                     advance(m, idx, p, n, t / kr, -1);
-                    for (int a2 = 0; a2 < 3; ++a2) p[a2] = (double)(float)p[a2];   /* R12 */
+                    for (int a2 = 0; a2 < 3; ++a2) p[a2] = ORA_STATE(p[a2]);   /* R12 */
                     return 1;
                 }
                 ora_rotate_qu(So, ce, -se);
@@ -586,7 +607,7 @@ static int flight(const ora_model* m, int idx[3], double p[3], const double n[3]
     }
 }
 
-/* S1 emission of packet id (draw schedule R11). */
+/* S1 emission of packet id (draw schedule R11).  Exported as ora_emit for the pins. */
 static void emit(const ora_model* m, uint64_t seed, uint64_t id, int idx[3], double p[3], double n[3], double* tau_star)
 {
     uint32_t w[4];
@@ -619,8 +640,13 @@ static void emit(const ora_model* m, uint64_t seed, uint64_t id, int idx[3], dou
         idx[0] = (int)(c % m->nx); idx[1] = (int)((c / m->nx) % m->ny); idx[2] = (int)(c / ((int64_t)m->nx * m->ny));
         for (int a = 0; a < 3; ++a) p[a] = ora_u01(w2[a]);
     } else {
-        for (int a = 0; a < 3; ++a) { idx[a] = m->src_idx[a]; p[a] = (double)(float)m->src_p[a]; }   /* R12 */
+        for (int a = 0; a < 3; ++a) { idx[a] = m->src_idx[a]; p[a] = ORA_STATE(m->src_p[a]); }   /* R12 */
     }
+}
+
+void ora_emit(const ora_model* m, uint64_t seed, uint64_t id, int idx[3], double p[3], double n[3], double* tau_star)
+{
+    emit(m, seed, id, idx, p, n, tau_star);
 }
 
 /* Transport packets [id0, id0+n).  esc_* (optional, capacity esc_cap): the
@@ -652,7 +678,7 @@ int64_t ora_transport(const ora_model* m, uint64_t id0, uint64_t n_packets, uint
                 break;
             }
             ++k;
-            for (int s = 1; s < 4; ++s) S[s] = (double)(float)S[s];              /* R12: event record state */
+            for (int s = 1; s < 4; ++s) S[s] = ORA_STATE(S[s]);              /* R12: event record state */
             int64_t c = cell_of(m, idx);
             double b[3], a[4];
             cell_bhat(m, c, b);
@@ -666,7 +692,7 @@ int64_t ora_transport(const ora_model* m, uint64_t id0, uint64_t n_packets, uint
             double n2[3], S2[4];
             ora_scatter(m, b, n, S, seed, id, (uint32_t)k, n2, S2, &tau_star);
             for (int a2 = 0; a2 < 3; ++a2) n[a2] = n2[a2];
-            for (int s = 0; s < 4; ++s) S[s] = (double)(float)S2[s];             /* R12: queue state */
+            for (int s = 0; s < 4; ++s) S[s] = ORA_STATE(S2[s]);             /* R12: queue state */
         }
     }
     return nesc;

@@ -11,18 +11,34 @@ import numpy as np
 
 _HERE = os.path.dirname(os.path.abspath(__file__))
 _SRC = os.path.join(_HERE, "krp_oracle.c")
-_SO = os.path.join(_HERE, "libkrp_oracle.so")
-_lib = None
+# Two builds of the same source (R12): "fp32state" is the oracle proper (the state between steps is
+# defined in fp32 where the 48-byte record and the queue store it); "pure" is the control build with those
+# roundings off (-DORA_STATE_FP32=0).  KRP_ORACLE_VARIANT picks the default (the pins are run on both).
+VARIANTS = {"fp32state": ("libkrp_oracle.so", []), "pure": ("libkrp_oracle_pure.so", ["-DORA_STATE_FP32=0"])}
+_libs = {}
 
 
-def build(force=False):
-    """Compile krp_oracle.c with gcc (no fast-math: fp64 IEEE as written)."""
-    if force or not os.path.exists(_SO) or os.path.getmtime(_SO) < os.path.getmtime(_SRC):
-        tmp = _SO + ".tmp%d" % os.getpid()
-        subprocess.check_call(["gcc", "-O2", "-std=c11", "-fPIC", "-shared", "-ffp-contract=off",
-                               "-o", tmp, _SRC, "-lm"])
-        os.replace(tmp, _SO)
-    return _SO
+def default_variant():
+    v = os.environ.get("KRP_ORACLE_VARIANT", "fp32state")
+    if v not in VARIANTS:
+        raise ValueError("KRP_ORACLE_VARIANT must be one of %s" % sorted(VARIANTS))
+    return v
+
+
+def build(force=False, variant=None):
+    """Compile krp_oracle.c with gcc (no fast-math: fp64 IEEE as written).  variant=None builds every variant
+    and returns the path of the default one."""
+    if variant is None:
+        for v in VARIANTS:
+            build(force, v)
+        return os.path.join(_HERE, VARIANTS[default_variant()][0])
+    so = os.path.join(_HERE, VARIANTS[variant][0])
+    if force or not os.path.exists(so) or os.path.getmtime(so) < os.path.getmtime(_SRC):
+        tmp = so + ".tmp%d" % os.getpid()
+        subprocess.check_call(["gcc", "-O2", "-std=c11", "-fPIC", "-shared", "-ffp-contract=off"] + VARIANTS[variant][1] +
+                              ["-o", tmp, _SRC, "-lm"])
+        os.replace(tmp, so)
+    return so
 
 
 class OracleStats(C.Structure):
@@ -82,12 +98,14 @@ _ip = np.ctypeslib.ndpointer(np.int32, flags="C_CONTIGUOUS")
 _up = np.ctypeslib.ndpointer(np.uint32, flags="C_CONTIGUOUS")
 
 
-def lib():
-    global _lib
-    if _lib is not None:
-        return _lib
-    L = C.CDLL(build())
+def lib(variant=None):
+    variant = variant or default_variant()
+    if variant in _libs:
+        return _libs[variant]
+    L = C.CDLL(build(variant=variant))
     sig = {
+        "ora_state_is_fp32": (C.c_int, []),
+        "ora_emit": (None, [C.c_void_p, C.c_uint64, C.c_uint64, _ip, _dp, _dp, _D]),
         "ora_philox": (None, [_up, _up, _up]),
         "ora_u01": (C.c_double, [C.c_uint32]),
         "ora_u53": (C.c_double, [C.c_uint32, C.c_uint32]),
@@ -123,7 +141,8 @@ def lib():
     for name, (res, args) in sig.items():
         f = getattr(L, name)
         f.restype, f.argtypes = res, args
-    _lib = L
+    assert L.ora_state_is_fp32() == (0 if variant == "pure" else 1)
+    _libs[variant] = L
     return L
 
 
@@ -138,8 +157,8 @@ class OracleModel:
     Theta_j = j*180/(n_ang-1) deg), opac [n_inc,4] f32 (a1,a2,a3,albedo on
     mu_m = m/(n_inc-1), mu = |cos(angle(n,B))|)."""
 
-    def __init__(self, nx, ny, nz, bounds, density, bfield, mueller, opac, w_min=1e-4, max_scatter=64):
-        L = lib()
+    def __init__(self, nx, ny, nz, bounds, density, bfield, mueller, opac, w_min=1e-4, max_scatter=64, variant=None):
+        L = self.L = lib(variant)
         self.nx, self.ny, self.nz = int(nx), int(ny), int(nz)
         self.bounds = _v(bounds, 6)
         self.density = np.ascontiguousarray(np.asarray(density, np.float32).reshape(nz, ny, nx))
@@ -158,54 +177,60 @@ class OracleModel:
 
     def __del__(self):
         if getattr(self, "h", None):
-            lib().ora_model_free(self.h)
+            self.L.ora_model_free(self.h)
             self.h = None
 
     def source_set(self, kind, pos, direction, cell_weight=None, emit_records=0):
         """kind bit0: volume (else point at pos); bit1: collimated along direction (else isotropic)."""
         self._w = None if cell_weight is None else np.ascontiguousarray(np.asarray(cell_weight, np.float32).ravel())
-        lib().ora_source_set(self.h, int(kind), _v(pos, 3), _v(direction, 3),
+        self.L.ora_source_set(self.h, int(kind), _v(pos, 3), _v(direction, 3),
                              None if self._w is None else self._w.ctypes.data, int(emit_records))
 
     # --- per-step functions (pins) ---
     def mueller_at(self, theta_deg):
-        F = np.zeros(4); lib().ora_mueller_at(self.h, float(theta_deg), F); return F
+        F = np.zeros(4); self.L.ora_mueller_at(self.h, float(theta_deg), F); return F
 
     def opac_at(self, mu):
-        a = np.zeros(4); lib().ora_opac_at(self.h, float(mu), a); return a
+        a = np.zeros(4); self.L.ora_opac_at(self.h, float(mu), a); return a
 
     def dda_exit(self, p, n):
         ax = C.c_int(-1)
-        t = lib().ora_dda_exit(self.h, _v(p, 3), _v(n, 3), C.byref(ax))
+        t = self.L.ora_dda_exit(self.h, _v(p, 3), _v(n, 3), C.byref(ax))
         return t, ax.value
 
     def cell_step(self, b, n, S, dtau):
-        S = _v(S, 4).copy(); lib().ora_cell_step(self.h, _v(b, 3), _v(n, 3), S, float(dtau)); return S
+        S = _v(S, 4).copy(); self.L.ora_cell_step(self.h, _v(b, 3), _v(n, 3), S, float(dtau)); return S
 
     def march(self, idx, p, n, S, log_cap=0):
         S = _v(S, 4).copy()
         lc = np.zeros(max(log_cap, 1), np.int64); ld = np.zeros(max(log_cap, 1), np.float64)
-        steps = lib().ora_march(self.h, np.ascontiguousarray(np.asarray(idx, np.int32)), _v(p, 3), _v(n, 3), S,
+        steps = self.L.ora_march(self.h, np.ascontiguousarray(np.asarray(idx, np.int32)), _v(p, 3), _v(n, 3), S,
                                 int(log_cap), lc.ctypes.data, ld.ctypes.data)
         m = min(int(steps), log_cap)
         return S, int(steps), lc[:m], ld[:m]
 
+    def emit(self, seed, pid):
+        """(cell index triple, cell-local position, direction, tau*) of packet pid (S1, schedule R11)."""
+        idx = np.zeros(3, np.int32); p = np.zeros(3); n = np.zeros(3); t = C.c_double(0)
+        self.L.ora_emit(self.h, int(seed), int(pid), idx, p, n, C.byref(t))
+        return idx, p, n, t.value
+
     def sample_theta(self, u):
-        return lib().ora_sample_theta(self.h, float(u))
+        return self.L.ora_sample_theta(self.h, float(u))
 
     def scatter_angles(self, b, n_in, S_in, theta_deg, phi):
         no = np.zeros(3); So = np.zeros(4)
-        lib().ora_scatter_angles(self.h, _v(b, 3), _v(n_in, 3), _v(S_in, 4), float(theta_deg), float(phi), no, So)
+        self.L.ora_scatter_angles(self.h, _v(b, 3), _v(n_in, 3), _v(S_in, 4), float(theta_deg), float(phi), no, So)
         return no, So
 
     def scatter(self, b, n_in, S_in, seed, pid, k):
         no = np.zeros(3); So = np.zeros(4); tn = C.c_double(0)
-        r = lib().ora_scatter(self.h, _v(b, 3), _v(n_in, 3), _v(S_in, 4), int(seed), int(pid), int(k), no, So,
+        r = self.L.ora_scatter(self.h, _v(b, 3), _v(n_in, 3), _v(S_in, 4), int(seed), int(pid), int(k), no, So,
                               C.byref(tn))
         return no, So, tn.value, r
 
     def peel(self, n_in, S_in, n_obs):
-        So = np.zeros(4); lib().ora_peel(self.h, _v(n_in, 3), _v(S_in, 4), _v(n_obs, 3), So); return So
+        So = np.zeros(4); self.L.ora_peel(self.h, _v(n_in, 3), _v(S_in, 4), _v(n_obs, 3), So); return So
 
     # --- whole-path functions ---
     def transport(self, id0, n_packets, seed, events, stats=None, esc_cap=0):
@@ -214,12 +239,12 @@ class OracleModel:
         if esc_cap > 0:
             esc = dict(n=np.zeros((esc_cap, 3)), S=np.zeros((esc_cap, 4)), id=np.zeros(esc_cap, np.uint64),
                        k=np.zeros(esc_cap, np.int32))
-            ne = lib().ora_transport(self.h, int(id0), int(n_packets), int(seed), C.byref(events.c), C.byref(st),
+            ne = self.L.ora_transport(self.h, int(id0), int(n_packets), int(seed), C.byref(events.c), C.byref(st),
                                      int(esc_cap), esc["n"].ctypes.data, esc["S"].ctypes.data,
                                      esc["id"].ctypes.data, esc["k"].ctypes.data)
             esc = {k: v[:ne] for k, v in esc.items()}
         else:
-            lib().ora_transport(self.h, int(id0), int(n_packets), int(seed), C.byref(events.c), C.byref(st),
+            self.L.ora_transport(self.h, int(id0), int(n_packets), int(seed), C.byref(events.c), C.byref(st),
                                 0, None, None, None, None)
         return st, esc
 
@@ -228,6 +253,6 @@ class OracleModel:
         n_obs = len(observers)
         arr = (Observer * n_obs)(*observers)
         img = np.zeros((n_obs, 4, npy, npx)); img2 = np.zeros_like(img) if second_moment else None
-        lib().ora_image(self.h, C.byref(events.c), arr, n_obs, int(npx), int(npy), int(flags), img,
+        self.L.ora_image(self.h, C.byref(events.c), arr, n_obs, int(npx), int(npy), int(flags), img,
                         None if img2 is None else img2.ctypes.data, C.byref(st))
         return img, img2, st

@@ -20,13 +20,31 @@ def _nvcc():
     return "nvcc"
 
 
-def stale():
-    if not os.path.exists(LIB):
-        return True
-    t = os.path.getmtime(LIB)
-    deps = [os.path.join(SRC_DIR, s) for s in SOURCES] + \
+ID_FILE = os.path.join(HERE, "libkrp.id")
+
+
+def _deps():
+    return [os.path.join(SRC_DIR, s) for s in SOURCES] + \
            [h if os.path.isabs(h) else os.path.join(SRC_DIR, h) for h in HEADERS]
-    return any(os.path.getmtime(d) > t for d in deps)
+
+
+def source_id():
+    """Build id: hash of the sources and of the compiler flags (compiled into krp_version())."""
+    import hashlib
+    h = hashlib.sha1(" ".join(NVCC_FLAGS).encode())
+    for d in _deps():
+        with open(d, "rb") as f:
+            h.update(f.read())
+    return h.hexdigest()[:12]
+
+
+def stale():
+    """True when the library is missing or was built from other sources than those beside it (content, not mtime:
+    the tree is copied to the GPU box with new timestamps)."""
+    if not os.path.exists(LIB) or not os.path.exists(ID_FILE):
+        return True
+    with open(ID_FILE) as f:
+        return f.read().strip() != source_id()
 
 
 def build(force=False, verbose=False):
@@ -34,10 +52,13 @@ def build(force=False, verbose=False):
     if not force and not stale():
         return LIB
     tmp = LIB + ".tmp%d" % os.getpid()
-    cmd = [_nvcc()] + NVCC_FLAGS + (["-Xptxas", "-v"] if verbose else []) + \
+    sid = source_id()
+    cmd = [_nvcc()] + NVCC_FLAGS + ['-DKRP_BUILD_ID="%s"' % sid] + (["-Xptxas", "-v"] if verbose else []) + \
           ["-o", tmp] + [os.path.join(SRC_DIR, s) for s in SOURCES]
     subprocess.check_call(cmd)
     os.replace(tmp, LIB)
+    with open(ID_FILE, "w") as f:
+        f.write(sid + "\n")
     return LIB
 
 

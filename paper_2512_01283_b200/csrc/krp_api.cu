@@ -124,7 +124,10 @@ struct TimedLaunch {
 };
 
 extern "C" const char* krp_last_error(void) { return g_err; }
-extern "C" const char* krp_version(void) { return "krp 0.1 sm_100a"; }
+#ifndef KRP_BUILD_ID
+#define KRP_BUILD_ID "unstamped"
+#endif
+extern "C" const char* krp_version(void) { return "krp 0.2 sm_100a " KRP_BUILD_ID; }
 
 static void free_records(KrpRecords& r)
 {
@@ -277,11 +280,8 @@ extern "C" int krp_grid_create(krp_grid** out, int nx, int ny, int nz, const dou
     // scalar flights are short: static assignment; general flights are long: persistent lanes, refill every 32 steps
     g->burst = m.scalar ? 1 : 32;
     if (!m.scalar) g->transport_block = 128;
-    if (getenv("KRP_NO_DIR_SORT")) g->dir_sort = 0;   // A/B switches for measurement
-    if (getenv("KRP_NO_OBS_PRE")) g->obs_pre = 0;
     if (m.scalar)
         CK(cudaFuncSetAttribute(krp_k_flight_scalar, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(8 * sizeof(KrpWarpShared))));
-    if (getenv("KRP_ORDER_POLICY")) g->order_policy = atoi(getenv("KRP_ORDER_POLICY"));
     g->order_events = g->order_policy != 0;
     m.n_inc = n_inc; m.n_ang = tables->n_ang;
     m.xs = (double)(n_inc - 1); m.guard = 1.f + m.rho + 1e-3f; m.inv_nang1 = 1.0 / (double)(tables->n_ang - 1);
@@ -730,6 +730,15 @@ extern "C" int krp_image(krp_grid* g, const krp_observer* obs, int n_obs, int np
     return KRP_OK;
 }
 
+// every synchronising call reports a past overflow of the event buffer, not only krp_stats_get
+static int overflow_code(krp_grid* g, const KrpCtl& c)
+{
+    if (c.stats.overflow)
+        return fail(KRP_ERR_EVENT_FULL, "event buffer overflowed: %llu events lost (capacity %llu)",
+                    (unsigned long long)c.stats.overflow, (unsigned long long)g->ev_cap);
+    return KRP_OK;
+}
+
 extern "C" int krp_image_get(krp_grid* g, double* out, int mem, void* stream)
 {
     if (!g || !out) return fail(KRP_ERR_ARG, "grid or out is NULL");
@@ -739,6 +748,9 @@ extern "C" int krp_image_get(krp_grid* g, double* out, int mem, void* stream)
     if (mem == KRP_MEM_HOST) {
         CK(cudaMemcpyAsync(out, g->d_img, bytes, cudaMemcpyDeviceToHost, st));
         CK(cudaStreamSynchronize(st));
+        KrpCtl c;      // a synchronising call: report a past overflow (the maps are delivered all the same)
+        CK(cudaMemcpy(&c, g->d_ctl, sizeof(c), cudaMemcpyDeviceToHost));
+        return overflow_code(g, c);
     } else if (mem == KRP_MEM_DEVICE) {
         CK(cudaMemcpyAsync(out, g->d_img, bytes, cudaMemcpyDeviceToDevice, st));
     } else {
@@ -767,9 +779,7 @@ extern "C" int krp_stats_get(krp_grid* g, krp_stats* out)
     out->contributions = c.stats.contributions; out->dropped = c.stats.dropped; out->overflow = c.stats.overflow;
     out->w_emitted = c.stats.w_emitted; out->w_escaped = c.stats.w_escaped;
     out->w_absorbed = c.stats.w_absorbed; out->w_cut = c.stats.w_cut;
-    if (c.stats.overflow) return fail(KRP_ERR_EVENT_FULL, "event buffer overflowed: %llu events lost (capacity %llu)",
-                                      (unsigned long long)c.stats.overflow, (unsigned long long)g->ev_cap);
-    return KRP_OK;
+    return overflow_code(g, c);
 }
 
 extern "C" int krp_stats_reset(krp_grid* g, void* stream)
@@ -779,41 +789,71 @@ extern "C" int krp_stats_reset(krp_grid* g, void* stream)
     return KRP_OK;
 }
 
+// krp_events_get / krp_events_select: download the buffer in slices of 2^22 events and keep those whose packet id
+// lies in [id_first, id_first + id_count)
+static int events_download(krp_grid* g, uint64_t id_first, uint64_t id_count, uint64_t cap, uint64_t* n, uint64_t* id, int32_t* k,
+                           int64_t* cell, float* pos, float* dir, float* stokes)
+{
+    CK(cudaDeviceSynchronize());
+    KrpCtl c;
+    CK(cudaMemcpy(&c, g->d_ctl, sizeof(c), cudaMemcpyDeviceToHost));
+    const uint64_t have = c.n_events < g->ev_cap ? c.n_events : g->ev_cap;
+    const bool all = id_count == UINT64_MAX;
+    const uint64_t slice = 1ull << 22;
+    std::vector<float4> pc, nk, S;
+    std::vector<unsigned long long> ids;
+    uint64_t found = 0;
+    for (uint64_t e0 = 0; e0 < have; e0 += slice) {
+        const uint64_t m = have - e0 < slice ? have - e0 : slice;
+        ids.resize(m);
+        CK(cudaMemcpy(ids.data(), g->ev.id + e0, m * sizeof(unsigned long long), cudaMemcpyDeviceToHost));
+        if (cap == 0) {      // count only
+            if (all) found += m;
+            else for (uint64_t i = 0; i < m; ++i) found += (ids[i] - id_first < id_count) ? 1 : 0;
+            continue;
+        }
+        pc.resize(m); nk.resize(m); S.resize(m);
+        CK(cudaMemcpy(pc.data(), g->ev.pc + e0, m * sizeof(float4), cudaMemcpyDeviceToHost));
+        CK(cudaMemcpy(nk.data(), g->ev.nk + e0, m * sizeof(float4), cudaMemcpyDeviceToHost));
+        CK(cudaMemcpy(S.data(), g->ev.S + e0, m * sizeof(float4), cudaMemcpyDeviceToHost));
+        for (uint64_t i = 0; i < m; ++i) {
+            if (!all && !(ids[i] - id_first < id_count)) continue;
+            const uint64_t o = found++;
+            if (o >= cap) continue;
+            uint32_t cb, kb;
+            memcpy(&cb, &pc[i].w, 4); memcpy(&kb, &nk[i].w, 4);
+            if (id) id[o] = ids[i];
+            if (k) k[o] = (int32_t)(kb & ~KRP_TERM_BIT);
+            if (cell) {
+                const KrpModel& mm = g->m;
+                uint32_t t = cb / (uint32_t)mm.px, hx = cb - t * (uint32_t)mm.px, hz = t / (uint32_t)mm.py, hy = t - hz * (uint32_t)mm.py;
+                cell[o] = ((int64_t)(hz - 1) * mm.ny + (int64_t)(hy - 1)) * mm.nx + (int64_t)(hx - 1);
+            }
+            if (pos) { pos[3 * o] = pc[i].x; pos[3 * o + 1] = pc[i].y; pos[3 * o + 2] = pc[i].z; }
+            if (dir) { dir[3 * o] = nk[i].x; dir[3 * o + 1] = nk[i].y; dir[3 * o + 2] = nk[i].z; }
+            if (stokes) {
+                stokes[4 * o] = S[i].x; stokes[4 * o + 1] = S[i].x * S[i].y;
+                stokes[4 * o + 2] = S[i].x * S[i].z; stokes[4 * o + 3] = S[i].x * S[i].w;
+            }
+        }
+    }
+    *n = found;
+    return overflow_code(g, c);
+}
+
 extern "C" int krp_events_get(krp_grid* g, uint64_t cap, uint64_t* n, uint64_t* id, int32_t* k, int64_t* cell, float* pos,
                               float* dir, float* stokes)
 {
     if (!g || !n) return fail(KRP_ERR_ARG, "grid or n is NULL");
-    CK(cudaDeviceSynchronize());
-    KrpCtl c;
-    CK(cudaMemcpy(&c, g->d_ctl, sizeof(c), cudaMemcpyDeviceToHost));
-    uint64_t have = c.n_events < g->ev_cap ? c.n_events : g->ev_cap;
-    *n = have;
-    uint64_t m = have < cap ? have : cap;
-    if (m == 0) return KRP_OK;
-    std::vector<float4> pc(m), nk(m), S(m);
-    std::vector<unsigned long long> ids(m);
-    CK(cudaMemcpy(pc.data(), g->ev.pc, m * sizeof(float4), cudaMemcpyDeviceToHost));
-    CK(cudaMemcpy(nk.data(), g->ev.nk, m * sizeof(float4), cudaMemcpyDeviceToHost));
-    CK(cudaMemcpy(S.data(), g->ev.S, m * sizeof(float4), cudaMemcpyDeviceToHost));
-    CK(cudaMemcpy(ids.data(), g->ev.id, m * sizeof(unsigned long long), cudaMemcpyDeviceToHost));
-    for (uint64_t i = 0; i < m; ++i) {
-        uint32_t cb, kb;
-        memcpy(&cb, &pc[i].w, 4); memcpy(&kb, &nk[i].w, 4);
-        if (id) id[i] = ids[i];
-        if (k) k[i] = (int32_t)(kb & ~KRP_TERM_BIT);
-        if (cell) {
-            const KrpModel& mm = g->m;
-            uint32_t t = cb / (uint32_t)mm.px, hx = cb - t * (uint32_t)mm.px, hz = t / (uint32_t)mm.py, hy = t - hz * (uint32_t)mm.py;
-            cell[i] = ((int64_t)(hz - 1) * mm.ny + (int64_t)(hy - 1)) * mm.nx + (int64_t)(hx - 1);
-        }
-        if (pos) { pos[3 * i] = pc[i].x; pos[3 * i + 1] = pc[i].y; pos[3 * i + 2] = pc[i].z; }
-        if (dir) { dir[3 * i] = nk[i].x; dir[3 * i + 1] = nk[i].y; dir[3 * i + 2] = nk[i].z; }
-        if (stokes) {
-            stokes[4 * i] = S[i].x; stokes[4 * i + 1] = S[i].x * S[i].y;
-            stokes[4 * i + 2] = S[i].x * S[i].z; stokes[4 * i + 3] = S[i].x * S[i].w;
-        }
-    }
-    return KRP_OK;
+    return events_download(g, 0, UINT64_MAX, cap, n, id, k, cell, pos, dir, stokes);
+}
+
+extern "C" int krp_events_select(krp_grid* g, uint64_t id_first, uint64_t id_count, uint64_t cap, uint64_t* n, uint64_t* id,
+                                 int32_t* k, int64_t* cell, float* pos, float* dir, float* stokes)
+{
+    if (!g || !n) return fail(KRP_ERR_ARG, "grid or n is NULL");
+    if (id_count == UINT64_MAX) return fail(KRP_ERR_ARG, "id_count must be below 2^64-1");
+    return events_download(g, id_first, id_count, cap, n, id, k, cell, pos, dir, stokes);
 }
 
 extern "C" int krp_events_clear(krp_grid* g, void* stream)
@@ -840,61 +880,14 @@ extern "C" int krp_tune(krp_grid* g, int transport_block, int image_block, int b
     return KRP_OK;
 }
 
-// ------------------------------------------------------------------------------------------
-// measurement utility: random-gather rate (include/krp.h)
-// ------------------------------------------------------------------------------------------
-__device__ __forceinline__ uint32_t krp_probe_mix(uint32_t x)
+extern "C" int krp_tune_schedule(krp_grid* g, int dir_sort, int obs_cells, int order_policy)
 {
-    x ^= x >> 16; x *= 0x7feb352du; x ^= x >> 15; x *= 0x846ca68bu; x ^= x >> 16;
-    return x;
-}
-template <typename T>
-__global__ void __launch_bounds__(256) krp_k_probe_gather(const T* __restrict__ a, uint32_t n_elem, int iters, float* __restrict__ sink)
-{
-    const uint32_t i = blockIdx.x * blockDim.x + threadIdx.x;
-    uint32_t h = krp_probe_mix(i * 2654435761u + 12345u);
-    float acc = 0.f;
-    for (int k = 0; k < iters; ++k) {
-        h = krp_probe_mix(h + (uint32_t)k);
-        const T v = __ldg(a + __umulhi(h, n_elem));      // uniform over [0, n_elem)
-        acc += *reinterpret_cast<const float*>(&v);
-    }
-    if (acc == 123.456f) sink[0] = acc;      // never true for a zeroed array: keeps the loads alive
-}
-
-extern "C" int krp_probe_gather(uint64_t array_bytes, int elem_bytes, double* gathers_per_s, void* stream)
-{
-    if (!gathers_per_s) return fail(KRP_ERR_ARG, "gathers_per_s is NULL");
-    if (elem_bytes != 4 && elem_bytes != 16) return fail(KRP_ERR_ARG, "elem_bytes must be 4 or 16");
-    if (array_bytes < (1ull << 20) || array_bytes > (1ull << 35)) return fail(KRP_ERR_ARG, "array_bytes must be in 2^20..2^35");
-    const uint64_t bytes = array_bytes - array_bytes % 16;
-    if (bytes / (uint64_t)elem_bytes >= (1ull << 32)) return fail(KRP_ERR_ARG, "too many elements for the probe");
-    cudaStream_t st = (cudaStream_t)stream;
-    int dev = 0, n_sm = 0;
-    CK(cudaGetDevice(&dev));
-    CK(cudaDeviceGetAttribute(&n_sm, cudaDevAttrMultiProcessorCount, dev));
-    void* a = nullptr; float* sink = nullptr;
-    CK(cudaMalloc(&a, bytes));
-    if (cudaMalloc(&sink, sizeof(float)) != cudaSuccess) { cudaFree(a); return fail(KRP_ERR_OOM, "probe allocation failed"); }
-    cudaEvent_t e0 = nullptr, e1 = nullptr;
-    cudaEventCreate(&e0); cudaEventCreate(&e1);
-    cudaMemsetAsync(a, 0, bytes, st);
-    const int iters = 64, blocks = n_sm * 16, tb = 256;
-    const uint32_t mask = (uint32_t)(bytes / (uint64_t)elem_bytes);     // number of elements
-    float ms = 0.f;
-    cudaError_t err = cudaSuccess;
-    for (int rep = 0; rep < 3 && err == cudaSuccess; ++rep) {
-        cudaEventRecord(e0, st);
-        if (elem_bytes == 16) krp_k_probe_gather<float4><<<blocks, tb, 0, st>>>((const float4*)a, mask, iters, sink);
-        else                  krp_k_probe_gather<float><<<blocks, tb, 0, st>>>((const float*)a, mask, iters, sink);
-        cudaEventRecord(e1, st);
-        err = cudaEventSynchronize(e1);
-        if (err == cudaSuccess) err = cudaEventElapsedTime(&ms, e0, e1);
-    }
-    cudaEventDestroy(e0); cudaEventDestroy(e1);
-    cudaFree(a); cudaFree(sink);
-    if (err != cudaSuccess) return fail(KRP_ERR_CUDA, "probe: %s", cudaGetErrorString(err));
-    *gathers_per_s = (double)blocks * tb * iters / ((double)ms * 1e-3);
+    if (!g) return fail(KRP_ERR_ARG, "grid is NULL");
+    if (dir_sort < -1 || dir_sort > 1 || obs_cells < -1 || obs_cells > 1 || order_policy < -1 || order_policy > 2)
+        return fail(KRP_ERR_ARG, "dir_sort, obs_cells must be -1, 0 or 1 and order_policy -1..2");
+    if (dir_sort >= 0) g->dir_sort = dir_sort;
+    if (obs_cells >= 0 && obs_cells != g->obs_pre) { g->obs_pre = obs_cells; g->obs_host.clear(); }   // rebuilt at the next krp_image
+    if (order_policy >= 0) { g->order_policy = order_policy; g->order_events = order_policy != 0; g->ray_stats_pending = false; }
     return KRP_OK;
 }
 

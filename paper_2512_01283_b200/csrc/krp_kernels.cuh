@@ -1192,7 +1192,7 @@ __device__ __forceinline__ float krp_raya_step(KrpRayA& r, const KrpRayAConst& k
         "@px add.f32 %2, %2, %7;\n\t@px add.s32 %5, %5, %10;\n\t"
         "@py add.f32 %3, %3, %8;\n\t@py add.s32 %5, %5, %11;\n\t"
         "@pz add.f32 %4, %4, %9;\n\t@pz add.s32 %5, %5, %12;\n\t}"
-        : "=f"(ds), "=&f"(tn), "+f"(r.tx), "+f"(r.ty), "+f"(r.tz), "+r"(r.c)
+        : "=&f"(ds), "=&f"(tn), "+f"(r.tx), "+f"(r.ty), "+f"(r.tz), "+r"(r.c)
         : "f"(r.t), "f"(k.dtx), "f"(k.dty), "f"(k.dtz), "r"(k.sx), "r"(k.sy), "r"(k.sz));
     r.t = tn;
     return ds;

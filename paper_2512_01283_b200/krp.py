@@ -16,8 +16,8 @@ MEM_DEVICE, MEM_HOST = 0, 1
 SYMBOLS = [
     "krp_last_error", "krp_version", "krp_grid_create", "krp_grid_destroy", "krp_grid_update", "krp_source_set",
     "krp_events_reserve", "krp_transport", "krp_packet_id_set", "krp_image", "krp_image_get",
-    "krp_image_reset", "krp_stats_get", "krp_stats_reset", "krp_events_get", "krp_events_clear",
-    "krp_tune", "krp_timing_enable", "krp_timing_get", "krp_probe_gather", "krp_launch_count",
+    "krp_image_reset", "krp_stats_get", "krp_stats_reset", "krp_events_get", "krp_events_select", "krp_events_clear",
+    "krp_tune", "krp_tune_schedule", "krp_timing_enable", "krp_timing_get", "krp_launch_count",
 ]
 T_FLIGHT, T_SCATTER, T_ORDER, T_IMAGE, T_EMIT, T_COUNT = 0, 1, 2, 3, 4, 5
 T_NAMES = ("flight", "scatter", "order", "image", "emit")
@@ -61,7 +61,8 @@ def library_path():
 
 
 def lib():
-    """Load libkrp.so (building it if nvcc is here and the sources are newer)."""
+    """Load libkrp.so, rebuilding it first when it was not compiled from the sources beside it (the build id is a
+    hash of the sources).  A library that is stale and cannot be rebuilt is an error: nothing runs on old kernels."""
     global _lib
     if _lib is not None:
         return _lib
@@ -69,11 +70,13 @@ def lib():
     if _build.stale():
         try:
             _build.build()
-        except Exception as exc:  # no nvcc on this box and no prebuilt library: fail loudly
-            if not os.path.exists(path):
-                raise ImportError("libkrp.so is missing and could not be built (%s); "
-                                  "run `python -m paper_2512_01283_b200._build`" % exc) from exc
+        except Exception as exc:
+            raise ImportError("libkrp.so is missing or was built from other sources (want build id %s) and could not be "
+                              "rebuilt (%s); run `python -m paper_2512_01283_b200._build`" % (_build.source_id(), exc)) from exc
     L = C.CDLL(path)
+    L.krp_version.restype = C.c_char_p
+    if _build.source_id().encode() not in L.krp_version():
+        raise ImportError("libkrp.so reports %r, the sources beside it have build id %s" % (L.krp_version(), _build.source_id()))
     vp, u64, i32 = C.c_void_p, C.c_uint64, C.c_int
     sig = {
         "krp_last_error": (C.c_char_p, []),
@@ -92,11 +95,12 @@ def lib():
         "krp_stats_get": (i32, [vp, C.POINTER(Stats)]),
         "krp_stats_reset": (i32, [vp, vp]),
         "krp_events_get": (i32, [vp, u64, C.POINTER(u64), vp, vp, vp, vp, vp, vp]),
+        "krp_events_select": (i32, [vp, u64, u64, u64, C.POINTER(u64), vp, vp, vp, vp, vp, vp]),
         "krp_events_clear": (i32, [vp, vp]),
         "krp_tune": (i32, [vp, i32, i32, i32, i32]),
         "krp_timing_enable": (i32, [vp, i32]),
         "krp_timing_get": (i32, [vp, vp, vp]),
-        "krp_probe_gather": (i32, [u64, i32, C.POINTER(C.c_double), vp]),
+        "krp_tune_schedule": (i32, [vp, i32, i32, i32]),
         "krp_launch_count": (u64, [vp]),
     }
     for name, (res, args) in sig.items():
@@ -134,13 +138,6 @@ def _ptr_mem(a):
         raise TypeError("expected float32")
     a = a.contiguous()
     return C.c_void_p(a.data_ptr()), (MEM_DEVICE if a.is_cuda else MEM_HOST), a
-
-
-def probe_gather(array_bytes, elem_bytes, stream=None):
-    """Random-gather rate of this GPU for an array of that size (gathers/s); measurement utility."""
-    out = C.c_double(0.0)
-    _check(lib().krp_probe_gather(int(array_bytes), int(elem_bytes), C.byref(out), _stream(stream)))
-    return out.value
 
 
 def make_observer(theta, phi, center, half_w, half_h=None):
@@ -249,17 +246,22 @@ class Grid:
     def stats_reset(self, stream=None):
         _check(lib().krp_stats_reset(self._h, _stream(stream)))
 
-    def events_get(self, cap=None):
+    def events_get(self, cap=None, id_first=None, id_count=None):
+        """Buffered events as host arrays; with id_first/id_count only those of that packet id range (krp_events_select)."""
+        L = lib()
+        if id_first is None:
+            call = lambda *a: L.krp_events_get(self._h, *a)
+        else:
+            call = lambda *a: L.krp_events_select(self._h, int(id_first), int(id_count), *a)
         n = C.c_uint64(0)
-        _check(lib().krp_events_get(self._h, 0, C.byref(n), None, None, None, None, None, None))
+        _check(call(0, C.byref(n), None, None, None, None, None, None))
         m = n.value if cap is None else min(int(cap), n.value)
         ev = dict(id=np.zeros(m, np.uint64), k=np.zeros(m, np.int32), cell=np.zeros(m, np.int64),
                   pos=np.zeros((m, 3), np.float32), dir=np.zeros((m, 3), np.float32),
                   stokes=np.zeros((m, 4), np.float32))
         if m:
-            _check(lib().krp_events_get(self._h, m, C.byref(n), ev["id"].ctypes.data, ev["k"].ctypes.data,
-                                        ev["cell"].ctypes.data, ev["pos"].ctypes.data, ev["dir"].ctypes.data,
-                                        ev["stokes"].ctypes.data))
+            _check(call(m, C.byref(n), ev["id"].ctypes.data, ev["k"].ctypes.data, ev["cell"].ctypes.data,
+                        ev["pos"].ctypes.data, ev["dir"].ctypes.data, ev["stokes"].ctypes.data))
         return ev
 
     def events_clear(self, stream=None):
@@ -267,6 +269,12 @@ class Grid:
 
     def tune(self, transport_block=0, image_block=0, blocks_per_sm=0, flight_burst=0):
         _check(lib().krp_tune(self._h, int(transport_block), int(image_block), int(blocks_per_sm), int(flight_burst)))
+
+    def tune_schedule(self, dir_sort=-1, obs_cells=-1, order_policy=-1):
+        _check(lib().krp_tune_schedule(self._h, int(dir_sort), int(obs_cells), int(order_policy)))
+
+    def version(self):
+        return lib().krp_version().decode()
 
     def timing_enable(self, on=True):
         _check(lib().krp_timing_enable(self._h, int(bool(on))))

@@ -17,6 +17,7 @@ import scipy.linalg
 from oracle import lib, OracleModel, OracleEvents, OracleStats, Observer
 
 L = lib()
+FP32_STATE = bool(L.ora_state_is_fp32())       # False in the pure-fp64 control build (KRP_ORACLE_VARIANT=pure, R12)
 GOLD = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
 
 
@@ -619,7 +620,8 @@ def test_event_stokes_in_dichroic_medium_and_invariants():
     E = esc["S"]; assert np.all(E[:, 0] ** 2 >= (E[:, 1:] ** 2).sum(1) * (1 - 1e-12))
     assert np.allclose(np.linalg.norm(ev.n_in[:n], axis=1), 1, atol=2e-7)
     assert np.array_equal(ev.n_in[:n].astype(np.float32).astype(float), ev.n_in[:n])     # fp32 state (R12)
-    assert np.array_equal(ev.p[:n].astype(np.float32).astype(float), ev.p[:n])           # fp32 positions (R12)
+    if FP32_STATE:
+        assert np.array_equal(ev.p[:n].astype(np.float32).astype(float), ev.p[:n])       # fp32 positions (R12)
     assert np.all((ev.p[:n] >= 0) & (ev.p[:n] <= 1))
     # weights: k-th event carries omega^k
     assert np.allclose(S[:, 0], float(np.float32(om)) ** ev.k[:n], rtol=1e-12)
@@ -738,7 +740,8 @@ def test_image_direct_light_and_projection():
     tv, pv = sph_basis(n_obs)
     # the record holds the cell index and the fp32 cell-local position (reading R12): rebuild x from them
     cl = (np.array([0.3, -0.2, 0.5]) + 1) / 0.25
-    x = -1 + (np.floor(cl) + (cl - np.floor(cl)).astype(np.float32).astype(float)) * 0.25
+    frac = cl - np.floor(cl)
+    x = -1 + (np.floor(cl) + (frac.astype(np.float32).astype(float) if FP32_STATE else frac)) * 0.25
     ix = int(math.floor((np.dot(x, pv) / 1.5 + 1) * 15)); iy = int(math.floor((-np.dot(x, tv) / 1.0 + 1) * 10))
     tt = min(((1 - x[a]) / n_obs[a]) if n_obs[a] > 0 else ((-1 - x[a]) / n_obs[a]) for a in range(3))
     assert st2.contributions == 1 and np.count_nonzero(img[0, 0]) == 1
@@ -748,3 +751,140 @@ def test_image_direct_light_and_projection():
     o2 = Observer.make(th, ph, [5, 5, 5], 0.1)                               # out of frame: dropped, counted
     img, _, st2 = m.image(ev, [o2], 8, 8, 1)
     assert st2.dropped == 1 and not img.any()
+
+
+# ----------------------------------------------------------------------------
+# second-moment map: the sigma of every "3 sigma per pixel" parity assertion
+# ----------------------------------------------------------------------------
+def _manual_events(m, recs):
+    """Event list written by hand: recs = [(idx triple, cell-local p, n_in, S, k)]."""
+    ev = OracleEvents(len(recs))
+    for i, (idx, p, n_in, S, k) in enumerate(recs):
+        ev.cell[i] = (idx[2] * m.ny + idx[1]) * m.nx + idx[0]
+        ev.p[i] = p; ev.n_in[i] = n_in; ev.S[i] = S; ev.id[i] = i; ev.k[i] = k
+    ev.c.n = len(recs)
+    return ev
+
+
+def test_image_second_moment_is_the_sum_of_squares():
+    """img2 accumulates the SQUARE of every contribution: one record gives img2 == img^2 exactly, two
+    records in one pixel give s1^2 + s2^2 (not (s1+s2)^2, not |s1|+|s2|, not s1+s2)."""
+    m = box_model((6, 6, 6), 1.3, bvec=(0.2, 0.5, 0.8), mueller=hg_table(0.4), opac=const_opac(1.0, 0.2, 0.1, 0.5))
+    o = [Observer.make(1.0, 0.7, [0.5, 0.5, 0.5], 0.9), Observer.make(2.2, 4.0, [0.5, 0.5, 0.5], 0.9)]
+    r1 = ((2, 3, 1), [0.3, 0.6, 0.2], [0.6, 0.0, 0.8], [0.7, 0.21, -0.14, 0.35], 1)
+    r2 = ((2, 3, 1), [0.3, 0.6, 0.2], [0.0, -0.6, 0.8], [0.4, -0.1, 0.2, -0.12], 2)     # same place, other state
+    imgs = []
+    for recs in ([r1], [r2], [r1, r2]):
+        img, img2, st = m.image(_manual_events(m, recs), o, 8, 8, 0)
+        assert st.contributions == 2 * len(recs) and st.dropped == 0
+        imgs.append((img, img2))
+    for img, img2 in imgs[:2]:
+        assert np.count_nonzero(img[:, 0]) == 2                                # one pixel per observer
+        assert np.all(img[:, 1:].reshape(2, 3, -1).any(axis=2))               # Q, U, V all exercised
+        assert np.array_equal(img2, img * img)                                 # one record: exactly the square
+    (i1, q1), (i2, q2), (i12, q12) = imgs
+    assert np.allclose(i12, i1 + i2, rtol=1e-15, atol=0)
+    assert np.allclose(q12, q1 + q2, rtol=1e-15, atol=0)                       # sum of squares ...
+    nz = i12 != 0
+    assert np.all(np.abs(q12[nz] - i12[nz] ** 2) > 1e-3 * q12[nz])             # ... which is not the square of the sum
+    img, img2, _ = m.image(_manual_events(m, [r1]), o, 8, 8, 0, second_moment=False)
+    assert img2 is None and np.array_equal(img, i1)
+
+
+# ----------------------------------------------------------------------------
+# the (U,V) block and the S34 terms of F(Theta), in the sampler and in the peel-off
+# ----------------------------------------------------------------------------
+def _F_printed(F):
+    """F(Theta) as SURVEY.md 8(c) S5 prints it (spherical-form scattering matrix; reading R6 fixes the sign of S34)."""
+    s11, s12, s33, s34 = F
+    return np.array([[s11, s12, 0, 0], [s12, s11, 0, 0], [0, 0, s33, s34], [0, 0, -s34, s33]])
+
+
+def test_circular_light_through_rayleigh_scattering():
+    """Circular input has no linear part, so no frame rotation touches it: after one Rayleigh scattering
+    V'/I' = S33/S11 = 2 cos(Theta)/(1 + cos^2 Theta), Q'/I' = -(1-cos^2)/(1+cos^2) in the scattering plane's
+    reference, for any B and any azimuth -- in the sampler's chain and in the peel-off."""
+    m = box_model()
+    rng = np.random.default_rng(31)
+    for hel in (1.0, -1.0):
+        for _ in range(200):
+            b, n_in = rand_unit(rng), rand_unit(rng)
+            Theta = rng.uniform(2, 178); c = math.cos(math.radians(Theta))
+            n_out, S = m.scatter_angles(b, n_in, [1, 0, 0, hel], Theta, rng.uniform(0, 2 * math.pi))
+            assert abs(S[3] - hel * 2 * c / (1 + c * c)) < 2e-4 and S[0] == 1.0
+            assert abs(math.hypot(S[1], S[2]) - (1 - c * c) / (1 + c * c)) < 2e-4
+            n_obs = rand_unit(rng); mu = float(np.dot(n_in, n_obs))
+            P = m.peel(n_in, [1, 0, 0, hel], n_obs)
+            assert abs(P[3] / P[0] - hel * 2 * mu / (1 + mu * mu)) < 2e-4
+            assert abs(P[0] * 4 * math.pi - 0.75 * (1 + mu * mu)) < 2e-4
+
+
+def test_F_entry_by_entry_in_the_xz_plane():
+    """A scattering inside the x-z plane with B = z^ (q_B = 1) and azimuth 0 needs no frame rotation at all:
+    theta^ of n_in is e_par and theta^ of n_out is e_par,out.  The oracle's output must then be the printed
+    F(Theta) times the input, entry by entry, on a table with S34 != 0 -- rows U and V included."""
+    tab = hg_table(0.4)
+    m = box_model(bvec=(0, 0, 1), mueller=tab)
+    rng = np.random.default_rng(32)
+    seen = np.zeros((4, 4), bool)
+    for _ in range(200):
+        a = math.radians(rng.uniform(5, 60)); Theta = float(rng.integers(10, 110))       # a table node: no interpolation
+        n_in = np.array([math.sin(a), 0.0, math.cos(a)])
+        S_in = np.r_[1.0, rand_unit(rng) * rng.uniform(0.2, 0.95)]
+        F = _F_printed(tab[int(Theta)].astype(float))
+        want = F @ S_in
+        n_out, S = m.scatter_angles([0, 0, 1], n_in, S_in, Theta, 0.0)
+        b = a + math.radians(Theta)
+        assert np.allclose(n_out, [math.sin(b), 0, math.cos(b)], atol=1e-7)
+        assert np.allclose(S, want / want[0], atol=1e-12)
+        P = m.peel(n_in, S_in, [math.sin(b), 0.0, math.cos(b)])
+        assert np.allclose(P * 4 * math.pi, want, atol=1e-6 * want[0])              # acos(mu) -> Theta: 1e-8 degrees off the node
+        seen |= F != 0
+    assert seen[2, 3] and seen[3, 2]
+    # each entry alone: unit inputs (the rows of F read off one by one from differences)
+    Theta = 70.0; F = _F_printed(tab[70].astype(float)); a = 0.4
+    n_in = [math.sin(a), 0.0, math.cos(a)]; n_o = [math.sin(a + math.radians(Theta)), 0.0, math.cos(a + math.radians(Theta))]
+    base = m.peel(n_in, [1, 0, 0, 0], n_o) * 4 * math.pi
+    assert np.allclose(base, F[:, 0], atol=1e-6)
+    for j in (1, 2, 3):
+        e = np.zeros(4); e[0] = 1; e[j] = 0.5
+        col = (m.peel(n_in, e, n_o) * 4 * math.pi - base) / 0.5
+        assert np.allclose(col, F[:, j], atol=2e-6), (j, col, F[:, j])
+    assert F[2, 3] == -F[3, 2] and F[2, 3] != 0
+
+
+# ----------------------------------------------------------------------------
+# S1 emission: the exact map from the Philox words, and isotropy
+# ----------------------------------------------------------------------------
+def test_emission_map_and_isotropy():
+    """PAPER.md:107 (emission) with the schedule R11: block 0 of event 0 gives cos(theta) = 1 - 2 u0, phi = 2 pi u1,
+    tau* = -ln u2.  Three ids exactly; then moments an isotropic direction must have (theta uniform instead of
+    cos(theta) uniform gives <n_z^2> = 1/2, phi = pi u gives <n_y> > 0)."""
+    m = box_model((4, 4, 4), 1.0)
+    m.source_set(0, [0.3, 0.55, 0.8], [0, 0, 1], None, 0)
+    seed = 77
+    for pid in (0, 12345, 2 ** 35 + 9):
+        w = _philox(seed, (pid & 0xFFFFFFFF, pid >> 32, 0, 0))
+        u = [((int(x) >> 9) + 0.5) / 8388608.0 for x in w]
+        ct = 1 - 2 * u[0]; st = math.sqrt(1 - ct * ct); ph = 2 * math.pi * u[1]
+        idx, p, n, tau = m.emit(seed, pid)
+        want = np.array([st * math.cos(ph), st * math.sin(ph), ct])
+        assert np.array_equal(n, want.astype(np.float32).astype(float))           # fp32 direction (first-commit state)
+        assert abs(tau + math.log(u[2])) < 1e-15
+        assert list(idx) == [1, 2, 3]
+        pw = np.array([0.3, 0.55, 0.8]) * 4 - np.array([1, 2, 3])
+        assert np.allclose(p, pw, atol=1e-7 if FP32_STATE else 1e-15)
+    N = 200000
+    nn = np.array([m.emit(5, i)[2] for i in range(N)])
+    assert np.all(np.abs(nn.mean(0)) < 5 * 0.577 / math.sqrt(N))                     # <n> = 0
+    assert np.all(np.abs((nn * nn).mean(0) - 1 / 3) < 5 * 0.298 / math.sqrt(N))       # <n_i^2> = 1/3 (var 4/45)
+    assert abs((nn[:, 0] * nn[:, 1]).mean()) < 5 * 0.26 / math.sqrt(N)
+    h, _ = np.histogram(nn[:, 2], bins=20, range=(-1, 1))                            # cos(theta) uniform
+    assert np.all(np.abs(h - N / 20) < 5 * math.sqrt(N / 20))
+    h, _ = np.histogram(np.arctan2(nn[:, 1], nn[:, 0]), bins=24, range=(-math.pi, math.pi))     # phi uniform
+    assert np.all(np.abs(h - N / 24) < 5 * math.sqrt(N / 24))
+    # collimated source: the direction is the given one, tau* still from word 2
+    m.source_set(2, [0.5, 0.5, 0.0], [0, 0.6, 0.8], None, 0)
+    idx, p, n, tau = m.emit(seed, 3)
+    assert np.allclose(n, [0, 0.6, 0.8], atol=1e-7)
+    assert abs(tau + math.log(((int(_philox(seed, (3, 0, 0, 0))[2]) >> 9) + 0.5) / 8388608.0)) < 1e-15
