@@ -550,12 +550,19 @@ static void push_event(ora_events* ev, ora_stats* st, int64_t cell, const double
     for (int s = 0; s < 4; ++s) ev->S[4*i+s] = scale * S[s];
 }
 
+typedef struct ora_observer { double theta, phi, center[3], half_w, half_h; } ora_observer;
+
+/* step 1 of the paper's two-step form (defined at the end of this file): optional hook of flight() */
+struct ora_deposit;
+static void deposit_segment(const ora_model* m, struct ora_deposit* dep, int64_t c, const double n[3], const double S_lab[4],
+                            const double a[4], double ce, double se, int rotated, double T, double W);
+
 /* One flight (S2-S4): start with I = 1; after every cell compare I with
  * e^{-tau*}; locate the event inside the cell with ora_event_solve.
  * Returns 1 at an event (S normalised to (1,q,u,v), idx/p at the event),
  * 0 when the packet left the grid. */
 static int flight(const ora_model* m, int idx[3], double p[3], const double n[3], double S[4],
-                  double tau_star, ora_stats* st)
+                  double tau_star, ora_stats* st, struct ora_deposit* dep, double W)
 {
     double target = exp(-tau_star);
     for (;;) {
@@ -572,12 +579,14 @@ static int flight(const ora_model* m, int idx[3], double p[3], const double n[3]
                 double Iout = S[0] * exp(-a[0] * dtau);
                 if (Iout <= target) {
                     double t = ora_event_solve(S[0], 0.0, a[0], 0.0, target);
+                    if (dep) deposit_segment(m, dep, c, n, S, a, 1.0, 0.0, 0, t, W);
                     advance(m, idx, p, n, t / kr, -1);
                     for (int a2 = 0; a2 < 3; ++a2) p[a2] = ORA_STATE(p[a2]);   /* R12 */
                     double I = S[0];
                     for (int s = 0; s < 4; ++s) S[s] /= I;
                     return 1;
                 }
+                if (dep) deposit_segment(m, dep, c, n, S, a, 1.0, 0.0, 0, dtau, W);
                 double e = exp(-a[0] * dtau);
                 for (int s = 0; s < 4; ++s) S[s] *= e;
             } else {
@@ -590,6 +599,7 @@ static int flight(const ora_model* m, int idx[3], double p[3], const double n[3]
                 ora_appA(So, a[0], a[1], a[2], dtau);
                 if (So[0] <= target) {
                     double t = ora_event_solve(Sg[0], Sg[1] / Sg[0], a[0], a[1], target);
+                    if (dep) deposit_segment(m, dep, c, n, S, a, ce, se, 1, t, W);
                     ora_appA(Sg, a[0], a[1], a[2], t);
                     double I = Sg[0];
                     for (int s = 0; s < 4; ++s) Sg[s] /= I;
@@ -599,6 +609,7 @@ static int flight(const ora_model* m, int idx[3], double p[3], const double n[3]
                     for (int a2 = 0; a2 < 3; ++a2) p[a2] = ORA_STATE(p[a2]);   /* R12 */
                     return 1;
                 }
+                if (dep) deposit_segment(m, dep, c, n, S, a, ce, se, 1, dtau, W);
                 ora_rotate_qu(So, ce, -se);
                 for (int s = 0; s < 4; ++s) S[s] = So[s];
             }
@@ -653,9 +664,10 @@ void ora_emit(const ora_model* m, uint64_t seed, uint64_t id, int idx[3], double
  * state of every packet that leaves the grid -- direction, W*(1,q,u,v) in
  * the lab reference of that direction, id -- used by the naive-estimator pin
  * (PAPER.md:115).  Returns the number of escape records written.          */
-int64_t ora_transport(const ora_model* m, uint64_t id0, uint64_t n_packets, uint64_t seed,
-                      ora_events* ev, ora_stats* st,
-                      int64_t esc_cap, double* esc_n, double* esc_S, uint64_t* esc_id, int32_t* esc_k)
+int64_t ora_transport2(const ora_model* m, uint64_t id0, uint64_t n_packets, uint64_t seed,
+                       ora_events* ev, ora_stats* st,
+                       int64_t esc_cap, double* esc_n, double* esc_S, uint64_t* esc_id, int32_t* esc_k,
+                       struct ora_deposit* dep)
 {
     int64_t nesc = 0;
     for (uint64_t id = id0; id < id0 + n_packets; ++id) {
@@ -666,7 +678,7 @@ int64_t ora_transport(const ora_model* m, uint64_t id0, uint64_t n_packets, uint
         if (m->emit_records) { push_event(ev, st, cell_of(m, idx), p, n, S, W, id, 0); st->records++; }
         int k = 0;
         for (;;) {
-            if (!flight(m, idx, p, n, S, tau_star, st)) {
+            if (!flight(m, idx, p, n, S, tau_star, st, dep, W)) {
                 st->w_escaped += W;
                 if (nesc < esc_cap) {
                     for (int a = 0; a < 3; ++a) esc_n[3*nesc+a] = n[a];
@@ -696,6 +708,13 @@ int64_t ora_transport(const ora_model* m, uint64_t id0, uint64_t n_packets, uint
         }
     }
     return nesc;
+}
+
+int64_t ora_transport(const ora_model* m, uint64_t id0, uint64_t n_packets, uint64_t seed,
+                      ora_events* ev, ora_stats* st,
+                      int64_t esc_cap, double* esc_n, double* esc_S, uint64_t* esc_id, int32_t* esc_k)
+{
+    return ora_transport2(m, id0, n_packets, seed, ev, st, esc_cap, esc_n, esc_S, esc_id, esc_k, NULL);
 }
 
 /* ------------------------------------------------------------------ */
@@ -728,8 +747,6 @@ void ora_peel(const ora_model* m, const double n_in[3], const double S_in[4], co
     ora_rotate_qu(S, dot3(eout, tho), dot3(tho, sh));
     for (int s = 0; s < 4; ++s) S_out[s] = S[s] / (4 * ORA_PI);
 }
-
-typedef struct ora_observer { double theta, phi, center[3], half_w, half_h; } ora_observer;
 
 /* Image every event toward every observer.  img/img2: [n_obs][4][ny][nx]
  * sums and sums of squares.  flags bit0: also image emission records (k=0)
@@ -766,6 +783,184 @@ void ora_image(const ora_model* m, const ora_events* ev, const ora_observer* obs
                 img[at] += S[s];
                 if (img2) img2[at] += S[s] * S[s];
             }
+        }
+    }
+}
+
+/* ================================================================== */
+/* NEXT-1 / NEXT-3: the paper's own two-step form (PAPER.md:113-123,   */
+/* eq. 11) and the in-cell solution WITH source terms (App. A,         */
+/* PAPER.md:296-328).  DESIGN.md section 12 states the readings.       */
+/* ================================================================== */
+
+/* A12 with sources: PAPER.md:302-328 (eq. A2-A3) with the matrix of R1.  src = (S1..S4) is the source per unit
+ * extinction optical depth, constant in the cell, in the same (grain-frame) reference as S.  The printed solution
+ * is the source-free one applied to S - S_s, plus S_s, with the stationary vector S_s of eq. A3. */
+void ora_appA_src(double S[4], double a1, double a2, double a3, const double src[4], double dtau)
+{
+    double Is = (a1 * src[0] - a2 * src[1]) / (a1 * a1 - a2 * a2);
+    double Qs = (a1 * src[1] - a2 * src[0]) / (a1 * a1 - a2 * a2);
+    double Us = (a1 * src[2] - a3 * src[3]) / (a1 * a1 + a3 * a3);
+    double Vs = (a1 * src[3] + a3 * src[2]) / (a1 * a1 + a3 * a3);
+    double D[4] = { S[0] - Is, S[1] - Qs, S[2] - Us, S[3] - Vs };
+    ora_appA(D, a1, a2, a3, dtau);
+    S[0] = Is + D[0]; S[1] = Qs + D[1]; S[2] = Us + D[2]; S[3] = Vs + D[3];
+}
+
+/* 16-point Gauss-Legendre nodes and weights on [-1,1], by Newton on P_16 (textbook construction) */
+static void gl16(double x[16], double w[16])
+{
+    const int n = 16;
+    for (int i = 0; i < n; ++i) {
+        double z = cos(ORA_PI * (i + 0.75) / (n + 0.5)), pp = 1.0;
+        for (int it = 0; it < 100; ++it) {
+            double p1 = 1.0, p2 = 0.0;
+            for (int j = 0; j < n; ++j) { double p3 = p2; p2 = p1; p1 = ((2.0 * j + 1.0) * z * p2 - j * p3) / (j + 1.0); }
+            pp = n * (z * p1 - p2) / (z * z - 1.0);
+            double dz = p1 / pp;
+            z -= dz;
+            if (fabs(dz) < 1e-16) break;
+        }
+        x[i] = z; w[i] = 2.0 / ((1.0 - z * z) * pp * pp);
+    }
+}
+
+/* Step 1 of the two-step scheme, one path segment ("each path integration segment (i.e., not only
+ * at scattering events) contributes to a scattering source function stored on the grid", S_pp = Z(Omega_cam;Omega_pp) I_pp).
+ * Reading R18: the deposit is the track-length form of the very estimator the event form uses.  A packet
+ * that is alive at extinction depth tau inside the segment has the normalised state s^(tau) = S~(tau)/I~(tau) (R7; S~ the
+ * source-free App. A solution from the state Sg at the start of the segment, grain-frame reference) and collides at the
+ * rate r(tau) = -I~'/I~ = alpha1 + alpha2 q^_g(tau) per unit depth, every collision sending out omega W Z s^.  The
+ * expected collision output of the segment is therefore omega W Z J with
+ *        J = int_0^T r(tau) s^(tau) dtau ,
+ * which this function returns (4 components, grain-frame reference; J[0] = expected number of collisions).  J[0] and
+ * J[1] have closed forms (pins); U and V do not, so all four are evaluated by composite 16-point Gauss-Legendre
+ * quadrature on sub-intervals of (|alpha2| + |alpha3|) h <= 0.5 (integrand analytic: error far below 1e-15). */
+void ora_segment_integral(const double Sg[4], double a1, double a2, double a3, double T, double J[4])
+{
+    static double gx[16], gw[16]; static int have = 0;
+    if (!have) { gl16(gx, gw); have = 1; }
+    for (int s = 0; s < 4; ++s) J[s] = 0.0;
+    if (!(T > 0.0)) return;
+    int nsub = (int)ceil((fabs(a2) + fabs(a3)) * T / 0.5);
+    if (nsub < 1) nsub = 1;
+    double h = T / nsub;
+    for (int k = 0; k < nsub; ++k) {
+        for (int i = 0; i < 16; ++i) {
+            double tau = (k + 0.5 * (gx[i] + 1.0)) * h;
+            double S[4] = { Sg[0], Sg[1], Sg[2], Sg[3] };
+            /* e^{+alpha1 tau} is divided out analytically: only ratios of the solution enter */
+            ora_appA(S, 0.0, a2, a3, tau);
+            double r = a1 + a2 * S[1] / S[0];
+            for (int s = 0; s < 4; ++s) J[s] += 0.5 * h * gw[i] * r * S[s] / S[0];
+        }
+    }
+}
+
+/* what step 1 accumulates: sgrid[ncell][n_obs][4], the expected collision output toward every camera in the reference
+ * theta^_obs, including omega W and the 1/(4 pi) of the peel-off, NOT attenuated (step 2 does that) and not divided by
+ * the cell volume; coll[ncell] (optional) = expected number of collisions times W (pin against the event counts). */
+typedef struct ora_deposit {
+    const ora_observer* obs; int n_obs;
+    double* sgrid; double* coll;
+    uint64_t segments;
+} ora_deposit;
+
+static void deposit_segment(const ora_model* m, ora_deposit* dep, int64_t c, const double n[3], const double S_lab[4],
+                            const double a[4], double ce, double se, int rotated, double T, double W)
+{
+    /* S_lab: state at the start of the segment in the lab reference of n; (ce, se): eta of eq. 6-7 when the cell is dichroic */
+    double Sg[4] = { S_lab[0], S_lab[1], S_lab[2], S_lab[3] }, J[4];
+    if (rotated) ora_rotate_qu(Sg, ce, se);
+    ora_segment_integral(Sg, a[0], a[1], a[2], T, J);
+    if (rotated) ora_rotate_qu(J, ce, -se);
+    if (dep->coll) dep->coll[c] += W * J[0];
+    double Jw[4] = { a[3] * W * J[0], a[3] * W * J[1], a[3] * W * J[2], a[3] * W * J[3] };
+    for (int o = 0; o < dep->n_obs; ++o) {
+        double no[3] = { sin(dep->obs[o].theta) * cos(dep->obs[o].phi), sin(dep->obs[o].theta) * sin(dep->obs[o].phi), cos(dep->obs[o].theta) };
+        double out[4];
+        ora_peel(m, n, Jw, no, out);
+        for (int s = 0; s < 4; ++s) dep->sgrid[((int64_t)c * dep->n_obs + o) * 4 + s] += out[s];
+    }
+    dep->segments++;
+}
+
+/* step 1 for packets [id0, id0+n): the ordinary transport (same packets, same events) with every path segment also
+ * deposited into sgrid / coll (either may be NULL) */
+void ora_transport_deposit(const ora_model* m, uint64_t id0, uint64_t n_packets, uint64_t seed, ora_events* ev, ora_stats* st,
+                           const ora_observer* obs, int n_obs, double* sgrid, double* coll, uint64_t* n_segments)
+{
+    ora_deposit dep = { obs, n_obs, sgrid, coll, 0 };
+    ora_transport2(m, id0, n_packets, seed, ev, st, 0, NULL, NULL, NULL, NULL, &dep);
+    if (n_segments) *n_segments = dep.segments;
+}
+
+/* Step 2: "a deterministic ray-tracing step by integrating eq. (8) along lines of sight toward the
+ * camera ... with the same cell-by-cell analytic integration": one ray per pixel, through the pixel centre, from the far
+ * side of the grid toward the observer, App. A WITH source terms in every cell.  Sources per unit extinction depth in
+ * cell c (reference theta^_obs, rotated into the grain frame for the solve):
+ *    scattering   sgrid[c][o][:] / (V_c kappa rho_c)        (step 1; V_c = cell volume)
+ *    thermal      (1 - omega) (alpha1, alpha2, 0, 0)_GF B_c  (eq. 8: alpha_abs B with B ~ (1,0,0,0); reading R19:
+ *                 alpha_abs = (1 - omega) alpha; emis[c] = B_c, may be NULL)
+ * The pixel receives radiance times the pixel's area (R14: image units are sums of packet contributions per pixel).
+ * img[n_obs][4][npy][npx] is added to. */
+void ora_image_rays(const ora_model* m, const double* sgrid, const float* emis, const ora_observer* obs, int n_obs,
+                    int npx, int npy, double* img, ora_stats* st)
+{
+    const int nn[3] = { m->nx, m->ny, m->nz };
+    const double vol = m->d[0] * m->d[1] * m->d[2];
+    for (int o = 0; o < n_obs; ++o) {
+        double no[3] = { sin(obs[o].theta) * cos(obs[o].phi), sin(obs[o].theta) * sin(obs[o].phi), cos(obs[o].theta) };
+        double tho[3], pho[3];
+        ora_basis(no, tho, pho);
+        const double apix = (2.0 * obs[o].half_w / npx) * (2.0 * obs[o].half_h / npy);
+        for (int iy = 0; iy < npy; ++iy) for (int ix = 0; ix < npx; ++ix) {
+            /* pixel centre on the image plane (R14: x along phi^_obs, y along -theta^_obs) */
+            double xi = ((ix + 0.5) * 2.0 / npx - 1.0) * obs[o].half_w, yi = ((iy + 0.5) * 2.0 / npy - 1.0) * obs[o].half_h;
+            double x0[3];
+            for (int a = 0; a < 3; ++a) x0[a] = obs[o].center[a] + xi * pho[a] - yi * tho[a];
+            /* the line x0 + s n_obs against the box: slab method */
+            double s_in = -INFINITY, s_out = INFINITY; int miss = 0;
+            for (int a = 0; a < 3; ++a) {
+                double lo = m->lo[a], hi = m->lo[a] + nn[a] * m->d[a];
+                if (no[a] == 0.0) { if (x0[a] < lo || x0[a] >= hi) miss = 1; continue; }
+                double t0 = (lo - x0[a]) / no[a], t1 = (hi - x0[a]) / no[a];
+                if (t0 > t1) { double t = t0; t0 = t1; t1 = t; }
+                if (t0 > s_in) s_in = t0;
+                if (t1 < s_out) s_out = t1;
+            }
+            if (miss || !(s_in < s_out)) continue;
+            int idx[3]; double p[3];
+            for (int a = 0; a < 3; ++a) {
+                double x = (x0[a] + s_in * no[a] - m->lo[a]) / m->d[a];
+                int i = (int)floor(x);
+                if (i < 0) i = 0;
+                if (i > nn[a] - 1) i = nn[a] - 1;
+                double f = x - i;
+                idx[a] = i; p[a] = f < 0 ? 0 : (f > 1 ? 1 : f);
+            }
+            double S[4] = { 0, 0, 0, 0 };
+            for (;;) {
+                int axis; double ds = ora_dda_exit(m, p, no, &axis);
+                int64_t c = cell_of(m, idx);
+                if (st) st->steps_image++;
+                double kr = m->kr[c];
+                if (kr > 0) {
+                    double b[3], a[4], src[4] = { 0, 0, 0, 0 };
+                    cell_bhat(m, c, b);
+                    ora_opac_at(m, mu_of(no, b), a);
+                    if (sgrid) for (int s = 0; s < 4; ++s) src[s] = sgrid[((int64_t)c * n_obs + o) * 4 + s] / (vol * kr);
+                    double q[4], ce = 1.0, se = 0.0;
+                    int rot = !(a[1] == 0.0 && a[2] == 0.0);
+                    if (rot) { ora_quat_from_B(b, q); ora_eta_gf(q, no, &ce, &se); ora_rotate_qu(S, ce, se); ora_rotate_qu(src, ce, se); }
+                    if (emis) { src[0] += (1.0 - a[3]) * a[0] * (double)emis[c]; src[1] += (1.0 - a[3]) * a[1] * (double)emis[c]; }
+                    ora_appA_src(S, a[0], a[1], a[2], src, kr * ds);
+                    if (rot) ora_rotate_qu(S, ce, -se);
+                }
+                if (!advance(m, idx, p, no, ds, axis)) break;
+            }
+            if (st) st->contributions++;
+            for (int s = 0; s < 4; ++s) img[(((int64_t)o * 4 + s) * npy + iy) * npx + ix] += apix * S[s];
         }
     }
 }

@@ -135,6 +135,13 @@ def lib(variant=None):
                                       C.POINTER(OracleStats), C.c_int64, C.c_void_p, C.c_void_p, C.c_void_p,
                                       C.c_void_p]),
         "ora_peel": (None, [C.c_void_p, _dp, _dp, _dp, _dp]),
+        "ora_appA_src": (None, [_dp, C.c_double, C.c_double, C.c_double, _dp, C.c_double]),
+        "ora_segment_integral": (None, [_dp, C.c_double, C.c_double, C.c_double, C.c_double, _dp]),
+        "ora_transport_deposit": (None, [C.c_void_p, C.c_uint64, C.c_uint64, C.c_uint64, C.POINTER(_Events),
+                                         C.POINTER(OracleStats), C.POINTER(Observer), C.c_int, C.c_void_p, C.c_void_p,
+                                         C.POINTER(C.c_uint64)]),
+        "ora_image_rays": (None, [C.c_void_p, C.c_void_p, C.c_void_p, C.POINTER(Observer), C.c_int, C.c_int, C.c_int, _dp,
+                                  C.POINTER(OracleStats)]),
         "ora_image": (None, [C.c_void_p, C.POINTER(_Events), C.POINTER(Observer), C.c_int, C.c_int, C.c_int,
                              C.c_int, _dp, C.c_void_p, C.POINTER(OracleStats)]),
     }
@@ -256,3 +263,33 @@ class OracleModel:
         self.L.ora_image(self.h, C.byref(events.c), arr, n_obs, int(npx), int(npy), int(flags), img,
                         None if img2 is None else img2.ctypes.data, C.byref(st))
         return img, img2, st
+
+    # --- the paper's two-step form (NEXT-1) and thermal emission in the ray step (NEXT-3) ---
+    def transport_deposit(self, id0, n_packets, seed, events, observers, stats=None, collisions=False):
+        """Transport as usual and deposit every path segment: returns (sgrid [ncell, n_obs, 4], coll [ncell] or None, segments)."""
+        st = stats if stats is not None else OracleStats()
+        n_obs = len(observers)
+        arr = (Observer * n_obs)(*observers)
+        ncell = self.nx * self.ny * self.nz
+        sgrid = np.zeros((ncell, n_obs, 4))
+        coll = np.zeros(ncell) if collisions else None
+        nseg = C.c_uint64(0)
+        self.L.ora_transport_deposit(self.h, int(id0), int(n_packets), int(seed), C.byref(events.c), C.byref(st), arr, n_obs,
+                                     sgrid.ctypes.data, None if coll is None else coll.ctypes.data, C.byref(nseg))
+        return sgrid, coll, nseg.value
+
+    def image_rays(self, sgrid, observers, npx, npy, emis=None, stats=None):
+        """One ray per pixel with App. A and source terms (scattering source sgrid and/or thermal emission emis [ncell] f32)."""
+        st = stats if stats is not None else OracleStats()
+        n_obs = len(observers)
+        arr = (Observer * n_obs)(*observers)
+        img = np.zeros((n_obs, 4, npy, npx))
+        if sgrid is not None:
+            sgrid = np.ascontiguousarray(sgrid, np.float64)
+            assert sgrid.size == self.nx * self.ny * self.nz * n_obs * 4
+        if emis is not None:
+            emis = np.ascontiguousarray(np.asarray(emis, np.float32).ravel())
+            assert emis.size == self.nx * self.ny * self.nz
+        self.L.ora_image_rays(self.h, None if sgrid is None else sgrid.ctypes.data, None if emis is None else emis.ctypes.data,
+                              arr, n_obs, int(npx), int(npy), img, C.byref(st))
+        return img, st

@@ -55,7 +55,8 @@ struct krp_grid {
     // imaging order (counting sort of the events by cell bin)
     unsigned int* d_bins = nullptr;
     uint32_t n_bins = 0;
-    int bin_shift = 0, sub_bits = 0;
+    KrpSortGeom sort_geom = { 5, 3, 1, 1 };
+    int sub_bits = 0;
     unsigned int* d_perm = nullptr;
     uint64_t perm_cap = 0;
     void* d_scan = nullptr;
@@ -367,10 +368,22 @@ extern "C" int krp_grid_create(krp_grid** out, int nx, int ny, int nz, const dou
     rc = upload_cells(g, density, bfield, mem, st);
     if (rc) return rc;
     m.kr = g->d_kr; m.cell = g->d_cell;
-    // bins of the imaging order: one cache line of cells per bin (32 x 4 B or 8 x 16 B), at most 2^25 bins
-    g->bin_shift = m.scalar ? 5 : 3;
-    while ((g->npad >> g->bin_shift) >= (1u << 25)) g->bin_shift++;
-    g->n_bins = (g->npad >> g->bin_shift) + 1;
+    // bins of the imaging order: blocks of 32^3 cells, inside a block one cache line of cells along x per bin
+    // (32 x 4 B or 8 x 16 B), at most 2^25 bins
+    {
+        KrpSortGeom& sg = g->sort_geom;
+        sg.B = 5; sg.ls = m.scalar ? 5 : 3;
+        sg.nbx = ((uint32_t)m.px + 31u) >> 5; sg.nby = ((uint32_t)m.py + 31u) >> 5;
+        const uint64_t nblk = (uint64_t)sg.nbx * sg.nby * (((uint32_t)nz + 2u + 31u) >> 5);
+        while (sg.ls < sg.B && (nblk << (3 * sg.B - sg.ls)) >= (1ull << 25)) sg.ls++;
+        if ((nblk << (3 * sg.B - sg.ls)) >= (1ull << 31)) return fail(KRP_ERR_ARG, "grid too large for the imaging order");
+        g->n_bins = (uint32_t)(nblk << (3 * sg.B - sg.ls)) + 1;
+        if (m.scalar) {       // plain cell order, one 128-byte line of cells per bin
+            sg.B = 0; sg.ls = 5;
+            while ((g->npad >> sg.ls) >= (1u << 25)) sg.ls++;
+            g->n_bins = (g->npad >> sg.ls) + 1;
+        }
+    }
     // sub-counters per bin against atomic contention in hot cells.  A grid of few bins (up to 2^17: C1, C2) collects hundreds
     // of events per bin and takes up to 128 counters per bin (four lines, 2^24 counters at most; measured on C2: 16 per bin
     // 0.85 ms, 64 0.86 ms, 128 0.57 ms, 256 0.61 ms); a large grid has a few events per bin and pays for every extra counter in the
@@ -685,10 +698,10 @@ extern "C" int krp_image(krp_grid* g, const krp_observer* obs, int n_obs, int np
     if (g->order_events) {
         CK(cudaMemsetAsync(g->d_bins, 0, sizeof(unsigned int) * ((size_t)g->n_bins + 1), st));
         const int sflags = flags | (g->ev_has_emission ? 0 : 2);       // bit 1: no emission records to look for
-        krp_k_sort_count<<<pers, 256, 0, st>>>(g->d_ctl, g->ev, g->bin_shift, g->sub_bits, sflags, g->d_bins);
+        krp_k_sort_count<<<pers, 256, 0, st>>>(g->m, g->d_ctl, g->ev, g->sort_geom, g->sub_bits, sflags, g->d_bins);
         CK(cub::DeviceScan::ExclusiveSum(g->d_scan, g->scan_bytes, g->d_bins, g->d_bins, (int)(g->n_bins + 1), st));
         krp_k_image_prep<<<1, 1, 0, st>>>(g->d_ctl, g->d_bins, g->n_bins);
-        krp_k_sort_scatter<<<pers, 256, 0, st>>>(g->d_ctl, g->ev, g->bin_shift, g->sub_bits, sflags, g->d_bins, g->d_perm);
+        krp_k_sort_scatter<<<pers, 256, 0, st>>>(g->m, g->d_ctl, g->ev, g->sort_geom, g->sub_bits, sflags, g->d_bins, g->d_perm);
         g->launches += 5;   // count, scan (2 kernels), prep, scatter
     } else {
         krp_k_image_prep_plain<<<1, 1, 0, st>>>(g->d_ctl);

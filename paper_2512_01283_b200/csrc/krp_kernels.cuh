@@ -1033,7 +1033,26 @@ __device__ __forceinline__ void krp_peel(const KrpModel& g, const float n[3], fl
 // fall into the same bin are counted (and given their slots) by one atomic of their first lane (__match_any_sync), on the
 // bin's sub-counter number (group index mod 2^sub_bits): the events next to a point source, which are a large share of
 // every group, would otherwise queue on the one L2 slice that holds their bin's counters.
-__global__ void __launch_bounds__(256) krp_k_sort_count(KrpCtl* ctl, KrpRecords ev, int shift, int sub_bits, int flags,
+// The bins are taken block-major: the grid is cut into blocks of 2^B cells per edge and a bin is one run of 2^ls cells
+// along x inside a block (a 128-byte line of cells), numbered block by block.  The minor order keeps the 32 rays of a
+// warp in neighbouring cells, as before; the major order keeps the rays that are marched at the same time (a few
+// hundred thousand, i.e. the events of a few blocks) inside one beam of cells along the line of sight, a few tens of
+// MB that stay in L2 -- in plain cell order the rays of one z-plane of start cells sweep the whole grid above it and
+// every window of the order streamed the observer's whole coefficient array from DRAM (C5: 228 GB per launch for a
+// 2 GiB array, profiles/r1d).
+struct KrpSortGeom { int B, ls; uint32_t nbx, nby; };
+__device__ __forceinline__ unsigned int krp_sort_bin(const KrpModel& g, const KrpSortGeom& sg, uint32_t cell)
+{
+    if (sg.B == 0) return cell >> sg.ls;       // plain cell order (scalar mode: the 4-byte grid sits in L2 whatever the order)
+    int hx, hy, hz;
+    krp_pad_coords(g, cell, hx, hy, hz);
+    const uint32_t m = (1u << sg.B) - 1u;
+    const uint32_t blk = (((uint32_t)hz >> sg.B) * sg.nby + ((uint32_t)hy >> sg.B)) * sg.nbx + ((uint32_t)hx >> sg.B);
+    const uint32_t in = ((((uint32_t)hz & m) << sg.B) | ((uint32_t)hy & m)) << (sg.B - sg.ls) | (((uint32_t)hx & m) >> sg.ls);
+    return (blk << (3 * sg.B - sg.ls)) | in;
+}
+
+__global__ void __launch_bounds__(256) krp_k_sort_count(KrpModel g, KrpCtl* ctl, KrpRecords ev, KrpSortGeom sg, int sub_bits, int flags,
                                                         unsigned int* __restrict__ bins)
 {
     unsigned long long n_ev = ctl->n_events;
@@ -1046,7 +1065,7 @@ __global__ void __launch_bounds__(256) krp_k_sort_count(KrpCtl* ctl, KrpRecords 
         // emission records take part only with direct light (flags bit 1: the buffer holds none, no need to look)
         bool valid = e < n_ev;
         if (valid && !(flags & 3) && (__float_as_uint(ev.nk[e].w) & ~KRP_TERM_BIT) == 0u) valid = false;
-        const unsigned int bin = valid ? (__float_as_uint(ev.pc[e].w) >> shift) : 0xffffffffu;
+        const unsigned int bin = valid ? krp_sort_bin(g, sg, __float_as_uint(ev.pc[e].w)) : 0xffffffffu;
         const unsigned int peers = __match_any_sync(0xffffffffu, bin);
         if (valid && lane == (unsigned int)(__ffs(peers) - 1))
             atomicAdd(bins + ((bin << sub_bits) | ((unsigned int)(e0 >> 5) & sub_mask)), (unsigned int)__popc(peers));
@@ -1054,7 +1073,7 @@ __global__ void __launch_bounds__(256) krp_k_sort_count(KrpCtl* ctl, KrpRecords 
 }
 
 // after the scan `bins` holds the first slot of every bin; the last thread publishes the total
-__global__ void __launch_bounds__(256) krp_k_sort_scatter(KrpCtl* ctl, KrpRecords ev, int shift, int sub_bits, int flags,
+__global__ void __launch_bounds__(256) krp_k_sort_scatter(KrpModel g, KrpCtl* ctl, KrpRecords ev, KrpSortGeom sg, int sub_bits, int flags,
                                                           unsigned int* __restrict__ bins, unsigned int* __restrict__ perm)
 {
     unsigned long long n_ev = ctl->n_events;
@@ -1066,7 +1085,7 @@ __global__ void __launch_bounds__(256) krp_k_sort_scatter(KrpCtl* ctl, KrpRecord
         const unsigned long long e = e0 + lane;
         bool valid = e < n_ev;
         if (valid && !(flags & 3) && (__float_as_uint(ev.nk[e].w) & ~KRP_TERM_BIT) == 0u) valid = false;
-        const unsigned int bin = valid ? (__float_as_uint(ev.pc[e].w) >> shift) : 0xffffffffu;
+        const unsigned int bin = valid ? krp_sort_bin(g, sg, __float_as_uint(ev.pc[e].w)) : 0xffffffffu;
         const unsigned int peers = __match_any_sync(0xffffffffu, bin);
         const int first = __ffs(peers) - 1;
         unsigned int base = 0u;

@@ -39,18 +39,21 @@ def _report(name, **kw):
 
 
 def _sequences(cfg, ora, gev, ids, name, pure=True, cap=None):
-    """Sequence agreement GPU vs the oracle (bar: >= 99.9 %, north_star), and -- reported, with a looser bar -- GPU vs the
-    pure-fp64-state control build of the oracle (R12)."""
+    """Sequence agreement of the CUDA path with the oracle (bar: >= 99.9 % of packets, north_star).  Reported beside it
+    (R12): its agreement with the pure-fp64-state control build of the oracle, and that of the oracle proper with
+    the control build.  Where those two fall below 1 (media that amplify a last-bit difference of an event position) they
+    fall together: the CUDA path must agree with the control as well as the oracle proper does."""
     frac, info = compare_sequences(ora, gev, ids)
     rec = dict(frac=frac, **show(info))
     if pure:
         ora_p, _, _, _ = oracle_run(cfg, int(ids[0]), len(ids), cap=cap, image=False, variant="pure")
         frac_p, info_p = compare_sequences(ora_p, gev, ids)
-        rec.update(frac_vs_pure=frac_p, fail_vs_pure=info_p["fail"])
+        frac_op, info_op = compare_sequences(ora_p, ora, ids)
+        rec.update(frac_vs_pure=frac_p, fail_vs_pure=info_p["fail"], oracle_vs_pure=frac_op, fail_oracle_vs_pure=info_op["fail"])
     _report(name, **rec)
     assert frac >= 0.999, show(info)
     if pure:
-        assert frac_p >= 0.98, show(info_p)
+        assert frac_p >= frac_op - 0.002, (show(info_p), show(info_op))
     return frac, info
 
 
