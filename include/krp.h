@@ -147,6 +147,31 @@ int krp_image(krp_grid* g, const krp_observer* obs, int n_obs, int npix_x, int n
 int krp_image_get(krp_grid* g, double* out, int mem, void* stream);
 int krp_image_reset(krp_grid* g, void* stream);
 
+/* ---- The paper's own two-step imaging (eq. 11) -------------------------------
+ * Step 1: while a source grid is open, krp_transport also deposits, for every path segment of every flight (not only at
+ * scattering events), the segment's expected scattered Stokes vector toward every camera,
+ * S_pp = Z(Omega_cam; Omega_pp) I_pp (reading R18), into S(Omega_cam, x): fp32, [cell][camera][I,Q,U,V],
+ * reference theta^_cam, including albedo, packet weight and the 1/(4 pi) of the phase matrix, not attenuated, not divided
+ * by the cell volume.  The packets and their scattering events are exactly those of a run without a source grid.
+ * Step 2: krp_image_rays marches ONE ray per pixel through the pixel centre from the far side of the grid toward the
+ * camera and integrates eq. 8 cell by cell with the analytic in-cell solution INCLUDING source terms (App. A,
+ * PAPER.md:296-328): the scattering source S / (V_cell kappa rho) of an open source grid and, when `emis` is given, the
+ * thermal source alpha_abs B of eq. 8 with alpha_abs = (1 - albedo) alpha (reading R19) and B = emis[cell] (array
+ * [nz][ny][nx], `mem` says where it lives; NULL = no thermal emission).  The result, radiance times pixel area (the unit
+ * of krp_image's maps, R14), is ADDED to the maps krp_image_get returns.
+ *   krp_sgrid_begin   opens (allocates and zeroes) the source grid for these cameras (n_obs <= 16); KRP_ERR_OOM if
+ *                     16 bytes x cells x n_obs do not fit.  Synchronises.
+ *   krp_sgrid_get     copies the grid to out ([nz][ny][nx][n_obs][4] floats), parity / debug.  Synchronises for HOST.
+ *   krp_sgrid_reset   zeroes it;  krp_sgrid_end  closes it and frees its memory.
+ *   krp_image_rays    obs must be the cameras of the open source grid (when one is open), else any cameras.
+ * Errors: KRP_ERR_STATE without an open grid (get/reset) or with neither a grid nor emis (image_rays). */
+int krp_sgrid_begin(krp_grid* g, const krp_observer* obs, int n_obs, void* stream);
+int krp_sgrid_get(krp_grid* g, float* out, int mem, void* stream);
+int krp_sgrid_reset(krp_grid* g, void* stream);
+int krp_sgrid_end(krp_grid* g);
+int krp_image_rays(krp_grid* g, const krp_observer* obs, int n_obs, int npix_x, int npix_y, const float* emis, int mem,
+                   void* stream);
+
 /* Counters (also the numerators of the roofline figures). */
 typedef struct krp_stats {
     uint64_t packets;         /* packets emitted */
@@ -157,6 +182,7 @@ typedef struct krp_stats {
     uint64_t contributions;   /* image contributions deposited */
     uint64_t dropped;         /* contributions that fell outside the frame */
     uint64_t overflow;        /* events lost to a full event buffer */
+    uint64_t segments;        /* path segments deposited into an open source grid (two-step form) */
     double w_emitted, w_escaped, w_absorbed, w_cut;
 } krp_stats;
 int krp_stats_get(krp_grid* g, krp_stats* out);  /* synchronises */
@@ -194,7 +220,8 @@ int krp_tune_schedule(krp_grid* g, int dir_sort, int obs_cells, int order_policy
  * krp_timing_get synchronises, adds up the elapsed times since the last call into ms[KRP_T_COUNT] and the
  * launch counts into launches[KRP_T_COUNT] (either may be NULL), and rearms.  At most 4096 launches are kept
  * between two krp_timing_get calls; later ones go untimed. */
-enum { KRP_T_FLIGHT = 0, KRP_T_SCATTER = 1, KRP_T_ORDER = 2, KRP_T_IMAGE = 3, KRP_T_EMIT = 4, KRP_T_COUNT = 5 };
+enum { KRP_T_FLIGHT = 0, KRP_T_SCATTER = 1, KRP_T_ORDER = 2, KRP_T_IMAGE = 3, KRP_T_EMIT = 4, KRP_T_DEPOSIT = 5, KRP_T_RAYS = 6,
+       KRP_T_COUNT = 7 };
 int krp_timing_enable(krp_grid* g, int on);
 int krp_timing_get(krp_grid* g, double* ms, uint64_t* launches);
 

@@ -3,6 +3,7 @@
 // except the one-off table preparation (Theta CDF, observer bases).
 #include "../../include/krp.h"
 #include "krp_kernels.cuh"
+#include "krp_twostep.cuh"
 
 #include <cub/device/device_scan.cuh>
 
@@ -45,7 +46,8 @@ struct krp_grid {
     float* d_stage_b = nullptr;
     int* d_bad = nullptr;
     bool has_bfield = false;
-    bool obs_cells_stale = false;   // cells changed since the per-observer coefficient arrays were built
+    bool obs_cells_stale = false;   // cells changed since the per-observer coefficient arrays were built (or never built)
+    bool obs_cells_failed = false;  // the arrays did not fit for the current observer set
     float4* d_opac = nullptr;
     float4* d_opA = nullptr;
     float4* d_opB = nullptr;
@@ -92,6 +94,14 @@ struct krp_grid {
     int n_obs = 0, npx = 0, npy = 0;
     std::vector<krp_observer> obs_host;
     std::vector<KrpObserverDev> obs_dev;
+    // the paper's two-step form: source grid S(Omega_cam, x), its cameras, per-flight path lengths
+    float* d_sgrid = nullptr;
+    int sg_n_obs = 0;
+    std::vector<krp_observer> sg_obs_host;
+    KrpObserverDev* d_sg_obs = nullptr;
+    double* d_flen = nullptr;
+    uint64_t flen_cap = 0;
+    float* d_emis = nullptr;        // padded thermal source of krp_image_rays
     uint64_t next_id = 0;
     uint64_t launches = 0;
     int max_waves = 0;
@@ -153,6 +163,7 @@ extern "C" int krp_grid_destroy(krp_grid* g)
     cudaFree(g->d_src_cdf); cudaFree(g->d_ctl); cudaFree(g->d_obs); cudaFree(g->d_img); cudaFree(g->d_obs_cells);
     cudaFree(g->d_opA); cudaFree(g->d_opB); cudaFree(g->d_opA_d); cudaFree(g->d_opB_d); cudaFree(g->d_bins); cudaFree(g->d_perm); cudaFree(g->d_scan);
     cudaFree(g->d_dir_bins); cudaFree(g->d_dir_scan); cudaFree(g->d_order);
+    cudaFree(g->d_sgrid); cudaFree(g->d_sg_obs); cudaFree(g->d_flen); cudaFree(g->d_emis);
     free_records(g->q[0]); free_records(g->q[1]); free_records(g->ev);
     for (cudaEvent_t e : g->t_ev) cudaEventDestroy(e);
     if (g->h_ray_stats) cudaFreeHost(g->h_ray_stats);
@@ -529,6 +540,13 @@ extern "C" int krp_transport(krp_grid* g, uint64_t n_packets, uint64_t seed, voi
             CK(cudaMemcpy(&g->d_ctl->ev_cap, &c64, sizeof(c64), cudaMemcpyHostToDevice));
         }
     }
+    if (g->d_sgrid && g->flen_cap < n_packets) {
+        CK(cudaStreamSynchronize(st));
+        cudaFree(g->d_flen); g->d_flen = nullptr; g->flen_cap = 0;
+        CK(cudaMalloc(&g->d_flen, sizeof(double) * n_packets));
+        g->flen_cap = n_packets;
+    }
+    double* flen = g->d_sgrid ? g->d_flen : nullptr;
     const unsigned n = (unsigned)n_packets;
     if (g->m.emit_records) g->ev_has_emission = 1;
     const int tb = g->transport_block;
@@ -582,11 +600,23 @@ extern "C" int krp_transport(krp_grid* g, uint64_t n_packets, uint64_t seed, voi
         krp_k_wave_prep<<<1, 1, 0, st>>>(g->d_ctl, in);
         { TimedLaunch tl(g, st, KRP_T_FLIGHT);
         const KrpEmitSrc es = w == 0 ? es0 : KrpEmitSrc{ nullptr, 0, 0 };
-        if (g->m.scalar && g->burst == 1) krp_k_flight_scalar_static<<<grid_f, tb, 0, st>>>(g->m, g->d_ctl, g->q[in], in, g->ev, es);
+        if (g->m.scalar && (g->burst == 1 || flen)) krp_k_flight_scalar_static<<<grid_f, tb, 0, st>>>(g->m, g->d_ctl, g->q[in], in, g->ev, es, flen);
         else if (g->m.scalar) krp_k_flight_scalar<<<grid_f, tb, (size_t)(tb / 32) * sizeof(KrpWarpShared), st>>>(g->m, g->d_ctl, g->q[in], in, g->ev, g->burst, es);
-        else if (tb <= 128) krp_k_flight_general<128, 5><<<grid_g, tb, 0, st>>>(g->m, g->d_ctl, g->q[in], in, g->ev, g->burst, es);
-        else                krp_k_flight_general<256, 3><<<grid_g, tb, 0, st>>>(g->m, g->d_ctl, g->q[in], in, g->ev, g->burst, es); }
+        else if (tb <= 128) krp_k_flight_general<128, 5><<<grid_g, tb, 0, st>>>(g->m, g->d_ctl, g->q[in], in, g->ev, g->burst, es, flen);
+        else                krp_k_flight_general<256, 3><<<grid_g, tb, 0, st>>>(g->m, g->d_ctl, g->q[in], in, g->ev, g->burst, es, flen); }
         g->launches += 2;
+        if (flen) {
+            // step 1 of the two-step form: the flights of this wave, re-marched over their path lengths, deposit into S
+            TimedLaunch tl(g, st, KRP_T_DEPOSIT);
+            const KrpEmitSrc es = w == 0 ? es0 : KrpEmitSrc{ nullptr, 0, 0 };
+            int G = 1;
+            while (G < g->sg_n_obs && G < 8) G <<= 1;
+            const unsigned need_d = (unsigned)(((uint64_t)n * G + 255u) / 256u);
+            const unsigned grid_d = need_d < pers ? need_d : pers;
+            if (g->m.scalar) krp_k_deposit<true><<<grid_d, 256, 0, st>>>(g->m, g->d_ctl, g->q[in], in, es, flen, g->d_sg_obs, g->sg_n_obs, G, g->d_sgrid, &g->d_ctl->sg_segments);
+            else             krp_k_deposit<false><<<grid_d, 256, 0, st>>>(g->m, g->d_ctl, g->q[in], in, es, flen, g->d_sg_obs, g->sg_n_obs, G, g->d_sgrid, &g->d_ctl->sg_segments);
+            g->launches++;
+        }
         if (w + 1 < g->max_waves) {
             TimedLaunch tl(g, st, KRP_T_SCATTER);
             krp_k_scatter<<<grid_s, 128, 0, st>>>(g->m, g->d_ctl, g->ev, g->q[1 - in], 1 - in, seed);
@@ -608,15 +638,41 @@ static void host_basis(const double n[3], double th[3], double ph[3])
     ph[0] = -sp; ph[1] = cp; ph[2] = 0.0;
 }
 
-extern "C" int krp_image(krp_grid* g, const krp_observer* obs, int n_obs, int npix_x, int npix_y, int flags, void* stream)
+// observer bases and launch constants of one camera
+static KrpObserverDev make_observer_dev(const krp_grid* g, const krp_observer& ob)
 {
-    if (!g) return fail(KRP_ERR_ARG, "grid is NULL");
+    KrpObserverDev od;
+    memset(&od, 0, sizeof(od));
+    double st_ = std::sin(ob.theta), ct_ = std::cos(ob.theta);
+    double n[3] = { st_ * std::cos(ob.phi), st_ * std::sin(ob.phi), ct_ }, th[3], ph[3];
+    host_basis(n, th, ph);
+    for (int a = 0; a < 3; ++a) {
+        od.n[a] = (float)n[a]; od.th[a] = (float)th[a]; od.ph[a] = (float)ph[a];
+        od.thd[a] = th[a]; od.phd[a] = ph[a]; od.center[a] = ob.center[a];
+    }
+    od.inv_hw = 1.0 / ob.half_w; od.inv_hh = 1.0 / ob.half_h;
+    const int strides[3] = { 1, g->m.px, (int)g->m.pxy };
+    for (int a = 0; a < 3; ++a) {
+        const float nf = od.n[a];
+        od.dt[a] = nf != 0.f ? g->m.d[a] / std::fabs(nf) : INFINITY;
+        od.stride[a] = nf > 0.f ? strides[a] : (nf < 0.f ? -strides[a] : 0);
+    }
+    return od;
+}
+
+static int check_observers(const krp_observer* obs, int n_obs, int npix_x, int npix_y)
+{
     if (!obs || n_obs < 1) return fail(KRP_ERR_ARG, "need at least one observer");
     if (npix_x < 1 || npix_y < 1) return fail(KRP_ERR_ARG, "pixel counts must be positive");
     for (int o = 0; o < n_obs; ++o)
         if (!(obs[o].half_w > 0.0) || !(obs[o].half_h > 0.0) || !std::isfinite(obs[o].theta) || !std::isfinite(obs[o].phi))
             return fail(KRP_ERR_ARG, "observer %d: half extents must be positive and angles finite", o);
-    cudaStream_t st = (cudaStream_t)stream;
+    return KRP_OK;
+}
+
+// maps and per-observer data of an observer set (krp_image, krp_image_rays): (re)built when the set or the pixel counts change
+static int setup_maps(krp_grid* g, const krp_observer* obs, int n_obs, int npix_x, int npix_y, cudaStream_t st, bool want_obs_cells)
+{
     bool same = g->d_img && g->n_obs == n_obs && g->npx == npix_x && g->npy == npix_y &&
                 memcmp(g->obs_host.data(), obs, sizeof(krp_observer) * n_obs) == 0;
     if (!same) {
@@ -626,44 +682,37 @@ extern "C" int krp_image(krp_grid* g, const krp_observer* obs, int n_obs, int np
         CK(cudaMalloc(&g->d_img, bytes));
         CK(cudaMemsetAsync(g->d_img, 0, bytes, st));
         std::vector<KrpObserverDev> od(n_obs);
-        for (int o = 0; o < n_obs; ++o) {
-            double st_ = std::sin(obs[o].theta), ct_ = std::cos(obs[o].theta);
-            double n[3] = { st_ * std::cos(obs[o].phi), st_ * std::sin(obs[o].phi), ct_ }, th[3], ph[3];
-            host_basis(n, th, ph);
-            for (int a = 0; a < 3; ++a) {
-                od[o].n[a] = (float)n[a]; od[o].th[a] = (float)th[a]; od[o].ph[a] = (float)ph[a];
-                od[o].thd[a] = th[a]; od[o].phd[a] = ph[a]; od[o].center[a] = obs[o].center[a];
-            }
-            od[o].inv_hw = 1.0 / obs[o].half_w; od[o].inv_hh = 1.0 / obs[o].half_h;
-            const int strides[3] = { 1, g->m.px, (int)g->m.pxy };
-            for (int a = 0; a < 3; ++a) {
-                const float nf = od[o].n[a];
-                od[o].dt[a] = nf != 0.f ? g->m.d[a] / std::fabs(nf) : INFINITY;
-                od[o].stride[a] = nf > 0.f ? strides[a] : (nf < 0.f ? -strides[a] : 0);
-            }
-        }
+        for (int o = 0; o < n_obs; ++o) od[o] = make_observer_dev(g, obs[o]);
         g->obs_dev = od;
         g->obs_host.assign(obs, obs + n_obs);
-        // I0b: per-observer cell coefficients (general mode), when n_obs arrays of 16 B per padded cell fit
         cudaFree(g->d_obs_cells); g->d_obs_cells = nullptr;
-        if (!g->m.scalar && g->obs_pre) {
-            size_t free_b = 0, total_b = 0;
-            CK(cudaMemGetInfo(&free_b, &total_b));
-            const size_t need = sizeof(float4) * (size_t)g->npad * (size_t)n_obs;
-            if (need + (4ull << 30) < free_b && cudaMalloc(&g->d_obs_cells, need) == cudaSuccess) {
-                const unsigned nb = (unsigned)((g->npad + 255u) / 256u);
-                for (int o = 0; o < n_obs; ++o)
-                    krp_k_obs_cells<<<nb, 256, 0, st>>>(g->m, od[o], g->npad, g->d_obs_cells + (size_t)o * g->npad);
-                CK(cudaGetLastError());
-                g->launches += (uint64_t)n_obs;
-                g->obs_cells_stale = false;
-            } else {
-                cudaGetLastError();
-                g->d_obs_cells = nullptr;
-            }
-        }
+        g->obs_cells_failed = false;
         g->n_obs = n_obs; g->npx = npix_x; g->npy = npix_y;
     }
+    // I0b: per-observer cell coefficients (general mode), when n_obs arrays of 16 B per padded cell fit
+    if (want_obs_cells && !g->d_obs_cells && !g->m.scalar && g->obs_pre && !g->obs_cells_failed) {
+        size_t free_b = 0, total_b = 0;
+        CK(cudaMemGetInfo(&free_b, &total_b));
+        const size_t need = sizeof(float4) * (size_t)g->npad * (size_t)n_obs;
+        if (need + (4ull << 30) < free_b && cudaMalloc(&g->d_obs_cells, need) == cudaSuccess) {
+            g->obs_cells_stale = true;
+        } else {
+            cudaGetLastError();
+            g->d_obs_cells = nullptr;
+            g->obs_cells_failed = true;      // not retried until the observer set changes
+        }
+    }
+    return KRP_OK;
+}
+
+extern "C" int krp_image(krp_grid* g, const krp_observer* obs, int n_obs, int npix_x, int npix_y, int flags, void* stream)
+{
+    if (!g) return fail(KRP_ERR_ARG, "grid is NULL");
+    int rc = check_observers(obs, n_obs, npix_x, npix_y);
+    if (rc) return rc;
+    cudaStream_t st = (cudaStream_t)stream;
+    rc = setup_maps(g, obs, n_obs, npix_x, npix_y, st, true);
+    if (rc) return rc;
     if (g->d_obs_cells && g->obs_cells_stale) {
         // the cells changed (krp_grid_update) since the coefficient arrays were built
         const unsigned nb = (unsigned)((g->npad + 255u) / 256u);
@@ -790,6 +839,7 @@ extern "C" int krp_stats_get(krp_grid* g, krp_stats* out)
     out->packets = c.stats.packets; out->events = c.stats.events; out->records = c.stats.records;
     out->steps_transport = c.stats.steps_transport; out->steps_image = c.stats.steps_image;
     out->contributions = c.stats.contributions; out->dropped = c.stats.dropped; out->overflow = c.stats.overflow;
+    out->segments = c.sg_segments;
     out->w_emitted = c.stats.w_emitted; out->w_escaped = c.stats.w_escaped;
     out->w_absorbed = c.stats.w_absorbed; out->w_cut = c.stats.w_cut;
     return overflow_code(g, c);
@@ -799,6 +849,7 @@ extern "C" int krp_stats_reset(krp_grid* g, void* stream)
 {
     if (!g) return fail(KRP_ERR_ARG, "grid is NULL");
     CK(cudaMemsetAsync(&g->d_ctl->stats, 0, sizeof(KrpStatsDev), (cudaStream_t)stream));
+    CK(cudaMemsetAsync(&g->d_ctl->sg_segments, 0, sizeof(unsigned long long), (cudaStream_t)stream));
     return KRP_OK;
 }
 
@@ -901,6 +952,122 @@ extern "C" int krp_tune_schedule(krp_grid* g, int dir_sort, int obs_cells, int o
     if (dir_sort >= 0) g->dir_sort = dir_sort;
     if (obs_cells >= 0 && obs_cells != g->obs_pre) { g->obs_pre = obs_cells; g->obs_host.clear(); }   // rebuilt at the next krp_image
     if (order_policy >= 0) { g->order_policy = order_policy; g->order_events = order_policy != 0; g->ray_stats_pending = false; }
+    return KRP_OK;
+}
+
+// ------------------------------------------------------------------------------------------
+// the paper's two-step form (include/krp.h)
+// ------------------------------------------------------------------------------------------
+extern "C" int krp_sgrid_end(krp_grid* g)
+{
+    if (!g) return fail(KRP_ERR_ARG, "grid is NULL");
+    CK(cudaDeviceSynchronize());
+    cudaFree(g->d_sgrid); g->d_sgrid = nullptr;
+    cudaFree(g->d_sg_obs); g->d_sg_obs = nullptr;
+    g->sg_n_obs = 0; g->sg_obs_host.clear();
+    return KRP_OK;
+}
+
+extern "C" int krp_sgrid_begin(krp_grid* g, const krp_observer* obs, int n_obs, void* stream)
+{
+    if (!g) return fail(KRP_ERR_ARG, "grid is NULL");
+    int rc = check_observers(obs, n_obs, 1, 1);
+    if (rc) return rc;
+    if (n_obs > KRP_SG_MAX_OBS) return fail(KRP_ERR_ARG, "a source grid holds at most %d cameras", KRP_SG_MAX_OBS);
+    cudaStream_t st = (cudaStream_t)stream;
+    rc = krp_sgrid_end(g);
+    if (rc) return rc;
+    const size_t bytes = sizeof(float) * 4 * (size_t)g->npad * (size_t)n_obs;
+    if (cudaMalloc(&g->d_sgrid, bytes) != cudaSuccess) {
+        cudaGetLastError(); g->d_sgrid = nullptr;
+        return fail(KRP_ERR_OOM, "source grid of %zu bytes does not fit", bytes);
+    }
+    CK(cudaMemsetAsync(g->d_sgrid, 0, bytes, st));
+    std::vector<KrpObserverDev> od(n_obs);
+    for (int o = 0; o < n_obs; ++o) od[o] = make_observer_dev(g, obs[o]);
+    CK(cudaMalloc(&g->d_sg_obs, sizeof(KrpObserverDev) * n_obs));
+    CK(cudaMemcpyAsync(g->d_sg_obs, od.data(), sizeof(KrpObserverDev) * n_obs, cudaMemcpyHostToDevice, st));
+    CK(cudaStreamSynchronize(st));
+    g->sg_n_obs = n_obs;
+    g->sg_obs_host.assign(obs, obs + n_obs);
+    return KRP_OK;
+}
+
+extern "C" int krp_sgrid_reset(krp_grid* g, void* stream)
+{
+    if (!g) return fail(KRP_ERR_ARG, "grid is NULL");
+    if (!g->d_sgrid) return fail(KRP_ERR_STATE, "no source grid is open");
+    CK(cudaMemsetAsync(g->d_sgrid, 0, sizeof(float) * 4 * (size_t)g->npad * (size_t)g->sg_n_obs, (cudaStream_t)stream));
+    return KRP_OK;
+}
+
+extern "C" int krp_sgrid_get(krp_grid* g, float* out, int mem, void* stream)
+{
+    if (!g || !out) return fail(KRP_ERR_ARG, "grid or out is NULL");
+    if (!g->d_sgrid) return fail(KRP_ERR_STATE, "no source grid is open");
+    if (mem != KRP_MEM_DEVICE && mem != KRP_MEM_HOST) return fail(KRP_ERR_ARG, "mem must be KRP_MEM_DEVICE or KRP_MEM_HOST");
+    cudaStream_t st = (cudaStream_t)stream;
+    const size_t n4 = (size_t)g->m.ncell * (size_t)g->sg_n_obs;
+    float4* tmp = nullptr;
+    float4* dst = (float4*)out;
+    if (mem == KRP_MEM_HOST) { CK(cudaMalloc(&tmp, sizeof(float4) * n4)); dst = tmp; }
+    krp_k_sgrid_unpad<<<(unsigned)((n4 + 255) / 256), 256, 0, st>>>(g->m, (const float4*)g->d_sgrid, g->sg_n_obs, dst);
+    g->launches++;
+    cudaError_t e = cudaGetLastError();
+    if (e == cudaSuccess && mem == KRP_MEM_HOST) {
+        e = cudaMemcpyAsync(out, tmp, sizeof(float4) * n4, cudaMemcpyDeviceToHost, st);
+        if (e == cudaSuccess) e = cudaStreamSynchronize(st);
+    }
+    cudaFree(tmp);
+    if (e != cudaSuccess) return fail(KRP_ERR_CUDA, "krp_sgrid_get: %s", cudaGetErrorString(e));
+    return KRP_OK;
+}
+
+extern "C" int krp_image_rays(krp_grid* g, const krp_observer* obs, int n_obs, int npix_x, int npix_y, const float* emis, int mem,
+                              void* stream)
+{
+    if (!g) return fail(KRP_ERR_ARG, "grid is NULL");
+    int rc = check_observers(obs, n_obs, npix_x, npix_y);
+    if (rc) return rc;
+    if (!g->d_sgrid && !emis) return fail(KRP_ERR_STATE, "krp_image_rays needs an open source grid or a thermal source");
+    if (emis && mem != KRP_MEM_DEVICE && mem != KRP_MEM_HOST) return fail(KRP_ERR_ARG, "mem must be KRP_MEM_DEVICE or KRP_MEM_HOST");
+    if (g->d_sgrid && (n_obs != g->sg_n_obs || memcmp(g->sg_obs_host.data(), obs, sizeof(krp_observer) * n_obs) != 0))
+        return fail(KRP_ERR_ARG, "the observers must be the cameras of the open source grid");
+    if ((size_t)npix_x * npix_y >= (1ull << 31)) return fail(KRP_ERR_ARG, "too many pixels");
+    cudaStream_t st = (cudaStream_t)stream;
+    rc = setup_maps(g, obs, n_obs, npix_x, npix_y, st, false);
+    if (rc) return rc;
+    const float* d_em = nullptr;
+    if (emis) {
+        // the caller's [nz][ny][nx] array into the padded order of the cells
+        if (!g->d_emis) CK(cudaMalloc(&g->d_emis, sizeof(float) * (size_t)g->npad));
+        const float* src = emis;
+        float* stage = nullptr;
+        if (mem == KRP_MEM_HOST) {
+            CK(cudaMalloc(&stage, sizeof(float) * (size_t)g->m.ncell));
+            CK(cudaMemcpyAsync(stage, emis, sizeof(float) * (size_t)g->m.ncell, cudaMemcpyHostToDevice, st));
+            src = stage;
+        }
+        krp_k_pad_scalar<<<(unsigned)((g->npad + 255u) / 256u), 256, 0, st>>>(g->m, src, g->npad, g->d_emis);
+        g->launches++;
+        if (stage) { CK(cudaStreamSynchronize(st)); cudaFree(stage); }
+        d_em = g->d_emis;
+    }
+    const int npix = npix_x * npix_y;
+    for (int o = 0; o < n_obs; ++o) {
+        KrpRayObs ro;
+        const double st_ = std::sin(obs[o].theta), ct_ = std::cos(obs[o].theta);
+        const double n[3] = { st_ * std::cos(obs[o].phi), st_ * std::sin(obs[o].phi), ct_ };
+        double th[3], ph[3];
+        host_basis(n, th, ph);
+        for (int a = 0; a < 3; ++a) { ro.n[a] = n[a]; ro.th[a] = th[a]; ro.ph[a] = ph[a]; ro.center[a] = obs[o].center[a]; }
+        ro.half_w = obs[o].half_w; ro.half_h = obs[o].half_h;
+        TimedLaunch tl(g, st, KRP_T_RAYS);
+        if (g->m.scalar) krp_k_image_rays<true><<<(npix + 127) / 128, 128, 0, st>>>(g->m, g->d_ctl, ro, o, n_obs, npix_x, npix_y, g->d_sgrid, d_em, g->d_img);
+        else             krp_k_image_rays<false><<<(npix + 127) / 128, 128, 0, st>>>(g->m, g->d_ctl, ro, o, n_obs, npix_x, npix_y, g->d_sgrid, d_em, g->d_img);
+        g->launches++;
+    }
+    CK(cudaGetLastError());
     return KRP_OK;
 }
 

@@ -92,6 +92,7 @@ struct KrpCtl {
     unsigned int work[2];          // dynamic work counters of the flight kernels
     unsigned int n_sorted;         // events in the sorted order of the current imaging pass
     unsigned int img_work[KRP_MAX_OBS_PACK];   // per-observer warp-tile counters of the imaging pass
+    unsigned long long sg_segments;            // path segments deposited into the source grid (two-step form)
     KrpStatsDev stats;
 };
 
@@ -225,6 +226,23 @@ __device__ __forceinline__ void krp_event_pos(const KrpModel& g, const float n[3
         double x = (double)p0[a] + (double)n[a] * s * g.inv_dd[a] - (double)(h[a] - h0[a]);
         pe[a] = (float)fmin(fmax(x, 0.0), 1.0);
     }
+}
+
+// path length of a flight from its start (cell c0, local p0) to its event (cell c, local pe), fp64: what the flight
+// kernels hand to the deposit step of the two-step form (krp_twostep.cuh)
+__device__ __forceinline__ double krp_path_length(const KrpModel& g, const float n[3], const float p0[3], uint32_t c0,
+                                                  const float pe[3], uint32_t c)
+{
+    int h0[3], h[3];
+    krp_pad_coords(g, c0, h0[0], h0[1], h0[2]);
+    krp_pad_coords(g, c, h[0], h[1], h[2]);
+    double s = 0.0, nn = 0.0;
+#pragma unroll
+    for (int a = 0; a < 3; ++a) {
+        s += (double)n[a] * ((double)(h[a] - h0[a]) + ((double)pe[a] - (double)p0[a])) * g.dd[a];
+        nn += (double)n[a] * (double)n[a];
+    }
+    return s / nn;
 }
 
 // The same re-based march with the distances in fp64: used by the general-mode flight, where the optical

@@ -431,7 +431,7 @@ __global__ void __launch_bounds__(256, 3) krp_k_flight_scalar(KrpModel g, KrpCtl
 // The same flight with a static assignment (one queue entry per thread and grid stride, the warp's 32 flights
 // start and are closed together): no refill logic at all.  Cheaper when flights are short (C2: a point source
 // inside a dense ring, most flights end within a few cells), selected with flight_burst = 1.
-__global__ void __launch_bounds__(256, 4) krp_k_flight_scalar_static(KrpModel g, KrpCtl* ctl, KrpRecords q, int in, KrpRecords ev, KrpEmitSrc es)
+__global__ void __launch_bounds__(256, 4) krp_k_flight_scalar_static(KrpModel g, KrpCtl* ctl, KrpRecords q, int in, KrpRecords ev, KrpEmitSrc es, double* __restrict__ flen)
 {
     const unsigned int n_items = ctl->q_count[in];
     KrpFlightTally tl = { 0, 0, 0, 0.0, 0.0, 0.0 };
@@ -470,11 +470,16 @@ __global__ void __launch_bounds__(256, 4) krp_k_flight_scalar_static(KrpModel g,
         krp_pad_coords(g, c0, h0[0], h0[1], h0[2]);
         krp_pad_coords(g, c_cur, h1[0], h1[1], h1[2]);
         const int crossings = abs(h1[0] - h0[0]) + abs(h1[1] - h0[1]) + abs(h1[2] - h0[2]);
-        if (!hit) { tl.steps += (unsigned long long)crossings; tl.w_esc += (double)S0.x; continue; }
+        if (!hit) {
+            tl.steps += (unsigned long long)crossings; tl.w_esc += (double)S0.x;
+            if (flen) flen[item] = __longlong_as_double(0x7ff0000000000000ll);       // two-step form: deposit to the grid edge
+            continue;
+        }
         tl.steps += (unsigned long long)(crossings + 1);
         const double moved = D / ((double)g.a1c * (double)kr_cur);
         float pe[3];
         krp_event_pos(g, n, p0, c0, c_cur, ax_cur, moved, pe);
+        if (flen) flen[item] = krp_path_length(g, n, p0, c0, pe, c_cur);
         krp_event_append(g, ctl, ev, id, c_cur, pe, n, __float_as_uint(nk.w), S0.x, g.omc, S0.y, S0.z, S0.w, tl);
     }
     krp_tally_flush(tl, ctl);
@@ -665,7 +670,7 @@ __device__ __forceinline__ void krp_appA_to_d(double i, double qg, double ug, do
 // Two builds: blocks of up to 128 threads, five per SM (20 warps, 96 registers: the default, measured best of 16, 18, 20, 24 and 32
 // warps per SM on C4 and C5) and blocks of up to 256 threads, three per SM (24 warps, 80 registers) for krp_tune's larger blocks.
 template <int TPB, int MINB>
-__global__ void __launch_bounds__(TPB, MINB) krp_k_flight_general(KrpModel g, KrpCtl* ctl, KrpRecords q, int in, KrpRecords ev, int n_burst, KrpEmitSrc es)
+__global__ void __launch_bounds__(TPB, MINB) krp_k_flight_general(KrpModel g, KrpCtl* ctl, KrpRecords q, int in, KrpRecords ev, int n_burst, KrpEmitSrc es, double* __restrict__ flen)
 {
     const unsigned int n_items = ctl->q_count[in];
     KrpFlightTally tl = { 0, 0, 0, 0.0, 0.0, 0.0 };
@@ -714,10 +719,12 @@ __global__ void __launch_bounds__(TPB, MINB) krp_k_flight_general(KrpModel g, Kr
             pe[1] = krp_locald(n[1], ray.ry, g.inv_dd[1], moved, pc.y);
             pe[2] = krp_locald(n[2], ray.rz, g.inv_dd[2], moved, pc.z);
             tl.steps += nsteps;
+            if (flen) { const float p0[3] = { pc.x, pc.y, pc.z }; flen[item] = krp_path_length(g, n, p0, __float_as_uint(pc.w), pe, ray.c); }
             krp_event_append(g, ctl, ev, id_, ray.c, pe, n, __float_as_uint(nk.w), S0_.x, cc.omega,
                              (float)qs, (float)us, (float)vs, tl);
             status = KRP_IDLE;
         } else if (status == KRP_ESC) {
+            if (flen) flen[item] = __longlong_as_double(0x7ff0000000000000ll);
             tl.steps += nsteps;
             tl.w_esc += es.order ? 1.0 : (double)q.S[item].x;
             status = KRP_IDLE;
@@ -972,7 +979,11 @@ __device__ __forceinline__ void krp_rot_qu_f(float& Q, float& U, float ce, float
     Q = q; U = u;
 }
 
-__device__ __forceinline__ void krp_peel(const KrpModel& g, const float n[3], float4 Se, const KrpObserverDev& ob, float S[4])
+// The geometry of one peel-off, which depends on the incoming direction and the observer only: rotation of the Stokes
+// reference into the scattering plane (cos, sin of twice the angle), F(Theta_obs) times 1/(4 pi), rotation to theta^_obs.
+struct KrpPeelGeom { float c2i, s2i, F[4], c2o, s2o; };
+
+__device__ __forceinline__ void krp_peel_setup(const KrpModel& g, const float n[3], const KrpObserverDev& ob, KrpPeelGeom& pg)
 {
     // spherical basis of n (eq. 4-5, R10) and the unit normal of the scattering plane with the hardware reciprocal
     // square root (2 ulp): this runs once per (event, observer), and IEEE divisions and square roots were a fifth of it
@@ -995,26 +1006,42 @@ __device__ __forceinline__ void krp_peel(const KrpModel& g, const float n[3], fl
     else { const float r = rsqrtf(ss); sn = ss * r; sh[0] *= r; sh[1] *= r; sh[2] *= r; }
     // e_par = s^ x n_in: reference of the incoming ray in the scattering plane
     float ep[3] = { sh[1] * n[2] - sh[2] * n[1], sh[2] * n[0] - sh[0] * n[2], sh[0] * n[1] - sh[1] * n[0] };
-    float I = Se.x, Q = Se.x * Se.y, U = Se.x * Se.z, V = Se.x * Se.w;
-    krp_rot_qu_f(Q, U, th[0] * ep[0] + th[1] * ep[1] + th[2] * ep[2], ph[0] * ep[0] + ph[1] * ep[1] + ph[2] * ep[2]);
+    {
+        const float ce = th[0] * ep[0] + th[1] * ep[1] + th[2] * ep[2], se = ph[0] * ep[0] + ph[1] * ep[1] + ph[2] * ep[2];
+        pg.c2i = ce * ce - se * se; pg.s2i = 2.f * se * ce;
+    }
     // scattering angle from atan2(|n x n_obs|, n.n_obs): well conditioned at both poles
     // (in units of the table spacing: the Mueller row is linear in it, R13)
     const float x = atan2f(sn, mu) * g.nang1_over_pi;
-    float F[4];
     {
         const int j = max(0, min((int)x, g.n_ang - 2));
         const float w = x - (float)j, w0 = 1.f - w;
         const float4 a = g.mueller[j], b = g.mueller[j + 1];
-        F[0] = w0 * a.x + w * b.x; F[1] = w0 * a.y + w * b.y; F[2] = w0 * a.z + w * b.z; F[3] = w0 * a.w + w * b.w;
+        const float c = 0.07957747154594767f;   // 1/(4 pi)
+        pg.F[0] = c * (w0 * a.x + w * b.x); pg.F[1] = c * (w0 * a.y + w * b.y); pg.F[2] = c * (w0 * a.z + w * b.z); pg.F[3] = c * (w0 * a.w + w * b.w);
     }
-    float I2 = F[0] * I + F[1] * Q, Q2 = F[1] * I + F[0] * Q;
-    float U2 = F[2] * U + F[3] * V, V2 = -F[3] * U + F[2] * V;
     // e_out = s^ x n_obs, then to theta^_obs
     float eo[3] = { sh[1] * ob.n[2] - sh[2] * ob.n[1], sh[2] * ob.n[0] - sh[0] * ob.n[2], sh[0] * ob.n[1] - sh[1] * ob.n[0] };
-    krp_rot_qu_f(Q2, U2, eo[0] * ob.th[0] + eo[1] * ob.th[1] + eo[2] * ob.th[2],
-                 ob.th[0] * sh[0] + ob.th[1] * sh[1] + ob.th[2] * sh[2]);
-    const float c = 0.07957747154594767f;   // 1/(4 pi)
-    S[0] = c * I2; S[1] = c * Q2; S[2] = c * U2; S[3] = c * V2;
+    {
+        const float ce = eo[0] * ob.th[0] + eo[1] * ob.th[1] + eo[2] * ob.th[2], se = ob.th[0] * sh[0] + ob.th[1] * sh[1] + ob.th[2] * sh[2];
+        pg.c2o = ce * ce - se * se; pg.s2o = 2.f * se * ce;
+    }
+}
+
+// (I,Q,U,V) in the lab reference of the incoming direction -> Stokes vector sent toward the observer, reference theta^_obs
+__device__ __forceinline__ void krp_peel_apply(const KrpPeelGeom& pg, float I, float Q, float U, float V, float S[4])
+{
+    const float q = pg.c2i * Q + pg.s2i * U, u = -pg.s2i * Q + pg.c2i * U;
+    const float I2 = pg.F[0] * I + pg.F[1] * q, Q2 = pg.F[1] * I + pg.F[0] * q;
+    const float U2 = pg.F[2] * u + pg.F[3] * V, V2 = -pg.F[3] * u + pg.F[2] * V;
+    S[0] = I2; S[1] = pg.c2o * Q2 + pg.s2o * U2; S[2] = -pg.s2o * Q2 + pg.c2o * U2; S[3] = V2;
+}
+
+__device__ __forceinline__ void krp_peel(const KrpModel& g, const float n[3], float4 Se, const KrpObserverDev& ob, float S[4])
+{
+    KrpPeelGeom pg;
+    krp_peel_setup(g, n, ob, pg);
+    krp_peel_apply(pg, Se.x, Se.x * Se.y, Se.x * Se.z, Se.x * Se.w, S);
 }
 
 // ------------------------------------------------------------------------------------------
@@ -1155,12 +1182,15 @@ __device__ __forceinline__ void krp_appA_delta_thin(float x, float y, float i, f
 // reciprocal out of the march and halves its traffic through the L1 data pipe (profiles/: the shared-memory
 // table reads were 49 % of that pipe on C5).  Used when n_obs such arrays fit in device memory.
 // ------------------------------------------------------------------------------------------
+// Encoding of the first component: >= 0  kappa*rho*alpha1 of a cell the march may treat with the short series (thin for
+// every possible segment: max(|kappa rho alpha2|, |kappa rho alpha3|) x cell diagonal < 0.1); finite and < 0  minus that value
+// for a cell that needs the full in-cell solution; -inf  halo.  The march's hot loop then runs on one sign test per cell.
 __global__ void __launch_bounds__(256) krp_k_obs_cells(KrpModel g, const KrpObserverDev ob, uint32_t npad, float4* __restrict__ out)
 {
     const uint32_t c = blockIdx.x * blockDim.x + threadIdx.x;
     if (c >= npad) return;
     const float4 cl = g.cell[c];
-    float4 o = make_float4(cl.x, 0.f, 0.f, 0.f);
+    float4 o = make_float4(cl.x < 0.f ? -KRP_INF_F : cl.x, 0.f, 0.f, 0.f);
     if (cl.x > 0.f) {
         const int nseg = g.n_inc - 1;
         const float mu = fminf(fabsf(ob.n[0] * cl.y + ob.n[1] * cl.z + ob.n[2] * cl.w), 1.f);
@@ -1174,6 +1204,8 @@ __global__ void __launch_bounds__(256) krp_k_obs_cells(KrpModel g, const KrpObse
         o.y = cl.x * fmaf(tb.y, x, ta.y);
         o.z = cl.x * fmaf(tb.z, x, ta.z);
         o.w = aa + bb < 1e-24f ? 0.f : atan2f(2.f * a * b, aa - bb);   // cos 2eta ~ a^2 - b^2, sin 2eta ~ 2ab (R2)
+        const float diag = sqrtf(g.d[0] * g.d[0] + g.d[1] * g.d[1] + g.d[2] * g.d[2]);
+        if (fmaxf(fabsf(o.y), fabsf(o.z)) * diag >= 0.1f) o.x = -o.x;
     }
     out[c] = o;
 }
@@ -1291,35 +1323,46 @@ __global__ void __launch_bounds__(256, SCALAR ? KRP_IMAGE_SCALAR_MIN_BLOCKS : KR
                 r.c = c_n;                                 // the halo cell that ended the ray
                 A = g.a1c * tau;
             } else if (PRE) {
-                // march over the observer's own coefficient array {kr a1, kr a2, kr a3, 2 eta}
+                // march over the observer's own coefficient array {kr a1 (sign: thin / thick / halo), kr a2, kr a3, 2 eta}
                 float i = S[0], qs = S[1], us = S[2], vs = S[3];
                 float4 cl = __ldg(obs_cell + r.c);
+                for (;;) {
+                    // hot loop: cells that are thin whatever the segment (also empty ones: the update is then the identity)
 #pragma unroll 2
-                do {
-                    const float ds = krp_raya_step(r, rc);
-                    const float4 cn = __ldg(obs_cell + r.c);    // next cell, in flight during the update below
-                    if (cl.x > 0.f) {
+                    while (cl.x >= 0.f) {
+                        const float ds = krp_raya_step(r, rc);
+                        const float4 cn = __ldg(obs_cell + r.c);    // next cell, in flight during the update below
                         const float xx = cl.y * ds, yy = cl.z * ds;
                         float s2, c2;
                         __sincosf(cl.w, &s2, &c2);
                         const float qg = c2 * qs + s2 * us, ug = c2 * us - s2 * qs;   // eq. 7
-                        if (fmaxf(fabsf(xx), fabsf(yy)) < 0.1f) {
-                            float di, dqg, dug, dv;
-                            krp_appA_delta_thin(xx, yy, i, qg, ug, vs, di, dqg, dug, dv);
-                            i += di; vs += dv;
-                            qs += c2 * dqg - s2 * dug;
-                            us += s2 * dqg + c2 * dug;
-                            A = fmaf(cl.x, ds, A);
-                        } else {
-                            float qg2 = qg, ug2 = ug, vg2 = vs, di, i_new, depth;
-                            krp_appA(i, qg2, ug2, vg2, make_float4(cl.x, cl.y, cl.z, 0.f), ds, di, i_new, depth);
-                            i = i_new; A += depth; vs = vg2;
-                            qs = c2 * qg2 - s2 * ug2; us = s2 * qg2 + c2 * ug2;
-                            if (A > 104.f) { cl = cn; break; }      // e^{-A} is exactly 0 in fp32 from here on
-                        }
+                        // delta form S += R(-eta) dP R(eta) S with the two-term series (|xx|, |yy| < 0.1), written as chains of
+                        // FFMAs: 16 for the update, the increments never materialised
+                        const float x2 = xx * xx, y2 = yy * yy;
+                        const float sh = fmaf(xx * x2, 1.f / 6.f, xx), chm1 = x2 * fmaf(x2, 1.f / 24.f, 0.5f);
+                        const float sy = fmaf(yy * y2, -1.f / 6.f, yy), cym1 = y2 * fmaf(y2, 1.f / 24.f, -0.5f);
+                        const float dqg = fmaf(qg, chm1, -(i * sh)), dug = fmaf(ug, cym1, -(vs * sy));
+                        i = fmaf(-qg, sh, fmaf(i, chm1, i));
+                        vs = fmaf(ug, sy, fmaf(vs, cym1, vs));
+                        qs = fmaf(c2, dqg, fmaf(-s2, dug, qs));
+                        us = fmaf(s2, dqg, fmaf(c2, dug, us));
+                        A = fmaf(cl.x, ds, A);
+                        cl = cn;
                     }
-                    cl = cn;
-                } while (cl.x >= 0.f);
+                    if (cl.x == -KRP_INF_F) break;              // halo: the ray has left the grid
+                    {   // a cell that may be thick: full in-cell solution
+                        const float ds = krp_raya_step(r, rc);
+                        const float4 cn = __ldg(obs_cell + r.c);
+                        float s2, c2;
+                        __sincosf(cl.w, &s2, &c2);
+                        float qg2 = c2 * qs + s2 * us, ug2 = c2 * us - s2 * qs, vg2 = vs, di, i_new, depth;
+                        krp_appA(i, qg2, ug2, vg2, make_float4(-cl.x, cl.y, cl.z, 0.f), ds, di, i_new, depth);
+                        i = i_new; A += depth; vs = vg2;
+                        qs = c2 * qg2 - s2 * ug2; us = s2 * qg2 + c2 * ug2;
+                        cl = cn;
+                        if (A > 104.f) break;                   // e^{-A} is exactly 0 in fp32 from here on
+                    }
+                }
                 S[0] = i; S[1] = qs; S[2] = us; S[3] = vs;
             } else {
                 float i = S[0], qs = S[1], us = S[2], vs = S[3];

@@ -18,9 +18,10 @@ SYMBOLS = [
     "krp_events_reserve", "krp_transport", "krp_packet_id_set", "krp_image", "krp_image_get",
     "krp_image_reset", "krp_stats_get", "krp_stats_reset", "krp_events_get", "krp_events_select", "krp_events_clear",
     "krp_tune", "krp_tune_schedule", "krp_timing_enable", "krp_timing_get", "krp_launch_count",
+    "krp_sgrid_begin", "krp_sgrid_get", "krp_sgrid_reset", "krp_sgrid_end", "krp_image_rays",
 ]
-T_FLIGHT, T_SCATTER, T_ORDER, T_IMAGE, T_EMIT, T_COUNT = 0, 1, 2, 3, 4, 5
-T_NAMES = ("flight", "scatter", "order", "image", "emit")
+T_FLIGHT, T_SCATTER, T_ORDER, T_IMAGE, T_EMIT, T_DEPOSIT, T_RAYS, T_COUNT = 0, 1, 2, 3, 4, 5, 6, 7
+T_NAMES = ("flight", "scatter", "order", "image", "emit", "deposit", "rays")
 
 
 class KrpError(RuntimeError):
@@ -46,7 +47,7 @@ class Observer(C.Structure):
 
 class Stats(C.Structure):
     _fields_ = [(n, C.c_uint64) for n in ("packets", "events", "records", "steps_transport", "steps_image",
-                                          "contributions", "dropped", "overflow")] + \
+                                          "contributions", "dropped", "overflow", "segments")] + \
                [(n, C.c_double) for n in ("w_emitted", "w_escaped", "w_absorbed", "w_cut")]
 
     def as_dict(self):
@@ -102,6 +103,11 @@ def lib():
         "krp_timing_get": (i32, [vp, vp, vp]),
         "krp_tune_schedule": (i32, [vp, i32, i32, i32]),
         "krp_launch_count": (u64, [vp]),
+        "krp_sgrid_begin": (i32, [vp, C.POINTER(Observer), i32, vp]),
+        "krp_sgrid_get": (i32, [vp, vp, i32, vp]),
+        "krp_sgrid_reset": (i32, [vp, vp]),
+        "krp_sgrid_end": (i32, [vp]),
+        "krp_image_rays": (i32, [vp, C.POINTER(Observer), i32, i32, i32, vp, i32, vp]),
     }
     for name, (res, args) in sig.items():
         f = getattr(L, name)
@@ -266,6 +272,34 @@ class Grid:
 
     def events_clear(self, stream=None):
         _check(lib().krp_events_clear(self._h, _stream(stream)))
+
+    # --- the paper's two-step form ---
+    def sgrid_begin(self, observers, stream=None):
+        n = len(observers)
+        arr = (Observer * n)(*observers)
+        _check(lib().krp_sgrid_begin(self._h, arr, n, _stream(stream)))
+        self._sg_n_obs = n
+
+    def sgrid_get(self, stream=None):
+        """Source grid as a numpy array [nz, ny, nx, n_obs, 4] (fp32)."""
+        nx, ny, nz = self.shape
+        out = np.empty((nz, ny, nx, self._sg_n_obs, 4), np.float32)
+        _check(lib().krp_sgrid_get(self._h, C.c_void_p(out.ctypes.data), MEM_HOST, _stream(stream)))
+        return out
+
+    def sgrid_reset(self, stream=None):
+        _check(lib().krp_sgrid_reset(self._h, _stream(stream)))
+
+    def sgrid_end(self):
+        _check(lib().krp_sgrid_end(self._h))
+
+    def image_rays(self, observers, npix_x, npix_y, emis=None, stream=None):
+        n = len(observers)
+        arr = (Observer * n)(*observers)
+        eptr, emem, keep = _ptr_mem(emis)
+        _check(lib().krp_image_rays(self._h, arr, n, int(npix_x), int(npix_y), eptr, MEM_DEVICE if emem is None else emem,
+                                    _stream(stream)))
+        self.n_obs, self.npx, self.npy = n, int(npix_x), int(npix_y)
 
     def tune(self, transport_block=0, image_block=0, blocks_per_sm=0, flight_burst=0):
         _check(lib().krp_tune(self._h, int(transport_block), int(image_block), int(blocks_per_sm), int(flight_burst)))
