@@ -60,6 +60,10 @@ def parse_args():
     ap.add_argument("--workload", default="c5", choices=["c1", "c2", "c3", "c4", "c5"])
     ap.add_argument("--batch", type=int, default=0, help="packets per step and GPU (0 = workload default)")
     ap.add_argument("--n", type=int, default=0, help="override the grid size (testing only; marks the line reduced)")
+    ap.add_argument("--form", default="events", choices=["events", "twostep"],
+                    help="events: the north_star's form (per-event imaging, the contract's metric); twostep: the paper's own form "
+                         "(every segment deposited into S(Omega_cam, x), one ray per pixel at the end of the timed steps)")
+    ap.add_argument("--tune", default="", help="measurement only: transport_block,image_block,blocks_per_sm,flight_burst for krp_tune (0 keeps)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
@@ -314,6 +318,8 @@ def run_krp(args):
     weight = None if w_host is None else torch.from_numpy(np.ascontiguousarray(w_host, np.float32).ravel()).to(dev)
     obs = [krp.make_observer(o["theta"], o["phi"], o["center"], o["half_w"], o["half_h"]) for o in cfg["observers"]]
     g = make_grid(krp, cfg, dens, bf, weight)
+    if args.tune:
+        g.tune(*[int(x) for x in args.tune.split(",")])
 
     # pilot (untimed): events per packet of this workload, to size the event buffer once
     pilot = min(batch, 1 << 16)
@@ -331,6 +337,10 @@ def run_krp(args):
     E = lambda: torch.cuda.Event(enable_timing=True)
     marks = [(E(), E(), E()) for _ in range(args.steps)]
 
+    twostep = args.form == "twostep"
+    if twostep:
+        g.sgrid_begin(obs)
+
     def step(i, mark=None):
         first, cnt = shard.step_id_range(i, rank, world, batch)
         g.packet_id_set(first)
@@ -340,7 +350,10 @@ def run_krp(args):
         g.transport(cnt, seed)
         if mark:
             mark[1].record()
-        g.image(obs, npix, npix)
+        if twostep:
+            g.events_clear()               # the paper's form does not use the event buffer
+        else:
+            g.image(obs, npix, npix)
         if mark:
             mark[2].record()
 
@@ -357,6 +370,8 @@ def run_krp(args):
     t_start.record()
     for i in range(args.steps):
         step(args.warmup + i, marks[i])
+    if twostep:
+        g.image_rays(obs, npix, npix)      # step 2 of the paper's form, once for all packets of the timed steps
     t_end.record()
     barrier()
     clocks = sampler.stop() if sampler else None
@@ -407,6 +422,10 @@ def run_krp(args):
     kernels = {}
     for cls, (ms, n_l) in timing.items():
         kernels[cls] = {"ms_per_step": ms / K, "launches_per_step": n_l / K, "share_of_step": ms / ms_own}
+    if twostep:
+        work["image"] = dict(kernel="krp_k_deposit", steps=st["segments"], bytes=st["segments"] * (A["cell_bytes"] + 32 * n_obs),
+                             inst=st["segments"] * 150)
+        timing = dict(timing, image=timing["deposit"])
     dom = max(("image", "flight"), key=lambda c: timing[c][0])
     per_class = {}
     for cls in ("image", "flight"):
@@ -515,7 +534,7 @@ def main():
         return run_reference(args)
     r = run_krp(args)
     r["grid"].close()
-    e2e = None if args.no_e2e else run_e2e(args, r)
+    e2e = None if (args.no_e2e or args.form == "twostep") else run_e2e(args, r)
     if r["world"] > 1:
         import torch.distributed as dist
         dist.barrier()
@@ -533,7 +552,7 @@ def main():
         "dtype": ("f32 march with f64 optical depth, f64 image sums" if r["mode"] == "scalar"
                   else "f64 flights (event location), f32 imaging march, f64 image sums"), "data": "synthetic",
         "config": {"workload": cfg["name"], "grid": [cfg["nx"], cfg["ny"], cfg["nz"]], "packets_per_step_per_gpu": r["batch"],
-                   "observers": len(cfg["observers"]), "npix": cfg["npix"], "cell_layout": r["mode"],
+                   "observers": len(cfg["observers"]), "npix": cfg["npix"], "cell_layout": r["mode"], "form": args.form,
                    "job_packets": cfg["n_packets"], "events_per_packet": r["epp"],
                    "l2": "flushed every step by a 256 MiB memset inside the timed region",
                    "launch": "flights: %s; imaging: one launch per observer over events ordered by cell bin" %

@@ -77,6 +77,7 @@ struct krp_grid {
     KrpCtl* d_ctl = nullptr;
     KrpRecords q[2] = {};
     uint64_t q_cap = 0;
+    KrpHits hits = {};              // general mode: hit queue of the current wave (capacity q_cap)
     KrpRecords ev = {};
     uint64_t ev_cap = 0;
     bool ev_reserved = false;
@@ -140,6 +141,22 @@ extern "C" const char* krp_last_error(void) { return g_err; }
 #endif
 extern "C" const char* krp_version(void) { return "krp 0.2 sm_100a " KRP_BUILD_ID; }
 
+static void free_hits(KrpHits& h)
+{
+    cudaFree(h.ic); cudaFree(h.Di); cudaFree(h.qu); cudaFree(h.vr); cudaFree(h.ryz);
+    h = KrpHits{};
+}
+
+static int alloc_hits(KrpHits& h, uint64_t cap)
+{
+    CK(cudaMalloc(&h.ic, cap * sizeof(uint2)));
+    CK(cudaMalloc(&h.Di, cap * sizeof(double2)));
+    CK(cudaMalloc(&h.qu, cap * sizeof(double2)));
+    CK(cudaMalloc(&h.vr, cap * sizeof(double2)));
+    CK(cudaMalloc(&h.ryz, cap * sizeof(double2)));
+    return KRP_OK;
+}
+
 static void free_records(KrpRecords& r)
 {
     cudaFree(r.pc); cudaFree(r.nk); cudaFree(r.S); cudaFree(r.tau); cudaFree(r.id);
@@ -164,7 +181,7 @@ extern "C" int krp_grid_destroy(krp_grid* g)
     cudaFree(g->d_opA); cudaFree(g->d_opB); cudaFree(g->d_opA_d); cudaFree(g->d_opB_d); cudaFree(g->d_bins); cudaFree(g->d_perm); cudaFree(g->d_scan);
     cudaFree(g->d_dir_bins); cudaFree(g->d_dir_scan); cudaFree(g->d_order);
     cudaFree(g->d_sgrid); cudaFree(g->d_sg_obs); cudaFree(g->d_flen); cudaFree(g->d_emis);
-    free_records(g->q[0]); free_records(g->q[1]); free_records(g->ev);
+    free_records(g->q[0]); free_records(g->q[1]); free_records(g->ev); free_hits(g->hits);
     for (cudaEvent_t e : g->t_ev) cudaEventDestroy(e);
     if (g->h_ray_stats) cudaFreeHost(g->h_ray_stats);
     if (g->ray_stats_ev) cudaEventDestroy(g->ray_stats_ev);
@@ -519,10 +536,14 @@ extern "C" int krp_transport(krp_grid* g, uint64_t n_packets, uint64_t seed, voi
     cudaStream_t st = (cudaStream_t)stream;
     if (g->q_cap < n_packets) {
         CK(cudaStreamSynchronize(st));
-        free_records(g->q[0]); free_records(g->q[1]); g->q_cap = 0;
+        free_records(g->q[0]); free_records(g->q[1]); free_hits(g->hits); g->q_cap = 0;
         for (int s = 0; s < 2; ++s) {
             int rc = alloc_records(g->q[s], n_packets, true);
             if (rc) { free_records(g->q[0]); free_records(g->q[1]); return rc; }
+        }
+        if (!g->m.scalar) {
+            int rc = alloc_hits(g->hits, n_packets);
+            if (rc) { free_records(g->q[0]); free_records(g->q[1]); free_hits(g->hits); return rc; }
         }
         g->q_cap = n_packets;
     }
@@ -602,8 +623,13 @@ extern "C" int krp_transport(krp_grid* g, uint64_t n_packets, uint64_t seed, voi
         const KrpEmitSrc es = w == 0 ? es0 : KrpEmitSrc{ nullptr, 0, 0 };
         if (g->m.scalar && (g->burst == 1 || flen)) krp_k_flight_scalar_static<<<grid_f, tb, 0, st>>>(g->m, g->d_ctl, g->q[in], in, g->ev, es, flen);
         else if (g->m.scalar) krp_k_flight_scalar<<<grid_f, tb, (size_t)(tb / 32) * sizeof(KrpWarpShared), st>>>(g->m, g->d_ctl, g->q[in], in, g->ev, g->burst, es);
-        else if (tb <= 128) krp_k_flight_general<128, 5><<<grid_g, tb, 0, st>>>(g->m, g->d_ctl, g->q[in], in, g->ev, g->burst, es, flen);
-        else                krp_k_flight_general<256, 3><<<grid_g, tb, 0, st>>>(g->m, g->d_ctl, g->q[in], in, g->ev, g->burst, es, flen); }
+        else {
+            if (tb <= 128) krp_k_flight_general<128, 5><<<grid_g, tb, 0, st>>>(g->m, g->d_ctl, g->q[in], in, g->hits, g->burst, es, flen);
+            else           krp_k_flight_general<256, 3><<<grid_g, tb, 0, st>>>(g->m, g->d_ctl, g->q[in], in, g->hits, g->burst, es, flen);
+            // the flights that reached their event cell: event location, record, albedo weighting, all lanes busy
+            krp_k_event_general<<<grid_s, 128, 0, st>>>(g->m, g->d_ctl, g->q[in], in, g->hits, g->ev, es, flen);
+            g->launches++;
+        } }
         g->launches += 2;
         if (flen) {
             // step 1 of the two-step form: the flights of this wave, re-marched over their path lengths, deposit into S

@@ -93,6 +93,7 @@ struct KrpCtl {
     unsigned int n_sorted;         // events in the sorted order of the current imaging pass
     unsigned int img_work[KRP_MAX_OBS_PACK];   // per-observer warp-tile counters of the imaging pass
     unsigned long long sg_segments;            // path segments deposited into the source grid (two-step form)
+    unsigned int n_hits;                       // general mode: flights of the current wave that ended in an event (hit queue fill)
     KrpStatsDev stats;
 };
 
@@ -103,6 +104,16 @@ struct KrpRecords {
     float4* S;                  // {W, q, u, v}: weight and normalised Stokes, lab reference of n
     double* tau;                // queue only: optical depth to the next event
     unsigned long long* id;     // global packet id
+};
+
+// general mode: what a marching lane leaves behind when its flight reaches the cell of its event -- the state at the
+// entry of that cell.  A converged kernel (krp_k_event_general) locates the event and writes the record.
+struct KrpHits {
+    uint2* ic;                  // {queue item, padded cell id}
+    double2* Di;                // {scalar depth still to go D, normalised intensity i}
+    double2* qu;                // {q, u} lab reference
+    double2* vr;                // {v, distance to the next x face}
+    double2* ryz;               // {distance to the next y face, to the next z face}
 };
 
 struct KrpObserverDev {

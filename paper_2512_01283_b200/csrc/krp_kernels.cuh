@@ -158,6 +158,7 @@ __global__ void krp_k_wave_prep(KrpCtl* ctl, int in)
     ctl->ev_begin = ctl->n_events;
     ctl->q_count[1 - in] = 0;
     ctl->work[0] = 0;
+    ctl->n_hits = 0;
 }
 
 
@@ -670,7 +671,7 @@ __device__ __forceinline__ void krp_appA_to_d(double i, double qg, double ug, do
 // Two builds: blocks of up to 128 threads, five per SM (20 warps, 96 registers: the default, measured best of 16, 18, 20, 24 and 32
 // warps per SM on C4 and C5) and blocks of up to 256 threads, three per SM (24 warps, 80 registers) for krp_tune's larger blocks.
 template <int TPB, int MINB>
-__global__ void __launch_bounds__(TPB, MINB) krp_k_flight_general(KrpModel g, KrpCtl* ctl, KrpRecords q, int in, KrpRecords ev, int n_burst, KrpEmitSrc es, double* __restrict__ flen)
+__global__ void __launch_bounds__(TPB, MINB) krp_k_flight_general(KrpModel g, KrpCtl* ctl, KrpRecords q, int in, KrpHits hits, int n_burst, KrpEmitSrc es, double* __restrict__ flen)
 {
     const unsigned int n_items = ctl->q_count[in];
     KrpFlightTally tl = { 0, 0, 0, 0.0, 0.0, 0.0 };
@@ -688,40 +689,17 @@ __global__ void __launch_bounds__(TPB, MINB) krp_k_flight_general(KrpModel g, Kr
     float4 cl = make_float4(0.f, 0.f, 0.f, 1.f), cl_f = cl;
     bool fresh = false;
     for (;;) {
-        // refill point: the lanes whose flight ended during the last burst close it together
+        // refill point: a lane whose flight reached the cell of its event leaves the entry state in the hit queue (one
+        // reservation for all such lanes of the warp) -- event location, record and albedo weighting run in their own,
+        // fully converged kernel (krp_k_event_general) instead of inside the marching warp
         if (status == KRP_HIT) {
-            // the state is that of the entry into the event cell: solve for t, evolve to t, normalise to I = 1 (R7)
-            const double ds = krp_rayd_ds(ray);
-            KrpCellCoef cc;
-            krp_cell_coef(g, cl, nd, xs, ds, cc);
-            const double R = D + log(i);
-            double moved;
-            if (cc.a2 == 0.0 && cc.a3 == 0.0) {
-                moved = (R / cc.a1) / (double)cl.x;
-                const double inv = 1.0 / i;
-                qs *= inv; us *= inv; vs *= inv;
-            } else {
-                const double bx = cl.y, by = cl.z, bz = cl.w;
-                double c2, s2;
-                krp_eta2_d(th[0] * bx + th[1] * by + th[2] * bz, ph[0] * bx + ph[1] * by, c2, s2);      // phi^_z = 0
-                const double qg_e = c2 * qs + s2 * us, ug_e = -s2 * qs + c2 * us;
-                const double t = krp_event_solve_d(R, qg_e / i, cc.a1, cc.a2, cc.dtau);
-                double qt, ut, vt;
-                krp_appA_to_d(i, qg_e, ug_e, vs, cc.a2, cc.a3, t, qt, ut, vt);
-                qs = c2 * qt - s2 * ut; us = s2 * qt + c2 * ut; vs = vt;
-                moved = t / (double)cl.x;
-            }
-            float4 pc, nk, S0_; double tau_; unsigned long long id_;
-            krp_item_load(g, q, es, item, pc, nk, S0_, tau_, id_);
-            const float n[3] = { nk.x, nk.y, nk.z };
-            float pe[3];
-            pe[0] = krp_locald(n[0], ray.rx, g.inv_dd[0], moved, pc.x);
-            pe[1] = krp_locald(n[1], ray.ry, g.inv_dd[1], moved, pc.y);
-            pe[2] = krp_locald(n[2], ray.rz, g.inv_dd[2], moved, pc.z);
+            const unsigned int slot = krp_reserve32(&ctl->n_hits);
+            hits.ic[slot] = make_uint2(item, ray.c);
+            hits.Di[slot] = make_double2(D, i);
+            hits.qu[slot] = make_double2(qs, us);
+            hits.vr[slot] = make_double2(vs, ray.rx);
+            hits.ryz[slot] = make_double2(ray.ry, ray.rz);
             tl.steps += nsteps;
-            if (flen) { const float p0[3] = { pc.x, pc.y, pc.z }; flen[item] = krp_path_length(g, n, p0, __float_as_uint(pc.w), pe, ray.c); }
-            krp_event_append(g, ctl, ev, id_, ray.c, pe, n, __float_as_uint(nk.w), S0_.x, cc.omega,
-                             (float)qs, (float)us, (float)vs, tl);
             status = KRP_IDLE;
         } else if (status == KRP_ESC) {
             if (flen) flen[item] = __longlong_as_double(0x7ff0000000000000ll);
@@ -783,13 +761,25 @@ __global__ void __launch_bounds__(TPB, MINB) krp_k_flight_general(KrpModel g, Kr
                     double i_new, qg, ug, vg, depth;
                     krp_appA_d(i, qg_e, ug_e, vs, cc, i_new, qg, ug, vg, depth);
                     const double Dn = D - depth;
-                    // ln i >= u - u^2 for u = i - 1 in [-1/2, 0] (and >= 0 above): the fp64 log, which a warp would execute
-                    // for the one or two lanes that are near their event, is taken only when this bound does not already
-                    // rule the event out
+                    // The event test is ln i_new + Dn <= 0.  The fp64 log (~110 instructions, which a warp would execute for the
+                    // one or two lanes that are near their event: 27 % of all warp-steps on C4, profiles/r2g) is bracketed first:
+                    // for |u| <= 1/4, u = i_new - 1, the series P4 = u - u^2/2 + u^3/3 - u^4/4 has |ln(1+u) - P4| <= |u|^5/(5 (1 - |u|))
+                    // <= 4/15 |u|^5, so the decision is settled unless P4 + Dn lies within that band of zero -- only then the log itself
                     if (near_end) {
                         const double u = i_new - 1.0;
-                        const double lb = u >= 0.0 ? 0.0 : (u >= -0.5 ? u - u * u : -1e300);
-                        if (lb + Dn <= 0.0 && log(i_new) + Dn <= 0.0) { status = KRP_HIT; continue; }   // state stays at cell entry
+                        bool hit;
+                        if (fabs(u) <= 0.25) {
+                            const double u2 = u * u;
+                            const double p4 = u + u2 * (-0.5 + u * (1.0 / 3.0 - 0.25 * u));
+                            const double band = (4.0 / 15.0) * u2 * u2 * fabs(u);
+                            const double v = p4 + Dn;
+                            if (v > band) hit = false;
+                            else if (v < -band) hit = true;
+                            else hit = log(i_new) + Dn <= 0.0;
+                        } else {
+                            hit = log(i_new) + Dn <= 0.0;
+                        }
+                        if (hit) { status = KRP_HIT; continue; }   // state stays at cell entry
                     }
                     qs = c2 * qg - s2 * ug; us = s2 * qg + c2 * ug; vs = vg;
                     i = i_new; D = Dn;
@@ -805,6 +795,80 @@ __global__ void __launch_bounds__(TPB, MINB) krp_k_flight_general(KrpModel g, Kr
     }
     krp_tally_flush(tl, ctl);
 }
+// T4/T5, general mode: one thread per flight that ended in an event.  From the state at the entry of the event cell:
+// solve for the depth t of the event (krp_event_solve_d), evolve the Stokes vector to t and normalise it to I = 1 (R7),
+// place the event, write the record (slot = first event of the wave + hit index: coalesced, no atomic), weight by the albedo.
+__global__ void __launch_bounds__(128) krp_k_event_general(KrpModel g, KrpCtl* ctl, KrpRecords q, int in, KrpHits hits, KrpRecords ev,
+                                                           KrpEmitSrc es, double* __restrict__ flen)
+{
+    const unsigned int n_hits = ctl->n_hits;
+    const unsigned long long ev_begin = ctl->ev_begin, ev_cap = ctl->ev_cap;
+    KrpFlightTally tl = { 0, 0, 0, 0.0, 0.0, 0.0 };
+    for (unsigned int h = blockIdx.x * blockDim.x + threadIdx.x; h < n_hits; h += gridDim.x * blockDim.x) {
+        const uint2 ic = hits.ic[h];
+        const double2 Di = hits.Di[h], qu = hits.qu[h], vr = hits.vr[h], ryz = hits.ryz[h];
+        const unsigned int item = ic.x; const uint32_t cell = ic.y;
+        const double D = Di.x, i = Di.y;
+        double qs = qu.x, us = qu.y, vs = vr.x;
+        const double rx = vr.y, ry = ryz.x, rz = ryz.y;
+        float4 pc, nk, S0; double tau_; unsigned long long id;
+        krp_item_load(g, q, es, item, pc, nk, S0, tau_, id);
+        const float n[3] = { nk.x, nk.y, nk.z };
+        // the flight's direction constants, exactly as the marching kernel set them up
+        double nd[3] = { n[0], n[1], n[2] }, th[3], ph[3];
+        krp_basis_unit_d(nd, th, ph);
+        {
+            const double inv_n = krp_rsqrt_near1(nd[0] * nd[0] + nd[1] * nd[1] + nd[2] * nd[2]);
+            nd[0] *= inv_n; nd[1] *= inv_n; nd[2] *= inv_n;
+        }
+        const float4 cl = g.cell[cell];
+        const double ds = fmin(rx, fmin(ry, rz));
+        KrpCellCoef cc;
+        krp_cell_coef(g, cl, nd, g.xs, ds, cc);
+        const double R = D + log(i);
+        double moved;
+        if (cc.a2 == 0.0 && cc.a3 == 0.0) {
+            moved = (R / cc.a1) / (double)cl.x;
+            const double inv = 1.0 / i;
+            qs *= inv; us *= inv; vs *= inv;
+        } else {
+            const double bx = cl.y, by = cl.z, bz = cl.w;
+            double c2, s2;
+            krp_eta2_d(th[0] * bx + th[1] * by + th[2] * bz, ph[0] * bx + ph[1] * by, c2, s2);      // phi^_z = 0
+            const double qg_e = c2 * qs + s2 * us, ug_e = -s2 * qs + c2 * us;
+            const double t = krp_event_solve_d(R, qg_e / i, cc.a1, cc.a2, cc.dtau);
+            double qt, ut, vt;
+            krp_appA_to_d(i, qg_e, ug_e, vs, cc.a2, cc.a3, t, qt, ut, vt);
+            qs = c2 * qt - s2 * ut; us = s2 * qt + c2 * ut; vs = vt;
+            moved = t / (double)cl.x;
+        }
+        float pe[3];
+        pe[0] = krp_locald(n[0], rx, g.inv_dd[0], moved, pc.x);
+        pe[1] = krp_locald(n[1], ry, g.inv_dd[1], moved, pc.y);
+        pe[2] = krp_locald(n[2], rz, g.inv_dd[2], moved, pc.z);
+        if (flen) { const float p0[3] = { pc.x, pc.y, pc.z }; flen[item] = krp_path_length(g, n, p0, __float_as_uint(pc.w), pe, cell); }
+        // T5: record, albedo weighting, termination (R12)
+        const float W = S0.x, Wn = cc.omega * W;
+        const uint32_t kn = __float_as_uint(nk.w) + 1u;
+        const bool term = (Wn < g.w_min) || ((int)kn >= g.max_scatter);
+        tl.w_abs += (double)W - (double)Wn;
+        const unsigned long long slot = ev_begin + h;
+        if (slot < ev_cap) {
+            ev.pc[slot] = make_float4(pe[0], pe[1], pe[2], __uint_as_float(cell));
+            ev.nk[slot] = make_float4(n[0], n[1], n[2], __uint_as_float(kn | (term ? KRP_TERM_BIT : 0u)));
+            ev.S[slot] = make_float4(Wn, (float)qs, (float)us, (float)vs);
+            ev.id[slot] = id;
+            ++tl.n_ev;
+            if (term) tl.w_cut += (double)Wn;
+        } else {
+            ++tl.n_over;
+            tl.w_cut += (double)Wn;
+        }
+    }
+    if (blockIdx.x == 0 && threadIdx.x == 0) atomicAdd(&ctl->n_events, (unsigned long long)n_hits);   // may run past ev_cap: clamped by the readers
+    krp_tally_flush(tl, ctl);
+}
+
 // ------------------------------------------------------------------------------------------
 // quaternion helpers (eq. 1-3): q = (w, a);  q* v q  and  q v q*  for a pure
 // quaternion v, expanded from the Hamilton product:  v -+ 2w (a x v) + 2 a x (a x v).
