@@ -237,7 +237,15 @@ typedef struct ora_model {
     double src_pos[3], src_dir[3];
     double* src_cdf;      /* owned, [ncell] running sum of cell weights, or NULL */
     int64_t src_cell; int src_idx[3]; double src_p[3];
+    int periodic;         /* bit a set: axis a is periodic, reading R20 */
 } ora_model;
+
+/* Periodic boundary conditions (the cylinder test: "our use of periodic boundary conditions").
+ * Reading R20: a packet or an imaging ray that leaves through a face of a periodic axis re-enters through the opposite
+ * face at the same cell-local position; after ORA_MAX_WRAPS such crossings it counts as having left the grid (a ray
+ * that runs parallel to the open faces of an empty periodic box would never end). */
+#define ORA_MAX_WRAPS 4096
+void ora_model_set_periodic(ora_model* m, int mask) { m->periodic = mask & 7; }
 
 void ora_model_free(ora_model* m)
 {
@@ -371,7 +379,7 @@ double ora_dda_exit(const ora_model* m, const double p[3], const double n[3], in
 
 /* move ds along n inside the cell; if axis >= 0 also cross that face.
  * Returns 0 when the packet leaves the grid. */
-static int advance(const ora_model* m, int idx[3], double p[3], const double n[3], double ds, int axis)
+static int advance_w(const ora_model* m, int idx[3], double p[3], const double n[3], double ds, int axis, int* wraps)
 {
     int nn[3] = { m->nx, m->ny, m->nz };
     for (int a = 0; a < 3; ++a) {
@@ -383,9 +391,17 @@ static int advance(const ora_model* m, int idx[3], double p[3], const double n[3
     if (axis >= 0) {
         if (n[axis] > 0) { idx[axis] += 1; p[axis] = 0.0; }
         else             { idx[axis] -= 1; p[axis] = 1.0; }
-        if (idx[axis] < 0 || idx[axis] >= nn[axis]) return 0;
+        if (idx[axis] < 0 || idx[axis] >= nn[axis]) {
+            if (!((m->periodic >> axis) & 1) || !wraps || *wraps >= ORA_MAX_WRAPS) return 0;
+            ++*wraps;                                                  /* R20 */
+            idx[axis] = idx[axis] < 0 ? nn[axis] - 1 : 0;
+        }
     }
     return 1;
+}
+static int advance(const ora_model* m, int idx[3], double p[3], const double n[3], double ds, int axis)
+{
+    return advance_w(m, idx, p, n, ds, axis, NULL);
 }
 
 static int64_t cell_of(const ora_model* m, const int idx[3])
@@ -420,6 +436,7 @@ int64_t ora_march(const ora_model* m, const int idx0[3], const double p0[3], con
     int idx[3] = { idx0[0], idx0[1], idx0[2] };
     double p[3] = { p0[0], p0[1], p0[2] };
     int64_t steps = 0;
+    int wraps = 0;
     for (;;) {
         int axis; double ds = ora_dda_exit(m, p, n, &axis);
         int64_t c = cell_of(m, idx);
@@ -427,7 +444,7 @@ int64_t ora_march(const ora_model* m, const int idx0[3], const double p0[3], con
         ++steps;
         double kr = m->kr[c];
         if (kr > 0) { double b[3]; cell_bhat(m, c, b); ora_cell_step(m, b, n, S, kr * ds); }
-        if (!advance(m, idx, p, n, ds, axis)) break;
+        if (!advance_w(m, idx, p, n, ds, axis, &wraps)) break;
     }
     return steps;
 }
@@ -565,6 +582,7 @@ static int flight(const ora_model* m, int idx[3], double p[3], const double n[3]
                   double tau_star, ora_stats* st, struct ora_deposit* dep, double W)
 {
     double target = exp(-tau_star);
+    int wraps = 0;
     for (;;) {
         int axis; double ds = ora_dda_exit(m, p, n, &axis);
         int64_t c = cell_of(m, idx);
@@ -614,7 +632,7 @@ static int flight(const ora_model* m, int idx[3], double p[3], const double n[3]
                 for (int s = 0; s < 4; ++s) S[s] = So[s];
             }
         }
-        if (!advance(m, idx, p, n, ds, axis)) return 0;
+        if (!advance_w(m, idx, p, n, ds, axis, &wraps)) return 0;
     }
 }
 
@@ -923,16 +941,18 @@ void ora_image_rays(const ora_model* m, const double* sgrid, const float* emis, 
             double s_in = -INFINITY, s_out = INFINITY; int miss = 0;
             for (int a = 0; a < 3; ++a) {
                 double lo = m->lo[a], hi = m->lo[a] + nn[a] * m->d[a];
+                if ((m->periodic >> a) & 1) continue;                     /* R20: a periodic axis does not clip the line ... */
                 if (no[a] == 0.0) { if (x0[a] < lo || x0[a] >= hi) miss = 1; continue; }
                 double t0 = (lo - x0[a]) / no[a], t1 = (hi - x0[a]) / no[a];
                 if (t0 > t1) { double t = t0; t0 = t1; t1 = t; }
                 if (t0 > s_in) s_in = t0;
                 if (t1 < s_out) s_out = t1;
             }
-            if (miss || !(s_in < s_out)) continue;
+            if (miss || !(s_in < s_out) || s_in == -INFINITY) continue;
             int idx[3]; double p[3];
             for (int a = 0; a < 3; ++a) {
                 double x = (x0[a] + s_in * no[a] - m->lo[a]) / m->d[a];
+                if ((m->periodic >> a) & 1) x -= floor(x / nn[a]) * nn[a];  /* ... its coordinate is taken modulo the box */
                 int i = (int)floor(x);
                 if (i < 0) i = 0;
                 if (i > nn[a] - 1) i = nn[a] - 1;
@@ -940,6 +960,7 @@ void ora_image_rays(const ora_model* m, const double* sgrid, const float* emis, 
                 idx[a] = i; p[a] = f < 0 ? 0 : (f > 1 ? 1 : f);
             }
             double S[4] = { 0, 0, 0, 0 };
+            int wraps = 0;
             for (;;) {
                 int axis; double ds = ora_dda_exit(m, p, no, &axis);
                 int64_t c = cell_of(m, idx);
@@ -957,7 +978,7 @@ void ora_image_rays(const ora_model* m, const double* sgrid, const float* emis, 
                     ora_appA_src(S, a[0], a[1], a[2], src, kr * ds);
                     if (rot) ora_rotate_qu(S, ce, -se);
                 }
-                if (!advance(m, idx, p, no, ds, axis)) break;
+                if (!advance_w(m, idx, p, no, ds, axis, &wraps)) break;
             }
             if (st) st->contributions++;
             for (int s = 0; s < 4; ++s) img[(((int64_t)o * 4 + s) * npy + iy) * npx + ix] += apix * S[s];

@@ -121,6 +121,7 @@ def lib(variant=None):
         "ora_model_create": (C.c_void_p, [C.c_int, C.c_int, C.c_int, _dp, C.c_void_p, C.c_void_p,
                                           C.c_int, _fp, C.c_int, _fp, C.c_double, C.c_int]),
         "ora_model_free": (None, [C.c_void_p]),
+        "ora_model_set_periodic": (None, [C.c_void_p, C.c_int]),
         "ora_source_set": (None, [C.c_void_p, C.c_int, _dp, _dp, C.c_void_p, C.c_int]),
         "ora_mueller_at": (None, [C.c_void_p, C.c_double, _dp]),
         "ora_opac_at": (None, [C.c_void_p, C.c_double, _dp]),
@@ -186,6 +187,10 @@ class OracleModel:
         if getattr(self, "h", None):
             self.L.ora_model_free(self.h)
             self.h = None
+
+    def set_periodic(self, mask):
+        """bit a of mask: axis a (0 x, 1 y, 2 z) is periodic (reading R20)."""
+        self.L.ora_model_set_periodic(self.h, int(mask))
 
     def source_set(self, kind, pos, direction, cell_weight=None, emit_records=0):
         """kind bit0: volume (else point at pos); bit1: collimated along direction (else isotropic)."""

@@ -261,3 +261,80 @@ def test_two_step_image_equals_event_image_in_expectation():
     assert np.all(err < 0.02 * ref)
     assert np.abs(tot_g.mean(0)[:, 1:3]).max() > 0.05 * ref[:, 0].max()                        # a polarised case
     assert np.all(np.abs(map_g - map_e) < 0.06 * map_e + 0.01 * map_e.max())
+
+
+# ----------------------------------------------------------------------------
+# NEXT-3: periodic boundaries, reading R20
+# ----------------------------------------------------------------------------
+def test_periodic_box_is_an_infinite_slab():
+    """Periodic in x and y, open in z: an isotropic point source in the mid-plane of a uniform pure absorber of half
+    depth tau escapes with probability int_0^1 e^{-tau/mu} dmu = E_2(tau) (scipy.special.expn); the open box loses
+    packets through its sides and gives more.  A source moved by a fraction of the box gives the same events up to the shift."""
+    import scipy.special
+    tau, N = 1.5, 100000
+    m = box_model((8, 8, 8), 2 * tau, opac=const_opac(1, 0, 0, 0.0))      # kappa rho = 2 tau per unit length, half height 1/2
+    m.source_set(0, [0.5, 0.5, 0.5], [0, 0, 1], None, 0)
+    ev = OracleEvents(2 * N)
+    st_open, _ = m.transport(0, N, 6, ev)
+    m.set_periodic(3)
+    ev = OracleEvents(2 * N)
+    st_per, _ = m.transport(0, N, 6, ev)
+    want = float(scipy.special.expn(2, tau))
+    assert abs(st_per.w_escaped / N - want) < 4 * math.sqrt(want * (1 - want) / N)
+    assert st_open.w_escaped / N > want + 0.05
+    # translation by (3/8, -2/8, 0) of the source in the periodic box: same packets, same depths, cells shifted modulo the box
+    m.source_set(0, [0.5 + 3 / 8, 0.5 - 2 / 8, 0.5], [0, 0, 1], None, 0)
+    ev2 = OracleEvents(2 * N)
+    st2, _ = m.transport(0, N, 6, ev2)
+    assert ev2.n == ev.n and st2.w_escaped == st_per.w_escaped and st2.steps_transport == st_per.steps_transport
+    c1, c2 = ev.cell[:ev.n], ev2.cell[:ev.n]
+    x1, y1, z1 = c1 % 8, (c1 // 8) % 8, c1 // 64
+    assert np.array_equal((x1 + 3) % 8, c2 % 8) and np.array_equal((y1 - 2) % 8, (c2 // 8) % 8) and np.array_equal(z1, c2 // 64)
+    assert np.allclose(ev.p[:ev.n], ev2.p[:ev.n], atol=1e-6)
+
+
+def test_periodic_march_wraps_and_ends_at_the_open_faces():
+    """An oblique ray in a box periodic in x only: the logged cells wrap in x, the segments add up to the chord to the
+    nearest open face (y or z), the optical depth is kappa rho times that chord; fully periodic and parallel to every open
+    face it ends after ORA_MAX_WRAPS crossings."""
+    kr = float(np.float32(0.7))                                              # densities reach the oracle as fp32
+    m = box_model((5, 4, 6), kr, opac=const_opac(1, 0, 0, 0.5), bounds=(0, 5, 0, 4, 0, 6))
+    m.set_periodic(1)
+    n = np.array([0.9, 0.1, 0.42]); n /= np.linalg.norm(n)
+    S, steps, cells, ds = m.march([1, 1, 0], [0.3, 0.4, 0.0], n, [1, 0, 0, 0], log_cap=400)
+    chord = min((4 - 1.4) / n[1], 6.0 / n[2])
+    assert abs(ds.sum() - chord) < 1e-12 and abs(S[0] - math.exp(-kr * chord)) < 1e-15
+    xs = cells % 5
+    assert steps == len(cells) and np.all(np.diff(xs) % 5 <= 1) and (np.diff(xs) == -4).sum() == int((1.3 + n[0] * chord) // 5)
+    m.set_periodic(0)
+    S0, steps0, _, ds0 = m.march([1, 1, 0], [0.3, 0.4, 0.0], n, [1, 0, 0, 0], log_cap=400)
+    assert abs(ds0.sum() - (5 - 1.3) / n[0]) < 1e-12                       # open box: leaves through the x face first
+    m.set_periodic(7)
+    S, steps, cells, ds = m.march([1, 1, 0], [0.3, 0.4, 0.5], [1.0, 0.0, 0.0], [1, 0, 0, 0], log_cap=10)
+    assert steps == 4 + 4096 * 5                                            # 4 cells to the face, 4096 wraps of 5 cells, the next wrap refused
+    # imaging ray of one emission record through the periodic box: W/(4 pi) e^{-tau of the wrapped path}
+    m.set_periodic(1)
+    m.source_set(0, [1.3, 1.4, 0.0], [0, 0, 1], None, 1)
+    ev = OracleEvents(4)
+    m.transport(0, 1, 1, ev); ev.c.n = 1
+    th, ph = math.acos(n[2]), math.atan2(n[1], n[0])
+    img, _, st = m.image(ev, [Observer.make(th, ph, [2.5, 2, 3], 30.0)], 1, 1, 1)
+    assert abs(img[0, 0, 0, 0] - math.exp(-kr * chord) / (4 * math.pi)) < 1e-15
+
+
+def test_pixel_rays_in_a_periodic_slab():
+    """Thermal emission of a uniform slab periodic in x and y, seen at inclination mu: every pixel ray crosses the same depth
+    tau/mu wherever it enters, so every pixel holds B (1 - e^{-tau/mu}) times its area -- also pixels whose line misses the
+    box of one period; open in x and y the oblique rays are cut short."""
+    tau = 0.8
+    m = box_model((6, 6, 3), tau, opac=const_opac(1, 0, 0, 0.0), bounds=(0, 2, 0, 2, 0, 1))
+    o = Observer.make(math.radians(50), math.radians(20), [1, 1, 0.5], 3.0)
+    mu = math.cos(math.radians(50))
+    emis = np.full((3, 6, 6), 1.7, np.float32)
+    m.set_periodic(3)
+    img, st = m.image_rays(None, [o], 8, 8, emis=emis)
+    apix = (6.0 / 8) ** 2
+    assert np.allclose(img[0, 0], float(np.float32(1.7)) * (1 - math.exp(-float(np.float32(tau)) / mu)) * apix, rtol=1e-12)
+    m.set_periodic(0)
+    img0, _ = m.image_rays(None, [o], 8, 8, emis=emis)
+    assert (img0[0, 0] == 0).sum() > 20 and img0[0, 0].max() < img[0, 0].max() * (1 + 1e-12)
