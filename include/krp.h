@@ -69,6 +69,10 @@ typedef struct krp_tables {
     const float* opacity;
     float w_min;
     int max_scatter;
+    int periodic;     /* bit a set: axis a (0 x, 1 y, 2 z) is periodic (reading R20): packets and imaging rays
+                         that leave through a face of that axis re-enter through the opposite face; after 4096 such crossings a
+                         ray counts as having left the grid.  A periodic model uses the 16-byte cell layout.  A source grid
+                         (krp_sgrid_begin) cannot be opened on a periodic model (KRP_ERR_STATE). */
 } krp_tables;
 
 /* Build a model.  bounds = xlo,xhi,ylo,yhi,zlo,zhi (HOST).  density [nz][ny][nx] >= 0 is

@@ -196,6 +196,7 @@ static int check_tables(const krp_tables* t)
     if (t->n_inc < 1 || t->n_inc > 1024 || !t->opacity) return fail(KRP_ERR_ARG, "tables: n_inc must be in 1..1024 and opacity non-NULL");
     if (!(t->w_min >= 0.f)) return fail(KRP_ERR_ARG, "tables: w_min must be >= 0");
     if (t->max_scatter < 1) return fail(KRP_ERR_ARG, "tables: max_scatter must be >= 1");
+    if (t->periodic < 0 || t->periodic > 7) return fail(KRP_ERR_ARG, "tables: periodic must be a mask of the bits 1 (x), 2 (y), 4 (z)");
     for (int j = 0; j < t->n_ang; ++j) {
         const float* f = t->mueller + 4 * j;
         for (int s = 0; s < 4; ++s)
@@ -304,7 +305,8 @@ extern "C" int krp_grid_create(krp_grid** out, int nx, int ny, int nz, const dou
         dichroic = dichroic || op[4 * j + 1] != 0.f || op[4 * j + 2] != 0.f;
         rho = std::fmax(rho, std::fabs(op[4 * j + 1]) / op[4 * j]);
     }
-    m.scalar = (constant && !dichroic && bfield == nullptr) ? 1 : 0;
+    m.periodic = tables->periodic;
+    m.scalar = (constant && !dichroic && bfield == nullptr && !m.periodic) ? 1 : 0;
     m.a1c = op[0]; m.omc = op[3]; m.rho = rho;
     // scalar flights are short: static assignment; general flights are long: persistent lanes, refill every 32 steps
     g->burst = m.scalar ? 1 : 32;
@@ -1000,6 +1002,7 @@ extern "C" int krp_sgrid_begin(krp_grid* g, const krp_observer* obs, int n_obs, 
     int rc = check_observers(obs, n_obs, 1, 1);
     if (rc) return rc;
     if (n_obs > KRP_SG_MAX_OBS) return fail(KRP_ERR_ARG, "a source grid holds at most %d cameras", KRP_SG_MAX_OBS);
+    if (g->m.periodic) return fail(KRP_ERR_STATE, "a source grid cannot be opened on a model with periodic boundaries");
     cudaStream_t st = (cudaStream_t)stream;
     rc = krp_sgrid_end(g);
     if (rc) return rc;

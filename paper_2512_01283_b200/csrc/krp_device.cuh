@@ -50,6 +50,7 @@ struct KrpModel {
     float w_min;
     int max_scatter;
     int scalar;
+    int periodic;          // bit a: axis a is periodic (R20); only with the 16-byte cell layout
     // source
     int src_kind, emit_records;
     float src_n[3];
@@ -77,6 +78,24 @@ __device__ __forceinline__ void krp_pad_coords(const KrpModel& g, uint32_t c, in
     const uint32_t z = krp_fastdiv(t, g.py_m, g.py_s);
     hy = (int)(t - z * (uint32_t)g.py);
     hz = (int)z;
+}
+
+// Periodic boundaries (R20).  `c` is a halo cell, reached from an interior cell by crossing one face: exactly
+// one of its padded coordinates is out of range.  If that axis is periodic, c becomes the cell behind the opposite face and
+// off[axis] takes the jump (so that unwrapped coordinates can still be formed); returns false when the axis is open.
+#define KRP_MAX_WRAPS 4096
+__device__ __forceinline__ bool krp_wrap(const KrpModel& g, uint32_t& c, int off[3])
+{
+    int hx, hy, hz;
+    krp_pad_coords(g, c, hx, hy, hz);
+    if (hx == 0)              { if (!(g.periodic & 1)) return false; c += (uint32_t)g.nx; off[0] -= g.nx; }
+    else if (hx == g.nx + 1)  { if (!(g.periodic & 1)) return false; c -= (uint32_t)g.nx; off[0] += g.nx; }
+    else if (hy == 0)         { if (!(g.periodic & 2)) return false; c += (uint32_t)(g.ny * g.px); off[1] -= g.ny; }
+    else if (hy == g.ny + 1)  { if (!(g.periodic & 2)) return false; c -= (uint32_t)(g.ny * g.px); off[1] += g.ny; }
+    else if (hz == 0)         { if (!(g.periodic & 4)) return false; c += (uint32_t)g.nz * g.pxy; off[2] -= g.nz; }
+    else if (hz == g.nz + 1)  { if (!(g.periodic & 4)) return false; c -= (uint32_t)g.nz * g.pxy; off[2] += g.nz; }
+    else return false;
+    return true;
 }
 
 struct KrpStatsDev {

@@ -684,7 +684,7 @@ __global__ void __launch_bounds__(TPB, MINB) krp_k_flight_general(KrpModel g, Kr
     double nd[3] = { 0.0, 0.0, 1.0 }, th[3] = { 0.0, 0.0, 0.0 }, ph[3] = { 0.0, 0.0, 0.0 };
     double D = 0.0, i = 1.0, qs = 0.0, us = 0.0, vs = 0.0;
     float arm = 0.f;        // tau*/guard minus the fp32 sum of alpha1 dtau: the fp64 event test is armed once it is <= 0
-    unsigned int nsteps = 0;
+    unsigned int nsteps = 0, nwrap = 0;
     KrpRayD ray = {};
     float4 cl = make_float4(0.f, 0.f, 0.f, 1.f), cl_f = cl;
     bool fresh = false;
@@ -724,7 +724,7 @@ __global__ void __launch_bounds__(TPB, MINB) krp_k_flight_general(KrpModel g, Kr
             }
             D = tau0; i = 1.0;
             qs = S0.y; us = S0.z; vs = S0.w;      // lab reference
-            arm = (float)tau0 * inv_guard; nsteps = 0;
+            arm = (float)tau0 * inv_guard; nsteps = 0; nwrap = 0;
             status = KRP_RUN;
         }
         if (!__any_sync(0xffffffffu, status == KRP_RUN)) break;
@@ -790,7 +790,13 @@ __global__ void __launch_bounds__(TPB, MINB) krp_k_flight_general(KrpModel g, Kr
             ray.rz = (ax | ay) ? ray.rz - ds : ray.tz;
             ray.c = c_next;
             cl = cn;
-            if (cl.x < 0.f) status = KRP_ESC;        // halo: the packet left the grid
+            if (cl.x < 0.f) {                        // halo: the packet left the grid -- or crosses a periodic face (R20)
+                int off[3] = { 0, 0, 0 };
+                if (g.periodic && nwrap < KRP_MAX_WRAPS && krp_wrap(g, ray.c, off)) {
+                    ++nwrap;
+                    asm volatile("ld.global.nc.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(cl.x), "=f"(cl.y), "=f"(cl.z), "=f"(cl.w) : "l"(g.cell + ray.c));
+                } else status = KRP_ESC;
+            }
         }
     }
     krp_tally_flush(tl, ctl);
@@ -1369,6 +1375,7 @@ __global__ void __launch_bounds__(256, SCALAR ? KRP_IMAGE_SCALAR_MIN_BLOCKS : KR
             r.ty = ob.n[1] > 0.f ? (1.f - pc.y) * ob.dt[1] : (ob.n[1] < 0.f ? pc.y * ob.dt[1] : KRP_INF_F);
             r.tz = ob.n[2] > 0.f ? (1.f - pc.z) * ob.dt[2] : (ob.n[2] < 0.f ? pc.z * ob.dt[2] : KRP_INF_F);
             float A = 0.f;
+            int woff[3] = { 0, 0, 0 }, nwrap = 0;       // periodic boundaries: cells jumped per axis, faces re-entered
             if (SCALAR) {
                 // two gathers in flight: the cell after next is requested before the next one is tested
                 float tau = 0.f;
@@ -1413,7 +1420,11 @@ __global__ void __launch_bounds__(256, SCALAR ? KRP_IMAGE_SCALAR_MIN_BLOCKS : KR
                         A = fmaf(cl.x, ds, A);
                         cl = cn;
                     }
-                    if (cl.x == -KRP_INF_F) break;              // halo: the ray has left the grid
+                    if (cl.x == -KRP_INF_F) {                   // halo: the ray has left the grid -- or crosses a periodic face (R20)
+                        // (a ray that has gone dark stops here as well: beyond A = 104 the carried vector would only grow, R20 allows 4096 periods)
+                        if (g.periodic && A <= 104.f && nwrap < KRP_MAX_WRAPS && krp_wrap(g, r.c, woff)) { ++nwrap; cl = __ldg(obs_cell + r.c); continue; }
+                        break;
+                    }
                     {   // a cell that may be thick: full in-cell solution
                         const float ds = krp_raya_step(r, rc);
                         const float4 cn = __ldg(obs_cell + r.c);
@@ -1431,6 +1442,7 @@ __global__ void __launch_bounds__(256, SCALAR ? KRP_IMAGE_SCALAR_MIN_BLOCKS : KR
             } else {
                 float i = S[0], qs = S[1], us = S[2], vs = S[3];
                 float4 cl = __ldg(g.cell + r.c);
+                for (;;) {
                 do {
                     const float ds = krp_raya_step(r, rc);
                     const float4 cn = __ldg(g.cell + r.c);      // next cell, in flight during the update below
@@ -1464,11 +1476,14 @@ __global__ void __launch_bounds__(256, SCALAR ? KRP_IMAGE_SCALAR_MIN_BLOCKS : KR
                             krp_appA(i, qg2, ug2, vg2, make_float4(a1, a2, a3, 0.f), dtau, di, i_new, depth);
                             i = i_new; A += depth; vs = vg2;
                             qs = c2t * qg2 - s2t * ug2; us = s2t * qg2 + c2t * ug2;
-                            if (A > 104.f) { cl = cn; break; }      // e^{-A} is exactly 0 in fp32 from here on
+                            if (A > 104.f) { cl = cn; A = KRP_INF_F; break; }      // e^{-A} is exactly 0 in fp32 from here on
                         }
                     }
                     cl = cn;
                 } while (cl.x >= 0.f);
+                if (A > 104.f || !(g.periodic && nwrap < KRP_MAX_WRAPS && krp_wrap(g, r.c, woff))) break;
+                ++nwrap; cl = __ldg(g.cell + r.c);           // periodic face (R20): go on from the opposite side
+                }
                 S[0] = i; S[1] = qs; S[2] = us; S[3] = vs;
             }
             const float att = expf(-A);
@@ -1476,7 +1491,7 @@ __global__ void __launch_bounds__(256, SCALAR ? KRP_IMAGE_SCALAR_MIN_BLOCKS : KR
             int h0[3], h1[3];
             krp_pad_coords(g, c0, h0[0], h0[1], h0[2]);
             krp_pad_coords(g, r.c, h1[0], h1[1], h1[2]);
-            steps += (unsigned long long)(abs(h1[0] - h0[0]) + abs(h1[1] - h0[1]) + abs(h1[2] - h0[2]));
+            steps += (unsigned long long)(abs(h1[0] + woff[0] - h0[0]) + abs(h1[1] + woff[1] - h0[1]) + abs(h1[2] + woff[2] - h0[2]));
             // I3: orthographic projection of the event position (fp64, once per ray)
             const double x[3] = { g.lo[0] + ((double)(h0[0] - 1) + (double)pc.x) * g.dd[0] - ob.center[0],
                                   g.lo[1] + ((double)(h0[1] - 1) + (double)pc.y) * g.dd[1] - ob.center[1],

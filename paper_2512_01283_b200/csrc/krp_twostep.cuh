@@ -203,17 +203,20 @@ __global__ void __launch_bounds__(128) krp_k_image_rays(KrpModel g, KrpCtl* ctl,
         bool miss = false;
         for (int a = 0; a < 3; ++a) {
             const double lo = g.lo[a], hi = g.lo[a] + (double)nn[a] * g.dd[a];
+            if ((g.periodic >> a) & 1) continue;          // R20: a periodic axis does not clip the line, its coordinate is taken modulo the box
             if (ob.n[a] == 0.0) { if (x0[a] < lo || x0[a] >= hi) miss = true; continue; }
             double t0 = (lo - x0[a]) / ob.n[a], t1 = (hi - x0[a]) / ob.n[a];
             if (t0 > t1) { const double t = t0; t0 = t1; t1 = t; }
             s_in = fmax(s_in, t0); s_out = fmin(s_out, t1);
         }
-        if (!miss && s_in < s_out) {
+        if (!miss && s_in < s_out && s_in != -inf) {
             hit = 1;
+            int nwrap = 0;
             // entry cell and cell-local position; per axis the distance to the next face and the face spacing (re-based march)
             int idx[3]; double r[3], tt[3]; int sgn[3];
             for (int a = 0; a < 3; ++a) {
-                const double x = (x0[a] + s_in * ob.n[a] - g.lo[a]) * g.inv_dd[a];
+                double x = (x0[a] + s_in * ob.n[a] - g.lo[a]) * g.inv_dd[a];
+                if ((g.periodic >> a) & 1) x -= floor(x / (double)nn[a]) * (double)nn[a];
                 int i = (int)floor(x);
                 i = max(0, min(i, nn[a] - 1));
                 const double p = fmin(fmax(x - (double)i, 0.0), 1.0);
@@ -273,7 +276,11 @@ __global__ void __launch_bounds__(128) krp_k_image_rays(KrpModel g, KrpCtl* ctl,
                 }
                 // cross the face; leaving the grid ends the ray
                 idx[ax] += sgn[ax];
-                if (idx[ax] < 0 || idx[ax] >= nn[ax]) break;
+                if (idx[ax] < 0 || idx[ax] >= nn[ax]) {
+                    if (!((g.periodic >> ax) & 1) || nwrap >= KRP_MAX_WRAPS) break;
+                    ++nwrap;
+                    idx[ax] = idx[ax] < 0 ? nn[ax] - 1 : 0;
+                }
                 for (int a = 0; a < 3; ++a) r[a] = (a == ax) ? tt[a] : r[a] - ds;
             }
             const double apix = (2.0 * ob.half_w / (double)npx) * (2.0 * ob.half_h / (double)npy);

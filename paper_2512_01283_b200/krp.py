@@ -32,7 +32,7 @@ class KrpError(RuntimeError):
 
 class Tables(C.Structure):
     _fields_ = [("n_ang", C.c_int), ("mueller", C.c_void_p), ("n_inc", C.c_int), ("opacity", C.c_void_p),
-                ("w_min", C.c_float), ("max_scatter", C.c_int)]
+                ("w_min", C.c_float), ("max_scatter", C.c_int), ("periodic", C.c_int)]
 
 
 class Source(C.Structure):
@@ -159,7 +159,7 @@ class Grid:
     """Owner of one krp_grid handle.  Methods mirror the C entry points one to one."""
 
     def __init__(self, nx, ny, nz, bounds, density, bfield, mueller, opacity, w_min=1e-4, max_scatter=64,
-                 stream=None):
+                 stream=None, periodic=0):
         L = lib()
         self._h = C.c_void_p()
         dptr, dmem, dkeep = _ptr_mem(density)
@@ -168,7 +168,7 @@ class Grid:
             raise ValueError("density and bfield must live in the same memory space")
         mu = np.ascontiguousarray(np.asarray(mueller, np.float32).reshape(-1, 4))
         op = np.ascontiguousarray(np.asarray(opacity, np.float32).reshape(-1, 4))
-        t = Tables(mu.shape[0], mu.ctypes.data, op.shape[0], op.ctypes.data, float(w_min), int(max_scatter))
+        t = Tables(mu.shape[0], mu.ctypes.data, op.shape[0], op.ctypes.data, float(w_min), int(max_scatter), int(periodic))
         b = (C.c_double * 6)(*[float(x) for x in bounds])
         self.shape = (int(nx), int(ny), int(nz))
         self.bounds = [float(x) for x in bounds]

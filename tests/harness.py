@@ -11,6 +11,8 @@ def oracle_model(cfg, variant=None):
                     cfg["opacity"], w_min=cfg["w_min"], max_scatter=cfg["max_scatter"], variant=variant)
     s = cfg["source"]
     m.source_set(s["kind"], s["pos"], s["dir"], s.get("cell_weight"), s.get("emit_records", 0))
+    if cfg.get("periodic"):
+        m.set_periodic(cfg["periodic"])
     return m
 
 
@@ -44,7 +46,7 @@ def gpu_grid(cfg, device="cuda", host_inputs=False):
         dens = torch.from_numpy(cfg["density"]).to(device)
         bf = None if cfg["bfield"] is None else torch.from_numpy(cfg["bfield"]).to(device)
     g = krp.Grid(cfg["nx"], cfg["ny"], cfg["nz"], cfg["bounds"], dens, bf, cfg["mueller"], cfg["opacity"],
-                 w_min=cfg["w_min"], max_scatter=cfg["max_scatter"])
+                 w_min=cfg["w_min"], max_scatter=cfg["max_scatter"], periodic=cfg.get("periodic", 0))
     s = cfg["source"]
     w = s.get("cell_weight")
     if w is not None:
