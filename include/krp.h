@@ -176,6 +176,20 @@ int krp_sgrid_end(krp_grid* g);
 int krp_image_rays(krp_grid* g, const krp_observer* obs, int n_obs, int npix_x, int npix_y, const float* emis, int mem,
                    void* stream);
 
+/* ---- Frequency bins ("For each frequency bin ... the transfer equation reads": eq. 8 holds per bin, the bins
+ * do not exchange energy) -------------------------------------------------------------------------------------------
+ * krp_freq_define gives the model n_freq bins, each with its own tables (tables[b], HOST, as for krp_grid_create; the
+ * `periodic` field is ignored) and its own density factor: kappa*rho of bin b = kappa_scale[b] x the model's (the dust
+ * is the same, its opacity per unit mass differs).  All bins use the cell layout chosen at krp_grid_create, so a model
+ * whose first table was direction-independent and non-dichroic and that has no field accepts only such tables
+ * (KRP_ERR_ARG otherwise).  krp_freq_select makes bin b the current one: krp_transport, krp_image, krp_image_rays,
+ * krp_image_get and krp_image_reset then act on that bin (its tables, its density, its own maps; the observer set and
+ * the pixel counts are common to all bins).  Buffered events belong to the bin they were transported in: image them before
+ * selecting another bin (KRP_ERR_STATE if the buffer is not empty; it synchronises to check).  Bin 0 is current after
+ * krp_freq_define.  A model without krp_freq_define has the single bin of krp_grid_create. */
+int krp_freq_define(krp_grid* g, int n_freq, const krp_tables* tables, const float* kappa_scale, void* stream);
+int krp_freq_select(krp_grid* g, int bin, void* stream);
+
 /* Counters (also the numerators of the roofline figures). */
 typedef struct krp_stats {
     uint64_t packets;         /* packets emitted */

@@ -34,8 +34,28 @@ static int fail(int code, const char* fmt, ...)
                         cudaGetErrorString(e_));                                                   \
     } while (0)
 
+// One set of lookup tables on the device with the model constants derived from it: one per frequency bin
+// (eq. 8 holds per frequency bin; include/krp.h krp_freq_define)
+struct TableSet {
+    float4* d_opac = nullptr; float4* d_opA = nullptr; float4* d_opB = nullptr;
+    double4* d_opA_d = nullptr; double4* d_opB_d = nullptr;
+    float4* d_mueller = nullptr; double* d_cdf = nullptr;
+    int n_inc = 0, n_ang = 0, max_scatter = 0, max_waves = 0;
+    float a1c = 0, omc = 0, rho = 0, w_min = 0;
+    bool constant = true, dichroic = false;
+    float kscale = 1.f;             // density factor of the bin: kappa*rho of the bin = kscale x the model's
+    double* d_img = nullptr;        // the bin's maps (same observer set and size for all bins)
+};
+
+static void free_tables(TableSet& t);
+static int apply_scale(struct krp_grid* g, float k, cudaStream_t st);
+
 struct krp_grid {
     KrpModel m;
+    std::vector<TableSet> bins;     // frequency bins (at least one)
+    int cur_bin = 0;
+    float* d_base = nullptr;        // kappa*rho of the model in the padded order (kept once a bin scales the density)
+    float cur_scale = 1.f;
     int device = 0, n_sm = 0;
     // owned device memory
     float* d_kr = nullptr;          // = d_kr_alloc + margin
@@ -48,11 +68,6 @@ struct krp_grid {
     bool has_bfield = false;
     bool obs_cells_stale = false;   // cells changed since the per-observer coefficient arrays were built (or never built)
     bool obs_cells_failed = false;  // the arrays did not fit for the current observer set
-    float4* d_opac = nullptr;
-    float4* d_opA = nullptr;
-    float4* d_opB = nullptr;
-    double4* d_opA_d = nullptr;
-    double4* d_opB_d = nullptr;
     uint32_t npad = 0;
     // imaging order (counting sort of the events by cell bin)
     unsigned int* d_bins = nullptr;
@@ -71,8 +86,6 @@ struct krp_grid {
     int dir_sort = 1;
     unsigned int* d_order = nullptr;
     uint64_t order_cap = 0;
-    float4* d_mueller = nullptr;
-    double* d_cdf = nullptr;
     double* d_src_cdf = nullptr;
     KrpCtl* d_ctl = nullptr;
     KrpRecords q[2] = {};
@@ -105,7 +118,6 @@ struct krp_grid {
     float* d_emis = nullptr;        // padded thermal source of krp_image_rays
     uint64_t next_id = 0;
     uint64_t launches = 0;
-    int max_waves = 0;
     int transport_block = 256, image_block = 256, blocks_per_sm = 8;   // general mode: transport_block 128 (krp_grid_create)
     int bps_tuned = 0;
     int ev_has_emission = 0;        // emission records (k = 0) may be in the event buffer
@@ -176,9 +188,11 @@ static int alloc_records(KrpRecords& r, uint64_t cap, bool with_tau)
 extern "C" int krp_grid_destroy(krp_grid* g)
 {
     if (!g) return KRP_OK;
-    cudaFree(g->d_kr_alloc); cudaFree(g->d_cell_alloc); cudaFree(g->d_stage_den); cudaFree(g->d_stage_b); cudaFree(g->d_bad); cudaFree(g->d_opac); cudaFree(g->d_mueller); cudaFree(g->d_cdf);
+    cudaFree(g->d_kr_alloc); cudaFree(g->d_cell_alloc); cudaFree(g->d_stage_den); cudaFree(g->d_stage_b); cudaFree(g->d_bad); cudaFree(g->d_base);
+    if (!g->bins.empty()) g->bins[g->cur_bin].d_img = nullptr;      // the current bin's maps are g->d_img, freed below
+    for (TableSet& t : g->bins) free_tables(t);
     cudaFree(g->d_src_cdf); cudaFree(g->d_ctl); cudaFree(g->d_obs); cudaFree(g->d_img); cudaFree(g->d_obs_cells);
-    cudaFree(g->d_opA); cudaFree(g->d_opB); cudaFree(g->d_opA_d); cudaFree(g->d_opB_d); cudaFree(g->d_bins); cudaFree(g->d_perm); cudaFree(g->d_scan);
+    cudaFree(g->d_bins); cudaFree(g->d_perm); cudaFree(g->d_scan);
     cudaFree(g->d_dir_bins); cudaFree(g->d_dir_scan); cudaFree(g->d_order);
     cudaFree(g->d_sgrid); cudaFree(g->d_sg_obs); cudaFree(g->d_flen); cudaFree(g->d_emis);
     free_records(g->q[0]); free_records(g->q[1]); free_records(g->ev); free_hits(g->hits);
@@ -215,6 +229,100 @@ static int check_tables(const krp_tables* t)
     return KRP_OK;
 }
 
+static void free_tables(TableSet& t)
+{
+    cudaFree(t.d_opac); cudaFree(t.d_opA); cudaFree(t.d_opB); cudaFree(t.d_opA_d); cudaFree(t.d_opB_d); cudaFree(t.d_mueller);
+    cudaFree(t.d_cdf); cudaFree(t.d_img);
+    t = TableSet{};
+}
+
+// T0: upload one table set and derive the constants the kernels need from it
+static int build_tables(const krp_tables* tables, TableSet& t, cudaStream_t st)
+{
+    // opacity table: n_inc = 1 becomes two equal rows so that the kernels always interpolate
+    const int n_inc = tables->n_inc == 1 ? 2 : tables->n_inc;
+    std::vector<float> op(4 * (size_t)n_inc);
+    for (int j = 0; j < n_inc; ++j)
+        memcpy(&op[4 * j], tables->opacity + 4 * (tables->n_inc == 1 ? 0 : j), 4 * sizeof(float));
+    t.constant = true; t.dichroic = false;
+    float rho = 0.f;
+    for (int j = 0; j < n_inc; ++j) {
+        for (int s = 0; s < 4; ++s) t.constant = t.constant && (op[4 * j + s] == op[s]);
+        t.dichroic = t.dichroic || op[4 * j + 1] != 0.f || op[4 * j + 2] != 0.f;
+        rho = std::fmax(rho, std::fabs(op[4 * j + 1]) / op[4 * j]);
+    }
+    t.a1c = op[0]; t.omc = op[3]; t.rho = rho;
+    t.n_inc = n_inc; t.n_ang = tables->n_ang;
+    t.w_min = tables->w_min; t.max_scatter = tables->max_scatter;
+    // number of waves that can contain live packets: the weight after k scatterings is <= omega_max^k
+    {
+        float om_max = 0.f;
+        for (int j = 0; j < n_inc; ++j) om_max = std::fmax(om_max, op[4 * j + 3]);
+        int waves = tables->max_scatter;
+        if (om_max <= 0.f) waves = 1;
+        else if (om_max < 1.f && tables->w_min > 0.f) {
+            double kk = std::ceil(std::log((double)tables->w_min) / std::log((double)om_max)) + 1.0;
+            if (kk < waves) waves = (int)std::fmax(kk, 1.0);
+        }
+        t.max_waves = waves;
+    }
+    CK(cudaMalloc(&t.d_opac, sizeof(float4) * n_inc));
+    CK(cudaMemcpyAsync(t.d_opac, op.data(), sizeof(float4) * n_inc, cudaMemcpyHostToDevice, st));
+    // the same table as intercept + slope per segment of x = mu*(n_inc-1): value = A_j + B_j x on [j, j+1]
+    std::vector<float> A(4 * (size_t)(n_inc - 1)), B(4 * (size_t)(n_inc - 1));
+    std::vector<double> Ad(4 * (size_t)(n_inc - 1)), Bd(4 * (size_t)(n_inc - 1));
+    for (int j = 0; j + 1 < n_inc; ++j)
+        for (int s = 0; s < 4; ++s) {
+            double a = op[4 * j + s], b = op[4 * (j + 1) + s];
+            B[4 * j + s] = (float)(b - a); A[4 * j + s] = (float)(a - (b - a) * j);
+            Bd[4 * j + s] = b - a; Ad[4 * j + s] = a - (b - a) * j;
+        }
+    CK(cudaMalloc(&t.d_opA, sizeof(float4) * (n_inc - 1)));
+    CK(cudaMalloc(&t.d_opB, sizeof(float4) * (n_inc - 1)));
+    CK(cudaMemcpyAsync(t.d_opA, A.data(), sizeof(float4) * (n_inc - 1), cudaMemcpyHostToDevice, st));
+    CK(cudaMemcpyAsync(t.d_opB, B.data(), sizeof(float4) * (n_inc - 1), cudaMemcpyHostToDevice, st));
+    CK(cudaMalloc(&t.d_opA_d, sizeof(double4) * (n_inc - 1)));
+    CK(cudaMalloc(&t.d_opB_d, sizeof(double4) * (n_inc - 1)));
+    CK(cudaMemcpyAsync(t.d_opA_d, Ad.data(), sizeof(double4) * (n_inc - 1), cudaMemcpyHostToDevice, st));
+    CK(cudaMemcpyAsync(t.d_opB_d, Bd.data(), sizeof(double4) * (n_inc - 1), cudaMemcpyHostToDevice, st));
+    CK(cudaMalloc(&t.d_mueller, sizeof(float4) * t.n_ang));
+    CK(cudaMemcpyAsync(t.d_mueller, tables->mueller, sizeof(float4) * t.n_ang, cudaMemcpyHostToDevice, st));
+    // Theta CDF: trapezoid of S11 sin(Theta) on the nodes, fp64 (R13)
+    std::vector<double> cdf(t.n_ang);
+    {
+        const double h = KRP_PI_D / (t.n_ang - 1);
+        double acc = 0.0, prev = 0.0;
+        cdf[0] = 0.0;
+        for (int j = 1; j < t.n_ang; ++j) {
+            double cur = (double)tables->mueller[4 * j] * std::sin(j * h);
+            acc += 0.5 * (prev + cur);
+            cdf[j] = acc;
+            prev = cur;
+        }
+        for (int j = 0; j < t.n_ang; ++j) cdf[j] /= acc;
+        cdf[t.n_ang - 1] = 1.0;
+    }
+    CK(cudaMalloc(&t.d_cdf, sizeof(double) * t.n_ang));
+    CK(cudaMemcpyAsync(t.d_cdf, cdf.data(), sizeof(double) * t.n_ang, cudaMemcpyHostToDevice, st));
+    CK(cudaStreamSynchronize(st));          // the host vectors are locals
+    return KRP_OK;
+}
+
+// make bin b's tables the ones the kernels see
+static void apply_tables(krp_grid* g, int b)
+{
+    KrpModel& m = g->m;
+    const TableSet& t = g->bins[b];
+    m.opac = t.d_opac; m.opA = t.d_opA; m.opB = t.d_opB; m.opA_d = t.d_opA_d; m.opB_d = t.d_opB_d;
+    m.mueller = t.d_mueller; m.cdf = t.d_cdf;
+    m.n_inc = t.n_inc; m.n_ang = t.n_ang;
+    m.a1c = t.a1c; m.omc = t.omc; m.rho = t.rho;
+    m.xs = (double)(t.n_inc - 1); m.guard = 1.f + t.rho + 1e-3f; m.inv_nang1 = 1.0 / (double)(t.n_ang - 1);
+    m.nang1_over_pi = (float)((double)(t.n_ang - 1) / 3.14159265358979323846);
+    m.w_min = t.w_min; m.max_scatter = t.max_scatter;
+    g->cur_bin = b;
+}
+
 // T0: (re)pack the caller's density / field arrays into the padded cell array of g (halo included)
 static int upload_cells(krp_grid* g, const float* density, const float* bfield, int mem, cudaStream_t st)
 {
@@ -245,6 +353,13 @@ static int upload_cells(krp_grid* g, const float* density, const float* bfield, 
     CK(cudaStreamSynchronize(st));
     if (bad) return fail(KRP_ERR_ARG, "density has %d negative, NaN or infinite cells", bad);
     g->obs_cells_stale = true;
+    if (g->d_base) {       // frequency bins scale the density: keep the new model values and re-apply the current factor
+        const float k = g->cur_scale;
+        krp_k_save_base<<<nb, tb, 0, st>>>(g->npad, g->d_kr, g->d_cell, g->d_base);
+        g->launches++;
+        g->cur_scale = 1.f;
+        return apply_scale(g, k, st);
+    }
     return KRP_OK;
 }
 
@@ -293,91 +408,19 @@ extern "C" int krp_grid_create(krp_grid** out, int nx, int ny, int nz, const dou
         m.d[a] = (float)m.dd[a];
         m.inv_dd[a] = 1.0 / m.dd[a];
     }
-    // opacity table: n_inc = 1 becomes two equal rows so that the kernels always interpolate
-    const int n_inc = tables->n_inc == 1 ? 2 : tables->n_inc;
-    std::vector<float> op(4 * (size_t)n_inc);
-    for (int j = 0; j < n_inc; ++j)
-        memcpy(&op[4 * j], tables->opacity + 4 * (tables->n_inc == 1 ? 0 : j), 4 * sizeof(float));
-    bool constant = true, dichroic = false;
-    float rho = 0.f;
-    for (int j = 0; j < n_inc; ++j) {
-        for (int s = 0; s < 4; ++s) constant = constant && (op[4 * j + s] == op[s]);
-        dichroic = dichroic || op[4 * j + 1] != 0.f || op[4 * j + 2] != 0.f;
-        rho = std::fmax(rho, std::fabs(op[4 * j + 1]) / op[4 * j]);
-    }
+    // tables of the first (and, until krp_freq_define, only) frequency bin
+    g->bins.resize(1);
+    rc = build_tables(tables, g->bins[0], st);
+    if (rc) return rc;
     m.periodic = tables->periodic;
-    m.scalar = (constant && !dichroic && bfield == nullptr && !m.periodic) ? 1 : 0;
-    m.a1c = op[0]; m.omc = op[3]; m.rho = rho;
+    m.scalar = (g->bins[0].constant && !g->bins[0].dichroic && bfield == nullptr && !m.periodic) ? 1 : 0;
+    apply_tables(g, 0);
     // scalar flights are short: static assignment; general flights are long: persistent lanes, refill every 32 steps
     g->burst = m.scalar ? 1 : 32;
     if (!m.scalar) g->transport_block = 128;
     if (m.scalar)
         CK(cudaFuncSetAttribute(krp_k_flight_scalar, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)(8 * sizeof(KrpWarpShared))));
     g->order_events = g->order_policy != 0;
-    m.n_inc = n_inc; m.n_ang = tables->n_ang;
-    m.xs = (double)(n_inc - 1); m.guard = 1.f + m.rho + 1e-3f; m.inv_nang1 = 1.0 / (double)(tables->n_ang - 1);
-    m.nang1_over_pi = (float)((double)(tables->n_ang - 1) / 3.14159265358979323846);
-    m.w_min = tables->w_min; m.max_scatter = tables->max_scatter;
-    // number of waves that can contain live packets: the weight after k scatterings is <= omega_max^k
-    {
-        float om_max = 0.f;
-        for (int j = 0; j < n_inc; ++j) om_max = std::fmax(om_max, op[4 * j + 3]);
-        int waves = tables->max_scatter;
-        if (om_max <= 0.f) waves = 1;
-        else if (om_max < 1.f && tables->w_min > 0.f) {
-            double kk = std::ceil(std::log((double)tables->w_min) / std::log((double)om_max)) + 1.0;
-            if (kk < waves) waves = (int)std::fmax(kk, 1.0);
-        }
-        g->max_waves = waves;
-    }
-    CK(cudaMalloc(&g->d_opac, sizeof(float4) * n_inc));
-    CK(cudaMemcpyAsync(g->d_opac, op.data(), sizeof(float4) * n_inc, cudaMemcpyHostToDevice, st));
-    {   // the same table as intercept + slope per segment of x = mu*(n_inc-1): value = A_j + B_j x on [j, j+1]
-        std::vector<float> A(4 * (size_t)(n_inc - 1)), B(4 * (size_t)(n_inc - 1));
-        for (int j = 0; j + 1 < n_inc; ++j)
-            for (int s = 0; s < 4; ++s) {
-                double a = op[4 * j + s], b = op[4 * (j + 1) + s];
-                B[4 * j + s] = (float)(b - a);
-                A[4 * j + s] = (float)(a - (b - a) * j);
-            }
-        CK(cudaMalloc(&g->d_opA, sizeof(float4) * (n_inc - 1)));
-        CK(cudaMalloc(&g->d_opB, sizeof(float4) * (n_inc - 1)));
-        CK(cudaMemcpyAsync(g->d_opA, A.data(), sizeof(float4) * (n_inc - 1), cudaMemcpyHostToDevice, st));
-        CK(cudaMemcpyAsync(g->d_opB, B.data(), sizeof(float4) * (n_inc - 1), cudaMemcpyHostToDevice, st));
-        std::vector<double> Ad(4 * (size_t)(n_inc - 1)), Bd(4 * (size_t)(n_inc - 1));
-        for (int j = 0; j + 1 < n_inc; ++j)
-            for (int s = 0; s < 4; ++s) {
-                double a = op[4 * j + s], b = op[4 * (j + 1) + s];
-                Bd[4 * j + s] = b - a;
-                Ad[4 * j + s] = a - (b - a) * j;
-            }
-        CK(cudaMalloc(&g->d_opA_d, sizeof(double4) * (n_inc - 1)));
-        CK(cudaMalloc(&g->d_opB_d, sizeof(double4) * (n_inc - 1)));
-        CK(cudaMemcpyAsync(g->d_opA_d, Ad.data(), sizeof(double4) * (n_inc - 1), cudaMemcpyHostToDevice, st));
-        CK(cudaMemcpyAsync(g->d_opB_d, Bd.data(), sizeof(double4) * (n_inc - 1), cudaMemcpyHostToDevice, st));
-        CK(cudaStreamSynchronize(st));          // A, B are locals
-        m.opA = g->d_opA; m.opB = g->d_opB; m.opA_d = g->d_opA_d; m.opB_d = g->d_opB_d;
-    }
-    CK(cudaMalloc(&g->d_mueller, sizeof(float4) * m.n_ang));
-    CK(cudaMemcpyAsync(g->d_mueller, tables->mueller, sizeof(float4) * m.n_ang, cudaMemcpyHostToDevice, st));
-    // Theta CDF: trapezoid of S11 sin(Theta) on the nodes, fp64 (R13)
-    std::vector<double> cdf(m.n_ang);
-    {
-        const double h = KRP_PI_D / (m.n_ang - 1);
-        double acc = 0.0, prev = 0.0;
-        cdf[0] = 0.0;
-        for (int j = 1; j < m.n_ang; ++j) {
-            double cur = (double)tables->mueller[4 * j] * std::sin(j * h);
-            acc += 0.5 * (prev + cur);
-            cdf[j] = acc;
-            prev = cur;
-        }
-        for (int j = 0; j < m.n_ang; ++j) cdf[j] /= acc;
-        cdf[m.n_ang - 1] = 1.0;
-    }
-    CK(cudaMalloc(&g->d_cdf, sizeof(double) * m.n_ang));
-    CK(cudaMemcpyAsync(g->d_cdf, cdf.data(), sizeof(double) * m.n_ang, cudaMemcpyHostToDevice, st));
-    m.opac = g->d_opac; m.mueller = g->d_mueller; m.cdf = g->d_cdf;
 
     // cells: packed into the padded layout (one-cell halo with kappa*rho = -1).  A margin of one padded plane on
     // either side keeps the look-ahead loads of the marches (one cell past the halo cell that ends a ray) inside
@@ -618,7 +661,7 @@ extern "C" int krp_transport(krp_grid* g, uint64_t n_packets, uint64_t seed, voi
     const unsigned grid_g = need < pers_g ? need : pers_g;
     unsigned grid_s = (n + 127u) / 128u;
     if (grid_s > pers * 2) grid_s = pers * 2;
-    for (int w = 0; w < g->max_waves; ++w) {
+    for (int w = 0; w < g->bins[g->cur_bin].max_waves; ++w) {
         const int in = w & 1;
         krp_k_wave_prep<<<1, 1, 0, st>>>(g->d_ctl, in);
         { TimedLaunch tl(g, st, KRP_T_FLIGHT);
@@ -645,7 +688,7 @@ extern "C" int krp_transport(krp_grid* g, uint64_t n_packets, uint64_t seed, voi
             else             krp_k_deposit<false><<<grid_d, 256, 0, st>>>(g->m, g->d_ctl, g->q[in], in, es, flen, g->d_sg_obs, g->sg_n_obs, G, g->d_sgrid, &g->d_ctl->sg_segments);
             g->launches++;
         }
-        if (w + 1 < g->max_waves) {
+        if (w + 1 < g->bins[g->cur_bin].max_waves) {
             TimedLaunch tl(g, st, KRP_T_SCATTER);
             krp_k_scatter<<<grid_s, 128, 0, st>>>(g->m, g->d_ctl, g->ev, g->q[1 - in], 1 - in, seed);
             g->launches++;
@@ -1098,6 +1141,80 @@ extern "C" int krp_image_rays(krp_grid* g, const krp_observer* obs, int n_obs, i
     }
     CK(cudaGetLastError());
     return KRP_OK;
+}
+
+// ------------------------------------------------------------------------------------------
+// frequency bins (include/krp.h)
+// ------------------------------------------------------------------------------------------
+static int apply_scale(krp_grid* g, float k, cudaStream_t st)
+{
+    if (k == g->cur_scale) return KRP_OK;
+    const unsigned nb = (unsigned)((g->npad + 255u) / 256u);
+    if (!g->d_base) {
+        CK(cudaMalloc(&g->d_base, sizeof(float) * (size_t)g->npad));
+        krp_k_save_base<<<nb, 256, 0, st>>>(g->npad, g->d_kr, g->d_cell, g->d_base);
+        g->launches++;
+    }
+    krp_k_rescale<<<nb, 256, 0, st>>>(g->npad, g->d_base, k, g->d_kr, g->d_cell);
+    g->launches++;
+    CK(cudaGetLastError());
+    g->cur_scale = k;
+    g->obs_cells_stale = true;
+    return KRP_OK;
+}
+
+extern "C" int krp_freq_select(krp_grid* g, int bin, void* stream)
+{
+    if (!g) return fail(KRP_ERR_ARG, "grid is NULL");
+    if (bin < 0 || bin >= (int)g->bins.size()) return fail(KRP_ERR_ARG, "bin must be in 0..%d", (int)g->bins.size() - 1);
+    cudaStream_t st = (cudaStream_t)stream;
+    if (bin == g->cur_bin) return KRP_OK;
+    CK(cudaStreamSynchronize(st));
+    KrpCtl c;
+    CK(cudaMemcpy(&c, g->d_ctl, sizeof(c), cudaMemcpyDeviceToHost));
+    if (c.n_events != 0) return fail(KRP_ERR_STATE, "image (or clear) the buffered events before selecting another frequency bin");
+    g->bins[g->cur_bin].d_img = g->d_img;            // park the maps of the bin we leave
+    double* img = g->bins[bin].d_img;
+    if (!img && g->d_img) {                           // same observer set and size for every bin
+        const size_t bytes = sizeof(double) * 4 * (size_t)g->n_obs * g->npx * g->npy;
+        CK(cudaMalloc(&img, bytes));
+        CK(cudaMemsetAsync(img, 0, bytes, st));
+    }
+    g->d_img = img;
+    g->bins[bin].d_img = nullptr;                     // owned through g->d_img while current
+    apply_tables(g, bin);
+    return apply_scale(g, g->bins[bin].kscale, st);
+}
+
+extern "C" int krp_freq_define(krp_grid* g, int n_freq, const krp_tables* tables, const float* kappa_scale, void* stream)
+{
+    if (!g || !tables || !kappa_scale) return fail(KRP_ERR_ARG, "grid, tables or kappa_scale is NULL");
+    if (n_freq < 1 || n_freq > 4096) return fail(KRP_ERR_ARG, "n_freq must be in 1..4096");
+    cudaStream_t st = (cudaStream_t)stream;
+    for (int b = 0; b < n_freq; ++b) {
+        int rc = check_tables(tables + b);
+        if (rc) return rc;
+        if (!(kappa_scale[b] > 0.f) || !std::isfinite(kappa_scale[b])) return fail(KRP_ERR_ARG, "kappa_scale[%d] must be positive and finite", b);
+    }
+    CK(cudaStreamSynchronize(st));
+    KrpCtl c;
+    CK(cudaMemcpy(&c, g->d_ctl, sizeof(c), cudaMemcpyDeviceToHost));
+    if (c.n_events != 0) return fail(KRP_ERR_STATE, "krp_freq_define with a non-empty event buffer");
+    std::vector<TableSet> nb(n_freq);
+    for (int b = 0; b < n_freq; ++b) {
+        int rc = build_tables(tables + b, nb[b], st);
+        if (!rc && g->m.scalar && !(nb[b].constant && !nb[b].dichroic))
+            rc = fail(KRP_ERR_ARG, "bin %d needs the 16-byte cell layout: create the model with a field or a direction-dependent table", b);
+        if (rc) { for (TableSet& t : nb) free_tables(t); return rc; }
+        nb[b].kscale = kappa_scale[b];
+    }
+    // the maps of the old bins go; those of the current one are g->d_img
+    cudaFree(g->d_img); g->d_img = nullptr; g->obs_host.clear();
+    g->bins[g->cur_bin].d_img = nullptr;
+    for (TableSet& t : g->bins) free_tables(t);
+    g->bins.swap(nb);
+    apply_tables(g, 0);
+    return apply_scale(g, g->bins[0].kscale, st);
 }
 
 extern "C" int krp_timing_enable(krp_grid* g, int on)

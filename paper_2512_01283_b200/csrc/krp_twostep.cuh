@@ -317,3 +317,21 @@ __global__ void krp_k_sgrid_unpad(KrpModel g, const float4* __restrict__ sg, int
     const uint32_t iz = t / (uint32_t)g.ny; const int iy = (int)(t - iz * (uint32_t)g.ny);
     out[i] = sg[(size_t)krp_pad_id(g, ix, iy, (int)iz) * n_obs + o];
 }
+
+// ------------------------------------------------------------------------------------------
+// frequency bins: kappa*rho of a bin = factor x the model's.  base holds the model's values in the
+// padded order (halo -1); the cell arrays take base x factor.
+// ------------------------------------------------------------------------------------------
+__global__ void krp_k_save_base(uint32_t npad, const float* __restrict__ kr, const float4* __restrict__ cell, float* __restrict__ base)
+{
+    const uint32_t c = blockIdx.x * blockDim.x + threadIdx.x;
+    if (c < npad) base[c] = kr ? kr[c] : cell[c].x;
+}
+__global__ void krp_k_rescale(uint32_t npad, const float* __restrict__ base, float factor, float* __restrict__ kr, float4* __restrict__ cell)
+{
+    const uint32_t c = blockIdx.x * blockDim.x + threadIdx.x;
+    if (c >= npad) return;
+    const float b = base[c], v = b < 0.f ? b : b * factor;
+    if (kr) kr[c] = v;
+    if (cell) cell[c].x = v;
+}

@@ -18,7 +18,7 @@ SYMBOLS = [
     "krp_events_reserve", "krp_transport", "krp_packet_id_set", "krp_image", "krp_image_get",
     "krp_image_reset", "krp_stats_get", "krp_stats_reset", "krp_events_get", "krp_events_select", "krp_events_clear",
     "krp_tune", "krp_tune_schedule", "krp_timing_enable", "krp_timing_get", "krp_launch_count",
-    "krp_sgrid_begin", "krp_sgrid_get", "krp_sgrid_reset", "krp_sgrid_end", "krp_image_rays",
+    "krp_sgrid_begin", "krp_sgrid_get", "krp_sgrid_reset", "krp_sgrid_end", "krp_image_rays", "krp_freq_define", "krp_freq_select",
 ]
 T_FLIGHT, T_SCATTER, T_ORDER, T_IMAGE, T_EMIT, T_DEPOSIT, T_RAYS, T_COUNT = 0, 1, 2, 3, 4, 5, 6, 7
 T_NAMES = ("flight", "scatter", "order", "image", "emit", "deposit", "rays")
@@ -103,6 +103,8 @@ def lib():
         "krp_timing_get": (i32, [vp, vp, vp]),
         "krp_tune_schedule": (i32, [vp, i32, i32, i32]),
         "krp_launch_count": (u64, [vp]),
+        "krp_freq_define": (i32, [vp, i32, C.POINTER(Tables), vp, vp]),
+        "krp_freq_select": (i32, [vp, i32, vp]),
         "krp_sgrid_begin": (i32, [vp, C.POINTER(Observer), i32, vp]),
         "krp_sgrid_get": (i32, [vp, vp, i32, vp]),
         "krp_sgrid_reset": (i32, [vp, vp]),
@@ -272,6 +274,23 @@ class Grid:
 
     def events_clear(self, stream=None):
         _check(lib().krp_events_clear(self._h, _stream(stream)))
+
+    # --- frequency bins ---
+    def freq_define(self, tables, kappa_scale, stream=None):
+        """tables: list of (mueller [n_ang,4], opacity [n_inc,4], w_min, max_scatter) per bin; kappa_scale: density factor per bin."""
+        n = len(tables)
+        keep = []
+        arr = (Tables * n)()
+        for b, (mu, op, w_min, max_scatter) in enumerate(tables):
+            mu = np.ascontiguousarray(np.asarray(mu, np.float32).reshape(-1, 4)); op = np.ascontiguousarray(np.asarray(op, np.float32).reshape(-1, 4))
+            keep += [mu, op]
+            arr[b] = Tables(mu.shape[0], mu.ctypes.data, op.shape[0], op.ctypes.data, float(w_min), int(max_scatter), 0)
+        ks = np.ascontiguousarray(np.asarray(kappa_scale, np.float32))
+        assert ks.size == n
+        _check(lib().krp_freq_define(self._h, n, arr, C.c_void_p(ks.ctypes.data), _stream(stream)))
+
+    def freq_select(self, b, stream=None):
+        _check(lib().krp_freq_select(self._h, int(b), _stream(stream)))
 
     # --- the paper's two-step form ---
     def sgrid_begin(self, observers, stream=None):
