@@ -6,5 +6,5 @@ Plain fp64 CPU oracle of the Kratos-polrad hot path (arxiv 2512.01283), in C
 legs may import this package.  It imports nothing from the CUDA package.
 """
 from .pyoracle import (  # noqa: F401
-    build, lib, OracleModel, OracleEvents, OracleStats, Observer,
+    build, lib, OracleModel, OracleEvents, OracleStats, Observer, OracleZTable,
 )

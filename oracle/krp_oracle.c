@@ -238,7 +238,14 @@ typedef struct ora_model {
     double* src_cdf;      /* owned, [ncell] running sum of cell weights, or NULL */
     int64_t src_cell; int src_idx[3]; double src_p[3];
     int periodic;         /* bit a set: axis a is periodic, reading R20 */
+    const struct ora_ztable* ztab;   /* borrowed; non-NULL: scatter and peel with the full Z(Omega;Omega') (NEXT-2, R21) */
 } ora_model;
+struct ora_ztable;
+void ora_model_set_ztable(ora_model* m, const struct ora_ztable* z) { m->ztab = z; }
+int ora_scatter_z(const struct ora_ztable* z, const double b[3], const double n_in[3], const double S_in[4],
+                  uint64_t seed, uint64_t id, uint32_t k, double n_out[3], double S_out[4], double* tau_next);
+void ora_peel_z(const struct ora_ztable* z, const double b[3], const double n_in[3], const double S_in[4], const double n_obs[3],
+                double S_out[4]);
 
 /* Periodic boundary conditions (the cylinder test: "our use of periodic boundary conditions").
  * Reading R20: a packet or an imaging ray that leaves through a face of a periodic axis re-enters through the opposite
@@ -720,7 +727,8 @@ int64_t ora_transport2(const ora_model* m, uint64_t id0, uint64_t n_packets, uin
             W *= om;
             if (W < m->w_min || k >= m->max_scatter) { st->w_cut += W; break; }
             double n2[3], S2[4];
-            ora_scatter(m, b, n, S, seed, id, (uint32_t)k, n2, S2, &tau_star);
+            if (m->ztab) ora_scatter_z(m->ztab, b, n, S, seed, id, (uint32_t)k, n2, S2, &tau_star);
+            else ora_scatter(m, b, n, S, seed, id, (uint32_t)k, n2, S2, &tau_star);
             for (int a2 = 0; a2 < 3; ++a2) n[a2] = n2[a2];
             for (int s = 0; s < 4; ++s) S[s] = ORA_STATE(S2[s]);             /* R12: queue state */
         }
@@ -785,6 +793,10 @@ void ora_image(const ora_model* m, const ora_events* ev, const ora_observer* obs
             if (ev->k[e] == 0) {
                 if (!(flags & 1)) continue;
                 S[0] = Se[0] / (4 * ORA_PI); S[1] = S[2] = S[3] = 0.0;
+            } else if (m->ztab) {
+                double b[3];
+                cell_bhat(m, c, b);
+                ora_peel_z(m->ztab, b, nin, Se, no, S);
             } else {
                 ora_peel(m, nin, Se, no, S);
             }
@@ -984,4 +996,172 @@ void ora_image_rays(const ora_model* m, const double* sgrid, const float* emis, 
             for (int s = 0; s < 4; ++s) img[(((int64_t)o * 4 + s) * npy + iy) * npx + ix] += apix * S[s];
         }
     }
+}
+
+/* ================================================================== */
+/* NEXT-2: the full aligned-grain scattering matrix Z(Omega; Omega')   */
+/* in the grain frame (PAPER.md:103-105 eq. 10, :107-109, :129).       */
+/* Reading R21.  The dipole formulas of the     */
+/* paper's grain model are not in the paper's text, so Z is a user     */
+/* table ("interpolation tables"):                        */
+/*   Z[i][o][d][4][4], incidence angle vartheta_in = i 180/(n_ti-1),   */
+/*   outgoing polar angle vartheta_out = o 180/(n_to-1), azimuth       */
+/*   difference dphi = phi_out - phi_in = d 360/n_dp (periodic), all   */
+/*   in the Grain Frame (z_GF = B^); both Stokes vectors referenced to */
+/*   (theta^', phi^') of their own direction in that frame (eq. 4-5).  */
+/*   Trilinear interpolation in the three angles.                      */
+/* ================================================================== */
+typedef struct ora_ztable {
+    int n_ti, n_to, n_dp;
+    float* Z;            /* owned copy of the caller's fp32 table */
+    double* norm;        /* [n_ti][4]: (1/4pi) closed-surface integral of row 1 of Z over outgoing directions, per incidence node */
+    double* bound;       /* [n_ti]: max over outgoing nodes of Z11 + sqrt(Z12^2 + Z13^2 + Z14^2) */
+} ora_ztable;
+
+void ora_ztable_free(ora_ztable* z) { if (z) { free(z->Z); free(z->norm); free(z->bound); free(z); } }
+
+ora_ztable* ora_ztable_create(int n_ti, int n_to, int n_dp, const float* Z)
+{
+    ora_ztable* z = (ora_ztable*)calloc(1, sizeof(ora_ztable));
+    z->n_ti = n_ti; z->n_to = n_to; z->n_dp = n_dp;
+    size_t n = (size_t)n_ti * n_to * n_dp * 16;
+    z->Z = (float*)malloc(sizeof(float) * n);
+    memcpy(z->Z, Z, sizeof(float) * n);
+    z->norm = (double*)calloc((size_t)n_ti * 4, sizeof(double));
+    z->bound = (double*)calloc((size_t)n_ti, sizeof(double));
+    /* per incidence node: trapezoid in vartheta_out of sin(vartheta_out) x (mean over the dphi nodes), times 1/2
+     * (= (1/4pi) int dOmega), for the four elements of row 1; and the bound of the rejection sampler */
+    double dth = ORA_PI / (n_to - 1);
+    for (int i = 0; i < n_ti; ++i) {
+        for (int o = 0; o < n_to; ++o) {
+            double w = (o == 0 || o == n_to - 1 ? 0.5 : 1.0) * sin(o * dth) * dth * 0.5;
+            for (int d = 0; d < n_dp; ++d) {
+                const float* e = z->Z + (((size_t)i * n_to + o) * n_dp + d) * 16;
+                for (int s = 0; s < 4; ++s) z->norm[4 * i + s] += w * (double)e[s] / n_dp;
+                double b = (double)e[0] + sqrt((double)e[1] * e[1] + (double)e[2] * e[2] + (double)e[3] * e[3]);
+                if (b > z->bound[i]) z->bound[i] = b;
+            }
+        }
+    }
+    return z;
+}
+
+/* trilinear interpolation; angles in degrees, dphi any real (periodic) */
+void ora_ztable_at(const ora_ztable* z, double ti_deg, double to_deg, double dphi_deg, double M[16])
+{
+    double xi = ti_deg * (z->n_ti - 1) / 180.0, xo = to_deg * (z->n_to - 1) / 180.0;
+    double xd = dphi_deg * z->n_dp / 360.0;
+    xd -= floor(xd / z->n_dp) * z->n_dp;
+    int i = (int)floor(xi), o = (int)floor(xo), d = (int)floor(xd);
+    if (i < 0) i = 0;
+    if (i > z->n_ti - 2) i = z->n_ti - 2;
+    if (o < 0) o = 0;
+    if (o > z->n_to - 2) o = z->n_to - 2;
+    if (d > z->n_dp - 1) d = z->n_dp - 1;
+    double wi = xi - i, wo = xo - o, wd = xd - d;
+    int d1 = (d + 1) % z->n_dp;
+    for (int k = 0; k < 16; ++k) M[k] = 0.0;
+    for (int a = 0; a < 2; ++a) for (int b = 0; b < 2; ++b) for (int c = 0; c < 2; ++c) {
+        double w = (a ? wi : 1 - wi) * (b ? wo : 1 - wo) * (c ? wd : 1 - wd);
+        const float* e = z->Z + (((size_t)(i + a) * z->n_to + (o + b)) * z->n_dp + (c ? d1 : d)) * 16;
+        for (int k = 0; k < 16; ++k) M[k] += w * (double)e[k];
+    }
+}
+
+/* (1/4pi) int dOmega_out of the scattered intensity for the grain-frame state S (any normalisation), incidence angle ti:
+ * linear interpolation of the per-node integrals.  It normalises the phase function: the probability density of the
+ * outgoing direction is I_out / (4 pi N). */
+double ora_ztable_norm(const ora_ztable* z, double ti_deg, const double Sg[4])
+{
+    double xi = ti_deg * (z->n_ti - 1) / 180.0;
+    int i = (int)floor(xi);
+    if (i < 0) i = 0;
+    if (i > z->n_ti - 2) i = z->n_ti - 2;
+    double w = xi - i, N = 0.0;
+    for (int s = 0; s < 4; ++s) N += ((1 - w) * z->norm[4 * i + s] + w * z->norm[4 * (i + 1) + s]) * Sg[s];
+    return N;
+}
+
+static void angles_gf(const double v[3], double* polar_deg, double* azim_deg)
+{
+    double r = sqrt(dot3(v, v));
+    double c = v[2] / r;
+    if (c > 1) c = 1;
+    if (c < -1) c = -1;
+    *polar_deg = acos(c) * 180.0 / ORA_PI;
+    *azim_deg = (v[0] * v[0] + v[1] * v[1] >= 1e-24) ? atan2(v[1], v[0]) * 180.0 / ORA_PI : 0.0;
+}
+
+/* Peel-off with the full Z: Stokes vector sent toward n_obs by a scattering of the state S_in (lab reference of n_in) on a
+ * grain aligned with b: into the grain frame (eq. 2, 3, 6, 7), Z s, back to the reference theta^_obs; divided by 4 pi N so
+ * that its I component integrates to S_in[0] over all observer directions. */
+void ora_peel_z(const struct ora_ztable* z, const double b[3], const double n_in[3], const double S_in[4], const double n_obs[3],
+                double S_out[4])
+{
+    double q[4], ce, se, ng[3], og[3], ti, pi_, to, po, M[16];
+    ora_quat_from_B(b, q);
+    ora_rot_to_gf(q, n_in, ng);
+    ora_rot_to_gf(q, n_obs, og);
+    double S[4] = { S_in[0], S_in[1], S_in[2], S_in[3] };
+    ora_eta_gf(q, n_in, &ce, &se);
+    ora_rotate_qu(S, ce, se);
+    angles_gf(ng, &ti, &pi_);
+    angles_gf(og, &to, &po);
+    ora_ztable_at(z, ti, to, po - pi_, M);
+    double N = ora_ztable_norm(z, ti, S);
+    double R[4];
+    for (int r = 0; r < 4; ++r) R[r] = (M[4*r] * S[0] + M[4*r+1] * S[1] + M[4*r+2] * S[2] + M[4*r+3] * S[3]) / (4 * ORA_PI * N) * S[0];
+    /* (the event's weight rides on S[0]: the phase function is normalised for the state s = S/S[0]; N is linear in S) */
+    ora_eta_gf(q, n_obs, &ce, &se);
+    ora_rotate_qu(R, ce, -se);
+    for (int r = 0; r < 4; ++r) S_out[r] = R[r];
+}
+
+/* Scattering with the full Z (S5 with reading R21).  Rejection sampling of the outgoing direction (after
+ * Whitney & Wolff 2002): candidates isotropic in the grain frame, cos(vartheta_out) = 1 - 2u, dphi = 2 pi u', accepted when
+ * u'' * bound < I_out(candidate) = row 1 of Z . s, bound = the larger of the two bracketing incidence nodes' bounds.
+ * Draws (R11): block 0 of event k = (cos, dphi, accept, next tau*), block b >= 1 = (cos, dphi, accept, -), at most 256
+ * candidates (the last one is taken).  Returns the number of candidates used. */
+int ora_scatter_z(const struct ora_ztable* z, const double b[3], const double n_in[3], const double S_in[4],
+                  uint64_t seed, uint64_t id, uint32_t k, double n_out[3], double S_out[4], double* tau_next)
+{
+    double q[4], ce, se, ng[3], ti, pi_;
+    ora_quat_from_B(b, q);
+    ora_rot_to_gf(q, n_in, ng);
+    double S[4] = { 1.0, S_in[1] / S_in[0], S_in[2] / S_in[0], S_in[3] / S_in[0] };
+    ora_eta_gf(q, n_in, &ce, &se);
+    ora_rotate_qu(S, ce, se);
+    angles_gf(ng, &ti, &pi_);
+    double xi = ti * (z->n_ti - 1) / 180.0;
+    int i = (int)floor(xi);
+    if (i < 0) i = 0;
+    if (i > z->n_ti - 2) i = z->n_ti - 2;
+    double bound = z->bound[i] > z->bound[i + 1] ? z->bound[i] : z->bound[i + 1];
+    uint32_t w[4];
+    double M[16], to = 0, dp = 0;
+    int rounds = 0;
+    for (uint32_t blk = 0; ; ++blk) {
+        draw(seed, id, k, blk, w);
+        if (blk == 0) *tau_next = -log(ora_u01(w[3]));
+        double ct = 1.0 - 2.0 * ora_u01(w[0]);
+        to = acos(ct) * 180.0 / ORA_PI;
+        dp = 360.0 * ora_u01(w[1]);
+        ora_ztable_at(z, ti, to, dp, M);
+        double Iout = M[0] * S[0] + M[1] * S[1] + M[2] * S[2] + M[3] * S[3];
+        ++rounds;
+        if (ora_u01(w[2]) * bound < Iout || rounds >= 256) break;
+    }
+    double R[4];
+    for (int r = 0; r < 4; ++r) R[r] = M[4*r] * S[0] + M[4*r+1] * S[1] + M[4*r+2] * S[2] + M[4*r+3] * S[3];
+    double I = R[0];
+    R[0] = 1.0; R[1] /= I; R[2] /= I; R[3] /= I;
+    /* outgoing direction in the grain frame, then to the lab (inverse of eq. 3), fp32 state (R12) */
+    double tr = to * ORA_PI / 180.0, pr = (pi_ + dp) * ORA_PI / 180.0;
+    double og[3] = { sin(tr) * cos(pr), sin(tr) * sin(pr), cos(tr) }, nl[3];
+    ora_rot_to_lab(q, og, nl);
+    for (int a = 0; a < 3; ++a) n_out[a] = (double)(float)nl[a];
+    ora_eta_gf(q, n_out, &ce, &se);
+    ora_rotate_qu(R, ce, -se);
+    for (int s = 0; s < 4; ++s) S_out[s] = R[s];
+    return rounds;
 }

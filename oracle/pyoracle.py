@@ -143,6 +143,13 @@ def lib(variant=None):
                                          C.POINTER(C.c_uint64)]),
         "ora_image_rays": (None, [C.c_void_p, C.c_void_p, C.c_void_p, C.POINTER(Observer), C.c_int, C.c_int, C.c_int, _dp,
                                   C.POINTER(OracleStats)]),
+        "ora_ztable_create": (C.c_void_p, [C.c_int, C.c_int, C.c_int, _fp]),
+        "ora_ztable_free": (None, [C.c_void_p]),
+        "ora_ztable_at": (None, [C.c_void_p, C.c_double, C.c_double, C.c_double, _dp]),
+        "ora_ztable_norm": (C.c_double, [C.c_void_p, C.c_double, _dp]),
+        "ora_peel_z": (None, [C.c_void_p, _dp, _dp, _dp, _dp, _dp]),
+        "ora_scatter_z": (C.c_int, [C.c_void_p, _dp, _dp, _dp, C.c_uint64, C.c_uint64, C.c_uint32, _dp, _dp, _D]),
+        "ora_model_set_ztable": (None, [C.c_void_p, C.c_void_p]),
         "ora_image": (None, [C.c_void_p, C.POINTER(_Events), C.POINTER(Observer), C.c_int, C.c_int, C.c_int,
                              C.c_int, _dp, C.c_void_p, C.POINTER(OracleStats)]),
     }
@@ -187,6 +194,11 @@ class OracleModel:
         if getattr(self, "h", None):
             self.L.ora_model_free(self.h)
             self.h = None
+
+    def set_ztable(self, ztab):
+        """Scatter and peel with the full Z (OracleZTable) instead of the F(Theta) table; None switches back."""
+        self._ztab = ztab
+        self.L.ora_model_set_ztable(self.h, None if ztab is None else ztab.h)
 
     def set_periodic(self, mask):
         """bit a of mask: axis a (0 x, 1 y, 2 z) is periodic (reading R20)."""
@@ -298,3 +310,31 @@ class OracleModel:
         self.L.ora_image_rays(self.h, None if sgrid is None else sgrid.ctypes.data, None if emis is None else emis.ctypes.data,
                               arr, n_obs, int(npx), int(npy), img, C.byref(st))
         return img, st
+
+
+class OracleZTable:
+    """Full scattering matrix of aligned grains in the grain frame, Z[n_ti, n_to, n_dp, 4, 4] (fp32), reading R21."""
+
+    def __init__(self, Z, variant=None):
+        self.L = lib(variant)
+        self.Z = np.ascontiguousarray(np.asarray(Z, np.float32))
+        assert self.Z.ndim == 5 and self.Z.shape[3:] == (4, 4)
+        self.h = self.L.ora_ztable_create(self.Z.shape[0], self.Z.shape[1], self.Z.shape[2], self.Z.reshape(-1))
+
+    def __del__(self):
+        if getattr(self, "h", None):
+            self.L.ora_ztable_free(self.h); self.h = None
+
+    def at(self, ti_deg, to_deg, dphi_deg):
+        M = np.zeros(16); self.L.ora_ztable_at(self.h, float(ti_deg), float(to_deg), float(dphi_deg), M); return M.reshape(4, 4)
+
+    def norm(self, ti_deg, Sg):
+        return self.L.ora_ztable_norm(self.h, float(ti_deg), _v(Sg, 4))
+
+    def peel(self, b, n_in, S_in, n_obs):
+        So = np.zeros(4); self.L.ora_peel_z(self.h, _v(b, 3), _v(n_in, 3), _v(S_in, 4), _v(n_obs, 3), So); return So
+
+    def scatter(self, b, n_in, S_in, seed, pid, k):
+        no = np.zeros(3); So = np.zeros(4); tn = C.c_double(0)
+        r = self.L.ora_scatter_z(self.h, _v(b, 3), _v(n_in, 3), _v(S_in, 4), int(seed), int(pid), int(k), no, So, C.byref(tn))
+        return no, So, tn.value, r

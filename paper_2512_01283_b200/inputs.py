@@ -53,6 +53,32 @@ def aligned_opacity(ratio=1.1, circ=0.02, albedo=0.5, n_inc=N_INC):
     return np.stack([1 + h * s2, h * s2, circ * s2, np.full_like(mu, albedo)], 1).astype(np.float32)
 
 
+def dipole_ztable(n_ti=37, n_to=37, n_dp=72, a_par=1.0, a_perp=1.0):
+    """Synthetic full scattering matrix of aligned grains: an induced dipole with polarizability
+    a_par along the grain axis (z of the grain frame) and a_perp across it (complex numbers allowed), Z[n_ti, n_to, n_dp, 4, 4]
+    on incidence angle, outgoing polar angle and azimuth difference, Stokes vectors referenced to (theta^, phi^) of each
+    direction in the grain frame (eq. 4-5), normalised so that the isotropic case is the Rayleigh matrix with mean(Z11) = 1.
+    A stand-in for the paper's dipole-approximation grain model, whose formulas are not in the paper's text."""
+    ti = np.radians(np.linspace(0.0, 180.0, n_ti))[:, None, None]
+    to = np.radians(np.linspace(0.0, 180.0, n_to))[None, :, None]
+    dp = np.radians(np.arange(n_dp) * 360.0 / n_dp)[None, None, :]
+    one = np.ones(np.broadcast_shapes(ti.shape, to.shape, dp.shape))
+    A = np.array([a_perp, a_perp, a_par], complex)
+    thi = np.stack([np.cos(ti) * one, 0 * one, -np.sin(ti) * one], -1)
+    phi = np.stack([0 * one, one, 0 * one], -1)
+    tho = np.stack([np.cos(to) * np.cos(dp) * one, np.cos(to) * np.sin(dp) * one, -np.sin(to) * one], -1)
+    pho = np.stack([-np.sin(dp) * one, np.cos(dp) * one, 0 * one], -1)
+    J = np.empty(one.shape + (2, 2), complex)
+    for r, eo in enumerate((tho, pho)):
+        for c, ei in enumerate((thi, phi)):
+            J[..., r, c] = (eo * A * ei).sum(-1)
+    # Mueller matrix of a Jones matrix: M = T (J kron J*) T^-1, coherency vector (tt*, tp*, pt*, pp*), V = i (tp* - pt*)
+    T = np.array([[1, 0, 0, 1], [1, 0, 0, -1], [0, 1, 1, 0], [0, 1j, -1j, 0]], complex)
+    K = np.einsum("...ab,...cd->...acbd", J, J.conj()).reshape(one.shape + (4, 4))
+    M = np.einsum("ij,...jk,kl->...il", T, K, np.linalg.inv(T)).real
+    return (1.5 * M).astype(np.float32)
+
+
 # ------------------------------------------------------------------------------------------
 # fields
 # ------------------------------------------------------------------------------------------
