@@ -190,6 +190,19 @@ int krp_image_rays(krp_grid* g, const krp_observer* obs, int n_obs, int npix_x, 
 int krp_freq_define(krp_grid* g, int n_freq, const krp_tables* tables, const float* kappa_scale, void* stream);
 int krp_freq_select(krp_grid* g, int bin, void* stream);
 
+/* ---- Full scattering matrix of aligned grains (eq. 10: "Z(Omega; Omega') depends on both the scattering angle
+ * and the local magnetic field orientation"; :107-109, :129 rejection sampling, reading R21) ------------
+ * Z (HOST, copied): [n_ti][n_to][n_dp][4][4] floats on the incidence angle vartheta_in = i 180/(n_ti-1) degrees, the outgoing
+ * polar angle vartheta_out = o 180/(n_to-1) and the azimuth difference dphi = phi_out - phi_in = d 360/n_dp (periodic), all in the
+ * Grain Frame (z_GF = B^ of the event cell, eq. 2-3); incoming and outgoing Stokes vectors are referenced to (theta^', phi^') of
+ * their own direction in that frame (eq. 4-5).  Trilinear interpolation.  Z[..][0][0] > 0 and row 1 must keep the scattered
+ * intensity positive for every physical Stokes vector.  With a Z table set, krp_transport samples the outgoing direction by
+ * rejection against row 1 of Z . s and applies Z (instead of the Theta, phi sampling and F(Theta) of krp_tables.mueller), and
+ * krp_image peels every event off with Z / (4 pi N), N the table's own integral of the scattered intensity.  The opacity table,
+ * albedo and event location are unchanged.  Needs the 16-byte cell layout (a field or a direction-dependent table at
+ * krp_grid_create; KRP_ERR_ARG otherwise) and no open source grid (KRP_ERR_STATE).  Z = NULL returns to F(Theta). */
+int krp_zmatrix_set(krp_grid* g, int n_ti, int n_to, int n_dp, const float* Z, void* stream);
+
 /* Counters (also the numerators of the roofline figures). */
 typedef struct krp_stats {
     uint64_t packets;         /* packets emitted */

@@ -116,6 +116,7 @@ struct krp_grid {
     double* d_flen = nullptr;
     uint64_t flen_cap = 0;
     float* d_emis = nullptr;        // padded thermal source of krp_image_rays
+    float* d_zt = nullptr; double* d_zt_norm = nullptr; double* d_zt_bound = nullptr;   // full Z of aligned grains (krp_zmatrix_set)
     uint64_t next_id = 0;
     uint64_t launches = 0;
     int transport_block = 256, image_block = 256, blocks_per_sm = 8;   // general mode: transport_block 128 (krp_grid_create)
@@ -195,6 +196,7 @@ extern "C" int krp_grid_destroy(krp_grid* g)
     cudaFree(g->d_bins); cudaFree(g->d_perm); cudaFree(g->d_scan);
     cudaFree(g->d_dir_bins); cudaFree(g->d_dir_scan); cudaFree(g->d_order);
     cudaFree(g->d_sgrid); cudaFree(g->d_sg_obs); cudaFree(g->d_flen); cudaFree(g->d_emis);
+    cudaFree(g->d_zt); cudaFree(g->d_zt_norm); cudaFree(g->d_zt_bound);
     free_records(g->q[0]); free_records(g->q[1]); free_records(g->ev); free_hits(g->hits);
     for (cudaEvent_t e : g->t_ev) cudaEventDestroy(e);
     if (g->h_ray_stats) cudaFreeHost(g->h_ray_stats);
@@ -690,7 +692,8 @@ extern "C" int krp_transport(krp_grid* g, uint64_t n_packets, uint64_t seed, voi
         }
         if (w + 1 < g->bins[g->cur_bin].max_waves) {
             TimedLaunch tl(g, st, KRP_T_SCATTER);
-            krp_k_scatter<<<grid_s, 128, 0, st>>>(g->m, g->d_ctl, g->ev, g->q[1 - in], 1 - in, seed);
+            if (g->m.z.zt) krp_k_scatter<true><<<grid_s, 128, 0, st>>>(g->m, g->d_ctl, g->ev, g->q[1 - in], 1 - in, seed);
+            else         krp_k_scatter<false><<<grid_s, 128, 0, st>>>(g->m, g->d_ctl, g->ev, g->q[1 - in], 1 - in, seed);
             g->launches++;
         }
     }
@@ -835,13 +838,15 @@ extern "C" int krp_image(krp_grid* g, const krp_observer* obs, int n_obs, int np
         const int slot = o % KRP_MAX_OBS_PACK;
         if (o > 0 && slot == 0) { krp_k_image_rewind<<<1, 1, 0, st>>>(g->d_ctl); g->launches++; }
         TimedLaunch tli(g, st, KRP_T_IMAGE);
-        if (g->m.scalar)
-            krp_k_image<true, false><<<pers, tb, 0, st>>>(g->m, g->d_ctl, g->ev, perm, g->obs_dev[o], nullptr, slot, o, npix_x, npix_y, flags, g->d_img);
-        else if (g->d_obs_cells)
-            krp_k_image<false, true><<<pers, tb, 0, st>>>(g->m, g->d_ctl, g->ev, perm, g->obs_dev[o],
-                                                          g->d_obs_cells + (size_t)o * g->npad, slot, o, npix_x, npix_y, flags, g->d_img);
-        else
-            krp_k_image<false, false><<<pers, tb, smem, st>>>(g->m, g->d_ctl, g->ev, perm, g->obs_dev[o], nullptr, slot, o, npix_x, npix_y, flags, g->d_img);
+        const bool zt = g->m.z.zt != nullptr;
+        float4* oc = g->d_obs_cells ? g->d_obs_cells + (size_t)o * g->npad : nullptr;
+#define KRP_IMG_ARGS g->m, g->d_ctl, g->ev, perm, g->obs_dev[o], oc, slot, o, npix_x, npix_y, flags, g->d_img
+        if (g->m.scalar)          krp_k_image<true, false, false><<<pers, tb, 0, st>>>(KRP_IMG_ARGS);
+        else if (oc && !zt)       krp_k_image<false, true, false><<<pers, tb, 0, st>>>(KRP_IMG_ARGS);
+        else if (oc)              krp_k_image<false, true, true><<<pers, tb, 0, st>>>(KRP_IMG_ARGS);
+        else if (!zt)             krp_k_image<false, false, false><<<pers, tb, smem, st>>>(KRP_IMG_ARGS);
+        else                      krp_k_image<false, false, true><<<pers, tb, smem, st>>>(KRP_IMG_ARGS);
+#undef KRP_IMG_ARGS
         g->launches++;
     }
     krp_k_events_clear<<<1, 1, 0, st>>>(g->d_ctl);
@@ -1046,6 +1051,7 @@ extern "C" int krp_sgrid_begin(krp_grid* g, const krp_observer* obs, int n_obs, 
     if (rc) return rc;
     if (n_obs > KRP_SG_MAX_OBS) return fail(KRP_ERR_ARG, "a source grid holds at most %d cameras", KRP_SG_MAX_OBS);
     if (g->m.periodic) return fail(KRP_ERR_STATE, "a source grid cannot be opened on a model with periodic boundaries");
+    if (g->m.z.zt) return fail(KRP_ERR_STATE, "a source grid cannot be opened while a full Z table is set");
     cudaStream_t st = (cudaStream_t)stream;
     rc = krp_sgrid_end(g);
     if (rc) return rc;
@@ -1215,6 +1221,49 @@ extern "C" int krp_freq_define(krp_grid* g, int n_freq, const krp_tables* tables
     g->bins.swap(nb);
     apply_tables(g, 0);
     return apply_scale(g, g->bins[0].kscale, st);
+}
+
+// ------------------------------------------------------------------------------------------
+// full scattering matrix of aligned grains (include/krp.h)
+// ------------------------------------------------------------------------------------------
+extern "C" int krp_zmatrix_set(krp_grid* g, int n_ti, int n_to, int n_dp, const float* Z, void* stream)
+{
+    if (!g) return fail(KRP_ERR_ARG, "grid is NULL");
+    cudaStream_t st = (cudaStream_t)stream;
+    CK(cudaStreamSynchronize(st));
+    cudaFree(g->d_zt); cudaFree(g->d_zt_norm); cudaFree(g->d_zt_bound);
+    g->d_zt = nullptr; g->d_zt_norm = nullptr; g->d_zt_bound = nullptr;
+    g->m.z = KrpZt{ nullptr, nullptr, nullptr, 0, 0, 0 };
+    if (!Z) return KRP_OK;
+    if (g->m.scalar) return fail(KRP_ERR_ARG, "a Z table needs the 16-byte cell layout: create the model with a field or a direction-dependent table");
+    if (g->d_sgrid) return fail(KRP_ERR_STATE, "close the source grid before setting a Z table");
+    if (n_ti < 2 || n_to < 2 || n_dp < 2 || (uint64_t)n_ti * n_to * n_dp > (1ull << 26)) return fail(KRP_ERR_ARG, "Z table: need n_ti, n_to, n_dp >= 2 and at most 2^26 nodes");
+    const size_t nn = (size_t)n_ti * n_to * n_dp;
+    std::vector<double> norm(4 * (size_t)n_ti, 0.0), bound(n_ti, 0.0);
+    // per incidence node: (1/4pi) integral over outgoing directions of row 1 (trapezoid in vartheta_out with sin, mean over dphi),
+    // and the bound of the rejection sampler max(Z11 + |(Z12, Z13, Z14)|)
+    const double dth = KRP_PI_D / (n_to - 1);
+    for (int i = 0; i < n_ti; ++i)
+        for (int o = 0; o < n_to; ++o) {
+            const double w = (o == 0 || o == n_to - 1 ? 0.5 : 1.0) * std::sin(o * dth) * dth * 0.5;
+            for (int d = 0; d < n_dp; ++d) {
+                const float* e = Z + (((size_t)i * n_to + o) * n_dp + d) * 16;
+                for (int k = 0; k < 16; ++k) if (!std::isfinite(e[k])) return fail(KRP_ERR_ARG, "Z table: entry is not finite");
+                if (!(e[0] > 0.f)) return fail(KRP_ERR_ARG, "Z table: Z11 must be positive (node %d,%d,%d)", i, o, d);
+                for (int s = 0; s < 4; ++s) norm[4 * i + s] += w * (double)e[s] / n_dp;
+                const double b = (double)e[0] + std::sqrt((double)e[1] * e[1] + (double)e[2] * e[2] + (double)e[3] * e[3]);
+                if (b > bound[i]) bound[i] = b;
+            }
+        }
+    CK(cudaMalloc(&g->d_zt, sizeof(float) * 16 * nn));
+    CK(cudaMalloc(&g->d_zt_norm, sizeof(double) * 4 * n_ti));
+    CK(cudaMalloc(&g->d_zt_bound, sizeof(double) * n_ti));
+    CK(cudaMemcpyAsync(g->d_zt, Z, sizeof(float) * 16 * nn, cudaMemcpyHostToDevice, st));
+    CK(cudaMemcpyAsync(g->d_zt_norm, norm.data(), sizeof(double) * 4 * n_ti, cudaMemcpyHostToDevice, st));
+    CK(cudaMemcpyAsync(g->d_zt_bound, bound.data(), sizeof(double) * n_ti, cudaMemcpyHostToDevice, st));
+    CK(cudaStreamSynchronize(st));
+    g->m.z = KrpZt{ g->d_zt, g->d_zt_norm, g->d_zt_bound, n_ti, n_to, n_dp };
+    return KRP_OK;
 }
 
 extern "C" int krp_timing_enable(krp_grid* g, int on)

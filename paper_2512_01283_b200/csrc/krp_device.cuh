@@ -18,6 +18,14 @@
 // ------------------------------------------------------------------------------------------
 // by-value kernel parameters
 // ------------------------------------------------------------------------------------------
+// full scattering matrix Z(Omega;Omega') of aligned grains in the grain frame (R21)
+struct KrpZt {
+    const float* zt;       // [ni][no][nd][16], or NULL
+    const double* norm;    // [ni][4]  (1/4pi) integral of row 1 over outgoing directions
+    const double* bound;   // [ni]     bound of the rejection sampler
+    int ni, no, nd;
+};
+
 struct KrpModel {
     int nx, ny, nz;
     uint32_t ncell;
@@ -51,6 +59,8 @@ struct KrpModel {
     int max_scatter;
     int scalar;
     int periodic;          // bit a: axis a is periodic (R20); only with the 16-byte cell layout
+    // full scattering matrix Z(Omega;Omega') of aligned grains in the grain frame (R21), or zt = NULL: F(Theta) of `mueller`
+    KrpZt z;
     // source
     int src_kind, emit_records;
     float src_n[3];

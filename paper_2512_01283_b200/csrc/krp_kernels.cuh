@@ -902,11 +902,79 @@ __device__ __forceinline__ void krp_rot_qu(double& Q, double& U, double c2, doub
 }
 
 // ------------------------------------------------------------------------------------------
+// NEXT-2: full scattering matrix Z(vartheta_in, vartheta_out, dphi) in the grain frame (R21): trilinear interpolation of
+// `rows` rows (row 1 alone decides the acceptance of a candidate direction), angles in degrees, dphi periodic
+// ------------------------------------------------------------------------------------------
+template <typename T>
+__device__ __forceinline__ void krp_zt_at(const KrpZt g, T ti_deg, T to_deg, T dphi_deg, int rows, T M[16])
+{
+    const T xi = ti_deg * (T)(g.ni - 1) / T(180), xo = to_deg * (T)(g.no - 1) / T(180);
+    T xd = dphi_deg * (T)g.nd / T(360);
+    xd -= floor(xd / (T)g.nd) * (T)g.nd;
+    int i = max(0, min((int)floor(xi), g.ni - 2)), o = max(0, min((int)floor(xo), g.no - 2)), d = min((int)floor(xd), g.nd - 1);
+    const T wi = xi - (T)i, wo = xo - (T)o, wd = xd - (T)d;
+    const int d1 = (d + 1) % g.nd;
+    for (int k = 0; k < 4 * rows; ++k) M[k] = T(0);
+#pragma unroll
+    for (int a = 0; a < 2; ++a)
+#pragma unroll
+        for (int b = 0; b < 2; ++b)
+#pragma unroll
+            for (int c = 0; c < 2; ++c) {
+                const T w = (a ? wi : T(1) - wi) * (b ? wo : T(1) - wo) * (c ? wd : T(1) - wd);
+                const float4* e = reinterpret_cast<const float4*>(g.zt + (((size_t)(i + a) * g.no + (o + b)) * g.nd + (c ? d1 : d)) * 16);
+                for (int r = 0; r < rows; ++r) {
+                    const float4 v = __ldg(e + r);
+                    M[4 * r] += w * (T)v.x; M[4 * r + 1] += w * (T)v.y; M[4 * r + 2] += w * (T)v.z; M[4 * r + 3] += w * (T)v.w;
+                }
+            }
+}
+
+// I1 with the full Z (R21): both directions into the grain frame of the event cell (z_GF = B^, x_GF, y_GF = theta^, phi^ of B^:
+// eq. 2 is R_z(phi_B) R_y(theta_B)), Stokes reference lab -> grain frame (eq. 6-7), Z s / (4 pi N), back to theta^_obs.
+__device__ __forceinline__ void krp_peel_z(const KrpZt g, const float bh[3], const float n[3], float4 Se, const float on[3], const float oth[3], const float oph[3], float S[4])
+{
+    float thB[3], phB[3], th[3], ph[3];
+    krp_basis<float>(bh, thB, phB);
+    krp_basis<float>(n, th, ph);
+    const float inv_b = rsqrtf(bh[0] * bh[0] + bh[1] * bh[1] + bh[2] * bh[2]);
+    const float ngx = n[0] * thB[0] + n[1] * thB[1] + n[2] * thB[2], ngy = n[0] * phB[0] + n[1] * phB[1], ngz = (n[0] * bh[0] + n[1] * bh[1] + n[2] * bh[2]) * inv_b;
+    const float ogx = on[0] * thB[0] + on[1] * thB[1] + on[2] * thB[2], ogy = on[0] * phB[0] + on[1] * phB[1],
+                ogz = (on[0] * bh[0] + on[1] * bh[1] + on[2] * bh[2]) * inv_b;
+    const float r2d = 57.29577951308232f;
+    const float ti = atan2f(sqrtf(ngx * ngx + ngy * ngy), ngz) * r2d, to = atan2f(sqrtf(ogx * ogx + ogy * ogy), ogz) * r2d;
+    const float pi_ = (ngx * ngx + ngy * ngy >= 1e-24f) ? atan2f(ngy, ngx) * r2d : 0.f;
+    const float po = (ogx * ogx + ogy * ogy >= 1e-24f) ? atan2f(ogy, ogx) * r2d : 0.f;
+    float c2, s2;
+    krp_eta2<float>(th[0] * bh[0] + th[1] * bh[1] + th[2] * bh[2], ph[0] * bh[0] + ph[1] * bh[1], c2, s2);
+    const float I = Se.x, Q = Se.x * (c2 * Se.y + s2 * Se.z), U = Se.x * (c2 * Se.z - s2 * Se.y), V = Se.x * Se.w;   // eq. 7
+    float M[16];
+    krp_zt_at<float>(g, ti, to, po - pi_, 4, M);
+    // N: linear interpolation of the per-node integrals of row 1
+    float N;
+    {
+        const float xi = ti * (float)(g.ni - 1) * (1.f / 180.f);
+        const int i = max(0, min((int)xi, g.ni - 2));
+        const float w = xi - (float)i;
+        const double* a = g.norm + 4 * i;
+        N = ((1.f - w) * (float)a[0] + w * (float)a[4]) * I + ((1.f - w) * (float)a[1] + w * (float)a[5]) * Q
+          + ((1.f - w) * (float)a[2] + w * (float)a[6]) * U + ((1.f - w) * (float)a[3] + w * (float)a[7]) * V;
+    }
+    const float f = 0.07957747154594767f * I / N;
+    float R[4];
+#pragma unroll
+    for (int r = 0; r < 4; ++r) R[r] = f * (M[4 * r] * I + M[4 * r + 1] * Q + M[4 * r + 2] * U + M[4 * r + 3] * V);
+    krp_eta2<float>(oth[0] * bh[0] + oth[1] * bh[1] + oth[2] * bh[2], oph[0] * bh[0] + oph[1] * bh[1] + oph[2] * bh[2], c2, s2);
+    S[0] = R[0]; S[1] = c2 * R[1] - s2 * R[2]; S[2] = s2 * R[1] + c2 * R[2]; S[3] = R[3];
+}
+
+// ------------------------------------------------------------------------------------------
 // T6  scattering (step S5 of DESIGN.md).  One thread per event
 // of the wave, fp64.  Draws of block 0 of event k: (Theta, phi candidate, accept, next tau*);
 // blocks >= 1: two more (phi, accept) pairs each, at most 64 rounds.
 // ------------------------------------------------------------------------------------------
-__global__ void __launch_bounds__(128, 8) krp_k_scatter(KrpModel g, KrpCtl* ctl, KrpRecords ev, KrpRecords qo, int out,
+template <bool ZT>      // ZT: the outgoing direction and Stokes vector come from the full Z table (NEXT-2), else from F(Theta)
+__global__ void __launch_bounds__(128, ZT ? 4 : 8) krp_k_scatter(KrpModel g, KrpCtl* ctl, KrpRecords ev, KrpRecords qo, int out,
                                                      unsigned long long seed)
 {
     const unsigned long long e0 = ctl->ev_begin;
@@ -954,9 +1022,49 @@ __global__ void __launch_bounds__(128, 8) krp_k_scatter(KrpModel g, KrpCtl* ctl,
             double r = krp_rsqrt_near1(krp_dot(ng, ng));       // a rotation of a direction that is unit to fp32 rounding
             ng[0] *= r; ng[1] *= r; ng[2] *= r;
         }
+        double tau_next, nog[3];
+        if (ZT) {
+            // NEXT-2 (R21): outgoing direction by rejection sampling against the full Z: candidates isotropic in the
+            // grain frame, block 0 of event k = (cos, dphi, accept, next tau*), block b >= 1 = (cos, dphi, accept, -), at most 256
+            const double r2d = 57.29577951308232087680;
+            const double ti = acos(fmin(fmax(ng[2], -1.0), 1.0)) * r2d;
+            const double pin = (ng[0] * ng[0] + ng[1] * ng[1] >= 1e-24) ? atan2(ng[1], ng[0]) * r2d : 0.0;
+            double bound;
+            {
+                const double xi = ti * (double)(g.z.ni - 1) / 180.0;
+                const int i = max(0, min((int)floor(xi), g.z.ni - 2));
+                bound = fmax(g.z.bound[i], g.z.bound[i + 1]);
+            }
+            double to = 0.0, dp = 0.0;
+            tau_next = 0.0;
+            int rounds = 0;
+            for (uint32_t blk = 0; ; ++blk) {
+                const uint4 w = krp_philox(seed, id, kb, blk);
+                if (blk == 0u) tau_next = -log(krp_u01(w.w));
+                to = acos(1.0 - 2.0 * krp_u01(w.x)) * r2d;
+                dp = 360.0 * krp_u01(w.y);
+                double M1[16];
+                krp_zt_at<double>(g.z, ti, to, dp, 1, M1);
+                const double Iout = M1[0] + M1[1] * Q + M1[2] * U + M1[3] * V;
+                ++rounds;
+                if (krp_u01(w.z) * bound < Iout || rounds >= 256) break;
+            }
+            double M[16];
+            krp_zt_at<double>(g.z, ti, to, dp, 4, M);
+            {
+                const double I2 = M[0] + M[1] * Q + M[2] * U + M[3] * V, inv = 1.0 / I2;
+                const double Q2 = M[4] + M[5] * Q + M[6] * U + M[7] * V, U2 = M[8] + M[9] * Q + M[10] * U + M[11] * V,
+                             V2 = M[12] + M[13] * Q + M[14] * U + M[15] * V;
+                Q = Q2 * inv; U = U2 * inv; V = V2 * inv;      // referenced to theta^ of the outgoing direction in the grain frame
+            }
+            double st, ct, sp, cp;
+            sincos(to * (KRP_PI_D / 180.0), &st, &ct);
+            sincos((pin + dp) * (KRP_PI_D / 180.0), &sp, &cp);
+            nog[0] = st * cp; nog[1] = st * sp; nog[2] = ct;
+        } else {
         // draws
         uint4 w = krp_philox(seed, id, kb, 0u);
-        const double tau_next = -log(krp_u01(w.w));
+        tau_next = -log(krp_u01(w.w));
         double theta;   // Theta from the piecewise-linear CDF (R13), in units of the table spacing 180 deg/(n_ang-1)
         {
             double u = krp_u01(w.x);
@@ -1000,7 +1108,7 @@ __global__ void __launch_bounds__(128, 8) krp_k_scatter(KrpModel g, KrpCtl* ctl,
         krp_basis_unit_d(ng, thp, php);
         double st, ct;
         sincospi(theta * g.inv_nang1, &st, &ct);
-        double epar[3], nog[3], eout[3], shat[3];
+        double epar[3], eout[3], shat[3];
         for (int j = 0; j < 3; ++j) epar[j] = cphi * thp[j] + sphi * php[j];
         for (int j = 0; j < 3; ++j) nog[j] = ct * ng[j] + st * epar[j];
         krp_rot_qu(Q, U, cphi * cphi - sphi * sphi, 2.0 * sphi * cphi);      // reference e_par
@@ -1017,6 +1125,7 @@ __global__ void __launch_bounds__(128, 8) krp_k_scatter(KrpModel g, KrpCtl* ctl,
         {
             double ce = krp_dot(eout, th2), se = krp_dot(th2, shat);
             krp_rot_qu(Q, U, ce * ce - se * se, 2.0 * se * ce);                // reference theta^ of n'_GF
+        }
         }
         // back to the lab: inverse of eq. 3, direction stored in fp32 (R12)
         double nl[3] = { nog[0], nog[1], nog[2] };
@@ -1319,8 +1428,8 @@ __device__ __forceinline__ float krp_raya_step(KrpRayA& r, const KrpRayAConst& k
     return ds;
 }
 
-template <bool SCALAR, bool PRE>
-__global__ void __launch_bounds__(256, SCALAR ? KRP_IMAGE_SCALAR_MIN_BLOCKS : KRP_IMAGE_MIN_BLOCKS) krp_k_image(KrpModel g, KrpCtl* ctl, KrpRecords ev,
+template <bool SCALAR, bool PRE, bool ZT>      // ZT: peel-off with the full Z of aligned grains (NEXT-2) instead of F(Theta)
+__global__ void __launch_bounds__(256, SCALAR ? KRP_IMAGE_SCALAR_MIN_BLOCKS : (ZT ? 4 : KRP_IMAGE_MIN_BLOCKS)) krp_k_image(KrpModel g, KrpCtl* ctl, KrpRecords ev,
                                                    const unsigned int* __restrict__ perm, const KrpObserverDev ob,
                                                    const float4* __restrict__ obs_cell,
                                                    int slot, int obs_index, int npx, int npy, int flags, double* __restrict__ img)
@@ -1365,10 +1474,17 @@ __global__ void __launch_bounds__(256, SCALAR ? KRP_IMAGE_SCALAR_MIN_BLOCKS : KR
             const float4 pc = ev.pc[e], Se = ev.S[e];
             const uint32_t k = __float_as_uint(nk.w) & ~KRP_TERM_BIT;
             float S[4];
-            if (k == 0u) { S[0] = Se.x * 0.07957747154594767f; S[1] = S[2] = S[3] = 0.f; }
-            else { const float n[3] = { nk.x, nk.y, nk.z }; krp_peel(g, n, Se, ob, S); }
-            // ray set-up
             const uint32_t c0 = __float_as_uint(pc.w);
+            if (k == 0u) { S[0] = Se.x * 0.07957747154594767f; S[1] = S[2] = S[3] = 0.f; }
+            else {
+                const float n[3] = { nk.x, nk.y, nk.z };
+                if (ZT) {                    // full Z of aligned grains: the peel-off depends on the field of the event cell (R21)
+                    const float4 cb = __ldg(g.cell + c0);
+                    const float bh[3] = { cb.y, cb.z, cb.w };
+                    krp_peel_z(g.z, bh, n, Se, rc.n, rc.th, rc.ph, S);
+                } else krp_peel(g, n, Se, ob, S);
+            }
+            // ray set-up
             KrpRayA r;
             r.t = 0.f; r.c = c0;
             r.tx = ob.n[0] > 0.f ? (1.f - pc.x) * ob.dt[0] : (ob.n[0] < 0.f ? pc.x * ob.dt[0] : KRP_INF_F);

@@ -18,7 +18,7 @@ SYMBOLS = [
     "krp_events_reserve", "krp_transport", "krp_packet_id_set", "krp_image", "krp_image_get",
     "krp_image_reset", "krp_stats_get", "krp_stats_reset", "krp_events_get", "krp_events_select", "krp_events_clear",
     "krp_tune", "krp_tune_schedule", "krp_timing_enable", "krp_timing_get", "krp_launch_count",
-    "krp_sgrid_begin", "krp_sgrid_get", "krp_sgrid_reset", "krp_sgrid_end", "krp_image_rays", "krp_freq_define", "krp_freq_select",
+    "krp_sgrid_begin", "krp_sgrid_get", "krp_sgrid_reset", "krp_sgrid_end", "krp_image_rays", "krp_freq_define", "krp_freq_select", "krp_zmatrix_set",
 ]
 T_FLIGHT, T_SCATTER, T_ORDER, T_IMAGE, T_EMIT, T_DEPOSIT, T_RAYS, T_COUNT = 0, 1, 2, 3, 4, 5, 6, 7
 T_NAMES = ("flight", "scatter", "order", "image", "emit", "deposit", "rays")
@@ -68,7 +68,10 @@ def lib():
     if _lib is not None:
         return _lib
     path = _build.LIB
-    if _build.stale():
+    override = os.environ.get("KRP_LIBRARY")          # development: a library built with other compile-time options (A/B runs)
+    if override:
+        path = override
+    elif _build.stale():
         try:
             _build.build()
         except Exception as exc:
@@ -76,7 +79,7 @@ def lib():
                               "rebuilt (%s); run `python -m paper_2512_01283_b200._build`" % (_build.source_id(), exc)) from exc
     L = C.CDLL(path)
     L.krp_version.restype = C.c_char_p
-    if _build.source_id().encode() not in L.krp_version():
+    if not override and _build.source_id().encode() not in L.krp_version():
         raise ImportError("libkrp.so reports %r, the sources beside it have build id %s" % (L.krp_version(), _build.source_id()))
     vp, u64, i32 = C.c_void_p, C.c_uint64, C.c_int
     sig = {
@@ -103,6 +106,7 @@ def lib():
         "krp_timing_get": (i32, [vp, vp, vp]),
         "krp_tune_schedule": (i32, [vp, i32, i32, i32]),
         "krp_launch_count": (u64, [vp]),
+        "krp_zmatrix_set": (i32, [vp, i32, i32, i32, vp, vp]),
         "krp_freq_define": (i32, [vp, i32, C.POINTER(Tables), vp, vp]),
         "krp_freq_select": (i32, [vp, i32, vp]),
         "krp_sgrid_begin": (i32, [vp, C.POINTER(Observer), i32, vp]),
@@ -274,6 +278,16 @@ class Grid:
 
     def events_clear(self, stream=None):
         _check(lib().krp_events_clear(self._h, _stream(stream)))
+
+    # --- full scattering matrix of aligned grains ---
+    def zmatrix_set(self, Z, stream=None):
+        """Z[n_ti, n_to, n_dp, 4, 4] (fp32) in the grain frame, or None to return to the F(Theta) table."""
+        if Z is None:
+            _check(lib().krp_zmatrix_set(self._h, 0, 0, 0, None, _stream(stream)))
+            return
+        Z = np.ascontiguousarray(np.asarray(Z, np.float32))
+        assert Z.ndim == 5 and Z.shape[3:] == (4, 4)
+        _check(lib().krp_zmatrix_set(self._h, Z.shape[0], Z.shape[1], Z.shape[2], C.c_void_p(Z.ctypes.data), _stream(stream)))
 
     # --- frequency bins ---
     def freq_define(self, tables, kappa_scale, stream=None):

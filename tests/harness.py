@@ -2,7 +2,7 @@
 (paper_2512_01283_b200.inputs) and compare their outputs.  No arithmetic of the method here."""
 import numpy as np
 
-from oracle import OracleModel, OracleEvents, OracleStats, Observer as OraObserver
+from oracle import OracleModel, OracleEvents, OracleStats, OracleZTable, Observer as OraObserver
 
 
 def oracle_model(cfg, variant=None):
@@ -13,6 +13,8 @@ def oracle_model(cfg, variant=None):
     m.source_set(s["kind"], s["pos"], s["dir"], s.get("cell_weight"), s.get("emit_records", 0))
     if cfg.get("periodic"):
         m.set_periodic(cfg["periodic"])
+    if cfg.get("ztable") is not None:
+        m.set_ztable(OracleZTable(cfg["ztable"], variant=variant))
     return m
 
 
@@ -52,6 +54,8 @@ def gpu_grid(cfg, device="cuda", host_inputs=False):
     if w is not None:
         w = torch.from_numpy(np.ascontiguousarray(w, np.float32).ravel()).to(device)
     g.source_set(s["kind"], s["pos"], s["dir"], w, s.get("emit_records", 0))
+    if cfg.get("ztable") is not None:
+        g.zmatrix_set(cfg["ztable"])
     return g
 
 
