@@ -15,6 +15,10 @@
 #include <new>
 #include <vector>
 
+#ifndef KRP_SORT_BLOCK_LOG2
+#define KRP_SORT_BLOCK_LOG2 6      // blocks of 64^3 cells in the imaging order (C5 imaging: 16^3 383 ms, 32^3 364 ms, 64^3 357 ms; profiles/r2q_README.md)
+#endif
+
 static thread_local char g_err[512] = "";
 
 static int fail(int code, const char* fmt, ...)
@@ -393,6 +397,7 @@ extern "C" int krp_grid_create(krp_grid** out, int nx, int ny, int nz, const dou
     m.nx = nx; m.ny = ny; m.nz = nz; m.ncell = (uint32_t)((uint64_t)nx * ny * nz);
     m.px = nx + 2; m.py = ny + 2; m.pxy = (uint32_t)m.px * (uint32_t)m.py;
     g->npad = m.pxy * (uint32_t)(nz + 2);
+    m.npad = g->npad;
     {
         auto magic = [](uint32_t d, uint32_t& mm, uint32_t& ss) {
             uint32_t l = 0;
@@ -443,13 +448,14 @@ extern "C" int krp_grid_create(krp_grid** out, int nx, int ny, int nz, const dou
     rc = upload_cells(g, density, bfield, mem, st);
     if (rc) return rc;
     m.kr = g->d_kr; m.cell = g->d_cell;
-    // bins of the imaging order: blocks of 32^3 cells, inside a block one cache line of cells along x per bin
+    // bins of the imaging order: blocks of 64^3 cells, inside a block one cache line of cells along x per bin
     // (32 x 4 B or 8 x 16 B), at most 2^25 bins
     {
         KrpSortGeom& sg = g->sort_geom;
-        sg.B = 5; sg.ls = m.scalar ? 5 : 3;
-        sg.nbx = ((uint32_t)m.px + 31u) >> 5; sg.nby = ((uint32_t)m.py + 31u) >> 5;
-        const uint64_t nblk = (uint64_t)sg.nbx * sg.nby * (((uint32_t)nz + 2u + 31u) >> 5);
+        sg.B = KRP_SORT_BLOCK_LOG2; sg.ls = m.scalar ? 5 : 3;
+        const uint32_t bm = (1u << sg.B) - 1u;
+        sg.nbx = ((uint32_t)m.px + bm) >> sg.B; sg.nby = ((uint32_t)m.py + bm) >> sg.B;
+        const uint64_t nblk = (uint64_t)sg.nbx * sg.nby * (((uint32_t)nz + 2u + bm) >> sg.B);
         while (sg.ls < sg.B && (nblk << (3 * sg.B - sg.ls)) >= (1ull << 25)) sg.ls++;
         if ((nblk << (3 * sg.B - sg.ls)) >= (1ull << 31)) return fail(KRP_ERR_ARG, "grid too large for the imaging order");
         g->n_bins = (uint32_t)(nblk << (3 * sg.B - sg.ls)) + 1;
@@ -682,12 +688,12 @@ extern "C" int krp_transport(krp_grid* g, uint64_t n_packets, uint64_t seed, voi
             // step 1 of the two-step form: the flights of this wave, re-marched over their path lengths, deposit into S
             TimedLaunch tl(g, st, KRP_T_DEPOSIT);
             const KrpEmitSrc es = w == 0 ? es0 : KrpEmitSrc{ nullptr, 0, 0 };
-            int G = 1;
-            while (G < g->sg_n_obs && G < 8) G <<= 1;
-            const unsigned need_d = (unsigned)(((uint64_t)n * G + 255u) / 256u);
-            const unsigned grid_d = need_d < pers ? need_d : pers;
-            if (g->m.scalar) krp_k_deposit<true><<<grid_d, 256, 0, st>>>(g->m, g->d_ctl, g->q[in], in, es, flen, g->d_sg_obs, g->sg_n_obs, G, g->d_sgrid, &g->d_ctl->sg_segments);
-            else             krp_k_deposit<false><<<grid_d, 256, 0, st>>>(g->m, g->d_ctl, g->q[in], in, es, flen, g->d_sg_obs, g->sg_n_obs, G, g->d_sgrid, &g->d_ctl->sg_segments);
+            const unsigned need_d = (n + 127u) / 128u;
+            const unsigned pers_d = (unsigned)g->n_sm * 8u;
+            const unsigned grid_d = need_d < pers_d ? need_d : pers_d;
+            const size_t smem_d = (size_t)g->sg_n_obs * 2 * 128 * sizeof(float4);
+            if (g->m.scalar) krp_k_deposit<true><<<grid_d, 128, smem_d, st>>>(g->m, g->d_ctl, g->q[in], in, es, flen, g->d_sg_obs, g->sg_n_obs, g->d_sgrid, &g->d_ctl->sg_segments);
+            else             krp_k_deposit<false><<<grid_d, 128, smem_d, st>>>(g->m, g->d_ctl, g->q[in], in, es, flen, g->d_sg_obs, g->sg_n_obs, g->d_sgrid, &g->d_ctl->sg_segments);
             g->launches++;
         }
         if (w + 1 < g->bins[g->cur_bin].max_waves) {
@@ -1068,6 +1074,9 @@ extern "C" int krp_sgrid_begin(krp_grid* g, const krp_observer* obs, int n_obs, 
     CK(cudaStreamSynchronize(st));
     g->sg_n_obs = n_obs;
     g->sg_obs_host.assign(obs, obs + n_obs);
+    const int smem_d = n_obs * 2 * 128 * (int)sizeof(float4);
+    CK(cudaFuncSetAttribute(krp_k_deposit<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_d));
+    CK(cudaFuncSetAttribute(krp_k_deposit<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, smem_d));
     return KRP_OK;
 }
 

@@ -58,6 +58,7 @@ struct KrpModel {
     float w_min;
     int max_scatter;
     int scalar;
+    uint32_t npad;         // padded cells (px * py * (nz+2)); the cell arrays have a margin of pxy elements on either side
     int periodic;          // bit a: axis a is periodic (R20); only with the 16-byte cell layout
     // full scattering matrix Z(Omega;Omega') of aligned grains in the grain frame (R21), or zt = NULL: F(Theta) of `mueller`
     KrpZt z;
@@ -68,6 +69,15 @@ struct KrpModel {
     float src_p[3];
     const double* src_cdf; // [ncell] running sum of cell weights (unpadded order) or NULL
 };
+
+// Bounds check of every cell gather, compiled in with -DKRP_CHECK only (profiles/r2_bounds_check.md; compute-sanitizer is
+// closed on this pool): an index outside the allocation (padded array plus its margin of one plane on either side, which the
+// look-ahead loads may touch) traps, and the next synchronising call of the library returns KRP_ERR_CUDA.
+#ifdef KRP_CHECK
+#define KRP_CK(g, c) do { const long long c_ = (long long)(int)(c); if (c_ < -(long long)(g).pxy || c_ >= (long long)(g).npad + (long long)(g).pxy) __trap(); } while (0)
+#else
+#define KRP_CK(g, c) do { } while (0)
+#endif
 
 __device__ __forceinline__ uint32_t krp_pad_id(const KrpModel& g, int ix, int iy, int iz)
 {

@@ -373,6 +373,7 @@ __global__ void __launch_bounds__(256, 3) krp_k_flight_scalar(KrpModel g, KrpCtl
                 p0[0] = pc_.x; p0[1] = pc_.y; p0[2] = pc_.z; c0 = __float_as_uint(pc_.w);
                 krp_ray_init(g, c0, p0, n, ray);
                 ax = -1;
+                KRP_CK(g, ray.c);
                 kr = __ldg(g.kr + ray.c);
                 status = KRP_RUN;
             }
@@ -420,6 +421,7 @@ __global__ void __launch_bounds__(256, 3) krp_k_flight_scalar(KrpModel g, KrpCtl
                 } else {
                     D -= (double)dt1;
                     krp_ray_advance(ray, ax);
+                    KRP_CK(g, ray.c);
                     kr = __ldg(g.kr + ray.c);
                     if (kr < 0.f) status = KRP_ESC;  // halo: the packet left the grid
                 }
@@ -450,14 +452,17 @@ __global__ void __launch_bounds__(256, 4) krp_k_flight_scalar_static(KrpModel g,
         bool hit = false;
         int ax_cur = -1, ax_nxt, ax_new;
         uint32_t c_cur = ray.c;
+        KRP_CK(g, c_cur);
         float kr_cur = __ldg(g.kr + c_cur);
         float ds_cur = krp_ray_advance(ray, ax_nxt);
         uint32_t c_nxt = ray.c;
+        KRP_CK(g, c_nxt);
         float kr_nxt = __ldg(g.kr + c_nxt);
         float ds_nxt = krp_ray_advance(ray, ax_new);
 #pragma unroll 2
         for (;;) {
             const uint32_t c_new = ray.c;
+            KRP_CK(g, (int)c_new);
             const float kr_new = __ldg(g.kr + (int)c_new);       // signed: the look-ahead may sit before the array's first cell
             const float dt1 = g.a1c * kr_cur * ds_cur;
             if ((double)dt1 >= D) { hit = true; break; }      // event inside the current cell
@@ -714,6 +719,7 @@ __global__ void __launch_bounds__(TPB, MINB) krp_k_flight_general(KrpModel g, Kr
             krp_rayd_init(g, __float_as_uint(pc.w), p0, n, ray);
             // the first cell of the new flight goes to registers of its own and is taken over one step later: the warp's other
             // flights march on while it is in flight (a register is scoreboarded per warp, whoever's lanes wait for it)
+            KRP_CK(g, ray.c);
             asm volatile("ld.global.nc.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(cl_f.x), "=f"(cl_f.y), "=f"(cl_f.z), "=f"(cl_f.w) : "l"(g.cell + ray.c));
             fresh = true;
             nd[0] = n[0]; nd[1] = n[1]; nd[2] = n[2];
@@ -744,6 +750,7 @@ __global__ void __launch_bounds__(TPB, MINB) krp_k_flight_general(KrpModel g, Kr
             // the next cell is requested now, so that its latency overlaps the fp64 update of this one
             const uint32_t c_next = ray.c + (uint32_t)(ax ? ray.sx : (ay ? ray.sy : ray.sz));
             float4 cn;      // a load the compiler may neither duplicate nor move: it has to be in flight during the update below
+            KRP_CK(g, c_next);
             asm volatile("ld.global.nc.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(cn.x), "=f"(cn.y), "=f"(cn.z), "=f"(cn.w) : "l"(g.cell + c_next));
             if (cl.x > 0.f) {
                 KrpCellCoef cc;
@@ -794,6 +801,7 @@ __global__ void __launch_bounds__(TPB, MINB) krp_k_flight_general(KrpModel g, Kr
                 int off[3] = { 0, 0, 0 };
                 if (g.periodic && nwrap < KRP_MAX_WRAPS && krp_wrap(g, ray.c, off)) {
                     ++nwrap;
+                    KRP_CK(g, ray.c);
                     asm volatile("ld.global.nc.v4.f32 {%0, %1, %2, %3}, [%4];" : "=f"(cl.x), "=f"(cl.y), "=f"(cl.z), "=f"(cl.w) : "l"(g.cell + ray.c));
                 } else status = KRP_ESC;
             }
@@ -1479,6 +1487,7 @@ __global__ void __launch_bounds__(256, SCALAR ? KRP_IMAGE_SCALAR_MIN_BLOCKS : (Z
             else {
                 const float n[3] = { nk.x, nk.y, nk.z };
                 if (ZT) {                    // full Z of aligned grains: the peel-off depends on the field of the event cell (R21)
+                    KRP_CK(g, c0);
                     const float4 cb = __ldg(g.cell + c0);
                     const float bh[3] = { cb.y, cb.z, cb.w };
                     krp_peel_z(g.z, bh, n, Se, rc.n, rc.th, rc.ph, S);
@@ -1495,13 +1504,16 @@ __global__ void __launch_bounds__(256, SCALAR ? KRP_IMAGE_SCALAR_MIN_BLOCKS : (Z
             if (SCALAR) {
                 // two gathers in flight: the cell after next is requested before the next one is tested
                 float tau = 0.f;
+                KRP_CK(g, r.c);
                 float kr_c = __ldg(g.kr + r.c);            // current cell (inside the grid)
                 float ds_c = krp_raya_step(r, rc);
+                KRP_CK(g, r.c);
                 float kr_n = __ldg(g.kr + r.c);            // next cell
                 uint32_t c_n = r.c;
 #pragma unroll 2
                 for (;;) {
                     const float ds_n = krp_raya_step(r, rc);
+                    KRP_CK(g, (int)r.c);
                     const float kr_nn = __ldg(g.kr + (int)r.c); // look-ahead (may lie one cell past the halo, on either side: margin, signed index)
                     tau = fmaf(kr_c, ds_c, tau);
                     if (kr_n < 0.f) break;
@@ -1512,37 +1524,24 @@ __global__ void __launch_bounds__(256, SCALAR ? KRP_IMAGE_SCALAR_MIN_BLOCKS : (Z
             } else if (PRE) {
                 // march over the observer's own coefficient array {kr a1 (sign: thin / thick / halo), kr a2, kr a3, 2 eta}
                 float i = S[0], qs = S[1], us = S[2], vs = S[3];
+                KRP_CK(g, r.c);
                 float4 cl = __ldg(obs_cell + r.c);
-                for (;;) {
-                    // hot loop: cells that are thin whatever the segment (also empty ones: the update is then the identity)
+                // One loop, one sign test per cell: >= 0 thin whatever the segment (also empty cells: the update is then the
+                // identity), < 0 rare -- a cell that may be thick, or the halo.  The rare cases sit behind a forward branch inside the
+                // same loop, so that the lanes of a warp re-join at the next cell (as two nested loops a lane that met a thick cell
+                // waited for all others to finish their rays: 25.9 of 32 threads active, profiles/r2m).
 #pragma unroll 2
-                    while (cl.x >= 0.f) {
+                for (;;) {
+                    if (cl.x < 0.f) {
+                        if (cl.x == -KRP_INF_F) {               // halo: the ray has left the grid -- or crosses a periodic face (R20)
+                            // (a ray that has gone dark stops here as well: beyond A = 104 the carried vector would only grow, R20 allows 4096 periods)
+                            KRP_CK(g, r.c);
+                            if (g.periodic && A <= 104.f && nwrap < KRP_MAX_WRAPS && krp_wrap(g, r.c, woff)) { ++nwrap; cl = __ldg(obs_cell + r.c); continue; }
+                            break;
+                        }
+                        // a cell that may be thick: full in-cell solution
                         const float ds = krp_raya_step(r, rc);
-                        const float4 cn = __ldg(obs_cell + r.c);    // next cell, in flight during the update below
-                        const float xx = cl.y * ds, yy = cl.z * ds;
-                        float s2, c2;
-                        __sincosf(cl.w, &s2, &c2);
-                        const float qg = c2 * qs + s2 * us, ug = c2 * us - s2 * qs;   // eq. 7
-                        // delta form S += R(-eta) dP R(eta) S with the two-term series (|xx|, |yy| < 0.1), written as chains of
-                        // FFMAs: 16 for the update, the increments never materialised
-                        const float x2 = xx * xx, y2 = yy * yy;
-                        const float sh = fmaf(xx * x2, 1.f / 6.f, xx), chm1 = x2 * fmaf(x2, 1.f / 24.f, 0.5f);
-                        const float sy = fmaf(yy * y2, -1.f / 6.f, yy), cym1 = y2 * fmaf(y2, 1.f / 24.f, -0.5f);
-                        const float dqg = fmaf(qg, chm1, -(i * sh)), dug = fmaf(ug, cym1, -(vs * sy));
-                        i = fmaf(-qg, sh, fmaf(i, chm1, i));
-                        vs = fmaf(ug, sy, fmaf(vs, cym1, vs));
-                        qs = fmaf(c2, dqg, fmaf(-s2, dug, qs));
-                        us = fmaf(s2, dqg, fmaf(c2, dug, us));
-                        A = fmaf(cl.x, ds, A);
-                        cl = cn;
-                    }
-                    if (cl.x == -KRP_INF_F) {                   // halo: the ray has left the grid -- or crosses a periodic face (R20)
-                        // (a ray that has gone dark stops here as well: beyond A = 104 the carried vector would only grow, R20 allows 4096 periods)
-                        if (g.periodic && A <= 104.f && nwrap < KRP_MAX_WRAPS && krp_wrap(g, r.c, woff)) { ++nwrap; cl = __ldg(obs_cell + r.c); continue; }
-                        break;
-                    }
-                    {   // a cell that may be thick: full in-cell solution
-                        const float ds = krp_raya_step(r, rc);
+                        KRP_CK(g, r.c);
                         const float4 cn = __ldg(obs_cell + r.c);
                         float s2, c2;
                         __sincosf(cl.w, &s2, &c2);
@@ -1552,15 +1551,37 @@ __global__ void __launch_bounds__(256, SCALAR ? KRP_IMAGE_SCALAR_MIN_BLOCKS : (Z
                         qs = c2 * qg2 - s2 * ug2; us = s2 * qg2 + c2 * ug2;
                         cl = cn;
                         if (A > 104.f) break;                   // e^{-A} is exactly 0 in fp32 from here on
+                        continue;
                     }
+                    const float ds = krp_raya_step(r, rc);
+                    KRP_CK(g, r.c);
+                    const float4 cn = __ldg(obs_cell + r.c);    // next cell, in flight during the update below
+                    const float xx = cl.y * ds, yy = cl.z * ds;
+                    float s2, c2;
+                    __sincosf(cl.w, &s2, &c2);
+                    const float qg = c2 * qs + s2 * us, ug = c2 * us - s2 * qs;   // eq. 7
+                    // delta form S += R(-eta) dP R(eta) S with the two-term series (|xx|, |yy| < 0.1), written as chains of
+                    // FFMAs: 16 for the update, the increments never materialised
+                    const float x2 = xx * xx, y2 = yy * yy;
+                    const float sh = fmaf(xx * x2, 1.f / 6.f, xx), chm1 = x2 * fmaf(x2, 1.f / 24.f, 0.5f);
+                    const float sy = fmaf(yy * y2, -1.f / 6.f, yy), cym1 = y2 * fmaf(y2, 1.f / 24.f, -0.5f);
+                    const float dqg = fmaf(qg, chm1, -(i * sh)), dug = fmaf(ug, cym1, -(vs * sy));
+                    i = fmaf(-qg, sh, fmaf(i, chm1, i));
+                    vs = fmaf(ug, sy, fmaf(vs, cym1, vs));
+                    qs = fmaf(c2, dqg, fmaf(-s2, dug, qs));
+                    us = fmaf(s2, dqg, fmaf(c2, dug, us));
+                    A = fmaf(cl.x, ds, A);
+                    cl = cn;
                 }
                 S[0] = i; S[1] = qs; S[2] = us; S[3] = vs;
             } else {
                 float i = S[0], qs = S[1], us = S[2], vs = S[3];
+                KRP_CK(g, r.c);
                 float4 cl = __ldg(g.cell + r.c);
                 for (;;) {
                 do {
                     const float ds = krp_raya_step(r, rc);
+                    KRP_CK(g, r.c);
                     const float4 cn = __ldg(g.cell + r.c);      // next cell, in flight during the update below
                     if (cl.x > 0.f) {
                         const float mu = fminf(fabsf(rc.n[0] * cl.y + rc.n[1] * cl.z + rc.n[2] * cl.w), 1.f);
@@ -1598,6 +1619,7 @@ __global__ void __launch_bounds__(256, SCALAR ? KRP_IMAGE_SCALAR_MIN_BLOCKS : (Z
                     cl = cn;
                 } while (cl.x >= 0.f);
                 if (A > 104.f || !(g.periodic && nwrap < KRP_MAX_WRAPS && krp_wrap(g, r.c, woff))) break;
+                KRP_CK(g, r.c);
                 ++nwrap; cl = __ldg(g.cell + r.c);           // periodic face (R20): go on from the opposite side
                 }
                 S[0] = i; S[1] = qs; S[2] = us; S[3] = vs;

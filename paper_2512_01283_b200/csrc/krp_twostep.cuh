@@ -8,10 +8,9 @@
 // B200 design against the paper's (one packet per warp, shared-memory reductions before global atomics):
 // S is laid out [cell][camera][4 Stokes] in fp32, so that all cameras of a cell share one or two 128-byte lines, and a
 // deposit is ONE vector reduction per camera (red.global.add.v4.f32, sm_90+) that the L2 slice applies in place -- no
-// shared-memory staging.  A flight is re-marched by a group of G lanes (G = cameras rounded up to a power of two, at most 8):
-// every lane of the group carries the peel-off geometry of its own camera in registers and issues that camera's
-// reduction, so the 4 flights of a warp (8 cameras) write four full lines per step.  The flights themselves are the
-// ordinary ones (same packets, same events): the flight kernels only hand over each flight's path length.
+// shared-memory staging of the sums.  A flight is re-marched by one lane, which holds the peel-off geometry of its flight
+// toward every camera in shared memory.  The flights themselves are the ordinary ones (same packets, same events): the
+// flight kernels only hand over each flight's path length.
 #pragma once
 #include "krp_kernels.cuh"
 
@@ -83,28 +82,32 @@ __device__ __forceinline__ void krp_segment_integral(float q0, float u0, float v
 
 // ------------------------------------------------------------------------------------------
 // step 1: deposit.  Work item = one flight of the wave (queue entry `item`, or the on-the-fly emission of the first
-// order), re-marched in fp32 over its known path length flen[item] (+inf: to the grid edge) by G lanes.
+// order), re-marched in fp32 over its known path length flen[item] (+inf: to the grid edge).  One flight per lane; the
+// peel-off geometry of the flight toward every camera (8 floats each) sits in shared memory, [camera][thread], so that
+// a segment costs the march and the segment integral once and per camera two 16-byte shared loads, ~20 FMAs and one
+// vector reduction.  (The first version marched every flight redundantly in G = 8 lanes, one camera per lane: C5 deposit
+// 1565 ms per 2^22 packets, profiles/r2e.)
 // ------------------------------------------------------------------------------------------
 template <bool SCALAR>
-__global__ void __launch_bounds__(256) krp_k_deposit(KrpModel g, KrpCtl* ctl, KrpRecords q, int in, KrpEmitSrc es,
+__global__ void __launch_bounds__(128) krp_k_deposit(KrpModel g, KrpCtl* ctl, KrpRecords q, int in, KrpEmitSrc es,
                                                      const double* __restrict__ flen, const KrpObserverDev* __restrict__ obs,
-                                                     int n_obs, int G, float* __restrict__ sgrid, unsigned long long* __restrict__ n_seg)
+                                                     int n_obs, float* __restrict__ sgrid, unsigned long long* __restrict__ n_seg)
 {
+    extern __shared__ float4 s_pg[];                 // [n_obs][2][blockDim.x]
     const unsigned int n_items = ctl->q_count[in];
-    const int sub = threadIdx.x & (G - 1);
-    const unsigned int group = (blockIdx.x * blockDim.x + threadIdx.x) / (unsigned)G, n_groups = gridDim.x * blockDim.x / (unsigned)G;
     unsigned long long segs = 0;
-    for (unsigned int item = group; item < n_items; item += n_groups) {
+    for (unsigned int item = blockIdx.x * blockDim.x + threadIdx.x; item < n_items; item += gridDim.x * blockDim.x) {
         float4 pc, nk, S0; double tau; unsigned long long id;
         krp_item_load(g, q, es, item, pc, nk, S0, tau, id);
         const float n[3] = { nk.x, nk.y, nk.z };
         const double Ld = flen[item];
         const float L = Ld > 3.0e38 ? KRP_INF_F : (float)Ld;
-        // this lane's cameras: sub, sub + G (at most two)
-        KrpPeelGeom pg[2];
-        const int o0 = sub, o1 = sub + G;
-        if (o0 < n_obs) krp_peel_setup(g, n, obs[o0], pg[0]);
-        if (o1 < n_obs) krp_peel_setup(g, n, obs[o1], pg[1]);
+        for (int o = 0; o < n_obs; ++o) {
+            KrpPeelGeom pg;
+            krp_peel_setup(g, n, obs[o], pg);
+            s_pg[(2 * o) * blockDim.x + threadIdx.x] = make_float4(pg.c2i, pg.s2i, pg.c2o, pg.s2o);
+            s_pg[(2 * o + 1) * blockDim.x + threadIdx.x] = make_float4(pg.F[0], pg.F[1], pg.F[2], pg.F[3]);
+        }
         // lab basis of n for the grain-frame rotation (general mode)
         float th[3] = { 0.f, 0.f, 0.f }, ph[3] = { 0.f, 0.f, 0.f };
         if (!SCALAR) krp_basis<float>(n, th, ph);
@@ -120,13 +123,14 @@ __global__ void __launch_bounds__(256) krp_k_deposit(KrpModel g, KrpCtl* ctl, Kr
         const float W = S0.x;
         for (;;) {
             float kr, bx = 0.f, by = 0.f, bz = 1.f;
+            KRP_CK(g, c);
             if (SCALAR) kr = __ldg(g.kr + c);
             else { const float4 cl = __ldg(g.cell + c); kr = cl.x; bx = cl.y; by = cl.z; bz = cl.w; }
             if (kr < 0.f) break;                                  // halo
             const float tn = fminf(tx, fminf(ty, tz));
             const bool last = tn >= L;
             const float len = (last ? L : tn) - t;
-            if (kr > 0.f && sub == 0) ++segs;                     // counted like the oracle's: also a segment of zero length
+            if (kr > 0.f) ++segs;                                 // counted like the oracle's: also a segment of zero length
             if (kr > 0.f && len > 0.f) {
                 float a1, a2, a3, om, c2 = 1.f, s2 = 0.f;
                 if (SCALAR) { a1 = g.a1c; a2 = 0.f; a3 = 0.f; om = g.omc; }
@@ -152,14 +156,14 @@ __global__ void __launch_bounds__(256) krp_k_deposit(KrpModel g, KrpCtl* ctl, Kr
                     qs = c2 * qT - s2 * uT; us = s2 * qT + c2 * uT; vs = vT;
                 }
                 const float w = om * W;
-                float out[4];
-                if (o0 < n_obs) {
-                    krp_peel_apply(pg[0], w * J[0], w * J[1], w * J[2], w * J[3], out);
-                    krp_red_v4(sgrid + ((size_t)c * n_obs + o0) * 4, out[0], out[1], out[2], out[3]);
-                }
-                if (o1 < n_obs) {
-                    krp_peel_apply(pg[1], w * J[0], w * J[1], w * J[2], w * J[3], out);
-                    krp_red_v4(sgrid + ((size_t)c * n_obs + o1) * 4, out[0], out[1], out[2], out[3]);
+                J[0] *= w; J[1] *= w; J[2] *= w; J[3] *= w;
+                float* cell_s = sgrid + (size_t)c * n_obs * 4;
+                for (int o = 0; o < n_obs; ++o) {
+                    const float4 r = s_pg[(2 * o) * blockDim.x + threadIdx.x], F = s_pg[(2 * o + 1) * blockDim.x + threadIdx.x];
+                    const float qq = r.x * J[1] + r.y * J[2], uu = -r.y * J[1] + r.x * J[2];          // into the scattering plane
+                    const float I2 = F.x * J[0] + F.y * qq, Q2 = F.y * J[0] + F.x * qq;
+                    const float U2 = F.z * uu + F.w * J[3], V2 = -F.w * uu + F.z * J[3];
+                    krp_red_v4(cell_s + 4 * o, I2, r.z * Q2 + r.w * U2, -r.w * Q2 + r.z * U2, V2);       // to theta^_cam
                 }
             }
             if (last) break;
