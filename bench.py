@@ -34,15 +34,17 @@ METRIC = "photon packets/sec (transport+imaging)"
 UNIT = "packets/s"
 
 # Algorithmic work per unit: bytes that must move and thread-instructions that must issue
-# per cell step of the two hot loops, for the two cell layouts, and per ray / flight outside the loop.
+# per cell step of the two hot loops, for the two cell layouts, and per ray / flight outside the loop.  The loop bodies
+# as ptxas emits them, with the counts marked, are in profiles/r2_sass_hot_loops.md (executed: 18.5 / 52 imaging,
+# 31 / ~230 flight); the algorithmic count is what the written-out algorithm needs:
 #   image_inst   scalar: min3, sub, 3 setp, 3 predicated fadd + 3 iadd, address, gather, fma, sentinel test, branch
-#                general (per-observer coefficient array): the same march + 2 products, sincos of 2 eta, rotation
-#                in, series of sinh/cosh-1/sin/cos-1, delta update rotated back, depth fma
+#                general (per-observer coefficient array): march 13, gather 3, sincos of 2 eta and rotation in 7, series
+#                of sinh/cosh-1/sin/cos-1 and the update as 16 chained FFMAs 22, loop test 3
 #   flight_inst  scalar: re-based march (13) + optical-depth product, fp64 compare and subtract, gather, tests
-#                general: fp64 re-based march, fp64 mu and alpha1, fp32 Stokes update, fp64 depth bookkeeping
+#                general: fp64 re-based march, fp64 mu and table segment, eta, App. A series, rotation, depth bookkeeping
 ALGO = {
     "scalar":  dict(cell_bytes=4,  image_inst=16, flight_inst=23, ray_inst=250, flight_fixed_inst=200),
-    "general": dict(cell_bytes=16, image_inst=56, flight_inst=110, ray_inst=250, flight_fixed_inst=300),
+    "general": dict(cell_bytes=16, image_inst=48, flight_inst=110, ray_inst=250, flight_fixed_inst=300),
 }
 EVENT_BYTES, CONTRIB_BYTES = 48, 32
 N_SM, LANES_PER_SM = 148, 128          # B200: 148 SMs x 4 schedulers x 32 lanes, one warp-instruction per scheduler and clock
@@ -452,11 +454,11 @@ def run_krp(args):
             rec["traffic"] = cap.get("dram_bytes")
             rec["capture"] = {k: cap.get(k) for k in ("files", "issue_pct", "dram_pct", "l2_pct", "l1_pct", "duration_ms",
                                                        "active_threads", "occupancy_pct", "registers")}
-            if cap.get("thread_inst_executed") and cap.get("duration_ms"):
-                # executed (not algorithmic) thread-instructions of the captured launch against the same issue ceiling,
-                # at the capture's own duration: what the SASS really issues, divergence included
-                rec["frac_alu_executed_in_capture"] = cap["thread_inst_executed"] / (cap["duration_ms"] * 1e-3) / alu_peak
-                rec["executed_over_algorithmic"] = None
+            if cap.get("warp_inst_executed") and cap.get("active_threads") and cap.get("duration_ms"):
+                # executed (not algorithmic) thread-instructions of the captured launch against the same issue ceiling, at the
+                # capture's own duration: what the SASS really issues, idle lanes excluded
+                rec["frac_alu_executed_in_capture"] = (cap["warp_inst_executed"] * cap["active_threads"] /
+                                                       (cap["duration_ms"] * 1e-3) / alu_peak)
         rec["bound"] = bound
         per_class[cls] = rec
     D = per_class[dom]
