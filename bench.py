@@ -558,7 +558,7 @@ def main():
                    "job_packets": cfg["n_packets"], "events_per_packet": r["epp"],
                    "l2": "flushed every step by a 256 MiB memset inside the timed region",
                    "launch": "flights: %s; imaging: one launch per observer over events ordered by cell bin" %
-                             ("static assignment" if r["mode"] == "scalar" else "persistent lanes, refill every 32 cell steps"),
+                             ("static assignment" if r["mode"] == "scalar" else "persistent lanes, refill distance chosen from the measured flight length"),
                    "parallelism": "packet ids sharded over %d GPU(s), grid replicated, one fp64 image all-reduce at job end" % r["world"],
                    "reduced": bool(args.n)},
         "scatterings_per_s": tot["events"] / sec,

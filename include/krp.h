@@ -238,7 +238,10 @@ int krp_events_clear(krp_grid* g, void* stream);
 /* Launch-shape knobs, for measurement only (0 keeps the current value): threads per block of the
  * flight and imaging kernels (multiples of 32 up to 256; defaults 256, general-mode flights 128),
  * persistent blocks per SM (default: 8; the general-mode flight fills an SM once, 640 threads), and
- * the number of cell steps a flight kernel takes between two points where idle lanes take new packets. */
+ * the number of cell steps a flight kernel takes between two points where idle lanes take new packets
+ * (default: scalar mode 1 = static assignment; general mode 32 until the library has seen the mean flight
+ * length of a batch, then 1, 8 or 16 for flights shorter than 3, shorter than 24, or longer; setting it
+ * here switches that choice off).  Results do not depend on any of these. */
 int krp_tune(krp_grid* g, int transport_block, int image_block, int blocks_per_sm, int flight_burst);
 /* Scheduling features, for A/B measurement and for the tests that show results do not depend on them (-1 keeps the
  * current value): dir_sort 1/0 = first flights of an isotropic point source taken in direction order / in id order;

@@ -106,6 +106,10 @@ struct krp_grid {
     unsigned long long ray_stats_prev[3] = { 0, 0, 0 };
     cudaEvent_t ray_stats_ev = nullptr;
     bool ray_stats_pending = false;
+    // refill distance of the general flight chosen from the measured flight length (read back without waiting, then frozen)
+    unsigned long long* h_flight_stats = nullptr;       // pinned: packets, events, records, steps_transport
+    cudaEvent_t flight_stats_ev = nullptr;
+    bool flight_stats_pending = false, burst_auto = true, burst_decided = false;
     float4* d_obs_cells = nullptr;  // [n_obs][npad] per-observer cell coefficients (general mode), or NULL
     int obs_pre = 1;
     double* d_img = nullptr;
@@ -204,6 +208,8 @@ extern "C" int krp_grid_destroy(krp_grid* g)
     free_records(g->q[0]); free_records(g->q[1]); free_records(g->ev); free_hits(g->hits);
     for (cudaEvent_t e : g->t_ev) cudaEventDestroy(e);
     if (g->h_ray_stats) cudaFreeHost(g->h_ray_stats);
+    if (g->h_flight_stats) cudaFreeHost(g->h_flight_stats);
+    if (g->flight_stats_ev) cudaEventDestroy(g->flight_stats_ev);
     if (g->ray_stats_ev) cudaEventDestroy(g->ray_stats_ev);
     delete g;
     return KRP_OK;
@@ -621,6 +627,19 @@ extern "C" int krp_transport(krp_grid* g, uint64_t n_packets, uint64_t seed, voi
         g->flen_cap = n_packets;
     }
     double* flen = g->d_sgrid ? g->d_flen : nullptr;
+    // General flight: cell steps between two refill points, from the mean flight length of the batches so far (counters read back
+    // without waiting; decided once, results do not depend on it).  Flights of one or two cells (C3: thick cells, 1.2 steps per
+    // flight) take a new queue entry after every step: 10.8 -> 8.8 ms per 2^22 packets; long flights (C4, C5: ~67 steps) refill
+    // every 16 steps (profiles/r2q_README.md).
+    if (!g->m.scalar && g->burst_auto && !g->burst_decided && g->flight_stats_pending && cudaEventQuery(g->flight_stats_ev) == cudaSuccess) {
+        g->flight_stats_pending = false;
+        const unsigned long long flights = g->h_flight_stats[0] + g->h_flight_stats[1], steps = g->h_flight_stats[3];
+        if (flights >= 10000ull) {
+            const double len = (double)steps / (double)flights;
+            g->burst = len < 3.0 ? 1 : (len < 24.0 ? 8 : 16);
+            g->burst_decided = true;
+        }
+    }
     const unsigned n = (unsigned)n_packets;
     if (g->m.emit_records) g->ev_has_emission = 1;
     const int tb = g->transport_block;
@@ -705,6 +724,15 @@ extern "C" int krp_transport(krp_grid* g, uint64_t n_packets, uint64_t seed, voi
     }
     CK(cudaGetLastError());
     g->next_id += n_packets;
+    if (!g->m.scalar && g->burst_auto && !g->burst_decided && !g->flight_stats_pending) {
+        if (!g->h_flight_stats) {
+            CK(cudaMallocHost(&g->h_flight_stats, 4 * sizeof(unsigned long long)));
+            CK(cudaEventCreateWithFlags(&g->flight_stats_ev, cudaEventDisableTiming));
+        }
+        CK(cudaMemcpyAsync(g->h_flight_stats, &g->d_ctl->stats.packets, 4 * sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
+        CK(cudaEventRecord(g->flight_stats_ev, st));
+        g->flight_stats_pending = true;
+    }
     return KRP_OK;
 }
 
@@ -1022,7 +1050,7 @@ extern "C" int krp_tune(krp_grid* g, int transport_block, int image_block, int b
     if (image_block) g->image_block = image_block;
     if (blocks_per_sm) { g->blocks_per_sm = blocks_per_sm; g->bps_tuned = 1; }
     if (flight_burst < 0 || flight_burst > 4096) return fail(KRP_ERR_ARG, "flight_burst must be in 0..4096");
-    if (flight_burst) g->burst = flight_burst;
+    if (flight_burst) { g->burst = flight_burst; g->burst_auto = false; }
     return KRP_OK;
 }
 
