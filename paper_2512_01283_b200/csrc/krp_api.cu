@@ -6,6 +6,7 @@
 #include "krp_twostep.cuh"
 
 #include <cub/device/device_scan.cuh>
+#include <cub/device/device_radix_sort.cuh>
 
 #include <cmath>
 #include <cstdarg>
@@ -101,7 +102,7 @@ struct krp_grid {
     KrpObserverDev* d_obs = nullptr;
     // ordering of the events before imaging: policy 0 never, 1 by the measured ray length, 2 always
     int order_policy = 1;
-    bool order_events = true;
+    bool order_events = true, order_decided = false;
     unsigned long long* h_ray_stats = nullptr;          // pinned: steps_image, contributions, dropped
     unsigned long long ray_stats_prev[3] = { 0, 0, 0 };
     cudaEvent_t ray_stats_ev = nullptr;
@@ -123,6 +124,10 @@ struct krp_grid {
     KrpObserverDev* d_sg_obs = nullptr;
     double* d_flen = nullptr;
     uint64_t flen_cap = 0;
+    unsigned short* d_dkeys[2] = { nullptr, nullptr };      // deposit: flights sorted by length (keys, item indices, cub scratch)
+    unsigned int* d_dvals[2] = { nullptr, nullptr };
+    void* d_dsort = nullptr;
+    size_t dsort_bytes = 0;
     float* d_emis = nullptr;        // padded thermal source of krp_image_rays
     float* d_zt = nullptr; double* d_zt_norm = nullptr; double* d_zt_bound = nullptr;   // full Z of aligned grains (krp_zmatrix_set)
     uint64_t next_id = 0;
@@ -204,6 +209,7 @@ extern "C" int krp_grid_destroy(krp_grid* g)
     cudaFree(g->d_bins); cudaFree(g->d_perm); cudaFree(g->d_scan);
     cudaFree(g->d_dir_bins); cudaFree(g->d_dir_scan); cudaFree(g->d_order);
     cudaFree(g->d_sgrid); cudaFree(g->d_sg_obs); cudaFree(g->d_flen); cudaFree(g->d_emis);
+    cudaFree(g->d_dkeys[0]); cudaFree(g->d_dkeys[1]); cudaFree(g->d_dvals[0]); cudaFree(g->d_dvals[1]); cudaFree(g->d_dsort);
     cudaFree(g->d_zt); cudaFree(g->d_zt_norm); cudaFree(g->d_zt_bound);
     free_records(g->q[0]); free_records(g->q[1]); free_records(g->ev); free_hits(g->hits);
     for (cudaEvent_t e : g->t_ev) cudaEventDestroy(e);
@@ -623,7 +629,15 @@ extern "C" int krp_transport(krp_grid* g, uint64_t n_packets, uint64_t seed, voi
     if (g->d_sgrid && g->flen_cap < n_packets) {
         CK(cudaStreamSynchronize(st));
         cudaFree(g->d_flen); g->d_flen = nullptr; g->flen_cap = 0;
+        cudaFree(g->d_dkeys[0]); cudaFree(g->d_dkeys[1]); cudaFree(g->d_dvals[0]); cudaFree(g->d_dvals[1]); cudaFree(g->d_dsort);
+        g->d_dkeys[0] = g->d_dkeys[1] = nullptr; g->d_dvals[0] = g->d_dvals[1] = nullptr; g->d_dsort = nullptr;
         CK(cudaMalloc(&g->d_flen, sizeof(double) * n_packets));
+        for (int k = 0; k < 2; ++k) {
+            CK(cudaMalloc(&g->d_dkeys[k], sizeof(unsigned short) * n_packets));
+            CK(cudaMalloc(&g->d_dvals[k], sizeof(unsigned int) * n_packets));
+        }
+        CK(cub::DeviceRadixSort::SortPairsDescending(nullptr, g->dsort_bytes, g->d_dkeys[0], g->d_dkeys[1], g->d_dvals[0], g->d_dvals[1], (int)n_packets, 0, 16, st));
+        CK(cudaMalloc(&g->d_dsort, g->dsort_bytes ? g->dsort_bytes : 16));
         g->flen_cap = n_packets;
     }
     double* flen = g->d_sgrid ? g->d_flen : nullptr;
@@ -707,12 +721,17 @@ extern "C" int krp_transport(krp_grid* g, uint64_t n_packets, uint64_t seed, voi
             // step 1 of the two-step form: the flights of this wave, re-marched over their path lengths, deposit into S
             TimedLaunch tl(g, st, KRP_T_DEPOSIT);
             const KrpEmitSrc es = w == 0 ? es0 : KrpEmitSrc{ nullptr, 0, 0 };
+            // flights of the wave sorted by the number of cells they cross (the queue's capacity is sorted: its fill is known on the device only)
+            const unsigned n_cap = (unsigned)g->flen_cap < n ? (unsigned)g->flen_cap : n;
+            krp_k_deposit_keys<<<(n_cap + 255u) / 256u, 256, 0, st>>>(g->m, g->d_ctl, g->q[in], in, es, flen, n_cap, g->d_dkeys[0], g->d_dvals[0]);
+            CK(cub::DeviceRadixSort::SortPairsDescending(g->d_dsort, g->dsort_bytes, g->d_dkeys[0], g->d_dkeys[1], g->d_dvals[0], g->d_dvals[1], (int)n_cap, 0, 16, st));
+            g->launches += 2;
             const unsigned need_d = (n + 127u) / 128u;
             const unsigned pers_d = (unsigned)g->n_sm * 8u;
             const unsigned grid_d = need_d < pers_d ? need_d : pers_d;
             const size_t smem_d = (size_t)g->sg_n_obs * 2 * 128 * sizeof(float4);
-            if (g->m.scalar) krp_k_deposit<true><<<grid_d, 128, smem_d, st>>>(g->m, g->d_ctl, g->q[in], in, es, flen, g->d_sg_obs, g->sg_n_obs, g->d_sgrid, &g->d_ctl->sg_segments);
-            else             krp_k_deposit<false><<<grid_d, 128, smem_d, st>>>(g->m, g->d_ctl, g->q[in], in, es, flen, g->d_sg_obs, g->sg_n_obs, g->d_sgrid, &g->d_ctl->sg_segments);
+            if (g->m.scalar) krp_k_deposit<true><<<grid_d, 128, smem_d, st>>>(g->m, g->d_ctl, g->q[in], in, es, flen, g->d_dvals[1], g->d_sg_obs, g->sg_n_obs, g->d_sgrid, &g->d_ctl->sg_segments);
+            else             krp_k_deposit<false><<<grid_d, 128, smem_d, st>>>(g->m, g->d_ctl, g->q[in], in, es, flen, g->d_dvals[1], g->d_sg_obs, g->sg_n_obs, g->d_sgrid, &g->d_ctl->sg_segments);
             g->launches++;
         }
         if (w + 1 < g->bins[g->cur_bin].max_waves) {
@@ -846,7 +865,12 @@ extern "C" int krp_image(krp_grid* g, const krp_observer* obs, int n_obs, int np
         // (the counters may have been reset by krp_stats_reset in between: then they count from zero)
         auto delta = [&](int j) { return g->h_ray_stats[j] >= g->ray_stats_prev[j] ? g->h_ray_stats[j] - g->ray_stats_prev[j] : g->h_ray_stats[j]; };
         const unsigned long long steps = delta(0), rays = delta(1) + delta(2);
-        if (rays > 0) g->order_events = g->order_policy == 2 || (g->order_policy == 1 && (double)steps / (double)rays >= 12.0);
+        // decided once, on the first pass that has marched a fair number of rays, then kept: step times stay reproducible from
+        // run to run also for models near the threshold
+        if (rays >= 100000ull && !g->order_decided) {
+            g->order_events = g->order_policy == 2 || (g->order_policy == 1 && (double)steps / (double)rays >= 12.0);
+            g->order_decided = true;
+        }
         g->ray_stats_prev[0] = g->h_ray_stats[0]; g->ray_stats_prev[1] = g->h_ray_stats[1]; g->ray_stats_prev[2] = g->h_ray_stats[2];
         g->ray_stats_pending = false;
     }
@@ -888,7 +912,7 @@ extern "C" int krp_image(krp_grid* g, const krp_observer* obs, int n_obs, int np
     g->launches++;
     CK(cudaGetLastError());
     // counters of this pass for the ordering decision of a later one (never waited for)
-    if (g->order_policy == 1 && !g->ray_stats_pending) {
+    if (g->order_policy == 1 && !g->order_decided && !g->ray_stats_pending) {
         if (!g->h_ray_stats) {
             CK(cudaMallocHost(&g->h_ray_stats, 3 * sizeof(unsigned long long)));
             g->h_ray_stats[0] = g->h_ray_stats[1] = g->h_ray_stats[2] = 0;
@@ -1061,7 +1085,7 @@ extern "C" int krp_tune_schedule(krp_grid* g, int dir_sort, int obs_cells, int o
         return fail(KRP_ERR_ARG, "dir_sort, obs_cells must be -1, 0 or 1 and order_policy -1..2");
     if (dir_sort >= 0) g->dir_sort = dir_sort;
     if (obs_cells >= 0 && obs_cells != g->obs_pre) { g->obs_pre = obs_cells; g->obs_host.clear(); }   // rebuilt at the next krp_image
-    if (order_policy >= 0) { g->order_policy = order_policy; g->order_events = order_policy != 0; g->ray_stats_pending = false; }
+    if (order_policy >= 0) { g->order_policy = order_policy; g->order_events = order_policy != 0; g->ray_stats_pending = false; g->order_decided = false; }
     return KRP_OK;
 }
 
