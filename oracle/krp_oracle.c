@@ -643,21 +643,20 @@ static int flight(const ora_model* m, int idx[3], double p[3], const double n[3]
     }
 }
 
-/* S1 emission of packet id (draw schedule R11).  Exported as ora_emit for the pins. */
-static void emit(const ora_model* m, uint64_t seed, uint64_t id, int idx[3], double p[3], double n[3], double* tau_star)
+/* S1 emission of packet id (draw schedule R11).  Exported as ora_emit / ora_emit_full for the pins.
+ * Thermal emission by aligned grains (kind bit2, with bit0; PAPER.md:95-97 eq. 8, :145; reading R22): the source term of
+ * eq. 8 is alpha_abs B with alpha_abs = (1 - omega) alpha (R19), i.e. per unit extinction depth the grain-frame vector
+ * (1 - omega(mu)) (alpha1(mu), alpha2(mu), 0, 0) B.  A packet of the Monte-Carlo step therefore leaves its cell in a
+ * direction drawn with density proportional to (1 - omega(mu)) alpha1(mu), mu = |n . B^| (rejection from isotropic
+ * candidates against the table's maximum; candidate k uses block 0 (k = 0) or block 2 + k of event 0: words
+ * (cos theta, phi, accept, tau* [block 0 only]); at most 64 candidates, the last one is taken), and carries
+ * (1, alpha2/alpha1, 0, 0) in the grain-frame reference, turned into the lab reference of n (eq. 6-7). */
+static void emit_full(const ora_model* m, uint64_t seed, uint64_t id, int idx[3], double p[3], double n[3], double* tau_star, double S[4])
 {
     uint32_t w[4];
     draw(seed, id, 0, 0, w);
     *tau_star = -log(ora_u01(w[2]));
-    if (m->src_kind & 2) {
-        for (int a = 0; a < 3; ++a) n[a] = m->src_dir[a];
-    } else {
-        double ct = 1.0 - 2.0 * ora_u01(w[0]);
-        double st = sqrt(1.0 - ct * ct);
-        double ph = 2 * ORA_PI * ora_u01(w[1]);
-        n[0] = st * cos(ph); n[1] = st * sin(ph); n[2] = ct;
-    }
-    for (int a = 0; a < 3; ++a) n[a] = (double)(float)n[a];          /* R12 */
+    S[0] = 1; S[1] = S[2] = S[3] = 0;
     if (m->src_kind & 1) {
         uint32_t w1[4], w2[4];
         draw(seed, id, 0, 1, w1);
@@ -678,6 +677,53 @@ static void emit(const ora_model* m, uint64_t seed, uint64_t id, int idx[3], dou
     } else {
         for (int a = 0; a < 3; ++a) { idx[a] = m->src_idx[a]; p[a] = ORA_STATE(m->src_p[a]); }   /* R12 */
     }
+    if (m->src_kind & 2) {
+        for (int a = 0; a < 3; ++a) n[a] = m->src_dir[a];
+        for (int a = 0; a < 3; ++a) n[a] = (double)(float)n[a];          /* R12 */
+        return;
+    }
+    int thermal = (m->src_kind & 4) && (m->src_kind & 1);
+    double b[3] = { 0, 0, 1 }, emax = 0.0;
+    if (thermal) {
+        cell_bhat(m, cell_of(m, idx), b);
+        for (int j = 0; j < m->n_inc; ++j) {
+            double e = (1.0 - (double)m->opac[4*j+3]) * (double)m->opac[4*j];
+            if (e > emax) emax = e;
+        }
+    }
+    for (int k = 0; ; ++k) {
+        if (k > 0) draw(seed, id, 0, 2 + k, w);
+        double ct = 1.0 - 2.0 * ora_u01(w[0]);
+        double st = sqrt(1.0 - ct * ct);
+        double ph = 2 * ORA_PI * ora_u01(w[1]);
+        n[0] = st * cos(ph); n[1] = st * sin(ph); n[2] = ct;
+        for (int a = 0; a < 3; ++a) n[a] = (double)(float)n[a];          /* R12 */
+        if (!thermal) return;
+        double a[4];
+        ora_opac_at(m, mu_of(n, b), a);
+        if (ora_u01(w[k == 0 ? 3 : 2]) * emax < (1.0 - a[3]) * a[0] || k >= 63) {
+            S[1] = a[1] / a[0];
+            if (a[1] != 0.0) {
+                double q[4], ce, se;
+                ora_quat_from_B(b, q);
+                ora_eta_gf(q, n, &ce, &se);
+                ora_rotate_qu(S, ce, -se);
+            }
+            for (int s2 = 1; s2 < 4; ++s2) S[s2] = ORA_STATE(S[s2]);      /* R12: queue state */
+            return;
+        }
+    }
+}
+
+static void emit(const ora_model* m, uint64_t seed, uint64_t id, int idx[3], double p[3], double n[3], double* tau_star)
+{
+    double S[4];
+    emit_full(m, seed, id, idx, p, n, tau_star, S);
+}
+
+void ora_emit_full(const ora_model* m, uint64_t seed, uint64_t id, int idx[3], double p[3], double n[3], double* tau_star, double S[4])
+{
+    emit_full(m, seed, id, idx, p, n, tau_star, S);
 }
 
 void ora_emit(const ora_model* m, uint64_t seed, uint64_t id, int idx[3], double p[3], double n[3], double* tau_star)
@@ -697,8 +743,8 @@ int64_t ora_transport2(const ora_model* m, uint64_t id0, uint64_t n_packets, uin
     int64_t nesc = 0;
     for (uint64_t id = id0; id < id0 + n_packets; ++id) {
         int idx[3]; double p[3], n[3], tau_star;
-        emit(m, seed, id, idx, p, n, &tau_star);
-        double W = 1.0, S[4] = { 1, 0, 0, 0 };
+        double W = 1.0, S[4];
+        emit_full(m, seed, id, idx, p, n, &tau_star, S);
         st->packets++; st->w_emitted += W;
         if (m->emit_records) { push_event(ev, st, cell_of(m, idx), p, n, S, W, id, 0); st->records++; }
         int k = 0;

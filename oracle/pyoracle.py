@@ -106,6 +106,7 @@ def lib(variant=None):
     sig = {
         "ora_state_is_fp32": (C.c_int, []),
         "ora_emit": (None, [C.c_void_p, C.c_uint64, C.c_uint64, _ip, _dp, _dp, _D]),
+        "ora_emit_full": (None, [C.c_void_p, C.c_uint64, C.c_uint64, _ip, _dp, _dp, _D, _dp]),
         "ora_philox": (None, [_up, _up, _up]),
         "ora_u01": (C.c_double, [C.c_uint32]),
         "ora_u53": (C.c_double, [C.c_uint32, C.c_uint32]),
@@ -238,6 +239,12 @@ class OracleModel:
         idx = np.zeros(3, np.int32); p = np.zeros(3); n = np.zeros(3); t = C.c_double(0)
         self.L.ora_emit(self.h, int(seed), int(pid), idx, p, n, C.byref(t))
         return idx, p, n, t.value
+
+    def emit_full(self, seed, pid):
+        """emit() plus the Stokes vector (1, q, u, v) the packet starts with (thermal emission of aligned grains: R22)."""
+        idx = np.zeros(3, np.int32); p = np.zeros(3); n = np.zeros(3); t = C.c_double(0); S = np.zeros(4)
+        self.L.ora_emit_full(self.h, int(seed), int(pid), idx, p, n, C.byref(t), S)
+        return idx, p, n, t.value, S
 
     def sample_theta(self, u):
         return self.L.ora_sample_theta(self.h, float(u))

@@ -338,3 +338,87 @@ def test_pixel_rays_in_a_periodic_slab():
     m.set_periodic(0)
     img0, _ = m.image_rays(None, [o], 8, 8, emis=emis)
     assert (img0[0, 0] == 0).sum() > 20 and img0[0, 0].max() < img[0, 0].max() * (1 + 1e-12)
+
+
+# ----------------------------------------------------------------------------
+# NEXT-3: thermal emission of aligned grains as the packet source of the Monte-Carlo step (reading R22)
+# ----------------------------------------------------------------------------
+def _aligned_table(n_inc=9, R=1.6, c3=0.1, om=0.3):
+    mu = np.linspace(0, 1, n_inc); s2 = 1 - mu * mu
+    return np.stack([1 + 0.5 * (R - 1) * s2, 0.5 * (R - 1) * s2, c3 * s2, om + 0.2 * mu], 1).astype(np.float32)
+
+
+def test_thermal_packets_follow_the_emissivity():
+    """kind = 5 (volume source, thermal): directions are distributed as (1 - omega(mu)) alpha1(mu), mu = |n . B^|, and the
+    packet carries (1, alpha2/alpha1, 0, 0) in the grain-frame reference: rotated back there (eq. 6-7) Q/I = alpha2/alpha1 at
+    the packet's own mu, U = V = 0.  Draws replayed from the Philox words for the first candidates."""
+    from test_oracle_pins import _philox
+    tab = _aligned_table()
+    b = np.array([0.48, -0.6, 0.64], np.float32).astype(float)
+    m = box_model((3, 3, 3), 1.0, bvec=b, opac=tab)
+    m.source_set(5, [0, 0, 0], [0, 0, 1], None, 0)
+    mu_n = np.linspace(0, 1, 9)
+    emis = (1 - tab[:, 3].astype(float)) * tab[:, 0].astype(float)
+    emax = emis.max()
+    N = 60000
+    mus = np.zeros(N); first = 0
+    q4 = np.zeros(4); L.ora_quat_from_B(b, q4)
+    import ctypes as C
+    for pid in range(N):
+        idx, p, n, tau, S = m.emit_full(11, pid)
+        mu = abs(float(np.dot(n, b))) / np.linalg.norm(n) / np.linalg.norm(b)
+        mus[pid] = mu
+        if pid < 2000:
+            a = m.opac_at(mu)
+            ce, se = C.c_double(), C.c_double(); L.ora_eta_gf(q4, n, C.byref(ce), C.byref(se))
+            Sg = S.copy(); L.ora_rotate_qu(Sg, ce.value, se.value)
+            assert abs(Sg[1] - a[1] / a[0]) < 2e-7 and abs(Sg[2]) < 2e-7 and Sg[3] == 0 and S[0] == 1      # fp32 (q,u,v) state (R12)
+            # the first candidate (block 0: cos theta, phi, -, accept = word 3) is taken exactly when its test passes
+            w = _philox(11, (pid, 0, 0, 0)); u = [((int(x) >> 9) + 0.5) / 8388608.0 for x in w]
+            ct = 1 - 2 * u[0]; st = math.sqrt(1 - ct * ct); ph = 2 * math.pi * u[1]
+            n0 = np.array([st * math.cos(ph), st * math.sin(ph), ct]).astype(np.float32).astype(float)
+            a0 = m.opac_at(abs(float(np.dot(n0, b))) / np.linalg.norm(n0) / np.linalg.norm(b))
+            took_first = np.array_equal(n, n0)
+            assert took_first == (u[3] * emax < (1 - a0[3]) * a0[0])
+            first += took_first
+            assert abs(tau + math.log(u[2])) < 1e-15
+    assert 0.5 * 2000 < first < 2000                                       # rejections happen
+    h, edges = np.histogram(mus, bins=8, range=(0, 1))
+    # isotropic candidates are uniform in mu; accepted density ~ emissivity(mu), piecewise linear on the nodes
+    fine = np.linspace(0, 1, 8001); dens = np.interp(fine, mu_n, emis)
+    want = np.array([dens[(fine >= a_) & (fine < b_)].sum() for a_, b_ in zip(edges[:-1], edges[1:])]); want /= want.sum()
+    assert np.all(np.abs(h / N - want) < 5 * np.sqrt(want / N)), (h / N, want)
+
+
+def test_thermal_packets_and_thermal_rays_agree():
+    """The two halves of NEXT-3 describe the same radiation: in an optically thin, non-scattering aligned cube the packets that
+    leave toward a direction (naive cone estimator) carry, per steradian, L_tot/N times their count, with
+    L_tot = 4 pi <(1 - omega) alpha1>_mu sum(kappa rho B V); the ray step's image toward that direction integrates to the same
+    radiant intensity, with the same Q/I = alpha2/alpha1 in the reference theta^_obs."""
+    tab = _aligned_table(om=0.0); tab[:, 3] = 0.0                                   # pure absorber / emitter
+    b = np.array([0.0, 0.0, 1.0])
+    kr, Bv, n = 0.02, 1.7, 4
+    m = box_model((n, n, n), kr, bvec=b, opac=tab, bounds=(-.5, .5, -.5, .5, -.5, .5))
+    m.source_set(5, [0, 0, 0], [0, 0, 1], None, 0)
+    N = 400000
+    ev = OracleEvents(4 * N)
+    st, esc = m.transport(0, N, 3, ev, esc_cap=N)
+    mu_n = np.linspace(0, 1, 9)
+    mean_emis = np.trapezoid(tab[:, 0].astype(float), mu_n)
+    L_tot = 4 * math.pi * mean_emis * float(np.float32(kr)) * Bv * 1.0
+    for th_deg in (90.0, 50.0):
+        th = math.radians(th_deg); no = np.array([math.sin(th), 0.0, math.cos(th)])
+        half = math.radians(15.0); dom = 2 * math.pi * (1 - math.cos(half))
+        sel = esc["n"] @ no > math.cos(half)
+        naive = esc["S"][sel].sum(0) / dom * L_tot / N                               # radiant intensity, lab reference of each packet
+        o = Observer.make(th, 0.0, [0, 0, 0], 0.9)
+        img, _ = m.image_rays(None, [o], 96, 96, emis=np.full(n ** 3, Bv, np.float32))
+        tot = img[0].sum(axis=(1, 2))
+        cnt = sel.sum()
+        assert cnt > 5000
+        assert abs(naive[0] / tot[0] - 1) < 4 / math.sqrt(cnt) + 0.02               # cone average of a smooth pattern, thin-limit e^{-tau}
+        # polarisation: B along z, observer in the x-z plane: the grain frame's +Q (E in the n-B plane) is +Q of theta^_obs
+        a = m.opac_at(abs(no[2]))
+        assert abs(tot[1] / tot[0] - a[1] / a[0]) < 5e-3 and abs(tot[2]) < 1e-12 * tot[0]      # thin limit: O(tau = 0.02) self-absorption
+        # packets inside the cone: their Q in their own lab reference is the same grain-frame Q (B = z: theta^' = theta^)
+        assert abs(naive[1] / naive[0] - a[1] / a[0]) < 0.03
