@@ -97,6 +97,12 @@ int krp_grid_update(krp_grid* g, const float* density, const float* bfield, int 
  *   kind bit0: 0 = all packets start at pos, 1 = start uniformly inside a cell drawn with
  *              probability proportional to cell_weight (DEVICE, [ncell]; NULL = uniform);
  *   kind bit1: 0 = isotropic directions, 1 = all along dir (need not be normalised).
+ *   kind bit2 (only as kind = 5): thermal emission of the grains themselves (eq. 8, alpha_abs B; reading R22):
+ *              positions as for bit0 (cell_weight = kappa*rho*B*V of the cell makes the cells emit in proportion), directions
+ *              drawn with density (1 - albedo(mu)) alpha1(mu), mu = |n^ . B^| of the emitting cell, Stokes vector
+ *              (1, alpha2/alpha1, 0, 0) in the grain-frame reference.  One packet then stands for L_tot / N with
+ *              L_tot = 4 pi <(1 - albedo) alpha1>_mu sum(kappa*rho*B*V); the direct thermal light is krp_image_rays' `emis`.
+ *              No emission records.  Set it again after krp_freq_select (it depends on the bin's table).
  *   emit_records != 0 also appends an "emission record" (event index k = 0) per packet so
  *   that krp_image(flags bit0) can add the direct, unscattered light.
  * Every packet starts unpolarised, Stokes (1,0,0,0), weight 1. */

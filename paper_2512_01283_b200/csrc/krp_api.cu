@@ -516,7 +516,8 @@ extern "C" int krp_grid_update(krp_grid* g, const float* density, const float* b
 extern "C" int krp_source_set(krp_grid* g, const krp_source* src, void* stream)
 {
     if (!g || !src) return fail(KRP_ERR_ARG, "grid or source is NULL");
-    if (src->kind < 0 || src->kind > 3) return fail(KRP_ERR_ARG, "source kind must be in 0..3");
+    if (src->kind < 0 || src->kind > 7 || ((src->kind & 4) && (src->kind & 3) != 1))
+        return fail(KRP_ERR_ARG, "source kind must be in 0..3, or 5 (thermal emission: volume source, isotropic candidates)");
     cudaStream_t st = (cudaStream_t)stream;
     KrpModel& m = g->m;
     if (src->kind & 2) {
@@ -524,6 +525,16 @@ extern "C" int krp_source_set(krp_grid* g, const krp_source* src, void* stream)
         if (!(nn > 0.0) || !std::isfinite(nn)) return fail(KRP_ERR_ARG, "collimated source needs a non-zero finite dir");
     }
     m.src_kind = src->kind; m.emit_records = src->emit_records ? 1 : 0;
+    if (src->kind & 4) {
+        if (m.emit_records) return fail(KRP_ERR_ARG, "a thermal source has no emission records: its direct light is krp_image_rays' thermal term");
+        // max over the table nodes of (1 - omega) alpha1, from the fp32 table in fp64 (R22)
+        const TableSet& t = g->bins[g->cur_bin];
+        std::vector<float> op(4 * (size_t)t.n_inc);
+        CK(cudaMemcpy(op.data(), t.d_opac, sizeof(float4) * t.n_inc, cudaMemcpyDeviceToHost));
+        double emax = 0.0;
+        for (int j = 0; j < t.n_inc; ++j) emax = std::fmax(emax, (1.0 - (double)op[4 * j + 3]) * (double)op[4 * j]);
+        m.src_emax = emax;
+    }
     const int dims[3] = { m.nx, m.ny, m.nz };
     int idx[3];
     for (int a = 0; a < 3; ++a) {

@@ -68,6 +68,7 @@ struct KrpModel {
     uint32_t src_cell;     // padded id
     float src_p[3];
     const double* src_cdf; // [ncell] running sum of cell weights (unpadded order) or NULL
+    double src_emax;       // thermal source (kind bit 2, R22): max over the table nodes of (1 - omega) alpha1
 };
 
 // Bounds check of every cell gather, compiled in with -DKRP_CHECK only (profiles/r2_bounds_check.md; compute-sanitizer is

@@ -131,10 +131,43 @@ __global__ void __launch_bounds__(256) krp_k_emit(KrpModel g, KrpCtl* ctl, KrpRe
         cell = g.src_cell; p[0] = g.src_p[0]; p[1] = g.src_p[1]; p[2] = g.src_p[2];
     }
     float4 pc = make_float4(p[0], p[1], p[2], __uint_as_float(cell));
+    float qe = 0.f, ue = 0.f;
+    if ((g.src_kind & 5) == 5 && !(g.src_kind & 2) && !g.scalar) {
+        // Thermal emission of aligned grains (R22; eq. 8): direction with density (1 - omega(mu)) alpha1(mu),
+        // mu = |n . B^| of the emitting cell, by rejection from isotropic candidates (candidate 0: block 0, accept = word 3;
+        // candidate k: block 2 + k, accept = word 2; at most 64), Stokes (1, alpha2/alpha1, 0, 0) in the grain-frame reference
+        const float4 cl = g.cell[cell];
+        const double b[3] = { cl.y, cl.z, cl.w };
+        const double inv_b = 1.0 / sqrt(b[0] * b[0] + b[1] * b[1] + b[2] * b[2]);
+        uint4 wk = w;
+        for (int k = 0; ; ++k) {
+            if (k > 0) {
+                wk = krp_philox(seed, id, 0u, (uint32_t)(2 + k));
+                const double ct = 1.0 - 2.0 * krp_u01(wk.x), st = sqrt(1.0 - ct * ct);
+                double sp, cp;
+                sincospi(2.0 * krp_u01(wk.y), &sp, &cp);
+                nn[0] = (float)(st * cp); nn[1] = (float)(st * sp); nn[2] = (float)ct;   // R12
+            }
+            const double nd[3] = { nn[0], nn[1], nn[2] };
+            const double mu = fmin(fabs(nd[0] * b[0] + nd[1] * b[1] + nd[2] * b[2]) * inv_b / sqrt(nd[0] * nd[0] + nd[1] * nd[1] + nd[2] * nd[2]), 1.0);
+            const double x = mu * g.xs;
+            const int j = min((int)x, g.n_inc - 2);
+            const double4 ta = g.opA_d[j], tb = g.opB_d[j];
+            const double a1 = fma(tb.x, x, ta.x), a2 = fma(tb.y, x, ta.y), om = fma(tb.w, x, ta.w);
+            if (krp_u01(k == 0 ? wk.w : wk.z) * g.src_emax < (1.0 - om) * a1 || k >= 63) {
+                double th[3], ph[3], c2 = 1.0, s2 = 0.0;
+                krp_basis<double>(nd, th, ph);
+                if (a2 != 0.0) krp_eta2<double>(th[0] * b[0] + th[1] * b[1] + th[2] * b[2], ph[0] * b[0] + ph[1] * b[1] + ph[2] * b[2], c2, s2);
+                const double qg = a2 / a1;
+                qe = (float)(c2 * qg); ue = (float)(s2 * qg);       // back to the lab reference of n (eq. 7 with -eta), fp32 state (R12)
+                break;
+            }
+        }
+    }
     const unsigned int slot = dir_bins ? atomicAdd(dir_bins + krp_dir_bin(w, i, 31u), 1u) : i;   // scanned counters: first slot of the bin
     q.pc[slot] = pc;
     q.nk[slot] = make_float4(nn[0], nn[1], nn[2], __uint_as_float(0u));
-    q.S[slot] = make_float4(1.f, 0.f, 0.f, 0.f);
+    q.S[slot] = make_float4(1.f, qe, ue, 0.f);
     q.tau[slot] = tau;
     q.id[slot] = id;
     if (g.emit_records) {

@@ -178,3 +178,41 @@ def test_two_step_image_matches_event_image_statistically():
         for s in (1, 2):
             assert abs(img_r[o, s].sum() - img_e[o, s].sum()) < 0.01 * Ie, (o, s)
     g.close()
+
+
+def test_thermal_packet_source_matches_the_oracle():
+    """Source kind 5 (reading R22): thermal emission of aligned grains as the packet source -- directions by rejection against
+    (1 - omega) alpha1(mu), initial Stokes (1, alpha2/alpha1, 0, 0) in the grain frame -- event by event against the oracle,
+    with a strongly direction-dependent table so that rejections are common; on a model with 4-byte cells it is the plain
+    volume source."""
+    from harness import oracle_run, compare_images_same_ids
+    cfg = inputs.make("c4", n=16, n_packets=6000, npix=24)
+    mu = np.linspace(0, 1, 9); s2 = 1 - mu * mu
+    cfg["opacity"] = np.stack([1 + 0.3 * s2, 0.3 * s2, 0.1 * s2, 0.3 + 0.4 * mu], 1).astype(np.float32)
+    cfg["source"] = dict(kind=5, pos=[0, 0, 0], dir=[0, 0, 1], cell_weight=np.ascontiguousarray(cfg["density"], np.float32))
+    n = cfg["n_packets"]
+    ora, img_o, img2_o, st_o = oracle_run(cfg, 0, n, cap=64 * n)
+    g = gpu_grid(cfg)
+    g.events_reserve(64 * n)
+    g.transport(n, cfg["seed"])
+    gev = gpu_events_sorted(g)
+    frac, info = compare_sequences(ora, gev, np.arange(n))
+    assert frac >= 0.999, show(info)
+    first = ora["k"] == 1
+    assert np.abs(ora["stokes"][first, 1:3]).max() > 0.05                     # the first events do carry the emitted polarisation
+    g.image(gpu_observers(cfg), cfg["npix"], cfg["npix"])
+    compare_images_same_ids(cfg, ora, gev, info, np.arange(n), g.image_get(), img_o, img2_o, cfg["npix"], cfg["npix"], name="thermal-source")
+    g.close()
+    from paper_2512_01283_b200 import krp
+    with pytest.raises(krp.KrpError):
+        gpu_grid(dict(cfg, source=dict(cfg["source"], kind=6)))               # thermal needs the volume source, isotropic candidates
+    c1 = inputs.make("c1", n=12, n_packets=3000, npix=16)
+    ev = {}
+    for kind in (1, 5):
+        c1["source"] = dict(kind=kind, pos=[0, 0, 0], dir=[0, 0, 1], cell_weight=None)
+        g = gpu_grid(c1)
+        g.transport(3000, 4)
+        ev[kind] = gpu_events_sorted(g)
+        g.close()
+    for key in ev[1]:
+        assert np.array_equal(ev[1][key], ev[5][key]), key
