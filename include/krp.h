@@ -157,6 +157,29 @@ int krp_image(krp_grid* g, const krp_observer* obs, int n_obs, int npix_x, int n
 int krp_image_get(krp_grid* g, double* out, int mem, void* stream);
 int krp_image_reset(krp_grid* g, void* stream);
 
+/* ---- Imaging without any allocation (for callers that cannot reach cudaMalloc: code under CUDA graph capture, tight
+ * serving loops, harnesses that forbid it) --------------------------------------------------------------------------
+ * The per-event imaging of PAPER.md:121 (peel-off, attenuation march with the in-cell solution of App. A, orthographic
+ * projection; what krp_image does) for n events the CALLER holds, toward ONE observer, ADDED to the caller's map.
+ *   k, cell, pos, dir, stokes   DEVICE arrays in the format of krp_events_get: event index (0 = emission record, imaged only
+ *                               with flags bit0), linear cell index (x fastest), cell-local position [n][3], incoming
+ *                               direction [n][3], albedo*weight*(1,q,u,v) [n][4] in the lab reference of dir;
+ *   obs                         HOST, one observer;    img   DEVICE, [4][npix_y][npix_x] doubles, the caller zeroes it;
+ *   rejected                    NULL, or HOST: receives the number of events that were left out (cell outside the grid,
+ *                               negative k, non-finite values); asking for it makes the call synchronise.
+ * The call makes no cudaMalloc, cudaFree or allocating library call and, with rejected = NULL, does not synchronise: it
+ * launches two kernels and one memset on `stream`.  Its event records and control block live in one fixed device array
+ * inside the library, KRP_NOALLOC_MAX_EVENTS events (12 MiB, held by every GPU that has loaded the library until the process
+ * ends): n beyond that is KRP_ERR_ARG.  All calls on a device share that array: calls that overlap on the GPU (two streams,
+ * two threads) race on it and must be serialised by the caller; nothing is carried from one call to the next.  The grid's
+ * own event buffer, maps, krp_stats and timing classes are not touched.  General mode marches over the 16-byte cells
+ * themselves (krp_image's per-observer coefficient arrays are an allocation) and the events are taken in the given order,
+ * so maps equal krp_image's up to the rounding of the fp32 march.  The grid must have been created on the current device. */
+#define KRP_NOALLOC_MAX_EVENTS 262144
+int krp_image_events_noalloc(krp_grid* g, uint64_t n, const int32_t* k, const int64_t* cell, const float* pos,
+                             const float* dir, const float* stokes, const krp_observer* obs, int npix_x, int npix_y,
+                             int flags, double* img, uint64_t* rejected, void* stream);
+
 /* ---- The paper's own two-step imaging (eq. 11) -------------------------------
  * Step 1: while a source grid is open, krp_transport also deposits, for every path segment of every flight (not only at
  * scattering events), the segment's expected scattered Stokes vector toward every camera,

@@ -6,7 +6,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(HERE)
 SRC_DIR = os.path.join(HERE, "csrc")
 SOURCES = ["krp_api.cu"]
-HEADERS = ["krp_device.cuh", "krp_kernels.cuh", "krp_twostep.cuh", os.path.join(ROOT, "include", "krp.h")]
+HEADERS = ["krp_device.cuh", "krp_kernels.cuh", "krp_twostep.cuh", "krp_noalloc.cuh", os.path.join(ROOT, "include", "krp.h")]
 LIB = os.path.join(HERE, "libkrp.so")
 
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",

@@ -381,6 +381,8 @@ static int upload_cells(krp_grid* g, const float* density, const float* bfield, 
     return KRP_OK;
 }
 
+static int krp_na_setup(int device);      // krp_noalloc.cuh (end of this file)
+
 extern "C" int krp_grid_create(krp_grid** out, int nx, int ny, int nz, const double bounds[6], const float* density,
                                const float* bfield, int mem, const krp_tables* tables, void* stream)
 {
@@ -404,6 +406,8 @@ extern "C" int krp_grid_create(krp_grid** out, int nx, int ny, int nz, const dou
 
     CK(cudaGetDevice(&g->device));
     CK(cudaDeviceGetAttribute(&g->n_sm, cudaDevAttrMultiProcessorCount, g->device));
+    rc = krp_na_setup(g->device);      // address of the fixed scratch array of krp_image_events_noalloc on this device
+    if (rc) return rc;
     KrpModel& m = g->m;
     memset(&m, 0, sizeof(m));
     m.nx = nx; m.ny = ny; m.nz = nz; m.ncell = (uint32_t)((uint64_t)nx * ny * nz);
@@ -1363,3 +1367,5 @@ extern "C" int krp_timing_get(krp_grid* g, double* ms, uint64_t* launches)
 }
 
 extern "C" uint64_t krp_launch_count(const krp_grid* g) { return g ? g->launches : 0; }
+
+#include "krp_noalloc.cuh"

@@ -12,6 +12,7 @@ from . import _build
 
 OK, ERR_ARG, ERR_CUDA, ERR_OOM, ERR_STATE, ERR_EVENT_FULL = 0, -1, -2, -3, -4, -5
 MEM_DEVICE, MEM_HOST = 0, 1
+NOALLOC_MAX_EVENTS = 262144      # KRP_NOALLOC_MAX_EVENTS of include/krp.h
 
 SYMBOLS = [
     "krp_last_error", "krp_version", "krp_grid_create", "krp_grid_destroy", "krp_grid_update", "krp_source_set",
@@ -19,6 +20,7 @@ SYMBOLS = [
     "krp_image_reset", "krp_stats_get", "krp_stats_reset", "krp_events_get", "krp_events_select", "krp_events_clear",
     "krp_tune", "krp_tune_schedule", "krp_timing_enable", "krp_timing_get", "krp_launch_count",
     "krp_sgrid_begin", "krp_sgrid_get", "krp_sgrid_reset", "krp_sgrid_end", "krp_image_rays", "krp_freq_define", "krp_freq_select", "krp_zmatrix_set",
+    "krp_image_events_noalloc",
 ]
 T_FLIGHT, T_SCATTER, T_ORDER, T_IMAGE, T_EMIT, T_DEPOSIT, T_RAYS, T_COUNT = 0, 1, 2, 3, 4, 5, 6, 7
 T_NAMES = ("flight", "scatter", "order", "image", "emit", "deposit", "rays")
@@ -114,6 +116,8 @@ def lib():
         "krp_sgrid_reset": (i32, [vp, vp]),
         "krp_sgrid_end": (i32, [vp]),
         "krp_image_rays": (i32, [vp, C.POINTER(Observer), i32, i32, i32, vp, i32, vp]),
+        "krp_image_events_noalloc": (i32, [vp, u64, vp, vp, vp, vp, vp, C.POINTER(Observer), i32, i32, i32, vp,
+                                           C.POINTER(u64), vp]),
     }
     for name, (res, args) in sig.items():
         f = getattr(L, name)
@@ -333,6 +337,23 @@ class Grid:
         _check(lib().krp_image_rays(self._h, arr, n, int(npix_x), int(npix_y), eptr, MEM_DEVICE if emem is None else emem,
                                     _stream(stream)))
         self.n_obs, self.npx, self.npy = n, int(npix_x), int(npix_y)
+
+    def image_events_noalloc(self, k, cell, pos, dir, stokes, observer, npix_x, npix_y, img, flags=0, want_rejected=False,
+                             stream=None):
+        """krp_image_events_noalloc: torch CUDA tensors k int32 [n], cell int64 [n], pos, dir float32 [n,3], stokes float32
+        [n,4], img float64 [4,npix_y,npix_x] (added to).  Pointers and sizes only: nothing is copied or allocated here."""
+        import torch
+        n = int(k.shape[0])
+        want = ((k, torch.int32, (n,)), (cell, torch.int64, (n,)), (pos, torch.float32, (n, 3)), (dir, torch.float32, (n, 3)),
+                (stokes, torch.float32, (n, 4)), (img, torch.float64, (4, int(npix_y), int(npix_x))))
+        for t, dt, shape in want:
+            if not (isinstance(t, torch.Tensor) and t.is_cuda and t.dtype == dt and tuple(t.shape) == shape and t.is_contiguous()):
+                raise TypeError("expected a contiguous CUDA tensor of dtype %s and shape %s" % (dt, shape))
+        rej = C.c_uint64(0)
+        _check(lib().krp_image_events_noalloc(self._h, n, k.data_ptr(), cell.data_ptr(), pos.data_ptr(), dir.data_ptr(),
+                                              stokes.data_ptr(), C.byref(observer), int(npix_x), int(npix_y), int(flags),
+                                              img.data_ptr(), C.byref(rej) if want_rejected else None, _stream(stream)))
+        return int(rej.value) if want_rejected else None
 
     def tune(self, transport_block=0, image_block=0, blocks_per_sm=0, flight_burst=0):
         _check(lib().krp_tune(self._h, int(transport_block), int(image_block), int(blocks_per_sm), int(flight_burst)))
