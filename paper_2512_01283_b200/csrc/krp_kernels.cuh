@@ -681,7 +681,7 @@ __device__ __forceinline__ void krp_appA_d(double i, double qg, double ug, doubl
         depth = c.dt1;
     } else {
         // thick cell: factor e^{-|alpha2 dtau|} moved into the scalar depth (no overflow at dtau ~ 1e3)
-        const double ax = fabs(x), E = exp(-2.0 * ax), sg = x > 0.0 ? 1.0 : -1.0, f = exp(-ax);
+        const double ax = fabs(x), f = exp(-ax), E = f * f, sg = x > 0.0 ? 1.0 : -1.0;      // one exponential for both factors
         i_n = 0.5 * ((i - sg * qg) + (i + sg * qg) * E);
         qg_n = 0.5 * ((qg - sg * i) + (qg + sg * i) * E);
         ug_n = f * un; v_n = f * vn;
