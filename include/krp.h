@@ -214,7 +214,8 @@ int krp_image_rays(krp_grid* g, const krp_observer* obs, int n_obs, int npix_x, 
  * (KRP_ERR_ARG otherwise).  krp_freq_select makes bin b the current one: krp_transport, krp_image, krp_image_rays,
  * krp_image_get and krp_image_reset then act on that bin (its tables, its density, its own maps; the observer set and
  * the pixel counts are common to all bins).  Buffered events belong to the bin they were transported in: image them before
- * selecting another bin (KRP_ERR_STATE if the buffer is not empty; it synchronises to check).  Bin 0 is current after
+ * selecting another bin (KRP_ERR_STATE if the buffer is not empty; it synchronises to check); an open source grid holds
+ * deposits of the current bin only: close it first (KRP_ERR_STATE otherwise).  Bin 0 is current after
  * krp_freq_define.  A model without krp_freq_define has the single bin of krp_grid_create. */
 int krp_freq_define(krp_grid* g, int n_freq, const krp_tables* tables, const float* kappa_scale, void* stream);
 int krp_freq_select(krp_grid* g, int bin, void* stream);

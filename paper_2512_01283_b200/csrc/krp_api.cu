@@ -1255,6 +1255,8 @@ extern "C" int krp_freq_select(krp_grid* g, int bin, void* stream)
     KrpCtl c;
     CK(cudaMemcpy(&c, g->d_ctl, sizeof(c), cudaMemcpyDeviceToHost));
     if (c.n_events != 0) return fail(KRP_ERR_STATE, "image (or clear) the buffered events before selecting another frequency bin");
+    // an open source grid holds the deposits of the current bin's opacities: mixing bins in it would be silent nonsense
+    if (g->d_sgrid) return fail(KRP_ERR_STATE, "close the source grid (krp_sgrid_end) before selecting another frequency bin");
     g->bins[g->cur_bin].d_img = g->d_img;            // park the maps of the bin we leave
     double* img = g->bins[bin].d_img;
     if (!img && g->d_img) {                           // same observer set and size for every bin

@@ -84,3 +84,19 @@ def test_grid_update_keeps_the_bins():
     frac, info = compare_sequences(ora, ev, np.arange(cfg["n_packets"]))
     assert frac >= 0.999, show(info)
     g.close()
+
+
+def test_bins_and_an_open_source_grid_do_not_mix():
+    """A source grid holds the deposits of the bin it was opened in: selecting another bin while it is open is refused."""
+    cfg = inputs.make("c1", n=12, n_packets=500, npix=16)
+    bins = _bins(False)
+    g = gpu_grid(cfg)
+    g.freq_define([(mu, op, cfg["w_min"], cfg["max_scatter"]) for mu, op, k in bins], [k for _, _, k in bins])
+    g.sgrid_begin(gpu_observers(cfg))
+    with pytest.raises(krp.KrpError) as ei:
+        g.freq_select(1)
+    assert ei.value.code == krp.ERR_STATE and "source grid" in str(ei.value)
+    g.freq_select(0)                      # the current bin: nothing to do
+    g.sgrid_end()
+    g.freq_select(1)
+    g.close()
