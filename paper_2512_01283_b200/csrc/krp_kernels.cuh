@@ -845,7 +845,11 @@ __global__ void __launch_bounds__(TPB, MINB) krp_k_flight_general(KrpModel g, Kr
 // T4/T5, general mode: one thread per flight that ended in an event.  From the state at the entry of the event cell:
 // solve for the depth t of the event (krp_event_solve_d), evolve the Stokes vector to t and normalise it to I = 1 (R7),
 // place the event, write the record (slot = first event of the wave + hit index: coalesced, no atomic), weight by the albedo.
-__global__ void __launch_bounds__(128) krp_k_event_general(KrpModel g, KrpCtl* ctl, KrpRecords q, int in, KrpHits hits, KrpRecords ev,
+// 64 registers (8 blocks per SM): a hit is three dependent reads away from its arithmetic (hit -> queue entry -> cell) and the kernel
+// waits for them (43 % of its stall samples on C3, profiles/r2r) -- warps in flight count for more than the 250 bytes of spills.
+// Measured on C3, flights + events per 2^22 packets: 118 registers (no bound) 8.29 ms, 96: 7.85, 80: 7.79, 64: 7.32; requesting the
+// next hit's queue entry and cell from L2 one iteration ahead made every variant slower (64 registers: 8.04 ms).
+__global__ void __launch_bounds__(128, 8) krp_k_event_general(KrpModel g, KrpCtl* ctl, KrpRecords q, int in, KrpHits hits, KrpRecords ev,
                                                            KrpEmitSrc es, double* __restrict__ flen)
 {
     const unsigned int n_hits = ctl->n_hits;
