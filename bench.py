@@ -66,6 +66,7 @@ def parse_args():
                     help="events: the north_star's form (per-event imaging, the contract's metric); twostep: the paper's own form "
                          "(every segment deposited into S(Omega_cam, x), one ray per pixel at the end of the timed steps)")
     ap.add_argument("--tune", default="", help="measurement only: transport_block,image_block,blocks_per_sm,flight_burst for krp_tune (0 keeps)")
+    ap.add_argument("--fused", type=int, default=-1, help="measurement only: krp_tune_fused(max_packets); -1 keeps the library's default")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
@@ -322,6 +323,8 @@ def run_krp(args):
     g = make_grid(krp, cfg, dens, bf, weight)
     if args.tune:
         g.tune(*[int(x) for x in args.tune.split(",")])
+    if args.fused >= 0:
+        g.tune_fused(args.fused)
 
     # pilot (untimed): events per packet of this workload, to size the event buffer once
     pilot = min(batch, 1 << 16)
@@ -417,7 +420,9 @@ def run_krp(args):
         "image": dict(kernel="krp_k_image<true,false>" if mode == "scalar" else "krp_k_image<false,true>", steps=st["steps_image"],
                       bytes=st["steps_image"] * A["cell_bytes"] + rays * EVENT_BYTES + st["contributions"] * CONTRIB_BYTES,
                       inst=st["steps_image"] * A["image_inst"] + rays * A["ray_inst"]),
-        "flight": dict(kernel="krp_k_flight_scalar_static" if mode == "scalar" else "krp_k_flight_general", steps=st["steps_transport"],
+        # scalar mode: one launch per step = the one-kernel form of small batches (krp_tune_fused), else one per scattering order
+        "flight": dict(kernel=("krp_k_packets_scalar" if timing["flight"][1] <= args.steps else "krp_k_flight_scalar_static")
+                       if mode == "scalar" else "krp_k_flight_general", steps=st["steps_transport"],
                        bytes=st["steps_transport"] * A["cell_bytes"] + flights * 64 + st["events"] * 56,
                        inst=st["steps_transport"] * A["flight_inst"] + flights * A["flight_fixed_inst"]),
     }

@@ -279,6 +279,13 @@ int krp_tune(krp_grid* g, int transport_block, int image_block, int blocks_per_s
  * effect at the next change of the observer set); order_policy 0 never / 1 by the measured ray length / 2 always order
  * the events by cell before imaging. */
 int krp_tune_schedule(krp_grid* g, int dir_sort, int obs_cells, int order_policy);
+/* Small batches in scalar mode (no field, constant non-dichroic opacity, F(Theta) scattering, no open source grid): a
+ * krp_transport call of at most max_packets packets runs as ONE kernel in which a thread follows a packet from emission to its
+ * end (flight, record, scattering, next flight: the kernel shape of PAPER.md:123) instead of one flight and one scattering
+ * launch per scattering order -- a batch that small is bound by launch latency as a wavefront.  Records are bit-identical to
+ * the wavefront's; their order in the event buffer differs.  Default 1048576 (measured on B200: the one kernel wins up to ~1.5e6
+ * packets on a 128^3 disk and beyond 4e6 on a 32^3 sphere); 0 = always the wavefront.  KRP_ERR_ARG if negative. */
+int krp_tune_fused(krp_grid* g, long long max_packets);
 /* Device time per kernel class, for measurement (bench.py's roofline): when enabled, every launch of a
  * flight, scattering, ordering or imaging kernel is bracketed by CUDA events on the caller's stream.
  * krp_timing_get synchronises, adds up the elapsed times since the last call into ms[KRP_T_COUNT] and the

@@ -89,6 +89,7 @@ struct krp_grid {
     size_t dir_scan_bytes = 0;
     size_t dir_bins_cap = 0;         // counters d_dir_bins holds
     int dir_sort = 1;
+    long long fused_max = 1048576;      // scalar mode: batches up to this many packets go through krp_k_packets_scalar (krp_tune_fused)
     unsigned int* d_order = nullptr;
     uint64_t order_cap = 0;
     double* d_src_cdf = nullptr;
@@ -671,6 +672,19 @@ extern "C" int krp_transport(krp_grid* g, uint64_t n_packets, uint64_t seed, voi
     }
     const unsigned n = (unsigned)n_packets;
     if (g->m.emit_records) g->ev_has_emission = 1;
+    if (g->m.scalar && !flen && !g->m.z.zt && (long long)n_packets <= g->fused_max && g->bins[g->cur_bin].max_waves > 1) {
+        // small batch, scalar mode: emission, then one kernel that follows every packet to its end (3 launches instead of 3 per order)
+        { TimedLaunch tl(g, st, KRP_T_EMIT);
+          krp_k_emit<<<(n + 255u) / 256u, 256, 0, st>>>(g->m, g->d_ctl, g->q[0], g->ev, g->next_id, n, seed, nullptr); }
+        krp_k_wave_prep<<<1, 1, 0, st>>>(g->d_ctl, 0);
+        { TimedLaunch tl(g, st, KRP_T_FLIGHT);
+          const unsigned need_p = (n + 127u) / 128u, pers_p = (unsigned)g->n_sm * 6u;
+          krp_k_packets_scalar<<<need_p < pers_p ? need_p : pers_p, 128, 0, st>>>(g->m, g->d_ctl, g->q[0], 0, g->ev, seed, g->bins[g->cur_bin].max_waves); }
+        g->launches += 3;
+        CK(cudaGetLastError());
+        g->next_id += n_packets;
+        return KRP_OK;
+    }
     const int tb = g->transport_block;
     const unsigned grid_all = (n + 255u) / 256u;
     KrpEmitSrc es0 = { nullptr, g->next_id, seed };     // first scattering order
@@ -1090,6 +1104,14 @@ extern "C" int krp_tune(krp_grid* g, int transport_block, int image_block, int b
     if (blocks_per_sm) { g->blocks_per_sm = blocks_per_sm; g->bps_tuned = 1; }
     if (flight_burst < 0 || flight_burst > 4096) return fail(KRP_ERR_ARG, "flight_burst must be in 0..4096");
     if (flight_burst) { g->burst = flight_burst; g->burst_auto = false; }
+    return KRP_OK;
+}
+
+extern "C" int krp_tune_fused(krp_grid* g, long long max_packets)
+{
+    if (!g) return fail(KRP_ERR_ARG, "grid is NULL");
+    if (max_packets < 0) return fail(KRP_ERR_ARG, "max_packets must be >= 0");
+    g->fused_max = max_packets;
     return KRP_OK;
 }
 

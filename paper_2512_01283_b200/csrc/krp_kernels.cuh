@@ -258,6 +258,7 @@ __device__ __forceinline__ void krp_event_append(const KrpModel& g, KrpCtl* ctl,
 #ifndef KRP_FLIGHT_CHUNK
 #define KRP_FLIGHT_CHUNK 128
 #endif
+template <unsigned int CHUNK = KRP_FLIGHT_CHUNK>
 __device__ __forceinline__ bool krp_take_work(unsigned int* counter, unsigned int n_items, bool idle, unsigned int& wbase,
                                               unsigned int& wleft, bool& more, unsigned int& item)
 {
@@ -269,10 +270,10 @@ __device__ __forceinline__ bool krp_take_work(unsigned int* counter, unsigned in
         if (want == 0u) break;
         if (wleft == 0u && more) {
             unsigned int b = 0;
-            if (lane == 0) b = atomicAdd(counter, (unsigned int)KRP_FLIGHT_CHUNK);
+            if (lane == 0) b = atomicAdd(counter, CHUNK);
             b = __shfl_sync(0xffffffffu, b, 0);
             if (b >= n_items) { more = false; }
-            else { wbase = b; wleft = min((unsigned int)KRP_FLIGHT_CHUNK, n_items - b); }
+            else { wbase = b; wleft = min(CHUNK, n_items - b); }
         }
         if (wleft == 0u) break;
         const unsigned rank = __popc(want & ((1u << lane) - 1u));
@@ -1018,7 +1019,166 @@ __device__ __forceinline__ void krp_peel_z(const KrpZt g, const float bh[3], con
 // of the wave, fp64.  Draws of block 0 of event k: (Theta, phi candidate, accept, next tau*);
 // blocks >= 1: two more (phi, accept) pairs each, at most 64 rounds.
 // ------------------------------------------------------------------------------------------
+// T6 for one event: from the stored pre-scatter state (direction n, Stokes (Q,U,V) of the record, lab reference of n) to the
+// outgoing direction in fp32 (R12), the scattered Stokes vector in the lab reference of that direction, and the next tau*.
+// kb = scattering order of the event (the Philox counter word), cell = padded cell id of the event.
 template <bool ZT>      // ZT: the outgoing direction and Stokes vector come from the full Z table (NEXT-2), else from F(Theta)
+__device__ __forceinline__ void krp_scatter_one(const KrpModel& g, unsigned long long seed, unsigned long long id, uint32_t kb,
+                                                const float4 nk, uint32_t cell, const float4 Se,
+                                                float nf[3], double& Q, double& U, double& V, double& tau_next)
+{
+    double b[3] = { 0.0, 0.0, 1.0 };
+    if (!g.scalar) { float4 cl = g.cell[cell]; b[0] = cl.y; b[1] = cl.z; b[2] = cl.w; }   // cell is a padded id
+    const double n[3] = { nk.x, nk.y, nk.z };
+    // A2: q_B from the direction angles of B (eq. 2).  Without a field (scalar mode) B^ = z^, q_B = 1: the grain
+    // frame is the lab frame and every step below that involves q_B or eta is the identity
+    double qB[4] = { 1.0, 0.0, 0.0, 0.0 };
+    double ng[3] = { n[0], n[1], n[2] };
+    double th[3], ph[3], c2 = 1.0, s2 = 0.0;
+    Q = Se.y; U = Se.z; V = Se.w;
+    if (!g.scalar) {
+        // half angles of theta_B in [0, pi] and phi_B in (-pi, pi] from their cosines and sines (no atan2, no sincos):
+        // cos(a/2) = sqrt((1 + cos a)/2), sin(a/2) = sin a / (2 cos(a/2)) on the side where that does not cancel
+        const double rho2 = b[0] * b[0] + b[1] * b[1], rho = sqrt(rho2);
+        const double inv_r = krp_rsqrt_near1(rho2 + b[2] * b[2]);       // B^ is unit to fp32 rounding
+        const double cth = b[2] * inv_r, sth = rho * inv_r;
+        double ch_t, sh_t, ch_p = 1.0, sh_p = 0.0;
+        if (cth >= 0.0) { ch_t = sqrt(0.5 * (1.0 + cth)); sh_t = sth / (2.0 * ch_t); }
+        else            { sh_t = sqrt(0.5 * (1.0 - cth)); ch_t = sth / (2.0 * sh_t); }
+        if (rho > 0.0) {
+            const double ir = 1.0 / rho, cph = b[0] * ir, sph = b[1] * ir;
+            if (cph >= 0.0) { ch_p = sqrt(0.5 * (1.0 + cph)); sh_p = sph / (2.0 * ch_p); }
+            else            { sh_p = copysign(sqrt(0.5 * (1.0 - cph)), sph); ch_p = sph / (2.0 * sh_p); }
+        }
+        qB[0] = ch_p * ch_t; qB[1] = -sh_p * sh_t; qB[2] = ch_p * sh_t; qB[3] = sh_p * ch_t;
+        // A3: direction in the grain frame (eq. 3)
+        krp_quat_rotate(qB, n, -1.0, ng);
+        // A5: Stokes reference lab -> grain frame
+        krp_basis_unit_d(n, th, ph);
+        krp_eta2<double>(krp_dot(th, b), krp_dot(ph, b), c2, s2);
+        krp_rot_qu(Q, U, c2, s2);
+    }
+    {
+        double r = krp_rsqrt_near1(krp_dot(ng, ng));       // a rotation of a direction that is unit to fp32 rounding
+        ng[0] *= r; ng[1] *= r; ng[2] *= r;
+    }
+    double nog[3];
+    if (ZT) {
+        // NEXT-2 (R21): outgoing direction by rejection sampling against the full Z: candidates isotropic in the
+        // grain frame, block 0 of event k = (cos, dphi, accept, next tau*), block b >= 1 = (cos, dphi, accept, -), at most 256
+        const double r2d = 57.29577951308232087680;
+        const double ti = acos(fmin(fmax(ng[2], -1.0), 1.0)) * r2d;
+        const double pin = (ng[0] * ng[0] + ng[1] * ng[1] >= 1e-24) ? atan2(ng[1], ng[0]) * r2d : 0.0;
+        double bound;
+        {
+            const double xi = ti * (double)(g.z.ni - 1) / 180.0;
+            const int i = max(0, min((int)floor(xi), g.z.ni - 2));
+            bound = fmax(g.z.bound[i], g.z.bound[i + 1]);
+        }
+        double to = 0.0, dp = 0.0;
+        tau_next = 0.0;
+        int rounds = 0;
+        for (uint32_t blk = 0; ; ++blk) {
+            const uint4 w = krp_philox(seed, id, kb, blk);
+            if (blk == 0u) tau_next = -log(krp_u01(w.w));
+            to = acos(1.0 - 2.0 * krp_u01(w.x)) * r2d;
+            dp = 360.0 * krp_u01(w.y);
+            double M1[16];
+            krp_zt_at<double>(g.z, ti, to, dp, 1, M1);
+            const double Iout = M1[0] + M1[1] * Q + M1[2] * U + M1[3] * V;
+            ++rounds;
+            if (krp_u01(w.z) * bound < Iout || rounds >= 256) break;
+        }
+        double M[16];
+        krp_zt_at<double>(g.z, ti, to, dp, 4, M);
+        {
+            const double I2 = M[0] + M[1] * Q + M[2] * U + M[3] * V, inv = 1.0 / I2;
+            const double Q2 = M[4] + M[5] * Q + M[6] * U + M[7] * V, U2 = M[8] + M[9] * Q + M[10] * U + M[11] * V,
+                         V2 = M[12] + M[13] * Q + M[14] * U + M[15] * V;
+            Q = Q2 * inv; U = U2 * inv; V = V2 * inv;      // referenced to theta^ of the outgoing direction in the grain frame
+        }
+        double st, ct, sp, cp;
+        sincos(to * (KRP_PI_D / 180.0), &st, &ct);
+        sincos((pin + dp) * (KRP_PI_D / 180.0), &sp, &cp);
+        nog[0] = st * cp; nog[1] = st * sp; nog[2] = ct;
+    } else {
+    // draws
+    uint4 w = krp_philox(seed, id, kb, 0u);
+    tau_next = -log(krp_u01(w.w));
+    double theta;   // Theta from the piecewise-linear CDF (R13), in units of the table spacing 180 deg/(n_ang-1)
+    {
+        double u = krp_u01(w.x);
+        int lo = 0, hi = g.n_ang - 1;
+        while (hi - lo > 1) { int mid = (lo + hi) >> 1; if (g.cdf[mid] <= u) lo = mid; else hi = mid; }
+        double wd = g.cdf[lo + 1] - g.cdf[lo];
+        double f = wd > 0.0 ? (u - g.cdf[lo]) / wd : 0.5;
+        theta = (double)lo + f;
+    }
+    // Theta in units of the table spacing: the Mueller row is linear in it (R13), Theta/180 deg = theta/(n_ang-1)
+    double F[4];
+    {
+        const int j = max(0, min((int)theta, g.n_ang - 2));
+        const double w1 = theta - (double)j, w0 = 1.0 - w1;
+        const float4 a = g.mueller[j], b2 = g.mueller[j + 1];
+        F[0] = w0 * (double)a.x + w1 * (double)b2.x; F[1] = w0 * (double)a.y + w1 * (double)b2.y;
+        F[2] = w0 * (double)a.z + w1 * (double)b2.z; F[3] = w0 * (double)a.w + w1 * (double)b2.w;
+    }
+    const double p12 = F[1] / F[0];
+    const double bound = 1.0 + fabs(p12) * sqrt(Q * Q + U * U);
+    double sphi, cphi;
+    sincospi(2.0 * krp_u01(w.y), &sphi, &cphi);           // phi = 2 pi u: no range reduction needed
+    bool ok;
+    {
+        double c2p = cphi * cphi - sphi * sphi, s2p = 2.0 * sphi * cphi;
+        ok = krp_u01(w.z) * bound < 1.0 + p12 * (Q * c2p + U * s2p);
+    }
+    int rounds = 1;
+    for (uint32_t blk = 1; !ok && rounds < 64; ++blk) {
+        uint4 x = krp_philox(seed, id, kb, blk);
+        uint32_t cand[2] = { x.x, x.z }, acc[2] = { x.y, x.w };
+        for (int h = 0; h < 2 && !ok && rounds < 64; ++h) {
+            sincospi(2.0 * krp_u01(cand[h]), &sphi, &cphi);
+            double c2p = cphi * cphi - sphi * sphi, s2p = 2.0 * sphi * cphi;
+            ok = krp_u01(acc[h]) * bound < 1.0 + p12 * (Q * c2p + U * s2p);
+            ++rounds;
+        }
+    }
+    // scattering in the grain frame
+    double thp[3], php[3];
+    krp_basis_unit_d(ng, thp, php);
+    double st, ct;
+    sincospi(theta * g.inv_nang1, &st, &ct);
+    double epar[3], eout[3], shat[3];
+    for (int j = 0; j < 3; ++j) epar[j] = cphi * thp[j] + sphi * php[j];
+    for (int j = 0; j < 3; ++j) nog[j] = ct * ng[j] + st * epar[j];
+    krp_rot_qu(Q, U, cphi * cphi - sphi * sphi, 2.0 * sphi * cphi);      // reference e_par
+    {
+        double I2 = F[0] + F[1] * Q, Q2 = F[1] + F[0] * Q;                  // F(Theta) (1,Q,U,V)
+        double U2 = F[2] * U + F[3] * V, V2 = -F[3] * U + F[2] * V;
+        const double inv = 1.0 / I2;
+        Q = Q2 * inv; U = U2 * inv; V = V2 * inv;
+    }
+    for (int j = 0; j < 3; ++j) eout[j] = ct * epar[j] - st * ng[j];
+    krp_cross(ng, epar, shat);
+    double th2[3], ph2[3];
+    krp_basis_unit_d(nog, th2, ph2);
+    {
+        double ce = krp_dot(eout, th2), se = krp_dot(th2, shat);
+        krp_rot_qu(Q, U, ce * ce - se * se, 2.0 * se * ce);                // reference theta^ of n'_GF
+    }
+    }
+    // back to the lab: inverse of eq. 3, direction stored in fp32 (R12)
+    double nl[3] = { nog[0], nog[1], nog[2] };
+    if (!g.scalar) krp_quat_rotate(qB, nog, 1.0, nl);
+    nf[0] = (float)nl[0]; nf[1] = (float)nl[1]; nf[2] = (float)nl[2];
+    if (!g.scalar) {
+        const double nd[3] = { nf[0], nf[1], nf[2] };
+        krp_basis_unit_d(nd, th, ph);
+        krp_eta2<double>(krp_dot(th, b), krp_dot(ph, b), c2, s2);
+        krp_rot_qu(Q, U, c2, -s2);
+    }}
+
+template <bool ZT>
 __global__ void __launch_bounds__(128, ZT ? 4 : 8) krp_k_scatter(KrpModel g, KrpCtl* ctl, KrpRecords ev, KrpRecords qo, int out,
                                                      unsigned long long seed)
 {
@@ -1032,156 +1192,9 @@ __global__ void __launch_bounds__(128, ZT ? 4 : 8) krp_k_scatter(KrpModel g, Krp
         const float4 pc = ev.pc[e], Se = ev.S[e];
         const unsigned long long id = ev.id[e];
         const uint32_t cell = __float_as_uint(pc.w);
-        double b[3] = { 0.0, 0.0, 1.0 };
-        if (!g.scalar) { float4 cl = g.cell[cell]; b[0] = cl.y; b[1] = cl.z; b[2] = cl.w; }   // cell is a padded id
-        const double n[3] = { nk.x, nk.y, nk.z };
-        // A2: q_B from the direction angles of B (eq. 2).  Without a field (scalar mode) B^ = z^, q_B = 1: the grain
-        // frame is the lab frame and every step below that involves q_B or eta is the identity
-        double qB[4] = { 1.0, 0.0, 0.0, 0.0 };
-        double ng[3] = { n[0], n[1], n[2] };
-        double th[3], ph[3], c2 = 1.0, s2 = 0.0;
-        double Q = Se.y, U = Se.z, V = Se.w;
-        if (!g.scalar) {
-            // half angles of theta_B in [0, pi] and phi_B in (-pi, pi] from their cosines and sines (no atan2, no sincos):
-            // cos(a/2) = sqrt((1 + cos a)/2), sin(a/2) = sin a / (2 cos(a/2)) on the side where that does not cancel
-            const double rho2 = b[0] * b[0] + b[1] * b[1], rho = sqrt(rho2);
-            const double inv_r = krp_rsqrt_near1(rho2 + b[2] * b[2]);       // B^ is unit to fp32 rounding
-            const double cth = b[2] * inv_r, sth = rho * inv_r;
-            double ch_t, sh_t, ch_p = 1.0, sh_p = 0.0;
-            if (cth >= 0.0) { ch_t = sqrt(0.5 * (1.0 + cth)); sh_t = sth / (2.0 * ch_t); }
-            else            { sh_t = sqrt(0.5 * (1.0 - cth)); ch_t = sth / (2.0 * sh_t); }
-            if (rho > 0.0) {
-                const double ir = 1.0 / rho, cph = b[0] * ir, sph = b[1] * ir;
-                if (cph >= 0.0) { ch_p = sqrt(0.5 * (1.0 + cph)); sh_p = sph / (2.0 * ch_p); }
-                else            { sh_p = copysign(sqrt(0.5 * (1.0 - cph)), sph); ch_p = sph / (2.0 * sh_p); }
-            }
-            qB[0] = ch_p * ch_t; qB[1] = -sh_p * sh_t; qB[2] = ch_p * sh_t; qB[3] = sh_p * ch_t;
-            // A3: direction in the grain frame (eq. 3)
-            krp_quat_rotate(qB, n, -1.0, ng);
-            // A5: Stokes reference lab -> grain frame
-            krp_basis_unit_d(n, th, ph);
-            krp_eta2<double>(krp_dot(th, b), krp_dot(ph, b), c2, s2);
-            krp_rot_qu(Q, U, c2, s2);
-        }
-        {
-            double r = krp_rsqrt_near1(krp_dot(ng, ng));       // a rotation of a direction that is unit to fp32 rounding
-            ng[0] *= r; ng[1] *= r; ng[2] *= r;
-        }
-        double tau_next, nog[3];
-        if (ZT) {
-            // NEXT-2 (R21): outgoing direction by rejection sampling against the full Z: candidates isotropic in the
-            // grain frame, block 0 of event k = (cos, dphi, accept, next tau*), block b >= 1 = (cos, dphi, accept, -), at most 256
-            const double r2d = 57.29577951308232087680;
-            const double ti = acos(fmin(fmax(ng[2], -1.0), 1.0)) * r2d;
-            const double pin = (ng[0] * ng[0] + ng[1] * ng[1] >= 1e-24) ? atan2(ng[1], ng[0]) * r2d : 0.0;
-            double bound;
-            {
-                const double xi = ti * (double)(g.z.ni - 1) / 180.0;
-                const int i = max(0, min((int)floor(xi), g.z.ni - 2));
-                bound = fmax(g.z.bound[i], g.z.bound[i + 1]);
-            }
-            double to = 0.0, dp = 0.0;
-            tau_next = 0.0;
-            int rounds = 0;
-            for (uint32_t blk = 0; ; ++blk) {
-                const uint4 w = krp_philox(seed, id, kb, blk);
-                if (blk == 0u) tau_next = -log(krp_u01(w.w));
-                to = acos(1.0 - 2.0 * krp_u01(w.x)) * r2d;
-                dp = 360.0 * krp_u01(w.y);
-                double M1[16];
-                krp_zt_at<double>(g.z, ti, to, dp, 1, M1);
-                const double Iout = M1[0] + M1[1] * Q + M1[2] * U + M1[3] * V;
-                ++rounds;
-                if (krp_u01(w.z) * bound < Iout || rounds >= 256) break;
-            }
-            double M[16];
-            krp_zt_at<double>(g.z, ti, to, dp, 4, M);
-            {
-                const double I2 = M[0] + M[1] * Q + M[2] * U + M[3] * V, inv = 1.0 / I2;
-                const double Q2 = M[4] + M[5] * Q + M[6] * U + M[7] * V, U2 = M[8] + M[9] * Q + M[10] * U + M[11] * V,
-                             V2 = M[12] + M[13] * Q + M[14] * U + M[15] * V;
-                Q = Q2 * inv; U = U2 * inv; V = V2 * inv;      // referenced to theta^ of the outgoing direction in the grain frame
-            }
-            double st, ct, sp, cp;
-            sincos(to * (KRP_PI_D / 180.0), &st, &ct);
-            sincos((pin + dp) * (KRP_PI_D / 180.0), &sp, &cp);
-            nog[0] = st * cp; nog[1] = st * sp; nog[2] = ct;
-        } else {
-        // draws
-        uint4 w = krp_philox(seed, id, kb, 0u);
-        tau_next = -log(krp_u01(w.w));
-        double theta;   // Theta from the piecewise-linear CDF (R13), in units of the table spacing 180 deg/(n_ang-1)
-        {
-            double u = krp_u01(w.x);
-            int lo = 0, hi = g.n_ang - 1;
-            while (hi - lo > 1) { int mid = (lo + hi) >> 1; if (g.cdf[mid] <= u) lo = mid; else hi = mid; }
-            double wd = g.cdf[lo + 1] - g.cdf[lo];
-            double f = wd > 0.0 ? (u - g.cdf[lo]) / wd : 0.5;
-            theta = (double)lo + f;
-        }
-        // Theta in units of the table spacing: the Mueller row is linear in it (R13), Theta/180 deg = theta/(n_ang-1)
-        double F[4];
-        {
-            const int j = max(0, min((int)theta, g.n_ang - 2));
-            const double w1 = theta - (double)j, w0 = 1.0 - w1;
-            const float4 a = g.mueller[j], b2 = g.mueller[j + 1];
-            F[0] = w0 * (double)a.x + w1 * (double)b2.x; F[1] = w0 * (double)a.y + w1 * (double)b2.y;
-            F[2] = w0 * (double)a.z + w1 * (double)b2.z; F[3] = w0 * (double)a.w + w1 * (double)b2.w;
-        }
-        const double p12 = F[1] / F[0];
-        const double bound = 1.0 + fabs(p12) * sqrt(Q * Q + U * U);
-        double sphi, cphi;
-        sincospi(2.0 * krp_u01(w.y), &sphi, &cphi);           // phi = 2 pi u: no range reduction needed
-        bool ok;
-        {
-            double c2p = cphi * cphi - sphi * sphi, s2p = 2.0 * sphi * cphi;
-            ok = krp_u01(w.z) * bound < 1.0 + p12 * (Q * c2p + U * s2p);
-        }
-        int rounds = 1;
-        for (uint32_t blk = 1; !ok && rounds < 64; ++blk) {
-            uint4 x = krp_philox(seed, id, kb, blk);
-            uint32_t cand[2] = { x.x, x.z }, acc[2] = { x.y, x.w };
-            for (int h = 0; h < 2 && !ok && rounds < 64; ++h) {
-                sincospi(2.0 * krp_u01(cand[h]), &sphi, &cphi);
-                double c2p = cphi * cphi - sphi * sphi, s2p = 2.0 * sphi * cphi;
-                ok = krp_u01(acc[h]) * bound < 1.0 + p12 * (Q * c2p + U * s2p);
-                ++rounds;
-            }
-        }
-        // scattering in the grain frame
-        double thp[3], php[3];
-        krp_basis_unit_d(ng, thp, php);
-        double st, ct;
-        sincospi(theta * g.inv_nang1, &st, &ct);
-        double epar[3], eout[3], shat[3];
-        for (int j = 0; j < 3; ++j) epar[j] = cphi * thp[j] + sphi * php[j];
-        for (int j = 0; j < 3; ++j) nog[j] = ct * ng[j] + st * epar[j];
-        krp_rot_qu(Q, U, cphi * cphi - sphi * sphi, 2.0 * sphi * cphi);      // reference e_par
-        {
-            double I2 = F[0] + F[1] * Q, Q2 = F[1] + F[0] * Q;                  // F(Theta) (1,Q,U,V)
-            double U2 = F[2] * U + F[3] * V, V2 = -F[3] * U + F[2] * V;
-            const double inv = 1.0 / I2;
-            Q = Q2 * inv; U = U2 * inv; V = V2 * inv;
-        }
-        for (int j = 0; j < 3; ++j) eout[j] = ct * epar[j] - st * ng[j];
-        krp_cross(ng, epar, shat);
-        double th2[3], ph2[3];
-        krp_basis_unit_d(nog, th2, ph2);
-        {
-            double ce = krp_dot(eout, th2), se = krp_dot(th2, shat);
-            krp_rot_qu(Q, U, ce * ce - se * se, 2.0 * se * ce);                // reference theta^ of n'_GF
-        }
-        }
-        // back to the lab: inverse of eq. 3, direction stored in fp32 (R12)
-        double nl[3] = { nog[0], nog[1], nog[2] };
-        if (!g.scalar) krp_quat_rotate(qB, nog, 1.0, nl);
-        const float nf[3] = { (float)nl[0], (float)nl[1], (float)nl[2] };
-        if (!g.scalar) {
-            const double nd[3] = { nf[0], nf[1], nf[2] };
-            krp_basis_unit_d(nd, th, ph);
-            krp_eta2<double>(krp_dot(th, b), krp_dot(ph, b), c2, s2);
-            krp_rot_qu(Q, U, c2, -s2);
-        }
+        float nf[3];
+        double Q, U, V, tau_next;
+        krp_scatter_one<ZT>(g, seed, id, kb, nk, cell, Se, nf, Q, U, V, tau_next);
         unsigned int slot = krp_reserve32(&ctl->q_count[out]);
         qo.pc[slot] = pc;
         qo.nk[slot] = make_float4(nf[0], nf[1], nf[2], __uint_as_float(kb));
@@ -1189,6 +1202,95 @@ __global__ void __launch_bounds__(128, ZT ? 4 : 8) krp_k_scatter(KrpModel g, Krp
         qo.tau[slot] = tau_next;
         qo.id[slot] = id;
     }
+}
+
+// T3-T7, scalar mode, small batches: one thread follows a packet from its queue entry to its end -- flight, event record,
+// scattering, next flight -- the shape the paper gives its own kernel.  A batch of 10^5 packets (BASELINE
+// configs[0]) fills the GPU once; as a wavefront it is 14 orders x 3 launches of a few microseconds of work each, i.e. launch
+// latency (0.72 ms per job of 10^5 packets against 0.30 ms), and the later orders hold a handful of packets.  Same arithmetic as
+// the wave path in the same order per packet (flight of krp_k_flight_scalar_static, krp_event_append, krp_scatter_one): the
+// records are bit-identical, only their order in the buffer differs.  Used for batches of at most krp_tune_fused() packets
+// (default 2^20; the wavefront wins from ~1.5e6 packets on, where its direction-ordered first flights and converged
+// scattering kernels outweigh its launches: profiles/r2r_README.md).
+// 80 registers, six blocks of 128 per SM: 10^5 packets are resident at once (C1, one packet per thread: 0.165 ms at 150
+// registers and three blocks, two rounds; 0.130 ms at 80; 0.143 ms at 64).
+__global__ void __launch_bounds__(128, 6) krp_k_packets_scalar(KrpModel g, KrpCtl* ctl, KrpRecords q, int in, KrpRecords ev,
+                                                            unsigned long long seed, int max_flights)
+{
+    const unsigned int n_items = ctl->q_count[in];
+    KrpFlightTally tl = { 0, 0, 0, 0.0, 0.0, 0.0 };
+    // Persistent lanes: a lane whose packet has ended takes the next queue entry at the top of the loop, where the warp is
+    // converged (one scattering order per turn: flight, record, scattering), so the lanes of a warp stay busy although most
+    // packets end after one or two events and a few live through all orders (6.8 of 32 lanes active with one packet per
+    // thread, profiles/r2s).
+    unsigned int wbase = 0, wleft = 0, item = 0;
+    bool more = true, alive = false;
+    float4 pc = make_float4(0.f, 0.f, 0.f, 0.f), nk = pc, S0 = pc;
+    double D = 0.0;
+    unsigned long long id = 0;
+    int f = 0;
+    for (;;) {
+        if (krp_take_work<32u>(&ctl->work[0], n_items, !alive, wbase, wleft, more, item)) {      // 32 per visit: a small batch spreads over all warps
+            pc = q.pc[item]; nk = q.nk[item]; S0 = q.S[item];
+            D = q.tau[item];
+            id = q.id[item];
+            alive = true; f = 0;
+        }
+        if (!__any_sync(0xffffffffu, alive)) break;
+        if (alive) {
+            const float n[3] = { nk.x, nk.y, nk.z };
+            const float p0[3] = { pc.x, pc.y, pc.z };
+            const uint32_t c0 = __float_as_uint(pc.w);
+            KrpRay ray;
+            krp_ray_init(g, c0, p0, n, ray);
+            uint32_t c_cur = ray.c;
+            int ax_cur = -1;
+            KRP_CK(g, c_cur);
+            float kr_cur = __ldg(g.kr + c_cur);
+            bool hit = false;
+            for (;;) {
+                int ax_n;
+                const float ds = krp_ray_advance(ray, ax_n);
+                KRP_CK(g, ray.c);
+                const float kr_nxt = __ldg(g.kr + ray.c);          // requested before the depth test of the current cell
+                const float dt1 = g.a1c * kr_cur * ds;
+                if ((double)dt1 >= D) { hit = true; break; }       // event inside the current cell
+                D -= (double)dt1;
+                c_cur = ray.c;
+                if (kr_nxt < 0.f) break;                           // halo: the packet left the grid
+                ax_cur = ax_n; kr_cur = kr_nxt;
+            }
+            int h0[3], h1[3];
+            krp_pad_coords(g, c0, h0[0], h0[1], h0[2]);
+            krp_pad_coords(g, c_cur, h1[0], h1[1], h1[2]);
+            const int crossings = abs(h1[0] - h0[0]) + abs(h1[1] - h0[1]) + abs(h1[2] - h0[2]);
+            alive = false;
+            if (!hit) { tl.steps += (unsigned long long)crossings; tl.w_esc += (double)S0.x; }
+            else {
+                tl.steps += (unsigned long long)(crossings + 1);
+                const double moved = D / ((double)g.a1c * (double)kr_cur);
+                float pe[3];
+                krp_event_pos(g, n, p0, c0, c_cur, ax_cur, moved, pe);
+                const uint32_t k = __float_as_uint(nk.w);
+                krp_event_append(g, ctl, ev, id, c_cur, pe, n, k, S0.x, g.omc, S0.y, S0.z, S0.w, tl);
+                // what krp_event_append stored: weight after the albedo, order, termination (R12)
+                const float Wn = g.omc * S0.x;
+                const uint32_t kn = k + 1u;
+                if (!((Wn < g.w_min) || ((int)kn >= g.max_scatter)) && ++f < max_flights) {
+                    const float4 Se = make_float4(Wn, S0.y, S0.z, S0.w);
+                    float nf[3];
+                    double Q, U, V, tau_next;
+                    krp_scatter_one<false>(g, seed, id, kn, make_float4(n[0], n[1], n[2], __uint_as_float(kn)), c_cur, Se, nf, Q, U, V, tau_next);
+                    pc = make_float4(pe[0], pe[1], pe[2], __uint_as_float(c_cur));
+                    nk = make_float4(nf[0], nf[1], nf[2], __uint_as_float(kn));
+                    S0 = make_float4(Wn, (float)Q, (float)U, (float)V);
+                    D = tau_next;
+                    alive = true;
+                }
+            }
+        }
+    }
+    krp_tally_flush(tl, ctl);
 }
 
 // ------------------------------------------------------------------------------------------

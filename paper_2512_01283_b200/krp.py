@@ -18,7 +18,7 @@ SYMBOLS = [
     "krp_last_error", "krp_version", "krp_grid_create", "krp_grid_destroy", "krp_grid_update", "krp_source_set",
     "krp_events_reserve", "krp_transport", "krp_packet_id_set", "krp_image", "krp_image_get",
     "krp_image_reset", "krp_stats_get", "krp_stats_reset", "krp_events_get", "krp_events_select", "krp_events_clear",
-    "krp_tune", "krp_tune_schedule", "krp_timing_enable", "krp_timing_get", "krp_launch_count",
+    "krp_tune", "krp_tune_schedule", "krp_tune_fused", "krp_timing_enable", "krp_timing_get", "krp_launch_count",
     "krp_sgrid_begin", "krp_sgrid_get", "krp_sgrid_reset", "krp_sgrid_end", "krp_image_rays", "krp_freq_define", "krp_freq_select", "krp_zmatrix_set",
     "krp_image_events_noalloc",
 ]
@@ -107,6 +107,7 @@ def lib():
         "krp_timing_enable": (i32, [vp, i32]),
         "krp_timing_get": (i32, [vp, vp, vp]),
         "krp_tune_schedule": (i32, [vp, i32, i32, i32]),
+        "krp_tune_fused": (i32, [vp, C.c_longlong]),
         "krp_launch_count": (u64, [vp]),
         "krp_zmatrix_set": (i32, [vp, i32, i32, i32, vp, vp]),
         "krp_freq_define": (i32, [vp, i32, C.POINTER(Tables), vp, vp]),
@@ -360,6 +361,9 @@ class Grid:
 
     def tune_schedule(self, dir_sort=-1, obs_cells=-1, order_policy=-1):
         _check(lib().krp_tune_schedule(self._h, int(dir_sort), int(obs_cells), int(order_policy)))
+
+    def tune_fused(self, max_packets):
+        _check(lib().krp_tune_fused(self._h, int(max_packets)))
 
     def version(self):
         return lib().krp_version().decode()

@@ -20,7 +20,7 @@ from harness import (oracle_run, gpu_grid, gpu_observers, gpu_events_sorted, com
 pytestmark = pytest.mark.gpu
 
 SMALL = {
-    "c1": dict(n=32, n_packets=100000, npix=64),         # BASELINE configs[0] in full (direction-ordered first flights)
+    "c1": dict(n=32, n_packets=100000, npix=64),         # BASELINE configs[0] in full (one-kernel form of small scalar batches)
     "c2": dict(n=48, n_packets=6000, npix=64),
     "c3": dict(n=12, n_packets=1500, npix=32),
     "c4": dict(n=40, n_packets=4000, npix=48),
@@ -306,15 +306,23 @@ def test_full_size_general_mode_sampled_ids(name, batch, ns):
 
 
 def test_launch_shapes_do_not_change_results():
-    """krp_tune knobs (static vs persistent flights, refill distance, block sizes, persistent blocks per SM) change
-    the schedule only: events are bit-identical, maps equal up to the order of the fp64 sums."""
-    for name, kw in (("c2", dict(n=32, n_packets=20000, npix=32)), ("c4", dict(n=24, n_packets=6000, npix=32))):
+    """krp_tune knobs (static vs persistent flights, refill distance, block sizes, persistent blocks per SM) and, in scalar
+    mode, the one-kernel form of small batches (krp_tune_fused: a thread follows a packet to its end) against the wavefront
+    change the schedule only: events are bit-identical, maps equal up to the order of the fp64 sums."""
+    for name, kw in (("c2", dict(n=32, n_packets=20000, npix=32)), ("c4", dict(n=24, n_packets=6000, npix=32)),
+                     ("c1", dict(n=32, n_packets=30000, npix=32))):
         cfg = inputs.make(name, **kw)
         ref_ev = ref_img = None
-        for tune in (dict(), dict(flight_burst=1), dict(flight_burst=5), dict(flight_burst=64, transport_block=128),
+        # the first entry runs the library's defaults (scalar mode: a batch this small takes the one-kernel form);
+        # every other entry the wavefront (fused = 0)
+        for tune in (dict(fused=None), dict(), dict(flight_burst=1), dict(flight_burst=5), dict(flight_burst=64, transport_block=128),
                      dict(blocks_per_sm=2, image_block=64), dict(blocks_per_sm=16, flight_burst=16),
                      dict(transport_block=256), dict(transport_block=64, blocks_per_sm=4)):   # both builds of the general flight
+            tune = dict(tune)
+            fused = tune.pop("fused", 0)
             g = gpu_grid(cfg)
+            if fused is not None:
+                g.tune_fused(fused)
             g.tune(**tune)
             g.timing_enable(True)
             g.transport(cfg["n_packets"], cfg["seed"])
@@ -323,12 +331,14 @@ def test_launch_shapes_do_not_change_results():
             img = g.image_get()
             tm = g.timing_get()
             assert tm["flight"][1] >= 1 and tm["image"][1] == len(cfg["observers"]) and tm["image"][0] > 0
+            if name in ("c1", "c2"):      # scalar mode: one flight launch in the one-kernel form, one per order as a wavefront
+                assert (tm["flight"][1] == 1) == (fused is None), (name, tune, fused, tm["flight"])
             if ref_ev is None:
                 ref_ev, ref_img = ev, img
             else:
                 for key in ref_ev:
-                    assert np.array_equal(ref_ev[key], ev[key]), (name, tune, key)
-                assert np.allclose(img, ref_img, rtol=1e-11, atol=1e-13 * ref_img[:, 0].max()), (name, tune)
+                    assert np.array_equal(ref_ev[key], ev[key]), (name, tune, fused, key)
+                assert np.allclose(img, ref_img, rtol=1e-11, atol=1e-13 * ref_img[:, 0].max()), (name, tune, fused)
             g.close()
 
 
