@@ -178,6 +178,9 @@ def test_empty_and_degenerate_inputs():
         g.stats_get()
     assert ei.value.code == krp.ERR_EVENT_FULL
     # bad arguments come back as error codes
+    with pytest.raises(krp.KrpError) as ei:
+        g.tune_fused(-1)
+    assert ei.value.code == krp.ERR_ARG
     with pytest.raises(krp.KrpError):
         krp.Grid(0, 4, 4, [0, 1, 0, 1, 0, 1], torch.zeros(16, device="cuda"), None, cfg["mueller"], cfg["opacity"])
     bad = cfg["opacity"].copy(); bad[0, 1] = 2.0

@@ -48,6 +48,8 @@ def test_null_arguments_return_error_codes_without_a_gpu():
     assert L.krp_transport(None, 10, 1, None) == krp.ERR_ARG
     assert L.krp_image(None, None, 0, 4, 4, 0, None) == krp.ERR_ARG
     assert L.krp_tune(None, 0, 0, 0, 0) == krp.ERR_ARG
+    assert L.krp_tune_fused(None, 1000) == krp.ERR_ARG
+    assert L.krp_tune_schedule(None, -1, -1, -1) == krp.ERR_ARG
     assert L.krp_timing_get(None, None, None) == krp.ERR_ARG
     assert L.krp_launch_count(None) == 0
     assert L.krp_grid_destroy(None) == krp.OK
