@@ -92,6 +92,15 @@ int krp_grid_destroy(krp_grid* g);
  * Re-packs the cells without re-allocating anything; buffered events and image maps are left as they are.
  * Synchronises (it reports bad densities).  Errors as krp_grid_create. */
 int krp_grid_update(krp_grid* g, const float* density, const float* bfield, int mem, void* stream);
+/* The same for HOST snapshots, in two halves, so that the host-to-device copy of the NEXT snapshot runs while the current one
+ * is still being transported and imaged: krp_grid_stage starts the copy of density/bfield (host arrays; pinned memory makes it
+ * asynchronous) into the model's staging buffers on `copy_stream` and returns at once; krp_grid_update_staged makes `stream`
+ * wait for that copy, re-packs the cells from it (after whatever `stream` still runs on the old cells) and synchronises like
+ * krp_grid_update.  One snapshot can be staged at a time: stage the next one only after the last krp_grid_update /
+ * krp_grid_update_staged has returned; a krp_grid_update with KRP_MEM_HOST in between overwrites a staged snapshot.
+ * Errors: KRP_ERR_ARG as krp_grid_update; KRP_ERR_STATE from krp_grid_update_staged when nothing is staged. */
+int krp_grid_stage(krp_grid* g, const float* density, const float* bfield, void* copy_stream);
+int krp_grid_update_staged(krp_grid* g, void* stream);
 
 /* Source of packets (PAPER.md:107 emission; R17).
  *   kind bit0: 0 = all packets start at pos, 1 = start uniformly inside a cell drawn with

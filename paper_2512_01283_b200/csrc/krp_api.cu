@@ -69,6 +69,8 @@ struct krp_grid {
     float4* d_cell_alloc = nullptr;
     float* d_stage_den = nullptr;   // staging of host inputs (krp_grid_create / krp_grid_update with KRP_MEM_HOST)
     float* d_stage_b = nullptr;
+    bool staged = false;            // krp_grid_stage: the staging buffers hold (or are receiving) a snapshot not yet packed
+    cudaEvent_t stage_ev = nullptr;
     int* d_bad = nullptr;
     bool has_bfield = false;
     bool obs_cells_stale = false;   // cells changed since the per-observer coefficient arrays were built (or never built)
@@ -203,7 +205,7 @@ static int alloc_records(KrpRecords& r, uint64_t cap, bool with_tau)
 extern "C" int krp_grid_destroy(krp_grid* g)
 {
     if (!g) return KRP_OK;
-    cudaFree(g->d_kr_alloc); cudaFree(g->d_cell_alloc); cudaFree(g->d_stage_den); cudaFree(g->d_stage_b); cudaFree(g->d_bad); cudaFree(g->d_base);
+    cudaFree(g->d_kr_alloc); cudaFree(g->d_cell_alloc); cudaFree(g->d_stage_den); cudaFree(g->d_stage_b); if (g->stage_ev) cudaEventDestroy(g->stage_ev); cudaFree(g->d_bad); cudaFree(g->d_base);
     if (!g->bins.empty()) g->bins[g->cur_bin].d_img = nullptr;      // the current bin's maps are g->d_img, freed below
     for (TableSet& t : g->bins) free_tables(t);
     cudaFree(g->d_src_cdf); cudaFree(g->d_ctl); cudaFree(g->d_obs); cudaFree(g->d_img); cudaFree(g->d_obs_cells);
@@ -343,6 +345,19 @@ static void apply_tables(krp_grid* g, int b)
 }
 
 // T0: (re)pack the caller's density / field arrays into the padded cell array of g (halo included)
+// host arrays -> the model's staging buffers (kept for later calls), asynchronously on st
+static int stage_copy(krp_grid* g, const float* density, const float* bfield, cudaStream_t st)
+{
+    KrpModel& m = g->m;
+    if (!g->d_stage_den) CK(cudaMalloc(&g->d_stage_den, sizeof(float) * (size_t)m.ncell));
+    CK(cudaMemcpyAsync(g->d_stage_den, density, sizeof(float) * (size_t)m.ncell, cudaMemcpyHostToDevice, st));
+    if (bfield && !m.scalar) {
+        if (!g->d_stage_b) CK(cudaMalloc(&g->d_stage_b, sizeof(float) * 3 * (size_t)m.ncell));
+        CK(cudaMemcpyAsync(g->d_stage_b, bfield, sizeof(float) * 3 * (size_t)m.ncell, cudaMemcpyHostToDevice, st));
+    }
+    return KRP_OK;
+}
+
 static int upload_cells(krp_grid* g, const float* density, const float* bfield, int mem, cudaStream_t st)
 {
     KrpModel& m = g->m;
@@ -350,15 +365,11 @@ static int upload_cells(krp_grid* g, const float* density, const float* bfield, 
     const float* d_b = bfield;
     const bool want_b = bfield && !m.scalar;
     if (mem == KRP_MEM_HOST) {
-        // staging buffers are kept for later krp_grid_update calls
-        if (!g->d_stage_den) CK(cudaMalloc(&g->d_stage_den, sizeof(float) * (size_t)m.ncell));
-        CK(cudaMemcpyAsync(g->d_stage_den, density, sizeof(float) * (size_t)m.ncell, cudaMemcpyHostToDevice, st));
+        g->staged = false;      // a staged snapshot that was never packed is overwritten
+        int rc = stage_copy(g, density, bfield, st);
+        if (rc) return rc;
         d_den = g->d_stage_den;
-        if (want_b) {
-            if (!g->d_stage_b) CK(cudaMalloc(&g->d_stage_b, sizeof(float) * 3 * (size_t)m.ncell));
-            CK(cudaMemcpyAsync(g->d_stage_b, bfield, sizeof(float) * 3 * (size_t)m.ncell, cudaMemcpyHostToDevice, st));
-            d_b = g->d_stage_b;
-        }
+        if (want_b) d_b = g->d_stage_b;
     }
     if (!g->d_bad) CK(cudaMalloc(&g->d_bad, sizeof(int)));
     CK(cudaMemsetAsync(g->d_bad, 0, sizeof(int), st));
@@ -516,6 +527,27 @@ extern "C" int krp_grid_update(krp_grid* g, const float* density, const float* b
     if (mem != KRP_MEM_DEVICE && mem != KRP_MEM_HOST) return fail(KRP_ERR_ARG, "mem must be KRP_MEM_DEVICE or KRP_MEM_HOST");
     if ((bfield != nullptr) != g->has_bfield) return fail(KRP_ERR_ARG, "bfield must be given exactly when the grid was created with one");
     return upload_cells(g, density, bfield, mem, (cudaStream_t)stream);
+}
+
+extern "C" int krp_grid_stage(krp_grid* g, const float* density, const float* bfield, void* copy_stream)
+{
+    if (!g || !density) return fail(KRP_ERR_ARG, "grid or density is NULL");
+    if ((bfield != nullptr) != g->has_bfield) return fail(KRP_ERR_ARG, "bfield must be given exactly when the grid was created with one");
+    if (!g->stage_ev) CK(cudaEventCreateWithFlags(&g->stage_ev, cudaEventDisableTiming));
+    int rc = stage_copy(g, density, bfield, (cudaStream_t)copy_stream);
+    if (rc) return rc;
+    CK(cudaEventRecord(g->stage_ev, (cudaStream_t)copy_stream));
+    g->staged = true;
+    return KRP_OK;
+}
+
+extern "C" int krp_grid_update_staged(krp_grid* g, void* stream)
+{
+    if (!g) return fail(KRP_ERR_ARG, "grid is NULL");
+    if (!g->staged) return fail(KRP_ERR_STATE, "no staged snapshot: call krp_grid_stage first");
+    CK(cudaStreamWaitEvent((cudaStream_t)stream, g->stage_ev, 0));
+    g->staged = false;
+    return upload_cells(g, g->d_stage_den, g->has_bfield ? g->d_stage_b : nullptr, KRP_MEM_DEVICE, (cudaStream_t)stream);
 }
 
 extern "C" int krp_source_set(krp_grid* g, const krp_source* src, void* stream)

@@ -15,7 +15,7 @@ MEM_DEVICE, MEM_HOST = 0, 1
 NOALLOC_MAX_EVENTS = 262144      # KRP_NOALLOC_MAX_EVENTS of include/krp.h
 
 SYMBOLS = [
-    "krp_last_error", "krp_version", "krp_grid_create", "krp_grid_destroy", "krp_grid_update", "krp_source_set",
+    "krp_last_error", "krp_version", "krp_grid_create", "krp_grid_destroy", "krp_grid_update", "krp_grid_stage", "krp_grid_update_staged", "krp_source_set",
     "krp_events_reserve", "krp_transport", "krp_packet_id_set", "krp_image", "krp_image_get",
     "krp_image_reset", "krp_stats_get", "krp_stats_reset", "krp_events_get", "krp_events_select", "krp_events_clear",
     "krp_tune", "krp_tune_schedule", "krp_tune_fused", "krp_timing_enable", "krp_timing_get", "krp_launch_count",
@@ -91,6 +91,8 @@ def lib():
                                   C.POINTER(Tables), vp]),
         "krp_grid_destroy": (i32, [vp]),
         "krp_grid_update": (i32, [vp, vp, vp, i32, vp]),
+        "krp_grid_stage": (i32, [vp, vp, vp, vp]),
+        "krp_grid_update_staged": (i32, [vp, vp]),
         "krp_source_set": (i32, [vp, C.POINTER(Source), vp]),
         "krp_events_reserve": (i32, [vp, u64]),
         "krp_transport": (i32, [vp, u64, u64, vp]),
@@ -206,6 +208,18 @@ class Grid:
         if bptr is not None and bmem != dmem:
             raise ValueError("density and bfield must live in the same memory space")
         _check(lib().krp_grid_update(self._h, dptr, bptr, dmem, _stream(stream)))
+
+    def stage(self, density, bfield=None, copy_stream=None):
+        """Start the host-to-device copy of the next snapshot (host arrays, pinned for an asynchronous copy) on copy_stream."""
+        dptr, dmem, dkeep = _ptr_mem(density)
+        bptr, bmem, bkeep = _ptr_mem(bfield)
+        if dmem != MEM_HOST or (bptr is not None and bmem != MEM_HOST):
+            raise ValueError("krp_grid_stage takes host arrays")
+        _check(lib().krp_grid_stage(self._h, dptr, bptr, _stream(copy_stream)))
+
+    def update_staged(self, stream=None):
+        """Re-pack the cells from the staged snapshot once its copy has arrived."""
+        _check(lib().krp_grid_update_staged(self._h, _stream(stream)))
 
     def source_set(self, kind=0, pos=None, direction=(0, 0, 1), cell_weight=None, emit_records=0, stream=None):
         s = Source()

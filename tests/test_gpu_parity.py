@@ -436,9 +436,29 @@ def test_grid_update_equals_a_new_grid():
         for key in ev_n:
             assert np.array_equal(ev_u[key], ev_n[key]), (name, key)
         assert np.allclose(img_u, img_n, rtol=1e-11, atol=1e-13 * img_n[:, 0].max())
+        from paper_2512_01283_b200 import krp
+        # the pipelined form: the copy of the next snapshot (pinned host arrays) starts on a copy stream while the model still
+        # works on the old cells, krp_grid_update_staged re-packs from it -- same records as the plain update
+        g.update(cfg["density"], cfg["bfield"])
+        pin = lambda a: None if a is None else torch.from_numpy(np.ascontiguousarray(a, np.float32)).pin_memory()
+        p_d, p_b = pin(dens2), pin(bf2)
+        with pytest.raises(krp.KrpError) as ei:
+            g.update_staged()
+        assert ei.value.code == krp.ERR_STATE
+        g.events_clear(); g.image_reset(); g.stats_reset(); g.packet_id_set(0)
+        g.transport(cfg["n_packets"], cfg["seed"])              # old cells, in flight while the copy runs
+        cs = torch.cuda.Stream()
+        g.stage(p_d.numpy(), None if p_b is None else p_b.numpy(), copy_stream=cs)
+        ev_old = gpu_events_sorted(g)
+        g.events_clear(); g.packet_id_set(0)
+        g.update_staged()
+        g.transport(cfg["n_packets"], cfg["seed"])
+        ev_s = gpu_events_sorted(g)
+        for key in ev_n:
+            assert np.array_equal(ev_s[key], ev_n[key]), (name, "staged", key)
+        assert not all(np.array_equal(ev_old[key], ev_n[key]) for key in ev_n)      # the old cells really were other cells
         # device arrays, and argument errors
         g.update(torch.from_numpy(dens2).cuda(), None if bf2 is None else torch.from_numpy(bf2).cuda())
-        from paper_2512_01283_b200 import krp
         with pytest.raises(krp.KrpError):
             g.update(-dens2, bf2)
         if bf2 is not None:
