@@ -258,9 +258,8 @@ __device__ __forceinline__ void krp_event_append(const KrpModel& g, KrpCtl* ctl,
 #ifndef KRP_FLIGHT_CHUNK
 #define KRP_FLIGHT_CHUNK 128
 #endif
-template <unsigned int CHUNK = KRP_FLIGHT_CHUNK>
 __device__ __forceinline__ bool krp_take_work(unsigned int* counter, unsigned int n_items, bool idle, unsigned int& wbase,
-                                              unsigned int& wleft, bool& more, unsigned int& item)
+                                              unsigned int& wleft, bool& more, unsigned int& item, const unsigned int CHUNK = KRP_FLIGHT_CHUNK)
 {
     const int lane = threadIdx.x & 31;
     bool got = false;
@@ -716,6 +715,10 @@ __global__ void __launch_bounds__(TPB, MINB) krp_k_flight_general(KrpModel g, Kr
     KrpFlightTally tl = { 0, 0, 0, 0.0, 0.0, 0.0 };
     const double xs = g.xs;
     const float inv_guard = 1.f / g.guard;
+    // queue entries a warp reserves per visit to the launch's work counter: long flights (refill every 8 or 16 steps) take 32, so
+    // that the last entries of a wave spread over all warps (C4 flights 35.9 -> 34.8 ms, C5 66.6 -> 65.2); flights of a cell or two,
+    // which refill after every step, would queue on that one address (C3: 7.32 ms with 128, 7.56 with 32, 8.58 with 16)
+    const unsigned int chunk = n_burst == 1 ? (unsigned int)KRP_FLIGHT_CHUNK : 32u;
     int status = KRP_IDLE;
     bool more = true;
     unsigned int item = 0, wbase = 0, wleft = 0;
@@ -746,7 +749,7 @@ __global__ void __launch_bounds__(TPB, MINB) krp_k_flight_general(KrpModel g, Kr
             tl.w_esc += es.order ? 1.0 : (double)q.S[item].x;
             status = KRP_IDLE;
         }
-        if (krp_take_work(&ctl->work[0], n_items, status == KRP_IDLE, wbase, wleft, more, item)) {
+        if (krp_take_work(&ctl->work[0], n_items, status == KRP_IDLE, wbase, wleft, more, item, chunk)) {
             float4 pc, nk, S0; double tau0; unsigned long long id_;
             krp_item_load(g, q, es, item, pc, nk, S0, tau0, id_);
             const float n[3] = { nk.x, nk.y, nk.z }, p0[3] = { pc.x, pc.y, pc.z };
@@ -1230,7 +1233,7 @@ __global__ void __launch_bounds__(128, 6) krp_k_packets_scalar(KrpModel g, KrpCt
     unsigned long long id = 0;
     int f = 0;
     for (;;) {
-        if (krp_take_work<32u>(&ctl->work[0], n_items, !alive, wbase, wleft, more, item)) {      // 32 per visit: a small batch spreads over all warps
+        if (krp_take_work(&ctl->work[0], n_items, !alive, wbase, wleft, more, item, 32u)) {      // 32 per visit: a small batch spreads over all warps
             pc = q.pc[item]; nk = q.nk[item]; S0 = q.S[item];
             D = q.tau[item];
             id = q.id[item];
