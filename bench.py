@@ -574,7 +574,9 @@ def main():
                    "job_packets": cfg["n_packets"], "events_per_packet": r["epp"],
                    "l2": "flushed every step by a 256 MiB memset inside the timed region",
                    "launch": "flights: %s; imaging: one launch per observer over events ordered by cell bin" %
-                             ("static assignment" if r["mode"] == "scalar" else "persistent lanes, refill distance chosen from the measured flight length"),
+                             (("one kernel per batch, a lane follows a packet to its end (krp_k_packets_scalar)"
+                               if r["roof"].get("kernels", {}).get("flight", {}).get("launches_per_step", 2) <= 1 else "static assignment, one launch per scattering order")
+                              if r["mode"] == "scalar" else "persistent lanes, refill distance chosen from the measured flight length"),
                    "parallelism": "packet ids sharded over %d GPU(s), grid replicated, one fp64 image all-reduce at job end" % r["world"],
                    "reduced": bool(args.n)},
         "scatterings_per_s": tot["events"] / sec,
