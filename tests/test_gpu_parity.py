@@ -289,6 +289,7 @@ def test_full_size_general_mode_sampled_ids(name, batch, ns):
     """BASELINE configs[2..4] at full grid and image size (64x64x256, 256^3, 512^3; general cell layout, persistent
     flights) in the launch configuration bench.py times (one batch of 2^22 / 2^23 / 2^22 packets): 10 000 packet ids
     from inside the batch replayed by the oracle one by one, sequences and maps of those ids."""
+    ns = int(os.environ.get("KRP_PARITY_NS", ns))       # a larger sample for a one-off run (profiles/r2r_README.md); the suite keeps 10 000
     cfg = inputs.make(name)
     g = gpu_grid(cfg)
     ids0 = 123456
