@@ -315,6 +315,13 @@ void ora_source_set(ora_model* m, int kind, const double pos[3], const double di
 {
     m->src_kind = kind; m->emit_records = emit_records;
     for (int a = 0; a < 3; ++a) { m->src_pos[a] = pos[a]; m->src_dir[a] = dir[a]; }
+    if (kind & 2) {
+        /* reading R23: light propagates "along direction (theta, phi)", a unit vector, and the march measures
+         * path length in units of |n|; the caller's `dir` "need not be normalised" (include/krp.h), so it is
+         * divided by its length here, in fp64, before the fp32 rounding of R12 at emission */
+        double nn = sqrt(dir[0] * dir[0] + dir[1] * dir[1] + dir[2] * dir[2]);
+        if (nn > 0.0) for (int a = 0; a < 3; ++a) m->src_dir[a] = dir[a] / nn;
+    }
     int n[3] = { m->nx, m->ny, m->nz };
     for (int a = 0; a < 3; ++a) {
         double x = (pos[a] - m->lo[a]) / m->d[a];

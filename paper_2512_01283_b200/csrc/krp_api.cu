@@ -574,6 +574,8 @@ extern "C" int krp_source_set(krp_grid* g, const krp_source* src, void* stream)
     }
     const int dims[3] = { m.nx, m.ny, m.nz };
     int idx[3];
+    // R23: `dir` need not be normalised -- divided by its length in fp64 here, rounded to fp32 (R12) below
+    const double dir_len = (src->kind & 2) ? std::sqrt(src->dir[0] * src->dir[0] + src->dir[1] * src->dir[1] + src->dir[2] * src->dir[2]) : 1.0;
     for (int a = 0; a < 3; ++a) {
         if (!std::isfinite(src->pos[a])) return fail(KRP_ERR_ARG, "source pos is not finite");
         double x = (src->pos[a] - m.lo[a]) / m.dd[a];
@@ -582,7 +584,7 @@ extern "C" int krp_source_set(krp_grid* g, const krp_source* src, void* stream)
         double p = x - i;
         p = p < 0.0 ? 0.0 : (p > 1.0 ? 1.0 : p);     // sources outside the box start on its surface
         idx[a] = i; m.src_p[a] = (float)p;
-        m.src_n[a] = (float)src->dir[a];
+        m.src_n[a] = (float)((src->kind & 2) ? src->dir[a] / dir_len : src->dir[a]);
     }
     m.src_cell = ((uint32_t)(idx[2] + 1) * (uint32_t)m.py + (uint32_t)(idx[1] + 1)) * (uint32_t)m.px + (uint32_t)(idx[0] + 1);
     cudaFree(g->d_src_cdf); g->d_src_cdf = nullptr; m.src_cdf = nullptr;

@@ -223,6 +223,42 @@ def test_thick_cells_and_collimated_beam():
         _images(cfg, ora, gev, info, np.arange(3000), g.image_get(), img_o, img2_o, "thick-%s" % (bvec,), npx=8, npy=8)
 
 
+def test_scalar_mode_source_kinds_in_both_forms():
+    """Scalar mode (no field, constant opacity) with the sources C1/C2 do not use -- a volume source weighted by the density,
+    a collimated beam from a point near a face, collimated packets starting all over the volume -- with and without emission
+    records, through the one-kernel form of small batches and through the wavefront: event by event against the oracle, and
+    the two forms against each other bit by bit."""
+    n = 20
+    base = inputs.make("c2", n=n, n_packets=5000, npix=24)
+    for label, src, flags in (("volume", dict(kind=1, pos=[0, 0, 0], dir=[0, 0, 1], cell_weight=np.ascontiguousarray(base["density"], np.float32)), 0),
+                              ("beam", dict(kind=2, pos=[0.03, -0.02, -0.49], dir=[0.1, 0.2, 1.0], cell_weight=None, emit_records=1), 1),
+                              ("volume-collimated", dict(kind=3, pos=[0, 0, 0], dir=[1.0, 0.3, -0.2], cell_weight=None), 0)):
+        cfg = dict(base, source=src)
+        npk = cfg["n_packets"]
+        ora, img_o, img2_o, st_o = oracle_run(cfg, 0, npk, flags=flags)
+        evs = []
+        for fused in (None, 0):
+            g = gpu_grid(cfg)
+            if fused is not None:
+                g.tune_fused(fused)
+            g.timing_enable(True)
+            g.transport(npk, cfg["seed"])
+            gev = gpu_events_sorted(g)
+            assert (g.timing_get()["flight"][1] == 1) == (fused is None)
+            frac, info = _sequences(cfg, ora, gev, np.arange(npk), "scalar-%s-%s" % (label, "one-kernel" if fused is None else "wavefront"), pure=False)
+            g.image(gpu_observers(cfg), cfg["npix"], cfg["npix"], flags=flags)
+            _images(cfg, ora, gev, info, np.arange(npk), g.image_get(), img_o, img2_o, "c2-%s" % label, flags=flags)
+            st = g.stats_get()
+            assert st["packets"] == npk and st["overflow"] == 0
+            assert abs(st["w_escaped"] + st["w_absorbed"] + st["w_cut"] - st["w_emitted"]) <= 1e-5 * npk
+            for kx in ("w_escaped", "w_absorbed", "w_cut"):
+                assert abs(st[kx] - st_o[kx]) <= 2e-3 * npk, (label, kx, st[kx], st_o[kx])
+            evs.append(gev)
+            g.close()
+        for key in evs[0]:
+            assert np.array_equal(evs[0][key], evs[1][key]), (label, key)
+
+
 def _sample_inside_a_batch(cfg, g, batch_id0, batch, first, ns, cap):
     """Transport one batch in the launch configuration bench.py times, pull the events of the id range [first, first+ns)
     out of it (krp_events_select), and check that a call over that range alone gives bit-identical events, which it leaves

@@ -582,6 +582,36 @@ def test_collimated_beam_pure_absorber_escape_fraction():
     assert abs(z.mean() - want) < 4 * 0.28 / math.sqrt(ev.n)
 
 
+def test_collimated_direction_is_normalised():
+    """Reading R23: the `dir` of a collimated source need not be normalised (include/krp.h) -- the packet direction is the unit
+    vector along it, so the optical depth along the beam does not scale with |dir|.  A beam along (0,0,3) through a pure
+    absorber of depth tau: escape fraction e^{-tau} (it would be e^{-tau/3} if the march took |dir| as path length per unit
+    parameter), the same packets escape as with (0,0,1), events at the same places with unit directions; and an oblique
+    beam along k*(1,2,2)/3 for k = 0.2, 1, 7 gives identical records."""
+    tau, N, seed = 2.0, 100000, 3
+    out = []
+    for k in (1.0, 3.0):
+        m = box_model((8, 8, 8), tau, opac=const_opac(1, 0, 0, 0.0))
+        m.source_set(2, [0.4, 0.6, 0.0], [0, 0, k], None, 0)
+        ev, st, esc = run_transport(m, N, seed, esc=True)
+        p = math.exp(-tau)
+        assert abs(st.w_escaped / N - p) < 4 * math.sqrt(p * (1 - p) / N), (k, st.w_escaped / N, p)
+        assert np.array_equal(ev.n_in[:ev.n], np.broadcast_to([0.0, 0.0, 1.0], (ev.n, 3)))
+        out.append((set(esc["id"]), ev.cell[:ev.n].copy(), ev.p[:ev.n].copy()))
+    assert out[0][0] == out[1][0] and np.array_equal(out[0][1], out[1][1]) and np.array_equal(out[0][2], out[1][2])
+    recs = []
+    for k in (0.2, 1.0, 7.0):
+        m = box_model((6, 6, 6), 3.0, opac=const_opac(1, 0, 0, 0.6))
+        m.source_set(2, [0.1, 0.2, 0.0], [k / 3, 2 * k / 3, 2 * k / 3], None, 0)
+        ev, st, esc = run_transport(m, 4000, 11, esc=True)
+        recs.append((ev.n, ev.cell[:ev.n].copy(), ev.p[:ev.n].copy(), ev.n_in[:ev.n].copy(), st.w_escaped))
+    for r in recs[1:]:
+        assert r[0] == recs[0][0] and np.array_equal(r[1], recs[0][1]) and r[4] == recs[0][4]
+        assert np.allclose(r[2], recs[0][2], atol=2e-7) and np.allclose(r[3], recs[0][3], atol=2e-7)     # dir/|dir| to fp64 rounding, then fp32
+    d0 = recs[0][3][0]
+    assert abs(float(np.dot(d0.astype(np.float64), d0.astype(np.float64))) - 1.0) < 3e-7
+
+
 def test_dichroic_survival_sampling():
     """Reading R7: the survival probability of a flight is I(s)/I(0) of App. A.
     Unpolarised beam, n perpendicular to B: escape fraction e^{-a1 tau} cosh(a2 tau) (P4)."""
