@@ -259,6 +259,52 @@ def test_scalar_mode_source_kinds_in_both_forms():
             assert np.array_equal(evs[0][key], evs[1][key]), (label, key)
 
 
+def test_non_cubic_cells_and_odd_dimensions():
+    """Every BASELINE workload has cubic cells and even dimensions.  Here: 13 x 7 x 21 cells of 0.1 x 0.05 x 0.07 in an
+    off-centre box, random density (and field), oblique observers with off-centre, non-square views -- scalar and general
+    cell layout, point and volume source, against the oracle event by event and map by map."""
+    import math as m
+    nx, ny, nz = 13, 7, 21
+    bounds = [-0.5, 0.8, 0.1, 0.45, -1.0, 0.47]
+    rng = np.random.default_rng(77)
+    obs = [dict(theta=m.radians(t), phi=m.radians(f), center=[0.15, 0.275, -0.265], half_w=hw, half_h=hh)
+           for t, f, hw, hh in ((0, 0, 0.8, 0.5), (57, 33, 0.9, 0.9), (90, -70, 1.0, 0.6), (141, 200, 0.7, 1.1))]
+    for name, general, kind in (("c2", False, 0), ("c4", True, 1), ("c5", True, 0)):
+        cfg = inputs.make(name, n=8, n_packets=4000, npix=20)
+        dens = np.exp(rng.uniform(m.log(0.05), m.log(30.0), size=(nz, ny, nx))).astype(np.float32)
+        dens[rng.uniform(size=dens.shape) < 0.15] = 0.0                                   # empty cells
+        bf = rng.normal(size=(nz, ny, nx, 3)).astype(np.float32) if general else None
+        src = dict(kind=kind, pos=[0.11, 0.31, -0.4], dir=[0, 0, 1], cell_weight=None)
+        cfg = dict(cfg, nx=nx, ny=ny, nz=nz, bounds=bounds, density=dens, bfield=bf, source=src, observers=obs, npix=20)
+        n = cfg["n_packets"]
+        from harness import oracle_model, oracle_observers
+        from oracle import OracleEvents, OracleStats
+        mo = oracle_model(cfg)
+        ev = OracleEvents(64 * n); st = OracleStats()
+        mo.transport(0, n, cfg["seed"], ev, st)
+        img_o, img2_o, _ = mo.image(ev, oracle_observers(cfg), 28, 20, flags=0, stats=st)
+        k = ev.n
+        order = np.lexsort((ev.k[:k], ev.id[:k]))
+        ora = dict(id=ev.id[:k][order], k=ev.k[:k][order], cell=ev.cell[:k][order], pos=ev.p[:k][order],
+                   dir=ev.n_in[:k][order], stokes=ev.S[:k][order])
+        for fused in ((None, 0) if not general else (None,)):
+            g = gpu_grid(cfg)
+            if fused is not None:
+                g.tune_fused(fused)
+            g.events_reserve(64 * n)
+            g.transport(n, cfg["seed"])
+            gev = gpu_events_sorted(g)
+            frac, info = _sequences(cfg, ora, gev, np.arange(n), "%s-13x7x21" % name, pure=False)
+            g.image(gpu_observers(cfg), 28, 20)
+            img_g = g.image_get()
+            _images(cfg, ora, gev, info, np.arange(n), img_g, img_o, img2_o, "%s-13x7x21" % name, npx=28, npy=20)
+            st_g = g.stats_get()
+            assert abs(st_g["steps_transport"] - st.steps_transport) <= 2e-3 * st.steps_transport + 2
+            assert abs(st_g["steps_image"] - st.steps_image) <= 2e-3 * st.steps_image + 2
+            assert abs(st_g["dropped"] - st.dropped) <= max(3, 2e-3 * st.dropped)
+            g.close()
+
+
 def _sample_inside_a_batch(cfg, g, batch_id0, batch, first, ns, cap):
     """Transport one batch in the launch configuration bench.py times, pull the events of the id range [first, first+ns)
     out of it (krp_events_select), and check that a call over that range alone gives bit-identical events, which it leaves

@@ -45,9 +45,24 @@ def _oracle_two_step(cfg, n, npix, emis=None):
     return m, sg.reshape(cfg["nz"], cfg["ny"], cfg["nx"], len(obs), 4), nseg, img, evd, st
 
 
-@pytest.mark.parametrize("name", sorted(CASES))
+def _non_cubic(name):
+    """13 x 7 x 21 cells of 0.1 x 0.05 x 0.07 in an off-centre box, random density with empty cells (and random field): none of the
+    BASELINE workloads has non-cubic cells or odd, unequal dimensions."""
+    nx, ny, nz = 13, 7, 21
+    rng = np.random.default_rng(78)
+    cfg = inputs.make(name, n=8, n_packets=4000, npix=24)
+    dens = np.exp(rng.uniform(math.log(0.05), math.log(30.0), size=(nz, ny, nx))).astype(np.float32)
+    dens[rng.uniform(size=dens.shape) < 0.15] = 0.0
+    bf = None if cfg["bfield"] is None else rng.normal(size=(nz, ny, nx, 3)).astype(np.float32)
+    obs = [dict(theta=math.radians(t), phi=math.radians(f), center=[0.15, 0.275, -0.265], half_w=hw, half_h=hh)
+           for t, f, hw, hh in ((0, 0, 0.8, 0.5), (57, 33, 0.9, 0.9), (141, 200, 0.7, 1.1))]
+    src = dict(kind=0 if cfg["bfield"] is None else 1, pos=[0.11, 0.31, -0.4], dir=[0, 0, 1], cell_weight=None)
+    return dict(cfg, nx=nx, ny=ny, nz=nz, bounds=[-0.5, 0.8, 0.1, 0.45, -1.0, 0.47], density=dens, bfield=bf, source=src, observers=obs)
+
+
+@pytest.mark.parametrize("name", sorted(CASES) + ["c2-13x7x21", "c4-13x7x21"])
 def test_source_grid_and_ray_image_against_the_oracle(name):
-    cfg = inputs.make(name, **CASES[name])
+    cfg = _non_cubic(name[:2]) if "-" in name else inputs.make(name, **CASES[name])
     n, npix = cfg["n_packets"], cfg["npix"]
     m, sg_o, nseg_o, img_o, ev_o, st_o = _oracle_two_step(cfg, n, npix)
     obs = gpu_observers(cfg)
