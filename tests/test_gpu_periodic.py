@@ -12,13 +12,16 @@ from harness import (oracle_run, oracle_model, oracle_observers, gpu_grid, gpu_o
 pytestmark = pytest.mark.gpu
 
 
-def _cfg(mask, dichroic):
+def _cfg(mask, dichroic, shape=None):
     cfg = inputs.make("c4" if dichroic else "c1", n=12, n_packets=6000, npix=24)
     rng = np.random.default_rng(17)
     n = 12
-    cfg["density"] = (1.5 * np.exp(0.6 * rng.normal(size=(n, n, n)))).astype(np.float32)          # no empty rim: packets do reach the faces
+    nx, ny, nz = shape or (n, n, n)
+    if shape:      # non-cubic cells, odd unequal dimensions (0.1 x 0.14 x 0.05), box still centred on the observers' centre
+        cfg.update(nx=nx, ny=ny, nz=nz, bounds=[-0.65, 0.65, -0.49, 0.49, -0.525, 0.525])
+    cfg["density"] = (1.5 * np.exp(0.6 * rng.normal(size=(nz, ny, nx)))).astype(np.float32)          # no empty rim: packets do reach the faces
     if dichroic:
-        cfg["bfield"] = rng.normal(size=(n, n, n, 3)).astype(np.float32)
+        cfg["bfield"] = rng.normal(size=(nz, ny, nx, 3)).astype(np.float32)
         cfg["source"] = dict(kind=1, pos=[0, 0, 0], dir=[0, 0, 1], cell_weight=None)
     else:
         cfg["source"] = dict(kind=0, pos=[0.31, -0.22, 0.05], dir=[0, 0, 1], cell_weight=None)
@@ -28,9 +31,10 @@ def _cfg(mask, dichroic):
     return cfg
 
 
-@pytest.mark.parametrize("mask,dichroic", [(3, False), (3, True), (5, True), (1, False)])
-def test_periodic_sequences_and_images(mask, dichroic):
-    cfg = _cfg(mask, dichroic)
+@pytest.mark.parametrize("mask,dichroic,shape", [(3, False, None), (3, True, None), (5, True, None), (1, False, None),
+                                                 (6, True, (13, 7, 21)), (2, False, (13, 7, 21))])
+def test_periodic_sequences_and_images(mask, dichroic, shape):
+    cfg = _cfg(mask, dichroic, shape)
     n = cfg["n_packets"]
     ora, img_o, img2_o, st_o = oracle_run(cfg, 0, n, cap=64 * n)
     g = gpu_grid(cfg)
