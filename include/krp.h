@@ -103,7 +103,8 @@ int krp_grid_stage(krp_grid* g, const float* density, const float* bfield, void*
 int krp_grid_update_staged(krp_grid* g, void* stream);
 
 /* Source of packets (PAPER.md:107 emission; R17).
- *   kind bit0: 0 = all packets start at pos, 1 = start uniformly inside a cell drawn with
+ *   kind bit0: 0 = all packets start at pos (a pos outside the box is moved to the nearest point of the box, coordinate by
+ *              coordinate: reading R24), 1 = start uniformly inside a cell drawn with
  *              probability proportional to cell_weight (DEVICE, [ncell]; NULL = uniform);
  *   kind bit1: 0 = isotropic directions, 1 = all along dir (need not be normalised).
  *   kind bit2 (only as kind = 5): thermal emission of the grains themselves (eq. 8, alpha_abs B; reading R22):

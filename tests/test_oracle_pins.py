@@ -612,6 +612,22 @@ def test_collimated_direction_is_normalised():
     assert abs(float(np.dot(d0.astype(np.float64), d0.astype(np.float64))) - 1.0) < 3e-7
 
 
+def test_source_outside_the_box_starts_on_its_surface():
+    """Reading R24: a source position outside the box is moved to the nearest point of the box, coordinate by coordinate --
+    the records equal those of a source placed at that point."""
+    recs = []
+    for pos in ([1.4, 0.6, -0.2], [1.0, 0.6, 0.0]):          # box [0,1]^3
+        m = box_model((6, 6, 6), 3.0, opac=const_opac(1, 0, 0, 0.6))
+        m.source_set(0, pos, [0, 0, 1.0], None, 0)
+        ev, st, esc = run_transport(m, 3000, 9, esc=True)
+        recs.append((ev.n, ev.cell[:ev.n].copy(), ev.p[:ev.n].copy(), ev.n_in[:ev.n].copy(), st.w_escaped))
+    a, b = recs
+    assert a[0] == b[0] and a[0] > 500 and a[4] == b[4]
+    for k in (1, 2, 3):
+        assert np.array_equal(a[k], b[k])
+    assert np.all((a[2] >= 0.0) & (a[2] <= 1.0))
+
+
 def test_dichroic_survival_sampling():
     """Reading R7: the survival probability of a flight is I(s)/I(0) of App. A.
     Unpolarised beam, n perpendicular to B: escape fraction e^{-a1 tau} cosh(a2 tau) (P4)."""
