@@ -329,7 +329,7 @@ void ora_source_set(ora_model* m, int kind, const double pos[3], const double di
         if (i < 0) i = 0;
         if (i > n[a] - 1) i = n[a] - 1;
         /* reading R24: a source position outside the box is moved to the nearest point of the box, coordinate by coordinate
-         * (the paper's sources all lie inside their grids; a packet has to start in a cell) */
+         * (the paper is silent: the sources of its tests lie inside their grids; a packet has to start in a cell) */
         double p = x - i;
         if (p < 0.0) p = 0.0;
         if (p > 1.0) p = 1.0;
