@@ -265,6 +265,39 @@ def test_scalar_mode_source_kinds_in_both_forms():
             assert np.array_equal(evs[0][key], evs[1][key]), (label, key)
 
 
+def test_termination_rules():
+    """R12: a packet ends when its weight falls below w_min or at its max_scatter-th event -- with limits other than the
+    defaults (1e-4, 64), an albedo of exactly 1 (only max_scatter ends a packet that stays inside) and w_min = 0, in both
+    cell layouts and both scalar forms: the number of scattering orders the library launches follows from these, so a
+    wrong count would drop or add events.  Events and the cut / absorbed / escaped weights against the oracle."""
+    for name, w_min, max_scatter, albedo in (("c1", 0.2, 64, None), ("c1", 1e-4, 2, None), ("c1", 0.0, 5, 1.0), ("c2", 0.0, 7, None),
+                                             ("c4", 0.3, 64, None), ("c4", 1e-4, 3, None), ("c4", 0.0, 4, 1.0), ("c4", 1e-4, 1, None)):
+        cfg = inputs.make(name, n=12, n_packets=3000, npix=16)
+        cfg["w_min"], cfg["max_scatter"] = w_min, max_scatter
+        if albedo is not None:
+            op = cfg["opacity"].copy(); op[:, 3] = albedo; cfg["opacity"] = op
+        n = cfg["n_packets"]
+        ora, img_o, img2_o, st_o = oracle_run(cfg, 0, n, cap=80 * n)
+        assert ora["k"].max() <= max_scatter
+        for fused in ((None, 0) if cfg["bfield"] is None else (None,)):
+            g = gpu_grid(cfg)
+            if fused is not None:
+                g.tune_fused(fused)
+            g.events_reserve(80 * n)
+            g.transport(n, cfg["seed"])
+            gev = gpu_events_sorted(g)
+            label = "%s-wmin%g-max%d-albedo%s" % (name, w_min, max_scatter, albedo)
+            frac, info = _sequences(cfg, ora, gev, np.arange(n), label, pure=False)
+            assert len(gev["id"]) == len(ora["id"]), (label, len(gev["id"]), len(ora["id"]))
+            g.image(gpu_observers(cfg), cfg["npix"], cfg["npix"])
+            _images(cfg, ora, gev, info, np.arange(n), g.image_get(), img_o, img2_o, label)
+            st = g.stats_get()
+            for kx in ("w_escaped", "w_absorbed", "w_cut"):
+                assert abs(st[kx] - st_o[kx]) <= 1e-5 * n + 1e-6 * abs(st_o[kx]), (label, kx, st[kx], st_o[kx])
+            assert abs(st["w_escaped"] + st["w_absorbed"] + st["w_cut"] - st["w_emitted"]) <= 1e-5 * n
+            g.close()
+
+
 def test_non_cubic_cells_and_odd_dimensions():
     """Every BASELINE workload has cubic cells and even dimensions.  Here: 13 x 7 x 21 cells of 0.1 x 0.05 x 0.07 in an
     off-centre box, random density (and field), oblique observers with off-centre, non-square views -- scalar and general
