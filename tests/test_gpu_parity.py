@@ -298,6 +298,44 @@ def test_termination_rules():
             g.close()
 
 
+def test_grids_of_one_cell_and_single_columns():
+    """The smallest grids: one cell, one column along each axis, a 2 x 1 x 3 slab -- halo, strides and the block-major imaging
+    order with dimensions of 1 -- in both cell layouts and both scalar forms, single packets included."""
+    import math as m
+    rng = np.random.default_rng(91)
+    obs = [dict(theta=m.radians(t), phi=m.radians(f), center=[0.0, 0.0, 0.0], half_w=1.2, half_h=0.9)
+           for t, f in ((0, 0), (65, 40), (90, 90), (120, -100))]
+    for dims in ((1, 1, 1), (1, 1, 9), (7, 1, 1), (1, 5, 1), (2, 1, 3)):
+        nx, ny, nz = dims
+        for general in (False, True):
+            base = inputs.make("c4" if general else "c2", n=8, n_packets=1500, npix=12)
+            dens = np.exp(rng.uniform(m.log(0.3), m.log(8.0), size=(nz, ny, nx))).astype(np.float32)
+            bf = rng.normal(size=(nz, ny, nx, 3)).astype(np.float32) if general else None
+            src = dict(kind=1 if general else 0, pos=[0.05, -0.1, 0.2], dir=[0, 0, 1], cell_weight=None)
+            cfg = dict(base, nx=nx, ny=ny, nz=nz, bounds=[-0.5, 0.5, -0.4, 0.4, -0.6, 0.6], density=dens, bfield=bf, source=src,
+                       observers=obs, npix=12)
+            for n in (1500, 1):
+                ora, img_o, img2_o, st_o = oracle_run(cfg, 0, n, cap=80 * n + 64)
+                for fused in ((None, 0) if not general else (None,)):
+                    g = gpu_grid(cfg)
+                    if fused is not None:
+                        g.tune_fused(fused)
+                    g.events_reserve(80 * n + 64)
+                    g.transport(n, cfg["seed"])
+                    gev = gpu_events_sorted(g)
+                    label = "%dx%dx%d-%s-n%d" % (nx, ny, nz, "general" if general else "scalar", n)
+                    frac, info = compare_sequences(ora, gev, np.arange(n))
+                    assert frac == 1.0 if n == 1 else frac >= 0.999, (label, show(info))
+                    g.image(gpu_observers(cfg), 12, 12)
+                    if len(ora["id"]):
+                        compare_images_same_ids(cfg, ora, gev, info, np.arange(n), g.image_get(), img_o, img2_o, 12, 12, name=label)
+                    else:
+                        assert np.all(g.image_get() == 0)
+                    st = g.stats_get()
+                    assert st["steps_transport"] == st_o["steps_transport"] or abs(st["steps_transport"] - st_o["steps_transport"]) <= 2e-3 * st_o["steps_transport"] + 1
+                    g.close()
+
+
 def test_non_cubic_cells_and_odd_dimensions():
     """Every BASELINE workload has cubic cells and even dimensions.  Here: 13 x 7 x 21 cells of 0.1 x 0.05 x 0.07 in an
     off-centre box, random density (and field), oblique observers with off-centre, non-square views -- scalar and general
