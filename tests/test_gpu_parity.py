@@ -336,6 +336,31 @@ def test_grids_of_one_cell_and_single_columns():
                     g.close()
 
 
+def test_packet_ids_and_seeds_beyond_32_bits():
+    """R11: Philox key = seed (lo, hi), counter = (id_lo, id_hi, k, block) -- packet ids above 2^32 (a job of 10^10 packets) and
+    a seed with high bits set reach the generator whole, in emission, scattering and both scalar forms."""
+    for name, npk in (("c1", 2000), ("c4", 2000), ("c5", 66000)):      # C5 with >= 2^16 packets: direction-ordered first flights
+        cfg = inputs.make(name, n=12, n_packets=npk, npix=16)
+        cfg["seed"] = (1 << 45) + 7
+        id0, n = (1 << 33) + 12345, cfg["n_packets"]
+        ora, img_o, img2_o, st_o = oracle_run(cfg, id0, n, cap=24 * n)
+        ora_low, _, _, _ = oracle_run(cfg, 12345, n, image=False, cap=24 * n)
+        assert len(ora["id"]) != len(ora_low["id"]) or not np.array_equal(ora["cell"], ora_low["cell"])      # the high word matters
+        for fused in ((None, 0) if cfg["bfield"] is None else (None,)):
+            g = gpu_grid(cfg)
+            if fused is not None:
+                g.tune_fused(fused)
+            g.packet_id_set(id0)
+            g.events_reserve(24 * n)
+            g.transport(n, cfg["seed"])
+            gev = gpu_events_sorted(g)
+            ids = np.arange(id0, id0 + n, dtype=np.uint64)
+            frac, info = _sequences(cfg, ora, gev, ids, "%s-id33-seed45" % name, pure=False)
+            g.image(gpu_observers(cfg), cfg["npix"], cfg["npix"])
+            _images(cfg, ora, gev, info, ids, g.image_get(), img_o, img2_o, "%s-id33" % name)
+            g.close()
+
+
 def test_non_cubic_cells_and_odd_dimensions():
     """Every BASELINE workload has cubic cells and even dimensions.  Here: 13 x 7 x 21 cells of 0.1 x 0.05 x 0.07 in an
     off-centre box, random density (and field), oblique observers with off-centre, non-square views -- scalar and general
