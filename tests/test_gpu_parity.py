@@ -361,6 +361,41 @@ def test_packet_ids_and_seeds_beyond_32_bits():
             g.close()
 
 
+def test_table_sizes():
+    """Tables at the ends of their size ranges: a Mueller table of 2 and 3 nodes (the Theta-CDF has one or two segments) and of
+    1801; an opacity table of 1 node with a field (constant, non-dichroic and dichroic: general layout, one table segment), of
+    2, 3 and 1024 nodes."""
+    def lin_mueller(n_ang):        # any positive S11 with |S12| <= S11 will do: linear in Theta between forward-peaked ends
+        th = np.linspace(0.0, math.pi, n_ang)
+        s11 = 1.6 - 0.35 * th
+        return np.stack([s11, -0.3 * s11 * np.sin(th) ** 2, 0.8 * s11 * np.cos(th), 0.1 * s11 * np.sin(th) ** 2], 1).astype(np.float32)
+    cases = [("c1", lin_mueller(2), None), ("c1", lin_mueller(3), None), ("c2", inputs.hg_mueller(0.4, 0.3, seed=5, n_ang=1801), None),
+             ("c4", lin_mueller(2), np.array([[1.0, 0.0, 0.0, 0.6]], np.float32)),
+             ("c4", lin_mueller(3), np.array([[1.0, 0.25, -0.1, 0.6]], np.float32)),
+             ("c4", None, inputs.aligned_opacity(1.3, 0.05, 0.55, n_inc=2)), ("c4", None, inputs.aligned_opacity(1.3, 0.05, 0.55, n_inc=3)),
+             ("c4", inputs.hg_mueller(0.4, 0.3, seed=6, n_ang=1801), inputs.aligned_opacity(1.2, 0.03, 0.5, n_inc=1024))]
+    for j, (name, mu, op) in enumerate(cases):
+        cfg = inputs.make(name, n=12, n_packets=2500, npix=16)
+        if mu is not None:
+            cfg["mueller"] = mu
+        if op is not None:
+            cfg["opacity"] = op
+        n = cfg["n_packets"]
+        ora, img_o, img2_o, st_o = oracle_run(cfg, 0, n, cap=40 * n)
+        for fused in ((None, 0) if cfg["bfield"] is None else (None,)):
+            g = gpu_grid(cfg)
+            if fused is not None:
+                g.tune_fused(fused)
+            g.events_reserve(40 * n)
+            g.transport(n, cfg["seed"])
+            gev = gpu_events_sorted(g)
+            label = "%s-tables%d" % (name, j)
+            frac, info = _sequences(cfg, ora, gev, np.arange(n), label, pure=False)
+            g.image(gpu_observers(cfg), cfg["npix"], cfg["npix"])
+            _images(cfg, ora, gev, info, np.arange(n), g.image_get(), img_o, img2_o, label)
+            g.close()
+
+
 def test_non_cubic_cells_and_odd_dimensions():
     """Every BASELINE workload has cubic cells and even dimensions.  Here: 13 x 7 x 21 cells of 0.1 x 0.05 x 0.07 in an
     off-centre box, random density (and field), oblique observers with off-centre, non-square views -- scalar and general
