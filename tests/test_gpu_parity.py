@@ -396,6 +396,39 @@ def test_table_sizes():
             g.close()
 
 
+def test_unaligned_cells_and_polar_observers():
+    """R10: cells whose field vector is zero are unaligned (B^ = z^), directions along the z axis take phi = 0 whatever the
+    observer's phi says -- a fifth of the cells without a field, observers at theta = 0 and 180 deg with phi != 0 and one along
+    -x, a collimated source along -z -- general layout, event by event and map by map."""
+    import math as m
+    cfg = inputs.make("c4", n=14, n_packets=3000, npix=20)
+    rng = np.random.default_rng(29)
+    bf = cfg["bfield"].copy()
+    bf[rng.uniform(size=bf.shape[:3]) < 0.2] = 0.0
+    cfg["bfield"] = bf
+    cfg["observers"] = [dict(theta=m.radians(t), phi=m.radians(f), center=[0.0, 0.0, 0.0], half_w=0.7, half_h=0.7)
+                        for t, f in ((0, 77), (180, -40), (90, 180), (180, 0))]
+    for src in (cfg["source"], dict(kind=3, pos=[0, 0, 0], dir=[0, 0, -2.0], cell_weight=None)):
+        c = dict(cfg, source=src)
+        n = c["n_packets"]
+        ora, img_o, img2_o, st_o = oracle_run(c, 0, n, cap=40 * n)
+        g = gpu_grid(c)
+        g.events_reserve(40 * n)
+        g.transport(n, c["seed"])
+        gev = gpu_events_sorted(g)
+        frac, info = _sequences(c, ora, gev, np.arange(n), "c4-unaligned-polar-kind%d" % src["kind"], pure=False)
+        g.image(gpu_observers(c), c["npix"], c["npix"])
+        img_g = g.image_get()
+        _images(c, ora, gev, info, np.arange(n), img_g, img_o, img2_o, "c4-unaligned-polar")
+        # and with the march that does its own look-ups
+        g.tune_schedule(obs_cells=0)
+        g.image_reset(); g.packet_id_set(0)
+        g.transport(n, c["seed"])
+        g.image(gpu_observers(c), c["npix"], c["npix"])
+        assert np.abs(g.image_get() - img_g).max() <= 2e-5 * np.abs(img_g[:, 0]).max()
+        g.close()
+
+
 def test_non_cubic_cells_and_odd_dimensions():
     """Every BASELINE workload has cubic cells and even dimensions.  Here: 13 x 7 x 21 cells of 0.1 x 0.05 x 0.07 in an
     off-centre box, random density (and field), oblique observers with off-centre, non-square views -- scalar and general
