@@ -335,7 +335,7 @@ class Grid:
     def sgrid_get(self, stream=None):
         """Source grid as a numpy array [nz, ny, nx, n_obs, 4] (fp32)."""
         nx, ny, nz = self.shape
-        out = np.empty((nz, ny, nx, self._sg_n_obs, 4), np.float32)
+        out = np.empty((nz, ny, nx, max(1, getattr(self, "_sg_n_obs", 0)), 4), np.float32)      # no open grid: the library says so
         _check(lib().krp_sgrid_get(self._h, C.c_void_p(out.ctypes.data), MEM_HOST, _stream(stream)))
         return out
 

@@ -103,6 +103,10 @@ def test_source_grid_and_ray_image_against_the_oracle(name):
     g.sgrid_reset()
     assert not g.sgrid_get().any()
     g.sgrid_end()
+    from paper_2512_01283_b200 import krp
+    with pytest.raises(krp.KrpError) as ei:       # no open grid any more
+        g.sgrid_get()
+    assert ei.value.code == krp.ERR_STATE
     g.close()
 
 
