@@ -506,7 +506,7 @@ def test_full_size_c2_sampled_ids():
     cfg = inputs.make("c2")
     g = gpu_grid(cfg)
     nb = 1 << 25
-    ids0, ns = 20000000, 12000                      # inside the third sub-batch
+    ids0, ns = 20000000, int(os.environ.get("KRP_PARITY_NS", 12000))     # inside the third sub-batch (a larger sample for a one-off run)
     gev, st_b = _sample_inside_a_batch(cfg, g, 0, nb, ids0, ns, int(nb * 0.9))
     ora, img_o, img2_o, st_o = oracle_run(cfg, ids0, ns)
     ids = np.arange(ids0, ids0 + ns)
