@@ -67,6 +67,7 @@ def parse_args():
                          "(every segment deposited into S(Omega_cam, x), one ray per pixel at the end of the timed steps)")
     ap.add_argument("--tune", default="", help="measurement only: transport_block,image_block,blocks_per_sm,flight_burst for krp_tune (0 keeps)")
     ap.add_argument("--fused", type=int, default=-1, help="measurement only: krp_tune_fused(max_packets); -1 keeps the library's default")
+    ap.add_argument("--schedule", default="", help="measurement only: dir_sort,obs_cells,order_policy for krp_tune_schedule (-1 keeps)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--cpu-seconds", type=float, default=15.0)
@@ -325,6 +326,8 @@ def run_krp(args):
         g.tune(*[int(x) for x in args.tune.split(",")])
     if args.fused >= 0:
         g.tune_fused(args.fused)
+    if args.schedule:
+        g.tune_schedule(*[int(x) for x in args.schedule.split(",")])
 
     # pilot (untimed): events per packet of this workload, to size the event buffer once
     pilot = min(batch, 1 << 16)

@@ -106,6 +106,9 @@ struct krp_grid {
     // ordering of the events before imaging: policy 0 never, 1 by the measured ray length, 2 always
     int order_policy = 1;
     bool order_events = true, order_decided = false;
+    unsigned long long pk_since_image = 0;                     // packets transported since the last krp_image
+    double acc_pn = 0.0, req_pn = 0.0, prev_pn = 0.0;          // sum over passes of packets x observers: running, at the last counter request, at the last evaluation
+    double events_per_packet = -1.0;                           // measured with the ordering decision (policy 1)
     unsigned long long* h_ray_stats = nullptr;          // pinned: steps_image, contributions, dropped
     unsigned long long ray_stats_prev[3] = { 0, 0, 0 };
     cudaEvent_t ray_stats_ev = nullptr;
@@ -717,6 +720,7 @@ extern "C" int krp_transport(krp_grid* g, uint64_t n_packets, uint64_t seed, voi
         g->launches += 3;
         CK(cudaGetLastError());
         g->next_id += n_packets;
+        g->pk_since_image += n_packets;
         return KRP_OK;
     }
     const int tb = g->transport_block;
@@ -806,6 +810,7 @@ extern "C" int krp_transport(krp_grid* g, uint64_t n_packets, uint64_t seed, voi
     }
     CK(cudaGetLastError());
     g->next_id += n_packets;
+    g->pk_since_image += n_packets;
     if (!g->m.scalar && g->burst_auto && !g->burst_decided && !g->flight_stats_pending) {
         if (!g->h_flight_stats) {
             CK(cudaMallocHost(&g->h_flight_stats, 4 * sizeof(unsigned long long)));
@@ -933,13 +938,26 @@ extern "C" int krp_image(krp_grid* g, const krp_observer* obs, int n_obs, int np
         if (rays >= 100000ull && !g->order_decided) {
             g->order_events = g->order_policy == 2 || (g->order_policy == 1 && (double)steps / (double)rays >= 12.0);
             g->order_decided = true;
+            if (g->req_pn > g->prev_pn) g->events_per_packet = (double)rays / (g->req_pn - g->prev_pn);
         }
         g->ray_stats_prev[0] = g->h_ray_stats[0]; g->ray_stats_prev[1] = g->h_ray_stats[1]; g->ray_stats_prev[2] = g->h_ray_stats[2];
+        g->prev_pn = g->req_pn;
         g->ray_stats_pending = false;
     }
-    const unsigned int* perm = g->order_events ? g->d_perm : nullptr;
+    // ... nor when the events are few and the cell array small: a pass of fewer than 2^18 events over an array of at most 32 MiB
+    // (its rays find their cells in L2 in any order) costs more to order than the order saves (C1, 10^5 packets on 32^3 cells:
+    // ordering + imaging 74 -> 49 us; C2 at 2^17 packets: 224 -> 175 us; at 2^20 packets the order wins, 458 against 506 us; on the
+    // 512^3 grid of C5 it wins at any size).  Host-side estimate, the same for every pass of equal size: packets since the last
+    // pass x the events per packet measured with the decision above.
+    const size_t cell_bytes = (size_t)g->npad * (g->m.scalar ? sizeof(float) : sizeof(float4));
+    const bool few = g->order_policy == 1 && g->events_per_packet >= 0.0 && cell_bytes <= ((size_t)32 << 20) &&
+                     (double)g->pk_since_image * g->events_per_packet < 262144.0;
+    const bool order_now = g->order_events && !few;
+    g->acc_pn += (double)g->pk_since_image * (double)n_obs;
+    g->pk_since_image = 0;
+    const unsigned int* perm = order_now ? g->d_perm : nullptr;
     { TimedLaunch tlo(g, st, KRP_T_ORDER);
-    if (g->order_events) {
+    if (order_now) {
         CK(cudaMemsetAsync(g->d_bins, 0, sizeof(unsigned int) * ((size_t)g->n_bins + 1), st));
         const int sflags = flags | (g->ev_has_emission ? 0 : 2);       // bit 1: no emission records to look for
         krp_k_sort_count<<<pers, 256, 0, st>>>(g->m, g->d_ctl, g->ev, g->sort_geom, g->sub_bits, sflags, g->d_bins);
@@ -985,6 +1003,7 @@ extern "C" int krp_image(krp_grid* g, const krp_observer* obs, int n_obs, int np
         CK(cudaMemcpyAsync(g->h_ray_stats, &g->d_ctl->stats.steps_image, 3 * sizeof(unsigned long long), cudaMemcpyDeviceToHost, st));
         CK(cudaEventRecord(g->ray_stats_ev, st));
         g->ray_stats_pending = true;
+        g->req_pn = g->acc_pn;
     }
     return KRP_OK;
 }
