@@ -429,6 +429,36 @@ def test_unaligned_cells_and_polar_observers():
         g.close()
 
 
+def test_small_passes_on_small_grids_are_imaged_unordered():
+    """krp_image orders the events by cell unless the rays are short or -- this test -- the pass is small and the cell array
+    fits L2 (fewer than 2^18 events, at most 32 MiB): the decision needs one measured pass of >= 10^5 rays, so the first
+    passes are ordered and the later ones are not (four launches fewer); the maps of every pass equal those of a model
+    that always orders, up to the order of the fp64 sums."""
+    cfg = inputs.make("c1", n=32, n_packets=100000, npix=48)
+    obs = gpu_observers(cfg)
+    maps, launches = {}, {}
+    for policy in (1, 2):
+        g = gpu_grid(cfg)
+        g.tune_schedule(order_policy=policy)
+        out, nl = [], []
+        for step in range(4):
+            g.packet_id_set(step * cfg["n_packets"])
+            g.image_reset()
+            g.transport(cfg["n_packets"], cfg["seed"])
+            before = g.launch_count()
+            g.image(obs, cfg["npix"], cfg["npix"])
+            nl.append(g.launch_count() - before)
+            out.append(g.image_get().copy())
+        maps[policy], launches[policy] = out, nl
+        assert g.stats_get()["overflow"] == 0
+        g.close()
+    assert launches[2] == [launches[2][0]] * 4                      # always ordered
+    assert launches[1][0] == launches[2][0]                         # first pass: nothing measured yet
+    assert launches[1][-1] == launches[2][0] - 4, (launches)        # later passes: image_prep_plain instead of count, 2 scan kernels, prep, scatter
+    for a, b in zip(maps[1], maps[2]):
+        assert np.allclose(a, b, rtol=1e-11, atol=1e-13 * b[:, 0].max())
+
+
 def test_non_cubic_cells_and_odd_dimensions():
     """Every BASELINE workload has cubic cells and even dimensions.  Here: 13 x 7 x 21 cells of 0.1 x 0.05 x 0.07 in an
     off-centre box, random density (and field), oblique observers with off-centre, non-square views -- scalar and general
