@@ -287,7 +287,7 @@ int krp_tune(krp_grid* g, int transport_block, int image_block, int blocks_per_s
  * current value): dir_sort 1/0 = first flights of an isotropic point source taken in direction order / in id order;
  * obs_cells 1/0 = per-observer cell coefficient arrays in the general-mode imaging march / look-ups in the march (takes
  * effect at the next change of the observer set); order_policy 0 never / 1 by the measured ray length (not below 12 cell
- * steps per ray) and the size of the pass (not for fewer than 2^18 events over a cell array of at most 32 MiB) / 2 always
+ * steps per ray) and the size of the pass (not for fewer than 2^18 events over a cell array of at most 12 MiB) / 2 always
  * order the events by cell before imaging. */
 int krp_tune_schedule(krp_grid* g, int dir_sort, int obs_cells, int order_policy);
 /* Small batches in scalar mode (no field, constant non-dichroic opacity, F(Theta) scattering, no open source grid): a

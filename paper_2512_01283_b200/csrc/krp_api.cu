@@ -944,13 +944,13 @@ extern "C" int krp_image(krp_grid* g, const krp_observer* obs, int n_obs, int np
         g->prev_pn = g->req_pn;
         g->ray_stats_pending = false;
     }
-    // ... nor when the events are few and the cell array small: a pass of fewer than 2^18 events over an array of at most 32 MiB
-    // (its rays find their cells in L2 in any order) costs more to order than the order saves (C1, 10^5 packets on 32^3 cells:
+    // ... nor when the events are few and the cell array small: a pass of fewer than 2^18 events over an array of at most 12 MiB,
+    // a tenth of L2 (its rays find their cells there in any order; at 15 MiB -- C5 at 96^3 -- the order still wins by 9 %) costs more to order than the order saves (C1, 10^5 packets on 32^3 cells:
     // ordering + imaging 74 -> 49 us; C2 at 2^17 packets: 224 -> 175 us; at 2^20 packets the order wins, 458 against 506 us; on the
     // 512^3 grid of C5 it wins at any size).  Host-side estimate, the same for every pass of equal size: packets since the last
     // pass x the events per packet measured with the decision above.
     const size_t cell_bytes = (size_t)g->npad * (g->m.scalar ? sizeof(float) : sizeof(float4));
-    const bool few = g->order_policy == 1 && g->events_per_packet >= 0.0 && cell_bytes <= ((size_t)32 << 20) &&
+    const bool few = g->order_policy == 1 && g->events_per_packet >= 0.0 && cell_bytes <= ((size_t)12 << 20) &&
                      (double)g->pk_since_image * g->events_per_packet < 262144.0;
     const bool order_now = g->order_events && !few;
     g->acc_pn += (double)g->pk_since_image * (double)n_obs;

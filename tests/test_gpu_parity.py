@@ -431,7 +431,7 @@ def test_unaligned_cells_and_polar_observers():
 
 def test_small_passes_on_small_grids_are_imaged_unordered():
     """krp_image orders the events by cell unless the rays are short or -- this test -- the pass is small and the cell array
-    fits L2 (fewer than 2^18 events, at most 32 MiB): the decision needs one measured pass of >= 10^5 rays, so the first
+    is a small part of L2 (fewer than 2^18 events, at most 12 MiB): the decision needs one measured pass of >= 10^5 rays, so the first
     passes are ordered and the later ones are not (four launches fewer); the maps of every pass equal those of a model
     that always orders, up to the order of the fp64 sums."""
     cfg = inputs.make("c1", n=32, n_packets=100000, npix=48)
